@@ -1,0 +1,425 @@
+/*
+ * genga_oracle.c -- CPU FP64 oracle for the GENGA level-0 hot path (see genga_oracle.h).
+ *
+ * TEST INFRASTRUCTURE, NOT THE PRODUCT.  Plain C99, FP64, sqrt + divide, j ascending,
+ * Neumaier-compensated sums; OpenMP over i only (each body's own sum has a fixed order, so
+ * results do not depend on the thread count).  No code is shared with the CUDA path.
+ *
+ * Citations: PAPER.md:NN = line NN of /root/reference/PAPER.md.  O1..O11 and G1..G11 are
+ * the oracle steps and readings of SURVEY.md section 8(c), restated in DESIGN.md section 3.
+ *
+ * Build:  gcc -std=c99 -O2 -ffp-contract=off -fopenmp -fPIC -shared genga_oracle.c -lm
+ */
+#include "genga_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ---- Neumaier compensated accumulator: value = s + c ------------------------------------ */
+typedef struct { double s, c; } nsum;
+
+static void nsum_add(nsum* a, double t)
+{
+    double S = a->s + t;
+    if (fabs(a->s) >= fabs(t)) a->c += (a->s - S) + t;
+    else                       a->c += (t - S) + a->s;
+    a->s = S;
+}
+static double nsum_value(const nsum* a) { return a->s + a->c; }
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ---- O4: changeover function, reading G1 ---------------------------------------------------
+ * PAPER.md:45 "A changeover function smoothly switches between the two levels (Chambers
+ * 1999)".  The formula is not printed; reading G1 takes the rational form
+ *   y = (r - 0.1 rc)/(0.9 rc);  K = 0 (y <= 0),  y^2/(2y^2 - 2y + 1) (0 < y < 1),  1 (y >= 1).
+ * rc <= 0 means "no changeover zone": K = 1 for every r > 0.                                  */
+double oracle_changeover(double r, double rcrit)
+{
+    if (!(rcrit > 0.0)) return (r > 0.0) ? 1.0 : 0.0;
+    double y = (r - 0.1 * rcrit) / (0.9 * rcrit);
+    if (y <= 0.0) return 0.0;
+    if (y >= 1.0) return 1.0;
+    return (y * y) / (2.0 * y * y - 2.0 * y + 1.0);
+}
+
+/* ---- O1: velocity conventions, reading G3 -------------------------------------------------
+ * stored v_i = v_h,i - (sum_j m_j v_h,j)/(M_star + sum_j m_j);
+ * inverse    v_h,i = v_i + (sum_j m_j v_j)/M_star.                                            */
+static void mass_weighted_velocity(int N, const double* m, const double* v, double out[3], double* mtot)
+{
+    nsum p[3] = {{0, 0}, {0, 0}, {0, 0}}, mt = {0, 0};
+    for (int j = 0; j < N; ++j) {
+        for (int k = 0; k < 3; ++k) nsum_add(&p[k], m[j] * v[3 * j + k]);
+        nsum_add(&mt, m[j]);
+    }
+    for (int k = 0; k < 3; ++k) out[k] = nsum_value(&p[k]);
+    if (mtot) *mtot = nsum_value(&mt);
+}
+
+void oracle_to_democratic(int N, const double* m, double* v, double M_star)
+{
+    double p[3], mt;
+    mass_weighted_velocity(N, m, v, p, &mt);
+    for (int i = 0; i < N; ++i)
+        for (int k = 0; k < 3; ++k) v[3 * i + k] -= p[k] / (M_star + mt);
+}
+
+void oracle_to_heliocentric(int N, const double* m, double* v, double M_star)
+{
+    double p[3];
+    mass_weighted_velocity(N, m, v, p, NULL);
+    for (int i = 0; i < N; ++i)
+        for (int k = 0; k < 3; ++k) v[3 * i + k] += p[k] / M_star;
+}
+
+/* ---- O2: critical radius, Eq. 1 ---------------------------------------------
+ *   r_crit,i = max(n1 R_H,i , n2 dt v_i),  R_H,i = a_i (m_i / 3 M_star)^(1/3).
+ * Readings G2b/G2c: a_i from vis-viva with the stored v and mu = G M_star (a_i = r_i when that
+ * is not a positive finite number); v_i = sqrt(G M_star / a_i).                               */
+void oracle_rcrit(int N, const double* m, const double* x, const double* v,
+                  const oracle_params* p, double* rcrit, double* semi, double* vkep)
+{
+    const double mu = p->G * p->M_star;
+    for (int i = 0; i < N; ++i) {
+        const double* xi = x + 3 * i;
+        const double* vi = v + 3 * i;
+        double r  = sqrt(xi[0] * xi[0] + xi[1] * xi[1] + xi[2] * xi[2]);
+        double v2 = vi[0] * vi[0] + vi[1] * vi[1] + vi[2] * vi[2];
+        double a  = 1.0 / (2.0 / r - v2 / mu);
+        if (!(a > 0.0) || !isfinite(a)) a = r;
+        double RH = a * cbrt(m[i] / (3.0 * p->M_star));
+        double vk = sqrt(mu / a);
+        double rc = fmax(p->n1 * RH, p->n2 * p->dt_rcrit * vk);
+        if (rcrit) rcrit[i] = rc;
+        if (semi)  semi[i]  = a;
+        if (vkep)  vkep[i]  = vk;
+    }
+}
+
+/* ---- O3: pair radius, reading G2 ----------------------------------------------------------- */
+double oracle_pair_rcrit(const oracle_params* p, double mi, double mj,
+                         double rci, double rcj, double ai, double aj,
+                         double vki, double vkj)
+{
+    if (p->pair_rule == ORACLE_PAIR_MUTUAL_HILL) {
+        double hill = p->n1 * cbrt((mi + mj) / (3.0 * p->M_star)) * (0.5 * (ai + aj));
+        double vel  = p->n2 * p->dt_rcrit * fmax(vki, vkj);
+        return fmax(hill, vel);
+    }
+    return fmax(rci, rcj);
+}
+
+/* ---- O2-O5: the kick acceleration (north_star; "the N^2 gravitational force
+ * terms") ---------------------------------------------------------------------------------- */
+void oracle_accel(int N, const double* m, const double* x, const double* v,
+                  const oracle_params* p, double* acc)
+{
+    double* rc = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* sa = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* vk = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    oracle_rcrit(N, m, x, v, p, rc, sa, vk);
+
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int i = 0; i < N; ++i) {
+        nsum a[3] = {{0, 0}, {0, 0}, {0, 0}};
+        for (int j = 0; j < N; ++j) {
+            if (j == i) continue;
+            double dx = x[3 * j + 0] - x[3 * i + 0];
+            double dy = x[3 * j + 1] - x[3 * i + 1];
+            double dz = x[3 * j + 2] - x[3 * i + 2];
+            double r2 = dx * dx + dy * dy + dz * dz;
+            double r  = sqrt(r2);
+            if (!(r > 0.0)) continue;                     /* coincident bodies: W = 0 */
+            double rcij = oracle_pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j]);
+            double W = oracle_changeover(r, rcij);
+            if (W == 0.0) continue;
+            double s = p->G * m[j] * W / (r2 * r);
+            nsum_add(&a[0], s * dx);
+            nsum_add(&a[1], s * dy);
+            nsum_add(&a[2], s * dz);
+        }
+        for (int k = 0; k < 3; ++k) acc[3 * i + k] = nsum_value(&a[k]);
+    }
+    free(rc); free(sa); free(vk);
+}
+
+/* ---- O6: encounter set, strict r < r_crit,ij (reading G6), PAPER.md:55 --------------------- */
+void oracle_encounter_pairs(int N, const double* m, const double* x, const double* v,
+                            const oracle_params* p, int* pairs, int cap, int* count)
+{
+    double* rc = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* sa = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* vk = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    oracle_rcrit(N, m, x, v, p, rc, sa, vk);
+    int n = 0;
+    for (int i = 0; i < N; ++i) {
+        for (int j = i + 1; j < N; ++j) {
+            double dx = x[3 * j + 0] - x[3 * i + 0];
+            double dy = x[3 * j + 1] - x[3 * i + 1];
+            double dz = x[3 * j + 2] - x[3 * i + 2];
+            double r  = sqrt(dx * dx + dy * dy + dz * dz);
+            double rcij = oracle_pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j]);
+            if (r < rcij) {
+                if (n < cap && pairs) { pairs[2 * n] = i; pairs[2 * n + 1] = j; }
+                ++n;
+            }
+        }
+    }
+    *count = n;
+    free(rc); free(sa); free(vk);
+}
+
+/* ---- O7: velocity update -------------------------------------------------------------------- */
+void oracle_kick(int N, const double* m, const double* x, double* v,
+                 const oracle_params* p, double tau, double* acc_out)
+{
+    double* a = (double*)malloc(sizeof(double) * 3 * (size_t)(N > 0 ? N : 1));
+    oracle_accel(N, m, x, v, p, a);
+    for (int i = 0; i < 3 * N; ++i) v[i] += tau * a[i];
+    if (acc_out) for (int i = 0; i < 3 * N; ++i) acc_out[i] = a[i];
+    free(a);
+}
+
+/* ---- O8: Sun-kick of the democratic-heliocentric split (reading G3) ------------------------ */
+void oracle_sunkick(int N, const double* m, double* x, const double* v,
+                    const oracle_params* p, double tau)
+{
+    double s[3];
+    mass_weighted_velocity(N, m, v, s, NULL);
+    for (int i = 0; i < N; ++i)
+        for (int k = 0; k < 3; ++k) x[3 * i + k] += tau * (s[k] / p->M_star);
+}
+
+/* ---- O9: Kepler drift, PAPER.md:43 ("Kepler orbit solver is always performed in double
+ * precision"), reading G4: the exact two-body map about mu = G M_star.
+ *
+ * Anomaly-difference form.  With r0 = |x0|, u = x0.v0, alpha = 2 mu/r0 - |v0|^2 = mu/a:
+ *  ellipse (alpha > 0): n = sqrt(mu/a^3); solve
+ *        dE - (1 - r0/a) sin dE + (u/(n a^2)) (1 - cos dE) = n dt                      (K)
+ *     f = 1 - (a/r0)(1 - cos dE),             g = dt - (dE - sin dE)/n,
+ *     r = a + (r0 - a) cos dE + (u/(n a)) sin dE,
+ *     fdot = -a^2 n sin dE /(r r0),           gdot = 1 - (a/r)(1 - cos dE).
+ *  hyperbola (alpha < 0): b = -a > 0, nu = sqrt(mu/b^3); the same with
+ *     sin -> sinh, (1 - cos) -> -(cosh - 1), i.e. with the functions
+ *     G1 = sinh dH/sqrt(beta), G2 = (cosh dH - 1)/beta, G3 = (sinh dH - dH)/beta^(3/2), beta = -alpha:
+ *        r0 G1 + u G2 + mu G3 = dt,   f = 1 - mu G2/r0,  g = dt - mu G3,
+ *        r = r0 cosh dH + u G1 + mu G2,  fdot = -mu G1/(r r0),  gdot = 1 - mu G2/r.
+ *  parabola (alpha = 0): G1 = s, G2 = s^2/2, G3 = s^3/6.
+ * x = f x0 + g v0, v = fdot x0 + gdot v0.  The root is unique (the left side is strictly
+ * increasing: its derivative is r/a resp. r/sqrt(beta) > 0); Newton with a bisection guard.     */
+
+typedef double (*kep_fn)(double xx, const double* c, double* deriv);
+
+static double kep_ell(double E, const double* c, double* d)
+{   /* c = {EC, ES, M}: E - EC sin E + ES (1 - cos E) - M */
+    double sE = sin(E), cE = cos(E);
+    *d = 1.0 - c[0] * cE + c[1] * sE;
+    return E - c[0] * sE + c[1] * (1.0 - cE) - c[2];
+}
+static double kep_hyp(double H, const double* c, double* d)
+{   /* c = {r0, u, mu, sqrt(beta), beta, dt} */
+    double sh = sinh(H), ch = cosh(H);
+    double G1 = sh / c[3], G2 = (ch - 1.0) / c[4], G3 = (sh - H) / (c[4] * c[3]);
+    *d = (c[0] * ch + c[1] * G1 + c[2] * G2) / c[3];
+    return c[0] * G1 + c[1] * G2 + c[2] * G3 - c[5];
+}
+static double kep_par(double s, const double* c, double* d)
+{   /* c = {r0, u, mu, dt} */
+    *d = c[0] + c[1] * s + 0.5 * c[2] * s * s;
+    return c[0] * s + 0.5 * c[1] * s * s + c[2] * s * s * s / 6.0 - c[3];
+}
+
+/* guarded Newton on a strictly increasing function, root bracketed in [lo, hi] */
+static int solve_increasing(kep_fn F, const double* c, double lo, double hi, double x0, double* root)
+{
+    double xx = x0;
+    if (!(xx > lo && xx < hi)) xx = 0.5 * (lo + hi);
+    for (int it = 0; it < 200; ++it) {
+        double d, f = F(xx, c, &d);
+        if (f == 0.0) { *root = xx; return 0; }
+        if (f > 0.0) hi = xx; else lo = xx;
+        double xn = xx - f / d;
+        if (!(xn > lo && xn < hi)) xn = 0.5 * (lo + hi);
+        double step = fabs(xn - xx);
+        xx = xn;
+        if (step <= 1e-16 * fmax(1.0, fabs(xx)) || hi - lo <= 4e-16 * fmax(1.0, fabs(xx))) {
+            *root = xx; return 0;
+        }
+    }
+    *root = xx;
+    return -1;
+}
+
+int oracle_kepler_drift_one(double mu, double dt, double x[3], double v[3])
+{
+    const double TWO_PI = 6.283185307179586476925286766559;
+    double r0 = sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+    double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+    double u  = x[0] * v[0] + x[1] * v[1] + x[2] * v[2];
+    double alpha = 2.0 * mu / r0 - v2;
+    double f, g, fd, gd;
+    int rcode = 0;
+
+    if (dt == 0.0) return 0;
+
+    if (alpha > 0.0) {
+        double a  = mu / alpha;
+        double n  = sqrt(mu / (a * a * a));
+        double EC = 1.0 - r0 / a;
+        double ES = u / (n * a * a);
+        double M  = n * dt;
+        double k  = floor(M / TWO_PI + 0.5);          /* whole revolutions */
+        double Mr = M - k * TWO_PI;
+        double c[3] = {EC, ES, Mr};
+        double dE;
+        rcode = solve_increasing(kep_ell, c, Mr - 3.2, Mr + 3.2, Mr, &dE);
+        double sE = sin(dE), cE = cos(dE);
+        double h  = sin(0.5 * dE);
+        double omc = 2.0 * h * h;                      /* 1 - cos dE */
+        double r  = a + (r0 - a) * cE + (u / (n * a)) * sE;
+        f  = 1.0 - (a / r0) * omc;
+        g  = dt - ((dE - sE) + k * TWO_PI) / n;
+        fd = -a * a * n * sE / (r * r0);
+        gd = 1.0 - (a / r) * omc;
+    } else if (alpha < 0.0) {
+        double beta = -alpha, sb = sqrt(beta);
+        double c[6] = {r0, u, mu, sb, beta, dt};
+        /* F(0) = -dt: bracket the root by doubling away from 0 in the direction of dt */
+        double lo = 0.0, hi = 0.0, d;
+        int guard = 0;
+        if (dt > 0.0) { hi = 0.5; while (kep_hyp(hi, c, &d) < 0.0 && ++guard < 64) { lo = hi; hi *= 2.0; } }
+        else          { lo = -0.5; while (kep_hyp(lo, c, &d) > 0.0 && ++guard < 64) { hi = lo; lo *= 2.0; } }
+        if (guard >= 64) return -1;
+        double H;
+        rcode = solve_increasing(kep_hyp, c, lo, hi, 0.5 * (lo + hi), &H);
+        double sh = sinh(H), ch = cosh(H);
+        double hh = sinh(0.5 * H);
+        double chm1 = 2.0 * hh * hh;                   /* cosh H - 1 */
+        double G1 = sh / sb, G2 = chm1 / beta, G3 = (sh - H) / (beta * sb);
+        double r  = r0 * ch + u * G1 + mu * G2;
+        f  = 1.0 - mu * G2 / r0;
+        g  = dt - mu * G3;
+        fd = -mu * G1 / (r * r0);
+        gd = 1.0 - mu * G2 / r;
+    } else {
+        double c[4] = {r0, u, mu, dt};
+        double lo = 0.0, hi = 0.0, d, s;
+        int guard = 0;
+        if (dt > 0.0) { hi = dt / r0; while (kep_par(hi, c, &d) < 0.0 && ++guard < 64) { lo = hi; hi *= 2.0; } }
+        else          { lo = dt / r0; while (kep_par(lo, c, &d) > 0.0 && ++guard < 64) { hi = lo; lo *= 2.0; } }
+        if (guard >= 64) return -1;
+        rcode = solve_increasing(kep_par, c, lo, hi, dt / r0, &s);
+        double G1 = s, G2 = 0.5 * s * s, G3 = s * s * s / 6.0;
+        double r  = r0 + u * G1 + mu * G2;
+        f  = 1.0 - mu * G2 / r0;
+        g  = dt - mu * G3;
+        fd = -mu * G1 / (r * r0);
+        gd = 1.0 - mu * G2 / r;
+    }
+
+    double nx[3], nv[3];
+    for (int k = 0; k < 3; ++k) {
+        nx[k] = f * x[k] + g * v[k];
+        nv[k] = fd * x[k] + gd * v[k];
+    }
+    for (int k = 0; k < 3; ++k) { x[k] = nx[k]; v[k] = nv[k]; }
+    return rcode;
+}
+
+int oracle_drift(int N, double* x, double* v, const oracle_params* p, double dt)
+{
+    const double mu = p->G * p->M_star;
+    int bad = 0;
+#pragma omp parallel for schedule(static) reduction(+ : bad)
+    for (int i = 0; i < N; ++i)
+        if (oracle_kepler_drift_one(mu, dt, x + 3 * i, v + 3 * i) != 0) ++bad;
+    return bad ? -1 : 0;
+}
+
+/* ---- O10: one level-0 step ("the symplectic integrator with a fixed step size
+ * wherein bodies revolve around the central mass (level 0)"; splitting per reading G3) ------ */
+static int sds(int N, const double* m, double* x, double* v, const oracle_params* p, double dt)
+{
+    oracle_sunkick(N, m, x, v, p, 0.5 * dt);
+    int rc = oracle_drift(N, x, v, p, dt);
+    oracle_sunkick(N, m, x, v, p, 0.5 * dt);
+    return rc;
+}
+
+int oracle_step(int N, const double* m, double* x, double* v,
+                const oracle_params* p, double dt)
+{
+    oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
+    int rc = sds(N, m, x, v, p, dt);
+    oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
+    return rc;
+}
+
+int oracle_run(int N, const double* m, double* x, double* v,
+               const oracle_params* p, double dt, int nsteps)
+{
+    int rc = 0;
+    if (nsteps <= 0) return 0;
+    oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
+    for (int s = 0; s < nsteps; ++s) {
+        if (sds(N, m, x, v, p, dt) != 0) rc = -1;
+        oracle_kick(N, m, x, v, p, (s + 1 < nsteps) ? dt : 0.5 * dt, NULL);
+    }
+    return rc;
+}
+
+/* ---- O11: diagnostics, PAPER.md:111 (Delta E/E = E(t)/E(0) - 1, likewise L), reading G5 ---- */
+void oracle_energy_angmom(int N, const double* m, const double* x, const double* v,
+                          const oracle_params* p, double* E, double L[3])
+{
+    nsum kin = {0, 0}, sol = {0, 0}, pot = {0, 0};
+    nsum P[3] = {{0, 0}, {0, 0}, {0, 0}}, Ls[3] = {{0, 0}, {0, 0}, {0, 0}};
+    for (int i = 0; i < N; ++i) {
+        const double* xi = x + 3 * i;
+        const double* vi = v + 3 * i;
+        double r  = sqrt(xi[0] * xi[0] + xi[1] * xi[1] + xi[2] * xi[2]);
+        double v2 = vi[0] * vi[0] + vi[1] * vi[1] + vi[2] * vi[2];
+        nsum_add(&kin, 0.5 * m[i] * v2);
+        nsum_add(&sol, p->G * p->M_star * m[i] / r);
+        for (int k = 0; k < 3; ++k) nsum_add(&P[k], m[i] * vi[k]);
+        nsum_add(&Ls[0], m[i] * (xi[1] * vi[2] - xi[2] * vi[1]));
+        nsum_add(&Ls[1], m[i] * (xi[2] * vi[0] - xi[0] * vi[2]));
+        nsum_add(&Ls[2], m[i] * (xi[0] * vi[1] - xi[1] * vi[0]));
+    }
+    /* pair potential: per-i partial sums in parallel, then added in i order */
+    double* part = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int i = 0; i < N; ++i) {
+        nsum q = {0, 0};
+        for (int j = i + 1; j < N; ++j) {
+            double dx = x[3 * j + 0] - x[3 * i + 0];
+            double dy = x[3 * j + 1] - x[3 * i + 1];
+            double dz = x[3 * j + 2] - x[3 * i + 2];
+            double r  = sqrt(dx * dx + dy * dy + dz * dz);
+            nsum_add(&q, p->G * m[i] * m[j] / r);
+        }
+        part[i] = nsum_value(&q);
+    }
+    for (int i = 0; i < N; ++i) nsum_add(&pot, part[i]);
+    free(part);
+
+    double px = nsum_value(&P[0]), py = nsum_value(&P[1]), pz = nsum_value(&P[2]);
+    nsum e = {0, 0};
+    nsum_add(&e, nsum_value(&kin));
+    nsum_add(&e, (px * px + py * py + pz * pz) / (2.0 * p->M_star));
+    nsum_add(&e, -nsum_value(&sol));
+    nsum_add(&e, -nsum_value(&pot));
+    *E = nsum_value(&e);
+    for (int k = 0; k < 3; ++k) L[k] = nsum_value(&Ls[k]);
+}

@@ -1,0 +1,107 @@
+/*
+ * genga_oracle.h -- CPU FP64 oracle for the GENGA level-0 hot path.
+ *
+ * TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may load this library.
+ * It shares no code, header, table or helper with the CUDA path under
+ * paper_2309_08217_b200/ and neither imports the other.
+ *
+ * What it computes follows /root/reference/PAPER.md (arXiv 2309.08217) where
+ * the paper speaks, and the readings G1..G11 of SURVEY.md section 8(c) /
+ * DESIGN.md section 3 where it is silent.  Every function is the plain
+ * definition written out: sqrt and divide, no rsqrt tricks, no blocking, no
+ * reordering, j ascending, Neumaier-compensated sums.
+ *
+ * Layout: m[N]; x, v, a are [N][3] row-major doubles; all pointers are HOST
+ * pointers.  x is heliocentric; v is the stored ("democratic", i.e.
+ * barycentric) velocity unless a function says otherwise.
+ *
+ * Pin status (see tests/test_oracle_*.py, marked "not gpu"):
+ *   oracle_changeover      pinned: limits, hand values, symmetry (G1 reading: "parity unpinned
+ *                          by PAPER.md" for the CHOICE of K -- the paper prints no formula)
+ *   oracle_rcrit           pinned: Eq. 1 by hand
+ *   oracle_accel           pinned: hand 3-/4-body values, n-gon closed form, sum m a = 0,
+ *                          torque = 0, 50-digit brute force
+ *   oracle_encounter_pairs pinned: brute force, constructed r_crit(1 -+ 1e-9) cases
+ *   oracle_drift           pinned: circular orbit, period return, scipy DOP853, invariants
+ *   oracle_step/run        pinned: 2nd-order convergence to a DOP853 inertial-frame solution
+ *   oracle_energy_angmom   pinned: two-body closed form, inertial-frame formula
+ */
+#ifndef GENGA_ORACLE_H
+#define GENGA_ORACLE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { ORACLE_PAIR_MAX = 0, ORACLE_PAIR_MUTUAL_HILL = 1 };
+
+typedef struct {
+    double G;         /* gravitational constant in the caller's units                */
+    double M_star;    /* central mass                                                */
+    double n1, n2;    /* Eq. 1 constants (3 and 0.4)                    */
+    double dt_rcrit;  /* the dt of Eq. 1's second term (reading G8: the step dt)     */
+    int    pair_rule; /* reading G2: how r_crit,ij follows from per-body quantities  */
+} oracle_params;
+
+/* O4, reading G1 (PAPER.md:45 names Chambers 1999; formula not printed). */
+double oracle_changeover(double r, double rcrit);
+
+/* O1: heliocentric velocities <-> stored barycentric ("democratic") ones.    */
+void oracle_to_democratic(int N, const double* m, double* v, double M_star);
+void oracle_to_heliocentric(int N, const double* m, double* v, double M_star);
+
+/* O2, Eq. 1.  Outputs may be NULL.  semi = a_i, vkep = v_K,i. */
+void oracle_rcrit(int N, const double* m, const double* x, const double* v,
+                  const oracle_params* p, double* rcrit, double* semi, double* vkep);
+
+/* O3: r_crit,ij from the per-body arrays returned by oracle_rcrit.           */
+double oracle_pair_rcrit(const oracle_params* p, double mi, double mj,
+                         double rci, double rcj, double ai, double aj,
+                         double vki, double vkj);
+
+/* O2-O5: a_i = sum_{j != i} G m_j K(r_ij, r_crit,ij) (x_j - x_i) / r_ij^3.   */
+void oracle_accel(int N, const double* m, const double* x, const double* v,
+                  const oracle_params* p, double* acc);
+
+/* O6: { (i,j): i<j, r_ij < r_crit,ij } in lexicographic order.  Writes at most
+ * cap pairs into pairs[cap][2]; *count receives the true total.              */
+void oracle_encounter_pairs(int N, const double* m, const double* x, const double* v,
+                            const oracle_params* p, int* pairs, int cap, int* count);
+
+/* O7: v_i += tau * a_i (a from oracle_accel on the current state).  acc_out
+ * may be NULL, else receives a.                                              */
+void oracle_kick(int N, const double* m, const double* x, double* v,
+                 const oracle_params* p, double tau, double* acc_out);
+
+/* O8, reading G3: x_i += tau * (sum_j m_j v_j) / M_star.                     */
+void oracle_sunkick(int N, const double* m, double* x, const double* v,
+                    const oracle_params* p, double tau);
+
+/* O9, reading G4: exact two-body propagation of one body about mu by dt,
+ * eccentric / hyperbolic anomaly-difference form.  Returns 0, or -1 if the
+ * root solve failed (never observed).                                        */
+int oracle_kepler_drift_one(double mu, double dt, double x[3], double v[3]);
+int oracle_drift(int N, double* x, double* v, const oracle_params* p, double dt);
+
+/* O10: K(dt/2) S(dt/2) D(dt) S(dt/2) K(dt/2).                                */
+int oracle_step(int N, const double* m, double* x, double* v,
+                const oracle_params* p, double dt);
+
+/* nsteps concatenated O10 steps with adjacent half-kicks merged:
+ * K(dt/2) [S D S K(dt)]^(nsteps-1) S D S K(dt/2); r_crit is recomputed at each
+ * force evaluation from the velocities of that moment (reading R7). */
+int oracle_run(int N, const double* m, double* x, double* v,
+               const oracle_params* p, double dt, int nsteps);
+
+/* O11.  E = sum m v^2/2 + |sum m v|^2/(2 M_star) - sum G M_star m/r
+ *                         - sum_{i<j} G m_i m_j / r_ij ;  L = sum m x cross v. */
+void oracle_energy_angmom(int N, const double* m, const double* x, const double* v,
+                          const oracle_params* p, double* E, double L[3]);
+
+int oracle_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
