@@ -1,0 +1,166 @@
+/*
+ * genga.h -- C ABI of libgenga_b200: the level-0 hot path of the GENGA hybrid symplectic
+ * N-body step (arXiv 2309.08217) as hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Citations: PAPER.md:NN = line NN of the paper text; G1..G12 / O1..O11 are the readings and
+ * oracle steps of SURVEY.md section 8(c), restated in DESIGN.md section 3.
+ *
+ * What is computed
+ *   kick: a_i = sum_{j != i} G m_j K(r_ij, r_crit,ij) (x_j - x_i)/r_ij^3,
+ *        K the changeover function (reading G1), r_crit,i from Eq. 1,
+ *        in FP64 or FP32 force precision ("Do Kick in single precision");
+ *        pairs with r_ij < r_crit,ij are recorded as close-encounter candidates.
+ *   drift ("the Kepler orbit solver is always performed in double precision"):
+ *        exact two-body propagation about mu = G M_star with universal-variable f and g.
+ *   step  (reading G3): K(dt/2) S(dt/2) D(dt) S(dt/2) K(dt/2) in democratic
+ *        heliocentric variables (heliocentric x, barycentric v).
+ *   energy_angmom: total energy E and angular momentum L of the stored state.
+ *
+ * Conventions
+ *   N        number of bodies, the star excluded.  N = 0 and N = 1 are valid.
+ *   m        [N]      FP64 masses.  m = 0 (test particle) is valid.
+ *   x, v, a  [N][3]   FP64, row-major (a contiguous (N,3) float64 tensor).  x is heliocentric.
+ *            The STORED velocity is barycentric ("democratic").  If params.v_is_heliocentric,
+ *            genga_create / genga_set_state convert the velocities they are given (O1).
+ *   DEVICE   pointer into CUDA device memory of the current device.
+ *   HOST     pointer into host memory (pinned memory makes the copies asynchronous).
+ *   Every call except the ones marked "synchronises" only enqueues work on params.stream.
+ *   The library never allocates device memory: all state lives in params.workspace, owned by the
+ *   caller (size from genga_workspace_bytes) and must stay valid until genga_destroy.
+ *   Input pointers are borrowed for the duration of the call (DEVICE inputs: until the enqueued
+ *   copy has run, i.e. stream order).  One handle is not thread-safe; handles share no state.
+ *   Return value: GENGA_OK (0) or a negative genga_status.  No exceptions, no abort.
+ *
+ * There is NO CPU fallback: without a CUDA device every compute call returns GENGA_ECUDA.
+ */
+#ifndef GENGA_H
+#define GENGA_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct genga_s* genga_handle;
+
+typedef enum {
+    GENGA_OK        =  0,
+    GENGA_EINVAL    = -1,   /* bad argument (NULL handle, N < 0, unknown precision, ...)            */
+    GENGA_ENOMEM    = -2,   /* params.workspace_bytes < genga_workspace_bytes(N, params)            */
+    GENGA_ECAPACITY = -3,   /* encounter-pair list overflow: first cap pairs written, *count = total */
+    GENGA_ECUDA     = -4,   /* a CUDA runtime call failed; genga_last_cuda_error() has the text      */
+    GENGA_ENOCONV   = -5    /* Kepler solver failed to converge for >= 1 body (state still written)  */
+} genga_status;
+
+/* PAPER.md:223 "Do Kick in single precision = 0 / 1". */
+typedef enum { GENGA_FP64 = 0, GENGA_FP32 = 1 } genga_precision;
+
+/* Reading G2: how r_crit,ij follows from per-body quantities.
+ *   PAIR_MAX         r_crit,ij = max(r_crit,i, r_crit,j)                      (Eq. 1 per body)
+ *   PAIR_MUTUAL_HILL r_crit,ij = max(n1 ((m_i+m_j)/(3 M_star))^(1/3) (a_i+a_j)/2,
+ *                                    n2 dt_rcrit max(v_K,i, v_K,j))           (BASELINE configs) */
+typedef enum { GENGA_PAIR_MAX = 0, GENGA_PAIR_MUTUAL_HILL = 1 } genga_pair_rule;
+
+typedef struct {
+    double G;                 /* gravitational constant in the caller's units (k^2 for AU, day, Msun)  */
+    double M_star;            /* central mass                                                          */
+    double n1, n2;            /* Eq. 1 (3 and 0.4; BASELINE configs: 3 and 0)              */
+    double dt_rcrit;          /* the dt of Eq. 1's second term (reading G8: the step dt)               */
+    int    pair_rule;         /* genga_pair_rule                                                       */
+    int    v_is_heliocentric; /* 1: velocities given to create/set_state are heliocentric (O1)         */
+    double lambda_near;       /* FP32 policy P32: pairs with r_ij < lambda_near * r_crit,ij (as bounded
+                                 per j-chunk) are evaluated in FP64.  <= 0 selects the default (8).    */
+    double near_floor;        /* FP32 policy P32: additionally every pair with r_ij < near_floor * max(|x_i|,
+                                 |x_j| bound) is evaluated in FP64 (position-rounding guard).
+                                 < 0 selects the default; 0 disables.                                   */
+    void*  stream;            /* cudaStream_t owned by the caller; NULL = the legacy default stream    */
+    void*  workspace;         /* DEVICE memory owned by the caller, 256-byte aligned                    */
+    size_t workspace_bytes;
+    int    pair_capacity;     /* capacity (pairs) of the encounter-pair list kept inside the workspace */
+    int    cand_capacity;     /* capacity of the internal (body, j-chunk) near-field candidate list;
+                                 <= 0 selects a default.  Overflow is handled exactly (slow path).      */
+} genga_params;
+
+/* Fill *p with the defaults: G = k^2 (k = 0.01720209895), M_star = 1, n1 = 3, n2 = 0,
+ * dt_rcrit = 0, PAIR_MUTUAL_HILL, v_is_heliocentric = 1, lambda_near/near_floor = defaults,
+ * stream/workspace = NULL, capacities = defaults.                                             */
+void   genga_default_params(genga_params* p);
+
+/* Bytes of DEVICE workspace a handle for N bodies needs with these params (capacities resolved). */
+size_t genga_workspace_bytes(int N, const genga_params* p);
+
+/* Create a handle; copies m, x, v (DEVICE pointers, [N], [N][3], [N][3]) into the workspace on
+ * params.stream.  m/x/v may be NULL (state zero-initialised; use genga_set_state* later).      */
+int genga_create(genga_handle* out, int N, const double* m, const double* x, const double* v,
+                 const genga_params* p);
+int genga_destroy(genga_handle h);
+
+/* Replace the state.  DEVICE pointers / HOST pointers.  Any of m, x, v may be NULL (kept).      */
+int genga_set_state(genga_handle h, const double* m, const double* x, const double* v);
+int genga_set_state_host(genga_handle h, const double* m, const double* x, const double* v);
+
+/* Kick: r_crit (Eq. 1), force evaluation in the given precision, encounter-pair list, and
+ * v_i += dt * a_i with exactly the dt given (dt < 0 allowed).  PAPER.md:43, 55, 223.            */
+int genga_kick(genga_handle h, double dt, int precision);
+
+/* Force evaluation only (as genga_kick with the velocity update left out).                      */
+int genga_accel(genga_handle h, int precision);
+
+/* Kepler drift only: every body propagated by dt about mu = G M_star (O9).         */
+int genga_drift(genga_handle h, double dt);
+
+/* Sun-kick only: x_i += tau * (sum_j m_j v_j) / M_star (reading G3; O8).                        */
+int genga_sunkick(genga_handle h, double tau);
+
+/* One step K(dt/2) S(dt/2) D(dt) S(dt/2) K(dt/2) (O10): two force evaluations.                  */
+int genga_step(genga_handle h, double dt, int precision);
+
+/* nsteps steps with adjacent half-kicks merged: K(dt/2) [S D S K(dt)]^(nsteps-1) S D S K(dt/2),
+ * nsteps + 1 force evaluations (reading R7).                                          */
+int genga_run(genga_handle h, double dt, int nsteps, int precision);
+
+/* Encounter pairs {(i,j): i < j, r_ij < r_crit,ij} of the LAST force evaluation.
+ * pairs_ij: HOST int[cap][2] (may be NULL if cap = 0); *count (HOST) receives the true total.
+ * Order unspecified.  Synchronises the stream.                                                  */
+int genga_encounter_pairs(genga_handle h, int* pairs_ij, int cap, int* count);
+
+/* E and L of the stored state (O11).  HOST outputs.  Synchronises the stream.     */
+int genga_energy_angmom(genga_handle h, double* E, double L[3]);
+
+/* Accessors.  DEVICE outputs (asynchronous) and HOST outputs (synchronise).  NULL = skip.
+ * x heliocentric; v as stored (barycentric) unless heliocentric_v != 0 (O1 inverse).            */
+int genga_get_state(genga_handle h, double* x, double* v, int heliocentric_v);
+int genga_get_state_host(genga_handle h, double* x, double* v, int heliocentric_v);
+int genga_get_accel(genga_handle h, double* a);          /* DEVICE [N][3]: a_i of the last force evaluation */
+int genga_get_rcrit(genga_handle h, double* rcrit);      /* DEVICE [N]: r_crit,i of the last force evaluation */
+
+/* Diagnostics of the last force evaluation: number of (body, j-chunk) near-field candidates and
+ * whether the candidate list overflowed (exact slow path taken).  HOST outputs.  Synchronises.  */
+int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed);
+
+/* Per-kernel device timing.  enable != 0 brackets every force-kernel launch with CUDA events on
+ * params.stream.  genga_kernel_time returns, for which = 0 (all-pairs kick kernel), 1 (near-field
+ * kernel), 2 (prep kernel), 3 (drift kernel), the summed milliseconds and launch count since the
+ * last reset (HOST outputs).  Synchronises.                                                     */
+int genga_set_profiling(genga_handle h, int enable);
+int genga_kernel_time(genga_handle h, int which, double* ms_total, long long* launches, int reset);
+
+/* Launches issued by this handle since creation (kernels only, not copies).                     */
+long long genga_launch_count(genga_handle h);
+
+int genga_synchronize(genga_handle h);
+const char* genga_strerror(int code);
+const char* genga_last_cuda_error(void);
+const char* genga_version(void);
+
+/* ALU peak probes: run a register-only dependent-chain kernel on every SM
+ * for iters iterations and return achieved instr throughput.  which: 0 FFMA, 1 FFMA2 (packed),
+ * 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H.  *ops_per_s (HOST) = lane-operations per second
+ * (an FFMA2 counts 2).  stream as in params.  Synchronises.                                     */
+int genga_peak_probe(int which, int iters, void* stream, double* ops_per_s, double* ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GENGA_H */

@@ -1,0 +1,430 @@
+// api.cu -- the C ABI of include/genga.h: argument checking, workspace carving, stream order of
+// the kernels, host<->device copies, per-kernel event timing.  No arithmetic of the method lives
+// here; every step of the path runs in the CUDA kernels of this directory.
+#include "genga_internal.cuh"
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+namespace genga {
+
+static thread_local char g_cuda_err[256] = "";
+
+static int cuda_fail(cudaError_t e, const char* where)
+{
+    std::snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    return GENGA_ECUDA;
+}
+#define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+#define LAUNCHED(h, name) do { ++(h)->launches; cudaError_t e_ = cudaGetLastError(); \
+                               if (e_ != cudaSuccess) return cuda_fail(e_, name); } while (0)
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static int padded(int N) { return (int)align_up((size_t)(N > 0 ? N : 1), PAD_BODIES); }
+
+static void resolve_caps(int N, const genga_params* p, int* pair_cap, int* cand_cap)
+{
+    long long pc = p->pair_capacity > 0 ? p->pair_capacity : (4LL * N + 1024);
+    long long cc = p->cand_capacity > 0 ? p->cand_capacity : (16LL * N + 65536);
+    if (pc > 0x3fffffff) pc = 0x3fffffff;
+    if (cc > 0x3fffffff) cc = 0x3fffffff;
+    *pair_cap = (int)pc; *cand_cap = (int)cc;
+}
+
+size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace* w)
+{
+    const size_t NP = (size_t)padded(N);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    const size_t o_m = take(NP * 8), o_x = take(NP * 24), o_v = take(NP * 24), o_a = take(NP * 24);
+    const size_t o_h = take(NP * 8), o_rc = take(NP * 8), o_sa = take(NP * 8), o_vk = take(NP * 8);
+    const size_t o_p64 = take(NP * 32), o_p32 = take(NP * 16), o_bi = take(NP * 16), o_bc = take(NP / CHUNK * 16);
+    const size_t o_cand = take((size_t)cand_cap * 8), o_pairs = take((size_t)pair_cap * 8);
+    const size_t o_red = take((size_t)RED_DOUBLES * 8), o_vt = take(NP * 24), o_ctr = take(sizeof(Counters));
+    if (w && base) {
+        char* b = static_cast<char*>(base);
+        w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
+        w->hcbrt = (double*)(b + o_h); w->rcrit = (double*)(b + o_rc); w->semi = (double*)(b + o_sa);
+        w->vkep = (double*)(b + o_vk); w->pk64 = (double4*)(b + o_p64); w->pk32 = (float4*)(b + o_p32);
+        w->bi = (BoundP*)(b + o_bi); w->bc = (BoundP*)(b + o_bc); w->cand = (int2*)(b + o_cand);
+        w->pairs = (int2*)(b + o_pairs); w->red = (double*)(b + o_red); w->vtmp = (double*)(b + o_vt);
+        w->ctr = (Counters*)(b + o_ctr);
+    }
+    return off;
+}
+
+// ---- profiling -------------------------------------------------------------------------------
+static int prof_flush(Handle* h, int which)
+{
+    for (int k = 0; k < h->evn[which]; ++k) {
+        CU(cudaEventSynchronize(h->ev1[which][k]));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, h->ev0[which][k], h->ev1[which][k]));
+        h->ms_total[which] += ms;
+        ++h->ms_launches[which];
+    }
+    h->evn[which] = 0;
+    return GENGA_OK;
+}
+
+struct ProfScope {
+    Handle* h; int which; bool on;
+    ProfScope(Handle* h_, int w_) : h(h_), which(w_), on(h_->prof != 0)
+    {
+        if (!on) return;
+        if (h->evn[which] == Handle::EVPOOL) prof_flush(h, which);
+        cudaEventRecord(h->ev0[which][h->evn[which]], h->stream);
+    }
+    ~ProfScope()
+    {
+        if (!on) return;
+        cudaEventRecord(h->ev1[which][h->evn[which]], h->stream);
+        ++h->evn[which];
+    }
+};
+
+// ---- force evaluation -------------------------------------------------------------------------
+static int force_eval(Handle* h, int precision)
+{
+    if (precision != GENGA_FP64 && precision != GENGA_FP32) return GENGA_EINVAL;
+    if (h->N == 0) return GENGA_OK;
+    PrepArgs a;
+    a.N = h->N; a.NP = h->NP;
+    a.G = h->p.G; a.M_star = h->p.M_star; a.n1 = h->p.n1; a.n2 = h->p.n2; a.dt_rcrit = h->p.dt_rcrit;
+    a.pair_rule = h->p.pair_rule;
+    if (precision == GENGA_FP32) { a.lambda = (float)h->lambda_near; a.floor_rel = (float)h->near_floor; }
+    else                         { a.lambda = 1.0f;                  a.floor_rel = 0.0f; }
+    { ProfScope ps(h, 2); launch_prep(h, a); }
+    LAUNCHED(h, "prep_kernel");
+    { ProfScope ps(h, 0); if (precision == GENGA_FP32) launch_kick32(h); else launch_kick64(h); }
+    LAUNCHED(h, "kick_kernel");
+    { ProfScope ps(h, 1); launch_nearfield(h); }
+    LAUNCHED(h, "nearfield_kernel");
+    return GENGA_OK;
+}
+
+static int to_democratic(Handle* h)
+{
+    if (h->N == 0) return GENGA_OK;
+    launch_momentum(h); LAUNCHED(h, "momentum_kernel");
+    launch_shift_v(h, -1.0); LAUNCHED(h, "shift_kernel");
+    return GENGA_OK;
+}
+
+}  // namespace genga
+
+using namespace genga;
+
+struct genga_s : public genga::Handle {};
+
+// S(dt/2) D(dt) S(dt/2): the middle of one step (reading G3)
+static int sds(genga_handle h, double dt)
+{
+    int rc;
+    if ((rc = genga_sunkick(h, 0.5 * dt)) != GENGA_OK) return rc;
+    if ((rc = genga_drift(h, dt)) != GENGA_OK) return rc;
+    return genga_sunkick(h, 0.5 * dt);
+}
+
+extern "C" {
+
+void genga_default_params(genga_params* p)
+{
+    if (!p) return;
+    std::memset(p, 0, sizeof(*p));
+    p->G = 0.01720209895 * 0.01720209895;
+    p->M_star = 1.0;
+    p->n1 = 3.0; p->n2 = 0.0; p->dt_rcrit = 0.0;
+    p->pair_rule = GENGA_PAIR_MUTUAL_HILL;
+    p->v_is_heliocentric = 1;
+    p->lambda_near = 0.0; p->near_floor = -1.0;
+    p->stream = nullptr; p->workspace = nullptr; p->workspace_bytes = 0;
+    p->pair_capacity = 0; p->cand_capacity = 0;
+}
+
+size_t genga_workspace_bytes(int N, const genga_params* p)
+{
+    if (N < 0 || !p) return 0;
+    int pc, cc;
+    resolve_caps(N, p, &pc, &cc);
+    return carve_workspace(N, pc, cc, nullptr, nullptr);
+}
+
+int genga_create(genga_handle* out, int N, const double* m, const double* x, const double* v, const genga_params* p)
+{
+    if (!out || !p || N < 0 || N > (1 << 24)) return GENGA_EINVAL;
+    if (!(p->M_star > 0.0) || !(p->G > 0.0)) return GENGA_EINVAL;
+    if (p->pair_rule != GENGA_PAIR_MAX && p->pair_rule != GENGA_PAIR_MUTUAL_HILL) return GENGA_EINVAL;
+    *out = nullptr;
+    int pc, cc;
+    resolve_caps(N, p, &pc, &cc);
+    const size_t need = carve_workspace(N, pc, cc, nullptr, nullptr);
+    if (!p->workspace || p->workspace_bytes < need) return GENGA_ENOMEM;
+    if ((reinterpret_cast<uintptr_t>(p->workspace) & 255u) != 0) return GENGA_EINVAL;
+
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+
+    genga_s* h = new (std::nothrow) genga_s();
+    if (!h) return GENGA_ENOMEM;
+    std::memset(static_cast<Handle*>(h), 0, sizeof(Handle));
+    h->N = N; h->NP = padded(N); h->nchunk = h->NP / CHUNK;
+    h->p = *p;
+    h->lambda_near = p->lambda_near > 0.0 ? p->lambda_near : 8.0;
+    h->near_floor  = p->near_floor >= 0.0 ? p->near_floor : (1.0 / 256.0);
+    if (h->lambda_near < 1.0) h->lambda_near = 1.0;
+    h->pair_cap = pc; h->cand_cap = cc;
+    h->stream = static_cast<cudaStream_t>(p->stream);
+    h->num_sms = sms;
+    carve_workspace(N, pc, cc, p->workspace, &h->w);
+
+    cudaError_t e = cudaMemsetAsync(p->workspace, 0, need, h->stream);
+    if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaMemsetAsync(workspace)"); }
+    launch_pad(h);
+    ++h->launches;
+    *out = h;
+    const int rc = genga_set_state(h, m, x, v);
+    if (rc != GENGA_OK) { delete h; *out = nullptr; return rc; }
+    return GENGA_OK;
+}
+
+int genga_destroy(genga_handle h)
+{
+    if (!h) return GENGA_EINVAL;
+    if (h->events_created) {
+        for (int w = 0; w < Handle::NKT; ++w)
+            for (int k = 0; k < Handle::EVPOOL; ++k) { cudaEventDestroy(h->ev0[w][k]); cudaEventDestroy(h->ev1[w][k]); }
+    }
+    delete h;
+    return GENGA_OK;
+}
+
+static int set_state_impl(genga_handle h, const double* m, const double* x, const double* v, cudaMemcpyKind kind)
+{
+    if (!h) return GENGA_EINVAL;
+    const size_t n = (size_t)h->N;
+    if (n == 0) return GENGA_OK;
+    if (m) CU(cudaMemcpyAsync(h->w.m, m, n * 8, kind, h->stream));
+    if (x) CU(cudaMemcpyAsync(h->w.x, x, n * 24, kind, h->stream));
+    if (v) CU(cudaMemcpyAsync(h->w.v, v, n * 24, kind, h->stream));
+    if (m) { launch_hcbrt(h); LAUNCHED(h, "hcbrt_kernel"); }
+    if (v && h->p.v_is_heliocentric) return to_democratic(h);
+    return GENGA_OK;
+}
+
+int genga_set_state(genga_handle h, const double* m, const double* x, const double* v)
+{
+    return set_state_impl(h, m, x, v, cudaMemcpyDeviceToDevice);
+}
+
+int genga_set_state_host(genga_handle h, const double* m, const double* x, const double* v)
+{
+    return set_state_impl(h, m, x, v, cudaMemcpyHostToDevice);
+}
+
+int genga_accel(genga_handle h, int precision)
+{
+    if (!h) return GENGA_EINVAL;
+    return force_eval(h, precision);
+}
+
+int genga_kick(genga_handle h, double dt, int precision)
+{
+    if (!h) return GENGA_EINVAL;
+    const int rc = force_eval(h, precision);
+    if (rc != GENGA_OK) return rc;
+    launch_velupdate(h, dt); LAUNCHED(h, "velupdate_kernel");
+    return GENGA_OK;
+}
+
+int genga_drift(genga_handle h, double dt)
+{
+    if (!h) return GENGA_EINVAL;
+    { ProfScope ps(h, 3); launch_drift(h, dt); }
+    LAUNCHED(h, "drift_kernel");
+    return GENGA_OK;
+}
+
+int genga_sunkick(genga_handle h, double tau)
+{
+    if (!h) return GENGA_EINVAL;
+    if (h->N == 0) return GENGA_OK;
+    launch_momentum(h); LAUNCHED(h, "momentum_kernel");
+    launch_sunkick(h, tau); LAUNCHED(h, "sunkick_kernel");
+    return GENGA_OK;
+}
+
+int genga_step(genga_handle h, double dt, int precision)
+{
+    if (!h) return GENGA_EINVAL;
+    int rc;
+    if ((rc = genga_kick(h, 0.5 * dt, precision)) != GENGA_OK) return rc;
+    if ((rc = sds(h, dt)) != GENGA_OK) return rc;
+    return genga_kick(h, 0.5 * dt, precision);
+}
+
+int genga_run(genga_handle h, double dt, int nsteps, int precision)
+{
+    if (!h || nsteps < 0) return GENGA_EINVAL;
+    if (nsteps == 0) return GENGA_OK;
+    int rc;
+    if ((rc = genga_kick(h, 0.5 * dt, precision)) != GENGA_OK) return rc;
+    for (int s = 0; s < nsteps; ++s) {
+        if ((rc = sds(h, dt)) != GENGA_OK) return rc;
+        if ((rc = genga_kick(h, (s + 1 < nsteps) ? dt : 0.5 * dt, precision)) != GENGA_OK) return rc;
+    }
+    return GENGA_OK;
+}
+
+int genga_encounter_pairs(genga_handle h, int* pairs_ij, int cap, int* count)
+{
+    if (!h || !count || cap < 0 || (cap > 0 && !pairs_ij)) return GENGA_EINVAL;
+    *count = 0;
+    if (h->N == 0) return GENGA_OK;
+    Counters c;
+    CU(cudaMemcpyAsync(&c, h->w.ctr, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    *count = (int)c.pair_count;
+    unsigned int have = c.pair_count < (unsigned int)h->pair_cap ? c.pair_count : (unsigned int)h->pair_cap;
+    unsigned int ncopy = have < (unsigned int)cap ? have : (unsigned int)cap;
+    if (ncopy) {
+        CU(cudaMemcpyAsync(pairs_ij, h->w.pairs, (size_t)ncopy * 8, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    return (c.pair_count > ncopy) ? GENGA_ECAPACITY : GENGA_OK;
+}
+
+int genga_energy_angmom(genga_handle h, double* E, double L[3])
+{
+    if (!h || !E || !L) return GENGA_EINVAL;
+    launch_energy(h); h->launches += 2;
+    { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_, "energy kernels"); }
+    double r[4];
+    CU(cudaMemcpyAsync(r, h->w.red, sizeof(r), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    *E = r[0]; L[0] = r[1]; L[1] = r[2]; L[2] = r[3];
+    return GENGA_OK;
+}
+
+static int get_state_impl(genga_handle h, double* x, double* v, int helio, cudaMemcpyKind kind)
+{
+    if (!h) return GENGA_EINVAL;
+    const size_t n = (size_t)h->N;
+    if (n == 0) return GENGA_OK;
+    if (x) CU(cudaMemcpyAsync(x, h->w.x, n * 24, kind, h->stream));
+    if (v) {
+        if (helio) {
+            launch_momentum(h); LAUNCHED(h, "momentum_kernel");
+            if (kind == cudaMemcpyDeviceToDevice) { launch_copy_v_helio(h, v); LAUNCHED(h, "copy_shift_kernel"); }
+            else {
+                launch_copy_v_helio(h, h->w.vtmp); LAUNCHED(h, "copy_shift_kernel");
+                CU(cudaMemcpyAsync(v, h->w.vtmp, n * 24, kind, h->stream));
+            }
+        } else {
+            CU(cudaMemcpyAsync(v, h->w.v, n * 24, kind, h->stream));
+        }
+    }
+    if (kind == cudaMemcpyDeviceToHost) CU(cudaStreamSynchronize(h->stream));
+    return GENGA_OK;
+}
+
+int genga_get_state(genga_handle h, double* x, double* v, int heliocentric_v)
+{
+    return get_state_impl(h, x, v, heliocentric_v, cudaMemcpyDeviceToDevice);
+}
+
+int genga_get_state_host(genga_handle h, double* x, double* v, int heliocentric_v)
+{
+    return get_state_impl(h, x, v, heliocentric_v, cudaMemcpyDeviceToHost);
+}
+
+int genga_get_accel(genga_handle h, double* a)
+{
+    if (!h || !a) return GENGA_EINVAL;
+    if (h->N) CU(cudaMemcpyAsync(a, h->w.a, (size_t)h->N * 24, cudaMemcpyDeviceToDevice, h->stream));
+    return GENGA_OK;
+}
+
+int genga_get_rcrit(genga_handle h, double* rcrit)
+{
+    if (!h || !rcrit) return GENGA_EINVAL;
+    if (h->N) CU(cudaMemcpyAsync(rcrit, h->w.rcrit, (size_t)h->N * 8, cudaMemcpyDeviceToDevice, h->stream));
+    return GENGA_OK;
+}
+
+int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed)
+{
+    if (!h) return GENGA_EINVAL;
+    Counters c;
+    std::memset(&c, 0, sizeof(c));
+    if (h->N) {
+        CU(cudaMemcpyAsync(&c, h->w.ctr, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    if (candidates) *candidates = (long long)c.cand_count;
+    if (overflowed) *overflowed = (int)c.overflow;
+    return c.noconv ? GENGA_ENOCONV : GENGA_OK;
+}
+
+int genga_set_profiling(genga_handle h, int enable)
+{
+    if (!h) return GENGA_EINVAL;
+    if (enable && !h->events_created) {
+        for (int w = 0; w < Handle::NKT; ++w)
+            for (int k = 0; k < Handle::EVPOOL; ++k) {
+                CU(cudaEventCreate(&h->ev0[w][k]));
+                CU(cudaEventCreate(&h->ev1[w][k]));
+            }
+        h->events_created = true;
+    }
+    if (!enable && h->prof) for (int w = 0; w < Handle::NKT; ++w) prof_flush(h, w);
+    h->prof = enable ? 1 : 0;
+    return GENGA_OK;
+}
+
+int genga_kernel_time(genga_handle h, int which, double* ms_total, long long* launches, int reset)
+{
+    if (!h || which < 0 || which >= Handle::NKT) return GENGA_EINVAL;
+    const int rc = prof_flush(h, which);
+    if (rc != GENGA_OK) return rc;
+    if (ms_total) *ms_total = h->ms_total[which];
+    if (launches) *launches = h->ms_launches[which];
+    if (reset) { h->ms_total[which] = 0.0; h->ms_launches[which] = 0; }
+    return GENGA_OK;
+}
+
+long long genga_launch_count(genga_handle h) { return h ? h->launches : 0; }
+
+int genga_synchronize(genga_handle h)
+{
+    if (!h) return GENGA_EINVAL;
+    CU(cudaStreamSynchronize(h->stream));
+    return GENGA_OK;
+}
+
+const char* genga_strerror(int code)
+{
+    switch (code) {
+        case GENGA_OK:        return "ok";
+        case GENGA_EINVAL:    return "invalid argument";
+        case GENGA_ENOMEM:    return "workspace too small";
+        case GENGA_ECAPACITY: return "encounter-pair list capacity exceeded";
+        case GENGA_ECUDA:     return "CUDA error";
+        case GENGA_ENOCONV:   return "Kepler solver did not converge";
+        default:              return "unknown error";
+    }
+}
+
+const char* genga_last_cuda_error(void) { return genga::g_cuda_err; }
+
+const char* genga_version(void) { return "genga_b200 0.1 (sm_100a)"; }
+
+int genga_peak_probe(int which, int iters, void* stream, double* ops_per_s, double* ms)
+{
+    return run_peak_probe(which, iters, static_cast<cudaStream_t>(stream), ops_per_s, ms);
+}
+
+}  // extern "C"

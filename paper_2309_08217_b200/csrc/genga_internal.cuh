@@ -1,0 +1,112 @@
+// genga_internal.cuh -- handle layout, workspace carving and kernel launchers shared by the
+// translation units of libgenga_b200.  Product code: nothing here is used by oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/genga.h"
+
+namespace genga {
+
+// ---- tiling constants -------------------------------------------------
+constexpr int CHUNK      = 64;                  // j-bodies per chunk: granularity of the near-field flag
+constexpr int STAGE_CH   = 8;                   // chunks per shared-memory stage
+constexpr int STAGE_J    = CHUNK * STAGE_CH;    // 512 j-bodies per stage
+constexpr int NSTAGE     = 2;                   // double buffering
+constexpr int KICK_NT    = 128;                 // threads per CTA of the all-pairs kernels
+constexpr int KICK32_I   = 4;                   // i-bodies per thread, FP32 kernel
+constexpr int KICK64_I   = 4;                   // i-bodies per thread, FP64 kernel
+constexpr int PAD_BODIES = 512;                 // N is padded to a multiple of this (stage and i-block size)
+constexpr double PAD_POS = 1.0e15;              // position of padding bodies (gm = 0, far from everything)
+
+// per-body / per-chunk parameters of the conservative near-field bound (all FP32, rounded up):
+//   B_ic = max( max(hq_i, Hq_c) * max(aq_i, Aq_c), max(rf_i, Rf_c) ),  bound_ic = B_ic^2
+struct __align__(16) BoundP { float hq, aq, rf, pad; };
+
+// j-side layouts.  FP32: two bodies per 32 bytes (packed for FFMA2 along j):
+//   float4 A = (x0, x1, y0, y1), float4 B = (z0, z1, gm0, gm1).
+// FP64: double4 (x, y, z, gm) per body.
+struct Counters {
+    unsigned int cand_count;     // (body, chunk) candidates pushed by the all-pairs kernel
+    unsigned int pair_count;     // encounter pairs appended by the near-field kernel
+    unsigned int noconv;         // bodies whose Kepler solve did not converge (sticky until read)
+    unsigned int overflow;       // 1 if the last near-field pass took the exact slow path
+};
+
+struct Workspace {
+    // state (API layout)
+    double* m;        // [NP]
+    double* x;        // [NP][3]
+    double* v;        // [NP][3]
+    double* a;        // [NP][3]  acceleration of the last force evaluation
+    // per-body derived
+    double* hcbrt;    // [NP] cbrt(m / 3 M_star), cached when masses change
+    double* rcrit;    // [NP]
+    double* semi;     // [NP]
+    double* vkep;     // [NP]
+    double4* pk64;    // [NP]   (x, y, z, G m)
+    float4*  pk32;    // [NP]   pair-interleaved, see above
+    BoundP*  bi;      // [NP]   per-body bound parameters
+    BoundP*  bc;      // [NP/CHUNK] per-chunk maxima
+    // lists
+    int2*    cand;    // [cand_cap] (body, chunk)
+    int2*    pairs;   // [pair_cap] (i, j), i < j
+    // scratch
+    double*  red;     // [RED_DOUBLES] reduction scratch / results
+    double*  vtmp;    // [NP][3] staging for heliocentric-velocity output
+    Counters* ctr;
+};
+
+constexpr int RED_DOUBLES = 8 + 8 * 1024;   // [0..7] results, rest per-block partials
+
+struct Handle {
+    int N, NP, nchunk;
+    genga_params p;
+    double lambda_near, near_floor;
+    int pair_cap, cand_cap;
+    cudaStream_t stream;
+    Workspace w;
+    int num_sms;
+    long long launches;
+    // profiling
+    int prof;
+    static constexpr int NKT = 4;
+    static constexpr int EVPOOL = 64;
+    cudaEvent_t ev0[NKT][EVPOOL], ev1[NKT][EVPOOL];
+    int evn[NKT];
+    double ms_total[NKT];
+    long long ms_launches[NKT];
+    bool events_created;
+};
+
+size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace* w);
+
+// ---- kernel launchers (each in its own .cu) ---------------------------------------------------
+struct PrepArgs {
+    int N, NP;
+    double G, M_star, n1, n2, dt_rcrit;
+    int pair_rule;
+    float lambda, floor_rel;     // near-field policy for this evaluation
+};
+void launch_hcbrt(const Handle* h);
+void launch_pad(const Handle* h);                            // padding bodies: x = (PAD_POS,0,0), v = 0, m = 0
+void launch_prep(const Handle* h, const PrepArgs& a);
+void launch_kick32(const Handle* h);
+void launch_kick64(const Handle* h);
+void launch_nearfield(const Handle* h);
+void launch_velupdate(const Handle* h, double tau);
+void launch_momentum(const Handle* h);                       // red[0..2] = sum m v, red[3] = sum m
+void launch_shift_v(const Handle* h, double scale);          // v_i += scale * red[0..2]   (O1)
+void launch_sunkick(const Handle* h, double tau);            // x_i += tau * red[0..2] / M_star
+void launch_drift(const Handle* h, double dt);
+void launch_energy(const Handle* h);                         // red[0] = E, red[1..3] = L
+void launch_copy_v_helio(const Handle* h, double* out);      // out = v + red[0..2]/M_star
+int  run_peak_probe(int which, int iters, cudaStream_t s, double* ops_per_s, double* ms);
+
+// occupancy-derived grid of the all-pairs kernels
+int kick32_grid(const Handle* h);
+int kick64_grid(const Handle* h);
+
+}  // namespace genga

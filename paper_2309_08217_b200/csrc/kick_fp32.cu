@@ -1,0 +1,210 @@
+// kick_fp32.cu -- the all-pairs long-range kick in FP32 force precision (PAPER.md:19, 43, 223:
+// "Do Kick in single precision = 1").
+//
+// a_i = sum_{j != i} G m_j (x_j - x_i) / r_ij^3 over FAR pairs, mixed-precision policy P32
+// (DESIGN.md section 3): separations from FP32-rounded positions, packed FP32 arithmetic
+// (FFMA2/FADD2/FMUL2: two j-bodies per instruction), MUFU.RSQ, FP32 partial sums over one
+// 64-body j-chunk, chunk partials accumulated in FP64.  A (body, chunk) whose smallest r^2 is
+// not above the conservative bound (lambda * r_crit upper bound, position-rounding floor) is NOT
+// added: it is pushed to the candidate list and re-evaluated pair by pair in FP64 with the
+// changeover function by the near-field kernel (encounter forces always in FP64).
+//
+// Layout: 4 i-bodies per thread in registers; j-bodies streamed through shared memory in
+// 512-body stages by bulk asynchronous copies; one CTA owns a contiguous run of (i-block, chunk)
+// units so that 148 x occupancy CTAs carry equal work.
+#include "tile_pipeline.cuh"
+
+namespace genga {
+
+namespace {
+
+typedef unsigned long long f2;   // two packed floats (lo = even j, hi = odd j)
+
+__device__ __forceinline__ f2 pk(float lo, float hi)
+{
+    f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r;
+}
+__device__ __forceinline__ void upk(f2 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f2 add2(f2 a, f2 b)
+{
+    f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r;
+}
+__device__ __forceinline__ f2 mul2(f2 a, f2 b)
+{
+    f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r;
+}
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c)
+{
+    f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r;
+}
+__device__ __forceinline__ float rsq(float a)
+{
+    float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r;
+}
+__device__ __forceinline__ float min3(float a, float b, float c)
+{
+    float r; asm("min.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c)); return r;
+}
+
+constexpr int I  = KICK32_I;
+constexpr int NT = KICK_NT;
+constexpr int BI = I * NT;                       // i-bodies per i-block (= PAD_BODIES)
+
+struct __align__(16) Smem32 {
+    float4   j[NSTAGE][STAGE_J];                 // pair-interleaved j data, 16 B per body
+    BoundP   bc[NSTAGE][STAGE_CH];
+    uint64_t full[NSTAGE];
+};
+
+__global__ void __launch_bounds__(NT, 4)
+kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
+{
+    __shared__ Smem32 sm;
+    const int tid = threadIdx.x;
+
+    if (tid == 0) {
+        for (int s = 0; s < NSTAGE; ++s) mbar_init(&sm.full[s], 1);
+        fence_barrier_init();
+    }
+    __syncthreads();
+    uint32_t phase[NSTAGE] = {0u, 0u};
+
+    const long long U = (long long)nib * nchunk;
+    long long u0 = (U * (long long)blockIdx.x) / (long long)gridDim.x;
+    const long long u1 = (U * (long long)(blockIdx.x + 1)) / (long long)gridDim.x;
+
+    const float* pkf = reinterpret_cast<const float*>(w.pk32);
+
+    while (u0 < u1) {
+        const int ib = (int)(u0 / nchunk);
+        const int c0 = (int)(u0 - (long long)ib * nchunk);
+        const int c1 = (int)min((long long)nchunk, (long long)c0 + (u1 - u0));
+        u0 += (c1 - c0);
+
+        // ---- i-side registers ------------------------------------------------------------
+        float nx[I], ny[I], nz[I], hq[I], aq[I], rf[I];
+        bool  live[I];
+        double Ax[I], Ay[I], Az[I];
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const int i = ib * BI + k * NT + tid;
+            const float* f = pkf + 8 * (i >> 1) + (i & 1);
+            nx[k] = -f[0]; ny[k] = -f[2]; nz[k] = -f[4];
+            const BoundP b = w.bi[i];
+            hq[k] = b.hq; aq[k] = b.aq; rf[k] = b.rf;
+            live[k] = i < N;
+            Ax[k] = 0.0; Ay[k] = 0.0; Az[k] = 0.0;
+        }
+
+        const int nst = (c1 - c0 + STAGE_CH - 1) / STAGE_CH;
+        auto issue = [&](int st) {
+            const int cs  = c0 + st * STAGE_CH;
+            const int nch = min(STAGE_CH, c1 - cs);
+            const int b   = st & 1;
+            const uint32_t bytes_j = (uint32_t)nch * CHUNK * 16u;
+            const uint32_t bytes_b = (uint32_t)nch * 16u;
+            fence_proxy_async();
+            mbar_expect_tx(&sm.full[b], bytes_j + bytes_b);
+            bulk_g2s(&sm.j[b][0], w.pk32 + (size_t)cs * CHUNK, bytes_j, &sm.full[b]);
+            bulk_g2s(&sm.bc[b][0], w.bc + cs, bytes_b, &sm.full[b]);
+        };
+        if (tid == 0) { issue(0); if (nst > 1) issue(1); }
+
+        for (int st = 0; st < nst; ++st) {
+            const int b   = st & 1;
+            const int cs  = c0 + st * STAGE_CH;
+            const int nch = min(STAGE_CH, c1 - cs);
+            mbar_wait(&sm.full[b], phase[b]);
+            phase[b] ^= 1u;
+
+            for (int ch = 0; ch < nch; ++ch) {
+                const BoundP Bc = sm.bc[b][ch];
+                f2 ax[I], ay[I], az[I];
+                float mn[I];
+#pragma unroll
+                for (int k = 0; k < I; ++k) { ax[k] = 0ull; ay[k] = 0ull; az[k] = 0ull; mn[k] = 3.0e38f; }
+
+                const float4* jp = &sm.j[b][ch * CHUNK];
+#pragma unroll 2
+                for (int jj = 0; jj < CHUNK / 2; ++jj) {
+                    const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
+                    const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y), gj = pk(B.z, B.w);
+#pragma unroll
+                    for (int k = 0; k < I; ++k) {
+                        const f2 dx = add2(xj, pk(nx[k], nx[k]));
+                        const f2 dy = add2(yj, pk(ny[k], ny[k]));
+                        const f2 dz = add2(zj, pk(nz[k], nz[k]));
+                        f2 r2 = mul2(dx, dx);
+                        r2 = fma2(dy, dy, r2);
+                        r2 = fma2(dz, dz, r2);
+                        float r2a, r2b; upk(r2, r2a, r2b);
+                        mn[k] = min3(mn[k], r2a, r2b);
+                        const f2 y = pk(rsq(r2a), rsq(r2b));
+                        const f2 t = mul2(y, y);
+                        f2 s = mul2(y, gj);
+                        s = mul2(s, t);
+                        ax[k] = fma2(s, dx, ax[k]);
+                        ay[k] = fma2(s, dy, ay[k]);
+                        az[k] = fma2(s, dz, az[k]);
+                    }
+                }
+
+                // ---- chunk end: keep the FP32 partial or hand the chunk to the near field ----
+#pragma unroll
+                for (int k = 0; k < I; ++k) {
+                    const float Bq = fmaxf(fmaxf(hq[k], Bc.hq) * fmaxf(aq[k], Bc.aq), fmaxf(rf[k], Bc.rf));
+                    const float bound = live[k] ? Bq * Bq : -1.0f;
+                    const bool keep = mn[k] > bound;
+                    float lo, hi;
+                    upk(ax[k], lo, hi); const float px = lo + hi;
+                    upk(ay[k], lo, hi); const float py = lo + hi;
+                    upk(az[k], lo, hi); const float pz = lo + hi;
+                    Ax[k] += keep ? (double)px : 0.0;
+                    Ay[k] += keep ? (double)py : 0.0;
+                    Az[k] += keep ? (double)pz : 0.0;
+                    const unsigned int bal = __ballot_sync(0xffffffffu, !keep);
+                    if (bal)
+                        push_candidates(bal, !keep, ib * BI + k * NT + tid, cs + ch,
+                                        &w.ctr->cand_count, w.cand, cand_cap);
+                }
+            }
+            __syncthreads();                       // every thread is done reading buffer b
+            if (tid == 0 && st + 2 < nst) issue(st + 2);
+        }
+
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            if (live[k]) {
+                const int i = ib * BI + k * NT + tid;
+                atomicAdd(&w.a[3 * i + 0], Ax[k]);
+                atomicAdd(&w.a[3 * i + 1], Ay[k]);
+                atomicAdd(&w.a[3 * i + 2], Az[k]);
+            }
+        }
+    }
+}
+
+}  // namespace
+
+int kick32_grid(const Handle* h)
+{
+    int occ = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kick32_kernel, NT, 0);
+    if (occ < 1) occ = 1;
+    return h->num_sms * occ;
+}
+
+void launch_kick32(const Handle* h)
+{
+    if (h->N == 0) return;
+    const int nib = h->NP / BI;
+    const long long U = (long long)nib * h->nchunk;
+    long long G = kick32_grid(h);
+    if (G > U) G = U;
+    kick32_kernel<<<(int)G, NT, 0, h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
+}
+
+}  // namespace genga

@@ -1,0 +1,183 @@
+// kick_fp64.cu -- the all-pairs long-range kick in FP64 (GENGA's default).
+//
+// a_i = sum_{j != i} G m_j (x_j - x_i) / r_ij^3 over pairs OUTSIDE the changeover zone, every
+// operation in FP64.  1/r^3 comes from the 20-bit MUFU.RSQ64H seed y0 and one cubic correction:
+//   t = y0^2, e = 1 - r^2 t, 1/r^3 = y0^3 (1 - e)^(-3/2) = y0^3 (1 + 3/2 e + 15/8 e^2) + O(e^3),
+// |e| <~ 2^-19 so the truncation is < 1e-17 relative.  16 FP64-pipe
+// instructions per pair.  A (body, 64-j chunk) whose smallest r^2 is not above the conservative
+// r_crit bound is not added but handed to the near-field kernel, which applies K pair by pair.
+#include "tile_pipeline.cuh"
+
+namespace genga {
+
+namespace {
+
+__device__ __forceinline__ double rsq64h(double a)
+{
+    double r; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r;
+}
+
+constexpr int I  = KICK64_I;
+constexpr int NT = KICK_NT;
+constexpr int BI = PAD_BODIES;                   // i-bodies per i-block
+static_assert(I * NT == BI, "FP64 i-block must equal the padding unit");
+
+struct __align__(16) Smem64 {
+    double4  j[NSTAGE][STAGE_J];                 // (x, y, z, G m), 32 B per body
+    BoundP   bc[NSTAGE][STAGE_CH];
+    uint64_t full[NSTAGE];
+};
+
+__global__ void __launch_bounds__(NT, 4)
+kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
+{
+    extern __shared__ __align__(16) unsigned char smraw[];
+    Smem64& sm = *reinterpret_cast<Smem64*>(smraw);
+    const int tid = threadIdx.x;
+
+    if (tid == 0) {
+        for (int s = 0; s < NSTAGE; ++s) mbar_init(&sm.full[s], 1);
+        fence_barrier_init();
+    }
+    __syncthreads();
+    uint32_t phase[NSTAGE] = {0u, 0u};
+
+    const long long U = (long long)nib * nchunk;
+    long long u0 = (U * (long long)blockIdx.x) / (long long)gridDim.x;
+    const long long u1 = (U * (long long)(blockIdx.x + 1)) / (long long)gridDim.x;
+
+    while (u0 < u1) {
+        const int ib = (int)(u0 / nchunk);
+        const int c0 = (int)(u0 - (long long)ib * nchunk);
+        const int c1 = (int)min((long long)nchunk, (long long)c0 + (u1 - u0));
+        u0 += (c1 - c0);
+
+        double xi[I], yi[I], zi[I];
+        float hq[I], aq[I], rf[I];
+        bool live[I];
+        double Ax[I], Ay[I], Az[I];
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const int i = ib * BI + k * NT + tid;
+            const double4 q = w.pk64[i];
+            xi[k] = q.x; yi[k] = q.y; zi[k] = q.z;
+            const BoundP b = w.bi[i];
+            hq[k] = b.hq; aq[k] = b.aq; rf[k] = b.rf;
+            live[k] = i < N;
+            Ax[k] = 0.0; Ay[k] = 0.0; Az[k] = 0.0;
+        }
+
+        const int nst = (c1 - c0 + STAGE_CH - 1) / STAGE_CH;
+        auto issue = [&](int st) {
+            const int cs  = c0 + st * STAGE_CH;
+            const int nch = min(STAGE_CH, c1 - cs);
+            const int b   = st & 1;
+            const uint32_t bytes_j = (uint32_t)nch * CHUNK * 32u;
+            const uint32_t bytes_b = (uint32_t)nch * 16u;
+            fence_proxy_async();
+            mbar_expect_tx(&sm.full[b], bytes_j + bytes_b);
+            bulk_g2s(&sm.j[b][0], w.pk64 + (size_t)cs * CHUNK, bytes_j, &sm.full[b]);
+            bulk_g2s(&sm.bc[b][0], w.bc + cs, bytes_b, &sm.full[b]);
+        };
+        if (tid == 0) { issue(0); if (nst > 1) issue(1); }
+
+        for (int st = 0; st < nst; ++st) {
+            const int b   = st & 1;
+            const int cs  = c0 + st * STAGE_CH;
+            const int nch = min(STAGE_CH, c1 - cs);
+            mbar_wait(&sm.full[b], phase[b]);
+            phase[b] ^= 1u;
+
+            for (int ch = 0; ch < nch; ++ch) {
+                const BoundP Bc = sm.bc[b][ch];
+                double ax[I], ay[I], az[I];
+                int mn[I];                        // high word of the smallest r^2 (orders like r^2 >= 0)
+#pragma unroll
+                for (int k = 0; k < I; ++k) { ax[k] = 0.0; ay[k] = 0.0; az[k] = 0.0; mn[k] = 0x7fffffff; }
+
+                const double4* jp = &sm.j[b][ch * CHUNK];
+#pragma unroll 2
+                for (int jj = 0; jj < CHUNK; ++jj) {
+                    const double4 J = jp[jj];
+#pragma unroll
+                    for (int k = 0; k < I; ++k) {
+                        const double dx = J.x - xi[k];
+                        const double dy = J.y - yi[k];
+                        const double dz = J.z - zi[k];
+                        double r2 = dx * dx;
+                        r2 = fma(dy, dy, r2);
+                        r2 = fma(dz, dz, r2);
+                        mn[k] = min(mn[k], __double2hiint(r2));
+                        const double y0 = rsq64h(r2);
+                        const double t  = y0 * y0;
+                        const double e  = fma(-r2, t, 1.0);
+                        const double c  = fma(1.875, e, 1.5);
+                        const double q  = (J.w * y0) * t;
+                        const double qe = q * e;
+                        const double s  = fma(qe, c, q);
+                        ax[k] = fma(s, dx, ax[k]);
+                        ay[k] = fma(s, dy, ay[k]);
+                        az[k] = fma(s, dz, az[k]);
+                    }
+                }
+
+#pragma unroll
+                for (int k = 0; k < I; ++k) {
+                    const float Bq = fmaxf(fmaxf(hq[k], Bc.hq) * fmaxf(aq[k], Bc.aq), fmaxf(rf[k], Bc.rf));
+                    // bound in FP64, rounded up by one FP32 ulp-ish factor; compare high words only:
+                    // equal high words count as "near" (conservative).
+                    const double bd = (double)Bq * (double)Bq * 1.000001;
+                    const int bh = live[k] ? __double2hiint(bd) : -1;
+                    const bool keep = mn[k] > bh;
+                    Ax[k] += keep ? ax[k] : 0.0;
+                    Ay[k] += keep ? ay[k] : 0.0;
+                    Az[k] += keep ? az[k] : 0.0;
+                    const unsigned int bal = __ballot_sync(0xffffffffu, !keep);
+                    if (bal)
+                        push_candidates(bal, !keep, ib * BI + k * NT + tid, cs + ch,
+                                        &w.ctr->cand_count, w.cand, cand_cap);
+                }
+            }
+            __syncthreads();
+            if (tid == 0 && st + 2 < nst) issue(st + 2);
+        }
+
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            if (live[k]) {
+                const int i = ib * BI + k * NT + tid;
+                atomicAdd(&w.a[3 * i + 0], Ax[k]);
+                atomicAdd(&w.a[3 * i + 1], Ay[k]);
+                atomicAdd(&w.a[3 * i + 2], Az[k]);
+            }
+        }
+    }
+}
+
+}  // namespace
+
+static bool s_attr_set = false;
+
+int kick64_grid(const Handle* h)
+{
+    if (!s_attr_set) {
+        cudaFuncSetAttribute(kick64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem64));
+        s_attr_set = true;
+    }
+    int occ = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kick64_kernel, NT, sizeof(Smem64));
+    if (occ < 1) occ = 1;
+    return h->num_sms * occ;
+}
+
+void launch_kick64(const Handle* h)
+{
+    if (h->N == 0) return;
+    const int nib = h->NP / BI;
+    const long long U = (long long)nib * h->nchunk;
+    long long G = kick64_grid(h);
+    if (G > U) G = U;
+    kick64_kernel<<<(int)G, NT, sizeof(Smem64), h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
+}
+
+}  // namespace genga
