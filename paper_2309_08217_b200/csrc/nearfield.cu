@@ -74,10 +74,10 @@ __device__ __forceinline__ void chunk_on_body(const NfParams& P, Workspace& w, i
             const double dx = q.x - xi, dy = q.y - yi, dz = q.z - zi;
             const double r2 = dx * dx + dy * dy + dz * dz;
             const double r  = sqrt(r2);
+            const double rc = pair_rcrit(P, mi, w.m[j], rci, w.rcrit[j], ai, w.semi[j], vki, w.vkep[j]);
+            enc = (i < j) && (r < rc);                     // coincident bodies (r = 0) are an encounter
             if (r > 0.0) {
-                const double rc = pair_rcrit(P, mi, w.m[j], rci, w.rcrit[j], ai, w.semi[j], vki, w.vkep[j]);
-                const double W  = changeover(r, rc);
-                enc = (i < j) && (r < rc);
+                const double W = changeover(r, rc);
                 if (W != 0.0) {
                     const double s = q.w * W / (r2 * r);
                     sx = s * dx; sy = s * dy; sz = s * dz;
