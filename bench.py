@@ -1,0 +1,395 @@
+#!/usr/bin/env python
+"""bench.py -- the headline benchmark of the GENGA level-0 hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--n N_BODIES] [--sweep]
+    python bench.py --impl reference ...        # the CPU oracle, as it stands, on the host cores
+
+One "step" is one pass of the whole hot path over the workload: S(dt/2) D(dt) S(dt/2) K(dt), the
+body of the merged-leapfrog loop of genga_run (one force evaluation per step: r_crit, packing,
+all-pairs kick, FP64 near field + encounter list, velocity update, Sun-kick, Kepler drift).
+The default workload is BASELINE.json configs[4]: 40 000 self-gravitating planetesimals.
+Metric: ordered pair interactions per second, N (N - 1) per force evaluation;
+steps/s and N x steps/s ("steps per second per particle") are reported beside it
+for FP32 (headline; the paper's contribution) and FP64 force precision.
+
+Prints ONE JSON line on rank 0.  Under torchrun every rank integrates its own, independently
+seeded, system of the same shape (the path shards over independent problems: weak scaling, no
+data-path collective); time is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pair interactions/s & steps/s per body at N=40k, FP32 vs FP64 forces"
+UNIT = "pair interactions/s"
+# flops per ordered pair interaction, the stated convention
+FLOP_FP32, FLOP_FP64 = 18.0, 25.0
+SMS, SM_MAX_HZ = 148, 1.965e9
+PEAK_FP32_TFLOPS = SMS * 128 * 2 * SM_MAX_HZ / 1e12      # 74.45: 128 FP32 lanes/SM, FMA = 2 flop
+PEAK_FP64_TFLOPS = SMS * 64 * 2 * SM_MAX_HZ / 1e12       # 37.22: 64 FP64 lanes/SM (DFMA probe confirms)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--n", type=int, default=None, help="override the body count of the config")
+    ap.add_argument("--sweep", action="store_true", help="also run the N = 2^10..2^17 sweep (extra JSON key)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed steps")
+    return ap.parse_args()
+
+
+def dist_env():
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")),
+            int(os.environ.get("WORLD_SIZE", "1")))
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        self.index, self.period = index, period_s
+        self.sm, self.reasons, self.power = [], set(), []
+        self.sm_max = None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nv = None
+
+    def _loop(self):
+        nv = self._nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+        }
+        while not self._stop.is_set():
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                for k, bit in names.items():
+                    if mask & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        return {"sm_mhz": statistics.median(self.sm) if self.sm else None,
+                "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons),
+                "power_w_max": max(self.power) if self.power else None, "samples": len(self.sm)}
+
+
+def make_workload(args, rank):
+    from paper_2309_08217_b200 import workloads as W
+    w = W.config(args.config, args.n)
+    if rank > 0 and args.config in (0, 1, 4):          # every rank its own independently seeded system
+        tot = {0: 2.5, 1: 5.0, 4: 5.0}[args.config]
+        w = W.planetesimal_disc(w.N, tot, w.seed + 7919 * rank, args.config, w.name, w.dt, w.nsteps)
+    return w
+
+
+def time_steps(torch, g, w, prec, steps, warmup, flush_buf, dist):
+    """K timed steps, each bracketed by CUDA events on the handle's stream; L2 flushed between."""
+    stream = torch.cuda.current_stream()
+    g.kick(0.5 * w.dt, prec)                           # opening half kick of the merged leapfrog
+    for _ in range(warmup):
+        g.leapfrog(w.dt, 1, prec)
+    g.synchronize()
+    for k in range(4):
+        g.kernel_time(k, reset=True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    l0 = g.launch_count()
+    t0 = time.perf_counter()
+    for s in range(steps):
+        if flush_buf is not None:
+            flush_buf.zero_()                          # > L2 capacity, untimed
+        ev[s][0].record(stream)
+        g.leapfrog(w.dt, 1, prec)
+        ev[s][1].record(stream)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    if dist is not None:
+        dist.barrier()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(ms))
+    launches = g.launch_count() - l0
+    kt = [g.kernel_time(k, reset=True) for k in range(4)]
+    return {"total_ms": total_ms, "ms_median": statistics.median(ms), "wall_s": wall,
+            "launches": launches, "kernel_ms": [(t / max(n, 1)) for t, n in kt],
+            "kernel_n": [n for _, n in kt]}
+
+
+def time_e2e(torch, g, w, prec, steps, warmup, flush_buf):
+    """The same step through the C ABI with HOST buffers: pinned host -> device copy of (m, x, v),
+    one step, device -> host read of (x, v); every step, inside the timed region."""
+    import numpy as np
+    stream = torch.cuda.current_stream()
+    m = torch.from_numpy(w.m).pin_memory()
+    x = torch.from_numpy(np.ascontiguousarray(w.x)).pin_memory()
+    v = torch.from_numpy(np.ascontiguousarray(w.v)).pin_memory()
+    xo, vo = torch.empty_like(x).pin_memory(), torch.empty_like(v).pin_memory()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for s in range(-warmup, steps):
+        if flush_buf is not None:
+            flush_buf.zero_()
+        if s >= 0:
+            ev[s][0].record(stream)
+        g.set_state_host(m, x, v)
+        g.leapfrog(w.dt, 1, prec)
+        g.get_state_host(xo, vo, heliocentric_v=True)  # synchronises
+        if s >= 0:
+            ev[s][1].record(stream)
+        x.copy_(xo); v.copy_(vo)                       # host-side hand-over to the next step
+    torch.cuda.synchronize()
+    total_ms = float(sum(a.elapsed_time(b) for a, b in ev))
+    h2d = m.numel() * 8 + x.numel() * 8 + v.numel() * 8
+    d2h = xo.numel() * 8 + vo.numel() * 8
+    return total_ms, h2d, d2h
+
+
+def cpu_oracle_steps(w, steps, warmup=0):
+    """The oracle, as it stands, on the host cores: `steps` merged-leapfrog steps (each one full
+    O(N^2) oracle force evaluation + Sun-kick + Kepler drift).  Returns (seconds, threads)."""
+    import oracle
+    p = oracle.Params(G=w.G, M_star=w.M_star, n1=w.n1, n2=w.n2, dt_rcrit=w.dt, pair_rule=w.pair_rule)
+    x, v = w.x.copy(), oracle.to_democratic(w.m, w.v, w.M_star)
+    times = []
+    for s in range(-warmup, steps):
+        t0 = time.perf_counter()
+        x = oracle.sunkick(w.m, x, v, p, 0.5 * w.dt)
+        x, v = oracle.drift(x, v, p, w.dt)
+        x = oracle.sunkick(w.m, x, v, p, 0.5 * w.dt)
+        v, _ = oracle.kick(w.m, x, v, p, w.dt)
+        if s >= 0:
+            times.append(time.perf_counter() - t0)
+    return times, oracle.num_threads()
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    w = make_workload(args, 0)
+    steps = max(1, min(args.steps, 3))                 # bounded sample: a few full O(N^2) steps
+    times, threads = cpu_oracle_steps(w, steps, warmup=min(args.warmup, 1))
+    pairs = w.N * (w.N - 1.0)
+    total = sum(times)
+    value = pairs * steps / total
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * total / steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "N": w.N, "dt_days": w.dt, "requested_steps": args.steps,
+                   "note": "CPU FP64 oracle (oracle/genga_oracle.c, -O2, OpenMP over i), not a GPU program"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                         "sample": f"{steps} full merged-leapfrog step(s) of the N={w.N} workload"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_cuda(args):
+    import torch
+    from paper_2309_08217_b200 import binding as B
+    from paper_2309_08217_b200 import workloads as W
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the GENGA hot path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    B.load()
+
+    w = make_workload(args, rank)
+    N, pairs = w.N, w.N * (w.N - 1.0)
+    dev = f"cuda:{local_rank}"
+    flush = None if args.no_flush else torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    res, e2e = {}, {}
+    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else local_rank)
+    with sampler:
+        for prec, name in ((B.FP32, "fp32"), (B.FP64, "fp64")):
+            g = B.from_workload(w, device=dev)
+            g.set_profiling(True)
+            r = time_steps(torch, g, w, prec, args.steps, args.warmup, flush, dist)
+            st = g.nearfield_stats()
+            r["candidates"], r["overflowed"] = st.candidates, st.overflowed
+            r["encounter_pairs"] = int(len(g.encounter_pairs(cap=4 * N + 1024)))
+            res[name] = r
+            g.close()
+    # energy / angular-momentum drift over the timed run length, both precisions (reported)
+    drift = {}
+    for prec, name in ((B.FP32, "fp32"), (B.FP64, "fp64")):
+        g = B.from_workload(w, device=dev)
+        E0, L0 = g.energy_angmom()
+        g.run(w.dt, args.steps, prec)
+        E1, L1 = g.energy_angmom()
+        import numpy as np
+        drift[name] = {"dE_over_E": E1 / E0 - 1.0,
+                       "dL_over_L": float(np.linalg.norm(L1) / np.linalg.norm(L0) - 1.0)}
+        g.close()
+    e2e_steps = min(args.steps, 50)
+    for prec, name in ((B.FP32, "fp32"), (B.FP64, "fp64")):
+        g = B.from_workload(w, device=dev)
+        ms, h2d, d2h = time_e2e(torch, g, w, prec, e2e_steps, min(args.warmup, 3), flush)
+        e2e[name] = (ms, h2d, d2h)
+        g.close()
+
+    # max over ranks of the timed totals
+    tot = torch.tensor([res["fp32"]["total_ms"], res["fp64"]["total_ms"], e2e["fp32"][0], e2e["fp64"][0]],
+                       dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+    t32, t64, te32, te64 = (float(t) for t in tot.tolist())
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    K = args.steps
+    def per_prec(name, total_ms, flop, peak):
+        r = res[name]
+        pps = world * pairs * K / (total_ms * 1e-3)
+        kick_ms = r["kernel_ms"][0]
+        tf = flop * pairs / (kick_ms * 1e-3) / 1e12
+        return {"pair_interactions_per_s": pps, "steps_per_s": K / (total_ms * 1e-3),
+                "body_steps_per_s": world * N * K / (total_ms * 1e-3), "ms_per_step": total_ms / K,
+                "kernel_ms": {"kick": r["kernel_ms"][0], "nearfield": r["kernel_ms"][1],
+                              "prep": r["kernel_ms"][2], "drift": r["kernel_ms"][3]},
+                "kick_kernel_pairs_per_s": pairs / (kick_ms * 1e-3),
+                "kick_kernel_tflops": tf, "kick_kernel_frac_of_peak": tf / peak,
+                "step_frac_of_peak": flop * pairs * K / (total_ms * 1e-3) / 1e12 / peak,
+                "flop_per_pair": flop, "nearfield_candidates": r["candidates"],
+                "candidate_overflow": r["overflowed"], "encounter_pairs_last": r["encounter_pairs"],
+                **drift[name]}
+    p32 = per_prec("fp32", t32, FLOP_FP32, PEAK_FP32_TFLOPS)
+    p64 = per_prec("fp64", t64, FLOP_FP64, PEAK_FP64_TFLOPS)
+
+    line = {
+        "metric": METRIC, "value": p32["pair_interactions_per_s"], "unit": UNIT, "n_gpus": world,
+        "steps": K, "warmup": args.warmup, "ms_per_step": t32 / K, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "N": N, "dt_days": w.dt, "headline_precision": "fp32",
+                   "step": "S(dt/2) D(dt) S(dt/2) K(dt): one force evaluation per step",
+                   "l2": "inputs are L2-resident by nature (1.6 MB); L2 flushed by a 256 MiB write between timed steps"
+                         if flush is not None else "no flush",
+                   "per_rank": "independent system per rank, no data-path collective"},
+        "precisions": {"fp32": p32, "fp64": p64},
+        "roofline": {"bound": "alu", "kernel": "kick32_kernel", "achieved": p32["kick_kernel_tflops"],
+                     "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s", "frac": p32["kick_kernel_frac_of_peak"],
+                     "traffic": None,
+                     "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md section 6); "
+                                    "MEASURED_PEAKS.json has no FP32/FP64 ALU figure",
+                     "flop_per_pair": FLOP_FP32,
+                     "fp64": {"kernel": "kick64_kernel", "achieved": p64["kick_kernel_tflops"],
+                              "peak": PEAK_FP64_TFLOPS, "frac": p64["kick_kernel_frac_of_peak"],
+                              "flop_per_pair": FLOP_FP64}},
+        "e2e": {"value": world * pairs * e2e_steps / (te32 * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": e2e["fp32"][1], "d2h_bytes_per_step": e2e["fp32"][2], "steps": e2e_steps,
+                "fp64_value": world * pairs * e2e_steps / (te64 * 1e-3)},
+        "gpu_launches": res["fp32"]["launches"],
+        "clocks": sampler.summary(),
+    }
+    return line, w
+
+
+def alu_probes():
+    """Measured issue rates of this GPU (register-only kernels, genga_peak_probe), as TFLOP/s."""
+    from paper_2309_08217_b200 import binding as B
+    out = {}
+    for which, name, flop in ((0, "ffma_tflops", 2.0), (1, "ffma2_tflops", 2.0), (2, "dfma_tflops", 2.0),
+                              (3, "mufu_rsq_gops", 1.0), (4, "mufu_rsq64h_gops", 1.0)):
+        ops, _ = B.peak_probe(which, 2048)
+        out[name] = ops * flop / (1e12 if flop == 2.0 else 1e9)
+    return out
+
+
+def run_sweep(args):
+    """N = 2^10 .. 2^17 (BASELINE.json configs[4]): N x steps/s per precision, device-timed."""
+    import torch
+    from paper_2309_08217_b200 import binding as B
+    from paper_2309_08217_b200 import workloads as W
+    out = []
+    for n in W.SWEEP_N:
+        w = W.config(4, n)
+        row = {"N": n}
+        steps = 50 if n <= 32768 else 10
+        for prec, name in ((B.FP32, "fp32"), (B.FP64, "fp64")):
+            g = B.from_workload(w)
+            g.set_profiling(True)
+            r = time_steps(torch, g, w, prec, steps, 3, None, None)
+            row[name] = {"ms_per_step": r["total_ms"] / steps, "body_steps_per_s": n * steps / (r["total_ms"] * 1e-3),
+                         "pair_interactions_per_s": n * (n - 1.0) * steps / (r["total_ms"] * 1e-3),
+                         "kick_kernel_ms": r["kernel_ms"][0], "nearfield_ms": r["kernel_ms"][1]}
+            g.close()
+        out.append(row)
+    return out
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    got = run_cuda(args)
+    if got is None:
+        return
+    line, w = got
+    line["alu_probe"] = alu_probes()
+    if line["n_gpus"] == 1 and not args.no_cpu_baseline:
+        times, threads = cpu_oracle_steps(w, 1 if w.N >= 20000 else 4)
+        pairs = w.N * (w.N - 1.0)
+        line["cpu_baseline"] = {"value": pairs * len(times) / sum(times), "unit": UNIT, "cores": threads,
+                                "kind": "oracle", "sample": f"{len(times)} full merged-leapfrog steps of the "
+                                f"N={w.N} workload ({sum(times):.1f} s of host time)"}
+    if args.sweep and line["n_gpus"] == 1:
+        line["sweep"] = run_sweep(args)
+    print(json.dumps(line), flush=True)
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -120,6 +120,11 @@ int genga_step(genga_handle h, double dt, int precision);
  * nsteps + 1 force evaluations (reading R7).                                          */
 int genga_run(genga_handle h, double dt, int nsteps, int precision);
 
+/* The body of that loop on its own: [S(dt/2) D(dt) S(dt/2) K(dt)]^nsteps, one force evaluation
+ * per step.  genga_kick(dt/2), genga_leapfrog(n), genga_kick(-dt/2) equals genga_run(n) up to
+ * rounding while r_crit does not depend on v (n2 = 0).                                          */
+int genga_leapfrog(genga_handle h, double dt, int nsteps, int precision);
+
 /* Encounter pairs {(i,j): i < j, r_ij < r_crit,ij} of the LAST force evaluation.
  * pairs_ij: HOST int[cap][2] (may be NULL if cap = 0); *count (HOST) receives the true total.
  * Order unspecified.  Synchronises the stream.                                                  */

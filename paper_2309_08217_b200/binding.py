@@ -24,7 +24,7 @@ OK, EINVAL, ENOMEM, ECAPACITY, ECUDA, ENOCONV = 0, -1, -2, -3, -4, -5
 SYMBOLS = [
     "genga_default_params", "genga_workspace_bytes", "genga_create", "genga_destroy",
     "genga_set_state", "genga_set_state_host", "genga_kick", "genga_accel", "genga_drift",
-    "genga_sunkick", "genga_step", "genga_run", "genga_encounter_pairs", "genga_energy_angmom",
+    "genga_sunkick", "genga_step", "genga_run", "genga_leapfrog", "genga_encounter_pairs", "genga_energy_angmom",
     "genga_get_state", "genga_get_state_host", "genga_get_accel", "genga_get_rcrit",
     "genga_nearfield_stats", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
     "genga_synchronize", "genga_strerror", "genga_last_cuda_error", "genga_version",
@@ -76,6 +76,7 @@ def load() -> ctypes.CDLL:
     L.genga_sunkick.argtypes = [vp, ctypes.c_double]
     L.genga_step.argtypes = [vp, ctypes.c_double, ctypes.c_int]
     L.genga_run.argtypes = [vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]
+    L.genga_leapfrog.argtypes = [vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]
     L.genga_encounter_pairs.argtypes = [vp, vp, ctypes.c_int, ip]
     L.genga_energy_angmom.argtypes = [vp, dp, dp]
     L.genga_get_state.argtypes = [vp, vp, vp, ctypes.c_int]
@@ -238,6 +239,9 @@ class Genga:
 
     def run(self, dt, nsteps, precision=FP64):
         _check(self._L.genga_run(self._h, float(dt), int(nsteps), int(precision)), "genga_run")
+
+    def leapfrog(self, dt, nsteps, precision=FP64):
+        _check(self._L.genga_leapfrog(self._h, float(dt), int(nsteps), int(precision)), "genga_leapfrog")
 
     def encounter_pairs(self, cap=None):
         """Returns an int32 numpy array (count, 2), i < j, of the last force evaluation."""

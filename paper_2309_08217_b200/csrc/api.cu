@@ -266,17 +266,26 @@ int genga_step(genga_handle h, double dt, int precision)
     return genga_kick(h, 0.5 * dt, precision);
 }
 
+int genga_leapfrog(genga_handle h, double dt, int nsteps, int precision)
+{
+    if (!h || nsteps < 0) return GENGA_EINVAL;
+    int rc;
+    for (int s = 0; s < nsteps; ++s) {
+        if ((rc = sds(h, dt)) != GENGA_OK) return rc;
+        if ((rc = genga_kick(h, dt, precision)) != GENGA_OK) return rc;
+    }
+    return GENGA_OK;
+}
+
 int genga_run(genga_handle h, double dt, int nsteps, int precision)
 {
     if (!h || nsteps < 0) return GENGA_EINVAL;
     if (nsteps == 0) return GENGA_OK;
     int rc;
     if ((rc = genga_kick(h, 0.5 * dt, precision)) != GENGA_OK) return rc;
-    for (int s = 0; s < nsteps; ++s) {
-        if ((rc = sds(h, dt)) != GENGA_OK) return rc;
-        if ((rc = genga_kick(h, (s + 1 < nsteps) ? dt : 0.5 * dt, precision)) != GENGA_OK) return rc;
-    }
-    return GENGA_OK;
+    if ((rc = genga_leapfrog(h, dt, nsteps - 1, precision)) != GENGA_OK) return rc;
+    if ((rc = sds(h, dt)) != GENGA_OK) return rc;
+    return genga_kick(h, 0.5 * dt, precision);
 }
 
 int genga_encounter_pairs(genga_handle h, int* pairs_ij, int cap, int* count)
@@ -366,7 +375,11 @@ int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed
     }
     if (candidates) *candidates = (long long)c.cand_count;
     if (overflowed) *overflowed = (int)c.overflow;
-    return c.noconv ? GENGA_ENOCONV : GENGA_OK;
+    if (c.noconv) {                                   // sticky until reported once
+        CU(cudaMemsetAsync(&h->w.ctr->noconv, 0, sizeof(unsigned int), h->stream));
+        return GENGA_ENOCONV;
+    }
+    return GENGA_OK;
 }
 
 int genga_set_profiling(genga_handle h, int enable)

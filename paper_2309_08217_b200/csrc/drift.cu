@@ -72,20 +72,27 @@ drift_kernel(int N, double mu, double dt_full, double* __restrict__ x, double* _
         s = s * (1.0 - 0.5 * a1 * s);
     }
     double c0 = 1, c1 = 1, c2 = 0.5, c3 = 1.0 / 6.0, G1 = 0, G2 = 0, r = r0;
-    bool ok = false;
+    bool ok = false, last = false;
     for (int it = 0; it < 32; ++it) {
         stumpff(alpha * s * s, c0, c1, c2, c3);
         G1 = s * c1;
         G2 = s * s * c2;
         const double G3 = s * s * s * c3;
-        const double F   = fma(r0, G1, fma(u, G2, mu * G3)) - dt;
-        r                = fma(r0, c0, fma(u, G1, mu * G2));
-        const double Fpp = fma(mu - alpha * r0, G1, u * c0);
+        const double t1 = r0 * G1, t2 = u * G2, t3 = mu * G3;
+        const double F  = ((t1 + t2) + t3) - dt;
+        r               = fma(r0, c0, fma(u, G1, mu * G2));
+        if (last) { ok = true; break; }                  // previous step was the final one
+        const double Fnoise = 4.0e-16 * (fabs(t1) + fabs(t2) + fabs(t3) + fabs(dt));
+        const double Fpp  = fma(mu - alpha * r0, G1, u * c0);
         const double disc = fabs(16.0 * r * r - 20.0 * F * Fpp);
         const double den  = r + copysign(sqrt(disc), r);
         const double ds   = -5.0 * F / den;
-        if (!(fabs(ds) > 1.0e-15 * fabs(s))) { ok = true; break; }   // G's at this s are final
+        // converged: the step is below the resolution of s, or the residual is rounding noise
+        if (!(fabs(ds) > 2.0e-15 * fabs(s)) || fabs(F) <= Fnoise) { ok = true; break; }
         s += ds;
+        // the iteration converges at third order: after a step below 1e-8 |s| the next
+        // correction is far below rounding, so only the G's are refreshed once more
+        last = fabs(ds) < 1.0e-8 * fabs(s);
     }
     if (!ok) atomicAdd(&ctr->noconv, 1u);
 
