@@ -70,16 +70,21 @@ typedef struct {
     int    pair_rule;         /* genga_pair_rule                                                       */
     int    v_is_heliocentric; /* 1: velocities given to create/set_state are heliocentric (O1)         */
     double lambda_near;       /* FP32 policy P32: pairs with r_ij < lambda_near * r_crit,ij (as bounded
-                                 per j-chunk) are evaluated in FP64.  <= 0 selects the default (8).    */
-    double near_floor;        /* FP32 policy P32: additionally every pair with r_ij < near_floor * max(|x_i|,
-                                 |x_j| bound) is evaluated in FP64 (position-rounding guard).
-                                 < 0 selects the default; 0 disables.                                   */
+                                 per j-chunk) are evaluated in FP64.  <= 0 selects the default (2).    */
+    double near_floor;        /* FP32 policy P32: the FP32 kernel sees positions relative to the origin
+                                 of each 64-body j-chunk; every pair with r_ij < near_floor * 2 R_chunk
+                                 (R_chunk = radius of the chunk about its origin) is evaluated in FP64
+                                 (position-rounding guard: relative separation error <= 2^-24 / near_floor).
+                                 < 0 selects the default (1/256); 0 disables.                           */
     void*  stream;            /* cudaStream_t owned by the caller; NULL = the legacy default stream    */
     void*  workspace;         /* DEVICE memory owned by the caller, 256-byte aligned                    */
     size_t workspace_bytes;
     int    pair_capacity;     /* capacity (pairs) of the encounter-pair list kept inside the workspace */
     int    cand_capacity;     /* capacity of the internal (body, j-chunk) near-field candidate list;
                                  <= 0 selects a default.  Overflow is handled exactly (slow path).      */
+    int    resort_every;      /* force evaluations between two refreshes of the internal body order
+                                 (heavy bodies first, then along a Hilbert curve in the x-y plane; a
+                                 performance hint only).  <= 0 selects the default (32).              */
 } genga_params;
 
 /* Fill *p with the defaults: G = k^2 (k = 0.01720209895), M_star = 1, n1 = 3, n2 = 0,
@@ -103,6 +108,10 @@ int genga_set_state_host(genga_handle h, const double* m, const double* x, const
 /* Kick: r_crit (Eq. 1), force evaluation in the given precision, encounter-pair list, and
  * v_i += dt * a_i with exactly the dt given (dt < 0 allowed).  PAPER.md:43, 55, 223.            */
 int genga_kick(genga_handle h, double dt, int precision);
+
+/* Refresh the internal body order now (it is refreshed automatically at the first force
+ * evaluation and then every params.resort_every evaluations).                                  */
+int genga_resort(genga_handle h);
 
 /* Force evaluation only (as genga_kick with the velocity update left out).                      */
 int genga_accel(genga_handle h, int precision);

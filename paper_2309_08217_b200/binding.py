@@ -23,7 +23,7 @@ OK, EINVAL, ENOMEM, ECAPACITY, ECUDA, ENOCONV = 0, -1, -2, -3, -4, -5
 # every symbol include/genga.h declares (tests check the library exports all of them)
 SYMBOLS = [
     "genga_default_params", "genga_workspace_bytes", "genga_create", "genga_destroy",
-    "genga_set_state", "genga_set_state_host", "genga_kick", "genga_accel", "genga_drift",
+    "genga_set_state", "genga_set_state_host", "genga_resort", "genga_kick", "genga_accel", "genga_drift",
     "genga_sunkick", "genga_step", "genga_run", "genga_leapfrog", "genga_encounter_pairs", "genga_energy_angmom",
     "genga_get_state", "genga_get_state_host", "genga_get_accel", "genga_get_rcrit",
     "genga_nearfield_stats", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
@@ -39,7 +39,7 @@ class GengaParams(ctypes.Structure):
         ("pair_rule", ctypes.c_int), ("v_is_heliocentric", ctypes.c_int),
         ("lambda_near", ctypes.c_double), ("near_floor", ctypes.c_double),
         ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
-        ("pair_capacity", ctypes.c_int), ("cand_capacity", ctypes.c_int),
+        ("pair_capacity", ctypes.c_int), ("cand_capacity", ctypes.c_int), ("resort_every", ctypes.c_int),
     ]
 
 
@@ -72,6 +72,7 @@ def load() -> ctypes.CDLL:
     L.genga_set_state_host.argtypes = [vp, vp, vp, vp]
     L.genga_kick.argtypes = [vp, ctypes.c_double, ctypes.c_int]
     L.genga_accel.argtypes = [vp, ctypes.c_int]
+    L.genga_resort.argtypes = [vp]
     L.genga_drift.argtypes = [vp, ctypes.c_double]
     L.genga_sunkick.argtypes = [vp, ctypes.c_double]
     L.genga_step.argtypes = [vp, ctypes.c_double, ctypes.c_int]
@@ -139,7 +140,7 @@ class Genga:
 
     def __init__(self, m, x, v, *, G=None, M_star=1.0, n1=3.0, n2=0.0, dt_rcrit=0.0,
                  pair_rule=PAIR_MUTUAL_HILL, v_is_heliocentric=True, lambda_near=0.0, near_floor=-1.0,
-                 pair_capacity=0, cand_capacity=0, stream=None, device=None):
+                 pair_capacity=0, cand_capacity=0, resort_every=0, stream=None, device=None):
         import torch
         self._torch = torch
         self._L = load()
@@ -154,6 +155,7 @@ class Genga:
         p.pair_rule, p.v_is_heliocentric = int(pair_rule), int(bool(v_is_heliocentric))
         p.lambda_near, p.near_floor = float(lambda_near), float(near_floor)
         p.pair_capacity, p.cand_capacity = int(pair_capacity), int(cand_capacity)
+        p.resort_every = int(resort_every)
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         p.stream = ctypes.c_void_p(self._stream.cuda_stream)
         nbytes = self._L.genga_workspace_bytes(self.N, ctypes.byref(p))
@@ -222,6 +224,9 @@ class Genga:
         return r
 
     # ---- the path ------------------------------------------------------------------------------
+    def resort(self):
+        _check(self._L.genga_resort(self._h), "genga_resort")
+
     def accel(self, precision=FP64):
         _check(self._L.genga_accel(self._h, int(precision)), "genga_accel")
 

@@ -40,17 +40,19 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
     const size_t o_m = take(NP * 8), o_x = take(NP * 24), o_v = take(NP * 24), o_a = take(NP * 24);
     const size_t o_h = take(NP * 8), o_rc = take(NP * 8), o_sa = take(NP * 8), o_vk = take(NP * 8);
-    const size_t o_p64 = take(NP * 32), o_p32 = take(NP * 16), o_bi = take(NP * 16), o_bc = take(NP / CHUNK * 16);
+    const size_t o_p64 = take(NP * 32), o_p32 = take(NP * 16), o_bi = take(NP * 16), o_bc = take(NP / CHUNK * sizeof(ChunkP));
     const size_t o_cand = take((size_t)cand_cap * 8), o_pairs = take((size_t)pair_cap * 8);
     const size_t o_red = take((size_t)RED_DOUBLES * 8), o_vt = take(NP * 24), o_ctr = take(sizeof(Counters));
+    const size_t o_ord = take(NP * 4), o_key = take(NP * 8), o_aux = take(NP * 32);
     if (w && base) {
         char* b = static_cast<char*>(base);
         w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
         w->hcbrt = (double*)(b + o_h); w->rcrit = (double*)(b + o_rc); w->semi = (double*)(b + o_sa);
         w->vkep = (double*)(b + o_vk); w->pk64 = (double4*)(b + o_p64); w->pk32 = (float4*)(b + o_p32);
-        w->bi = (BoundP*)(b + o_bi); w->bc = (BoundP*)(b + o_bc); w->cand = (int2*)(b + o_cand);
+        w->bi = (BoundP*)(b + o_bi); w->bc = (ChunkP*)(b + o_bc); w->cand = (int2*)(b + o_cand);
         w->pairs = (int2*)(b + o_pairs); w->red = (double*)(b + o_red); w->vtmp = (double*)(b + o_vt);
         w->ctr = (Counters*)(b + o_ctr);
+        w->order = (int*)(b + o_ord); w->keys = (unsigned long long*)(b + o_key); w->aux = (double4*)(b + o_aux);
     }
     return off;
 }
@@ -85,11 +87,27 @@ struct ProfScope {
     }
 };
 
+// Refresh the internal order (heavy bodies first, then by semi-major axis).
+static int resort(Handle* h)
+{
+    if (h->N == 0) return GENGA_OK;
+    launch_momentum(h); LAUNCHED(h, "momentum_kernel");     // red[3] = sum m (mean mass -> heavy class)
+    launch_sort(h); h->launches += 3;
+    { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_, "sort kernels"); }
+    h->evals_since_sort = 0;
+    return GENGA_OK;
+}
+
 // ---- force evaluation -------------------------------------------------------------------------
 static int force_eval(Handle* h, int precision)
 {
     if (precision != GENGA_FP64 && precision != GENGA_FP32) return GENGA_EINVAL;
     if (h->N == 0) return GENGA_OK;
+    if (h->evals_since_sort < 0 || h->evals_since_sort >= h->resort_every) {
+        const int rc = resort(h);
+        if (rc != GENGA_OK) return rc;
+    }
+    ++h->evals_since_sort;
     PrepArgs a;
     a.N = h->N; a.NP = h->NP;
     a.G = h->p.G; a.M_star = h->p.M_star; a.n1 = h->p.n1; a.n2 = h->p.n2; a.dt_rcrit = h->p.dt_rcrit;
@@ -142,6 +160,7 @@ void genga_default_params(genga_params* p)
     p->lambda_near = 0.0; p->near_floor = -1.0;
     p->stream = nullptr; p->workspace = nullptr; p->workspace_bytes = 0;
     p->pair_capacity = 0; p->cand_capacity = 0;
+    p->resort_every = 0;
 }
 
 size_t genga_workspace_bytes(int N, const genga_params* p)
@@ -154,7 +173,7 @@ size_t genga_workspace_bytes(int N, const genga_params* p)
 
 int genga_create(genga_handle* out, int N, const double* m, const double* x, const double* v, const genga_params* p)
 {
-    if (!out || !p || N < 0 || N > (1 << 24)) return GENGA_EINVAL;
+    if (!out || !p || N < 0 || N > (1 << 20)) return GENGA_EINVAL;
     if (!(p->M_star > 0.0) || !(p->G > 0.0)) return GENGA_EINVAL;
     if (p->pair_rule != GENGA_PAIR_MAX && p->pair_rule != GENGA_PAIR_MUTUAL_HILL) return GENGA_EINVAL;
     *out = nullptr;
@@ -173,10 +192,12 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     std::memset(static_cast<Handle*>(h), 0, sizeof(Handle));
     h->N = N; h->NP = padded(N); h->nchunk = h->NP / CHUNK;
     h->p = *p;
-    h->lambda_near = p->lambda_near > 0.0 ? p->lambda_near : 8.0;
+    h->lambda_near = p->lambda_near > 0.0 ? p->lambda_near : 2.0;
     h->near_floor  = p->near_floor >= 0.0 ? p->near_floor : (1.0 / 256.0);
     if (h->lambda_near < 1.0) h->lambda_near = 1.0;
     h->pair_cap = pc; h->cand_cap = cc;
+    h->resort_every = p->resort_every > 0 ? p->resort_every : 32;
+    h->evals_since_sort = -1;
     h->stream = static_cast<cudaStream_t>(p->stream);
     h->num_sms = sms;
     carve_workspace(N, pc, cc, p->workspace, &h->w);
@@ -223,6 +244,12 @@ int genga_set_state(genga_handle h, const double* m, const double* x, const doub
 int genga_set_state_host(genga_handle h, const double* m, const double* x, const double* v)
 {
     return set_state_impl(h, m, x, v, cudaMemcpyHostToDevice);
+}
+
+int genga_resort(genga_handle h)
+{
+    if (!h) return GENGA_EINVAL;
+    return resort(h);
 }
 
 int genga_accel(genga_handle h, int precision)

@@ -25,14 +25,23 @@ constexpr double PAD_POS = 1.0e15;              // position of padding bodies (g
 //   B_ic = max( max(hq_i, Hq_c) * max(aq_i, Aq_c), max(rf_i, Rf_c) ),  bound_ic = B_ic^2
 struct __align__(16) BoundP { float hq, aq, rf, pad; };
 
+// per-chunk record staged next to the j-tile: the maxima of the bound parameters over the chunk
+// and the origin of the chunk's local frame (FP32 policy P32: the FP32 kernel sees positions
+// relative to o; Rf already contains the frame guard floor * 2 * max_j |x_j - o|).
+struct __align__(16) ChunkP { double ox, oy, oz; float hq, aq, rf, rad; double pad_; };
+static_assert(sizeof(ChunkP) == 48, "ChunkP is staged with 16-byte bulk copies");
+
 // j-side layouts.  FP32: two bodies per 32 bytes (packed for FFMA2 along j):
 //   float4 A = (x0, x1, y0, y1), float4 B = (z0, z1, gm0, gm1).
 // FP64: double4 (x, y, z, gm) per body.
+// FP32 positions are relative to the origin of the body's own chunk (ChunkP).
 struct Counters {
     unsigned int cand_count;     // (body, chunk) candidates pushed by the all-pairs kernel
     unsigned int pair_count;     // encounter pairs appended by the near-field kernel
     unsigned int noconv;         // bodies whose Kepler solve did not converge (sticky until read)
     unsigned int overflow;       // 1 if the last near-field pass took the exact slow path
+    unsigned int ticket;         // block-completion ticket of the momentum reduction (0 between launches)
+    unsigned int extent_bits;    // float bits of max(|x|, |y|) over the bodies (Hilbert sort extent)
 };
 
 struct Workspace {
@@ -46,10 +55,14 @@ struct Workspace {
     double* rcrit;    // [NP]
     double* semi;     // [NP]
     double* vkep;     // [NP]
+    // arrays of one force evaluation, in the INTERNAL (sorted) order: slot s holds body order[s]
+    int*     order;   // [NP]   slot -> body index (API order); order[s] = s for the padding slots s >= N
+    unsigned long long* keys;   // [NP] sort keys (heavy class, semi-major axis, body index)
     double4* pk64;    // [NP]   (x, y, z, G m)
     float4*  pk32;    // [NP]   pair-interleaved, see above
+    double4* aux;     // [NP]   (m, r_crit, a, v_K): what the exact pair rule O3 needs
     BoundP*  bi;      // [NP]   per-body bound parameters
-    BoundP*  bc;      // [NP/CHUNK] per-chunk maxima
+    ChunkP*  bc;      // [NP/CHUNK] per-chunk maxima and frame origin
     // lists
     int2*    cand;    // [cand_cap] (body, chunk)
     int2*    pairs;   // [pair_cap] (i, j), i < j
@@ -59,7 +72,7 @@ struct Workspace {
     Counters* ctr;
 };
 
-constexpr int RED_DOUBLES = 8 + 8 * 1024;   // [0..7] results, rest per-block partials
+constexpr int RED_DOUBLES = 8 + 8 * 1024;   // [0..7] results, [8..8+4096) pair-potential partials, then momentum partials
 
 struct Handle {
     int N, NP, nchunk;
@@ -70,6 +83,10 @@ struct Handle {
     Workspace w;
     int num_sms;
     long long launches;
+    // internal order (a performance hint only: results never depend on it)
+    int resort_every;            // force evaluations between two sorts
+    int evals_since_sort;        // < 0: no order yet
+
     // profiling
     int prof;
     static constexpr int NKT = 4;
@@ -92,6 +109,7 @@ struct PrepArgs {
 };
 void launch_hcbrt(const Handle* h);
 void launch_pad(const Handle* h);                            // padding bodies: x = (PAD_POS,0,0), v = 0, m = 0
+void launch_sort(const Handle* h);                           // order[] by (heavy class, semi-major axis)
 void launch_prep(const Handle* h, const PrepArgs& a);
 void launch_kick32(const Handle* h);
 void launch_kick64(const Handle* h);

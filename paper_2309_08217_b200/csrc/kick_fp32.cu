@@ -54,8 +54,10 @@ constexpr int NT = KICK_NT;
 constexpr int BI = I * NT;                       // i-bodies per i-block (= PAD_BODIES)
 
 struct __align__(16) Smem32 {
-    float4   j[NSTAGE][STAGE_J];                 // pair-interleaved j data, 16 B per body
-    BoundP   bc[NSTAGE][STAGE_CH];
+    float4   j[NSTAGE][STAGE_J];                 // pair-interleaved j data (chunk-relative), 16 B per body
+    ChunkP   bc[NSTAGE][STAGE_CH];
+    double   xi[3][I][NT];                       // FP64 positions of this CTA's i-bodies
+    float    bp[3][I][NT];                       // their bound parameters (hq, aq, rf)
     uint64_t full[NSTAGE];
 };
 
@@ -76,26 +78,21 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
     long long u0 = (U * (long long)blockIdx.x) / (long long)gridDim.x;
     const long long u1 = (U * (long long)(blockIdx.x + 1)) / (long long)gridDim.x;
 
-    const float* pkf = reinterpret_cast<const float*>(w.pk32);
-
     while (u0 < u1) {
         const int ib = (int)(u0 / nchunk);
         const int c0 = (int)(u0 - (long long)ib * nchunk);
         const int c1 = (int)min((long long)nchunk, (long long)c0 + (u1 - u0));
         u0 += (c1 - c0);
 
-        // ---- i-side registers ------------------------------------------------------------
-        float nx[I], ny[I], nz[I], hq[I], aq[I], rf[I];
-        bool  live[I];
+        // ---- i-side: FP64 positions to shared memory (own column only), bound parameters to registers
         double Ax[I], Ay[I], Az[I];
 #pragma unroll
         for (int k = 0; k < I; ++k) {
             const int i = ib * BI + k * NT + tid;
-            const float* f = pkf + 8 * (i >> 1) + (i & 1);
-            nx[k] = -f[0]; ny[k] = -f[2]; nz[k] = -f[4];
+            const double4 q = w.pk64[i];
+            sm.xi[0][k][tid] = q.x; sm.xi[1][k][tid] = q.y; sm.xi[2][k][tid] = q.z;
             const BoundP b = w.bi[i];
-            hq[k] = b.hq; aq[k] = b.aq; rf[k] = b.rf;
-            live[k] = i < N;
+            sm.bp[0][k][tid] = b.hq; sm.bp[1][k][tid] = b.aq; sm.bp[2][k][tid] = b.rf;
             Ax[k] = 0.0; Ay[k] = 0.0; Az[k] = 0.0;
         }
 
@@ -105,7 +102,7 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
             const int nch = min(STAGE_CH, c1 - cs);
             const int b   = st & 1;
             const uint32_t bytes_j = (uint32_t)nch * CHUNK * 16u;
-            const uint32_t bytes_b = (uint32_t)nch * 16u;
+            const uint32_t bytes_b = (uint32_t)nch * (uint32_t)sizeof(ChunkP);
             fence_proxy_async();
             mbar_expect_tx(&sm.full[b], bytes_j + bytes_b);
             bulk_g2s(&sm.j[b][0], w.pk32 + (size_t)cs * CHUNK, bytes_j, &sm.full[b]);
@@ -121,11 +118,18 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
             phase[b] ^= 1u;
 
             for (int ch = 0; ch < nch; ++ch) {
-                const BoundP Bc = sm.bc[b][ch];
+                const ChunkP Bc = sm.bc[b][ch];
+                // i-positions in the chunk's frame: FP64 subtraction, then one rounding to FP32
+                float nx[I], ny[I], nz[I];
                 f2 ax[I], ay[I], az[I];
                 float mn[I];
 #pragma unroll
-                for (int k = 0; k < I; ++k) { ax[k] = 0ull; ay[k] = 0ull; az[k] = 0ull; mn[k] = 3.0e38f; }
+                for (int k = 0; k < I; ++k) {
+                    nx[k] = (float)(Bc.ox - sm.xi[0][k][tid]);
+                    ny[k] = (float)(Bc.oy - sm.xi[1][k][tid]);
+                    nz[k] = (float)(Bc.oz - sm.xi[2][k][tid]);
+                    ax[k] = 0ull; ay[k] = 0ull; az[k] = 0ull; mn[k] = 3.0e38f;
+                }
 
                 const float4* jp = &sm.j[b][ch * CHUNK];
 #pragma unroll 2
@@ -155,8 +159,9 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                 // ---- chunk end: keep the FP32 partial or hand the chunk to the near field ----
 #pragma unroll
                 for (int k = 0; k < I; ++k) {
-                    const float Bq = fmaxf(fmaxf(hq[k], Bc.hq) * fmaxf(aq[k], Bc.aq), fmaxf(rf[k], Bc.rf));
-                    const float bound = live[k] ? Bq * Bq : -1.0f;
+                    const float Bq = fmaxf(fmaxf(sm.bp[0][k][tid], Bc.hq) * fmaxf(sm.bp[1][k][tid], Bc.aq),
+                                           fmaxf(sm.bp[2][k][tid], Bc.rf));
+                    const float bound = (ib * BI + k * NT + tid < N) ? Bq * Bq : -1.0f;
                     const bool keep = mn[k] > bound;
                     float lo, hi;
                     upk(ax[k], lo, hi); const float px = lo + hi;
@@ -177,8 +182,8 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 
 #pragma unroll
         for (int k = 0; k < I; ++k) {
-            if (live[k]) {
-                const int i = ib * BI + k * NT + tid;
+            if (ib * BI + k * NT + tid < N) {
+                const int i = w.order[ib * BI + k * NT + tid];     // slot -> body (API order)
                 atomicAdd(&w.a[3 * i + 0], Ax[k]);
                 atomicAdd(&w.a[3 * i + 1], Ay[k]);
                 atomicAdd(&w.a[3 * i + 2], Az[k]);

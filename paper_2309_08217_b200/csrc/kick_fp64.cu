@@ -24,7 +24,8 @@ static_assert(I * NT == BI, "FP64 i-block must equal the padding unit");
 
 struct __align__(16) Smem64 {
     double4  j[NSTAGE][STAGE_J];                 // (x, y, z, G m), 32 B per body
-    BoundP   bc[NSTAGE][STAGE_CH];
+    ChunkP   bc[NSTAGE][STAGE_CH];
+    float    bp[3][I][NT];                       // bound parameters (hq, aq, rf) of this CTA's i-bodies
     uint64_t full[NSTAGE];
 };
 
@@ -53,8 +54,6 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
         u0 += (c1 - c0);
 
         double xi[I], yi[I], zi[I];
-        float hq[I], aq[I], rf[I];
-        bool live[I];
         double Ax[I], Ay[I], Az[I];
 #pragma unroll
         for (int k = 0; k < I; ++k) {
@@ -62,8 +61,7 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
             const double4 q = w.pk64[i];
             xi[k] = q.x; yi[k] = q.y; zi[k] = q.z;
             const BoundP b = w.bi[i];
-            hq[k] = b.hq; aq[k] = b.aq; rf[k] = b.rf;
-            live[k] = i < N;
+            sm.bp[0][k][tid] = b.hq; sm.bp[1][k][tid] = b.aq; sm.bp[2][k][tid] = b.rf;
             Ax[k] = 0.0; Ay[k] = 0.0; Az[k] = 0.0;
         }
 
@@ -73,7 +71,7 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
             const int nch = min(STAGE_CH, c1 - cs);
             const int b   = st & 1;
             const uint32_t bytes_j = (uint32_t)nch * CHUNK * 32u;
-            const uint32_t bytes_b = (uint32_t)nch * 16u;
+            const uint32_t bytes_b = (uint32_t)nch * (uint32_t)sizeof(ChunkP);
             fence_proxy_async();
             mbar_expect_tx(&sm.full[b], bytes_j + bytes_b);
             bulk_g2s(&sm.j[b][0], w.pk64 + (size_t)cs * CHUNK, bytes_j, &sm.full[b]);
@@ -89,7 +87,7 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
             phase[b] ^= 1u;
 
             for (int ch = 0; ch < nch; ++ch) {
-                const BoundP Bc = sm.bc[b][ch];
+                const ChunkP Bc = sm.bc[b][ch];
                 double ax[I], ay[I], az[I];
                 int mn[I];                        // high word of the smallest r^2 (orders like r^2 >= 0)
 #pragma unroll
@@ -123,11 +121,12 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 
 #pragma unroll
                 for (int k = 0; k < I; ++k) {
-                    const float Bq = fmaxf(fmaxf(hq[k], Bc.hq) * fmaxf(aq[k], Bc.aq), fmaxf(rf[k], Bc.rf));
+                    const float Bq = fmaxf(fmaxf(sm.bp[0][k][tid], Bc.hq) * fmaxf(sm.bp[1][k][tid], Bc.aq),
+                                           fmaxf(sm.bp[2][k][tid], Bc.rf));
                     // bound in FP64, rounded up by one FP32 ulp-ish factor; compare high words only:
                     // equal high words count as "near" (conservative).
                     const double bd = (double)Bq * (double)Bq * 1.000001;
-                    const int bh = live[k] ? __double2hiint(bd) : -1;
+                    const int bh = (ib * BI + k * NT + tid < N) ? __double2hiint(bd) : -1;
                     const bool keep = mn[k] > bh;
                     Ax[k] += keep ? ax[k] : 0.0;
                     Ay[k] += keep ? ay[k] : 0.0;
@@ -144,8 +143,8 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 
 #pragma unroll
         for (int k = 0; k < I; ++k) {
-            if (live[k]) {
-                const int i = ib * BI + k * NT + tid;
+            if (ib * BI + k * NT + tid < N) {
+                const int i = w.order[ib * BI + k * NT + tid];     // slot -> body (API order)
                 atomicAdd(&w.a[3 * i + 0], Ax[k]);
                 atomicAdd(&w.a[3 * i + 1], Ay[k]);
                 atomicAdd(&w.a[3 * i + 2], Az[k]);

@@ -58,33 +58,74 @@ __device__ __forceinline__ void append_pair(bool flag, int i, int j, Workspace& 
     }
 }
 
-// force of chunk c on body i, summed over the warp; lanes return the same total
-__device__ __forceinline__ void chunk_on_body(const NfParams& P, Workspace& w, int i, int c,
-                                              double xi, double yi, double zi, double mi, double rci,
-                                              double ai, double vki, double& fx, double& fy, double& fz)
+__device__ __forceinline__ double rsq64h(double a)
+{
+    double r; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r;
+}
+
+// what the warp holds of body (slot) si while it walks a chunk
+struct IBody {
+    int    slot, body;
+    double x, y, z;
+    double m, rc, a, vk;
+    float  hq, aq, rf;
+};
+
+__device__ __forceinline__ IBody load_ibody(const Workspace& w, int si)
+{
+    IBody b;
+    b.slot = si; b.body = w.order[si];
+    const double4 p = w.pk64[si]; b.x = p.x; b.y = p.y; b.z = p.z;
+    const double4 q = w.aux[si];  b.m = q.x; b.rc = q.y; b.a = q.z; b.vk = q.w;
+    const BoundP bp = w.bi[si];   b.hq = bp.hq; b.aq = bp.aq; b.rf = bp.rf;
+    return b;
+}
+
+// Force of chunk c on the body in slot si, partial per lane (two j per lane).  A pair outside the
+// conservative pair bound (the same bound the all-pairs kernels use per chunk, here per pair) has
+// K = 1 exactly and cannot be an encounter: it takes the cheap refined-rsqrt path.  Every other
+// pair is evaluated with plain sqrt / divide / cbrt: exact r < r_crit test, K, force.
+__device__ __forceinline__ void chunk_on_body(const NfParams& P, Workspace& w, const IBody& I, int c,
+                                              double& fx, double& fy, double& fz)
 {
     const int lane = threadIdx.x & 31;
 #pragma unroll
     for (int h = 0; h < CHUNK / 32; ++h) {
-        const int j = c * CHUNK + h * 32 + lane;
+        const int sj = c * CHUNK + h * 32 + lane;
         double sx = 0.0, sy = 0.0, sz = 0.0;
         bool enc = false;
-        if (j < P.N && j != i) {
-            const double4 q = w.pk64[j];
-            const double dx = q.x - xi, dy = q.y - yi, dz = q.z - zi;
-            const double r2 = dx * dx + dy * dy + dz * dz;
-            const double r  = sqrt(r2);
-            const double rc = pair_rcrit(P, mi, w.m[j], rci, w.rcrit[j], ai, w.semi[j], vki, w.vkep[j]);
-            enc = (i < j) && (r < rc);                     // coincident bodies (r = 0) are an encounter
-            if (r > 0.0) {
-                const double W = changeover(r, rc);
-                if (W != 0.0) {
-                    const double s = q.w * W / (r2 * r);
-                    sx = s * dx; sy = s * dy; sz = s * dz;
+        int bj = 0;
+        if (sj < P.N && sj != I.slot) {
+            const double4 q = w.pk64[sj];
+            const BoundP  b = w.bi[sj];
+            const double dx = q.x - I.x, dy = q.y - I.y, dz = q.z - I.z;
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            const float  Bq = fmaxf(fmaxf(I.hq, b.hq) * fmaxf(I.aq, b.aq), fmaxf(I.rf, b.rf));
+            const double bd = (double)Bq * (double)Bq * 1.000001;
+            if (r2 > bd) {
+                const double y0 = rsq64h(r2);
+                const double t  = y0 * y0;
+                const double e  = fma(-r2, t, 1.0);
+                const double cc = fma(1.875, e, 1.5);
+                const double g  = (q.w * y0) * t;
+                const double s  = fma(g * e, cc, g);
+                sx = s * dx; sy = s * dy; sz = s * dz;
+            } else {
+                const double4 A = w.aux[sj];
+                const double r  = sqrt(r2);
+                const double rc = pair_rcrit(P, I.m, A.x, I.rc, A.y, I.a, A.z, I.vk, A.w);
+                enc = (I.slot < sj) && (r < rc);           // coincident bodies (r = 0) are an encounter
+                if (enc) bj = w.order[sj];
+                if (r > 0.0) {
+                    const double W = changeover(r, rc);
+                    if (W != 0.0) {
+                        const double s = q.w * W / (r2 * r);
+                        sx = s * dx; sy = s * dy; sz = s * dz;
+                    }
                 }
             }
         }
-        append_pair(enc, i, j, w, P.pair_cap);
+        append_pair(enc, min(I.body, bj), max(I.body, bj), w, P.pair_cap);
         fx += sx; fy += sy; fz += sz;
     }
 }
@@ -107,28 +148,25 @@ nearfield_kernel(NfParams P, Workspace w)
     if (count <= P.cand_cap) {
         for (unsigned int q = warp; q < count; q += nwarp) {
             const int2 cd = w.cand[q];
-            const int i = cd.x, c = cd.y;
-            const double4 pi = w.pk64[i];
+            const IBody I = load_ibody(w, cd.x);
             double fx = 0.0, fy = 0.0, fz = 0.0;
-            chunk_on_body(P, w, i, c, pi.x, pi.y, pi.z, w.m[i], w.rcrit[i], w.semi[i], w.vkep[i], fx, fy, fz);
+            chunk_on_body(P, w, I, cd.y, fx, fy, fz);
             fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
             if (lane == 0) {
-                atomicAdd(&w.a[3 * i + 0], fx);
-                atomicAdd(&w.a[3 * i + 1], fy);
-                atomicAdd(&w.a[3 * i + 2], fz);
+                atomicAdd(&w.a[3 * I.body + 0], fx);
+                atomicAdd(&w.a[3 * I.body + 1], fy);
+                atomicAdd(&w.a[3 * I.body + 2], fz);
             }
         }
     } else {
         // exact slow path: the candidate list overflowed, redo every body against every chunk
         if (warp == 0 && lane == 0) w.ctr->overflow = 1u;
-        for (int i = warp; i < P.N; i += nwarp) {
-            const double4 pi = w.pk64[i];
-            const double mi = w.m[i], rci = w.rcrit[i], ai = w.semi[i], vki = w.vkep[i];
+        for (int si = warp; si < P.N; si += nwarp) {
+            const IBody I = load_ibody(w, si);
             double fx = 0.0, fy = 0.0, fz = 0.0;
-            for (int c = 0; c < P.nchunk; ++c)
-                chunk_on_body(P, w, i, c, pi.x, pi.y, pi.z, mi, rci, ai, vki, fx, fy, fz);
+            for (int c = 0; c < P.nchunk; ++c) chunk_on_body(P, w, I, c, fx, fy, fz);
             fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
-            if (lane == 0) { w.a[3 * i + 0] = fx; w.a[3 * i + 1] = fy; w.a[3 * i + 2] = fz; }
+            if (lane == 0) { w.a[3 * I.body + 0] = fx; w.a[3 * I.body + 1] = fy; w.a[3 * I.body + 2] = fz; }
         }
     }
 }

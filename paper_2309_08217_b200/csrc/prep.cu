@@ -31,17 +31,97 @@ __device__ __forceinline__ unsigned int warp_max_u32(unsigned int v)
     return __reduce_max_sync(0xffffffffu, v);
 }
 
+
+// ---- internal order ---------------------------------------------------------------------------
+// The all-pairs kernels flag (body, 64-j chunk) units with ONE conservative bound per unit, and
+// the FP32 kernel works in a local frame per chunk, so a chunk should hold bodies that are alike
+// and close together.  Bodies are therefore kept in an internal order: bodies much heavier than
+// the mean first (their large r_crit then stays in a few chunks), then along a Hilbert curve over
+// the x-y plane (the discs are thin).  The order is a performance hint only: every bound is
+// computed from the actual chunk contents, so results never depend on it beyond summation order.
+// key = [light:1][Hilbert index:31][body index:32]: distinct keys, so ranks are a permutation.
+__global__ void extent_kernel(int N, const double* __restrict__ x, unsigned int* __restrict__ extent_bits)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float e = 0.f;
+    if (i < N) {
+        e = fmaxf(fabsf((float)x[3 * i]), fabsf((float)x[3 * i + 1]));
+        if (!(e < 3.0e38f)) e = 0.f;                          // NaN / inf positions do not set the extent
+    }
+    const unsigned int w = __reduce_max_sync(0xffffffffu, __float_as_uint(e));
+    if ((threadIdx.x & 31) == 0 && w) atomicMax(extent_bits, w);
+}
+
+// index of cell (cx, cy) of a 2^15 x 2^15 grid along the Hilbert curve (30 bits)
+__device__ __forceinline__ unsigned int hilbert_xy2d(unsigned int cx, unsigned int cy)
+{
+    unsigned int d = 0;
+    for (unsigned int s = 1u << 14; s > 0; s >>= 1) {
+        const unsigned int rx = (cx & s) ? 1u : 0u, ry = (cy & s) ? 1u : 0u;
+        d += s * s * ((3u * rx) ^ ry);
+        if (ry == 0) {
+            if (rx == 1) { cx = s - 1 - cx; cy = s - 1 - cy; }
+            const unsigned int t = cx; cx = cy; cy = t;
+        }
+        cx &= (s - 1); cy &= (s - 1);
+    }
+    return d;
+}
+
+__global__ void sortkey_kernel(int N, double M_star, const double* __restrict__ x,
+                               const double* __restrict__ hcbrt, const double* __restrict__ red,
+                               const unsigned int* __restrict__ extent_bits, unsigned long long* __restrict__ keys)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float ext = fmaxf(__uint_as_float(*extent_bits), 1.0e-30f);
+    const float sc  = 16383.5f / ext;                                    // [-ext, ext] -> [0, 32767]
+    const float fx = fminf(fmaxf(fmaf((float)x[3 * i], sc, 16383.5f), 0.f), 32767.f);
+    const float fy = fminf(fmaxf(fmaf((float)x[3 * i + 1], sc, 16383.5f), 0.f), 32767.f);
+    const unsigned int cx = (fx == fx) ? (unsigned int)fx : 0u, cy = (fy == fy) ? (unsigned int)fy : 0u;
+    const double href = cbrt(red[3] / ((double)N * 3.0 * M_star));      // Hill factor of the mean mass
+    const unsigned long long light = (hcbrt[i] > 1.5 * href) ? 0ull : 1ull;
+    keys[i] = (light << 63) | ((unsigned long long)hilbert_xy2d(cx, cy) << 32) | (unsigned int)i;
+}
+
+// Rank sort: order[#{j : key_j < key_i}] = i.  O(N^2) integer compares, but it runs only when
+// the order is refreshed (every resort_every force evaluations), never per step.
+constexpr int RANK_NT = 256;
+__global__ void __launch_bounds__(RANK_NT)
+ranksort_kernel(int N, int NP, const unsigned long long* __restrict__ keys, int* __restrict__ order)
+{
+    __shared__ unsigned long long sk[RANK_NT * 4];
+    const int i = blockIdx.x * RANK_NT + threadIdx.x;
+    const unsigned long long ki = (i < N) ? keys[i] : 0ull;
+    int rank = 0;
+    for (int base = 0; base < N; base += RANK_NT * 4) {
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int j = base + q * RANK_NT + threadIdx.x;
+            sk[q * RANK_NT + threadIdx.x] = (j < N) ? keys[j] : ~0ull;
+        }
+        __syncthreads();
+#pragma unroll 8
+        for (int jj = 0; jj < RANK_NT * 4; ++jj) rank += (sk[jj] < ki) ? 1 : 0;
+    }
+    if (i < N) order[rank] = i;
+    else if (i < NP) order[i] = i;
+}
+
 // One thread per (padded) body.  Eq. 1:  r_crit,i = max(n1 R_H,i, n2 dt v_i), R_H,i = a_i (m_i/3M)^(1/3);
 // a_i from vis-viva with the stored velocity (readings G2b, G2c); v_i = sqrt(G M / a_i).
 __global__ void __launch_bounds__(PREP_NT)
 prep_kernel(PrepArgs A, Workspace w)
 {
-    __shared__ unsigned int smax[PREP_NT / 32][3];
-    const int i = blockIdx.x * PREP_NT + threadIdx.x;      // grid covers NP exactly (NP % 512 == 0)
-    const bool live = i < A.N;
+    __shared__ unsigned int smax[PREP_NT / 32][4];
+    const int s = blockIdx.x * PREP_NT + threadIdx.x;      // slot; grid covers NP exactly (NP % 512 == 0)
+    const bool live = s < A.N;
+    const int i = w.order[s];                              // body held by this slot (= s for padding)
 
     double px = PAD_POS, py = 0.0, pz = 0.0, gm = 0.0;
     float hq = 0.f, aq = 0.f, rf = 0.f;
+    double4 ax4 = make_double4(0.0, 0.0, 0.0, 0.0);
     if (live) {
         const double mu = A.G * A.M_star;
         px = w.x[3 * i + 0]; py = w.x[3 * i + 1]; pz = w.x[3 * i + 2];
@@ -54,18 +134,20 @@ prep_kernel(PrepArgs A, Workspace w)
         const double vk = sqrt(mu / sa);
         const double rc = fmax(A.n1 * (sa * h), A.n2 * A.dt_rcrit * vk);
         w.rcrit[i] = rc; w.semi[i] = sa; w.vkep[i] = vk;
-        gm = A.G * w.m[i];
+        const double mi = w.m[i];
+        gm = A.G * mi;
+        ax4 = make_double4(mi, rc, sa, vk);
 
         const double lam = (double)A.lambda * (1.0 + 1.0e-6);
         double dhq, daq, drf;
         if (A.pair_rule == GENGA_PAIR_MUTUAL_HILL) {
             dhq = lam * A.n1 * 1.2599210498948732 * h;     // cbrt(2) * h_i bounds cbrt((m_i+m_j)/3M)
             daq = sa;
-            drf = fmax((double)A.floor_rel * r, lam * A.n2 * A.dt_rcrit * vk);
+            drf = lam * A.n2 * A.dt_rcrit * vk;
         } else {
             dhq = lam * rc;
             daq = 1.0;
-            drf = (double)A.floor_rel * r;
+            drf = 0.0;
         }
         hq = __double2float_ru(dhq); aq = __double2float_ru(daq); rf = __double2float_ru(drf);
         if (!(hq >= 0.f)) hq = 3.0e38f;                     // NaN state: flag everything
@@ -73,31 +155,53 @@ prep_kernel(PrepArgs A, Workspace w)
         if (!(rf >= 0.f)) rf = 3.0e38f;
     }
     w.a[3 * i + 0] = 0.0; w.a[3 * i + 1] = 0.0; w.a[3 * i + 2] = 0.0;
-    w.pk64[i] = make_double4(px, py, pz, gm);
+    w.pk64[s] = make_double4(px, py, pz, gm);
+    w.aux[s]  = ax4;
+    // local frame of this slot's chunk: origin = position of the chunk's first slot (FP32 policy P32)
+    double ox = PAD_POS, oy = 0.0, oz = 0.0;
     {
-        float* f = reinterpret_cast<float*>(w.pk32) + 8 * (i >> 1) + (i & 1);
-        f[0] = (float)px; f[2] = (float)py; f[4] = (float)pz; f[6] = (float)gm;
+        const int s0 = s & ~(CHUNK - 1);
+        if (s0 < A.N) { const int i0 = w.order[s0]; ox = w.x[3 * i0 + 0]; oy = w.x[3 * i0 + 1]; oz = w.x[3 * i0 + 2]; }
+    }
+    const double qx = px - ox, qy = py - oy, qz = pz - oz;
+    float rad = 0.f;                                        // |x - o|, rounded up; padding does not count
+    if (live) {
+        rad = __double2float_ru(sqrt(qx * qx + qy * qy + qz * qz) * (1.0 + 1.0e-9));
+        if (!(rad >= 0.f)) rad = 3.0e38f;
+    }
+    {
+        float* f = reinterpret_cast<float*>(w.pk32) + 8 * (s >> 1) + (s & 1);
+        f[0] = (float)qx; f[2] = (float)qy; f[4] = (float)qz; f[6] = (float)gm;
     }
     BoundP b; b.hq = hq; b.aq = aq; b.rf = rf; b.pad = live ? 1.f : 0.f;
-    w.bi[i] = b;
+    w.bi[s] = b;
 
     // per-chunk maxima (CHUNK = 64 = two warps); non-negative floats order like unsigned ints
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned int m0 = warp_max_u32(__float_as_uint(hq));
     unsigned int m1 = warp_max_u32(__float_as_uint(aq));
     unsigned int m2 = warp_max_u32(__float_as_uint(rf));
-    if (lane == 0) { smax[wid][0] = m0; smax[wid][1] = m1; smax[wid][2] = m2; }
+    unsigned int m3 = warp_max_u32(__float_as_uint(rad));
+    if (lane == 0) { smax[wid][0] = m0; smax[wid][1] = m1; smax[wid][2] = m2; smax[wid][3] = m3; }
     __syncthreads();
     if (threadIdx.x < PREP_NT / CHUNK) {
         const int c = threadIdx.x;
-        BoundP q;
-        q.hq = __uint_as_float(max(smax[2 * c][0], smax[2 * c + 1][0]));
-        q.aq = __uint_as_float(max(smax[2 * c][1], smax[2 * c + 1][1]));
-        q.rf = __uint_as_float(max(smax[2 * c][2], smax[2 * c + 1][2]));
-        q.pad = 0.f;
-        w.bc[blockIdx.x * (PREP_NT / CHUNK) + c] = q;
+        ChunkP q;
+        q.hq  = __uint_as_float(max(smax[2 * c][0], smax[2 * c + 1][0]));
+        q.aq  = __uint_as_float(max(smax[2 * c][1], smax[2 * c + 1][1]));
+        q.rad = __uint_as_float(max(smax[2 * c][3], smax[2 * c + 1][3]));
+        // frame guard: pairs closer than floor * 2 R_chunk go to FP64 (relative rounding error of
+        // the FP32 separation <= 2^-24 (1 + 2 R_chunk / r))
+        q.rf  = fmaxf(__uint_as_float(max(smax[2 * c][2], smax[2 * c + 1][2])),
+                      __fmul_ru(__fmul_ru(2.0f * A.floor_rel, q.rad), 1.000001f));
+        q.pad_ = 0.0;
+        const int cg = blockIdx.x * (PREP_NT / CHUNK) + c;
+        const int s0 = cg * CHUNK;
+        q.ox = PAD_POS; q.oy = 0.0; q.oz = 0.0;
+        if (s0 < A.N) { const int i0 = w.order[s0]; q.ox = w.x[3 * i0 + 0]; q.oy = w.x[3 * i0 + 1]; q.oz = w.x[3 * i0 + 2]; }
+        w.bc[cg] = q;
     }
-    if (i == 0) { w.ctr->cand_count = 0u; w.ctr->pair_count = 0u; w.ctr->overflow = 0u; }
+    if (s == 0) { w.ctr->cand_count = 0u; w.ctr->pair_count = 0u; w.ctr->overflow = 0u; }
 }
 
 // O7: v_i += tau a_i
@@ -107,32 +211,59 @@ __global__ void velupdate_kernel(int n3, double tau, const double* __restrict__ 
     if (k < n3) v[k] = fma(tau, a[k], v[k]);
 }
 
-// red[0..2] = sum_j m_j v_j, red[3] = sum_j m_j.  One block, fixed reduction tree (deterministic).
-__global__ void __launch_bounds__(1024)
-momentum_kernel(int N, const double* __restrict__ m, const double* __restrict__ v, double* __restrict__ red)
+// red[0..2] = sum_j m_j v_j, red[3] = sum_j m_j.  Every block reduces its slice to a partial
+// (red[MOM_PART + 4 b ..]); the last block to finish (ticket) combines the partials with a fixed
+// assignment and tree, so the result is bitwise reproducible for a given N.
+constexpr int MOM_NT = 256;
+constexpr int MOM_PART = 8 + 4096;                 // partials live in the upper half of red[]
+constexpr int MOM_MAXB = 512;
+
+__device__ __forceinline__ void warp_sum4(double& a, double& b, double& c, double& d)
 {
-    __shared__ double s[32][4];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o); b += __shfl_down_sync(0xffffffffu, b, o);
+        c += __shfl_down_sync(0xffffffffu, c, o); d += __shfl_down_sync(0xffffffffu, d, o);
+    }
+}
+
+__global__ void __launch_bounds__(MOM_NT)
+momentum_kernel(int N, const double* __restrict__ m, const double* __restrict__ v, double* __restrict__ red,
+                unsigned int* __restrict__ ticket)
+{
+    __shared__ double s[MOM_NT / 32][4];
+    __shared__ bool last;
     double p0 = 0, p1 = 0, p2 = 0, mt = 0;
-    for (int i = threadIdx.x; i < N; i += 1024) {
+    for (int i = blockIdx.x * MOM_NT + threadIdx.x; i < N; i += gridDim.x * MOM_NT) {
         const double mi = m[i];
         p0 = fma(mi, v[3 * i + 0], p0); p1 = fma(mi, v[3 * i + 1], p1); p2 = fma(mi, v[3 * i + 2], p2);
         mt += mi;
     }
-    for (int o = 16; o > 0; o >>= 1) {
-        p0 += __shfl_down_sync(0xffffffffu, p0, o); p1 += __shfl_down_sync(0xffffffffu, p1, o);
-        p2 += __shfl_down_sync(0xffffffffu, p2, o); mt += __shfl_down_sync(0xffffffffu, mt, o);
-    }
+    warp_sum4(p0, p1, p2, mt);
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (lane == 0) { s[wid][0] = p0; s[wid][1] = p1; s[wid][2] = p2; s[wid][3] = mt; }
     __syncthreads();
     if (wid == 0) {
-        p0 = s[lane][0]; p1 = s[lane][1]; p2 = s[lane][2]; mt = s[lane][3];
-        for (int o = 16; o > 0; o >>= 1) {
-            p0 += __shfl_down_sync(0xffffffffu, p0, o); p1 += __shfl_down_sync(0xffffffffu, p1, o);
-            p2 += __shfl_down_sync(0xffffffffu, p2, o); mt += __shfl_down_sync(0xffffffffu, mt, o);
+        const bool in = lane < MOM_NT / 32;
+        p0 = in ? s[lane][0] : 0.0; p1 = in ? s[lane][1] : 0.0; p2 = in ? s[lane][2] : 0.0; mt = in ? s[lane][3] : 0.0;
+        warp_sum4(p0, p1, p2, mt);
+        if (lane == 0) {
+            double* q = red + MOM_PART + 4 * blockIdx.x;
+            q[0] = p0; q[1] = p1; q[2] = p2; q[3] = mt;
+            __threadfence();
+            last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
         }
-        if (lane == 0) { red[0] = p0; red[1] = p1; red[2] = p2; red[3] = mt; }
     }
+    __syncthreads();
+    if (!last || wid != 0) return;
+    __threadfence();
+    p0 = p1 = p2 = mt = 0.0;
+    for (int b = lane; b < (int)gridDim.x; b += 32) {
+        const volatile double* q = red + MOM_PART + 4 * b;
+        p0 += q[0]; p1 += q[1]; p2 += q[2]; mt += q[3];
+    }
+    warp_sum4(p0, p1, p2, mt);
+    if (lane == 0) { red[0] = p0; red[1] = p1; red[2] = p2; red[3] = mt; *ticket = 0u; }
 }
 
 // q_i[k] += scale * red[k]: O1 (q = v, scale = -1/(M_star + sum m) with red[3], or +1/M_star) and
@@ -170,6 +301,16 @@ void launch_pad(const Handle* h)
     pad_kernel<<<(n + 255) / 256, 256, 0, h->stream>>>(h->N, h->NP, h->w.m, h->w.x, h->w.v);
 }
 
+void launch_sort(const Handle* h)
+{
+    if (h->N == 0) return;
+    cudaMemsetAsync(&h->w.ctr->extent_bits, 0, sizeof(unsigned int), h->stream);
+    extent_kernel<<<(h->N + 255) / 256, 256, 0, h->stream>>>(h->N, h->w.x, &h->w.ctr->extent_bits);
+    sortkey_kernel<<<(h->N + 255) / 256, 256, 0, h->stream>>>(h->N, h->p.M_star, h->w.x, h->w.hcbrt, h->w.red,
+                                                              &h->w.ctr->extent_bits, h->w.keys);
+    ranksort_kernel<<<h->NP / RANK_NT, RANK_NT, 0, h->stream>>>(h->N, h->NP, h->w.keys, h->w.order);
+}
+
 void launch_prep(const Handle* h, const PrepArgs& a)
 {
     if (h->NP == 0) return;
@@ -185,7 +326,11 @@ void launch_velupdate(const Handle* h, double tau)
 
 void launch_momentum(const Handle* h)
 {
-    momentum_kernel<<<1, 1024, 0, h->stream>>>(h->N, h->w.m, h->w.v, h->w.red);
+    int blocks = (h->N + MOM_NT * 4 - 1) / (MOM_NT * 4);
+    if (blocks < 1) blocks = 1;
+    if (blocks > h->num_sms) blocks = h->num_sms;
+    if (blocks > MOM_MAXB) blocks = MOM_MAXB;
+    momentum_kernel<<<blocks, MOM_NT, 0, h->stream>>>(h->N, h->w.m, h->w.v, h->w.red, &h->w.ctr->ticket);
 }
 
 void launch_shift_v(const Handle* h, double scale)
