@@ -160,6 +160,13 @@ int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed
 int genga_set_profiling(genga_handle h, int enable);
 int genga_kernel_time(genga_handle h, int which, double* ms_total, long long* launches, int reset);
 
+/* Kernel configuration ("tuning", cf. GENGA's self-tuning): key 0 selects the
+ * launch/tiling variant of the FP32 all-pairs kernel, key 1 of the FP64 one; value in
+ * [0, genga_num_variants(key)); 0 is the default.  Results are identical up to summation order. */
+int genga_set_tuning(genga_handle h, int key, int value);
+int genga_num_variants(int key);
+const char* genga_variant_name(int key, int value);
+
 /* Launches issued by this handle since creation (kernels only, not copies).                     */
 long long genga_launch_count(genga_handle h);
 

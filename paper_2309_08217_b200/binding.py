@@ -28,7 +28,7 @@ SYMBOLS = [
     "genga_get_state", "genga_get_state_host", "genga_get_accel", "genga_get_rcrit",
     "genga_nearfield_stats", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
     "genga_synchronize", "genga_strerror", "genga_last_cuda_error", "genga_version",
-    "genga_peak_probe",
+    "genga_peak_probe", "genga_set_tuning", "genga_num_variants", "genga_variant_name",
 ]
 
 
@@ -93,6 +93,9 @@ def load() -> ctypes.CDLL:
     L.genga_last_cuda_error.argtypes = []; L.genga_last_cuda_error.restype = ctypes.c_char_p
     L.genga_version.argtypes = []; L.genga_version.restype = ctypes.c_char_p
     L.genga_peak_probe.argtypes = [ctypes.c_int, ctypes.c_int, vp, dp, dp]
+    L.genga_set_tuning.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+    L.genga_num_variants.argtypes = [ctypes.c_int]
+    L.genga_variant_name.argtypes = [ctypes.c_int, ctypes.c_int]; L.genga_variant_name.restype = ctypes.c_char_p
     for name in SYMBOLS:
         fn = getattr(L, name)
         if fn.restype is ctypes.c_int and name not in ("genga_launch_count",):
@@ -123,6 +126,14 @@ def peak_probe(which: int, iters: int = 4096, stream: int = 0):
     _check(load().genga_peak_probe(which, iters, ctypes.c_void_p(stream), ctypes.byref(ops), ctypes.byref(ms)),
            "genga_peak_probe")
     return ops.value, ms.value
+
+
+def num_variants(key: int) -> int:
+    return int(load().genga_num_variants(int(key)))
+
+
+def variant_name(key: int, value: int) -> str:
+    return load().genga_variant_name(int(key), int(value)).decode()
 
 
 def _dptr(t):
@@ -282,6 +293,9 @@ class Genga:
         _check(self._L.genga_kernel_time(self._h, int(which), ctypes.byref(ms), ctypes.byref(n), int(reset)),
                "genga_kernel_time")
         return ms.value, int(n.value)
+
+    def set_tuning(self, key, value):
+        _check(self._L.genga_set_tuning(self._h, int(key), int(value)), "genga_set_tuning")
 
     def launch_count(self) -> int:
         return int(self._L.genga_launch_count(self._h))

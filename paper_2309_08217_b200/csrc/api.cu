@@ -462,6 +462,25 @@ const char* genga_last_cuda_error(void) { return genga::g_cuda_err; }
 
 const char* genga_version(void) { return "genga_b200 0.1 (sm_100a)"; }
 
+int genga_set_tuning(genga_handle h, int key, int value)
+{
+    if (!h || key < 0 || key > 1) return GENGA_EINVAL;
+    const int n = key == 0 ? kick32_num_variants() : kick64_num_variants();
+    if (value < 0 || value >= n) return GENGA_EINVAL;
+    h->tune[key] = value;
+    return GENGA_OK;
+}
+
+int genga_num_variants(int key)
+{
+    return key == 0 ? kick32_num_variants() : key == 1 ? kick64_num_variants() : 0;
+}
+
+const char* genga_variant_name(int key, int value)
+{
+    return key == 0 ? kick32_variant_name(value) : key == 1 ? kick64_variant_name(value) : "";
+}
+
 int genga_peak_probe(int which, int iters, void* stream, double* ops_per_s, double* ms)
 {
     return run_peak_probe(which, iters, static_cast<cudaStream_t>(stream), ops_per_s, ms);

@@ -15,9 +15,6 @@ constexpr int CHUNK      = 64;                  // j-bodies per chunk: granulari
 constexpr int STAGE_CH   = 8;                   // chunks per shared-memory stage
 constexpr int STAGE_J    = CHUNK * STAGE_CH;    // 512 j-bodies per stage
 constexpr int NSTAGE     = 2;                   // double buffering
-constexpr int KICK_NT    = 128;                 // threads per CTA of the all-pairs kernels
-constexpr int KICK32_I   = 4;                   // i-bodies per thread, FP32 kernel
-constexpr int KICK64_I   = 4;                   // i-bodies per thread, FP64 kernel
 constexpr int PAD_BODIES = 512;                 // N is padded to a multiple of this (stage and i-block size)
 constexpr double PAD_POS = 1.0e15;              // position of padding bodies (gm = 0, far from everything)
 
@@ -84,6 +81,7 @@ struct Handle {
     int num_sms;
     long long launches;
     // internal order (a performance hint only: results never depend on it)
+    int tune[4];                 // genga_set_tuning: [0] kick32 variant, [1] kick64 variant
     int resort_every;            // force evaluations between two sorts
     int evals_since_sort;        // < 0: no order yet
 
@@ -126,5 +124,9 @@ int  run_peak_probe(int which, int iters, cudaStream_t s, double* ops_per_s, dou
 // occupancy-derived grid of the all-pairs kernels
 int kick32_grid(const Handle* h);
 int kick64_grid(const Handle* h);
+int kick32_num_variants();
+int kick64_num_variants();
+const char* kick32_variant_name(int v);
+const char* kick64_variant_name(int v);
 
 }  // namespace genga

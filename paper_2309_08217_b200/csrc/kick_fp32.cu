@@ -49,22 +49,27 @@ __device__ __forceinline__ float min3(float a, float b, float c)
     float r; asm("min.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c)); return r;
 }
 
-constexpr int I  = KICK32_I;
-constexpr int NT = KICK_NT;
-constexpr int BI = I * NT;                       // i-bodies per i-block (= PAD_BODIES)
-
+// Kernel configuration: I i-bodies per thread, NT threads per CTA (I * NT = 512 = one i-block),
+// MINB CTAs per SM asked of ptxas (caps the registers), ACCS: FP64 accumulators in shared memory
+// instead of registers, UNR: unroll factor of the j-pair loop.
+template <int I, int NT, bool ACCS>
 struct __align__(16) Smem32 {
     float4   j[NSTAGE][STAGE_J];                 // pair-interleaved j data (chunk-relative), 16 B per body
     ChunkP   bc[NSTAGE][STAGE_CH];
     double   xi[3][I][NT];                       // FP64 positions of this CTA's i-bodies
-    float    bp[3][I][NT];                       // their bound parameters (hq, aq, rf)
+    double   acc[ACCS ? 3 : 1][ACCS ? I : 1][ACCS ? NT : 1];   // FP64 accumulators (ACCS)
+    float    bp[3][I][NT];                       // bound parameters (hq, aq, rf) of the i-bodies
     uint64_t full[NSTAGE];
 };
 
-__global__ void __launch_bounds__(NT, 4)
+template <int I, int NT, int MINB, bool ACCS, int UNR>
+__global__ void __launch_bounds__(NT, MINB)
 kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 {
-    __shared__ Smem32 sm;
+    constexpr int BI = I * NT;
+    static_assert(PAD_BODIES % BI == 0, "i-blocks tile the padding unit");
+    extern __shared__ __align__(16) unsigned char smraw[];
+    Smem32<I, NT, ACCS>& sm = *reinterpret_cast<Smem32<I, NT, ACCS>*>(smraw);
     const int tid = threadIdx.x;
 
     if (tid == 0) {
@@ -72,7 +77,7 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
         fence_barrier_init();
     }
     __syncthreads();
-    uint32_t phase[NSTAGE] = {0u, 0u};
+    uint32_t phase = 0u;                           // bit b = parity of stage buffer b
 
     const long long U = (long long)nib * nchunk;
     long long u0 = (U * (long long)blockIdx.x) / (long long)gridDim.x;
@@ -84,8 +89,8 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
         const int c1 = (int)min((long long)nchunk, (long long)c0 + (u1 - u0));
         u0 += (c1 - c0);
 
-        // ---- i-side: FP64 positions to shared memory (own column only), bound parameters to registers
-        double Ax[I], Ay[I], Az[I];
+        // ---- i-side: FP64 positions and bound parameters to shared memory (own column only)
+        double Ax[ACCS ? 1 : I], Ay[ACCS ? 1 : I], Az[ACCS ? 1 : I];
 #pragma unroll
         for (int k = 0; k < I; ++k) {
             const int i = ib * BI + k * NT + tid;
@@ -93,7 +98,8 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
             sm.xi[0][k][tid] = q.x; sm.xi[1][k][tid] = q.y; sm.xi[2][k][tid] = q.z;
             const BoundP b = w.bi[i];
             sm.bp[0][k][tid] = b.hq; sm.bp[1][k][tid] = b.aq; sm.bp[2][k][tid] = b.rf;
-            Ax[k] = 0.0; Ay[k] = 0.0; Az[k] = 0.0;
+            if (ACCS) { sm.acc[0][k][tid] = 0.0; sm.acc[1][k][tid] = 0.0; sm.acc[2][k][tid] = 0.0; }
+            else      { Ax[k] = 0.0; Ay[k] = 0.0; Az[k] = 0.0; }
         }
 
         const int nst = (c1 - c0 + STAGE_CH - 1) / STAGE_CH;
@@ -114,25 +120,28 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
             const int b   = st & 1;
             const int cs  = c0 + st * STAGE_CH;
             const int nch = min(STAGE_CH, c1 - cs);
-            mbar_wait(&sm.full[b], phase[b]);
-            phase[b] ^= 1u;
+            mbar_wait(&sm.full[b], (phase >> b) & 1u);
+            phase ^= 1u << b;
 
             for (int ch = 0; ch < nch; ++ch) {
-                const ChunkP Bc = sm.bc[b][ch];
+                const ChunkP& Bc = sm.bc[b][ch];
                 // i-positions in the chunk's frame: FP64 subtraction, then one rounding to FP32
                 float nx[I], ny[I], nz[I];
                 f2 ax[I], ay[I], az[I];
                 float mn[I];
+                {
+                    const double ox = Bc.ox, oy = Bc.oy, oz = Bc.oz;
 #pragma unroll
-                for (int k = 0; k < I; ++k) {
-                    nx[k] = (float)(Bc.ox - sm.xi[0][k][tid]);
-                    ny[k] = (float)(Bc.oy - sm.xi[1][k][tid]);
-                    nz[k] = (float)(Bc.oz - sm.xi[2][k][tid]);
-                    ax[k] = 0ull; ay[k] = 0ull; az[k] = 0ull; mn[k] = 3.0e38f;
+                    for (int k = 0; k < I; ++k) {
+                        nx[k] = (float)(ox - sm.xi[0][k][tid]);
+                        ny[k] = (float)(oy - sm.xi[1][k][tid]);
+                        nz[k] = (float)(oz - sm.xi[2][k][tid]);
+                        ax[k] = 0ull; ay[k] = 0ull; az[k] = 0ull; mn[k] = 3.0e38f;
+                    }
                 }
 
                 const float4* jp = &sm.j[b][ch * CHUNK];
-#pragma unroll 2
+#pragma unroll UNR
                 for (int jj = 0; jj < CHUNK / 2; ++jj) {
                     const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
                     const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y), gj = pk(B.z, B.w);
@@ -157,19 +166,28 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                 }
 
                 // ---- chunk end: keep the FP32 partial or hand the chunk to the near field ----
+                const float Hc = Bc.hq, Ac = Bc.aq, Rc = Bc.rf;
 #pragma unroll
                 for (int k = 0; k < I; ++k) {
-                    const float Bq = fmaxf(fmaxf(sm.bp[0][k][tid], Bc.hq) * fmaxf(sm.bp[1][k][tid], Bc.aq),
-                                           fmaxf(sm.bp[2][k][tid], Bc.rf));
+                    const float Bq = fmaxf(fmaxf(sm.bp[0][k][tid], Hc) * fmaxf(sm.bp[1][k][tid], Ac),
+                                           fmaxf(sm.bp[2][k][tid], Rc));
                     const float bound = (ib * BI + k * NT + tid < N) ? Bq * Bq : -1.0f;
                     const bool keep = mn[k] > bound;
                     float lo, hi;
                     upk(ax[k], lo, hi); const float px = lo + hi;
                     upk(ay[k], lo, hi); const float py = lo + hi;
                     upk(az[k], lo, hi); const float pz = lo + hi;
-                    Ax[k] += keep ? (double)px : 0.0;
-                    Ay[k] += keep ? (double)py : 0.0;
-                    Az[k] += keep ? (double)pz : 0.0;
+                    if (ACCS) {
+                        if (keep) {
+                            sm.acc[0][k][tid] += (double)px;
+                            sm.acc[1][k][tid] += (double)py;
+                            sm.acc[2][k][tid] += (double)pz;
+                        }
+                    } else {
+                        Ax[k] += keep ? (double)px : 0.0;
+                        Ay[k] += keep ? (double)py : 0.0;
+                        Az[k] += keep ? (double)pz : 0.0;
+                    }
                     const unsigned int bal = __ballot_sync(0xffffffffu, !keep);
                     if (bal)
                         push_candidates(bal, !keep, ib * BI + k * NT + tid, cs + ch,
@@ -184,20 +202,68 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
         for (int k = 0; k < I; ++k) {
             if (ib * BI + k * NT + tid < N) {
                 const int i = w.order[ib * BI + k * NT + tid];     // slot -> body (API order)
-                atomicAdd(&w.a[3 * i + 0], Ax[k]);
-                atomicAdd(&w.a[3 * i + 1], Ay[k]);
-                atomicAdd(&w.a[3 * i + 2], Az[k]);
+                atomicAdd(&w.a[3 * i + 0], ACCS ? sm.acc[0][k][tid] : Ax[ACCS ? 0 : k]);
+                atomicAdd(&w.a[3 * i + 1], ACCS ? sm.acc[1][k][tid] : Ay[ACCS ? 0 : k]);
+                atomicAdd(&w.a[3 * i + 2], ACCS ? sm.acc[2][k][tid] : Az[ACCS ? 0 : k]);
             }
         }
     }
 }
 
+// ---- variants (genga_set_tuning key 0) ---------------------------------------------------------
+typedef void (*kick32_fn)(int, int, int, Workspace, unsigned int);
+struct Variant32 { kick32_fn fn; int nt; int bi; size_t smem; const char* name; };
+
+#define V32(I_, NT_, MINB_, ACCS_, UNR_) \
+    { kick32_kernel<I_, NT_, MINB_, ACCS_, UNR_>, NT_, I_ * NT_, sizeof(Smem32<I_, NT_, ACCS_>), \
+      "I" #I_ " NT" #NT_ " minB" #MINB_ " accS" #ACCS_ " unr" #UNR_ }
+
+const Variant32 g_variants32[] = {
+    V32(2, 256, 2, false, 2),     // 0: default
+    V32(4, 128, 4, false, 2),
+    V32(2, 256, 2, false, 4),
+    V32(2, 256, 2, false, 8),
+    V32(2, 256, 2, false, 1),
+    V32(2, 256, 2, true, 2),
+    V32(2, 256, 2, true, 4),
+    V32(2, 128, 4, false, 2),
+    V32(2, 128, 4, false, 4),
+    V32(2, 128, 4, true, 4),
+    V32(2, 128, 5, true, 4),
+    V32(2, 128, 6, true, 4),
+    V32(1, 512, 1, false, 4),
+    V32(1, 512, 1, false, 8),
+    V32(1, 256, 2, false, 8),
+    V32(1, 256, 3, false, 8),
+    V32(1, 128, 6, false, 8),
+    V32(2, 64, 8, false, 4),
+    V32(4, 64, 8, false, 2),
+    V32(4, 128, 3, false, 4),
+    V32(4, 128, 3, true, 4),
+};
+constexpr int NVAR32 = (int)(sizeof(g_variants32) / sizeof(g_variants32[0]));
+bool g_attr32[NVAR32] = {};
+
+const Variant32& variant32(int v)
+{
+    if (v < 0 || v >= NVAR32) v = 0;
+    if (!g_attr32[v]) {
+        cudaFuncSetAttribute(g_variants32[v].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_variants32[v].smem);
+        g_attr32[v] = true;
+    }
+    return g_variants32[v];
+}
+
 }  // namespace
+
+int kick32_num_variants() { return NVAR32; }
+const char* kick32_variant_name(int v) { return (v >= 0 && v < NVAR32) ? g_variants32[v].name : ""; }
 
 int kick32_grid(const Handle* h)
 {
+    const Variant32& V = variant32(h->tune[0]);
     int occ = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kick32_kernel, NT, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn, V.nt, V.smem);
     if (occ < 1) occ = 1;
     return h->num_sms * occ;
 }
@@ -205,11 +271,12 @@ int kick32_grid(const Handle* h)
 void launch_kick32(const Handle* h)
 {
     if (h->N == 0) return;
-    const int nib = h->NP / BI;
+    const Variant32& V = variant32(h->tune[0]);
+    const int nib = h->NP / V.bi;
     const long long U = (long long)nib * h->nchunk;
     long long G = kick32_grid(h);
     if (G > U) G = U;
-    kick32_kernel<<<(int)G, NT, 0, h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
+    V.fn<<<(int)G, V.nt, V.smem, h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
 }
 
 }  // namespace genga

@@ -17,11 +17,7 @@ __device__ __forceinline__ double rsq64h(double a)
     double r; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r;
 }
 
-constexpr int I  = KICK64_I;
-constexpr int NT = KICK_NT;
-constexpr int BI = PAD_BODIES;                   // i-bodies per i-block
-static_assert(I * NT == BI, "FP64 i-block must equal the padding unit");
-
+template <int I, int NT>
 struct __align__(16) Smem64 {
     double4  j[NSTAGE][STAGE_J];                 // (x, y, z, G m), 32 B per body
     ChunkP   bc[NSTAGE][STAGE_CH];
@@ -29,11 +25,14 @@ struct __align__(16) Smem64 {
     uint64_t full[NSTAGE];
 };
 
-__global__ void __launch_bounds__(NT, 4)
+template <int I, int NT, int MINB, int UNR>
+__global__ void __launch_bounds__(NT, MINB)
 kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 {
+    constexpr int BI = I * NT;
+    static_assert(PAD_BODIES % BI == 0, "i-blocks tile the padding unit");
     extern __shared__ __align__(16) unsigned char smraw[];
-    Smem64& sm = *reinterpret_cast<Smem64*>(smraw);
+    Smem64<I, NT>& sm = *reinterpret_cast<Smem64<I, NT>*>(smraw);
     const int tid = threadIdx.x;
 
     if (tid == 0) {
@@ -41,7 +40,7 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
         fence_barrier_init();
     }
     __syncthreads();
-    uint32_t phase[NSTAGE] = {0u, 0u};
+    uint32_t phase = 0u;                           // bit b = parity of stage buffer b
 
     const long long U = (long long)nib * nchunk;
     long long u0 = (U * (long long)blockIdx.x) / (long long)gridDim.x;
@@ -83,8 +82,8 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
             const int b   = st & 1;
             const int cs  = c0 + st * STAGE_CH;
             const int nch = min(STAGE_CH, c1 - cs);
-            mbar_wait(&sm.full[b], phase[b]);
-            phase[b] ^= 1u;
+            mbar_wait(&sm.full[b], (phase >> b) & 1u);
+            phase ^= 1u << b;
 
             for (int ch = 0; ch < nch; ++ch) {
                 const ChunkP Bc = sm.bc[b][ch];
@@ -94,7 +93,7 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                 for (int k = 0; k < I; ++k) { ax[k] = 0.0; ay[k] = 0.0; az[k] = 0.0; mn[k] = 0x7fffffff; }
 
                 const double4* jp = &sm.j[b][ch * CHUNK];
-#pragma unroll 2
+#pragma unroll UNR
                 for (int jj = 0; jj < CHUNK; ++jj) {
                     const double4 J = jp[jj];
 #pragma unroll
@@ -137,7 +136,7 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                                         &w.ctr->cand_count, w.cand, cand_cap);
                 }
             }
-            __syncthreads();
+            __syncthreads();                       // every thread is done reading buffer b
             if (tid == 0 && st + 2 < nst) issue(st + 2);
         }
 
@@ -153,18 +152,52 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
     }
 }
 
+typedef void (*kick64_fn)(int, int, int, Workspace, unsigned int);
+struct Variant64 { kick64_fn fn; int nt; int bi; size_t smem; const char* name; };
+
+#define V64(I_, NT_, MINB_, UNR_) \
+    { kick64_kernel<I_, NT_, MINB_, UNR_>, NT_, I_ * NT_, sizeof(Smem64<I_, NT_>), "I" #I_ " NT" #NT_ " minB" #MINB_ " unr" #UNR_ }
+
+const Variant64 g_variants64[] = {
+    V64(2, 256, 2, 4),            // 0: default
+    V64(4, 128, 4, 2),
+    V64(2, 256, 2, 8),
+    V64(2, 256, 1, 4),
+    V64(2, 128, 4, 4),
+    V64(2, 128, 3, 4),
+    V64(2, 128, 4, 8),
+    V64(1, 512, 2, 4),
+    V64(1, 512, 2, 8),
+    V64(1, 256, 4, 8),
+    V64(1, 256, 3, 8),
+    V64(1, 128, 8, 8),
+    V64(4, 128, 3, 4),
+    V64(4, 64, 6, 2),
+    V64(2, 64, 8, 4),
+};
+constexpr int NVAR64 = (int)(sizeof(g_variants64) / sizeof(g_variants64[0]));
+bool g_attr64[NVAR64] = {};
+
+const Variant64& variant64(int v)
+{
+    if (v < 0 || v >= NVAR64) v = 0;
+    if (!g_attr64[v]) {
+        cudaFuncSetAttribute(g_variants64[v].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_variants64[v].smem);
+        g_attr64[v] = true;
+    }
+    return g_variants64[v];
+}
+
 }  // namespace
 
-static bool s_attr_set = false;
+int kick64_num_variants() { return NVAR64; }
+const char* kick64_variant_name(int v) { return (v >= 0 && v < NVAR64) ? g_variants64[v].name : ""; }
 
 int kick64_grid(const Handle* h)
 {
-    if (!s_attr_set) {
-        cudaFuncSetAttribute(kick64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem64));
-        s_attr_set = true;
-    }
+    const Variant64& V = variant64(h->tune[1]);
     int occ = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kick64_kernel, NT, sizeof(Smem64));
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn, V.nt, V.smem);
     if (occ < 1) occ = 1;
     return h->num_sms * occ;
 }
@@ -172,11 +205,12 @@ int kick64_grid(const Handle* h)
 void launch_kick64(const Handle* h)
 {
     if (h->N == 0) return;
-    const int nib = h->NP / BI;
+    const Variant64& V = variant64(h->tune[1]);
+    const int nib = h->NP / V.bi;
     const long long U = (long long)nib * h->nchunk;
     long long G = kick64_grid(h);
     if (G > U) G = U;
-    kick64_kernel<<<(int)G, NT, sizeof(Smem64), h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
+    V.fn<<<(int)G, V.nt, V.smem, h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
 }
 
 }  // namespace genga

@@ -51,6 +51,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
 
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
 // Append (body, chunk) for every lane with flag set; one atomic per warp (__ballot_sync + popc).
 // Must be executed by all 32 lanes.  Entries past the capacity are dropped; the count keeps
 // growing so that the near-field kernel can see the overflow and take the exact path.
