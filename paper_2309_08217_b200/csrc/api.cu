@@ -44,6 +44,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_cand = take((size_t)cand_cap * 8), o_pairs = take((size_t)pair_cap * 8);
     const size_t o_red = take((size_t)RED_DOUBLES * 8), o_vt = take(NP * 24), o_ctr = take(sizeof(Counters));
     const size_t o_ord = take(NP * 4), o_key = take(NP * 8), o_aux = take(NP * 32);
+    const size_t o_mom = take((8 + 4 * (NP / 128 + 1)) * 8);
     if (w && base) {
         char* b = static_cast<char*>(base);
         w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
@@ -53,6 +54,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
         w->pairs = (int2*)(b + o_pairs); w->red = (double*)(b + o_red); w->vtmp = (double*)(b + o_vt);
         w->ctr = (Counters*)(b + o_ctr);
         w->order = (int*)(b + o_ord); w->keys = (unsigned long long*)(b + o_key); w->aux = (double4*)(b + o_aux);
+        w->mom = (double*)(b + o_mom);
     }
     return off;
 }
@@ -99,7 +101,7 @@ static int resort(Handle* h)
 }
 
 // ---- force evaluation -------------------------------------------------------------------------
-static int force_eval(Handle* h, int precision)
+static int force_eval(Handle* h, int precision, double preshift = 0.0)
 {
     if (precision != GENGA_FP64 && precision != GENGA_FP32) return GENGA_EINVAL;
     if (h->N == 0) return GENGA_OK;
@@ -112,6 +114,7 @@ static int force_eval(Handle* h, int precision)
     a.N = h->N; a.NP = h->NP;
     a.G = h->p.G; a.M_star = h->p.M_star; a.n1 = h->p.n1; a.n2 = h->p.n2; a.dt_rcrit = h->p.dt_rcrit;
     a.pair_rule = h->p.pair_rule;
+    a.preshift = preshift;
     if (precision == GENGA_FP32) { a.lambda = (float)h->lambda_near; a.floor_rel = (float)h->near_floor; }
     else                         { a.lambda = 1.0f;                  a.floor_rel = 0.0f; }
     { ProfScope ps(h, 2); launch_prep(h, a); }
@@ -137,13 +140,28 @@ using namespace genga;
 
 struct genga_s : public genga::Handle {};
 
-// S(dt/2) D(dt) S(dt/2): the middle of one step (reading G3)
-static int sds(genga_handle h, double dt)
+// K(tau): force evaluation, v += tau a, and (fused) the momentum of the new velocities.  preshift:
+// a pending Sun-kick S(preshift) with the momentum the fused drift left in mom[SLOT_B].
+static int kick_fused(genga_handle h, double tau, int precision, double preshift)
 {
-    int rc;
-    if ((rc = genga_sunkick(h, 0.5 * dt)) != GENGA_OK) return rc;
-    if ((rc = genga_drift(h, dt)) != GENGA_OK) return rc;
-    return genga_sunkick(h, 0.5 * dt);
+    const int rc = force_eval(h, precision, preshift);
+    if (rc != GENGA_OK) return rc;
+    if (h->N == 0) return GENGA_OK;
+    launch_velupdate_mom(h, tau); LAUNCHED(h, "velupdate_mom_kernel");
+    h->mom_a_valid = true;
+    return GENGA_OK;
+}
+
+// S(dt/2) D(dt) of one step in ONE kernel (reading G3); the closing S(dt/2) is left pending for the
+// prep kernel of the kick that always follows inside genga_step / genga_run / genga_leapfrog.
+static int sd_fused(genga_handle h, double dt)
+{
+    if (h->N == 0) return GENGA_OK;
+    if (!h->mom_a_valid) { launch_momentum_slot_a(h); LAUNCHED(h, "momentum_kernel"); }
+    { ProfScope ps(h, 3); launch_shift_drift_mom(h, 0.5 * dt, dt); }
+    LAUNCHED(h, "shift_drift_mom_kernel");
+    h->mom_a_valid = false;
+    return GENGA_OK;
 }
 
 extern "C" {
@@ -230,7 +248,8 @@ static int set_state_impl(genga_handle h, const double* m, const double* x, cons
     if (n == 0) return GENGA_OK;
     if (m) CU(cudaMemcpyAsync(h->w.m, m, n * 8, kind, h->stream));
     if (x) CU(cudaMemcpyAsync(h->w.x, x, n * 24, kind, h->stream));
-    if (v) CU(cudaMemcpyAsync(h->w.v, v, n * 24, kind, h->stream));
+    if (v) { CU(cudaMemcpyAsync(h->w.v, v, n * 24, kind, h->stream)); h->mom_a_valid = false; }
+    if (m) h->mom_a_valid = false;
     if (m) { launch_hcbrt(h); LAUNCHED(h, "hcbrt_kernel"); }
     if (v && h->p.v_is_heliocentric) return to_democratic(h);
     return GENGA_OK;
@@ -261,10 +280,7 @@ int genga_accel(genga_handle h, int precision)
 int genga_kick(genga_handle h, double dt, int precision)
 {
     if (!h) return GENGA_EINVAL;
-    const int rc = force_eval(h, precision);
-    if (rc != GENGA_OK) return rc;
-    launch_velupdate(h, dt); LAUNCHED(h, "velupdate_kernel");
-    return GENGA_OK;
+    return kick_fused(h, dt, precision, 0.0);
 }
 
 int genga_drift(genga_handle h, double dt)
@@ -272,6 +288,7 @@ int genga_drift(genga_handle h, double dt)
     if (!h) return GENGA_EINVAL;
     { ProfScope ps(h, 3); launch_drift(h, dt); }
     LAUNCHED(h, "drift_kernel");
+    h->mom_a_valid = false;
     return GENGA_OK;
 }
 
@@ -288,9 +305,9 @@ int genga_step(genga_handle h, double dt, int precision)
 {
     if (!h) return GENGA_EINVAL;
     int rc;
-    if ((rc = genga_kick(h, 0.5 * dt, precision)) != GENGA_OK) return rc;
-    if ((rc = sds(h, dt)) != GENGA_OK) return rc;
-    return genga_kick(h, 0.5 * dt, precision);
+    if ((rc = kick_fused(h, 0.5 * dt, precision, 0.0)) != GENGA_OK) return rc;
+    if ((rc = sd_fused(h, dt)) != GENGA_OK) return rc;
+    return kick_fused(h, 0.5 * dt, precision, 0.5 * dt);
 }
 
 int genga_leapfrog(genga_handle h, double dt, int nsteps, int precision)
@@ -298,8 +315,8 @@ int genga_leapfrog(genga_handle h, double dt, int nsteps, int precision)
     if (!h || nsteps < 0) return GENGA_EINVAL;
     int rc;
     for (int s = 0; s < nsteps; ++s) {
-        if ((rc = sds(h, dt)) != GENGA_OK) return rc;
-        if ((rc = genga_kick(h, dt, precision)) != GENGA_OK) return rc;
+        if ((rc = sd_fused(h, dt)) != GENGA_OK) return rc;
+        if ((rc = kick_fused(h, dt, precision, 0.5 * dt)) != GENGA_OK) return rc;
     }
     return GENGA_OK;
 }
@@ -309,10 +326,10 @@ int genga_run(genga_handle h, double dt, int nsteps, int precision)
     if (!h || nsteps < 0) return GENGA_EINVAL;
     if (nsteps == 0) return GENGA_OK;
     int rc;
-    if ((rc = genga_kick(h, 0.5 * dt, precision)) != GENGA_OK) return rc;
+    if ((rc = kick_fused(h, 0.5 * dt, precision, 0.0)) != GENGA_OK) return rc;
     if ((rc = genga_leapfrog(h, dt, nsteps - 1, precision)) != GENGA_OK) return rc;
-    if ((rc = sds(h, dt)) != GENGA_OK) return rc;
-    return genga_kick(h, 0.5 * dt, precision);
+    if ((rc = sd_fused(h, dt)) != GENGA_OK) return rc;
+    return kick_fused(h, 0.5 * dt, precision, 0.5 * dt);
 }
 
 int genga_encounter_pairs(genga_handle h, int* pairs_ij, int cap, int* count)

@@ -10,6 +10,7 @@
 //     f = 1 - mu G2 / r0,  g = r0 G1 + u G2 (= dt - mu G3),  fdot = -mu G1 / (r r0),  gdot = 1 - mu G2 / r.
 // This is a different formulation from the oracle's eccentric-anomaly-difference form on purpose.
 #include "genga_internal.cuh"
+#include "momentum.cuh"
 
 namespace genga {
 
@@ -48,13 +49,10 @@ __device__ __forceinline__ void stumpff(double z, double& c0, double& c1, double
     }
 }
 
-__global__ void __launch_bounds__(128)
-drift_kernel(int N, double mu, double dt_full, double* __restrict__ x, double* __restrict__ v, Counters* ctr)
+// Propagate one body by dt_full about mu (in place).  Returns false if the iteration did not converge.
+__device__ __forceinline__ bool kepler_drift(double mu, double dt_full, double& x0, double& y0, double& z0,
+                                             double& vx, double& vy, double& vz)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N || dt_full == 0.0) return;
-    const double x0 = x[3 * i], y0 = x[3 * i + 1], z0 = x[3 * i + 2];
-    const double vx = v[3 * i], vy = v[3 * i + 1], vz = v[3 * i + 2];
     const double r0 = sqrt(x0 * x0 + y0 * y0 + z0 * z0);
     const double v2 = vx * vx + vy * vy + vz * vz;
     const double u  = x0 * vx + y0 * vy + z0 * vz;
@@ -67,7 +65,7 @@ drift_kernel(int N, double mu, double dt_full, double* __restrict__ x, double* _
     }
 
     double s = dt / r0;                                  // first-order start
-    {   // second/third-order refinement of the start (series of s in dt)
+    {   // second-order refinement of the start (series of s in dt)
         const double a1 = u / (r0 * r0);
         s = s * (1.0 - 0.5 * a1 * s);
     }
@@ -94,18 +92,54 @@ drift_kernel(int N, double mu, double dt_full, double* __restrict__ x, double* _
         // correction is far below rounding, so only the G's are refreshed once more
         last = fabs(ds) < 1.0e-8 * fabs(s);
     }
-    if (!ok) atomicAdd(&ctr->noconv, 1u);
 
     const double f  = 1.0 - mu * G2 / r0;
     const double g  = fma(r0, G1, u * G2);
     const double fd = -mu * G1 / (r * r0);
     const double gd = 1.0 - mu * G2 / r;
-    x[3 * i]     = fma(f, x0, g * vx);
-    x[3 * i + 1] = fma(f, y0, g * vy);
-    x[3 * i + 2] = fma(f, z0, g * vz);
-    v[3 * i]     = fma(fd, x0, gd * vx);
-    v[3 * i + 1] = fma(fd, y0, gd * vy);
-    v[3 * i + 2] = fma(fd, z0, gd * vz);
+    const double nx = fma(f, x0, g * vx), ny = fma(f, y0, g * vy), nz = fma(f, z0, g * vz);
+    const double wx = fma(fd, x0, gd * vx), wy = fma(fd, y0, gd * vy), wz = fma(fd, z0, gd * vz);
+    x0 = nx; y0 = ny; z0 = nz; vx = wx; vy = wy; vz = wz;
+    return ok;
+}
+
+constexpr int DRIFT_NT = 128;
+
+__global__ void __launch_bounds__(DRIFT_NT)
+drift_kernel(int N, double mu, double dt_full, double* __restrict__ x, double* __restrict__ v, Counters* ctr)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N || dt_full == 0.0) return;
+    double x0 = x[3 * i], y0 = x[3 * i + 1], z0 = x[3 * i + 2];
+    double vx = v[3 * i], vy = v[3 * i + 1], vz = v[3 * i + 2];
+    if (!kepler_drift(mu, dt_full, x0, y0, z0, vx, vy, vz)) atomicAdd(&ctr->noconv, 1u);
+    x[3 * i] = x0; x[3 * i + 1] = y0; x[3 * i + 2] = z0;
+    v[3 * i] = vx; v[3 * i + 1] = vy; v[3 * i + 2] = vz;
+}
+
+// The middle of a fused step: Sun-kick S(tau_pre) with the momentum in mom[SLOT_A] (O8), Kepler drift
+// D(dt) (O9), and the momentum of the drifted velocities into mom[SLOT_B] for the closing Sun-kick,
+// which the next prep kernel applies.
+__global__ void __launch_bounds__(DRIFT_NT)
+shift_drift_mom_kernel(int N, double mu, double dt_full, double shift_scale, double* __restrict__ x,
+                       double* __restrict__ v, const double* __restrict__ m, double* __restrict__ mom, Counters* ctr)
+{
+    const int i = blockIdx.x * DRIFT_NT + threadIdx.x;
+    double p0 = 0, p1 = 0, p2 = 0, mt = 0;
+    if (i < N) {
+        double x0 = fma(shift_scale, mom[MOM_SLOT_A + 0], x[3 * i]);
+        double y0 = fma(shift_scale, mom[MOM_SLOT_A + 1], x[3 * i + 1]);
+        double z0 = fma(shift_scale, mom[MOM_SLOT_A + 2], x[3 * i + 2]);
+        double vx = v[3 * i], vy = v[3 * i + 1], vz = v[3 * i + 2];
+        if (dt_full != 0.0) {
+            if (!kepler_drift(mu, dt_full, x0, y0, z0, vx, vy, vz)) atomicAdd(&ctr->noconv, 1u);
+            v[3 * i] = vx; v[3 * i + 1] = vy; v[3 * i + 2] = vz;
+        }
+        x[3 * i] = x0; x[3 * i + 1] = y0; x[3 * i + 2] = z0;
+        const double mi = m[i];
+        p0 = mi * vx; p1 = mi * vy; p2 = mi * vz; mt = mi;
+    }
+    grid_momentum(p0, p1, p2, mt, mom + MOM_PARTIALS, mom + MOM_SLOT_B, &ctr->ticket);
 }
 
 }  // namespace
@@ -114,6 +148,13 @@ void launch_drift(const Handle* h, double dt)
 {
     if (h->N == 0) return;
     drift_kernel<<<(h->N + 127) / 128, 128, 0, h->stream>>>(h->N, h->p.G * h->p.M_star, dt, h->w.x, h->w.v, h->w.ctr);
+}
+
+void launch_shift_drift_mom(const Handle* h, double tau_pre, double dt)
+{
+    if (h->N == 0) return;
+    shift_drift_mom_kernel<<<(h->N + DRIFT_NT - 1) / DRIFT_NT, DRIFT_NT, 0, h->stream>>>(
+        h->N, h->p.G * h->p.M_star, dt, tau_pre / h->p.M_star, h->w.x, h->w.v, h->w.m, h->w.mom, h->w.ctr);
 }
 
 }  // namespace genga

@@ -66,6 +66,7 @@ struct Workspace {
     // scratch
     double*  red;     // [RED_DOUBLES] reduction scratch / results
     double*  vtmp;    // [NP][3] staging for heliocentric-velocity output
+    double*  mom;     // momentum slots and per-block partials of the fused step (momentum.cuh)
     Counters* ctr;
 };
 
@@ -81,6 +82,7 @@ struct Handle {
     int num_sms;
     long long launches;
     // internal order (a performance hint only: results never depend on it)
+    bool mom_a_valid;            // mom[SLOT_A] holds sum m v of the stored velocities
     int tune[4];                 // genga_set_tuning: [0] kick32 variant, [1] kick64 variant
     int resort_every;            // force evaluations between two sorts
     int evals_since_sort;        // < 0: no order yet
@@ -104,6 +106,7 @@ struct PrepArgs {
     double G, M_star, n1, n2, dt_rcrit;
     int pair_rule;
     float lambda, floor_rel;     // near-field policy for this evaluation
+    double preshift;             // pending Sun-kick: x += preshift * mom[SLOT_B] / M_star before anything else
 };
 void launch_hcbrt(const Handle* h);
 void launch_pad(const Handle* h);                            // padding bodies: x = (PAD_POS,0,0), v = 0, m = 0
@@ -114,6 +117,9 @@ void launch_kick64(const Handle* h);
 void launch_nearfield(const Handle* h);
 void launch_velupdate(const Handle* h, double tau);
 void launch_momentum(const Handle* h);                       // red[0..2] = sum m v, red[3] = sum m
+void launch_momentum_slot_a(const Handle* h);                // the same into mom[SLOT_A]
+void launch_velupdate_mom(const Handle* h, double tau);      // v += tau a; mom[SLOT_A] = sum m v
+void launch_shift_drift_mom(const Handle* h, double tau_pre, double dt);   // S(tau_pre) D(dt); mom[SLOT_B] = sum m v
 void launch_shift_v(const Handle* h, double scale);          // v_i += scale * red[0..2]   (O1)
 void launch_sunkick(const Handle* h, double tau);            // x_i += tau * red[0..2] / M_star
 void launch_drift(const Handle* h, double dt);

@@ -40,6 +40,18 @@ __device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c)
 {
     f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r;
 }
+// MODE 0: add/mul/fma as written; MODE 1: every packed add and mul issued as an FFMA2
+// (x * 1 + y, x * y + (-0)): bitwise the same results, one opcode for the FMA pipe.
+template <int MODE> __device__ __forceinline__ f2 addm(f2 a, f2 b)
+{
+    if (MODE == 1) return fma2(a, 0x3f8000003f800000ull, b);
+    return add2(a, b);
+}
+template <int MODE> __device__ __forceinline__ f2 mulm(f2 a, f2 b)
+{
+    if (MODE == 1) return fma2(a, b, 0x8000000080000000ull);
+    return mul2(a, b);
+}
 __device__ __forceinline__ float rsq(float a)
 {
     float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r;
@@ -62,7 +74,7 @@ struct __align__(16) Smem32 {
     uint64_t full[NSTAGE];
 };
 
-template <int I, int NT, int MINB, bool ACCS, int UNR>
+template <int I, int NT, int MINB, bool ACCS, int UNR, bool PIPE, int MODE>
 __global__ void __launch_bounds__(NT, MINB)
 kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 {
@@ -141,27 +153,84 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                 }
 
                 const float4* jp = &sm.j[b][ch * CHUNK];
+                if (!PIPE) {
 #pragma unroll UNR
-                for (int jj = 0; jj < CHUNK / 2; ++jj) {
-                    const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
-                    const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y), gj = pk(B.z, B.w);
+                    for (int jj = 0; jj < CHUNK / 2; ++jj) {
+                        const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
+                        const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y), gj = pk(B.z, B.w);
+#pragma unroll
+                        for (int k = 0; k < I; ++k) {
+                            const f2 dx = addm<MODE>(xj, pk(nx[k], nx[k]));
+                            const f2 dy = addm<MODE>(yj, pk(ny[k], ny[k]));
+                            const f2 dz = addm<MODE>(zj, pk(nz[k], nz[k]));
+                            f2 r2 = mulm<MODE>(dx, dx);
+                            r2 = fma2(dy, dy, r2);
+                            r2 = fma2(dz, dz, r2);
+                            float r2a, r2b; upk(r2, r2a, r2b);
+                            mn[k] = min3(mn[k], r2a, r2b);
+                            const f2 y = pk(rsq(r2a), rsq(r2b));
+                            const f2 t = mulm<MODE>(y, y);
+                            f2 s = mulm<MODE>(y, gj);
+                            s = mulm<MODE>(s, t);
+                            ax[k] = fma2(s, dx, ax[k]);
+                            ay[k] = fma2(s, dy, ay[k]);
+                            az[k] = fma2(s, dz, az[k]);
+                        }
+                    }
+                } else {
+                    // software pipeline: separations, r^2 and MUFU of pair jj + 1 are issued before the
+                    // multiply/accumulate half of pair jj, so the MUFU latency hides behind FMA work
+                    f2 dxp[I], dyp[I], dzp[I], yp[I], gp;
+                    {
+                        const float4 A = jp[0], B = jp[1];
+                        const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y);
+                        gp = pk(B.z, B.w);
+#pragma unroll
+                        for (int k = 0; k < I; ++k) {
+                            dxp[k] = add2(xj, pk(nx[k], nx[k]));
+                            dyp[k] = add2(yj, pk(ny[k], ny[k]));
+                            dzp[k] = add2(zj, pk(nz[k], nz[k]));
+                            f2 r2 = mul2(dxp[k], dxp[k]);
+                            r2 = fma2(dyp[k], dyp[k], r2);
+                            r2 = fma2(dzp[k], dzp[k], r2);
+                            float r2a, r2b; upk(r2, r2a, r2b);
+                            mn[k] = min3(mn[k], r2a, r2b);
+                            yp[k] = pk(rsq(r2a), rsq(r2b));
+                        }
+                    }
+#pragma unroll UNR
+                    for (int jj = 1; jj < CHUNK / 2; ++jj) {
+                        const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
+                        const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y), gj = pk(B.z, B.w);
+#pragma unroll
+                        for (int k = 0; k < I; ++k) {
+                            const f2 dx = add2(xj, pk(nx[k], nx[k]));
+                            const f2 dy = add2(yj, pk(ny[k], ny[k]));
+                            const f2 dz = add2(zj, pk(nz[k], nz[k]));
+                            f2 r2 = mul2(dx, dx);
+                            r2 = fma2(dy, dy, r2);
+                            r2 = fma2(dz, dz, r2);
+                            float r2a, r2b; upk(r2, r2a, r2b);
+                            mn[k] = min3(mn[k], r2a, r2b);
+                            const f2 yn = pk(rsq(r2a), rsq(r2b));
+                            const f2 t = mul2(yp[k], yp[k]);
+                            f2 s = mul2(yp[k], gp);
+                            s = mul2(s, t);
+                            ax[k] = fma2(s, dxp[k], ax[k]);
+                            ay[k] = fma2(s, dyp[k], ay[k]);
+                            az[k] = fma2(s, dzp[k], az[k]);
+                            dxp[k] = dx; dyp[k] = dy; dzp[k] = dz; yp[k] = yn;
+                        }
+                        gp = gj;
+                    }
 #pragma unroll
                     for (int k = 0; k < I; ++k) {
-                        const f2 dx = add2(xj, pk(nx[k], nx[k]));
-                        const f2 dy = add2(yj, pk(ny[k], ny[k]));
-                        const f2 dz = add2(zj, pk(nz[k], nz[k]));
-                        f2 r2 = mul2(dx, dx);
-                        r2 = fma2(dy, dy, r2);
-                        r2 = fma2(dz, dz, r2);
-                        float r2a, r2b; upk(r2, r2a, r2b);
-                        mn[k] = min3(mn[k], r2a, r2b);
-                        const f2 y = pk(rsq(r2a), rsq(r2b));
-                        const f2 t = mul2(y, y);
-                        f2 s = mul2(y, gj);
+                        const f2 t = mul2(yp[k], yp[k]);
+                        f2 s = mul2(yp[k], gp);
                         s = mul2(s, t);
-                        ax[k] = fma2(s, dx, ax[k]);
-                        ay[k] = fma2(s, dy, ay[k]);
-                        az[k] = fma2(s, dz, az[k]);
+                        ax[k] = fma2(s, dxp[k], ax[k]);
+                        ay[k] = fma2(s, dyp[k], ay[k]);
+                        az[k] = fma2(s, dzp[k], az[k]);
                     }
                 }
 
@@ -214,32 +283,19 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 typedef void (*kick32_fn)(int, int, int, Workspace, unsigned int);
 struct Variant32 { kick32_fn fn; int nt; int bi; size_t smem; const char* name; };
 
-#define V32(I_, NT_, MINB_, ACCS_, UNR_) \
-    { kick32_kernel<I_, NT_, MINB_, ACCS_, UNR_>, NT_, I_ * NT_, sizeof(Smem32<I_, NT_, ACCS_>), \
-      "I" #I_ " NT" #NT_ " minB" #MINB_ " accS" #ACCS_ " unr" #UNR_ }
+#define V32(I_, NT_, MINB_, ACCS_, UNR_, PIPE_, MODE_) \
+    { kick32_kernel<I_, NT_, MINB_, ACCS_, UNR_, PIPE_, MODE_>, NT_, I_ * NT_, sizeof(Smem32<I_, NT_, ACCS_>), \
+      "I" #I_ " NT" #NT_ " minB" #MINB_ " accS" #ACCS_ " unr" #UNR_ " pipe" #PIPE_ " mode" #MODE_ }
 
 const Variant32 g_variants32[] = {
-    V32(2, 256, 2, false, 2),     // 0: default
-    V32(4, 128, 4, false, 2),
-    V32(2, 256, 2, false, 4),
-    V32(2, 256, 2, false, 8),
-    V32(2, 256, 2, false, 1),
-    V32(2, 256, 2, true, 2),
-    V32(2, 256, 2, true, 4),
-    V32(2, 128, 4, false, 2),
-    V32(2, 128, 4, false, 4),
-    V32(2, 128, 4, true, 4),
-    V32(2, 128, 5, true, 4),
-    V32(2, 128, 6, true, 4),
-    V32(1, 512, 1, false, 4),
-    V32(1, 512, 1, false, 8),
-    V32(1, 256, 2, false, 8),
-    V32(1, 256, 3, false, 8),
-    V32(1, 128, 6, false, 8),
-    V32(2, 64, 8, false, 4),
-    V32(4, 64, 8, false, 2),
-    V32(4, 128, 3, false, 4),
-    V32(4, 128, 3, true, 4),
+    V32(2, 256, 2, false, 2, false, 0),     // 0: default
+    V32(1, 512, 1, false, 4, false, 0),
+    V32(2, 256, 2, true, 2, false, 0),
+    V32(4, 128, 3, true, 4, false, 0),
+    V32(4, 128, 4, false, 2, false, 0),
+    V32(2, 128, 4, false, 4, false, 0),
+    V32(2, 256, 2, false, 4, true, 0),
+    V32(2, 256, 2, false, 2, false, 1),
 };
 constexpr int NVAR32 = (int)(sizeof(g_variants32) / sizeof(g_variants32[0]));
 bool g_attr32[NVAR32] = {};

@@ -2,6 +2,7 @@
 // packing of the j-side arrays, the conservative near-field bound parameters, velocity update,
 // momentum reduction, Sun-kick (reading G3) and the velocity-convention shifts (O1).
 #include "genga_internal.cuh"
+#include "momentum.cuh"
 
 namespace genga {
 
@@ -115,6 +116,7 @@ __global__ void __launch_bounds__(PREP_NT)
 prep_kernel(PrepArgs A, Workspace w)
 {
     __shared__ unsigned int smax[PREP_NT / 32][4];
+    __shared__ double sorg[PREP_NT / CHUNK][3];
     const int s = blockIdx.x * PREP_NT + threadIdx.x;      // slot; grid covers NP exactly (NP % 512 == 0)
     const bool live = s < A.N;
     const int i = w.order[s];                              // body held by this slot (= s for padding)
@@ -125,6 +127,12 @@ prep_kernel(PrepArgs A, Workspace w)
     if (live) {
         const double mu = A.G * A.M_star;
         px = w.x[3 * i + 0]; py = w.x[3 * i + 1]; pz = w.x[3 * i + 2];
+        if (A.preshift != 0.0) {                           // pending Sun-kick S(tau) of the fused step (O8)
+            const double sc = A.preshift / A.M_star;
+            px = fma(sc, w.mom[MOM_SLOT_B + 0], px); py = fma(sc, w.mom[MOM_SLOT_B + 1], py);
+            pz = fma(sc, w.mom[MOM_SLOT_B + 2], pz);
+            w.x[3 * i + 0] = px; w.x[3 * i + 1] = py; w.x[3 * i + 2] = pz;
+        }
         const double vx = w.v[3 * i + 0], vy = w.v[3 * i + 1], vz = w.v[3 * i + 2];
         const double r  = sqrt(px * px + py * py + pz * pz);
         const double v2 = vx * vx + vy * vy + vz * vz;
@@ -157,12 +165,14 @@ prep_kernel(PrepArgs A, Workspace w)
     w.a[3 * i + 0] = 0.0; w.a[3 * i + 1] = 0.0; w.a[3 * i + 2] = 0.0;
     w.pk64[s] = make_double4(px, py, pz, gm);
     w.aux[s]  = ax4;
-    // local frame of this slot's chunk: origin = position of the chunk's first slot (FP32 policy P32)
-    double ox = PAD_POS, oy = 0.0, oz = 0.0;
-    {
-        const int s0 = s & ~(CHUNK - 1);
-        if (s0 < A.N) { const int i0 = w.order[s0]; ox = w.x[3 * i0 + 0]; oy = w.x[3 * i0 + 1]; oz = w.x[3 * i0 + 2]; }
+    // local frame of this slot's chunk: origin = position of the chunk's first slot (FP32 policy P32),
+    // handed over through shared memory (the chunk's 64 slots are two warps of this block)
+    if ((s & (CHUNK - 1)) == 0) {
+        const int c = threadIdx.x / CHUNK;
+        sorg[c][0] = px; sorg[c][1] = py; sorg[c][2] = pz;
     }
+    __syncthreads();
+    const double ox = sorg[threadIdx.x / CHUNK][0], oy = sorg[threadIdx.x / CHUNK][1], oz = sorg[threadIdx.x / CHUNK][2];
     const double qx = px - ox, qy = py - oy, qz = pz - oz;
     float rad = 0.f;                                        // |x - o|, rounded up; padding does not count
     if (live) {
@@ -195,11 +205,8 @@ prep_kernel(PrepArgs A, Workspace w)
         q.rf  = fmaxf(__uint_as_float(max(smax[2 * c][2], smax[2 * c + 1][2])),
                       __fmul_ru(__fmul_ru(2.0f * A.floor_rel, q.rad), 1.000001f));
         q.pad_ = 0.0;
-        const int cg = blockIdx.x * (PREP_NT / CHUNK) + c;
-        const int s0 = cg * CHUNK;
-        q.ox = PAD_POS; q.oy = 0.0; q.oz = 0.0;
-        if (s0 < A.N) { const int i0 = w.order[s0]; q.ox = w.x[3 * i0 + 0]; q.oy = w.x[3 * i0 + 1]; q.oz = w.x[3 * i0 + 2]; }
-        w.bc[cg] = q;
+        q.ox = sorg[c][0]; q.oy = sorg[c][1]; q.oz = sorg[c][2];
+        w.bc[blockIdx.x * (PREP_NT / CHUNK) + c] = q;
     }
     if (s == 0) { w.ctr->cand_count = 0u; w.ctr->pair_count = 0u; w.ctr->overflow = 0u; }
 }
@@ -211,59 +218,38 @@ __global__ void velupdate_kernel(int n3, double tau, const double* __restrict__ 
     if (k < n3) v[k] = fma(tau, a[k], v[k]);
 }
 
-// red[0..2] = sum_j m_j v_j, red[3] = sum_j m_j.  Every block reduces its slice to a partial
-// (red[MOM_PART + 4 b ..]); the last block to finish (ticket) combines the partials with a fixed
-// assignment and tree, so the result is bitwise reproducible for a given N.
+// out[0..2] = sum_j m_j v_j, out[3] = sum_j m_j (momentum.cuh: fixed-tree, last block combines).
 constexpr int MOM_NT = 256;
-constexpr int MOM_PART = 8 + 4096;                 // partials live in the upper half of red[]
-constexpr int MOM_MAXB = 512;
-
-__device__ __forceinline__ void warp_sum4(double& a, double& b, double& c, double& d)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        a += __shfl_down_sync(0xffffffffu, a, o); b += __shfl_down_sync(0xffffffffu, b, o);
-        c += __shfl_down_sync(0xffffffffu, c, o); d += __shfl_down_sync(0xffffffffu, d, o);
-    }
-}
 
 __global__ void __launch_bounds__(MOM_NT)
-momentum_kernel(int N, const double* __restrict__ m, const double* __restrict__ v, double* __restrict__ red,
-                unsigned int* __restrict__ ticket)
+momentum_kernel(int N, const double* __restrict__ m, const double* __restrict__ v, double* __restrict__ partials,
+                double* __restrict__ out, unsigned int* __restrict__ ticket)
 {
-    __shared__ double s[MOM_NT / 32][4];
-    __shared__ bool last;
     double p0 = 0, p1 = 0, p2 = 0, mt = 0;
     for (int i = blockIdx.x * MOM_NT + threadIdx.x; i < N; i += gridDim.x * MOM_NT) {
         const double mi = m[i];
         p0 = fma(mi, v[3 * i + 0], p0); p1 = fma(mi, v[3 * i + 1], p1); p2 = fma(mi, v[3 * i + 2], p2);
         mt += mi;
     }
-    warp_sum4(p0, p1, p2, mt);
-    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (lane == 0) { s[wid][0] = p0; s[wid][1] = p1; s[wid][2] = p2; s[wid][3] = mt; }
-    __syncthreads();
-    if (wid == 0) {
-        const bool in = lane < MOM_NT / 32;
-        p0 = in ? s[lane][0] : 0.0; p1 = in ? s[lane][1] : 0.0; p2 = in ? s[lane][2] : 0.0; mt = in ? s[lane][3] : 0.0;
-        warp_sum4(p0, p1, p2, mt);
-        if (lane == 0) {
-            double* q = red + MOM_PART + 4 * blockIdx.x;
-            q[0] = p0; q[1] = p1; q[2] = p2; q[3] = mt;
-            __threadfence();
-            last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
-        }
+    grid_momentum(p0, p1, p2, mt, partials, out, ticket);
+}
+
+// O7 fused with the momentum of the new velocities: v_i += tau a_i; mom[SLOT_A] = sum m v.
+__global__ void __launch_bounds__(MOM_NT)
+velupdate_mom_kernel(int N, double tau, const double* __restrict__ a, double* __restrict__ v,
+                     const double* __restrict__ m, double* __restrict__ mom, unsigned int* __restrict__ ticket)
+{
+    const int i = blockIdx.x * MOM_NT + threadIdx.x;
+    double p0 = 0, p1 = 0, p2 = 0, mt = 0;
+    if (i < N) {
+        const double mi = m[i];
+        const double v0 = fma(tau, a[3 * i + 0], v[3 * i + 0]);
+        const double v1 = fma(tau, a[3 * i + 1], v[3 * i + 1]);
+        const double v2 = fma(tau, a[3 * i + 2], v[3 * i + 2]);
+        v[3 * i + 0] = v0; v[3 * i + 1] = v1; v[3 * i + 2] = v2;
+        p0 = mi * v0; p1 = mi * v1; p2 = mi * v2; mt = mi;
     }
-    __syncthreads();
-    if (!last || wid != 0) return;
-    __threadfence();
-    p0 = p1 = p2 = mt = 0.0;
-    for (int b = lane; b < (int)gridDim.x; b += 32) {
-        const volatile double* q = red + MOM_PART + 4 * b;
-        p0 += q[0]; p1 += q[1]; p2 += q[2]; mt += q[3];
-    }
-    warp_sum4(p0, p1, p2, mt);
-    if (lane == 0) { red[0] = p0; red[1] = p1; red[2] = p2; red[3] = mt; *ticket = 0u; }
+    grid_momentum(p0, p1, p2, mt, mom + MOM_PARTIALS, mom + MOM_SLOT_A, ticket);
 }
 
 // q_i[k] += scale * red[k]: O1 (q = v, scale = -1/(M_star + sum m) with red[3], or +1/M_star) and
@@ -324,13 +310,31 @@ void launch_velupdate(const Handle* h, double tau)
     velupdate_kernel<<<(n3 + 255) / 256, 256, 0, h->stream>>>(n3, tau, h->w.a, h->w.v);
 }
 
-void launch_momentum(const Handle* h)
+static int momentum_blocks(const Handle* h)
 {
     int blocks = (h->N + MOM_NT * 4 - 1) / (MOM_NT * 4);
     if (blocks < 1) blocks = 1;
     if (blocks > h->num_sms) blocks = h->num_sms;
-    if (blocks > MOM_MAXB) blocks = MOM_MAXB;
-    momentum_kernel<<<blocks, MOM_NT, 0, h->stream>>>(h->N, h->w.m, h->w.v, h->w.red, &h->w.ctr->ticket);
+    return blocks;
+}
+
+void launch_momentum(const Handle* h)
+{
+    momentum_kernel<<<momentum_blocks(h), MOM_NT, 0, h->stream>>>(h->N, h->w.m, h->w.v, h->w.mom + MOM_PARTIALS,
+                                                                   h->w.red, &h->w.ctr->ticket);
+}
+
+void launch_momentum_slot_a(const Handle* h)
+{
+    momentum_kernel<<<momentum_blocks(h), MOM_NT, 0, h->stream>>>(h->N, h->w.m, h->w.v, h->w.mom + MOM_PARTIALS,
+                                                                   h->w.mom + MOM_SLOT_A, &h->w.ctr->ticket);
+}
+
+void launch_velupdate_mom(const Handle* h, double tau)
+{
+    if (h->N == 0) return;
+    velupdate_mom_kernel<<<(h->N + MOM_NT - 1) / MOM_NT, MOM_NT, 0, h->stream>>>(h->N, tau, h->w.a, h->w.v, h->w.m,
+                                                                                 h->w.mom, &h->w.ctr->ticket);
 }
 
 void launch_shift_v(const Handle* h, double scale)
