@@ -153,10 +153,10 @@ int genga_get_rcrit(genga_handle h, double* rcrit);      /* DEVICE [N]: r_crit,i
  * whether the candidate list overflowed (exact slow path taken).  HOST outputs.  Synchronises.  */
 int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed);
 
-/* Per-kernel device timing.  enable != 0 brackets every force-kernel launch with CUDA events on
- * params.stream.  genga_kernel_time returns, for which = 0 (all-pairs kick kernel), 1 (near-field
- * kernel), 2 (prep kernel), 3 (drift kernel), the summed milliseconds and launch count since the
- * last reset (HOST outputs).  Synchronises.                                                     */
+/* Per-kernel device timing.  enable is a bit mask: bit k brackets every launch of kernel class k with
+ * CUDA events on params.stream; classes: 0 all-pairs kick kernel, 1 near-field kernel, 2 prep kernel,
+ * 3 drift kernel (15 = all, 0 = off).  genga_kernel_time returns, for class which, the summed
+ * milliseconds and launch count since the last reset (HOST outputs).  Synchronises.              */
 int genga_set_profiling(genga_handle h, int enable);
 int genga_kernel_time(genga_handle h, int which, double* ms_total, long long* launches, int reset);
 
@@ -164,6 +164,11 @@ int genga_kernel_time(genga_handle h, int which, double* ms_total, long long* la
  * launch/tiling variant of the FP32 all-pairs kernel, key 1 of the FP64 one; value in
  * [0, genga_num_variants(key)); 0 is the default.  Results are identical up to summation order. */
 int genga_set_tuning(genga_handle h, int key, int value);
+/* Time every variant of the given precision's all-pairs kernel on the current state (force evaluation
+ * = prep + all-pairs + near field, 1 warm-up + 3 timed runs each) and keep the fastest.  HOST
+ * outputs (may be NULL): the chosen variant and its time.  The stored state is unchanged; the
+ * acceleration and pair list are those of the last timed evaluation.  Synchronises.               */
+int genga_autotune(genga_handle h, int precision, int* chosen, double* ms_best);
 int genga_num_variants(int key);
 const char* genga_variant_name(int key, int value);
 

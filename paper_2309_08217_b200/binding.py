@@ -28,7 +28,7 @@ SYMBOLS = [
     "genga_get_state", "genga_get_state_host", "genga_get_accel", "genga_get_rcrit",
     "genga_nearfield_stats", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
     "genga_synchronize", "genga_strerror", "genga_last_cuda_error", "genga_version",
-    "genga_peak_probe", "genga_set_tuning", "genga_num_variants", "genga_variant_name",
+    "genga_peak_probe", "genga_set_tuning", "genga_autotune", "genga_num_variants", "genga_variant_name",
 ]
 
 
@@ -94,6 +94,7 @@ def load() -> ctypes.CDLL:
     L.genga_version.argtypes = []; L.genga_version.restype = ctypes.c_char_p
     L.genga_peak_probe.argtypes = [ctypes.c_int, ctypes.c_int, vp, dp, dp]
     L.genga_set_tuning.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+    L.genga_autotune.argtypes = [vp, ctypes.c_int, ip, dp]
     L.genga_num_variants.argtypes = [ctypes.c_int]
     L.genga_variant_name.argtypes = [ctypes.c_int, ctypes.c_int]; L.genga_variant_name.restype = ctypes.c_char_p
     for name in SYMBOLS:
@@ -285,7 +286,9 @@ class Genga:
         return NearfieldStats(int(c.value), bool(o.value))
 
     def set_profiling(self, enable=True):
-        _check(self._L.genga_set_profiling(self._h, int(bool(enable))), "genga_set_profiling")
+        """enable: True (all kernel classes), False, or a bit mask (1 kick, 2 near field, 4 prep, 8 drift)."""
+        mask = 15 if enable is True else int(enable)
+        _check(self._L.genga_set_profiling(self._h, mask), "genga_set_profiling")
 
     def kernel_time(self, which, reset=False):
         """(total ms, launches) of kernel class which: 0 all-pairs kick, 1 near field, 2 prep, 3 drift."""
@@ -296,6 +299,12 @@ class Genga:
 
     def set_tuning(self, key, value):
         _check(self._L.genga_set_tuning(self._h, int(key), int(value)), "genga_set_tuning")
+
+    def autotune(self, precision):
+        """genga_autotune: returns (chosen variant, its force-evaluation time in ms)."""
+        v, ms = ctypes.c_int(0), ctypes.c_double(0)
+        _check(self._L.genga_autotune(self._h, int(precision), ctypes.byref(v), ctypes.byref(ms)), "genga_autotune")
+        return int(v.value), float(ms.value)
 
     def launch_count(self) -> int:
         return int(self._L.genga_launch_count(self._h))

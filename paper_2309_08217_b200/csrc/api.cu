@@ -75,7 +75,7 @@ static int prof_flush(Handle* h, int which)
 
 struct ProfScope {
     Handle* h; int which; bool on;
-    ProfScope(Handle* h_, int w_) : h(h_), which(w_), on(h_->prof != 0)
+    ProfScope(Handle* h_, int w_) : h(h_), which(w_), on(((h_->prof >> w_) & 1) != 0)
     {
         if (!on) return;
         if (h->evn[which] == Handle::EVPOOL) prof_flush(h, which);
@@ -115,6 +115,7 @@ static int force_eval(Handle* h, int precision, double preshift = 0.0)
     a.G = h->p.G; a.M_star = h->p.M_star; a.n1 = h->p.n1; a.n2 = h->p.n2; a.dt_rcrit = h->p.dt_rcrit;
     a.pair_rule = h->p.pair_rule;
     a.preshift = preshift;
+    a.scaled = (precision == GENGA_FP32 && kick32_variant_scaled(h->tune[0])) ? 1 : 0;
     if (precision == GENGA_FP32) { a.lambda = (float)h->lambda_near; a.floor_rel = (float)h->near_floor; }
     else                         { a.lambda = 1.0f;                  a.floor_rel = 0.0f; }
     { ProfScope ps(h, 2); launch_prep(h, a); }
@@ -438,7 +439,7 @@ int genga_set_profiling(genga_handle h, int enable)
         h->events_created = true;
     }
     if (!enable && h->prof) for (int w = 0; w < Handle::NKT; ++w) prof_flush(h, w);
-    h->prof = enable ? 1 : 0;
+    h->prof = enable & 15;
     return GENGA_OK;
 }
 
@@ -486,6 +487,42 @@ int genga_set_tuning(genga_handle h, int key, int value)
     if (value < 0 || value >= n) return GENGA_EINVAL;
     h->tune[key] = value;
     return GENGA_OK;
+}
+
+// Self-tuning in the sense of PAPER.md:55 ("tries configurations ... before the run"): time the
+// force evaluation (prep + all-pairs + near field) of every variant on the current state and keep
+// the fastest.  The state is not modified (only the acceleration / pair list of the last evaluation).
+int genga_autotune(genga_handle h, int precision, int* chosen, double* ms_best)
+{
+    if (!h || (precision != GENGA_FP64 && precision != GENGA_FP32)) return GENGA_EINVAL;
+    const int key = precision == GENGA_FP32 ? 0 : 1;
+    const int n = key == 0 ? kick32_num_variants() : kick64_num_variants();
+    if (h->N == 0) { if (chosen) *chosen = h->tune[key]; if (ms_best) *ms_best = 0.0; return GENGA_OK; }
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+    const int prof = h->prof; h->prof = 0;
+    int best = h->tune[key], rc = GENGA_OK;
+    double best_ms = 1.0e300;
+    for (int v = 0; v < n && rc == GENGA_OK; ++v) {
+        h->tune[key] = v;
+        if ((rc = force_eval(h, precision)) != GENGA_OK) break;             // warm-up (and first-use setup)
+        double ms_min = 1.0e300;
+        for (int rep = 0; rep < 3 && rc == GENGA_OK; ++rep) {
+            cudaEventRecord(e0, h->stream);
+            rc = force_eval(h, precision);
+            cudaEventRecord(e1, h->stream);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = GENGA_ECUDA; break; }
+            float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+            if (ms < ms_min) ms_min = ms;
+        }
+        if (rc == GENGA_OK && ms_min < best_ms) { best_ms = ms_min; best = v; }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    h->prof = prof;
+    h->tune[key] = best;
+    if (chosen) *chosen = best;
+    if (ms_best) *ms_best = best_ms;
+    return rc;
 }
 
 int genga_num_variants(int key)

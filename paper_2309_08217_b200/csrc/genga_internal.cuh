@@ -11,8 +11,8 @@
 namespace genga {
 
 // ---- tiling constants -------------------------------------------------
-constexpr int CHUNK      = 64;                  // j-bodies per chunk: granularity of the near-field flag
-constexpr int STAGE_CH   = 8;                   // chunks per shared-memory stage
+constexpr int CHUNK      = 128;                 // j-bodies per chunk: granularity of the near-field flag
+constexpr int STAGE_CH   = 4;                  // chunks per shared-memory stage
 constexpr int STAGE_J    = CHUNK * STAGE_CH;    // 512 j-bodies per stage
 constexpr int NSTAGE     = 2;                   // double buffering
 constexpr int PAD_BODIES = 512;                 // N is padded to a multiple of this (stage and i-block size)
@@ -25,7 +25,7 @@ struct __align__(16) BoundP { float hq, aq, rf, pad; };
 // per-chunk record staged next to the j-tile: the maxima of the bound parameters over the chunk
 // and the origin of the chunk's local frame (FP32 policy P32: the FP32 kernel sees positions
 // relative to o; Rf already contains the frame guard floor * 2 * max_j |x_j - o|).
-struct __align__(16) ChunkP { double ox, oy, oz; float hq, aq, rf, rad; double pad_; };
+struct __align__(16) ChunkP { double ox, oy, oz; float hq, aq, rf, rad; float q2max, pad_; };
 static_assert(sizeof(ChunkP) == 48, "ChunkP is staged with 16-byte bulk copies");
 
 // j-side layouts.  FP32: two bodies per 32 bytes (packed for FFMA2 along j):
@@ -90,7 +90,7 @@ struct Handle {
     // profiling
     int prof;
     static constexpr int NKT = 4;
-    static constexpr int EVPOOL = 64;
+    static constexpr int EVPOOL = 256;
     cudaEvent_t ev0[NKT][EVPOOL], ev1[NKT][EVPOOL];
     int evn[NKT];
     double ms_total[NKT];
@@ -106,6 +106,7 @@ struct PrepArgs {
     double G, M_star, n1, n2, dt_rcrit;
     int pair_rule;
     float lambda, floor_rel;     // near-field policy for this evaluation
+    int scaled;                  // FP32 j-records in the mass-scaled form (kick_fp32.cu, SC variants)
     double preshift;             // pending Sun-kick: x += preshift * mom[SLOT_B] / M_star before anything else
 };
 void launch_hcbrt(const Handle* h);
@@ -131,6 +132,7 @@ int  run_peak_probe(int which, int iters, cudaStream_t s, double* ops_per_s, dou
 int kick32_grid(const Handle* h);
 int kick64_grid(const Handle* h);
 int kick32_num_variants();
+bool kick32_variant_scaled(int v);      // does this variant read mass-scaled j-records?
 int kick64_num_variants();
 const char* kick32_variant_name(int v);
 const char* kick64_variant_name(int v);

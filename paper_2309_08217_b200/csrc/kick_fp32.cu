@@ -40,18 +40,6 @@ __device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c)
 {
     f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r;
 }
-// MODE 0: add/mul/fma as written; MODE 1: every packed add and mul issued as an FFMA2
-// (x * 1 + y, x * y + (-0)): bitwise the same results, one opcode for the FMA pipe.
-template <int MODE> __device__ __forceinline__ f2 addm(f2 a, f2 b)
-{
-    if (MODE == 1) return fma2(a, 0x3f8000003f800000ull, b);
-    return add2(a, b);
-}
-template <int MODE> __device__ __forceinline__ f2 mulm(f2 a, f2 b)
-{
-    if (MODE == 1) return fma2(a, b, 0x8000000080000000ull);
-    return mul2(a, b);
-}
 __device__ __forceinline__ float rsq(float a)
 {
     float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r;
@@ -59,6 +47,52 @@ __device__ __forceinline__ float rsq(float a)
 __device__ __forceinline__ float min3(float a, float b, float c)
 {
     float r; asm("min.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c)); return r;
+}
+
+constexpr float EPS2 = 1.0e-30f;   // added to r^2 so that the self pair (d = 0 exactly) contributes 0, not NaN;
+                                   // 1e-15 au: nothing for any pair the FP32 path keeps (r > lambda r_crit)
+
+// One j-chunk against the I i-bodies of this thread.  SELF: the chunk holds this warp's own
+// slots; the self pair is then left out of the smallest-r^2 tracking (slot index compare), so a
+// body's own chunk is flagged only if a DIFFERENT body is near.
+template <int I, int UNR, bool SELF, bool SC>
+__device__ __forceinline__ void pair_loop(const float4* __restrict__ jp, const float (&nx)[I], const float (&ny)[I],
+                                          const float (&nz)[I], f2 (&ax)[I], f2 (&ay)[I], f2 (&az)[I],
+                                          float (&mn)[I], const int (&self_off)[I])
+{
+    const f2 eps = pk(EPS2, EPS2);
+#pragma unroll UNR
+    for (int jj = 0; jj < CHUNK / 2; ++jj) {
+        const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
+        const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y), gj = pk(B.z, B.w);
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            // plain: d = x_j - x_i.  mass-scaled (SC): D = q_j x_j - q_j x_i with q = (G m)^(-1/2)
+            const f2 dx = SC ? fma2(gj, pk(nx[k], nx[k]), xj) : add2(xj, pk(nx[k], nx[k]));
+            const f2 dy = SC ? fma2(gj, pk(ny[k], ny[k]), yj) : add2(yj, pk(ny[k], ny[k]));
+            const f2 dz = SC ? fma2(gj, pk(nz[k], nz[k]), zj) : add2(zj, pk(nz[k], nz[k]));
+            f2 r2 = (SELF && !SC) ? fma2(dx, dx, eps) : mul2(dx, dx);
+            r2 = fma2(dy, dy, r2);
+            r2 = fma2(dz, dz, r2);
+            float r2a, r2b; upk(r2, r2a, r2b);
+            float ya, yb;
+            if (SELF) {
+                const bool sa = (2 * jj == self_off[k]), sb = (2 * jj + 1 == self_off[k]);
+                mn[k] = min3(mn[k], sa ? 3.0e38f : r2a, sb ? 3.0e38f : r2b);
+                ya = rsq(r2a); yb = rsq(r2b);
+                if (SC) { ya = sa ? 0.f : ya; yb = sb ? 0.f : yb; }   // D_self is rounding residue, not 0
+            } else {
+                mn[k] = min3(mn[k], r2a, r2b);
+                ya = rsq(r2a); yb = rsq(r2b);
+            }
+            const f2 y = pk(ya, yb);
+            const f2 t = mul2(y, y);
+            f2 s = SC ? mul2(t, y) : mul2(mul2(y, gj), t);       // SC: |D|^-3 = G m / r^3 / q
+            ax[k] = fma2(s, dx, ax[k]);
+            ay[k] = fma2(s, dy, ay[k]);
+            az[k] = fma2(s, dz, az[k]);
+        }
+    }
 }
 
 // Kernel configuration: I i-bodies per thread, NT threads per CTA (I * NT = 512 = one i-block),
@@ -74,7 +108,7 @@ struct __align__(16) Smem32 {
     uint64_t full[NSTAGE];
 };
 
-template <int I, int NT, int MINB, bool ACCS, int UNR, bool PIPE, int MODE>
+template <int I, int NT, int MINB, bool ACCS, int UNR, bool SC>
 __global__ void __launch_bounds__(NT, MINB)
 kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 {
@@ -153,94 +187,25 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                 }
 
                 const float4* jp = &sm.j[b][ch * CHUNK];
-                if (!PIPE) {
-#pragma unroll UNR
-                    for (int jj = 0; jj < CHUNK / 2; ++jj) {
-                        const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
-                        const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y), gj = pk(B.z, B.w);
+                // offset of each own slot inside this chunk (outside [0, CHUNK) unless it is the own chunk);
+                // warp-uniform decision: a warp's 32 slots of one k lie in one chunk
+                int self_off[I];
+                bool self = false;
 #pragma unroll
-                        for (int k = 0; k < I; ++k) {
-                            const f2 dx = addm<MODE>(xj, pk(nx[k], nx[k]));
-                            const f2 dy = addm<MODE>(yj, pk(ny[k], ny[k]));
-                            const f2 dz = addm<MODE>(zj, pk(nz[k], nz[k]));
-                            f2 r2 = mulm<MODE>(dx, dx);
-                            r2 = fma2(dy, dy, r2);
-                            r2 = fma2(dz, dz, r2);
-                            float r2a, r2b; upk(r2, r2a, r2b);
-                            mn[k] = min3(mn[k], r2a, r2b);
-                            const f2 y = pk(rsq(r2a), rsq(r2b));
-                            const f2 t = mulm<MODE>(y, y);
-                            f2 s = mulm<MODE>(y, gj);
-                            s = mulm<MODE>(s, t);
-                            ax[k] = fma2(s, dx, ax[k]);
-                            ay[k] = fma2(s, dy, ay[k]);
-                            az[k] = fma2(s, dz, az[k]);
-                        }
-                    }
-                } else {
-                    // software pipeline: separations, r^2 and MUFU of pair jj + 1 are issued before the
-                    // multiply/accumulate half of pair jj, so the MUFU latency hides behind FMA work
-                    f2 dxp[I], dyp[I], dzp[I], yp[I], gp;
-                    {
-                        const float4 A = jp[0], B = jp[1];
-                        const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y);
-                        gp = pk(B.z, B.w);
-#pragma unroll
-                        for (int k = 0; k < I; ++k) {
-                            dxp[k] = add2(xj, pk(nx[k], nx[k]));
-                            dyp[k] = add2(yj, pk(ny[k], ny[k]));
-                            dzp[k] = add2(zj, pk(nz[k], nz[k]));
-                            f2 r2 = mul2(dxp[k], dxp[k]);
-                            r2 = fma2(dyp[k], dyp[k], r2);
-                            r2 = fma2(dzp[k], dzp[k], r2);
-                            float r2a, r2b; upk(r2, r2a, r2b);
-                            mn[k] = min3(mn[k], r2a, r2b);
-                            yp[k] = pk(rsq(r2a), rsq(r2b));
-                        }
-                    }
-#pragma unroll UNR
-                    for (int jj = 1; jj < CHUNK / 2; ++jj) {
-                        const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
-                        const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y), gj = pk(B.z, B.w);
-#pragma unroll
-                        for (int k = 0; k < I; ++k) {
-                            const f2 dx = add2(xj, pk(nx[k], nx[k]));
-                            const f2 dy = add2(yj, pk(ny[k], ny[k]));
-                            const f2 dz = add2(zj, pk(nz[k], nz[k]));
-                            f2 r2 = mul2(dx, dx);
-                            r2 = fma2(dy, dy, r2);
-                            r2 = fma2(dz, dz, r2);
-                            float r2a, r2b; upk(r2, r2a, r2b);
-                            mn[k] = min3(mn[k], r2a, r2b);
-                            const f2 yn = pk(rsq(r2a), rsq(r2b));
-                            const f2 t = mul2(yp[k], yp[k]);
-                            f2 s = mul2(yp[k], gp);
-                            s = mul2(s, t);
-                            ax[k] = fma2(s, dxp[k], ax[k]);
-                            ay[k] = fma2(s, dyp[k], ay[k]);
-                            az[k] = fma2(s, dzp[k], az[k]);
-                            dxp[k] = dx; dyp[k] = dy; dzp[k] = dz; yp[k] = yn;
-                        }
-                        gp = gj;
-                    }
-#pragma unroll
-                    for (int k = 0; k < I; ++k) {
-                        const f2 t = mul2(yp[k], yp[k]);
-                        f2 s = mul2(yp[k], gp);
-                        s = mul2(s, t);
-                        ax[k] = fma2(s, dxp[k], ax[k]);
-                        ay[k] = fma2(s, dyp[k], ay[k]);
-                        az[k] = fma2(s, dzp[k], az[k]);
-                    }
+                for (int k = 0; k < I; ++k) {
+                    self_off[k] = ib * BI + k * NT + tid - (cs + ch) * CHUNK;
+                    self = self || (self_off[k] >= 0 && self_off[k] < CHUNK);
                 }
+                if (self) pair_loop<I, UNR, true, SC>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
+                else      pair_loop<I, UNR, false, SC>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
 
                 // ---- chunk end: keep the FP32 partial or hand the chunk to the near field ----
-                const float Hc = Bc.hq, Ac = Bc.aq, Rc = Bc.rf;
+                const float Hc = Bc.hq, Ac = Bc.aq, Rc = Bc.rf, Q2 = Bc.q2max;
 #pragma unroll
                 for (int k = 0; k < I; ++k) {
                     const float Bq = fmaxf(fmaxf(sm.bp[0][k][tid], Hc) * fmaxf(sm.bp[1][k][tid], Ac),
                                            fmaxf(sm.bp[2][k][tid], Rc));
-                    const float bound = (ib * BI + k * NT + tid < N) ? Bq * Bq : -1.0f;
+                    const float bound = (ib * BI + k * NT + tid < N) ? (SC ? Bq * Bq * Q2 : Bq * Bq) : -1.0f;
                     const bool keep = mn[k] > bound;
                     float lo, hi;
                     upk(ax[k], lo, hi); const float px = lo + hi;
@@ -281,21 +246,20 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 
 // ---- variants (genga_set_tuning key 0) ---------------------------------------------------------
 typedef void (*kick32_fn)(int, int, int, Workspace, unsigned int);
-struct Variant32 { kick32_fn fn; int nt; int bi; size_t smem; const char* name; };
+struct Variant32 { kick32_fn fn; int nt; int bi; size_t smem; bool scaled; const char* name; };
 
-#define V32(I_, NT_, MINB_, ACCS_, UNR_, PIPE_, MODE_) \
-    { kick32_kernel<I_, NT_, MINB_, ACCS_, UNR_, PIPE_, MODE_>, NT_, I_ * NT_, sizeof(Smem32<I_, NT_, ACCS_>), \
-      "I" #I_ " NT" #NT_ " minB" #MINB_ " accS" #ACCS_ " unr" #UNR_ " pipe" #PIPE_ " mode" #MODE_ }
+#define V32(I_, NT_, MINB_, ACCS_, UNR_, SC_) \
+    { kick32_kernel<I_, NT_, MINB_, ACCS_, UNR_, SC_>, NT_, I_ * NT_, sizeof(Smem32<I_, NT_, ACCS_>), SC_, \
+      "I" #I_ " NT" #NT_ " minB" #MINB_ " accS" #ACCS_ " unr" #UNR_ " scaled" #SC_ }
 
 const Variant32 g_variants32[] = {
-    V32(2, 256, 2, false, 2, false, 0),     // 0: default
-    V32(1, 512, 1, false, 4, false, 0),
-    V32(2, 256, 2, true, 2, false, 0),
-    V32(4, 128, 3, true, 4, false, 0),
-    V32(4, 128, 4, false, 2, false, 0),
-    V32(2, 128, 4, false, 4, false, 0),
-    V32(2, 256, 2, false, 4, true, 0),
-    V32(2, 256, 2, false, 2, false, 1),
+    V32(2, 256, 2, true, 2, false),      // 0: default
+    V32(2, 256, 2, false, 4, false),
+    V32(2, 256, 2, false, 2, false),
+    V32(2, 128, 4, false, 4, false),
+    V32(2, 256, 2, true, 4, true),       // mass-scaled j-records: 11 instead of 12 FMA-pipe operations per pair
+    V32(1, 512, 1, false, 4, true),
+    V32(2, 256, 2, false, 4, true),
 };
 constexpr int NVAR32 = (int)(sizeof(g_variants32) / sizeof(g_variants32[0]));
 bool g_attr32[NVAR32] = {};
@@ -313,6 +277,7 @@ const Variant32& variant32(int v)
 }  // namespace
 
 int kick32_num_variants() { return NVAR32; }
+bool kick32_variant_scaled(int v) { return (v >= 0 && v < NVAR32) ? g_variants32[v].scaled : false; }
 const char* kick32_variant_name(int v) { return (v >= 0 && v < NVAR32) ? g_variants32[v].name : ""; }
 
 int kick32_grid(const Handle* h)

@@ -17,6 +17,44 @@ __device__ __forceinline__ double rsq64h(double a)
     double r; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r;
 }
 
+constexpr double EPS2 = 1.0e-60;   // added to r^2 so that the self pair (d = 0 exactly) contributes 0, not NaN;
+                                   // changes no pair with r > 1e-22 au by even one ulp
+
+// One j-chunk against the I i-bodies of this thread.  SELF: the chunk holds this warp's own slots;
+// the self pair is left out of the smallest-r^2 tracking, so a body's own chunk is flagged only if
+// a DIFFERENT body is near.  mn tracks the high word of r^2 (orders like r^2 >= 0).
+template <int I, int UNR, bool SELF>
+__device__ __forceinline__ void pair_loop(const double4* __restrict__ jp, const double (&xi)[I], const double (&yi)[I],
+                                          const double (&zi)[I], double (&ax)[I], double (&ay)[I], double (&az)[I],
+                                          int (&mn)[I], const int (&self_off)[I])
+{
+#pragma unroll UNR
+    for (int jj = 0; jj < CHUNK; ++jj) {
+        const double4 J = jp[jj];
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const double dx = J.x - xi[k];
+            const double dy = J.y - yi[k];
+            const double dz = J.z - zi[k];
+            double r2 = SELF ? fma(dx, dx, EPS2) : dx * dx;
+            r2 = fma(dy, dy, r2);
+            r2 = fma(dz, dz, r2);
+            if (SELF) mn[k] = min(mn[k], (jj == self_off[k]) ? 0x7fffffff : __double2hiint(r2));
+            else      mn[k] = min(mn[k], __double2hiint(r2));
+            const double y0 = rsq64h(r2);
+            const double t  = y0 * y0;
+            const double e  = fma(-r2, t, 1.0);
+            const double c  = fma(1.875, e, 1.5);
+            const double q  = (J.w * y0) * t;
+            const double qe = q * e;
+            const double s  = fma(qe, c, q);
+            ax[k] = fma(s, dx, ax[k]);
+            ay[k] = fma(s, dy, ay[k]);
+            az[k] = fma(s, dz, az[k]);
+        }
+    }
+}
+
 template <int I, int NT>
 struct __align__(16) Smem64 {
     double4  j[NSTAGE][STAGE_J];                 // (x, y, z, G m), 32 B per body
@@ -93,30 +131,15 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                 for (int k = 0; k < I; ++k) { ax[k] = 0.0; ay[k] = 0.0; az[k] = 0.0; mn[k] = 0x7fffffff; }
 
                 const double4* jp = &sm.j[b][ch * CHUNK];
-#pragma unroll UNR
-                for (int jj = 0; jj < CHUNK; ++jj) {
-                    const double4 J = jp[jj];
+                int self_off[I];                  // offset of each own slot inside this chunk (warp-uniform range test)
+                bool self = false;
 #pragma unroll
-                    for (int k = 0; k < I; ++k) {
-                        const double dx = J.x - xi[k];
-                        const double dy = J.y - yi[k];
-                        const double dz = J.z - zi[k];
-                        double r2 = dx * dx;
-                        r2 = fma(dy, dy, r2);
-                        r2 = fma(dz, dz, r2);
-                        mn[k] = min(mn[k], __double2hiint(r2));
-                        const double y0 = rsq64h(r2);
-                        const double t  = y0 * y0;
-                        const double e  = fma(-r2, t, 1.0);
-                        const double c  = fma(1.875, e, 1.5);
-                        const double q  = (J.w * y0) * t;
-                        const double qe = q * e;
-                        const double s  = fma(qe, c, q);
-                        ax[k] = fma(s, dx, ax[k]);
-                        ay[k] = fma(s, dy, ay[k]);
-                        az[k] = fma(s, dz, az[k]);
-                    }
+                for (int k = 0; k < I; ++k) {
+                    self_off[k] = ib * BI + k * NT + tid - (cs + ch) * CHUNK;
+                    self = self || (self_off[k] >= 0 && self_off[k] < CHUNK);
                 }
+                if (self) pair_loop<I, UNR, true>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
+                else      pair_loop<I, UNR, false>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
 
 #pragma unroll
                 for (int k = 0; k < I; ++k) {
@@ -159,21 +182,12 @@ struct Variant64 { kick64_fn fn; int nt; int bi; size_t smem; const char* name; 
     { kick64_kernel<I_, NT_, MINB_, UNR_>, NT_, I_ * NT_, sizeof(Smem64<I_, NT_>), "I" #I_ " NT" #NT_ " minB" #MINB_ " unr" #UNR_ }
 
 const Variant64 g_variants64[] = {
-    V64(2, 256, 2, 4),            // 0: default
-    V64(4, 128, 4, 2),
+    V64(2, 256, 1, 4),            // 0: default
+    V64(2, 256, 2, 4),
     V64(2, 256, 2, 8),
-    V64(2, 256, 1, 4),
-    V64(2, 128, 4, 4),
     V64(2, 128, 3, 4),
-    V64(2, 128, 4, 8),
-    V64(1, 512, 2, 4),
-    V64(1, 512, 2, 8),
-    V64(1, 256, 4, 8),
     V64(1, 256, 3, 8),
-    V64(1, 128, 8, 8),
-    V64(4, 128, 3, 4),
     V64(4, 64, 6, 2),
-    V64(2, 64, 8, 4),
 };
 constexpr int NVAR64 = (int)(sizeof(g_variants64) / sizeof(g_variants64[0]));
 bool g_attr64[NVAR64] = {};

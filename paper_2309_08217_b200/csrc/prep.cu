@@ -115,7 +115,7 @@ ranksort_kernel(int N, int NP, const unsigned long long* __restrict__ keys, int*
 __global__ void __launch_bounds__(PREP_NT)
 prep_kernel(PrepArgs A, Workspace w)
 {
-    __shared__ unsigned int smax[PREP_NT / 32][4];
+    __shared__ unsigned int smax[PREP_NT / 32][5];
     __shared__ double sorg[PREP_NT / CHUNK][3];
     const int s = blockIdx.x * PREP_NT + threadIdx.x;      // slot; grid covers NP exactly (NP % 512 == 0)
     const bool live = s < A.N;
@@ -179,10 +179,25 @@ prep_kernel(PrepArgs A, Workspace w)
         rad = __double2float_ru(sqrt(qx * qx + qy * qy + qz * qz) * (1.0 + 1.0e-9));
         if (!(rad >= 0.f)) rad = 3.0e38f;
     }
+    // FP32 j-record.  Plain form: (x - o, G m).  Mass-scaled form (A.scaled): (q (x - o), q) with
+    // q = (G m)^(-1/2), so that D = q (x_j - x_i) gives G m d / r^3 = D / |D|^3 without a multiply by
+    // G m.  Bodies without (usable) mass and padding get a far-away dummy (1e18, 0, 0 | 0): their
+    // term underflows to exactly 0; a chunk holding a live massless body is always flagged (below).
+    const bool massive = live && (gm >= 1.0e-30) && (gm <= 1.0e30);
+    float q2 = 0.f;
     {
         float* f = reinterpret_cast<float*>(w.pk32) + 8 * (s >> 1) + (s & 1);
-        f[0] = (float)qx; f[2] = (float)qy; f[4] = (float)qz; f[6] = (float)gm;
+        if (!A.scaled) {
+            f[0] = (float)qx; f[2] = (float)qy; f[4] = (float)qz; f[6] = (float)gm;
+        } else if (massive) {
+            const double q = rsqrt(gm);
+            f[0] = (float)(q * qx); f[2] = (float)(q * qy); f[4] = (float)(q * qz); f[6] = (float)q;
+            q2 = __double2float_ru(q * q * (1.0 + 1.0e-6));
+        } else {
+            f[0] = 1.0e18f; f[2] = 0.f; f[4] = 0.f; f[6] = 0.f;
+        }
     }
+    const float rfc = (A.scaled && live && !massive) ? 3.0e38f : rf;   // massless j: (i, this chunk) always FP64
     BoundP b; b.hq = hq; b.aq = aq; b.rf = rf; b.pad = live ? 1.f : 0.f;
     w.bi[s] = b;
 
@@ -190,21 +205,25 @@ prep_kernel(PrepArgs A, Workspace w)
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned int m0 = warp_max_u32(__float_as_uint(hq));
     unsigned int m1 = warp_max_u32(__float_as_uint(aq));
-    unsigned int m2 = warp_max_u32(__float_as_uint(rf));
+    unsigned int m2 = warp_max_u32(__float_as_uint(rfc));
     unsigned int m3 = warp_max_u32(__float_as_uint(rad));
-    if (lane == 0) { smax[wid][0] = m0; smax[wid][1] = m1; smax[wid][2] = m2; smax[wid][3] = m3; }
+    unsigned int m4 = warp_max_u32(__float_as_uint(q2));
+    if (lane == 0) { smax[wid][0] = m0; smax[wid][1] = m1; smax[wid][2] = m2; smax[wid][3] = m3; smax[wid][4] = m4; }
     __syncthreads();
     if (threadIdx.x < PREP_NT / CHUNK) {
         const int c = threadIdx.x;
         ChunkP q;
-        q.hq  = __uint_as_float(max(smax[2 * c][0], smax[2 * c + 1][0]));
-        q.aq  = __uint_as_float(max(smax[2 * c][1], smax[2 * c + 1][1]));
-        q.rad = __uint_as_float(max(smax[2 * c][3], smax[2 * c + 1][3]));
+        unsigned int mx[5] = {0u, 0u, 0u, 0u, 0u};
+        for (int ww = 0; ww < CHUNK / 32; ++ww)
+            for (int t = 0; t < 5; ++t) mx[t] = max(mx[t], smax[c * (CHUNK / 32) + ww][t]);
+        q.hq  = __uint_as_float(mx[0]);
+        q.aq  = __uint_as_float(mx[1]);
+        q.rad = __uint_as_float(mx[3]);
         // frame guard: pairs closer than floor * 2 R_chunk go to FP64 (relative rounding error of
         // the FP32 separation <= 2^-24 (1 + 2 R_chunk / r))
-        q.rf  = fmaxf(__uint_as_float(max(smax[2 * c][2], smax[2 * c + 1][2])),
-                      __fmul_ru(__fmul_ru(2.0f * A.floor_rel, q.rad), 1.000001f));
-        q.pad_ = 0.0;
+        q.rf  = fmaxf(__uint_as_float(mx[2]), __fmul_ru(__fmul_ru(2.0f * A.floor_rel, q.rad), 1.000001f));
+        q.q2max = A.scaled ? __uint_as_float(mx[4]) : 1.0f;   // scales the bound to the kernel's r'^2 = q^2 r^2
+        q.pad_ = 0.f;
         q.ox = sorg[c][0]; q.oy = sorg[c][1]; q.oz = sorg[c][2];
         w.bc[blockIdx.x * (PREP_NT / CHUNK) + c] = q;
     }

@@ -282,3 +282,50 @@ def test_full_size_c4_kick_both_precisions():
     assert np.median(e32) <= 1e-5 and e32.max() <= 1e-4, (np.median(e32), e32.max())
     assert pair_set(p64) == pair_set(po) == pair_set(p32)
     assert not st64.overflowed and not st32.overflowed
+
+
+def _variant_cases():
+    B.load()
+    return [(0, v) for v in range(B.num_variants(0))] + [(1, v) for v in range(B.num_variants(1))]
+
+
+def test_every_kernel_variant_matches_the_oracle():
+    # genga_set_tuning only changes the launch/tiling variant (and, for the mass-scaled FP32
+    # variants, the j-record form): every variant must meet the same gates.  Config 2 has a mass
+    # spectrum (embryos + planetesimals); two test particles (m = 0) and a coincident pair are added.
+    w = W.config(2, 1700)
+    w.m[5] = 0.0
+    w.m[1203] = 0.0
+    w.x[900] = w.x[899]
+    ao, po, _ = oracle_accel(w)
+    for key, v in _variant_cases():
+        g = B.from_workload(w)
+        g.set_tuning(key, v)
+        prec = B.FP32 if key == 0 else B.FP64
+        g.accel(prec)
+        a = g.get_accel().cpu().numpy()
+        pairs = g.encounter_pairs()
+        g.close()
+        assert np.all(np.isfinite(a)), (key, v)
+        err = rel_err(a, ao)
+        if prec == B.FP64:
+            assert err.max() <= 1e-12, (key, v, err.max())
+        else:
+            assert np.median(err) <= 1e-5 and err.max() <= 1e-4, (key, v, np.median(err), err.max())
+        assert pair_set(pairs) == pair_set(po), (key, v)
+
+
+def test_autotune_picks_a_variant_and_keeps_the_state():
+    w = W.config(0, 3000)
+    g = B.from_workload(w)
+    x0, v0 = (t.clone() for t in g.get_state())
+    for prec in (B.FP32, B.FP64):
+        v, ms = g.autotune(prec)
+        assert 0 <= v < B.num_variants(0 if prec == B.FP32 else 1) and ms > 0
+    x1, v1 = g.get_state()
+    assert bool((x0 == x1).all()) and bool((v0 == v1).all())
+    ao, po, _ = oracle_accel(w)
+    g.accel(B.FP32)
+    assert rel_err(g.get_accel().cpu().numpy(), ao).max() <= 1e-4
+    assert pair_set(g.encounter_pairs()) == pair_set(po)
+    g.close()
