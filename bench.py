@@ -123,6 +123,20 @@ def make_workload(args, rank):
     return w
 
 
+def max_over_ranks(torch, dist, values, device):
+    """Every rank times its own system; the job's time is the slowest rank's (one all-reduce(MAX) of
+    the timed totals, after the timed region -- the data path itself has no collective)."""
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def whole_job_rate(world, units_per_rank_step, steps, total_ms):
+    """Units all ranks processed / the max-over-ranks time (weak scaling: fixed work per rank)."""
+    return world * units_per_rank_step * steps / (total_ms * 1e-3)
+
+
 def time_steps(torch, g, w, prec, steps, warmup, flush_buf, dist):
     """K timed steps, each bracketed by CUDA events on the handle's stream; L2 flushed between."""
     stream = torch.cuda.current_stream()
@@ -289,11 +303,8 @@ def run_cuda(args):
         g.close()
 
     # max over ranks of the timed totals
-    tot = torch.tensor([res["fp32"]["total_ms"], res["fp64"]["total_ms"], e2e["fp32"][0], e2e["fp64"][0]],
-                       dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
-    t32, t64, te32, te64 = (float(t) for t in tot.tolist())
+    t32, t64, te32, te64 = max_over_ranks(torch, dist, [res["fp32"]["total_ms"], res["fp64"]["total_ms"],
+                                                        e2e["fp32"][0], e2e["fp64"][0]], dev)
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -302,7 +313,7 @@ def run_cuda(args):
     K = args.steps
     def per_prec(name, total_ms, flop, peak):
         r = res[name]
-        pps = world * pairs * K / (total_ms * 1e-3)
+        pps = whole_job_rate(world, pairs, K, total_ms)
         kick_ms = r["kernel_ms"][0]
         tf = flop * pairs / (kick_ms * 1e-3) / 1e12
         return {"pair_interactions_per_s": pps, "steps_per_s": K / (total_ms * 1e-3),
@@ -338,9 +349,9 @@ def run_cuda(args):
                      "fp64": {"kernel": "kick64_kernel", "achieved": p64["kick_kernel_tflops"],
                               "peak": PEAK_FP64_TFLOPS, "frac": p64["kick_kernel_frac_of_peak"],
                               "flop_per_pair": FLOP_FP64}},
-        "e2e": {"value": world * pairs * e2e_steps / (te32 * 1e-3), "unit": UNIT,
+        "e2e": {"value": whole_job_rate(world, pairs, e2e_steps, te32), "unit": UNIT,
                 "h2d_bytes_per_step": e2e["fp32"][1], "d2h_bytes_per_step": e2e["fp32"][2], "steps": e2e_steps,
-                "fp64_value": world * pairs * e2e_steps / (te64 * 1e-3)},
+                "fp64_value": whole_job_rate(world, pairs, e2e_steps, te64)},
         "gpu_launches": res["fp32"]["launches"],
         "clocks": sampler.summary(),
     }
