@@ -45,6 +45,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_red = take((size_t)RED_DOUBLES * 8), o_vt = take(NP * 24), o_ctr = take(sizeof(Counters));
     const size_t o_ord = take(NP * 4), o_key = take(NP * 8), o_aux = take(NP * 32);
     const size_t o_mom = take((8 + 4 * (NP / 128 + 1)) * 8);
+    const size_t o_bk = take(NP * 8), o_sb = take((size_t)sort_buffer_words() * 4);
     if (w && base) {
         char* b = static_cast<char*>(base);
         w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
@@ -55,6 +56,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
         w->ctr = (Counters*)(b + o_ctr);
         w->order = (int*)(b + o_ord); w->keys = (unsigned long long*)(b + o_key); w->aux = (double4*)(b + o_aux);
         w->mom = (double*)(b + o_mom);
+        w->bkeys = (unsigned long long*)(b + o_bk); w->sortbuf = (unsigned int*)(b + o_sb);
     }
     return off;
 }
@@ -94,7 +96,7 @@ static int resort(Handle* h)
 {
     if (h->N == 0) return GENGA_OK;
     launch_momentum(h); LAUNCHED(h, "momentum_kernel");     // red[3] = sum m (mean mass -> heavy class)
-    launch_sort(h); h->launches += 3;
+    launch_sort(h); h->launches += 5;
     { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_, "sort kernels"); }
     h->evals_since_sort = 0;
     return GENGA_OK;

@@ -12,7 +12,7 @@ namespace genga {
 
 // ---- tiling constants -------------------------------------------------
 constexpr int CHUNK      = 128;                 // j-bodies per chunk: granularity of the near-field flag
-constexpr int STAGE_CH   = 4;                  // chunks per shared-memory stage
+constexpr int STAGE_CH   = 8;                  // chunks per shared-memory stage
 constexpr int STAGE_J    = CHUNK * STAGE_CH;    // 512 j-bodies per stage
 constexpr int NSTAGE     = 2;                   // double buffering
 constexpr int PAD_BODIES = 512;                 // N is padded to a multiple of this (stage and i-block size)
@@ -54,7 +54,9 @@ struct Workspace {
     double* vkep;     // [NP]
     // arrays of one force evaluation, in the INTERNAL (sorted) order: slot s holds body order[s]
     int*     order;   // [NP]   slot -> body index (API order); order[s] = s for the padding slots s >= N
-    unsigned long long* keys;   // [NP] sort keys (heavy class, semi-major axis, body index)
+    unsigned long long* keys;   // [NP] sort keys (heavy class, Hilbert index, body index)
+    unsigned long long* bkeys;  // [NP] the keys grouped by bucket
+    unsigned int* sortbuf;      // bucket histogram, starts and cursors of the sort
     double4* pk64;    // [NP]   (x, y, z, G m)
     float4*  pk32;    // [NP]   pair-interleaved, see above
     double4* aux;     // [NP]   (m, r_crit, a, v_K): what the exact pair rule O3 needs
@@ -111,6 +113,7 @@ struct PrepArgs {
 };
 void launch_hcbrt(const Handle* h);
 void launch_pad(const Handle* h);                            // padding bodies: x = (PAD_POS,0,0), v = 0, m = 0
+int  sort_buffer_words();
 void launch_sort(const Handle* h);                           // order[] by (heavy class, semi-major axis)
 void launch_prep(const Handle* h, const PrepArgs& a);
 void launch_kick32(const Handle* h);

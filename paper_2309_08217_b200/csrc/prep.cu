@@ -40,7 +40,10 @@ __device__ __forceinline__ unsigned int warp_max_u32(unsigned int v)
 // the mean first (their large r_crit then stays in a few chunks), then along a Hilbert curve over
 // the x-y plane (the discs are thin).  The order is a performance hint only: every bound is
 // computed from the actual chunk contents, so results never depend on it beyond summation order.
-// key = [light:1][Hilbert index:31][body index:32]: distinct keys, so ranks are a permutation.
+// key = [light:1][Hilbert index:30][0][body index:32]: distinct keys, so ranks are a permutation.
+constexpr int SORT_BITS = 13;                       // buckets = leading key bits: class + 12 Hilbert bits
+constexpr int SORT_NB   = 1 << SORT_BITS;
+
 __global__ void extent_kernel(int N, const double* __restrict__ x, unsigned int* __restrict__ extent_bits)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -71,7 +74,8 @@ __device__ __forceinline__ unsigned int hilbert_xy2d(unsigned int cx, unsigned i
 
 __global__ void sortkey_kernel(int N, double M_star, const double* __restrict__ x,
                                const double* __restrict__ hcbrt, const double* __restrict__ red,
-                               const unsigned int* __restrict__ extent_bits, unsigned long long* __restrict__ keys)
+                               const unsigned int* __restrict__ extent_bits, unsigned long long* __restrict__ keys,
+                               unsigned int* __restrict__ hist)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -82,32 +86,61 @@ __global__ void sortkey_kernel(int N, double M_star, const double* __restrict__ 
     const unsigned int cx = (fx == fx) ? (unsigned int)fx : 0u, cy = (fy == fy) ? (unsigned int)fy : 0u;
     const double href = cbrt(red[3] / ((double)N * 3.0 * M_star));      // Hill factor of the mean mass
     const unsigned long long light = (hcbrt[i] > 1.5 * href) ? 0ull : 1ull;
-    keys[i] = (light << 63) | ((unsigned long long)hilbert_xy2d(cx, cy) << 32) | (unsigned int)i;
+    const unsigned long long key = (light << 63) | ((unsigned long long)hilbert_xy2d(cx, cy) << 33) | (unsigned int)i;
+    keys[i] = key;
+    atomicAdd(&hist[(unsigned int)(key >> (64 - SORT_BITS))], 1u);
 }
 
-// Rank sort: order[#{j : key_j < key_i}] = i.  O(N^2) integer compares, but it runs only when
-// the order is refreshed (every resort_every force evaluations), never per step.
-constexpr int RANK_NT = 256;
-__global__ void __launch_bounds__(RANK_NT)
-ranksort_kernel(int N, int NP, const unsigned long long* __restrict__ keys, int* __restrict__ order)
+// Bucket sort on the leading SORT_BITS key bits, then exact ranks inside each bucket:
+//   hist (in sortkey_kernel) -> exclusive scan -> scatter into buckets (any order) -> rank of every
+//   key among the keys of its own bucket.  Keys are distinct, so the result is the exact sorted
+//   order whatever order the atomics ran in.  O(N) plus O(bucket size) per body.
+__global__ void __launch_bounds__(1024)
+sortscan_kernel(const unsigned int* __restrict__ hist, unsigned int* __restrict__ start, unsigned int* __restrict__ cursor)
 {
-    __shared__ unsigned long long sk[RANK_NT * 4];
-    const int i = blockIdx.x * RANK_NT + threadIdx.x;
-    const unsigned long long ki = (i < N) ? keys[i] : 0ull;
-    int rank = 0;
-    for (int base = 0; base < N; base += RANK_NT * 4) {
-        __syncthreads();
+    __shared__ unsigned int wsum[32];
+    constexpr int PER = SORT_NB / 1024;
+    unsigned int v[PER], tot = 0;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int j = base + q * RANK_NT + threadIdx.x;
-            sk[q * RANK_NT + threadIdx.x] = (j < N) ? keys[j] : ~0ull;
-        }
-        __syncthreads();
-#pragma unroll 8
-        for (int jj = 0; jj < RANK_NT * 4; ++jj) rank += (sk[jj] < ki) ? 1 : 0;
+    for (int k = 0; k < PER; ++k) { v[k] = hist[threadIdx.x * PER + k]; tot += v[k]; }
+    unsigned int inc = tot;                                      // inclusive scan over threads
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        unsigned int w = wsum[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, w, o); if (lane >= o) w += t; }
+        wsum[lane] = w;
     }
-    if (i < N) order[rank] = i;
-    else if (i < NP) order[i] = i;
+    __syncthreads();
+    unsigned int base = inc - tot + (wid ? wsum[wid - 1] : 0u);
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { start[threadIdx.x * PER + k] = base; cursor[threadIdx.x * PER + k] = base; base += v[k]; }
+}
+
+__global__ void sortscatter_kernel(int N, const unsigned long long* __restrict__ keys, unsigned int* __restrict__ cursor,
+                                   unsigned long long* __restrict__ bkeys)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const unsigned long long key = keys[i];
+    bkeys[atomicAdd(&cursor[(unsigned int)(key >> (64 - SORT_BITS))], 1u)] = key;
+}
+
+__global__ void sortrank_kernel(int N, int NP, const unsigned long long* __restrict__ bkeys,
+                                const unsigned int* __restrict__ start, int* __restrict__ order)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= N) { if (p < NP) order[p] = p; return; }
+    const unsigned long long key = bkeys[p];
+    const unsigned int b = (unsigned int)(key >> (64 - SORT_BITS));
+    const unsigned int s = start[b], e = (b + 1 < SORT_NB) ? start[b + 1] : (unsigned int)N;
+    unsigned int rank = 0;
+    for (unsigned int q = s; q < e; ++q) rank += (bkeys[q] < key) ? 1u : 0u;
+    order[s + rank] = (int)(unsigned int)(key & 0xffffffffull);
 }
 
 // One thread per (padded) body.  Eq. 1:  r_crit,i = max(n1 R_H,i, n2 dt v_i), R_H,i = a_i (m_i/3M)^(1/3);
@@ -309,12 +342,19 @@ void launch_pad(const Handle* h)
 void launch_sort(const Handle* h)
 {
     if (h->N == 0) return;
+    unsigned int* hist = h->w.sortbuf, *start = hist + SORT_NB, *cursor = start + SORT_NB;
     cudaMemsetAsync(&h->w.ctr->extent_bits, 0, sizeof(unsigned int), h->stream);
-    extent_kernel<<<(h->N + 255) / 256, 256, 0, h->stream>>>(h->N, h->w.x, &h->w.ctr->extent_bits);
-    sortkey_kernel<<<(h->N + 255) / 256, 256, 0, h->stream>>>(h->N, h->p.M_star, h->w.x, h->w.hcbrt, h->w.red,
-                                                              &h->w.ctr->extent_bits, h->w.keys);
-    ranksort_kernel<<<h->NP / RANK_NT, RANK_NT, 0, h->stream>>>(h->N, h->NP, h->w.keys, h->w.order);
+    cudaMemsetAsync(hist, 0, SORT_NB * sizeof(unsigned int), h->stream);
+    const int nb = (h->N + 255) / 256;
+    extent_kernel<<<nb, 256, 0, h->stream>>>(h->N, h->w.x, &h->w.ctr->extent_bits);
+    sortkey_kernel<<<nb, 256, 0, h->stream>>>(h->N, h->p.M_star, h->w.x, h->w.hcbrt, h->w.red,
+                                              &h->w.ctr->extent_bits, h->w.keys, hist);
+    sortscan_kernel<<<1, 1024, 0, h->stream>>>(hist, start, cursor);
+    sortscatter_kernel<<<nb, 256, 0, h->stream>>>(h->N, h->w.keys, cursor, h->w.bkeys);
+    sortrank_kernel<<<h->NP / 256, 256, 0, h->stream>>>(h->N, h->NP, h->w.bkeys, start, h->w.order);
 }
+
+int sort_buffer_words() { return 3 * SORT_NB; }
 
 void launch_prep(const Handle* h, const PrepArgs& a)
 {
