@@ -118,7 +118,11 @@ static int force_eval(Handle* h, int precision, double preshift = 0.0)
     a.pair_rule = h->p.pair_rule;
     a.preshift = preshift;
     a.scaled = (precision == GENGA_FP32 && kick32_variant_scaled(h->tune[0])) ? 1 : 0;
-    if (precision == GENGA_FP32) { a.lambda = (float)h->lambda_near; a.floor_rel = (float)h->near_floor; }
+    if (precision == GENGA_FP32) {
+        a.lambda = (float)h->lambda_near;
+        // never below 2^-18: closer pairs have no meaning in FP32 (and mass-scaled self/coincident residues stay flagged)
+        a.floor_rel = (float)(h->near_floor > 3.814697265625e-06 ? h->near_floor : 3.814697265625e-06);
+    }
     else                         { a.lambda = 1.0f;                  a.floor_rel = 0.0f; }
     { ProfScope ps(h, 2); launch_prep(h, a); }
     LAUNCHED(h, "prep_kernel");
