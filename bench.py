@@ -50,6 +50,9 @@ def parse_args():
     ap.add_argument("--sweep", action="store_true", help="also run the N = 2^10..2^17 sweep (extra JSON key)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed steps")
+    ap.add_argument("--report", action="store_true",
+                    help="run every BASELINE.json config (0-4) for its full step count in both precisions and print one "
+                         "JSON line per (config, precision): rates, fractions of peak, dE/E, dL/L, encounter counts")
     ap.add_argument("--no-autotune", action="store_true", help="keep the default kernel variants (no start-up self-tuning)")
     return ap.parse_args()
 
@@ -393,10 +396,68 @@ def run_sweep(args):
     return out
 
 
+def run_report(args):
+    """north_star: 'Report pair interactions/s and steps/s per body at each config ... relative energy and
+    angular-momentum drift over the run: reported for both precisions' (+ encounter pairs per step, config 1)."""
+    import numpy as np
+    import torch
+    from paper_2309_08217_b200 import binding as B
+    from paper_2309_08217_b200 import workloads as W
+    B.load()
+    for cfg in range(5):
+        w = W.config(cfg)
+        pairs = w.N * (w.N - 1.0)
+        for prec, name, flop, peak in ((B.FP32, "fp32", FLOP_FP32, PEAK_FP32_TFLOPS), (B.FP64, "fp64", FLOP_FP64, PEAK_FP64_TFLOPS)):
+            g = B.from_workload(w)
+            variant = 0 if args.no_autotune else g.autotune(prec)[0]
+            E0, L0 = g.energy_angmom()
+            g.run(w.dt, 3, prec)                                   # warm-up (3 steps of the same trajectory)
+            g.close()
+            g = B.from_workload(w)
+            g.set_tuning(0 if prec == B.FP32 else 1, variant)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            g.run(w.dt, w.nsteps, prec)                            # K(dt/2) [S D S K(dt)]^(n-1) S D S K(dt/2)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            E1, L1 = g.energy_angmom()
+            enc_last = int(len(g.encounter_pairs(cap=8 * w.N + 4096)))
+            st = g.nearfield_stats()
+            g.close()
+            evals = w.nsteps + 1
+            line = {"report": "config", "config": cfg, "workload": w.name, "N": w.N, "dt_days": w.dt, "steps": w.nsteps,
+                    "precision": name, "kernel_variant": B.variant_name(0 if prec == B.FP32 else 1, variant),
+                    "ms_per_step": ms / w.nsteps, "steps_per_s": w.nsteps / (ms * 1e-3),
+                    "body_steps_per_s": w.N * w.nsteps / (ms * 1e-3),
+                    "pair_interactions_per_s": pairs * evals / (ms * 1e-3),
+                    "step_frac_of_peak": flop * pairs * evals / (ms * 1e-3) / 1e12 / peak,
+                    "dE_over_E": E1 / E0 - 1.0,
+                    "dL_over_L": float(np.linalg.norm(L1) / np.linalg.norm(L0) - 1.0),
+                    "encounter_pairs_last_eval": enc_last, "nearfield_candidates_last_eval": st.candidates}
+            if cfg == 1:                                           # encounter-pair counts per step (untimed second run)
+                g = B.from_workload(w)
+                g.set_tuning(0 if prec == B.FP32 else 1, variant)
+                g.kick(0.5 * w.dt, prec)
+                counts = []
+                for _ in range(w.nsteps):
+                    g.leapfrog(w.dt, 1, prec)
+                    counts.append(len(g.encounter_pairs(cap=8 * w.N + 4096)))
+                g.close()
+                c = np.array(counts)
+                line["encounter_pairs_per_step"] = {"mean": float(c.mean()), "min": int(c.min()), "max": int(c.max()),
+                                                    "first": int(c[0]), "last": int(c[-1])}
+            print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.report:
+        run_report(args)
         return
     got = run_cuda(args)
     if got is None:

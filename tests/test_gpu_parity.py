@@ -329,3 +329,18 @@ def test_autotune_picks_a_variant_and_keeps_the_state():
     assert rel_err(g.get_accel().cpu().numpy(), ao).max() <= 1e-4
     assert pair_set(g.encounter_pairs()) == pair_set(po)
     g.close()
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_full_size_configs_1_to_3_kick_both_precisions(cfg):
+    # BASELINE.json configs 1-3 at their full sizes (6600, 8100, 10004 bodies)
+    w = W.config(cfg)
+    ao, po, rco = oracle_accel(w)
+    a64, p64, rc, st64 = gpu_accel(w, B.FP64)
+    a32, p32, _, st32 = gpu_accel(w, B.FP32)
+    assert np.max(np.abs(rc / rco - 1)) <= 1e-14
+    assert rel_err(a64, ao).max() <= 1e-12
+    e32 = rel_err(a32, ao)
+    assert np.median(e32) <= 1e-5 and e32.max() <= 1e-4, (np.median(e32), e32.max())
+    assert pair_set(p64) == pair_set(po) == pair_set(p32)
+    assert not st64.overflowed and not st32.overflowed
