@@ -85,6 +85,9 @@ typedef struct {
     int    resort_every;      /* force evaluations between two refreshes of the internal body order
                                  (heavy bodies first, then along a Hilbert curve in the x-y plane; a
                                  performance hint only).  <= 0 selects the default (32).              */
+    int    no_fused_step;     /* 1: genga_kick/step/run/leapfrog use the separate per-body kernels instead of the
+                                 one cooperative kernel per step (debugging; also taken if the device lacks
+                                 cooperative launch)                                                   */
 } genga_params;
 
 /* Fill *p with the defaults: G = k^2 (k = 0.01720209895), M_star = 1, n1 = 3, n2 = 0,
@@ -131,7 +134,7 @@ int genga_run(genga_handle h, double dt, int nsteps, int precision);
 
 /* The body of that loop on its own: [S(dt/2) D(dt) S(dt/2) K(dt)]^nsteps, one force evaluation
  * per step.  genga_kick(dt/2), genga_leapfrog(n), genga_kick(-dt/2) equals genga_run(n) up to
- * rounding while r_crit does not depend on v (n2 = 0).                                          */
+ * rounding as long as no pair sits inside a changeover zone (r_crit depends on v through a_i).   */
 int genga_leapfrog(genga_handle h, double dt, int nsteps, int precision);
 
 /* Encounter pairs {(i,j): i < j, r_ij < r_crit,ij} of the LAST force evaluation.

@@ -44,7 +44,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_cand = take((size_t)cand_cap * 8), o_pairs = take((size_t)pair_cap * 8);
     const size_t o_red = take((size_t)RED_DOUBLES * 8), o_vt = take(NP * 24), o_ctr = take(sizeof(Counters));
     const size_t o_ord = take(NP * 4), o_key = take(NP * 8), o_aux = take(NP * 32);
-    const size_t o_mom = take((8 + 4 * (NP / 128 + 1)) * 8);
+    const size_t o_mom = take((8 + 4 * (NP / 128 + 1) + 8 * (size_t)MOM_MAX_BLOCKS) * 8);
     const size_t o_bk = take(NP * 8), o_sb = take((size_t)sort_buffer_words() * 4);
     if (w && base) {
         char* b = static_cast<char*>(base);
@@ -103,15 +103,18 @@ static int resort(Handle* h)
 }
 
 // ---- force evaluation -------------------------------------------------------------------------
-static int force_eval(Handle* h, int precision, double preshift = 0.0)
+static int maybe_resort(Handle* h)
 {
-    if (precision != GENGA_FP64 && precision != GENGA_FP32) return GENGA_EINVAL;
-    if (h->N == 0) return GENGA_OK;
     if (h->evals_since_sort < 0 || h->evals_since_sort >= h->resort_every) {
         const int rc = resort(h);
         if (rc != GENGA_OK) return rc;
     }
     ++h->evals_since_sort;
+    return GENGA_OK;
+}
+
+static PrepArgs make_prep_args(const Handle* h, int precision, double preshift)
+{
     PrepArgs a;
     a.N = h->N; a.NP = h->NP;
     a.G = h->p.G; a.M_star = h->p.M_star; a.n1 = h->p.n1; a.n2 = h->p.n2; a.dt_rcrit = h->p.dt_rcrit;
@@ -124,12 +127,48 @@ static int force_eval(Handle* h, int precision, double preshift = 0.0)
         a.floor_rel = (float)(h->near_floor > 3.814697265625e-06 ? h->near_floor : 3.814697265625e-06);
     }
     else                         { a.lambda = 1.0f;                  a.floor_rel = 0.0f; }
-    { ProfScope ps(h, 2); launch_prep(h, a); }
-    LAUNCHED(h, "prep_kernel");
+    return a;
+}
+
+// all-pairs kernel + near-field kernel on the arrays the prep step packed
+static int launch_pairs(Handle* h, int precision)
+{
     { ProfScope ps(h, 0); if (precision == GENGA_FP32) launch_kick32(h); else launch_kick64(h); }
     LAUNCHED(h, "kick_kernel");
     { ProfScope ps(h, 1); launch_nearfield(h); }
     LAUNCHED(h, "nearfield_kernel");
+    return GENGA_OK;
+}
+
+static int force_eval(Handle* h, int precision, double preshift = 0.0)
+{
+    if (precision != GENGA_FP64 && precision != GENGA_FP32) return GENGA_EINVAL;
+    if (h->N == 0) return GENGA_OK;
+    const int rc = maybe_resort(h);
+    if (rc != GENGA_OK) return rc;
+    const PrepArgs a = make_prep_args(h, precision, preshift);
+    { ProfScope ps(h, 2); launch_prep(h, a); }
+    LAUNCHED(h, "prep_kernel");
+    return launch_pairs(h, precision);
+}
+
+// The fused per-body kernel (fused_step.cu): [v += tau_v a] [S(dt/2) D(dt)] [S(dt/2), r_crit, pack].
+static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_drift, double dt, bool do_prep)
+{
+    if (h->N == 0) return GENGA_OK;
+    OnBodyArgs a;
+    if (do_prep) {
+        const int rc = maybe_resort(h);
+        if (rc != GENGA_OK) return rc;
+    }
+    a.prep = make_prep_args(h, precision, 0.0);
+    a.do_vel = do_vel; a.do_drift = do_drift; a.do_prep = do_prep;
+    a.tau_v = tau_v; a.dt = dt; a.mu = h->p.G * h->p.M_star;
+    cudaError_t e;
+    { ProfScope ps(h, do_drift ? 3 : 2); e = launch_onbody(h, a, h->fused_blocks); }
+    ++h->launches;
+    if (e != cudaSuccess) return cuda_fail(e, "onbody_kernel (cooperative launch)");
+    h->mom_a_valid = !do_drift;          // slot A holds sum m v of the stored velocities unless the drift changed them
     return GENGA_OK;
 }
 
@@ -171,6 +210,38 @@ static int sd_fused(genga_handle h, double dt)
     return GENGA_OK;
 }
 
+// K(tau_first)? then n_sds times [S(dt/2) D(dt) S(dt/2) K(tau)], tau = tau_mid except tau_last for the last
+// one.  Fused path: one per-body kernel between two force evaluations (3 launches per step).
+static int sequence(genga_handle h, int precision, bool lead_kick, double tau_first, int n_sds, double dt,
+                    double tau_mid, double tau_last)
+{
+    if (precision != GENGA_FP64 && precision != GENGA_FP32) return GENGA_EINVAL;
+    int rc;
+    if (h->N == 0) return GENGA_OK;
+    if (h->fused_blocks <= 0) {                                     // no cooperative launch: the un-fused kernels
+        if (lead_kick && (rc = kick_fused(h, tau_first, precision, 0.0)) != GENGA_OK) return rc;
+        for (int k = 0; k < n_sds; ++k) {
+            if ((rc = sd_fused(h, dt)) != GENGA_OK) return rc;
+            if ((rc = kick_fused(h, k == n_sds - 1 ? tau_last : tau_mid, precision, 0.5 * dt)) != GENGA_OK) return rc;
+        }
+        return GENGA_OK;
+    }
+    bool pending = false;
+    double tau_prev = 0.0;
+    if (lead_kick) {
+        if ((rc = onbody(h, precision, false, 0.0, false, 0.0, true)) != GENGA_OK) return rc;
+        if ((rc = launch_pairs(h, precision)) != GENGA_OK) return rc;
+        pending = true; tau_prev = tau_first;
+    }
+    for (int k = 0; k < n_sds; ++k) {
+        if ((rc = onbody(h, precision, pending, tau_prev, true, dt, true)) != GENGA_OK) return rc;
+        if ((rc = launch_pairs(h, precision)) != GENGA_OK) return rc;
+        pending = true; tau_prev = (k == n_sds - 1) ? tau_last : tau_mid;
+    }
+    if (pending) return onbody(h, precision, true, tau_prev, false, 0.0, false);
+    return GENGA_OK;
+}
+
 extern "C" {
 
 void genga_default_params(genga_params* p)
@@ -186,6 +257,7 @@ void genga_default_params(genga_params* p)
     p->stream = nullptr; p->workspace = nullptr; p->workspace_bytes = 0;
     p->pair_capacity = 0; p->cand_capacity = 0;
     p->resort_every = 0;
+    p->no_fused_step = 0;
 }
 
 size_t genga_workspace_bytes(int N, const genga_params* p)
@@ -225,6 +297,11 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     h->evals_since_sort = -1;
     h->stream = static_cast<cudaStream_t>(p->stream);
     h->num_sms = sms;
+    {
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        h->fused_blocks = (coop && !p->no_fused_step) ? onbody_max_blocks(h) : 0;
+    }
     carve_workspace(N, pc, cc, p->workspace, &h->w);
 
     cudaError_t e = cudaMemsetAsync(p->workspace, 0, need, h->stream);
@@ -287,7 +364,7 @@ int genga_accel(genga_handle h, int precision)
 int genga_kick(genga_handle h, double dt, int precision)
 {
     if (!h) return GENGA_EINVAL;
-    return kick_fused(h, dt, precision, 0.0);
+    return sequence(h, precision, true, dt, 0, 0.0, 0.0, 0.0);
 }
 
 int genga_drift(genga_handle h, double dt)
@@ -311,32 +388,21 @@ int genga_sunkick(genga_handle h, double tau)
 int genga_step(genga_handle h, double dt, int precision)
 {
     if (!h) return GENGA_EINVAL;
-    int rc;
-    if ((rc = kick_fused(h, 0.5 * dt, precision, 0.0)) != GENGA_OK) return rc;
-    if ((rc = sd_fused(h, dt)) != GENGA_OK) return rc;
-    return kick_fused(h, 0.5 * dt, precision, 0.5 * dt);
+    return sequence(h, precision, true, 0.5 * dt, 1, dt, 0.5 * dt, 0.5 * dt);
 }
 
 int genga_leapfrog(genga_handle h, double dt, int nsteps, int precision)
 {
     if (!h || nsteps < 0) return GENGA_EINVAL;
-    int rc;
-    for (int s = 0; s < nsteps; ++s) {
-        if ((rc = sd_fused(h, dt)) != GENGA_OK) return rc;
-        if ((rc = kick_fused(h, dt, precision, 0.5 * dt)) != GENGA_OK) return rc;
-    }
-    return GENGA_OK;
+    if (nsteps == 0) return GENGA_OK;
+    return sequence(h, precision, false, 0.0, nsteps, dt, dt, dt);
 }
 
 int genga_run(genga_handle h, double dt, int nsteps, int precision)
 {
     if (!h || nsteps < 0) return GENGA_EINVAL;
     if (nsteps == 0) return GENGA_OK;
-    int rc;
-    if ((rc = kick_fused(h, 0.5 * dt, precision, 0.0)) != GENGA_OK) return rc;
-    if ((rc = genga_leapfrog(h, dt, nsteps - 1, precision)) != GENGA_OK) return rc;
-    if ((rc = sd_fused(h, dt)) != GENGA_OK) return rc;
-    return kick_fused(h, 0.5 * dt, precision, 0.5 * dt);
+    return sequence(h, precision, true, 0.5 * dt, nsteps, dt, dt, 0.5 * dt);
 }
 
 int genga_encounter_pairs(genga_handle h, int* pairs_ij, int cap, int* count)

@@ -84,6 +84,7 @@ struct Handle {
     int num_sms;
     long long launches;
     // internal order (a performance hint only: results never depend on it)
+    int fused_blocks;            // co-resident blocks of the fused per-body kernel; 0 = cooperative launch unavailable
     bool mom_a_valid;            // mom[SLOT_A] holds sum m v of the stored velocities
     int tune[4];                 // genga_set_tuning: [0] kick32 variant, [1] kick64 variant
     int resort_every;            // force evaluations between two sorts
@@ -111,6 +112,15 @@ struct PrepArgs {
     int scaled;                  // FP32 j-records in the mass-scaled form (kick_fp32.cu, SC variants)
     double preshift;             // pending Sun-kick: x += preshift * mom[SLOT_B] / M_star before anything else
 };
+struct OnBodyArgs {               // the fused per-body kernel of the step (fused_step.cu)
+    PrepArgs prep;
+    int do_vel, do_drift, do_prep;
+    double tau_v;                  // v += tau_v a          (do_vel)
+    double dt, mu;                 // S(dt/2) D(dt) S(dt/2)  (do_drift; the closing S is applied by phase 3)
+};
+constexpr int MOM_MAX_BLOCKS = 2048;   // most blocks whose momentum partials fit the workspace
+int  onbody_max_blocks(const Handle* h);
+cudaError_t launch_onbody(const Handle* h, const OnBodyArgs& a, int max_blocks);
 void launch_hcbrt(const Handle* h);
 void launch_pad(const Handle* h);                            // padding bodies: x = (PAD_POS,0,0), v = 0, m = 0
 int  sort_buffer_words();

@@ -1,0 +1,140 @@
+// prep_tile.cuh -- rows a1 + a2 of the path for one tile of 256 slots: critical radius (PAPER.md:49-53,
+// Eq. 1), packing of the j-side arrays in the internal order, chunk frames and the conservative
+// near-field bound parameters (DESIGN.md sections 3 and 6).  Shared by prep_kernel and the fused
+// per-body kernel of the step (fused_step.cu).
+#pragma once
+
+#include "genga_internal.cuh"
+
+namespace genga {
+
+constexpr int PREP_NT = 256;
+
+__device__ __forceinline__ unsigned int warp_max_u32(unsigned int v)
+{
+    return __reduce_max_sync(0xffffffffu, v);
+}
+
+// One thread per (padded) body.  Eq. 1:  r_crit,i = max(n1 R_H,i, n2 dt v_i), R_H,i = a_i (m_i/3M)^(1/3);
+// a_i from vis-viva with the stored velocity (readings G2b, G2c); v_i = sqrt(G M / a_i).
+// tile: which run of PREP_NT slots this block handles; (shx, shy, shz): a pending Sun-kick displacement
+// (O8) added to the positions first (and written back) if do_shift.  Must be called by all PREP_NT
+// threads of the block; ends with a __syncthreads, so it can be called in a loop.
+__device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int tile, bool do_shift,
+                                          double shx, double shy, double shz)
+{
+    __shared__ unsigned int smax[PREP_NT / 32][5];
+    __shared__ double sorg[PREP_NT / CHUNK][3];
+    const int s = tile * PREP_NT + threadIdx.x;            // slot; tiles cover NP exactly (NP % 512 == 0)
+    const bool live = s < A.N;
+    const int i = w.order[s];                              // body held by this slot (= s for padding)
+
+    double px = PAD_POS, py = 0.0, pz = 0.0, gm = 0.0;
+    float hq = 0.f, aq = 0.f, rf = 0.f;
+    double4 ax4 = make_double4(0.0, 0.0, 0.0, 0.0);
+    if (live) {
+        const double mu = A.G * A.M_star;
+        px = w.x[3 * i + 0]; py = w.x[3 * i + 1]; pz = w.x[3 * i + 2];
+        if (do_shift) {                                    // pending Sun-kick S(tau) of the fused step (O8)
+            px += shx; py += shy; pz += shz;
+            w.x[3 * i + 0] = px; w.x[3 * i + 1] = py; w.x[3 * i + 2] = pz;
+        }
+        const double vx = w.v[3 * i + 0], vy = w.v[3 * i + 1], vz = w.v[3 * i + 2];
+        const double r  = sqrt(px * px + py * py + pz * pz);
+        const double v2 = vx * vx + vy * vy + vz * vz;
+        double sa = 1.0 / (2.0 / r - v2 / mu);
+        if (!(sa > 0.0) || !isfinite(sa)) sa = r;
+        const double h  = w.hcbrt[i];
+        const double vk = sqrt(mu / sa);
+        const double rc = fmax(A.n1 * (sa * h), A.n2 * A.dt_rcrit * vk);
+        w.rcrit[i] = rc; w.semi[i] = sa; w.vkep[i] = vk;
+        const double mi = w.m[i];
+        gm = A.G * mi;
+        ax4 = make_double4(mi, rc, sa, vk);
+
+        const double lam = (double)A.lambda * (1.0 + 1.0e-6);
+        double dhq, daq, drf;
+        if (A.pair_rule == GENGA_PAIR_MUTUAL_HILL) {
+            dhq = lam * A.n1 * 1.2599210498948732 * h;     // cbrt(2) * h_i bounds cbrt((m_i+m_j)/3M)
+            daq = sa;
+            drf = lam * A.n2 * A.dt_rcrit * vk;
+        } else {
+            dhq = lam * rc;
+            daq = 1.0;
+            drf = 0.0;
+        }
+        hq = __double2float_ru(dhq); aq = __double2float_ru(daq); rf = __double2float_ru(drf);
+        if (!(hq >= 0.f)) hq = 3.0e38f;                     // NaN state: flag everything
+        if (!(aq >= 0.f)) aq = 3.0e38f;
+        if (!(rf >= 0.f)) rf = 3.0e38f;
+    }
+    w.a[3 * i + 0] = 0.0; w.a[3 * i + 1] = 0.0; w.a[3 * i + 2] = 0.0;
+    w.pk64[s] = make_double4(px, py, pz, gm);
+    w.aux[s]  = ax4;
+    // local frame of this slot's chunk: origin = position of the chunk's first slot (FP32 policy P32),
+    // handed over through shared memory (the chunk's 64 slots are two warps of this block)
+    if ((s & (CHUNK - 1)) == 0) {
+        const int c = threadIdx.x / CHUNK;
+        sorg[c][0] = px; sorg[c][1] = py; sorg[c][2] = pz;
+    }
+    __syncthreads();
+    const double ox = sorg[threadIdx.x / CHUNK][0], oy = sorg[threadIdx.x / CHUNK][1], oz = sorg[threadIdx.x / CHUNK][2];
+    const double qx = px - ox, qy = py - oy, qz = pz - oz;
+    float rad = 0.f;                                        // |x - o|, rounded up; padding does not count
+    if (live) {
+        rad = __double2float_ru(sqrt(qx * qx + qy * qy + qz * qz) * (1.0 + 1.0e-9));
+        if (!(rad >= 0.f)) rad = 3.0e38f;
+    }
+    // FP32 j-record.  Plain form: (x - o, G m).  Mass-scaled form (A.scaled): (q (x - o), q) with
+    // q = (G m)^(-1/2), so that D = q (x_j - x_i) gives G m d / r^3 = D / |D|^3 without a multiply by
+    // G m.  Bodies without (usable) mass and padding get a far-away dummy (1e18, 0, 0 | 0): their
+    // term underflows to exactly 0; a chunk holding a live massless body is always flagged (below).
+    const bool massive = live && (gm >= 1.0e-30) && (gm <= 1.0e30);
+    float q2 = 0.f;
+    {
+        float* f = reinterpret_cast<float*>(w.pk32) + 8 * (s >> 1) + (s & 1);
+        if (!A.scaled) {
+            f[0] = (float)qx; f[2] = (float)qy; f[4] = (float)qz; f[6] = (float)gm;
+        } else if (massive) {
+            const double q = rsqrt(gm);
+            f[0] = (float)(q * qx); f[2] = (float)(q * qy); f[4] = (float)(q * qz); f[6] = (float)q;
+            q2 = __double2float_ru(q * q * (1.0 + 1.0e-6));
+        } else {
+            f[0] = 1.0e18f; f[2] = 0.f; f[4] = 0.f; f[6] = 0.f;
+        }
+    }
+    const float rfc = (A.scaled && live && !massive) ? 3.0e38f : rf;   // massless j: (i, this chunk) always FP64
+    BoundP b; b.hq = hq; b.aq = aq; b.rf = rf; b.pad = live ? 1.f : 0.f;
+    w.bi[s] = b;
+
+    // per-chunk maxima (CHUNK = 64 = two warps); non-negative floats order like unsigned ints
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned int m0 = warp_max_u32(__float_as_uint(hq));
+    unsigned int m1 = warp_max_u32(__float_as_uint(aq));
+    unsigned int m2 = warp_max_u32(__float_as_uint(rfc));
+    unsigned int m3 = warp_max_u32(__float_as_uint(rad));
+    unsigned int m4 = warp_max_u32(__float_as_uint(q2));
+    if (lane == 0) { smax[wid][0] = m0; smax[wid][1] = m1; smax[wid][2] = m2; smax[wid][3] = m3; smax[wid][4] = m4; }
+    __syncthreads();
+    if (threadIdx.x < PREP_NT / CHUNK) {
+        const int c = threadIdx.x;
+        ChunkP q;
+        unsigned int mx[5] = {0u, 0u, 0u, 0u, 0u};
+        for (int ww = 0; ww < CHUNK / 32; ++ww)
+            for (int t = 0; t < 5; ++t) mx[t] = max(mx[t], smax[c * (CHUNK / 32) + ww][t]);
+        q.hq  = __uint_as_float(mx[0]);
+        q.aq  = __uint_as_float(mx[1]);
+        q.rad = __uint_as_float(mx[3]);
+        // frame guard: pairs closer than floor * 2 R_chunk go to FP64 (relative rounding error of
+        // the FP32 separation <= 2^-24 (1 + 2 R_chunk / r))
+        q.rf  = fmaxf(__uint_as_float(mx[2]), __fmul_ru(__fmul_ru(2.0f * A.floor_rel, q.rad), 1.000001f));
+        q.q2max = A.scaled ? __uint_as_float(mx[4]) : 1.0f;   // scales the bound to the kernel's r'^2 = q^2 r^2
+        q.pad_ = 0.f;
+        q.ox = sorg[c][0]; q.oy = sorg[c][1]; q.oz = sorg[c][2];
+        w.bc[tile * (PREP_NT / CHUNK) + c] = q;
+    }
+    if (s == 0) { w.ctr->cand_count = 0u; w.ctr->pair_count = 0u; w.ctr->overflow = 0u; }
+    __syncthreads();                                       // smax / sorg may be reused by the next tile
+}
+
+}  // namespace genga
