@@ -373,3 +373,32 @@ def test_fused_step_equals_separate_kernels():
     g.close()
     assert (np.linalg.norm(x - xo, axis=1) / np.linalg.norm(xo, axis=1)).max() <= 1e-11
     assert (np.linalg.norm(v - vo, axis=1) / np.linalg.norm(vo, axis=1)).max() <= 1e-8
+
+
+def test_sweep_maximum_size_131072_both_precisions():
+    # the largest size of BASELINE.json's N sweep (2^17 bodies, 1.7e10 ordered pairs): the oracle
+    # evaluates every pair on the host cores (tens of seconds)
+    w = W.config(4, 131072)
+    ao, po, _ = oracle_accel(w)
+    a64, p64, _, st64 = gpu_accel(w, B.FP64, pair_capacity=1 << 20)
+    a32, p32, _, st32 = gpu_accel(w, B.FP32, pair_capacity=1 << 20)
+    assert rel_err(a64, ao).max() <= 1e-12
+    e32 = rel_err(a32, ao)
+    assert np.median(e32) <= 1e-5 and e32.max() <= 1e-4, (np.median(e32), e32.max())
+    assert pair_set(p64) == pair_set(po) == pair_set(p32)
+    assert not st64.overflowed and not st32.overflowed
+
+
+def test_eq1_as_printed_at_config1_size():
+    # PAPER.md:51-53 with n1 = 3, n2 = 0.4, max rule, at 6600 bodies: the velocity term makes r_crit
+    # ~13x the Hill term, thousands of pairs sit inside the changeover zone
+    w = W.config(1)
+    kw = dict(n1=3.0, n2=0.4, pair_rule=B.PAIR_MAX)
+    ao, po, rco = oracle_accel(w, **kw)
+    assert len(po) > 1000
+    for prec, tol in ((B.FP64, 1e-12), (B.FP32, 1e-4)):
+        a, pairs, rc, st = gpu_accel(w, prec, pair_capacity=4 * len(po), **kw)
+        assert np.max(np.abs(rc / rco - 1)) <= 1e-14
+        assert rel_err(a, ao).max() <= tol
+        assert pair_set(pairs) == pair_set(po)
+        assert not st.overflowed
