@@ -39,7 +39,7 @@ def build(force: bool = False) -> str:
 class _Params(ctypes.Structure):
     _fields_ = [("G", ctypes.c_double), ("M_star", ctypes.c_double),
                 ("n1", ctypes.c_double), ("n2", ctypes.c_double),
-                ("dt_rcrit", ctypes.c_double), ("pair_rule", ctypes.c_int)]
+                ("dt_rcrit", ctypes.c_double), ("pair_rule", ctypes.c_int), ("n_big", ctypes.c_int)]
 
 
 @dataclass
@@ -51,9 +51,10 @@ class Params:
     n2: float = 0.0                        # BASELINE.json configs: "3 mutual Hill radii"
     dt_rcrit: float = 0.0
     pair_rule: int = PAIR_MUTUAL_HILL
+    n_big: int = -1                        # TP2 mode: pairs interact iff i < n_big or j < n_big
 
     def c(self) -> _Params:
-        return _Params(self.G, self.M_star, self.n1, self.n2, self.dt_rcrit, int(self.pair_rule))
+        return _Params(self.G, self.M_star, self.n1, self.n2, self.dt_rcrit, int(self.pair_rule), int(self.n_big))
 
 
 _lib = None

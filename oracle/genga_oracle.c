@@ -122,6 +122,13 @@ double oracle_pair_rcrit(const oracle_params* p, double mi, double mj,
 
 /* ---- O2-O5: the kick acceleration (north_star; "the N^2 gravitational force
  * terms") ---------------------------------------------------------------------------------- */
+/* TP2 mode ("the giant planets feel the forces of the planetesimals, but the
+ * planetesimals do not feel each other"; reading R9): does the pair (i, j) interact at all? */
+static int interacts(const oracle_params* p, int i, int j)
+{
+    return p->n_big < 0 || i < p->n_big || j < p->n_big;
+}
+
 void oracle_accel(int N, const double* m, const double* x, const double* v,
                   const oracle_params* p, double* acc)
 {
@@ -134,7 +141,7 @@ void oracle_accel(int N, const double* m, const double* x, const double* v,
     for (int i = 0; i < N; ++i) {
         nsum a[3] = {{0, 0}, {0, 0}, {0, 0}};
         for (int j = 0; j < N; ++j) {
-            if (j == i) continue;
+            if (j == i || !interacts(p, i, j)) continue;
             double dx = x[3 * j + 0] - x[3 * i + 0];
             double dy = x[3 * j + 1] - x[3 * i + 1];
             double dz = x[3 * j + 2] - x[3 * i + 2];
@@ -165,6 +172,7 @@ void oracle_encounter_pairs(int N, const double* m, const double* x, const doubl
     int n = 0;
     for (int i = 0; i < N; ++i) {
         for (int j = i + 1; j < N; ++j) {
+            if (!interacts(p, i, j)) continue;
             double dx = x[3 * j + 0] - x[3 * i + 0];
             double dy = x[3 * j + 1] - x[3 * i + 1];
             double dz = x[3 * j + 2] - x[3 * i + 2];
@@ -403,6 +411,7 @@ void oracle_energy_angmom(int N, const double* m, const double* x, const double*
     for (int i = 0; i < N; ++i) {
         nsum q = {0, 0};
         for (int j = i + 1; j < N; ++j) {
+            if (!interacts(p, i, j)) continue;
             double dx = x[3 * j + 0] - x[3 * i + 0];
             double dy = x[3 * j + 1] - x[3 * i + 1];
             double dz = x[3 * j + 2] - x[3 * i + 2];

@@ -26,6 +26,8 @@
  *   oracle_drift           pinned: circular orbit, period return, scipy DOP853, invariants
  *   oracle_step/run        pinned: 2nd-order convergence to a DOP853 inertial-frame solution
  *   oracle_energy_angmom   pinned: two-body closed form, inertial-frame formula
+ *   TP2 mode (n_big >= 0)  pinned: hand 3-body values, full-minus-subset identity against the
+ *                          pinned all-pairs path, sum m a = 0, bounded dt^2 energy error
  */
 #ifndef GENGA_ORACLE_H
 #define GENGA_ORACLE_H
@@ -42,6 +44,10 @@ typedef struct {
     double n1, n2;    /* Eq. 1 constants (3 and 0.4)                    */
     double dt_rcrit;  /* the dt of Eq. 1's second term (reading G8: the step dt)     */
     int    pair_rule; /* reading G2: how r_crit,ij follows from per-body quantities  */
+    int    n_big;     /* TP2 mode (reading R9): a pair (i, j)
+                         interacts iff i < n_big or j < n_big; n_big < 0: every pair
+                         interacts.  Other pairs exert no force, are no encounter
+                         candidates and carry no pair potential in E.              */
 } oracle_params;
 
 /* O4, reading G1 (PAPER.md:45 names Chambers 1999; formula not printed). */
