@@ -404,16 +404,19 @@ def run_report(args):
     from paper_2309_08217_b200 import binding as B
     from paper_2309_08217_b200 import workloads as W
     B.load()
-    for cfg in range(5):
-        w = W.config(cfg)
-        pairs = w.N * (w.N - 1.0)
+    cases = [(cfg, W.config(cfg), {}) for cfg in range(5)]
+    # NEXT-2: config 3 at the paper's 30 000 planetesimals in TP2 mode
+    cases.append(("3-tp2", W.config(3, 30000), {"n_big": 4}))
+    for cfg, w, kw in cases:
+        nb = kw.get("n_big", -1)
+        pairs = w.N * (w.N - 1.0) if nb < 0 else (2.0 * nb * (w.N - nb) + nb * (nb - 1.0))   # interacting ordered pairs
         for prec, name, flop, peak in ((B.FP32, "fp32", FLOP_FP32, PEAK_FP32_TFLOPS), (B.FP64, "fp64", FLOP_FP64, PEAK_FP64_TFLOPS)):
-            g = B.from_workload(w)
+            g = B.from_workload(w, **kw)
             variant = 0 if args.no_autotune else g.autotune(prec)[0]
             E0, L0 = g.energy_angmom()
             g.run(w.dt, 3, prec)                                   # warm-up (3 steps of the same trajectory)
             g.close()
-            g = B.from_workload(w)
+            g = B.from_workload(w, **kw)
             g.set_tuning(0 if prec == B.FP32 else 1, variant)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize()
@@ -428,7 +431,8 @@ def run_report(args):
             g.close()
             evals = w.nsteps + 1
             line = {"report": "config", "config": cfg, "workload": w.name, "N": w.N, "dt_days": w.dt, "steps": w.nsteps,
-                    "precision": name, "kernel_variant": B.variant_name(0 if prec == B.FP32 else 1, variant),
+                    "precision": name, "n_big": nb,
+                    "kernel_variant": "tp2_kernel (FP64)" if nb >= 0 else B.variant_name(0 if prec == B.FP32 else 1, variant),
                     "ms_per_step": ms / w.nsteps, "steps_per_s": w.nsteps / (ms * 1e-3),
                     "body_steps_per_s": w.N * w.nsteps / (ms * 1e-3),
                     "pair_interactions_per_s": pairs * evals / (ms * 1e-3),
@@ -437,7 +441,7 @@ def run_report(args):
                     "dL_over_L": float(np.linalg.norm(L1) / np.linalg.norm(L0) - 1.0),
                     "encounter_pairs_last_eval": enc_last, "nearfield_candidates_last_eval": st.candidates}
             if cfg == 1:                                           # encounter-pair counts per step (untimed second run)
-                g = B.from_workload(w)
+                g = B.from_workload(w, **kw)
                 g.set_tuning(0 if prec == B.FP32 else 1, variant)
                 g.kick(0.5 * w.dt, prec)
                 counts = []

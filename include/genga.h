@@ -85,6 +85,10 @@ typedef struct {
     int    resort_every;      /* force evaluations between two refreshes of the internal body order
                                  (heavy bodies first, then along a Hilbert curve in the x-y plane; a
                                  performance hint only).  <= 0 selects the default (32).              */
+    int    n_big;             /* TP2 mode ("the giant planets feel the forces of the planetesimals,
+                                 but the planetesimals do not feel each other"; reading R9): a pair
+                                 (i, j) interacts iff i < n_big or j < n_big.  < 0 (default): every pair.
+                                 The O(n_big N) pair sums of this mode always run in FP64.              */
     int    no_fused_step;     /* 1: genga_kick/step/run/leapfrog use the separate per-body kernels instead of the
                                  one cooperative kernel per step (debugging; also taken if the device lacks
                                  cooperative launch)                                                   */

@@ -45,6 +45,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_red = take((size_t)RED_DOUBLES * 8), o_vt = take(NP * 24), o_ctr = take(sizeof(Counters));
     const size_t o_ord = take(NP * 4), o_key = take(NP * 8), o_aux = take(NP * 32);
     const size_t o_mom = take((8 + 4 * (NP / 128 + 1) + 8 * (size_t)MOM_MAX_BLOCKS) * 8);
+    const size_t o_bs = take(NP * 4);
     const size_t o_bk = take(NP * 8), o_sb = take((size_t)sort_buffer_words() * 4);
     if (w && base) {
         char* b = static_cast<char*>(base);
@@ -56,6 +57,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
         w->ctr = (Counters*)(b + o_ctr);
         w->order = (int*)(b + o_ord); w->keys = (unsigned long long*)(b + o_key); w->aux = (double4*)(b + o_aux);
         w->mom = (double*)(b + o_mom);
+        w->bigslot = (int*)(b + o_bs);
         w->bkeys = (unsigned long long*)(b + o_bk); w->sortbuf = (unsigned int*)(b + o_sb);
     }
     return off;
@@ -119,6 +121,7 @@ static PrepArgs make_prep_args(const Handle* h, int precision, double preshift)
     a.N = h->N; a.NP = h->NP;
     a.G = h->p.G; a.M_star = h->p.M_star; a.n1 = h->p.n1; a.n2 = h->p.n2; a.dt_rcrit = h->p.dt_rcrit;
     a.pair_rule = h->p.pair_rule;
+    a.n_big = (h->p.n_big >= 0 && h->p.n_big < h->N) ? h->p.n_big : -1;
     a.preshift = preshift;
     a.scaled = (precision == GENGA_FP32 && kick32_variant_scaled(h->tune[0])) ? 1 : 0;
     if (precision == GENGA_FP32) {
@@ -133,6 +136,10 @@ static PrepArgs make_prep_args(const Handle* h, int precision, double preshift)
 // all-pairs kernel + near-field kernel on the arrays the prep step packed
 static int launch_pairs(Handle* h, int precision)
 {
+    if (h->p.n_big >= 0 && h->p.n_big < h->N) {          // TP2 mode: O(n_big N) pairs, FP64 (reading R9)
+        if (h->p.n_big > 0) { ProfScope ps(h, 0); launch_tp2(h); LAUNCHED(h, "tp2_kernel"); }
+        return GENGA_OK;
+    }
     { ProfScope ps(h, 0); if (precision == GENGA_FP32) launch_kick32(h); else launch_kick64(h); }
     LAUNCHED(h, "kick_kernel");
     { ProfScope ps(h, 1); launch_nearfield(h); }
@@ -258,6 +265,7 @@ void genga_default_params(genga_params* p)
     p->pair_capacity = 0; p->cand_capacity = 0;
     p->resort_every = 0;
     p->no_fused_step = 0;
+    p->n_big = -1;
 }
 
 size_t genga_workspace_bytes(int N, const genga_params* p)

@@ -56,6 +56,7 @@ struct Workspace {
     int*     order;   // [NP]   slot -> body index (API order); order[s] = s for the padding slots s >= N
     unsigned long long* keys;   // [NP] sort keys (heavy class, Hilbert index, body index)
     unsigned long long* bkeys;  // [NP] the keys grouped by bucket
+    int* bigslot;               // [NP] TP2 mode: slot of big body b (b < n_big)
     unsigned int* sortbuf;      // bucket histogram, starts and cursors of the sort
     double4* pk64;    // [NP]   (x, y, z, G m)
     float4*  pk32;    // [NP]   pair-interleaved, see above
@@ -108,6 +109,7 @@ struct PrepArgs {
     int N, NP;
     double G, M_star, n1, n2, dt_rcrit;
     int pair_rule;
+    int n_big;                   // TP2 mode (>= 0): prep also records the slots of the big bodies
     float lambda, floor_rel;     // near-field policy for this evaluation
     int scaled;                  // FP32 j-records in the mass-scaled form (kick_fp32.cu, SC variants)
     double preshift;             // pending Sun-kick: x += preshift * mom[SLOT_B] / M_star before anything else
@@ -129,6 +131,7 @@ void launch_prep(const Handle* h, const PrepArgs& a);
 void launch_kick32(const Handle* h);
 void launch_kick64(const Handle* h);
 void launch_nearfield(const Handle* h);
+void launch_tp2(const Handle* h);                            // TP2 mode: big bodies against all (FP64)
 void launch_velupdate(const Handle* h, double tau);
 void launch_momentum(const Handle* h);                       // red[0..2] = sum m v, red[3] = sum m
 void launch_momentum_slot_a(const Handle* h);                // the same into mom[SLOT_A]

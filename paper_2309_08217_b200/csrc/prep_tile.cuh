@@ -51,6 +51,7 @@ __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int t
         const double mi = w.m[i];
         gm = A.G * mi;
         ax4 = make_double4(mi, rc, sa, vk);
+        if (i < A.n_big) w.bigslot[i] = s;                 // TP2 mode: where the big bodies sit
 
         const double lam = (double)A.lambda * (1.0 + 1.0e-6);
         double dhq, daq, drf;

@@ -47,7 +47,8 @@ __device__ __forceinline__ double block_sum(double v, double* sh)
 // Block b owns i-tiles b and T-1-b (equal total work for every block): sum over j > i of
 // G m_j / r_ij, times m_i, summed over the block -> red[8 + b].
 __global__ void __launch_bounds__(ET)
-pairpot_kernel(int N, int T, double G, const double* __restrict__ x, const double* __restrict__ m, double* __restrict__ red)
+pairpot_kernel(int N, int T, double G, int n_big, const double* __restrict__ x, const double* __restrict__ m,
+               double* __restrict__ red)
 {
     __shared__ double4 sj[ET];
     __shared__ double sh[32];
@@ -77,13 +78,13 @@ pairpot_kernel(int N, int T, double G, const double* __restrict__ x, const doubl
                 const double dx = J.x - qA.x, dy = J.y - qA.y, dz = J.z - qA.z;
                 const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
                 const double y  = rsqrt_refined(r2);
-                potA = (j > iA) ? fma(J.w, y, potA) : potA;
+                potA = (j > iA && (iA < n_big || j < n_big)) ? fma(J.w, y, potA) : potA;   // TP2: interacting pairs only
             }
             if (doB) {
                 const double dx = J.x - qB.x, dy = J.y - qB.y, dz = J.z - qB.z;
                 const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
                 const double y  = rsqrt_refined(r2);
-                potB = (j > iB) ? fma(J.w, y, potB) : potB;
+                potB = (j > iB && (iB < n_big || j < n_big)) ? fma(J.w, y, potB) : potB;
             }
         }
     }
@@ -131,7 +132,8 @@ void launch_energy(const Handle* h)
     const int T = h->NP / ET;
     const int nblk = (T + 1) / 2;
     if (nblk > 0)
-        pairpot_kernel<<<nblk, ET, 0, h->stream>>>(h->N, T, h->p.G, h->w.x, h->w.m, h->w.red);
+        pairpot_kernel<<<nblk, ET, 0, h->stream>>>(h->N, T, h->p.G, (h->p.n_big >= 0 && h->p.n_big < h->N) ? h->p.n_big : h->N,
+                                                   h->w.x, h->w.m, h->w.red);
     energy_final_kernel<<<1, 1024, 0, h->stream>>>(h->N, nblk, h->p.G, h->p.M_star, h->w.m, h->w.x, h->w.v, h->w.red);
 }
 

@@ -402,3 +402,64 @@ def test_eq1_as_printed_at_config1_size():
         assert rel_err(a, ao).max() <= tol
         assert pair_set(pairs) == pair_set(po)
         assert not st.overflowed
+
+
+# ---- TP2 mode (reading R9): pairs interact iff one body is among the first n_big ----
+def _tp2_check(w, n_big, **kw):
+    p = oparams(w, n_big=n_big, **kw)
+    vd = oracle.to_democratic(w.m, w.v, w.M_star)
+    ao = oracle.accel(w.m, w.x, vd, p)
+    po = oracle.encounter_pairs(w.m, w.x, vd, p)
+    Eo, Lo = oracle.energy_angmom(w.m, w.x, vd, p)
+    scale = np.linalg.norm(ao, axis=1)
+    scale[scale == 0] = 1.0
+    for prec in (B.FP64, B.FP32):                       # the O(n_big N) sums run in FP64 for both flags
+        g = B.from_workload(w, n_big=n_big, pair_capacity=max(4 * len(po), 1024), **kw)
+        g.accel(prec)
+        a = g.get_accel().cpu().numpy()
+        pairs = g.encounter_pairs()
+        E, L = g.energy_angmom()
+        g.close()
+        assert (np.linalg.norm(a - ao, axis=1) / scale).max() <= 1e-12
+        assert pair_set(pairs) == pair_set(po)
+        assert all(i < j for i, j in pairs.tolist())
+        assert abs(E / Eo - 1) <= 1e-13 and np.linalg.norm(L - Lo) / np.linalg.norm(Lo) <= 1e-13
+    return ao, po
+
+
+def test_tp2_giants_and_disc_at_the_papers_size():
+    # four giant planets + 30 000 planetesimals that do not feel each other
+    w = W.config(3, 30000)
+    ao, po = _tp2_check(w, 4)
+    assert np.all(np.linalg.norm(ao, axis=1) > 0)
+
+
+def test_tp2_embryos_dense_zones_and_limits():
+    w = W.config(2, 1400)                               # 100 embryos are the big bodies
+    _, po = _tp2_check(w, 100, n1=3.0, n2=0.4, pair_rule=B.PAIR_MAX)
+    assert len(po) > 20
+    w = clustered(5, 700)
+    _tp2_check(w, 7)
+    _tp2_check(w, 0)                                    # nobody big: no forces, no pairs
+    # n_big >= N is the all-pairs path
+    ao, po, _ = oracle_accel(w)
+    a, pairs, _, _ = gpu_accel(w, B.FP64, n_big=w.N, pair_capacity=2 * len(po))
+    assert rel_err(a, ao).max() <= 1e-12 and pair_set(pairs) == pair_set(po)
+
+
+def test_tp2_trajectory_and_conservation():
+    w = W.config(3, 1500)
+    p = oparams(w, n_big=4)
+    vd = oracle.to_democratic(w.m, w.v, w.M_star)
+    xo, vo = oracle.run(w.m, w.x, vd, p, w.dt, 5)
+    g = B.from_workload(w, n_big=4)
+    E0, L0 = g.energy_angmom()
+    g.run(w.dt, 5, B.FP32)
+    x, v = (t.cpu().numpy() for t in g.get_state())
+    E1, L1 = g.energy_angmom()
+    g.close()
+    assert (np.linalg.norm(x - xo, axis=1) / np.linalg.norm(xo, axis=1)).max() <= 1e-10
+    assert (np.linalg.norm(v - vo, axis=1) / np.linalg.norm(vo, axis=1)).max() <= 1e-10
+    assert abs(np.linalg.norm(L1) / np.linalg.norm(L0) - 1) <= 1e-13
+    Eo1, _ = oracle.energy_angmom(w.m, xo, vo, p)
+    assert abs(E1 / Eo1 - 1) <= 1e-12
