@@ -295,7 +295,7 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     genga_s* h = new (std::nothrow) genga_s();
     if (!h) return GENGA_ENOMEM;
     std::memset(static_cast<Handle*>(h), 0, sizeof(Handle));
-    h->N = N; h->NP = padded(N); h->nchunk = h->NP / CHUNK;
+    h->N = N; h->NP = padded(N); h->nchunk = (N + CHUNK - 1) / CHUNK;        // j-chunks that hold a live body (pure padding is skipped)
     h->p = *p;
     h->lambda_near = p->lambda_near > 0.0 ? p->lambda_near : 2.0;
     h->near_floor  = p->near_floor >= 0.0 ? p->near_floor : (1.0 / 256.0);

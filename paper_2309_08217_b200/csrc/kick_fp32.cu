@@ -293,7 +293,7 @@ void launch_kick32(const Handle* h)
 {
     if (h->N == 0) return;
     const Variant32& V = variant32(h->tune[0]);
-    const int nib = h->NP / V.bi;
+    const int nib = (h->N + V.bi - 1) / V.bi;          // i-blocks that hold a live body
     const long long U = (long long)nib * h->nchunk;
     long long G = kick32_grid(h);
     if (G > U) G = U;

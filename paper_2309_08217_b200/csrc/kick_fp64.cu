@@ -220,7 +220,7 @@ void launch_kick64(const Handle* h)
 {
     if (h->N == 0) return;
     const Variant64& V = variant64(h->tune[1]);
-    const int nib = h->NP / V.bi;
+    const int nib = (h->N + V.bi - 1) / V.bi;          // i-blocks that hold a live body
     const long long U = (long long)nib * h->nchunk;
     long long G = kick64_grid(h);
     if (G > U) G = U;
