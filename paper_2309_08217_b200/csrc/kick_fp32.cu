@@ -262,16 +262,9 @@ const Variant32 g_variants32[] = {
     V32(2, 128, 4, false, 4, false),
 };
 constexpr int NVAR32 = (int)(sizeof(g_variants32) / sizeof(g_variants32[0]));
-bool g_attr32[NVAR32] = {};
-
 const Variant32& variant32(int v)
 {
-    if (v < 0 || v >= NVAR32) v = 0;
-    if (!g_attr32[v]) {
-        cudaFuncSetAttribute(g_variants32[v].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_variants32[v].smem);
-        g_attr32[v] = true;
-    }
-    return g_variants32[v];
+    return g_variants32[(v < 0 || v >= NVAR32) ? 0 : v];
 }
 
 }  // namespace
@@ -280,13 +273,22 @@ int kick32_num_variants() { return NVAR32; }
 bool kick32_variant_scaled(int v) { return (v >= 0 && v < NVAR32) ? g_variants32[v].scaled : false; }
 const char* kick32_variant_name(int v) { return (v >= 0 && v < NVAR32) ? g_variants32[v].name : ""; }
 
+// Grid of the current variant: SMs x resident CTAs.  The occupancy query and the dynamic-smem opt-in
+// are per device and per variant; the result is cached in the handle (one handle = one device).
 int kick32_grid(const Handle* h)
 {
-    const Variant32& V = variant32(h->tune[0]);
-    int occ = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn, V.nt, V.smem);
-    if (occ < 1) occ = 1;
-    return h->num_sms * occ;
+    const int v = h->tune[0];
+    Handle* hm = const_cast<Handle*>(h);
+    if (hm->grid_cache[0][0] != v + 1) {
+        const Variant32& V = variant32(v);
+        cudaFuncSetAttribute(V.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V.smem);
+        int occ = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn, V.nt, V.smem);
+        if (occ < 1) occ = 1;
+        hm->grid_cache[0][0] = v + 1;
+        hm->grid_cache[0][1] = h->num_sms * occ;
+    }
+    return hm->grid_cache[0][1];
 }
 
 void launch_kick32(const Handle* h)

@@ -190,16 +190,9 @@ const Variant64 g_variants64[] = {
     V64(4, 64, 6, 2),
 };
 constexpr int NVAR64 = (int)(sizeof(g_variants64) / sizeof(g_variants64[0]));
-bool g_attr64[NVAR64] = {};
-
 const Variant64& variant64(int v)
 {
-    if (v < 0 || v >= NVAR64) v = 0;
-    if (!g_attr64[v]) {
-        cudaFuncSetAttribute(g_variants64[v].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_variants64[v].smem);
-        g_attr64[v] = true;
-    }
-    return g_variants64[v];
+    return g_variants64[(v < 0 || v >= NVAR64) ? 0 : v];
 }
 
 }  // namespace
@@ -207,13 +200,22 @@ const Variant64& variant64(int v)
 int kick64_num_variants() { return NVAR64; }
 const char* kick64_variant_name(int v) { return (v >= 0 && v < NVAR64) ? g_variants64[v].name : ""; }
 
+// Grid of the current variant: SMs x resident CTAs.  The occupancy query and the dynamic-smem opt-in
+// are per device and per variant; the result is cached in the handle (one handle = one device).
 int kick64_grid(const Handle* h)
 {
-    const Variant64& V = variant64(h->tune[1]);
-    int occ = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn, V.nt, V.smem);
-    if (occ < 1) occ = 1;
-    return h->num_sms * occ;
+    const int v = h->tune[1];
+    Handle* hm = const_cast<Handle*>(h);
+    if (hm->grid_cache[1][0] != v + 1) {
+        const Variant64& V = variant64(v);
+        cudaFuncSetAttribute(V.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V.smem);
+        int occ = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn, V.nt, V.smem);
+        if (occ < 1) occ = 1;
+        hm->grid_cache[1][0] = v + 1;
+        hm->grid_cache[1][1] = h->num_sms * occ;
+    }
+    return hm->grid_cache[1][1];
 }
 
 void launch_kick64(const Handle* h)
