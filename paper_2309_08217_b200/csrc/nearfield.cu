@@ -81,20 +81,23 @@ __device__ __forceinline__ IBody load_ibody(const Workspace& w, int si)
     return b;
 }
 
-// Force of chunk c on the body in slot si, partial per lane (two j per lane).  A pair outside the
-// conservative pair bound (the same bound the all-pairs kernels use per chunk, here per pair) has
-// K = 1 exactly and cannot be an encounter: it takes the cheap refined-rsqrt path.  Every other
-// pair is evaluated with plain sqrt / divide / cbrt: exact r < r_crit test, K, force.
+// Force of chunk c on the body in slot si, partial per lane.  Two phases per (body, chunk):
+//  A  every pair outside the conservative pair bound (the bound the all-pairs kernels use per
+//     chunk, here per pair) has K = 1 exactly and cannot be an encounter: cheap refined-rsqrt term.
+//     The slots of the other pairs are compacted (__ballot_sync) into the warp's list in shared memory.
+//  B  the listed pairs, one per lane: plain sqrt / divide / cbrt, exact r < r_crit test, K, force;
+//     encounter pairs appended with one atomic per warp.
+// (One pass over the few near pairs with many lanes active, instead of one divergent pass per round.)
 __device__ __forceinline__ void chunk_on_body(const NfParams& P, Workspace& w, const IBody& I, int c,
-                                              double& fx, double& fy, double& fz)
+                                              int* __restrict__ near_list, double& fx, double& fy, double& fz)
 {
     const int lane = threadIdx.x & 31;
+    constexpr int H = CHUNK / 32;
+    int nnear = 0;
 #pragma unroll
-    for (int h = 0; h < CHUNK / 32; ++h) {
+    for (int h = 0; h < H; ++h) {
         const int sj = c * CHUNK + h * 32 + lane;
-        double sx = 0.0, sy = 0.0, sz = 0.0;
-        bool enc = false;
-        int bj = 0;
+        bool near = false;
         if (sj < P.N && sj != I.slot) {
             const double4 q = w.pk64[sj];
             const BoundP  b = w.bi[sj];
@@ -102,32 +105,54 @@ __device__ __forceinline__ void chunk_on_body(const NfParams& P, Workspace& w, c
             const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
             const float  Bq = fmaxf(fmaxf(I.hq, b.hq) * fmaxf(I.aq, b.aq), fmaxf(I.rf, b.rf));
             const double bd = (double)Bq * (double)Bq * 1.000001;
-            if (r2 > bd) {
+            near = !(r2 > bd);
+            if (!near) {
                 const double y0 = rsq64h(r2);
                 const double t  = y0 * y0;
                 const double e  = fma(-r2, t, 1.0);
                 const double cc = fma(1.875, e, 1.5);
                 const double g  = (q.w * y0) * t;
                 const double s  = fma(g * e, cc, g);
-                sx = s * dx; sy = s * dy; sz = s * dz;
-            } else {
-                const double4 A = w.aux[sj];
-                const double r  = sqrt(r2);
-                const double rc = pair_rcrit(P, I.m, A.x, I.rc, A.y, I.a, A.z, I.vk, A.w);
-                enc = (I.slot < sj) && (r < rc);           // coincident bodies (r = 0) are an encounter
-                if (enc) bj = w.order[sj];
-                if (r > 0.0) {
-                    const double W = changeover(r, rc);
-                    if (W != 0.0) {
-                        const double s = q.w * W / (r2 * r);
-                        sx = s * dx; sy = s * dy; sz = s * dz;
-                    }
+                fx = fma(s, dx, fx); fy = fma(s, dy, fy); fz = fma(s, dz, fz);
+            }
+        }
+        const unsigned int bal = __ballot_sync(0xffffffffu, near);
+        if (near) near_list[nnear + __popc(bal & ((1u << lane) - 1u))] = sj;
+        nnear += __popc(bal);
+    }
+    __syncwarp();
+    for (int k0 = 0; k0 < nnear; k0 += 32) {
+        const int k = k0 + lane;
+        int encj = -1;
+        if (k < nnear) {
+            const int sj = near_list[k];
+            const double4 q = w.pk64[sj];
+            const double4 A = w.aux[sj];
+            const double dx = q.x - I.x, dy = q.y - I.y, dz = q.z - I.z;
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            const double r  = sqrt(r2);
+            const double rc = pair_rcrit(P, I.m, A.x, I.rc, A.y, I.a, A.z, I.vk, A.w);
+            if ((I.slot < sj) && (r < rc)) encj = w.order[sj];       // coincident bodies (r = 0) are an encounter
+            if (r > 0.0) {
+                const double W = changeover(r, rc);
+                if (W != 0.0) {
+                    const double s = q.w * W / (r2 * r);
+                    fx = fma(s, dx, fx); fy = fma(s, dy, fy); fz = fma(s, dz, fz);
                 }
             }
         }
-        append_pair(enc, min(I.body, bj), max(I.body, bj), w, P.pair_cap);
-        fx += sx; fy += sy; fz += sz;
+        const unsigned int bal = __ballot_sync(0xffffffffu, encj >= 0);
+        if (bal) {
+            unsigned int base = 0;
+            if (lane == 0) base = atomicAdd(&w.ctr->pair_count, (unsigned int)__popc(bal));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (encj >= 0) {
+                const unsigned int idx = base + __popc(bal & ((1u << lane) - 1u));
+                if (idx < P.pair_cap) w.pairs[idx] = make_int2(min(I.body, encj), max(I.body, encj));
+            }
+        }
     }
+    __syncwarp();                                  // the list is reused by the next (body, chunk)
 }
 
 __device__ __forceinline__ double warp_sum(double v)
@@ -137,20 +162,22 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 8)
 nearfield_kernel(NfParams P, Workspace w)
 {
+    __shared__ int s_near[128 / 32][CHUNK];
     const int lane  = threadIdx.x & 31;
     const int warp  = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int nwarp = (gridDim.x * blockDim.x) >> 5;
     const unsigned int count = w.ctr->cand_count;
+    int* near_list = s_near[threadIdx.x >> 5];
 
     if (count <= P.cand_cap) {
         for (unsigned int q = warp; q < count; q += nwarp) {
             const int2 cd = w.cand[q];
             const IBody I = load_ibody(w, cd.x);
             double fx = 0.0, fy = 0.0, fz = 0.0;
-            chunk_on_body(P, w, I, cd.y, fx, fy, fz);
+            chunk_on_body(P, w, I, cd.y, near_list, fx, fy, fz);
             fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
             if (lane == 0) {
                 atomicAdd(&w.a[3 * I.body + 0], fx);
@@ -164,7 +191,7 @@ nearfield_kernel(NfParams P, Workspace w)
         for (int si = warp; si < P.N; si += nwarp) {
             const IBody I = load_ibody(w, si);
             double fx = 0.0, fy = 0.0, fz = 0.0;
-            for (int c = 0; c < P.nchunk; ++c) chunk_on_body(P, w, I, c, fx, fy, fz);
+            for (int c = 0; c < P.nchunk; ++c) chunk_on_body(P, w, I, c, near_list, fx, fy, fz);
             fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
             if (lane == 0) { w.a[3 * I.body + 0] = fx; w.a[3 * I.body + 1] = fy; w.a[3 * I.body + 2] = fz; }
         }
@@ -245,7 +272,7 @@ void launch_nearfield(const Handle* h)
     P.M_star = h->p.M_star; P.n1 = h->p.n1; P.n2dt = h->p.n2 * h->p.dt_rcrit;
     P.pair_rule = h->p.pair_rule;
     P.cand_cap = (unsigned int)h->cand_cap; P.pair_cap = (unsigned int)h->pair_cap;
-    int blocks = h->num_sms * 8;
+    int blocks = h->num_sms * 16;
     const long long need = ((long long)h->N + 3) / 4;            // at least one warp per body is enough
     if (blocks > need && need > 0) blocks = (int)((need < h->num_sms) ? h->num_sms : need);
     nearfield_kernel<<<blocks, 128, 0, h->stream>>>(P, h->w);
