@@ -39,7 +39,7 @@ def build(force: bool = False) -> str:
 class _Params(ctypes.Structure):
     _fields_ = [("G", ctypes.c_double), ("M_star", ctypes.c_double),
                 ("n1", ctypes.c_double), ("n2", ctypes.c_double),
-                ("dt_rcrit", ctypes.c_double), ("pair_rule", ctypes.c_int), ("n_big", ctypes.c_int)]
+                ("dt_rcrit", ctypes.c_double), ("pair_rule", ctypes.c_int), ("n_big", ctypes.c_int), ("weight_mode", ctypes.c_int)]
 
 
 @dataclass
@@ -52,9 +52,11 @@ class Params:
     dt_rcrit: float = 0.0
     pair_rule: int = PAIR_MUTUAL_HILL
     n_big: int = -1                        # TP2 mode: pairs interact iff i < n_big or j < n_big
+    weight_mode: int = 0                   # 0: W = K; 1: W = K - r dK/dr (reading R10)
 
     def c(self) -> _Params:
-        return _Params(self.G, self.M_star, self.n1, self.n2, self.dt_rcrit, int(self.pair_rule), int(self.n_big))
+        return _Params(self.G, self.M_star, self.n1, self.n2, self.dt_rcrit, int(self.pair_rule), int(self.n_big),
+                       int(self.weight_mode))
 
 
 _lib = None
@@ -69,6 +71,8 @@ def lib() -> ctypes.CDLL:
         L = ctypes.CDLL(build())
         L.oracle_changeover.restype = ctypes.c_double
         L.oracle_changeover.argtypes = [ctypes.c_double, ctypes.c_double]
+        L.oracle_weight.restype = ctypes.c_double
+        L.oracle_weight.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int]
         L.oracle_pair_rcrit.restype = ctypes.c_double
         L.oracle_pair_rcrit.argtypes = [_pp] + [ctypes.c_double] * 8
         L.oracle_to_democratic.argtypes = [ctypes.c_int, _dp, _dp, ctypes.c_double]
@@ -110,6 +114,11 @@ def num_threads() -> int:
 def changeover(r: float, rcrit: float) -> float:
     """O4 (reading G1)."""
     return float(lib().oracle_changeover(float(r), float(rcrit)))
+
+
+def weight(r: float, rcrit: float, mode: int) -> float:
+    """Pair weight W: mode 0 = K, mode 1 = K - r dK/dr (reading R10)."""
+    return float(lib().oracle_weight(float(r), float(rcrit), int(mode)))
 
 
 def to_democratic(m, v, M_star: float = 1.0) -> np.ndarray:

@@ -53,6 +53,21 @@ double oracle_changeover(double r, double rcrit)
     return (y * y) / (2.0 * y * y - 2.0 * y + 1.0);
 }
 
+/* Pair weight (reading G1b / R10).  mode 0: W = K (north_star: "weighted by the changeover function
+ * K").  mode 1: W = K - r dK/dr, the weight that makes the kick the gradient of the K-weighted pair
+ * potential -G m_i m_j K(r)/r:  -d/dr [K/r] = (K - r K')/r^2.  With y = (r - 0.1 rc)/(0.9 rc) and
+ * K = y^2/D, D = 2y^2 - 2y + 1:  dK/dy = 2y(1 - y)/D^2, dK/dr = dK/dy / (0.9 rc); K' = 0 outside 0<y<1. */
+double oracle_weight(double r, double rcrit, int mode)
+{
+    double K = oracle_changeover(r, rcrit);
+    if (mode == 0 || !(rcrit > 0.0)) return K;
+    double y = (r - 0.1 * rcrit) / (0.9 * rcrit);
+    if (y <= 0.0 || y >= 1.0) return K;
+    double D = 2.0 * y * y - 2.0 * y + 1.0;
+    double dKdr = (2.0 * y * (1.0 - y) / (D * D)) / (0.9 * rcrit);
+    return K - r * dKdr;
+}
+
 /* ---- O1: velocity conventions, reading G3 -------------------------------------------------
  * stored v_i = v_h,i - (sum_j m_j v_h,j)/(M_star + sum_j m_j);
  * inverse    v_h,i = v_i + (sum_j m_j v_j)/M_star.                                            */
@@ -149,7 +164,7 @@ void oracle_accel(int N, const double* m, const double* x, const double* v,
             double r  = sqrt(r2);
             if (!(r > 0.0)) continue;                     /* coincident bodies: W = 0 */
             double rcij = oracle_pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j]);
-            double W = oracle_changeover(r, rcij);
+            double W = oracle_weight(r, rcij, p->weight_mode);
             if (W == 0.0) continue;
             double s = p->G * m[j] * W / (r2 * r);
             nsum_add(&a[0], s * dx);

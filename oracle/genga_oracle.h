@@ -26,6 +26,8 @@
  *   oracle_drift           pinned: circular orbit, period return, scipy DOP853, invariants
  *   oracle_step/run        pinned: 2nd-order convergence to a DOP853 inertial-frame solution
  *   oracle_energy_angmom   pinned: two-body closed form, inertial-frame formula
+ *   oracle_weight mode 1   pinned: hand value at y = 1/2, limits, -r^2 d/dr[K/r] by central
+ *                          differences of the pinned K, two-body force = -grad of the potential
  *   TP2 mode (n_big >= 0)  pinned: hand 3-body values, full-minus-subset identity against the
  *                          pinned all-pairs path, sum m a = 0, bounded dt^2 energy error
  */
@@ -48,10 +50,14 @@ typedef struct {
                          interacts iff i < n_big or j < n_big; n_big < 0: every pair
                          interacts.  Other pairs exert no force, are no encounter
                          candidates and carry no pair potential in E.              */
+    int    weight_mode; /* 0: pair weight W = K (default); 1: W = K - r dK/dr, the gradient of
+                           the K-weighted pair potential (reading R10, NEXT-3)  */
 } oracle_params;
 
 /* O4, reading G1 (PAPER.md:45 names Chambers 1999; formula not printed). */
 double oracle_changeover(double r, double rcrit);
+/* Pair weight W(r, r_crit): mode 0 = K, mode 1 = K - r dK/dr (reading R10).    */
+double oracle_weight(double r, double rcrit, int mode);
 
 /* O1: heliocentric velocities <-> stored barycentric ("democratic") ones.    */
 void oracle_to_democratic(int N, const double* m, double* v, double M_star);
