@@ -89,6 +89,9 @@ typedef struct {
                                  but the planetesimals do not feel each other"; reading R9): a pair
                                  (i, j) interacts iff i < n_big or j < n_big.  < 0 (default): every pair.
                                  The O(n_big N) pair sums of this mode always run in FP64.              */
+    int    weight_mode;       /* pair weight inside a changeover zone (reading R10): 0 (default) W = K,
+                                 as north_star words it; 1: W = K - r dK/dr, the gradient of the pair
+                                 potential -G m_i m_j K / r (Hamiltonian-consistent level-0 kick)       */
     int    no_fused_step;     /* 1: genga_kick/step/run/leapfrog use the separate per-body kernels instead of the
                                  one cooperative kernel per step (debugging; also taken if the device lacks
                                  cooperative launch)                                                   */

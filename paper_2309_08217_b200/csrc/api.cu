@@ -266,6 +266,7 @@ void genga_default_params(genga_params* p)
     p->resort_every = 0;
     p->no_fused_step = 0;
     p->n_big = -1;
+    p->weight_mode = 0;
 }
 
 size_t genga_workspace_bytes(int N, const genga_params* p)
@@ -281,6 +282,7 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     if (!out || !p || N < 0 || N > (1 << 20)) return GENGA_EINVAL;
     if (!(p->M_star > 0.0) || !(p->G > 0.0)) return GENGA_EINVAL;
     if (p->pair_rule != GENGA_PAIR_MAX && p->pair_rule != GENGA_PAIR_MUTUAL_HILL) return GENGA_EINVAL;
+    if (p->weight_mode != 0 && p->weight_mode != 1) return GENGA_EINVAL;
     *out = nullptr;
     int pc, cc;
     resolve_caps(N, p, &pc, &cc);

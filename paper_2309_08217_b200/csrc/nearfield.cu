@@ -18,6 +18,7 @@ struct NfParams {
     int N, nchunk;
     double M_star, n1, n2dt;
     int pair_rule;
+    int weight_mode;                               // 0: W = K, 1: W = K - r dK/dr (reading R10)
     unsigned int cand_cap, pair_cap;
 };
 
@@ -33,14 +34,18 @@ __device__ __forceinline__ double pair_rcrit(const NfParams& P, double mi, doubl
     return fmax(rci, rcj);
 }
 
-// O4: K(r, r_crit), reading G1 (Chambers-1999 rational form)
-__device__ __forceinline__ double changeover(double r, double rc)
+// O4: pair weight W(r, r_crit).  K, reading G1 (Chambers-1999 rational form); mode 1 (reading R10):
+// K - r dK/dr, the weight that makes the kick the gradient of the pair potential -G m_i m_j K / r.
+__device__ __forceinline__ double changeover(double r, double rc, int mode)
 {
     if (!(rc > 0.0)) return (r > 0.0) ? 1.0 : 0.0;
     const double y = (r - 0.1 * rc) / (0.9 * rc);
     if (y <= 0.0) return 0.0;
     if (y >= 1.0) return 1.0;
-    return (y * y) / (2.0 * y * y - 2.0 * y + 1.0);
+    const double D = 2.0 * y * y - 2.0 * y + 1.0;
+    const double K = (y * y) / D;
+    if (mode == 0) return K;
+    return K - r * ((2.0 * y * (1.0 - y) / (D * D)) / (0.9 * rc));
 }
 
 __device__ __forceinline__ void append_pair(bool flag, int i, int j, Workspace& w, unsigned int cap)
@@ -134,7 +139,7 @@ __device__ __forceinline__ void chunk_on_body(const NfParams& P, Workspace& w, c
             const double rc = pair_rcrit(P, I.m, A.x, I.rc, A.y, I.a, A.z, I.vk, A.w);
             if ((I.slot < sj) && (r < rc)) encj = w.order[sj];       // coincident bodies (r = 0) are an encounter
             if (r > 0.0) {
-                const double W = changeover(r, rc);
+                const double W = changeover(r, rc, P.weight_mode);
                 if (W != 0.0) {
                     const double s = q.w * W / (r2 * r);
                     fx = fma(s, dx, fx); fy = fma(s, dy, fy); fz = fma(s, dz, fz);
@@ -232,7 +237,7 @@ tp2_kernel(NfParams P, int n_big, Workspace w)
                 const bool jbig = bj < n_big;
                 enc = (r < rc) && (!jbig || I.body < bj);      // coincident bodies (r = 0) are an encounter
                 if (r > 0.0) {
-                    const double W = changeover(r, rc);
+                    const double W = changeover(r, rc, P.weight_mode);
                     if (W != 0.0) {
                         const double u = W / (r2 * r);
                         const double sb = q.w * u;               // on b from j
@@ -270,7 +275,7 @@ void launch_nearfield(const Handle* h)
     NfParams P;
     P.N = h->N; P.nchunk = (h->N + CHUNK - 1) / CHUNK;
     P.M_star = h->p.M_star; P.n1 = h->p.n1; P.n2dt = h->p.n2 * h->p.dt_rcrit;
-    P.pair_rule = h->p.pair_rule;
+    P.pair_rule = h->p.pair_rule; P.weight_mode = h->p.weight_mode;
     P.cand_cap = (unsigned int)h->cand_cap; P.pair_cap = (unsigned int)h->pair_cap;
     int blocks = h->num_sms * 16;
     const long long need = ((long long)h->N + 3) / 4;            // at least one warp per body is enough
@@ -284,7 +289,7 @@ void launch_tp2(const Handle* h)
     NfParams P;
     P.N = h->N; P.nchunk = (h->N + CHUNK - 1) / CHUNK;
     P.M_star = h->p.M_star; P.n1 = h->p.n1; P.n2dt = h->p.n2 * h->p.dt_rcrit;
-    P.pair_rule = h->p.pair_rule;
+    P.pair_rule = h->p.pair_rule; P.weight_mode = h->p.weight_mode;
     P.cand_cap = (unsigned int)h->cand_cap; P.pair_cap = (unsigned int)h->pair_cap;
     const int per_block = TP2_NT * TP2_JPT;
     dim3 grid((h->N + per_block - 1) / per_block, h->p.n_big < 65535 ? h->p.n_big : 65535);

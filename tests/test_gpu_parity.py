@@ -463,3 +463,24 @@ def test_tp2_trajectory_and_conservation():
     assert abs(np.linalg.norm(L1) / np.linalg.norm(L0) - 1) <= 1e-13
     Eo1, _ = oracle.energy_angmom(w.m, xo, vo, p)
     assert abs(E1 / Eo1 - 1) <= 1e-12
+
+
+def test_weight_mode_k_minus_r_dk_dr():
+    # reading R10 (NEXT-3): W = K - r dK/dr inside the zones; a dense ring and Eq. 1 as printed put
+    # thousands of pairs there, also in TP2 mode
+    w = clustered(13, 800)
+    for extra in (dict(), dict(n1=3.0, n2=0.4, pair_rule=B.PAIR_MAX), dict(n_big=9)):
+        p = oparams(w, weight_mode=1, **extra)
+        vd = oracle.to_democratic(w.m, w.v, w.M_star)
+        ao = oracle.accel(w.m, w.x, vd, p)
+        a0 = oracle.accel(w.m, w.x, vd, oparams(w, **extra))
+        assert rel_err(ao, a0).max() > 1e-2                        # the two weights really differ here
+        po = oracle.encounter_pairs(w.m, w.x, vd, p)
+        for prec, tol in ((B.FP64, 1e-12), (B.FP32, 1e-4)):
+            g = B.from_workload(w, weight_mode=1, pair_capacity=4 * len(po) + 64, **extra)
+            g.accel(prec)
+            a = g.get_accel().cpu().numpy()
+            pairs = g.encounter_pairs()
+            g.close()
+            assert rel_err(a, ao).max() <= tol, (extra, prec, rel_err(a, ao).max())
+            assert pair_set(pairs) == pair_set(po)
