@@ -44,53 +44,77 @@ __device__ __forceinline__ double block_sum(double v, double* sh)
     return t;    // valid in thread 0
 }
 
-// Block b owns i-tiles b and T-1-b (equal total work for every block): sum over j > i of
-// G m_j / r_ij, times m_i, summed over the block -> red[8 + b].
-__global__ void __launch_bounds__(ET)
+// Pair potential sum_{i<j} G m_i m_j / r_ij over the upper triangle of 128 x 128 tiles.  The tile
+// pairs (ti <= tj), linearised row by row, are split evenly over the blocks; a thread holds one
+// i-body of the current row tile and walks the j-tile in shared memory (four independent chains).
+// TP2 mode: only pairs with i < n_big or j < n_big count (reading R9); tile pairs without any are
+// skipped.  Block b writes red[8 + b]; fixed assignment and order: bitwise reproducible.
+__device__ __forceinline__ void tile_of(long long u, int T, int& ti, int& tj)
+{
+    // row ti starts at S(ti) = ti T - ti (ti - 1) / 2; invert with a float guess, then correct
+    const double B = 2.0 * T + 1.0;
+    int t = (int)((B - sqrt(fmax(B * B - 8.0 * (double)u, 0.0))) * 0.5);
+    if (t < 0) t = 0;
+    if (t > T - 1) t = T - 1;
+    while (t > 0 && (long long)t * T - (long long)t * (t - 1) / 2 > u) --t;
+    while (t < T - 1 && (long long)(t + 1) * T - (long long)(t + 1) * t / 2 <= u) ++t;
+    ti = t;
+    tj = t + (int)(u - ((long long)t * T - (long long)t * (t - 1) / 2));
+}
+
+__global__ void __launch_bounds__(ET, 8)
 pairpot_kernel(int N, int T, double G, int n_big, const double* __restrict__ x, const double* __restrict__ m,
                double* __restrict__ red)
 {
     __shared__ double4 sj[ET];
     __shared__ double sh[32];
     const int tid = threadIdx.x;
-    const int tA = blockIdx.x, tB = T - 1 - blockIdx.x;
-    const int iA = tA * ET + tid, iB = tB * ET + tid;
-    const bool hasB = tB > tA;
-    const int iBB = hasB ? iB : iA;
-    const double4 qA = make_double4(x[3 * iA], x[3 * iA + 1], x[3 * iA + 2], 0.0);
-    const double4 qB = make_double4(x[3 * iBB], x[3 * iBB + 1], x[3 * iBB + 2], 0.0);
-    double potA = 0.0, potB = 0.0;
-
-    for (int tj = tA; tj < T; ++tj) {
+    const long long U = (long long)T * (T + 1) / 2;
+    const long long u0 = U * blockIdx.x / gridDim.x, u1 = U * (blockIdx.x + 1) / gridDim.x;
+    double part = 0.0;
+    int ti = -1, tj = 0, i = 0;
+    double xi = 0, yi = 0, zi = 0, mi = 0;
+    for (long long u = u0; u < u1; ++u) {
+        int nti, ntj;
+        if (ti < 0 || tj + 1 >= T) tile_of(u, T, nti, ntj); else { nti = ti; ntj = tj + 1; }
+        if (nti != ti) {
+            ti = nti; i = ti * ET + tid;
+            xi = x[3 * i]; yi = x[3 * i + 1]; zi = x[3 * i + 2];
+            mi = (i < N) ? m[i] : 0.0;
+        }
+        tj = ntj;
+        if (ti * ET >= n_big && tj * ET >= n_big) continue;          // TP2: no interacting pair in this tile pair
         __syncthreads();
         {
             const int j = tj * ET + tid;
             sj[tid] = make_double4(x[3 * j], x[3 * j + 1], x[3 * j + 2], G * m[j]);
         }
         __syncthreads();
-        const bool doB = hasB && tj >= tB;
         const int jbase = tj * ET;
-#pragma unroll 4
-        for (int jj = 0; jj < ET; ++jj) {
-            const double4 J = sj[jj];
-            const int j = jbase + jj;
-            {
-                const double dx = J.x - qA.x, dy = J.y - qA.y, dz = J.z - qA.z;
-                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                const double y  = rsqrt_refined(r2);
-                potA = (j > iA && (iA < n_big || j < n_big)) ? fma(J.w, y, potA) : potA;   // TP2: interacting pairs only
+        const bool plain = (tj > ti) && (jbase + ET <= n_big || ti * ET + ET <= n_big);   // every pair counts
+        double p0 = 0.0, p1 = 0.0, p2 = 0.0, p3 = 0.0;
+        if (plain) {
+#pragma unroll 2
+            for (int jj = 0; jj < ET; jj += 4) {
+                const double4 J0 = sj[jj], J1 = sj[jj + 1], J2 = sj[jj + 2], J3 = sj[jj + 3];
+                double dx, dy, dz;
+                dx = J0.x - xi; dy = J0.y - yi; dz = J0.z - zi; p0 = fma(J0.w, rsqrt_refined(fma(dz, dz, fma(dy, dy, dx * dx))), p0);
+                dx = J1.x - xi; dy = J1.y - yi; dz = J1.z - zi; p1 = fma(J1.w, rsqrt_refined(fma(dz, dz, fma(dy, dy, dx * dx))), p1);
+                dx = J2.x - xi; dy = J2.y - yi; dz = J2.z - zi; p2 = fma(J2.w, rsqrt_refined(fma(dz, dz, fma(dy, dy, dx * dx))), p2);
+                dx = J3.x - xi; dy = J3.y - yi; dz = J3.z - zi; p3 = fma(J3.w, rsqrt_refined(fma(dz, dz, fma(dy, dy, dx * dx))), p3);
             }
-            if (doB) {
-                const double dx = J.x - qB.x, dy = J.y - qB.y, dz = J.z - qB.z;
-                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                const double y  = rsqrt_refined(r2);
-                potB = (j > iB && (iB < n_big || j < n_big)) ? fma(J.w, y, potB) : potB;
+        } else {
+#pragma unroll 4
+            for (int jj = 0; jj < ET; ++jj) {
+                const double4 J = sj[jj];
+                const int j = jbase + jj;
+                const double dx = J.x - xi, dy = J.y - yi, dz = J.z - zi;
+                const double y  = rsqrt_refined(fma(dz, dz, fma(dy, dy, dx * dx)));
+                p0 = (j > i && (i < n_big || j < n_big)) ? fma(J.w, y, p0) : p0;
             }
         }
+        part = fma(mi, (p0 + p1) + (p2 + p3), part);
     }
-    double part = 0.0;
-    if (iA < N) part += m[iA] * potA;
-    if (hasB && iB < N) part += m[iB] * potB;
     const double tot = block_sum(part, sh);
     if (tid == 0) red[8 + blockIdx.x] = tot;
 }
@@ -130,7 +154,10 @@ energy_final_kernel(int N, int nparts, double G, double M_star, const double* __
 void launch_energy(const Handle* h)
 {
     const int T = h->NP / ET;
-    const int nblk = (T + 1) / 2;
+    long long want = (long long)T * (T + 1) / 2;
+    int nblk = h->num_sms * 16;
+    if (nblk > 4096) nblk = 4096;                        // partials red[8 .. 8 + 4096)
+    if (nblk > want) nblk = (int)want;
     if (nblk > 0)
         pairpot_kernel<<<nblk, ET, 0, h->stream>>>(h->N, T, h->p.G, (h->p.n_big >= 0 && h->p.n_big < h->N) ? h->p.n_big : h->N,
                                                    h->w.x, h->w.m, h->w.red);
