@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--report", action="store_true",
                     help="run every BASELINE.json config (0-4) for its full step count in both precisions and print one "
                          "JSON line per (config, precision): rates, fractions of peak, dE/E, dL/L, encounter counts")
+    ap.add_argument("--variant32", type=int, default=None, help="with --no-autotune: FP32 kernel variant (genga_set_tuning key 0)")
+    ap.add_argument("--variant64", type=int, default=None, help="with --no-autotune: FP64 kernel variant (genga_set_tuning key 1)")
     ap.add_argument("--no-autotune", action="store_true", help="keep the default kernel variants (no start-up self-tuning)")
     return ap.parse_args()
 
@@ -277,7 +279,12 @@ def run_cuda(args):
     with sampler:
         for prec, name in ((B.FP32, "fp32"), (B.FP64, "fp64")):
             g = B.from_workload(w, device=dev)
-            tuned[name] = g.autotune(prec) if not args.no_autotune else (0, None)   # start-up self-tuning, untimed
+            if not args.no_autotune:
+                tuned[name] = g.autotune(prec)                 # start-up self-tuning, untimed
+            else:
+                fixed = args.variant32 if prec == B.FP32 else args.variant64
+                tuned[name] = (fixed if fixed is not None else 0, None)
+                g.set_tuning(0 if prec == B.FP32 else 1, tuned[name][0])
             g.set_profiling(1)                         # CUDA events around the all-pairs kernel only
             r = time_steps(torch, g, w, prec, args.steps, args.warmup, flush, dist)
             st = g.nearfield_stats()

@@ -35,7 +35,8 @@ __global__ void pad_kernel(int N, int NP, double* __restrict__ m, double* __rest
 // the mean first (their large r_crit then stays in a few chunks), then along a Hilbert curve over
 // the x-y plane (the discs are thin).  The order is a performance hint only: every bound is
 // computed from the actual chunk contents, so results never depend on it beyond summation order.
-// key = [light:1][Hilbert index:30][0][body index:32]: distinct keys, so ranks are a permutation.
+// key = [class:2][Hilbert index:30][body index:32], class 0 heavy, 1 ordinary, 2 massless (test particles
+// last, so that they share few chunks); distinct keys, so ranks are a permutation.
 constexpr int SORT_BITS = 13;                       // buckets = leading key bits: class + 12 Hilbert bits
 constexpr int SORT_NB   = 1 << SORT_BITS;
 
@@ -80,8 +81,9 @@ __global__ void sortkey_kernel(int N, double M_star, const double* __restrict__ 
     const float fy = fminf(fmaxf(fmaf((float)x[3 * i + 1], sc, 16383.5f), 0.f), 32767.f);
     const unsigned int cx = (fx == fx) ? (unsigned int)fx : 0u, cy = (fy == fy) ? (unsigned int)fy : 0u;
     const double href = cbrt(red[3] / ((double)N * 3.0 * M_star));      // Hill factor of the mean mass
-    const unsigned long long light = (hcbrt[i] > 1.5 * href) ? 0ull : 1ull;
-    const unsigned long long key = (light << 63) | ((unsigned long long)hilbert_xy2d(cx, cy) << 33) | (unsigned int)i;
+    const double hi = hcbrt[i];
+    const unsigned long long cls = (hi > 1.5 * href) ? 0ull : ((hi > 0.0) ? 1ull : 2ull);
+    const unsigned long long key = (cls << 62) | ((unsigned long long)hilbert_xy2d(cx, cy) << 32) | (unsigned int)i;
     keys[i] = key;
     atomicAdd(&hist[(unsigned int)(key >> (64 - SORT_BITS))], 1u);
 }
