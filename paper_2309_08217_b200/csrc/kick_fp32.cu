@@ -55,7 +55,7 @@ constexpr float EPS2 = 1.0e-30f;   // added to r^2 so that the self pair (d = 0 
 // One j-chunk against the I i-bodies of this thread.  SELF: the chunk holds this warp's own
 // slots; the self pair is then left out of the smallest-r^2 tracking (slot index compare), so a
 // body's own chunk is flagged only if a DIFFERENT body is near.
-template <int I, int UNR, bool SELF, bool SC>
+template <int I, int UNR, bool SELF, bool SC, bool FAR>
 __device__ __forceinline__ void pair_loop(const float4* __restrict__ jp, const float (&nx)[I], const float (&ny)[I],
                                           const float (&nz)[I], f2 (&ax)[I], f2 (&ay)[I], f2 (&az)[I],
                                           float (&mn)[I], const int (&self_off)[I])
@@ -82,7 +82,7 @@ __device__ __forceinline__ void pair_loop(const float4* __restrict__ jp, const f
                 ya = rsq(r2a); yb = rsq(r2b);
                 if (SC) { ya = sa ? 0.f : ya; yb = sb ? 0.f : yb; }   // D_self is rounding residue, not 0
             } else {
-                mn[k] = min3(mn[k], r2a, r2b);
+                if (!FAR) mn[k] = min3(mn[k], r2a, r2b);      // FAR: the chunk's bounding sphere is out of reach
                 ya = rsq(r2a); yb = rsq(r2b);
             }
             const f2 y = pk(ya, yb);
@@ -196,16 +196,28 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                     self_off[k] = ib * BI + k * NT + tid - (cs + ch) * CHUNK;
                     self = self || (self_off[k] >= 0 && self_off[k] < CHUNK);
                 }
-                if (self) pair_loop<I, UNR, true, SC>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
-                else      pair_loop<I, UNR, false, SC>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
-
-                // ---- chunk end: keep the FP32 partial or hand the chunk to the near field ----
-                const float Hc = Bc.hq, Ac = Bc.aq, Rc = Bc.rf, Q2 = Bc.q2max;
+                // bound of this (body, chunk) and the sphere test: if every body of the warp is farther from the
+                // chunk's frame origin than bound + chunk radius, no pair of the chunk can be near (triangle
+                // inequality), and the loop without the smallest-r^2 tracking runs (one instruction less per two pairs)
+                const float Hc = Bc.hq, Ac = Bc.aq, Rc = Bc.rf, Q2 = Bc.q2max, Rad = Bc.rad;
+                float Bq[I];
+                bool far = true;
 #pragma unroll
                 for (int k = 0; k < I; ++k) {
-                    const float Bq = fmaxf(fmaxf(sm.bp[0][k][tid], Hc) * fmaxf(sm.bp[1][k][tid], Ac),
-                                           fmaxf(sm.bp[2][k][tid], Rc));
-                    const float bound = (ib * BI + k * NT + tid < N) ? (SC ? Bq * Bq * Q2 : Bq * Bq) : -1.0f;
+                    Bq[k] = fmaxf(fmaxf(sm.bp[0][k][tid], Hc) * fmaxf(sm.bp[1][k][tid], Ac), fmaxf(sm.bp[2][k][tid], Rc));
+                    const float reach = (Bq[k] + Rad) * 1.000004f;
+                    const float d2 = fmaf(nz[k], nz[k], fmaf(ny[k], ny[k], nx[k] * nx[k]));
+                    far = far && ((d2 > reach * reach) || (ib * BI + k * NT + tid >= N));
+                }
+                far = __all_sync(0xffffffffu, far);
+                if (self)     pair_loop<I, UNR, true, SC, false>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
+                else if (far) pair_loop<I, UNR, false, SC, true>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
+                else          pair_loop<I, UNR, false, SC, false>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
+
+                // ---- chunk end: keep the FP32 partial or hand the chunk to the near field ----
+#pragma unroll
+                for (int k = 0; k < I; ++k) {
+                    const float bound = (ib * BI + k * NT + tid < N) ? (SC ? Bq[k] * Bq[k] * Q2 : Bq[k] * Bq[k]) : -1.0f;
                     const bool keep = mn[k] > bound;
                     float lo, hi;
                     upk(ax[k], lo, hi); const float px = lo + hi;

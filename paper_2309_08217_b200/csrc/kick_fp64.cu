@@ -23,7 +23,7 @@ constexpr double EPS2 = 1.0e-60;   // added to r^2 so that the self pair (d = 0 
 // One j-chunk against the I i-bodies of this thread.  SELF: the chunk holds this warp's own slots;
 // the self pair is left out of the smallest-r^2 tracking, so a body's own chunk is flagged only if
 // a DIFFERENT body is near.  mn tracks the high word of r^2 (orders like r^2 >= 0).
-template <int I, int UNR, bool SELF>
+template <int I, int UNR, bool SELF, bool FAR>
 __device__ __forceinline__ void pair_loop(const double4* __restrict__ jp, const double (&xi)[I], const double (&yi)[I],
                                           const double (&zi)[I], double (&ax)[I], double (&ay)[I], double (&az)[I],
                                           int (&mn)[I], const int (&self_off)[I])
@@ -40,7 +40,7 @@ __device__ __forceinline__ void pair_loop(const double4* __restrict__ jp, const 
             r2 = fma(dy, dy, r2);
             r2 = fma(dz, dz, r2);
             if (SELF) mn[k] = min(mn[k], (jj == self_off[k]) ? 0x7fffffff : __double2hiint(r2));
-            else      mn[k] = min(mn[k], __double2hiint(r2));
+            else if (!FAR) mn[k] = min(mn[k], __double2hiint(r2));   // FAR: the chunk's bounding sphere is out of reach
             const double y0 = rsq64h(r2);
             const double t  = y0 * y0;
             const double e  = fma(-r2, t, 1.0);
@@ -138,13 +138,27 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                     self_off[k] = ib * BI + k * NT + tid - (cs + ch) * CHUNK;
                     self = self || (self_off[k] >= 0 && self_off[k] < CHUNK);
                 }
-                if (self) pair_loop<I, UNR, true>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
-                else      pair_loop<I, UNR, false>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
+                // sphere test (as in the FP32 kernel): every body of the warp farther from the chunk's frame origin
+                // than bound + chunk radius => no near pair in this chunk, the loop without the min tracking runs
+                float Bqk[I];
+                bool far = true;
+#pragma unroll
+                for (int k = 0; k < I; ++k) {
+                    Bqk[k] = fmaxf(fmaxf(sm.bp[0][k][tid], Bc.hq) * fmaxf(sm.bp[1][k][tid], Bc.aq),
+                                   fmaxf(sm.bp[2][k][tid], Bc.rf));
+                    const double reach = ((double)Bqk[k] + (double)Bc.rad) * 1.000001;
+                    const double ex = xi[k] - Bc.ox, ey = yi[k] - Bc.oy, ez = zi[k] - Bc.oz;
+                    const double d2 = fma(ez, ez, fma(ey, ey, ex * ex));
+                    far = far && ((d2 > reach * reach) || (ib * BI + k * NT + tid >= N));
+                }
+                far = __all_sync(0xffffffffu, far);
+                if (self)     pair_loop<I, UNR, true, false>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
+                else if (far) pair_loop<I, UNR, false, true>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
+                else          pair_loop<I, UNR, false, false>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
 
 #pragma unroll
                 for (int k = 0; k < I; ++k) {
-                    const float Bq = fmaxf(fmaxf(sm.bp[0][k][tid], Bc.hq) * fmaxf(sm.bp[1][k][tid], Bc.aq),
-                                           fmaxf(sm.bp[2][k][tid], Bc.rf));
+                    const float Bq = Bqk[k];
                     // bound in FP64, rounded up by one FP32 ulp-ish factor; compare high words only:
                     // equal high words count as "near" (conservative).
                     const double bd = (double)Bq * (double)Bq * 1.000001;
