@@ -303,7 +303,7 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     h->near_floor  = p->near_floor >= 0.0 ? p->near_floor : (1.0 / 256.0);
     if (h->lambda_near < 1.0) h->lambda_near = 1.0;
     h->pair_cap = pc; h->cand_cap = cc;
-    h->resort_every = p->resort_every > 0 ? p->resort_every : 32;
+    h->resort_every = p->resort_every > 0 ? p->resort_every : 8;
     h->evals_since_sort = -1;
     h->stream = static_cast<cudaStream_t>(p->stream);
     h->num_sms = sms;

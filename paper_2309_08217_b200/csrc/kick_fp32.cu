@@ -265,13 +265,13 @@ struct Variant32 { kick32_fn fn; int nt; int bi; size_t smem; bool scaled; const
       "I" #I_ " NT" #NT_ " minB" #MINB_ " accS" #ACCS_ " unr" #UNR_ " scaled" #SC_ }
 
 const Variant32 g_variants32[] = {
-    V32(2, 256, 2, true, 2, false),      // 0: default.  Plain j-records (x - o, G m): robust for any mass spectrum
-    V32(2, 256, 2, false, 4, false),
-    V32(2, 256, 2, false, 2, false),
+    V32(2, 256, 2, false, 4, false),     // 0: default.  Plain j-records (x - o, G m): robust for any mass spectrum
+    V32(2, 256, 2, true, 2, false),
     V32(2, 128, 4, false, 4, false),
-    V32(2, 256, 2, true, 4, true),       // 4: mass-scaled j-records, 11 instead of 12 FMA-pipe operations per pair;
-    V32(1, 512, 1, false, 4, true),      //    usually the fastest for discs of comparable masses (genga_autotune picks it);
-    V32(2, 256, 2, false, 4, true),      //    chunks holding massless bodies are always handed to the FP64 near field
+    V32(2, 256, 2, false, 4, true),      // 3: mass-scaled j-records, 11 instead of 12 FMA-pipe operations per pair;
+    V32(2, 256, 2, true, 4, true),       //    usually the fastest for discs of comparable masses (genga_autotune picks it);
+    V32(2, 128, 4, false, 4, true),      //    chunks holding massless bodies are always handed to the FP64 near field
+    V32(1, 512, 1, false, 4, true),
 };
 constexpr int NVAR32 = (int)(sizeof(g_variants32) / sizeof(g_variants32[0]));
 const Variant32& variant32(int v)

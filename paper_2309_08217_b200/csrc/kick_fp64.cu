@@ -196,12 +196,11 @@ struct Variant64 { kick64_fn fn; int nt; int bi; size_t smem; const char* name; 
     { kick64_kernel<I_, NT_, MINB_, UNR_>, NT_, I_ * NT_, sizeof(Smem64<I_, NT_>), "I" #I_ " NT" #NT_ " minB" #MINB_ " unr" #UNR_ }
 
 const Variant64 g_variants64[] = {
-    V64(2, 256, 1, 4),            // 0: default
+    V64(2, 256, 2, 8),            // 0: default
     V64(2, 256, 2, 4),
-    V64(2, 256, 2, 8),
+    V64(2, 256, 1, 4),
     V64(2, 128, 3, 4),
     V64(1, 256, 3, 8),
-    V64(4, 64, 6, 2),
 };
 constexpr int NVAR64 = (int)(sizeof(g_variants64) / sizeof(g_variants64[0]));
 const Variant64& variant64(int v)
