@@ -329,7 +329,8 @@ def run_cuda(args):
         return {"pair_interactions_per_s": pps, "steps_per_s": K / (total_ms * 1e-3),
                 "body_steps_per_s": world * N * K / (total_ms * 1e-3), "ms_per_step": total_ms / K,
                 "kernel_ms": {"kick": r["kernel_ms"][0], "nearfield": r["kernel_ms"][1],
-                              "prep": r["kernel_ms"][2], "drift": r["kernel_ms"][3]},
+                              "onbody_fused": r["kernel_ms"][3],      # velocity update + S D S + r_crit/packing, one kernel
+                              "prep_alone": r["kernel_ms"][2]},        # 0 unless a force evaluation ran outside a step
                 "kick_kernel_pairs_per_s": pairs / (kick_ms * 1e-3),
                 "kick_kernel_tflops": tf, "kick_kernel_frac_of_peak": tf / peak,
                 "step_frac_of_peak": flop * pairs * K / (total_ms * 1e-3) / 1e12 / peak,

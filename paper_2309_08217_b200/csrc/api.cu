@@ -226,6 +226,7 @@ static int sequence(genga_handle h, int precision, bool lead_kick, double tau_fi
     int rc;
     if (h->N == 0) return GENGA_OK;
     if (h->fused_blocks <= 0) {                                     // no cooperative launch: the un-fused kernels
+        if (h->pend_vel) return GENGA_EINVAL;                       // cannot happen: only the fused path defers
         if (lead_kick && (rc = kick_fused(h, tau_first, precision, 0.0)) != GENGA_OK) return rc;
         for (int k = 0; k < n_sds; ++k) {
             if ((rc = sd_fused(h, dt)) != GENGA_OK) return rc;
@@ -233,10 +234,13 @@ static int sequence(genga_handle h, int precision, bool lead_kick, double tau_fi
         }
         return GENGA_OK;
     }
-    bool pending = false;
-    double tau_prev = 0.0;
+    // The closing velocity update of a sequence is DEFERRED (h->pend_vel): it rides in the first per-body
+    // kernel of the next sequence, or is flushed by the first call that reads or replaces the state.
+    bool pending = h->pend_vel;
+    double tau_prev = h->pend_tau;
+    h->pend_vel = false;
     if (lead_kick) {
-        if ((rc = onbody(h, precision, false, 0.0, false, 0.0, true)) != GENGA_OK) return rc;
+        if ((rc = onbody(h, precision, pending, tau_prev, false, 0.0, true)) != GENGA_OK) return rc;
         if ((rc = launch_pairs(h, precision)) != GENGA_OK) return rc;
         pending = true; tau_prev = tau_first;
     }
@@ -245,8 +249,16 @@ static int sequence(genga_handle h, int precision, bool lead_kick, double tau_fi
         if ((rc = launch_pairs(h, precision)) != GENGA_OK) return rc;
         pending = true; tau_prev = (k == n_sds - 1) ? tau_last : tau_mid;
     }
-    if (pending) return onbody(h, precision, true, tau_prev, false, 0.0, false);
+    if (pending) { h->pend_vel = true; h->pend_tau = tau_prev; h->mom_a_valid = false; }
     return GENGA_OK;
+}
+
+// Apply a deferred velocity update (see sequence()).  Called by everything that reads or replaces x, v.
+static int flush_pending(genga_handle h)
+{
+    if (!h->pend_vel) return GENGA_OK;
+    h->pend_vel = false;
+    return onbody(h, GENGA_FP64, true, h->pend_tau, false, 0.0, false);
 }
 
 extern "C" {
@@ -338,6 +350,7 @@ int genga_destroy(genga_handle h)
 static int set_state_impl(genga_handle h, const double* m, const double* x, const double* v, cudaMemcpyKind kind)
 {
     if (!h) return GENGA_EINVAL;
+    { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     const size_t n = (size_t)h->N;
     if (n == 0) return GENGA_OK;
     if (m) CU(cudaMemcpyAsync(h->w.m, m, n * 8, kind, h->stream));
@@ -362,12 +375,14 @@ int genga_set_state_host(genga_handle h, const double* m, const double* x, const
 int genga_resort(genga_handle h)
 {
     if (!h) return GENGA_EINVAL;
+    { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     return resort(h);
 }
 
 int genga_accel(genga_handle h, int precision)
 {
     if (!h) return GENGA_EINVAL;
+    { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     return force_eval(h, precision);
 }
 
@@ -380,6 +395,7 @@ int genga_kick(genga_handle h, double dt, int precision)
 int genga_drift(genga_handle h, double dt)
 {
     if (!h) return GENGA_EINVAL;
+    { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     { ProfScope ps(h, 3); launch_drift(h, dt); }
     LAUNCHED(h, "drift_kernel");
     h->mom_a_valid = false;
@@ -389,6 +405,7 @@ int genga_drift(genga_handle h, double dt)
 int genga_sunkick(genga_handle h, double tau)
 {
     if (!h) return GENGA_EINVAL;
+    { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     if (h->N == 0) return GENGA_OK;
     launch_momentum(h); LAUNCHED(h, "momentum_kernel");
     launch_sunkick(h, tau); LAUNCHED(h, "sunkick_kernel");
@@ -436,6 +453,7 @@ int genga_encounter_pairs(genga_handle h, int* pairs_ij, int cap, int* count)
 int genga_energy_angmom(genga_handle h, double* E, double L[3])
 {
     if (!h || !E || !L) return GENGA_EINVAL;
+    { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     launch_energy(h); h->launches += 2;
     { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_, "energy kernels"); }
     double r[4];
@@ -448,6 +466,7 @@ int genga_energy_angmom(genga_handle h, double* E, double L[3])
 static int get_state_impl(genga_handle h, double* x, double* v, int helio, cudaMemcpyKind kind)
 {
     if (!h) return GENGA_EINVAL;
+    { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     const size_t n = (size_t)h->N;
     if (n == 0) return GENGA_OK;
     if (x) CU(cudaMemcpyAsync(x, h->w.x, n * 24, kind, h->stream));
@@ -577,6 +596,7 @@ int genga_set_tuning(genga_handle h, int key, int value)
 int genga_autotune(genga_handle h, int precision, int* chosen, double* ms_best)
 {
     if (!h || (precision != GENGA_FP64 && precision != GENGA_FP32)) return GENGA_EINVAL;
+    { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     const int key = precision == GENGA_FP32 ? 0 : 1;
     const int n = key == 0 ? kick32_num_variants() : kick64_num_variants();
     if (h->N == 0) { if (chosen) *chosen = h->tune[key]; if (ms_best) *ms_best = 0.0; return GENGA_OK; }

@@ -86,6 +86,8 @@ struct Handle {
     long long launches;
     // internal order (a performance hint only: results never depend on it)
     int fused_blocks;            // co-resident blocks of the fused per-body kernel; 0 = cooperative launch unavailable
+    bool pend_vel;               // a closing velocity update v += pend_tau a is still owed (api.cu: sequence)
+    double pend_tau;
     bool mom_a_valid;            // mom[SLOT_A] holds sum m v of the stored velocities
     int grid_cache[2][2];        // per kernel (FP32, FP64): variant + 1 it was computed for, grid size
     int tune[4];                 // genga_set_tuning: [0] kick32 variant, [1] kick64 variant
