@@ -353,11 +353,11 @@ def run_cuda(args):
         "precisions": {"fp32": p32, "fp64": p64},
         "roofline": {"bound": "alu", "kernel": "kick32_kernel", "achieved": p32["kick_kernel_tflops"],
                      "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s", "frac": p32["kick_kernel_frac_of_peak"],
-                     "traffic": 3.745e6,      # dram bytes read + written per kick32 launch (profiles/r1c, ncu --set full)
+                     "traffic": 3.742e6,      # dram bytes read + written per kick32 launch (profiles/r1d, ncu --set full)
                      "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md section 6); "
                                     "MEASURED_PEAKS.json has no FP32/FP64 ALU figure",
                      "flop_per_pair": FLOP_FP32,
-                     "fp64": {"kernel": "kick64_kernel", "traffic": 3.095e6, "achieved": p64["kick_kernel_tflops"],
+                     "fp64": {"kernel": "kick64_kernel", "traffic": 3.111e6, "achieved": p64["kick_kernel_tflops"],
                               "peak": PEAK_FP64_TFLOPS, "frac": p64["kick_kernel_frac_of_peak"],
                               "flop_per_pair": FLOP_FP64}},
         "e2e": {"value": whole_job_rate(world, pairs, e2e_steps, te32), "unit": UNIT,
