@@ -135,7 +135,6 @@ void launch_kick32(const Handle* h);
 void launch_kick64(const Handle* h);
 void launch_nearfield(const Handle* h);
 void launch_tp2(const Handle* h);                            // TP2 mode: big bodies against all (FP64)
-void launch_velupdate(const Handle* h, double tau);
 void launch_momentum(const Handle* h);                       // red[0..2] = sum m v, red[3] = sum m
 void launch_momentum_slot_a(const Handle* h);                // the same into mom[SLOT_A]
 void launch_velupdate_mom(const Handle* h, double tau);      // v += tau a; mom[SLOT_A] = sum m v

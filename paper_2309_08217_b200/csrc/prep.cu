@@ -150,13 +150,6 @@ prep_kernel(PrepArgs A, Workspace w)
               sc * w.mom[MOM_SLOT_B + 2]);
 }
 
-// O7: v_i += tau a_i
-__global__ void velupdate_kernel(int n3, double tau, const double* __restrict__ a, double* __restrict__ v)
-{
-    int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k < n3) v[k] = fma(tau, a[k], v[k]);
-}
-
 // out[0..2] = sum_j m_j v_j, out[3] = sum_j m_j (momentum.cuh: fixed-tree, last block combines).
 constexpr int MOM_NT = 256;
 
@@ -247,13 +240,6 @@ void launch_prep(const Handle* h, const PrepArgs& a)
 {
     if (h->NP == 0) return;
     prep_kernel<<<h->NP / PREP_NT, PREP_NT, 0, h->stream>>>(a, h->w);
-}
-
-void launch_velupdate(const Handle* h, double tau)
-{
-    if (h->N == 0) return;
-    const int n3 = 3 * h->N;
-    velupdate_kernel<<<(n3 + 255) / 256, 256, 0, h->stream>>>(n3, tau, h->w.a, h->w.v);
 }
 
 static int momentum_blocks(const Handle* h)

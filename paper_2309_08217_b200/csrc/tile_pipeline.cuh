@@ -51,11 +51,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
 
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-
 // Append (body, chunk) for every lane with flag set; one atomic per warp (__ballot_sync + popc).
 // Must be executed by all 32 lanes.  Entries past the capacity are dropped; the count keeps
 // growing so that the near-field kernel can see the overflow and take the exact path.
@@ -71,15 +66,6 @@ __device__ __forceinline__ void push_candidates(unsigned int ballot, bool flag, 
         const unsigned int idx = base + __popc(ballot & ((1u << lane) - 1u));
         if (idx < cap) list[idx] = make_int2(body, chunk);
     }
-}
-
-// Static partition of the (i-block, chunk) unit grid over the CTAs: CTA b owns units
-// [b U / G, (b+1) U / G) of the i-block-major linearisation.
-__device__ __forceinline__ void unit_range(long long U, int& ib, int& c0, long long& u0, long long& u1)
-{
-    u0 = (U * (long long)blockIdx.x) / (long long)gridDim.x;
-    u1 = (U * (long long)(blockIdx.x + 1)) / (long long)gridDim.x;
-    ib = 0; c0 = 0;
 }
 
 }  // namespace genga
