@@ -2,16 +2,20 @@
 // "Do Kick in single precision = 1").
 //
 // a_i = sum_{j != i} G m_j (x_j - x_i) / r_ij^3 over FAR pairs, mixed-precision policy P32
-// (DESIGN.md section 3): separations from FP32-rounded positions, packed FP32 arithmetic
-// (FFMA2/FADD2/FMUL2: two j-bodies per instruction), MUFU.RSQ, FP32 partial sums over one
-// 64-body j-chunk, chunk partials accumulated in FP64.  A (body, chunk) whose smallest r^2 is
-// not above the conservative bound (lambda * r_crit upper bound, position-rounding floor) is NOT
-// added: it is pushed to the candidate list and re-evaluated pair by pair in FP64 with the
-// changeover function by the near-field kernel (encounter forces always in FP64).
+// (DESIGN.md section 3): positions relative to the origin of each 128-body j-chunk (FP64
+// subtraction, one rounding to FP32), packed FP32 arithmetic (FFMA2/FADD2/FMUL2: two j-bodies per
+// instruction), MUFU.RSQ, FP32 partial sums over one chunk, chunk partials accumulated in FP64.
+// A (body, chunk) whose smallest r^2 (own slot left out) is not above the conservative bound
+// (lambda * r_crit upper bound, frame guard) is NOT added: it is pushed to the candidate list and
+// re-evaluated pair by pair in FP64 with the changeover function by the near-field kernel
+// (encounter forces always in FP64).  Chunks whose bounding sphere is out of reach of
+// every body of the warp run a copy of the loop without the smallest-r^2 tracking.
 //
-// Layout: 4 i-bodies per thread in registers; j-bodies streamed through shared memory in
-// 512-body stages by bulk asynchronous copies; one CTA owns a contiguous run of (i-block, chunk)
-// units so that 148 x occupancy CTAs carry equal work.
+// Layout: I i-bodies per thread (FP64 positions and bound parameters in shared memory); j-bodies
+// streamed through shared memory in 1024-body stages by bulk asynchronous copies (cp.async.bulk ->
+// UBLKCP, mbarrier completion, double buffered); one CTA owns a contiguous run of (i-block, chunk)
+// units so that 148 x occupancy CTAs carry equal work.  Variants (genga_set_tuning / genga_autotune)
+// differ in I, threads, registers, unroll, and plain vs mass-scaled j-records.
 #include "tile_pipeline.cuh"
 
 namespace genga {

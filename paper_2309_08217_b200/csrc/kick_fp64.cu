@@ -4,7 +4,7 @@
 // operation in FP64.  1/r^3 comes from the 20-bit MUFU.RSQ64H seed y0 and one cubic correction:
 //   t = y0^2, e = 1 - r^2 t, 1/r^3 = y0^3 (1 - e)^(-3/2) = y0^3 (1 + 3/2 e + 15/8 e^2) + O(e^3),
 // |e| <~ 2^-19 so the truncation is < 1e-17 relative.  16 FP64-pipe
-// instructions per pair.  A (body, 64-j chunk) whose smallest r^2 is not above the conservative
+// instructions per pair.  A (body, 128-j chunk) whose smallest r^2 (own slot left out) is not above the conservative
 // r_crit bound is not added but handed to the near-field kernel, which applies K pair by pair.
 #include "tile_pipeline.cuh"
 

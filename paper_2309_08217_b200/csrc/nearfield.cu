@@ -4,8 +4,8 @@
 // close-encounter pair list {(i,j): i<j, r_ij < r_crit,ij}, compacted with
 // __ballot_sync + one atomic per warp.
 //
-// One warp per candidate, two j-bodies per lane.  Plain sqrt/divide/cbrt: this path is rare
-// (about N + 2 x near pairs candidates) and must be exact.  If the candidate list overflowed,
+// One warp per candidate, four j-bodies per lane, two phases (cheap K = 1 terms; compacted near
+// pairs with plain sqrt/divide/cbrt: this path is rare and must be exact).  If the candidate list overflowed,
 // the kernel instead evaluates EVERY pair this way (one warp per body, overwriting a_i), so the
 // result never depends on the capacity.
 #include "genga_internal.cuh"
