@@ -415,6 +415,11 @@ def run_report(args):
     cases = [(cfg, W.config(cfg), {}) for cfg in range(5)]
     # NEXT-2: config 3 at the paper's 30 000 planetesimals in TP2 mode
     cases.append(("3-tp2", W.config(3, 30000), {"n_big": 4}))
+    # NEXT-4: Eq. 1 as printed (n1 = 3, n2 = 0.4, max rule) on the performance shape, 50 steps
+    w4 = W.config(4)
+    w4.nsteps = 50
+    cases.append(("4-eq1", w4, {"n1": 3.0, "n2": 0.4, "pair_rule": B.PAIR_MAX,
+                                "pair_capacity": 40 * w4.N, "cand_capacity": 64 * w4.N}))
     for cfg, w, kw in cases:
         nb = kw.get("n_big", -1)
         pairs = w.N * (w.N - 1.0) if nb < 0 else (2.0 * nb * (w.N - nb) + nb * (nb - 1.0))   # interacting ordered pairs
@@ -434,7 +439,7 @@ def run_report(args):
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1)
             E1, L1 = g.energy_angmom()
-            enc_last = int(len(g.encounter_pairs(cap=8 * w.N + 4096)))
+            enc_last = int(len(g.encounter_pairs(cap=max(8 * w.N + 4096, kw.get("pair_capacity", 0)))))
             st = g.nearfield_stats()
             g.close()
             evals = w.nsteps + 1
