@@ -380,6 +380,22 @@ def alu_probes():
     return out
 
 
+def cpu_oracle_kick(w, **kw):
+    """One oracle force evaluation + velocity update (oracle_kick) of workload w on the host cores: the
+    oracle timed beside the GPU per config / per sweep N.  Returns (seconds, pairs/s, threads)."""
+    import oracle
+    pk = dict(G=w.G, M_star=w.M_star, n1=w.n1, n2=w.n2, dt_rcrit=w.dt, pair_rule=w.pair_rule)
+    pk.update({k: v for k, v in kw.items() if k in ("n1", "n2", "pair_rule", "n_big")})
+    p = oracle.Params(**pk)
+    vd = oracle.to_democratic(w.m, w.v, w.M_star)
+    t0 = time.perf_counter()
+    oracle.kick(w.m, w.x.copy(), vd, p, w.dt)
+    dt = time.perf_counter() - t0
+    nb = pk.get("n_big", -1)
+    pairs = w.N * (w.N - 1.0) if nb < 0 else (2.0 * nb * (w.N - nb) + nb * (nb - 1.0))
+    return dt, pairs / dt, oracle.num_threads()
+
+
 def run_sweep(args):
     """N = 2^10 .. 2^17 (BASELINE.json configs[4]): N x steps/s per precision, device-timed."""
     import torch
@@ -400,6 +416,9 @@ def run_sweep(args):
                          "pair_interactions_per_s": n * (n - 1.0) * steps / (r["total_ms"] * 1e-3),
                          "kick_kernel_ms": r["kernel_ms"][0], "nearfield_ms": r["kernel_ms"][1]}
             g.close()
+        if not args.no_cpu_baseline:
+            sec, pps, thr = cpu_oracle_kick(w)
+            row["cpu_oracle_kick"] = {"seconds": sec, "pair_interactions_per_s": pps, "cores": thr}
         out.append(row)
     return out
 
@@ -422,6 +441,10 @@ def run_report(args):
                                 "pair_capacity": 40 * w4.N, "cand_capacity": 64 * w4.N}))
     for cfg, w, kw in cases:
         nb = kw.get("n_big", -1)
+        if not args.no_cpu_baseline:                               # the oracle beside it: one kick per config
+            sec, pps, thr = cpu_oracle_kick(w, **kw)
+            print(json.dumps({"report": "cpu_oracle_kick", "config": cfg, "workload": w.name, "N": w.N, "seconds": sec,
+                              "pair_interactions_per_s": pps, "cores": thr, "kind": "oracle"}), flush=True)
         pairs = w.N * (w.N - 1.0) if nb < 0 else (2.0 * nb * (w.N - nb) + nb * (nb - 1.0))   # interacting ordered pairs
         for prec, name, flop, peak in ((B.FP32, "fp32", FLOP_FP32, PEAK_FP32_TFLOPS), (B.FP64, "fp64", FLOP_FP64, PEAK_FP64_TFLOPS)):
             g = B.from_workload(w, **kw)
