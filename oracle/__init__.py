@@ -175,6 +175,33 @@ def encounter_pairs(m, x, v, p: Params) -> np.ndarray:
         cap = cnt.value
 
 
+def accel_subset(m, x, v, p: Params, sel) -> np.ndarray:
+    """O5 for the bodies ``sel`` only (sampled outputs at large N), shape (len(sel), 3)."""
+    m = _a(m); x = _a(x); v = _a(v)
+    sel = np.ascontiguousarray(sel, dtype=np.int32)
+    a = np.zeros((len(sel), 3))
+    c = p.c()
+    lib().oracle_accel_subset(len(m), _p(m), _p(x), _p(v), ctypes.byref(c), len(sel),
+                              sel.ctypes.data_as(_ip), _p(a))
+    return a
+
+
+def encounter_pairs_subset(m, x, v, p: Params, sel) -> set:
+    """O6 restricted to pairs touching a body of ``sel``: a set of (i, j), i < j."""
+    m = _a(m); x = _a(x); v = _a(v)
+    sel = np.ascontiguousarray(sel, dtype=np.int32)
+    c = p.c()
+    cnt = ctypes.c_int(0)
+    cap = 4096
+    while True:
+        buf = np.zeros((cap, 2), dtype=np.int32)
+        lib().oracle_encounter_pairs_subset(len(m), _p(m), _p(x), _p(v), ctypes.byref(c), len(sel),
+                                            sel.ctypes.data_as(_ip), buf.ctypes.data_as(_ip), cap, ctypes.byref(cnt))
+        if cnt.value <= cap:
+            return set(map(tuple, buf[:cnt.value].tolist()))
+        cap = cnt.value
+
+
 def kick(m, x, v, p: Params, tau: float):
     """O7: returns (v + tau a, a)."""
     m = _a(m); x = _a(x); v = _a(v).copy()

@@ -144,6 +144,30 @@ static int interacts(const oracle_params* p, int i, int j)
     return p->n_big < 0 || i < p->n_big || j < p->n_big;
 }
 
+/* O5 for one body i: sum over j != i, j ascending, Neumaier-compensated. */
+static void accel_one(int N, const double* m, const double* x, const oracle_params* p,
+                      const double* rc, const double* sa, const double* vk, int i, double out[3])
+{
+    nsum a[3] = {{0, 0}, {0, 0}, {0, 0}};
+    for (int j = 0; j < N; ++j) {
+        if (j == i || !interacts(p, i, j)) continue;
+        double dx = x[3 * j + 0] - x[3 * i + 0];
+        double dy = x[3 * j + 1] - x[3 * i + 1];
+        double dz = x[3 * j + 2] - x[3 * i + 2];
+        double r2 = dx * dx + dy * dy + dz * dz;
+        double r  = sqrt(r2);
+        if (!(r > 0.0)) continue;                     /* coincident bodies: W = 0 */
+        double rcij = oracle_pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j]);
+        double W = oracle_weight(r, rcij, p->weight_mode);
+        if (W == 0.0) continue;
+        double s = p->G * m[j] * W / (r2 * r);
+        nsum_add(&a[0], s * dx);
+        nsum_add(&a[1], s * dy);
+        nsum_add(&a[2], s * dz);
+    }
+    for (int k = 0; k < 3; ++k) out[k] = nsum_value(&a[k]);
+}
+
 void oracle_accel(int N, const double* m, const double* x, const double* v,
                   const oracle_params* p, double* acc)
 {
@@ -151,28 +175,52 @@ void oracle_accel(int N, const double* m, const double* x, const double* v,
     double* sa = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
     double* vk = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
     oracle_rcrit(N, m, x, v, p, rc, sa, vk);
-
 #pragma omp parallel for schedule(dynamic, 16)
-    for (int i = 0; i < N; ++i) {
-        nsum a[3] = {{0, 0}, {0, 0}, {0, 0}};
+    for (int i = 0; i < N; ++i) accel_one(N, m, x, p, rc, sa, vk, i, acc + 3 * i);
+    free(rc); free(sa); free(vk);
+}
+
+/* The same for the nsel bodies sel[0..nsel) only (sampled outputs at sizes where all N^2 pairs take too
+ * long on a CPU): acc[k] = a_{sel[k]}.                                                                */
+void oracle_accel_subset(int N, const double* m, const double* x, const double* v,
+                         const oracle_params* p, int nsel, const int* sel, double* acc)
+{
+    double* rc = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* sa = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* vk = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    oracle_rcrit(N, m, x, v, p, rc, sa, vk);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int k = 0; k < nsel; ++k) accel_one(N, m, x, p, rc, sa, vk, sel[k], acc + 3 * k);
+    free(rc); free(sa); free(vk);
+}
+
+/* O6 restricted to the pairs that touch one of the bodies sel[0..nsel): every (i, j), i = sel[k], j != i,
+ * with r_ij < r_crit,ij, written as (min, max); a pair with both ends selected appears twice.         */
+void oracle_encounter_pairs_subset(int N, const double* m, const double* x, const double* v,
+                                   const oracle_params* p, int nsel, const int* sel,
+                                   int* pairs, int cap, int* count)
+{
+    double* rc = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* sa = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* vk = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    oracle_rcrit(N, m, x, v, p, rc, sa, vk);
+    int n = 0;
+    for (int k = 0; k < nsel; ++k) {
+        int i = sel[k];
         for (int j = 0; j < N; ++j) {
             if (j == i || !interacts(p, i, j)) continue;
             double dx = x[3 * j + 0] - x[3 * i + 0];
             double dy = x[3 * j + 1] - x[3 * i + 1];
             double dz = x[3 * j + 2] - x[3 * i + 2];
-            double r2 = dx * dx + dy * dy + dz * dz;
-            double r  = sqrt(r2);
-            if (!(r > 0.0)) continue;                     /* coincident bodies: W = 0 */
+            double r  = sqrt(dx * dx + dy * dy + dz * dz);
             double rcij = oracle_pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j]);
-            double W = oracle_weight(r, rcij, p->weight_mode);
-            if (W == 0.0) continue;
-            double s = p->G * m[j] * W / (r2 * r);
-            nsum_add(&a[0], s * dx);
-            nsum_add(&a[1], s * dy);
-            nsum_add(&a[2], s * dz);
+            if (r < rcij) {
+                if (n < cap && pairs) { pairs[2 * n] = i < j ? i : j; pairs[2 * n + 1] = i < j ? j : i; }
+                ++n;
+            }
         }
-        for (int k = 0; k < 3; ++k) acc[3 * i + k] = nsum_value(&a[k]);
     }
+    *count = n;
     free(rc); free(sa); free(vk);
 }
 

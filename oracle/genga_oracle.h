@@ -76,6 +76,14 @@ double oracle_pair_rcrit(const oracle_params* p, double mi, double mj,
 void oracle_accel(int N, const double* m, const double* x, const double* v,
                   const oracle_params* p, double* acc);
 
+/* O5 / O6 for a sample of bodies sel[0..nsel): accelerations of those bodies; encounter pairs that
+ * touch one of them, as (min, max), a pair with both ends in the sample listed twice.            */
+void oracle_accel_subset(int N, const double* m, const double* x, const double* v,
+                         const oracle_params* p, int nsel, const int* sel, double* acc);
+void oracle_encounter_pairs_subset(int N, const double* m, const double* x, const double* v,
+                                   const oracle_params* p, int nsel, const int* sel,
+                                   int* pairs, int cap, int* count);
+
 /* O6: { (i,j): i<j, r_ij < r_crit,ij } in lexicographic order.  Writes at most
  * cap pairs into pairs[cap][2]; *count receives the true total.              */
 void oracle_encounter_pairs(int N, const double* m, const double* x, const double* v,

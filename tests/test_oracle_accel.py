@@ -190,3 +190,16 @@ def test_encounter_set_matches_numpy_brute_force():
     got = oracle.encounter_pairs(m, x, v, p)
     assert len(got) > 30
     assert got.tolist() == np.stack([ii, jj], 1).tolist()
+
+
+def test_subset_functions_equal_the_full_ones():
+    # the sampled-output forms used at sizes where all N^2 pairs take too long on a CPU
+    m, x, v = clustered_system(21, 300)
+    p = oracle.Params(G=1.0, n1=3.0, n2=0.4, dt_rcrit=0.02, pair_rule=oracle.PAIR_MAX)
+    a = oracle.accel(m, x, v, p)
+    pf = set(map(tuple, oracle.encounter_pairs(m, x, v, p).tolist()))
+    assert len(pf) > 10
+    sel = np.array(sorted({i for q in list(pf)[:7] for i in q} | {0, 299, 150}))
+    assert np.array_equal(oracle.accel_subset(m, x, v, p, sel), a[sel])
+    ps = oracle.encounter_pairs_subset(m, x, v, p, sel)
+    assert ps == {q for q in pf if q[0] in sel or q[1] in sel} and len(ps) >= 7
