@@ -505,7 +505,7 @@ def main():
     line, w = got
     line["alu_probe"] = alu_probes()
     if line["n_gpus"] == 1 and not args.no_cpu_baseline:
-        times, threads = cpu_oracle_steps(w, 1 if w.N >= 20000 else 4)
+        times, threads = cpu_oracle_steps(w, 4)          # ~10-20 s of host time at N = 40 000
         pairs = w.N * (w.N - 1.0)
         line["cpu_baseline"] = {"value": pairs * len(times) / sum(times), "unit": UNIT, "cores": threads,
                                 "kind": "oracle", "sample": f"{len(times)} full merged-leapfrog steps of the "
