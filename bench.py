@@ -488,6 +488,20 @@ def run_report(args):
                 c = np.array(counts)
                 line["encounter_pairs_per_step"] = {"mean": float(c.mean()), "min": int(c.min()), "max": int(c.max()),
                                                     "first": int(c[0]), "last": int(c[-1])}
+                # dE/E and dL/L every 100 steps (dE/E alike in both precisions, dL/L of the
+                # FP32 run a random walk some orders of magnitude above the FP64 one)
+                g = B.from_workload(w, **kw)
+                g.set_tuning(0 if prec == B.FP32 else 1, variant)
+                g.kick(0.5 * w.dt, prec)
+                series = []
+                for k in range(w.nsteps // 100):
+                    g.leapfrog(w.dt, 100, prec)
+                    g.kick(-0.5 * w.dt, prec)                          # synchronise v with x for the diagnostics ...
+                    Ek, Lk = g.energy_angmom()
+                    g.kick(0.5 * w.dt, prec)                           # ... and go on
+                    series.append([100 * (k + 1), Ek / E0 - 1.0, float(np.linalg.norm(Lk) / np.linalg.norm(L0) - 1.0)])
+                g.close()
+                line["drift_series_step_dE_dL"] = series
             print(json.dumps(line), flush=True)
 
 

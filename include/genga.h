@@ -84,7 +84,7 @@ typedef struct {
                                  <= 0 selects a default.  Overflow is handled exactly (slow path).      */
     int    resort_every;      /* force evaluations between two refreshes of the internal body order
                                  (heavy bodies first, then along a Hilbert curve in the x-y plane; a
-                                 performance hint only).  <= 0 selects the default (8).               */
+                                 performance hint only).  <= 0: default (8; 32 if N < 16384).              */
     int    n_big;             /* TP2 mode ("the giant planets feel the forces of the planetesimals,
                                  but the planetesimals do not feel each other"; reading R9): a pair
                                  (i, j) interacts iff i < n_big or j < n_big.  < 0 (default): every pair.

@@ -315,7 +315,10 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     h->near_floor  = p->near_floor >= 0.0 ? p->near_floor : (1.0 / 256.0);
     if (h->lambda_near < 1.0) h->lambda_near = 1.0;
     h->pair_cap = pc; h->cand_cap = cc;
-    h->resort_every = p->resort_every > 0 ? p->resort_every : 8;
+    // default: every 8 force evaluations where the all-pairs kernel dominates, every 32 for small systems
+    // (the refresh is five tiny kernels, ~25 us, which a 40 us step should not pay too often)
+    const bool tp2 = p->n_big >= 0 && p->n_big < N;             // O(n_big N) pairs: the order hardly matters
+    h->resort_every = p->resort_every > 0 ? p->resort_every : (tp2 ? 64 : (N >= 16384 ? 8 : 32));
     h->evals_since_sort = -1;
     h->stream = static_cast<cudaStream_t>(p->stream);
     h->num_sms = sms;
