@@ -353,6 +353,7 @@ int genga_destroy(genga_handle h)
 static int set_state_impl(genga_handle h, const double* m, const double* x, const double* v, cudaMemcpyKind kind)
 {
     if (!h) return GENGA_EINVAL;
+    if (v) h->pend_vel = false;                       // the owed update only touches v, which is replaced anyway
     { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     const size_t n = (size_t)h->N;
     if (n == 0) return GENGA_OK;
@@ -475,10 +476,11 @@ static int get_state_impl(genga_handle h, double* x, double* v, int helio, cudaM
     if (x) CU(cudaMemcpyAsync(x, h->w.x, n * 24, kind, h->stream));
     if (v) {
         if (helio) {
-            launch_momentum(h); LAUNCHED(h, "momentum_kernel");
-            if (kind == cudaMemcpyDeviceToDevice) { launch_copy_v_helio(h, v); LAUNCHED(h, "copy_shift_kernel"); }
+            const double* mom = h->w.mom;                      // slot A: sum m v of the stored velocities, if current
+            if (!h->mom_a_valid) { launch_momentum(h); LAUNCHED(h, "momentum_kernel"); mom = h->w.red; }
+            if (kind == cudaMemcpyDeviceToDevice) { launch_copy_v_helio(h, mom, v); LAUNCHED(h, "copy_shift_kernel"); }
             else {
-                launch_copy_v_helio(h, h->w.vtmp); LAUNCHED(h, "copy_shift_kernel");
+                launch_copy_v_helio(h, mom, h->w.vtmp); LAUNCHED(h, "copy_shift_kernel");
                 CU(cudaMemcpyAsync(v, h->w.vtmp, n * 24, kind, h->stream));
             }
         } else {

@@ -143,7 +143,7 @@ void launch_shift_v(const Handle* h, double scale);          // v_i += scale * r
 void launch_sunkick(const Handle* h, double tau);            // x_i += tau * red[0..2] / M_star
 void launch_drift(const Handle* h, double dt);
 void launch_energy(const Handle* h);                         // red[0] = E, red[1..3] = L
-void launch_copy_v_helio(const Handle* h, double* out);      // out = v + red[0..2]/M_star
+void launch_copy_v_helio(const Handle* h, const double* mom, double* out);   // out = v + mom[0..2]/M_star
 int  run_peak_probe(int which, int iters, cudaStream_t s, double* ops_per_s, double* ms);
 
 // occupancy-derived grid of the all-pairs kernels

@@ -287,11 +287,11 @@ void launch_sunkick(const Handle* h, double tau)
     shift_kernel<<<(n3 + 255) / 256, 256, 0, h->stream>>>(h->N, tau / h->p.M_star, 0, h->p.M_star, h->w.red, h->w.x);
 }
 
-void launch_copy_v_helio(const Handle* h, double* out)
+void launch_copy_v_helio(const Handle* h, const double* mom, double* out)
 {
     if (h->N == 0) return;
     const int n3 = 3 * h->N;
-    copy_shift_kernel<<<(n3 + 255) / 256, 256, 0, h->stream>>>(h->N, 1.0 / h->p.M_star, h->w.red, h->w.v, out);
+    copy_shift_kernel<<<(n3 + 255) / 256, 256, 0, h->stream>>>(h->N, 1.0 / h->p.M_star, mom, h->w.v, out);
 }
 
 }  // namespace genga
