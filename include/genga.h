@@ -72,7 +72,7 @@ typedef struct {
     double lambda_near;       /* FP32 policy P32: pairs with r_ij < lambda_near * r_crit,ij (as bounded
                                  per j-chunk) are evaluated in FP64.  <= 0 selects the default (2).    */
     double near_floor;        /* FP32 policy P32: the FP32 kernel sees positions relative to the origin
-                                 of each 64-body j-chunk; every pair with r_ij < near_floor * 2 R_chunk
+                                 of each j-chunk (params.chunk bodies); every pair with r_ij < near_floor * 2 R_chunk
                                  (R_chunk = radius of the chunk about its origin) is evaluated in FP64
                                  (position-rounding guard: relative separation error <= 2^-24 / near_floor).
                                  < 0 selects the default (1/256); 0 disables.                           */
@@ -85,6 +85,8 @@ typedef struct {
     int    resort_every;      /* force evaluations between two refreshes of the internal body order
                                  (heavy bodies first, then along a Hilbert curve in the x-y plane; a
                                  performance hint only).  <= 0: default (8; 32 if N < 16384).              */
+    int    chunk;             /* j-bodies per chunk (granularity of the near flag and of the FP32 frames): 64 or
+                                 128; anything else selects the default (128, or 64 for N < 14 000)       */
     int    n_big;             /* TP2 mode ("the giant planets feel the forces of the planetesimals,
                                  but the planetesimals do not feel each other"; reading R9): a pair
                                  (i, j) interacts iff i < n_big or j < n_big.  < 0 (default): every pair.

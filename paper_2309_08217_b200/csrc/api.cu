@@ -40,7 +40,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
     const size_t o_m = take(NP * 8), o_x = take(NP * 24), o_v = take(NP * 24), o_a = take(NP * 24);
     const size_t o_h = take(NP * 8), o_rc = take(NP * 8), o_sa = take(NP * 8), o_vk = take(NP * 8);
-    const size_t o_p64 = take(NP * 32), o_p32 = take(NP * 16), o_bi = take(NP * 16), o_bc = take(NP / CHUNK * sizeof(ChunkP));
+    const size_t o_p64 = take(NP * 32), o_p32 = take(NP * 16), o_bi = take(NP * 16), o_bc = take(NP / CHUNK_MIN * sizeof(ChunkP));
     const size_t o_cand = take((size_t)cand_cap * 8), o_pairs = take((size_t)pair_cap * 8);
     const size_t o_red = take((size_t)RED_DOUBLES * 8), o_vt = take(NP * 24), o_ctr = take(sizeof(Counters));
     const size_t o_ord = take(NP * 4), o_key = take(NP * 8), o_aux = take(NP * 32);
@@ -278,6 +278,7 @@ void genga_default_params(genga_params* p)
     p->resort_every = 0;
     p->no_fused_step = 0;
     p->n_big = -1;
+    p->chunk = 0;
     p->weight_mode = 0;
 }
 
@@ -309,7 +310,10 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     genga_s* h = new (std::nothrow) genga_s();
     if (!h) return GENGA_ENOMEM;
     std::memset(static_cast<Handle*>(h), 0, sizeof(Handle));
-    h->N = N; h->NP = padded(N); h->nchunk = (N + CHUNK - 1) / CHUNK;        // j-chunks that hold a live body (pure padding is skipped)
+    h->N = N; h->NP = padded(N);
+    // chunk size: 128, or 64 for small systems (twice the units to spread over the CTAs); params.chunk overrides
+    h->chunk = (p->chunk == CHUNK_MIN || p->chunk == CHUNK_MAX) ? p->chunk : (N < 14000 ? CHUNK_MIN : CHUNK_MAX);
+    h->nchunk = (N + h->chunk - 1) / h->chunk;      // j-chunks that hold a live body (pure padding is skipped)
     h->p = *p;
     h->lambda_near = p->lambda_near > 0.0 ? p->lambda_near : 2.0;
     h->near_floor  = p->near_floor >= 0.0 ? p->near_floor : (1.0 / 256.0);

@@ -58,6 +58,7 @@ __device__ __forceinline__ void block_partial(double p0, double p1, double p2, d
     __syncthreads();
 }
 
+template <int CHUNK>
 __global__ void __launch_bounds__(FUSED_NT)
 onbody_kernel(OnBodyArgs A, Workspace w)
 {
@@ -117,7 +118,7 @@ onbody_kernel(OnBodyArgs A, Workspace w)
     if (A.do_prep) {
         const int ntile = A.prep.NP / PREP_NT;
         for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x)
-            prep_tile(A.prep, w, tile, pending, shx, shy, shz);
+            prep_tile<CHUNK>(A.prep, w, tile, pending, shx, shy, shz);
     } else if (pending) {
         for (int i = gtid; i < N; i += gsz) { w.x[3 * i] += shx; w.x[3 * i + 1] += shy; w.x[3 * i + 2] += shz; }
     }
@@ -128,7 +129,10 @@ onbody_kernel(OnBodyArgs A, Workspace w)
 int onbody_max_blocks(const Handle* h)
 {
     int occ = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, onbody_kernel, FUSED_NT, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, onbody_kernel<CHUNK_MAX>, FUSED_NT, 0);
+    int occ2 = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, onbody_kernel<CHUNK_MIN>, FUSED_NT, 0);
+    if (occ2 < occ) occ = occ2;
     if (occ < 1) occ = 1;
     long long b = (long long)occ * h->num_sms;
     if (b > MOM_MAX_BLOCKS) b = MOM_MAX_BLOCKS;
@@ -144,7 +148,8 @@ cudaError_t launch_onbody(const Handle* h, const OnBodyArgs& a, int max_blocks)
     OnBodyArgs args = a;
     Workspace ws = h->w;
     void* params[] = {&args, &ws};
-    return cudaLaunchCooperativeKernel((const void*)onbody_kernel, dim3(blocks), dim3(FUSED_NT), params, 0, h->stream);
+    const void* fn = (h->chunk == CHUNK_MIN) ? (const void*)onbody_kernel<CHUNK_MIN> : (const void*)onbody_kernel<CHUNK_MAX>;
+    return cudaLaunchCooperativeKernel(fn, dim3(blocks), dim3(FUSED_NT), params, 0, h->stream);
 }
 
 }  // namespace genga

@@ -11,9 +11,12 @@
 namespace genga {
 
 // ---- tiling constants -------------------------------------------------
-constexpr int CHUNK      = 128;                 // j-bodies per chunk: granularity of the near-field flag
-constexpr int STAGE_CH   = 8;                  // chunks per shared-memory stage
-constexpr int STAGE_J    = CHUNK * STAGE_CH;    // 512 j-bodies per stage
+// j-bodies per chunk (granularity of the near-field flag and of the FP32 frames): a template parameter
+// CHUNK of the kernels, 128 by default and 64 for small systems, where the (i-block, chunk) units are too
+// few to spread evenly over the CTAs (Handle::chunk).
+constexpr int CHUNK_MIN  = 64;
+constexpr int CHUNK_MAX  = 128;
+constexpr int STAGE_J    = 1024;                // j-bodies per shared-memory stage (STAGE_J / CHUNK chunks)
 constexpr int NSTAGE     = 2;                   // double buffering
 constexpr int PAD_BODIES = 512;                 // N is padded to a multiple of this (stage and i-block size)
 constexpr double PAD_POS = 1.0e15;              // position of padding bodies (gm = 0, far from everything)
@@ -62,7 +65,7 @@ struct Workspace {
     float4*  pk32;    // [NP]   pair-interleaved, see above
     double4* aux;     // [NP]   (m, r_crit, a, v_K): what the exact pair rule O3 needs
     BoundP*  bi;      // [NP]   per-body bound parameters
-    ChunkP*  bc;      // [NP/CHUNK] per-chunk maxima and frame origin
+    ChunkP*  bc;      // [NP/chunk] per-chunk maxima and frame origin
     // lists
     int2*    cand;    // [cand_cap] (body, chunk)
     int2*    pairs;   // [pair_cap] (i, j), i < j
@@ -77,6 +80,7 @@ constexpr int RED_DOUBLES = 8 + 8 * 1024;   // [0..7] results, [8..8+4096) pair-
 
 struct Handle {
     int N, NP, nchunk;
+    int chunk;                   // CHUNK of this handle: 64 or 128
     genga_params p;
     double lambda_near, near_floor;
     int pair_cap, cand_cap;

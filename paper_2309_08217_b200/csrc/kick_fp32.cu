@@ -59,7 +59,7 @@ constexpr float EPS2 = 1.0e-30f;   // added to r^2 so that the self pair (d = 0 
 // One j-chunk against the I i-bodies of this thread.  SELF: the chunk holds this warp's own
 // slots; the self pair is then left out of the smallest-r^2 tracking (slot index compare), so a
 // body's own chunk is flagged only if a DIFFERENT body is near.
-template <int I, int UNR, bool SELF, bool SC, bool FAR>
+template <int I, int UNR, bool SELF, bool SC, bool FAR, int CHUNK>
 __device__ __forceinline__ void pair_loop(const float4* __restrict__ jp, const float (&nx)[I], const float (&ny)[I],
                                           const float (&nz)[I], f2 (&ax)[I], f2 (&ay)[I], f2 (&az)[I],
                                           float (&mn)[I], const int (&self_off)[I])
@@ -102,24 +102,25 @@ __device__ __forceinline__ void pair_loop(const float4* __restrict__ jp, const f
 // Kernel configuration: I i-bodies per thread, NT threads per CTA (I * NT = 512 = one i-block),
 // MINB CTAs per SM asked of ptxas (caps the registers), ACCS: FP64 accumulators in shared memory
 // instead of registers, UNR: unroll factor of the j-pair loop.
-template <int I, int NT, bool ACCS>
+template <int I, int NT, bool ACCS, int CHUNK>
 struct __align__(16) Smem32 {
     float4   j[NSTAGE][STAGE_J];                 // pair-interleaved j data (chunk-relative), 16 B per body
-    ChunkP   bc[NSTAGE][STAGE_CH];
+    ChunkP   bc[NSTAGE][STAGE_J / CHUNK];
     double   xi[3][I][NT];                       // FP64 positions of this CTA's i-bodies
     double   acc[ACCS ? 3 : 1][ACCS ? I : 1][ACCS ? NT : 1];   // FP64 accumulators (ACCS)
     float    bp[3][I][NT];                       // bound parameters (hq, aq, rf) of the i-bodies
     uint64_t full[NSTAGE];
 };
 
-template <int I, int NT, int MINB, bool ACCS, int UNR, bool SC>
+template <int I, int NT, int MINB, bool ACCS, int UNR, bool SC, int CHUNK>
 __global__ void __launch_bounds__(NT, MINB)
 kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 {
     constexpr int BI = I * NT;
     static_assert(PAD_BODIES % BI == 0, "i-blocks tile the padding unit");
     extern __shared__ __align__(16) unsigned char smraw[];
-    Smem32<I, NT, ACCS>& sm = *reinterpret_cast<Smem32<I, NT, ACCS>*>(smraw);
+    constexpr int STAGE_CH = STAGE_J / CHUNK;      // chunks per shared-memory stage
+    Smem32<I, NT, ACCS, CHUNK>& sm = *reinterpret_cast<Smem32<I, NT, ACCS, CHUNK>*>(smraw);
     const int tid = threadIdx.x;
 
     if (tid == 0) {
@@ -214,9 +215,9 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                     far = far && ((d2 > reach * reach) || (ib * BI + k * NT + tid >= N));
                 }
                 far = __all_sync(0xffffffffu, far);
-                if (self)     pair_loop<I, UNR, true, SC, false>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
-                else if (far) pair_loop<I, UNR, false, SC, true>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
-                else          pair_loop<I, UNR, false, SC, false>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
+                if (self)     pair_loop<I, UNR, true, SC, false, CHUNK>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
+                else if (far) pair_loop<I, UNR, false, SC, true, CHUNK>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
+                else          pair_loop<I, UNR, false, SC, false, CHUNK>(jp, nx, ny, nz, ax, ay, az, mn, self_off);
 
                 // ---- chunk end: keep the FP32 partial or hand the chunk to the near field ----
 #pragma unroll
@@ -262,10 +263,11 @@ kick32_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 
 // ---- variants (genga_set_tuning key 0) ---------------------------------------------------------
 typedef void (*kick32_fn)(int, int, int, Workspace, unsigned int);
-struct Variant32 { kick32_fn fn; int nt; int bi; size_t smem; bool scaled; const char* name; };
+struct Variant32 { kick32_fn fn[2]; int nt; int bi; size_t smem[2]; bool scaled; const char* name; };   // [0]: CHUNK 64, [1]: 128
 
 #define V32(I_, NT_, MINB_, ACCS_, UNR_, SC_) \
-    { kick32_kernel<I_, NT_, MINB_, ACCS_, UNR_, SC_>, NT_, I_ * NT_, sizeof(Smem32<I_, NT_, ACCS_>), SC_, \
+    { { kick32_kernel<I_, NT_, MINB_, ACCS_, UNR_, SC_, CHUNK_MIN>, kick32_kernel<I_, NT_, MINB_, ACCS_, UNR_, SC_, CHUNK_MAX> }, \
+      NT_, I_ * NT_, { sizeof(Smem32<I_, NT_, ACCS_, CHUNK_MIN>), sizeof(Smem32<I_, NT_, ACCS_, CHUNK_MAX>) }, SC_, \
       "I" #I_ " NT" #NT_ " minB" #MINB_ " accS" #ACCS_ " unr" #UNR_ " scaled" #SC_ }
 
 const Variant32 g_variants32[] = {
@@ -295,11 +297,12 @@ int kick32_grid(const Handle* h)
 {
     const int v = h->tune[0];
     Handle* hm = const_cast<Handle*>(h);
+    const int ci = (h->chunk == CHUNK_MIN) ? 0 : 1;
     if (hm->grid_cache[0][0] != v + 1) {
         const Variant32& V = variant32(v);
-        cudaFuncSetAttribute(V.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V.smem);
+        cudaFuncSetAttribute(V.fn[ci], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V.smem[ci]);
         int occ = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn, V.nt, V.smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn[ci], V.nt, V.smem[ci]);
         if (occ < 1) occ = 1;
         hm->grid_cache[0][0] = v + 1;
         hm->grid_cache[0][1] = h->num_sms * occ;
@@ -315,7 +318,8 @@ void launch_kick32(const Handle* h)
     const long long U = (long long)nib * h->nchunk;
     long long G = kick32_grid(h);
     if (G > U) G = U;
-    V.fn<<<(int)G, V.nt, V.smem, h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
+    const int ci = (h->chunk == CHUNK_MIN) ? 0 : 1;
+    V.fn[ci]<<<(int)G, V.nt, V.smem[ci], h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
 }
 
 }  // namespace genga

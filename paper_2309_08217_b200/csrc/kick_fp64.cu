@@ -23,7 +23,7 @@ constexpr double EPS2 = 1.0e-60;   // added to r^2 so that the self pair (d = 0 
 // One j-chunk against the I i-bodies of this thread.  SELF: the chunk holds this warp's own slots;
 // the self pair is left out of the smallest-r^2 tracking, so a body's own chunk is flagged only if
 // a DIFFERENT body is near.  mn tracks the high word of r^2 (orders like r^2 >= 0).
-template <int I, int UNR, bool SELF, bool FAR>
+template <int I, int UNR, bool SELF, bool FAR, int CHUNK>
 __device__ __forceinline__ void pair_loop(const double4* __restrict__ jp, const double (&xi)[I], const double (&yi)[I],
                                           const double (&zi)[I], double (&ax)[I], double (&ay)[I], double (&az)[I],
                                           int (&mn)[I], const int (&self_off)[I])
@@ -55,22 +55,23 @@ __device__ __forceinline__ void pair_loop(const double4* __restrict__ jp, const 
     }
 }
 
-template <int I, int NT>
+template <int I, int NT, int CHUNK>
 struct __align__(16) Smem64 {
     double4  j[NSTAGE][STAGE_J];                 // (x, y, z, G m), 32 B per body
-    ChunkP   bc[NSTAGE][STAGE_CH];
+    ChunkP   bc[NSTAGE][STAGE_J / CHUNK];
     float    bp[3][I][NT];                       // bound parameters (hq, aq, rf) of this CTA's i-bodies
     uint64_t full[NSTAGE];
 };
 
-template <int I, int NT, int MINB, int UNR>
+template <int I, int NT, int MINB, int UNR, int CHUNK>
 __global__ void __launch_bounds__(NT, MINB)
 kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 {
     constexpr int BI = I * NT;
     static_assert(PAD_BODIES % BI == 0, "i-blocks tile the padding unit");
     extern __shared__ __align__(16) unsigned char smraw[];
-    Smem64<I, NT>& sm = *reinterpret_cast<Smem64<I, NT>*>(smraw);
+    constexpr int STAGE_CH = STAGE_J / CHUNK;      // chunks per shared-memory stage
+    Smem64<I, NT, CHUNK>& sm = *reinterpret_cast<Smem64<I, NT, CHUNK>*>(smraw);
     const int tid = threadIdx.x;
 
     if (tid == 0) {
@@ -152,9 +153,9 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
                     far = far && ((d2 > reach * reach) || (ib * BI + k * NT + tid >= N));
                 }
                 far = __all_sync(0xffffffffu, far);
-                if (self)     pair_loop<I, UNR, true, false>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
-                else if (far) pair_loop<I, UNR, false, true>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
-                else          pair_loop<I, UNR, false, false>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
+                if (self)     pair_loop<I, UNR, true, false, CHUNK>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
+                else if (far) pair_loop<I, UNR, false, true, CHUNK>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
+                else          pair_loop<I, UNR, false, false, CHUNK>(jp, xi, yi, zi, ax, ay, az, mn, self_off);
 
 #pragma unroll
                 for (int k = 0; k < I; ++k) {
@@ -190,10 +191,11 @@ kick64_kernel(int N, int nchunk, int nib, Workspace w, unsigned int cand_cap)
 }
 
 typedef void (*kick64_fn)(int, int, int, Workspace, unsigned int);
-struct Variant64 { kick64_fn fn; int nt; int bi; size_t smem; const char* name; };
+struct Variant64 { kick64_fn fn[2]; int nt; int bi; size_t smem[2]; const char* name; };   // [0]: CHUNK 64, [1]: 128
 
 #define V64(I_, NT_, MINB_, UNR_) \
-    { kick64_kernel<I_, NT_, MINB_, UNR_>, NT_, I_ * NT_, sizeof(Smem64<I_, NT_>), "I" #I_ " NT" #NT_ " minB" #MINB_ " unr" #UNR_ }
+    { { kick64_kernel<I_, NT_, MINB_, UNR_, CHUNK_MIN>, kick64_kernel<I_, NT_, MINB_, UNR_, CHUNK_MAX> }, NT_, I_ * NT_, \
+      { sizeof(Smem64<I_, NT_, CHUNK_MIN>), sizeof(Smem64<I_, NT_, CHUNK_MAX>) }, "I" #I_ " NT" #NT_ " minB" #MINB_ " unr" #UNR_ }
 
 const Variant64 g_variants64[] = {
     V64(2, 256, 2, 8),            // 0: default
@@ -219,11 +221,12 @@ int kick64_grid(const Handle* h)
 {
     const int v = h->tune[1];
     Handle* hm = const_cast<Handle*>(h);
+    const int ci = (h->chunk == CHUNK_MIN) ? 0 : 1;
     if (hm->grid_cache[1][0] != v + 1) {
         const Variant64& V = variant64(v);
-        cudaFuncSetAttribute(V.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V.smem);
+        cudaFuncSetAttribute(V.fn[ci], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V.smem[ci]);
         int occ = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn, V.nt, V.smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, V.fn[ci], V.nt, V.smem[ci]);
         if (occ < 1) occ = 1;
         hm->grid_cache[1][0] = v + 1;
         hm->grid_cache[1][1] = h->num_sms * occ;
@@ -239,7 +242,8 @@ void launch_kick64(const Handle* h)
     const long long U = (long long)nib * h->nchunk;
     long long G = kick64_grid(h);
     if (G > U) G = U;
-    V.fn<<<(int)G, V.nt, V.smem, h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
+    const int ci = (h->chunk == CHUNK_MIN) ? 0 : 1;
+    V.fn[ci]<<<(int)G, V.nt, V.smem[ci], h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
 }
 
 }  // namespace genga

@@ -93,6 +93,7 @@ __device__ __forceinline__ IBody load_ibody(const Workspace& w, int si)
 //  B  the listed pairs, one per lane: plain sqrt / divide / cbrt, exact r < r_crit test, K, force;
 //     encounter pairs appended with one atomic per warp.
 // (One pass over the few near pairs with many lanes active, instead of one divergent pass per round.)
+template <int CHUNK>
 __device__ __forceinline__ void chunk_on_body(const NfParams& P, Workspace& w, const IBody& I, int c,
                                               int* __restrict__ near_list, double& fx, double& fy, double& fz)
 {
@@ -167,6 +168,7 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
+template <int CHUNK>
 __global__ void __launch_bounds__(128, 8)
 nearfield_kernel(NfParams P, Workspace w)
 {
@@ -182,7 +184,7 @@ nearfield_kernel(NfParams P, Workspace w)
             const int2 cd = w.cand[q];
             const IBody I = load_ibody(w, cd.x);
             double fx = 0.0, fy = 0.0, fz = 0.0;
-            chunk_on_body(P, w, I, cd.y, near_list, fx, fy, fz);
+            chunk_on_body<CHUNK>(P, w, I, cd.y, near_list, fx, fy, fz);
             fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
             if (lane == 0) {
                 atomicAdd(&w.a[3 * I.body + 0], fx);
@@ -196,7 +198,7 @@ nearfield_kernel(NfParams P, Workspace w)
         for (int si = warp; si < P.N; si += nwarp) {
             const IBody I = load_ibody(w, si);
             double fx = 0.0, fy = 0.0, fz = 0.0;
-            for (int c = 0; c < P.nchunk; ++c) chunk_on_body(P, w, I, c, near_list, fx, fy, fz);
+            for (int c = 0; c < P.nchunk; ++c) chunk_on_body<CHUNK>(P, w, I, c, near_list, fx, fy, fz);
             fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
             if (lane == 0) { w.a[3 * I.body + 0] = fx; w.a[3 * I.body + 1] = fy; w.a[3 * I.body + 2] = fz; }
         }
@@ -273,21 +275,22 @@ void launch_nearfield(const Handle* h)
 {
     if (h->N == 0) return;
     NfParams P;
-    P.N = h->N; P.nchunk = (h->N + CHUNK - 1) / CHUNK;
+    P.N = h->N; P.nchunk = h->nchunk;
     P.M_star = h->p.M_star; P.n1 = h->p.n1; P.n2dt = h->p.n2 * h->p.dt_rcrit;
     P.pair_rule = h->p.pair_rule; P.weight_mode = h->p.weight_mode;
     P.cand_cap = (unsigned int)h->cand_cap; P.pair_cap = (unsigned int)h->pair_cap;
     int blocks = h->num_sms * 16;
     const long long need = ((long long)h->N + 3) / 4;            // at least one warp per body is enough
     if (blocks > need && need > 0) blocks = (int)((need < h->num_sms) ? h->num_sms : need);
-    nearfield_kernel<<<blocks, 128, 0, h->stream>>>(P, h->w);
+    if (h->chunk == CHUNK_MIN) nearfield_kernel<CHUNK_MIN><<<blocks, 128, 0, h->stream>>>(P, h->w);
+    else                       nearfield_kernel<CHUNK_MAX><<<blocks, 128, 0, h->stream>>>(P, h->w);
 }
 
 void launch_tp2(const Handle* h)
 {
     if (h->N == 0 || h->p.n_big <= 0) return;
     NfParams P;
-    P.N = h->N; P.nchunk = (h->N + CHUNK - 1) / CHUNK;
+    P.N = h->N; P.nchunk = h->nchunk;
     P.M_star = h->p.M_star; P.n1 = h->p.n1; P.n2dt = h->p.n2 * h->p.dt_rcrit;
     P.pair_rule = h->p.pair_rule; P.weight_mode = h->p.weight_mode;
     P.cand_cap = (unsigned int)h->cand_cap; P.pair_cap = (unsigned int)h->pair_cap;

@@ -142,11 +142,12 @@ __global__ void sortrank_kernel(int N, int NP, const unsigned long long* __restr
 
 // a1 + a2 as a kernel of their own (genga_accel; the fused step uses fused_step.cu).  A.preshift: pending
 // Sun-kick with the momentum in mom[SLOT_B].
+template <int CHUNK>
 __global__ void __launch_bounds__(PREP_NT)
 prep_kernel(PrepArgs A, Workspace w)
 {
     const double sc = A.preshift / A.M_star;
-    prep_tile(A, w, blockIdx.x, A.preshift != 0.0, sc * w.mom[MOM_SLOT_B + 0], sc * w.mom[MOM_SLOT_B + 1],
+    prep_tile<CHUNK>(A, w, blockIdx.x, A.preshift != 0.0, sc * w.mom[MOM_SLOT_B + 0], sc * w.mom[MOM_SLOT_B + 1],
               sc * w.mom[MOM_SLOT_B + 2]);
 }
 
@@ -239,7 +240,8 @@ int sort_buffer_words() { return 3 * SORT_NB; }
 void launch_prep(const Handle* h, const PrepArgs& a)
 {
     if (h->NP == 0) return;
-    prep_kernel<<<h->NP / PREP_NT, PREP_NT, 0, h->stream>>>(a, h->w);
+    if (h->chunk == CHUNK_MIN) prep_kernel<CHUNK_MIN><<<h->NP / PREP_NT, PREP_NT, 0, h->stream>>>(a, h->w);
+    else                       prep_kernel<CHUNK_MAX><<<h->NP / PREP_NT, PREP_NT, 0, h->stream>>>(a, h->w);
 }
 
 static int momentum_blocks(const Handle* h)

@@ -20,6 +20,7 @@ __device__ __forceinline__ unsigned int warp_max_u32(unsigned int v)
 // tile: which run of PREP_NT slots this block handles; (shx, shy, shz): a pending Sun-kick displacement
 // (O8) added to the positions first (and written back) if do_shift.  Must be called by all PREP_NT
 // threads of the block; ends with a __syncthreads, so it can be called in a loop.
+template <int CHUNK>
 __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int tile, bool do_shift,
                                           double shx, double shy, double shz)
 {
@@ -108,7 +109,7 @@ __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int t
     BoundP b; b.hq = hq; b.aq = aq; b.rf = rf; b.pad = live ? 1.f : 0.f;
     w.bi[s] = b;
 
-    // per-chunk maxima (CHUNK = 64 = two warps); non-negative floats order like unsigned ints
+    // per-chunk maxima (a chunk is CHUNK / 32 warps of this block); non-negative floats order like unsigned ints
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned int m0 = warp_max_u32(__float_as_uint(hq));
     unsigned int m1 = warp_max_u32(__float_as_uint(aq));

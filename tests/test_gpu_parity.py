@@ -277,6 +277,9 @@ def test_full_size_c4_kick_both_precisions():
     ao, po, _ = oracle_accel(w)
     a64, p64, _, st64 = gpu_accel(w, B.FP64)
     a32, p32, _, st32 = gpu_accel(w, B.FP32)
+    a32b, p32b, _, _ = gpu_accel(w, B.FP32, chunk=64)            # the small-system chunk size at full size
+    e32b = rel_err(a32b, ao)
+    assert np.median(e32b) <= 1e-5 and e32b.max() <= 1e-4 and pair_set(p32b) == pair_set(po)
     assert rel_err(a64, ao).max() <= 1e-12
     e32 = rel_err(a32, ao)
     assert np.median(e32) <= 1e-5 and e32.max() <= 1e-4, (np.median(e32), e32.max())
@@ -298,21 +301,21 @@ def test_every_kernel_variant_matches_the_oracle():
     w.m[1203] = 0.0
     w.x[900] = w.x[899]
     ao, po, _ = oracle_accel(w)
-    for key, v in _variant_cases():
-        g = B.from_workload(w)
+    for key, v, chunk in [(k, vv, c) for (k, vv) in _variant_cases() for c in (64, 128)]:
+        g = B.from_workload(w, chunk=chunk)
         g.set_tuning(key, v)
         prec = B.FP32 if key == 0 else B.FP64
         g.accel(prec)
         a = g.get_accel().cpu().numpy()
         pairs = g.encounter_pairs()
         g.close()
-        assert np.all(np.isfinite(a)), (key, v)
+        assert np.all(np.isfinite(a)), (key, v, chunk)
         err = rel_err(a, ao)
         if prec == B.FP64:
-            assert err.max() <= 1e-12, (key, v, err.max())
+            assert err.max() <= 1e-12, (key, v, chunk, err.max())
         else:
-            assert np.median(err) <= 1e-5 and err.max() <= 1e-4, (key, v, np.median(err), err.max())
-        assert pair_set(pairs) == pair_set(po), (key, v)
+            assert np.median(err) <= 1e-5 and err.max() <= 1e-4, (key, v, chunk, np.median(err), err.max())
+        assert pair_set(pairs) == pair_set(po), (key, v, chunk)
 
 
 def test_autotune_picks_a_variant_and_keeps_the_state():
