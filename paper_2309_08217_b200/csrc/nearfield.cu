@@ -280,7 +280,7 @@ void launch_nearfield(const Handle* h)
     P.pair_rule = h->p.pair_rule; P.weight_mode = h->p.weight_mode;
     P.cand_cap = (unsigned int)h->cand_cap; P.pair_cap = (unsigned int)h->pair_cap;
     int blocks = h->num_sms * 16;
-    const long long need = ((long long)h->N + 3) / 4;            // at least one warp per body is enough
+    const long long need = ((long long)h->N + 15) / 16;          // a warp per four bodies is plenty (candidates << N)
     if (blocks > need && need > 0) blocks = (int)((need < h->num_sms) ? h->num_sms : need);
     if (h->chunk == CHUNK_MIN) nearfield_kernel<CHUNK_MIN><<<blocks, 128, 0, h->stream>>>(P, h->w);
     else                       nearfield_kernel<CHUNK_MAX><<<blocks, 128, 0, h->stream>>>(P, h->w);
