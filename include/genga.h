@@ -31,6 +31,10 @@
  *   copy has run, i.e. stream order).  One handle is not thread-safe; handles share no state.
  *   Return value: GENGA_OK (0) or a negative genga_status.  No exceptions, no abort.
  *
+ *   The workspace layout is private: read the state only through the accessors below.  (The closing
+ *   velocity update of genga_kick/step/run/leapfrog is deferred into the first kernel of the next such
+ *   call and is applied by any accessor or state-changing call that comes first.)
+ *
  * There is NO CPU fallback: without a CUDA device every compute call returns GENGA_ECUDA.
  */
 #ifndef GENGA_H
