@@ -40,7 +40,7 @@ class GengaParams(ctypes.Structure):
         ("lambda_near", ctypes.c_double), ("near_floor", ctypes.c_double),
         ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
         ("pair_capacity", ctypes.c_int), ("cand_capacity", ctypes.c_int), ("resort_every", ctypes.c_int),
-        ("chunk", ctypes.c_int), ("n_big", ctypes.c_int), ("weight_mode", ctypes.c_int), ("no_fused_step", ctypes.c_int),
+        ("chunk", ctypes.c_int), ("mega_nmax", ctypes.c_int), ("n_big", ctypes.c_int), ("weight_mode", ctypes.c_int), ("no_fused_step", ctypes.c_int),
     ]
 
 
@@ -153,7 +153,7 @@ class Genga:
 
     def __init__(self, m, x, v, *, G=None, M_star=1.0, n1=3.0, n2=0.0, dt_rcrit=0.0,
                  pair_rule=PAIR_MUTUAL_HILL, v_is_heliocentric=True, lambda_near=0.0, near_floor=-1.0,
-                 pair_capacity=0, cand_capacity=0, resort_every=0, chunk=0, n_big=-1, weight_mode=0, no_fused_step=False, stream=None, device=None):
+                 pair_capacity=0, cand_capacity=0, resort_every=0, chunk=0, mega_nmax=0, n_big=-1, weight_mode=0, no_fused_step=False, stream=None, device=None):
         import torch
         self._torch = torch
         self._L = load()
@@ -172,6 +172,7 @@ class Genga:
         p.no_fused_step = int(bool(no_fused_step))
         p.n_big = int(n_big)
         p.chunk = int(chunk)
+        p.mega_nmax = int(mega_nmax)
         p.weight_mode = int(weight_mode)
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         p.stream = ctypes.c_void_p(self._stream.cuda_stream)

@@ -217,6 +217,33 @@ static int sd_fused(genga_handle h, double dt)
     return GENGA_OK;
 }
 
+// The one-kernel step of small systems (mega_step.cu): usable for this call?
+static bool mega_ready(Handle* h, int precision)
+{
+    if (h->fused_blocks <= 0 || h->prof != 0 || h->N > h->mega_nmax) return false;
+    if (h->p.n_big >= 0 && h->p.n_big < h->N) return false;          // TP2 mode has its own pair kernel
+    const int pi = precision == GENGA_FP32 ? 1 : 0;
+    if (h->mega_blocks[pi] < 0) h->mega_blocks[pi] = mega_max_blocks(h, precision);
+    return h->mega_blocks[pi] > 0;
+}
+
+// [v += tau_v a] [S(dt/2) D(dt)] S(dt/2), r_crit, pack, all-pairs kick, near field: one cooperative launch.
+static int step_mega(Handle* h, int precision, bool do_vel, double tau_v, bool do_drift, double dt)
+{
+    const int rc = maybe_resort(h);
+    if (rc != GENGA_OK) return rc;
+    OnBodyArgs a;
+    a.prep = make_prep_args(h, precision, 0.0);
+    a.prep.scaled = 0;                                               // the fused all-pairs phase reads plain j-records
+    a.do_vel = do_vel; a.do_drift = do_drift; a.do_prep = 1;
+    a.tau_v = tau_v; a.dt = dt; a.mu = h->p.G * h->p.M_star;
+    const cudaError_t e = launch_step_mega(h, a, precision, h->mega_blocks[precision == GENGA_FP32 ? 1 : 0]);
+    ++h->launches;
+    if (e != cudaSuccess) return cuda_fail(e, "step_kernel (cooperative launch)");
+    h->mom_a_valid = !do_drift;
+    return GENGA_OK;
+}
+
 // K(tau_first)? then n_sds times [S(dt/2) D(dt) S(dt/2) K(tau)], tau = tau_mid except tau_last for the last
 // one.  Fused path: one per-body kernel between two force evaluations (3 launches per step).
 static int sequence(genga_handle h, int precision, bool lead_kick, double tau_first, int n_sds, double dt,
@@ -239,14 +266,21 @@ static int sequence(genga_handle h, int precision, bool lead_kick, double tau_fi
     bool pending = h->pend_vel;
     double tau_prev = h->pend_tau;
     h->pend_vel = false;
+    const bool mega = mega_ready(h, precision);                      // small system: one launch per force evaluation
     if (lead_kick) {
-        if ((rc = onbody(h, precision, pending, tau_prev, false, 0.0, true)) != GENGA_OK) return rc;
-        if ((rc = launch_pairs(h, precision)) != GENGA_OK) return rc;
+        if (mega) { if ((rc = step_mega(h, precision, pending, tau_prev, false, 0.0)) != GENGA_OK) return rc; }
+        else {
+            if ((rc = onbody(h, precision, pending, tau_prev, false, 0.0, true)) != GENGA_OK) return rc;
+            if ((rc = launch_pairs(h, precision)) != GENGA_OK) return rc;
+        }
         pending = true; tau_prev = tau_first;
     }
     for (int k = 0; k < n_sds; ++k) {
-        if ((rc = onbody(h, precision, pending, tau_prev, true, dt, true)) != GENGA_OK) return rc;
-        if ((rc = launch_pairs(h, precision)) != GENGA_OK) return rc;
+        if (mega) { if ((rc = step_mega(h, precision, pending, tau_prev, true, dt)) != GENGA_OK) return rc; }
+        else {
+            if ((rc = onbody(h, precision, pending, tau_prev, true, dt, true)) != GENGA_OK) return rc;
+            if ((rc = launch_pairs(h, precision)) != GENGA_OK) return rc;
+        }
         pending = true; tau_prev = (k == n_sds - 1) ? tau_last : tau_mid;
     }
     if (pending) { h->pend_vel = true; h->pend_tau = tau_prev; h->mom_a_valid = false; }
@@ -279,6 +313,7 @@ void genga_default_params(genga_params* p)
     p->no_fused_step = 0;
     p->n_big = -1;
     p->chunk = 0;
+    p->mega_nmax = 0;
     p->weight_mode = 0;
 }
 
@@ -330,6 +365,8 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
         h->fused_blocks = (coop && !p->no_fused_step) ? onbody_max_blocks(h) : 0;
+        h->mega_blocks[0] = h->mega_blocks[1] = -1;
+        h->mega_nmax = p->mega_nmax > 0 ? p->mega_nmax : (p->mega_nmax < 0 ? 0 : 3000);
     }
     carve_workspace(N, pc, cc, p->workspace, &h->w);
 

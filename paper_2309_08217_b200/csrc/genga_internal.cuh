@@ -89,6 +89,8 @@ struct Handle {
     int num_sms;
     long long launches;
     // internal order (a performance hint only: results never depend on it)
+    int mega_blocks[2];          // co-resident blocks of the one-kernel step per precision; 0 = not used, -1 = not queried yet
+    int mega_nmax;               // largest N that takes the one-kernel step
     int fused_blocks;            // co-resident blocks of the fused per-body kernel; 0 = cooperative launch unavailable
     bool pend_vel;               // a closing velocity update v += pend_tau a is still owed (api.cu: sequence)
     double pend_tau;
@@ -130,6 +132,8 @@ struct OnBodyArgs {               // the fused per-body kernel of the step (fuse
 constexpr int MOM_MAX_BLOCKS = 2048;   // most blocks whose momentum partials fit the workspace
 int  onbody_max_blocks(const Handle* h);
 cudaError_t launch_onbody(const Handle* h, const OnBodyArgs& a, int max_blocks);
+int  mega_max_blocks(const Handle* h, int precision);            // the one-kernel step of small systems (mega_step.cu)
+cudaError_t launch_step_mega(const Handle* h, const OnBodyArgs& a, int precision, int max_blocks);
 void launch_hcbrt(const Handle* h);
 void launch_pad(const Handle* h);                            // padding bodies: x = (PAD_POS,0,0), v = 0, m = 0
 int  sort_buffer_words();

@@ -1,0 +1,129 @@
+// onbody_body.cuh -- the O(N) rows of the step around the all-pairs kick in ONE cooperative kernel:
+//   phase 1  v_i += tau_v a_i (row a6, closing the previous kick)      and  P  = sum m v   (grid-wide)
+//   phase 2  x_i += (dt/2) P / M_star (row a7, Sun-kick, reading G3), Kepler drift D(dt) (row a8,
+//            always FP64)                                  and  P' = sum m v'  (grid-wide)
+//   phase 3  x_i += (dt/2) P' / M_star, then r_crit (Eq. 1), packing and bounds (rows a1, a2) for the
+//            next force evaluation.
+// Each phase is optional.  The two grid-wide sums are block partials combined by EVERY block in the
+// same fixed order after a grid.sync(), so all blocks hold bitwise the same P (and the result is
+// reproducible for a given grid).  A step is then 3 launches: this kernel, the all-pairs kernel,
+// the near-field kernel.
+#pragma once
+
+#include <cooperative_groups.h>
+
+#include "genga_internal.cuh"
+#include "kepler.cuh"
+#include "momentum.cuh"
+#include "prep_tile.cuh"
+
+namespace genga {
+namespace ob {
+
+namespace cg = cooperative_groups;
+
+
+constexpr int FUSED_NT = PREP_NT;          // 256: prep_tile needs exactly this block size
+
+// Sum of the per-block partials part[4 b + k], b < nblk, by one warp with a fixed assignment and tree.
+__device__ __forceinline__ void combine_partials(const double* __restrict__ part, int nblk, double* s_out)
+{
+    if (threadIdx.x < 32) {
+        double p0 = 0, p1 = 0, p2 = 0, mt = 0;
+        for (int b = threadIdx.x; b < nblk; b += 32) {
+            const double* q = part + 4 * b;
+            p0 += __ldcg(q + 0); p1 += __ldcg(q + 1); p2 += __ldcg(q + 2); mt += __ldcg(q + 3);
+        }
+        warp_sum4(p0, p1, p2, mt);
+        if (threadIdx.x == 0) { s_out[0] = p0; s_out[1] = p1; s_out[2] = p2; s_out[3] = mt; }
+    }
+    __syncthreads();
+}
+
+// block partial of (p0, p1, p2, mt) -> part[4 blockIdx.x ..]
+__device__ __forceinline__ void block_partial(double p0, double p1, double p2, double mt, double* __restrict__ part)
+{
+    __shared__ double s_w[FUSED_NT / 32][4];
+    warp_sum4(p0, p1, p2, mt);
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { s_w[wid][0] = p0; s_w[wid][1] = p1; s_w[wid][2] = p2; s_w[wid][3] = mt; }
+    __syncthreads();
+    if (wid == 0) {
+        const bool in = lane < FUSED_NT / 32;
+        p0 = in ? s_w[lane][0] : 0.0; p1 = in ? s_w[lane][1] : 0.0; p2 = in ? s_w[lane][2] : 0.0; mt = in ? s_w[lane][3] : 0.0;
+        warp_sum4(p0, p1, p2, mt);
+        if (lane == 0) {
+            double* q = part + 4 * blockIdx.x;
+            __stcg(q + 0, p0); __stcg(q + 1, p1); __stcg(q + 2, p2); __stcg(q + 3, mt);
+        }
+    }
+    __syncthreads();
+}
+
+// The kernel as a device function (a cooperative 1-D grid of FUSED_NT-thread blocks).
+template <int CHUNK>
+__device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, cg::grid_group& grid)
+{
+    __shared__ double sP[4];
+    const int N = A.prep.N;
+    const int gtid = blockIdx.x * FUSED_NT + threadIdx.x, gsz = gridDim.x * FUSED_NT;
+    double* part1 = w.mom + MOM_PARTIALS;
+    double* part2 = part1 + 4 * MOM_MAX_BLOCKS;
+
+    // ---- phase 1: close the previous kick, total momentum of the stored velocities ----------------
+    {
+        double p0 = 0, p1 = 0, p2 = 0, mt = 0;
+        for (int i = gtid; i < N; i += gsz) {
+            double v0 = w.v[3 * i + 0], v1 = w.v[3 * i + 1], v2 = w.v[3 * i + 2];
+            if (A.do_vel) {
+                v0 = fma(A.tau_v, w.a[3 * i + 0], v0); v1 = fma(A.tau_v, w.a[3 * i + 1], v1); v2 = fma(A.tau_v, w.a[3 * i + 2], v2);
+                w.v[3 * i + 0] = v0; w.v[3 * i + 1] = v1; w.v[3 * i + 2] = v2;
+            }
+            const double mi = w.m[i];
+            p0 = fma(mi, v0, p0); p1 = fma(mi, v1, p1); p2 = fma(mi, v2, p2); mt += mi;
+        }
+        block_partial(p0, p1, p2, mt, part1);
+        grid.sync();
+        combine_partials(part1, gridDim.x, sP);
+        if (blockIdx.x == 0 && threadIdx.x < 4) w.mom[MOM_SLOT_A + threadIdx.x] = sP[threadIdx.x];
+    }
+    double shx = 0.0, shy = 0.0, shz = 0.0;
+    bool pending = false;
+
+    // ---- phase 2: Sun-kick, Kepler drift, momentum of the drifted velocities --------------------------
+    if (A.do_drift) {
+        const double sc = 0.5 * A.dt / A.prep.M_star;
+        const double s0 = sc * sP[0], s1 = sc * sP[1], s2 = sc * sP[2];
+        __syncthreads();                                   // sP is rewritten below
+        double p0 = 0, p1 = 0, p2 = 0, mt = 0;
+        for (int i = gtid; i < N; i += gsz) {
+            double x0 = w.x[3 * i] + s0, y0 = w.x[3 * i + 1] + s1, z0 = w.x[3 * i + 2] + s2;
+            double vx = w.v[3 * i], vy = w.v[3 * i + 1], vz = w.v[3 * i + 2];
+            if (A.dt != 0.0) {
+                if (!kepler_drift(A.mu, A.dt, x0, y0, z0, vx, vy, vz)) atomicAdd(&w.ctr->noconv, 1u);
+                w.v[3 * i] = vx; w.v[3 * i + 1] = vy; w.v[3 * i + 2] = vz;
+            }
+            w.x[3 * i] = x0; w.x[3 * i + 1] = y0; w.x[3 * i + 2] = z0;
+            const double mi = w.m[i];
+            p0 = fma(mi, vx, p0); p1 = fma(mi, vy, p1); p2 = fma(mi, vz, p2); mt += mi;
+        }
+        block_partial(p0, p1, p2, mt, part2);
+        grid.sync();
+        combine_partials(part2, gridDim.x, sP);
+        if (blockIdx.x == 0 && threadIdx.x < 4) w.mom[MOM_SLOT_B + threadIdx.x] = sP[threadIdx.x];
+        shx = sc * sP[0]; shy = sc * sP[1]; shz = sc * sP[2];
+        pending = true;
+    }
+
+    // ---- phase 3: closing Sun-kick, r_crit, packing, bounds ------------------------------------------------
+    if (A.do_prep) {
+        const int ntile = A.prep.NP / PREP_NT;
+        for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x)
+            prep_tile<CHUNK>(A.prep, w, tile, pending, shx, shy, shz);
+    } else if (pending) {
+        for (int i = gtid; i < N; i += gsz) { w.x[3 * i] += shx; w.x[3 * i + 1] += shy; w.x[3 * i + 2] += shz; }
+    }
+}
+
+}  // namespace ob
+}  // namespace genga

@@ -497,3 +497,39 @@ def test_weight_mode_k_minus_r_dk_dr():
             g.close()
             assert rel_err(a, ao).max() <= tol, (extra, prec, rel_err(a, ao).max())
             assert pair_set(pairs) == pair_set(po)
+
+
+def test_one_kernel_step_of_small_systems():
+    # N <= params.mega_nmax: per-body kernel, all-pairs kick and near field run as phases of ONE cooperative
+    # kernel (mega_step.cu).  Same device functions, so the same results as the separate kernels and the oracle.
+    for w, kw in ((W.config(0), {}), (clustered(3, 700), {}), (W.config(2, 900), dict(n1=3.0, n2=0.4, pair_rule=B.PAIR_MAX))):
+        p = oparams(w, **kw)
+        vd = oracle.to_democratic(w.m, w.v, w.M_star)
+        vo, ao = oracle.kick(w.m, w.x, vd, p, w.dt)
+        po = oracle.encounter_pairs(w.m, w.x, vd, p)
+        xr, vr = oracle.run(w.m, w.x, vd, p, w.dt, 3)
+        for prec, tol in ((B.FP64, 1e-12), (B.FP32, 1e-4)):
+            res = {}
+            for nmax in (1 << 20, -1):                         # one-kernel step / separate kernels
+                g = B.from_workload(w, mega_nmax=nmax, pair_capacity=4 * len(po) + 64, **kw)
+                l0 = g.launch_count()
+                g.kick(w.dt, prec)
+                nl = g.launch_count() - l0
+                a = g.get_accel().cpu().numpy()
+                pairs = pair_set(g.encounter_pairs())
+                _, v = g.get_state()
+                assert rel_err(a, ao).max() <= tol and pairs == pair_set(po)
+                assert (np.linalg.norm(v.cpu().numpy() - vo, axis=1) / np.linalg.norm(vo, axis=1)).max() <= (1e-13 if prec == B.FP64 else 1e-9)
+                g.close()
+                g = B.from_workload(w, mega_nmax=nmax, **kw)
+                g.run(w.dt, 3, prec)
+                res[nmax] = tuple(t.cpu().numpy() for t in g.get_state()) + (nl,)
+                g.nearfield_stats()
+                g.close()
+                if prec == B.FP64:
+                    for got, ref in zip(res[nmax][:2], (xr, vr)):
+                        assert (np.linalg.norm(got - ref, axis=1) / np.linalg.norm(ref, axis=1)).max() <= 1e-11
+            assert res[1 << 20][2] < res[-1][2]                # fewer launches (the sort of the first evaluation included)
+            if prec == B.FP64:
+                for u, v_ in zip(res[1 << 20][:2], res[-1][:2]):
+                    assert (np.linalg.norm(u - v_, axis=1) / np.linalg.norm(v_, axis=1)).max() <= 1e-13
