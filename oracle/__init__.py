@@ -71,6 +71,8 @@ def lib() -> ctypes.CDLL:
         L = ctypes.CDLL(build())
         L.oracle_changeover.restype = ctypes.c_double
         L.oracle_changeover.argtypes = [ctypes.c_double, ctypes.c_double]
+        L.oracle_step_hybrid.restype = ctypes.c_int
+        L.oracle_step_hybrid.argtypes = [ctypes.c_int, _dp, _dp, _dp, _pp, ctypes.c_double, ctypes.c_int]
         L.oracle_weight.restype = ctypes.c_double
         L.oracle_weight.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int]
         L.oracle_pair_rcrit.restype = ctypes.c_double
@@ -244,6 +246,16 @@ def step(m, x, v, p: Params, dt: float):
     c = p.c()
     if lib().oracle_step(len(m), _p(m), _p(x), _p(v), ctypes.byref(c), float(dt)) != 0:
         raise RuntimeError("oracle Kepler solve did not converge")
+    return x, v
+
+
+def step_hybrid(m, x, v, p: Params, dt: float, nsub: int = 2000):
+    """NEXT-1 (reading R11): one hybrid step with the encounter complement; returns (x', v')."""
+    m = _a(m); x = _a(x).copy(); v = _a(v).copy()
+    c = p.c()
+    rc = lib().oracle_step_hybrid(len(m), _p(m), _p(x), _p(v), ctypes.byref(c), float(dt), int(nsub))
+    if rc != 0:
+        raise ValueError("oracle_step_hybrid needs weight_mode = 1 and nsub >= 1")
     return x, v
 
 

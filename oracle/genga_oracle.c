@@ -450,6 +450,87 @@ int oracle_run(int N, const double* m, double* x, double* v,
     return rc;
 }
 
+/* ---- NEXT-1: the encounter complement, reading R11 -------------------
+ * "a changeover function smoothly switches" a pair between the fixed-step level-0 integrator and
+ * the close-encounter integrator; encounter forces in double precision.  Hybrid symplectic split
+ * (Chambers 1999; democratic heliocentric as G3):
+ *   H_A = sum_i (|p_i|^2/2m_i - G M m_i/r_i) - sum_{i<j} G m_i m_j (1 - K(r_ij))/r_ij   Kepler + encounters
+ *   H_B = - sum_{i<j} G m_i m_j K(r_ij)/r_ij                                            the level-0 kick
+ *   H_C = |sum_i p_i|^2 / 2M                                                            the Sun-kick
+ *   step = B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2).
+ * B is oracle_kick with weight_mode = 1 (W = K - r K', the gradient of H_B).  A has no closed form once a pair
+ * is inside its zone; the oracle integrates the flow of H_A for ALL bodies numerically (classical RK4, nsub
+ * equal substeps: plain and slow, no encounter groups, no pair lists), with the pair weight
+ * Wc = 1 - W = (1 - K) + r K' and r_crit,ij held at the values of the opening force evaluation.  With no pair
+ * inside a zone Wc = 0 everywhere and A is the Kepler drift, so the step reduces to oracle_step.           */
+static void rhs_A(int N, const double* m, const oracle_params* p, const double* rc, const double* sa,
+                  const double* vk, const double* x, const double* v, double* dx, double* dv)
+{
+    const double mu = p->G * p->M_star;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        const double* xi = x + 3 * i;
+        double r2 = xi[0] * xi[0] + xi[1] * xi[1] + xi[2] * xi[2];
+        double r  = sqrt(r2);
+        double a[3] = {-mu * xi[0] / (r2 * r), -mu * xi[1] / (r2 * r), -mu * xi[2] / (r2 * r)};
+        for (int j = 0; j < N; ++j) {
+            if (j == i || !interacts(p, i, j)) continue;
+            double d[3] = {x[3 * j] - xi[0], x[3 * j + 1] - xi[1], x[3 * j + 2] - xi[2]};
+            double q2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            double q  = sqrt(q2);
+            if (!(q > 0.0)) continue;
+            double rcij = oracle_pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j]);
+            double Wc = 1.0 - oracle_weight(q, rcij, 1);
+            if (Wc == 0.0) continue;
+            double s = p->G * m[j] * Wc / (q2 * q);
+            a[0] += s * d[0]; a[1] += s * d[1]; a[2] += s * d[2];
+        }
+        for (int k = 0; k < 3; ++k) { dx[3 * i + k] = v[3 * i + k]; dv[3 * i + k] = a[k]; }
+    }
+}
+
+/* A(dt): nsub RK4 substeps of the flow of H_A with the given (fixed) critical radii. */
+void oracle_encounter_drift(int N, const double* m, double* x, double* v, const oracle_params* p,
+                            const double* rc, const double* sa, const double* vk, double dt, int nsub)
+{
+    size_t n3 = 3 * (size_t)(N > 0 ? N : 1);
+    double* buf = (double*)malloc(sizeof(double) * n3 * 10);
+    double *k1x = buf, *k1v = buf + n3, *k2x = buf + 2 * n3, *k2v = buf + 3 * n3, *k3x = buf + 4 * n3,
+           *k3v = buf + 5 * n3, *k4x = buf + 6 * n3, *k4v = buf + 7 * n3, *tx = buf + 8 * n3, *tv = buf + 9 * n3;
+    double h = dt / nsub;
+    for (int s = 0; s < nsub; ++s) {
+        rhs_A(N, m, p, rc, sa, vk, x, v, k1x, k1v);
+        for (int q = 0; q < 3 * N; ++q) { tx[q] = x[q] + 0.5 * h * k1x[q]; tv[q] = v[q] + 0.5 * h * k1v[q]; }
+        rhs_A(N, m, p, rc, sa, vk, tx, tv, k2x, k2v);
+        for (int q = 0; q < 3 * N; ++q) { tx[q] = x[q] + 0.5 * h * k2x[q]; tv[q] = v[q] + 0.5 * h * k2v[q]; }
+        rhs_A(N, m, p, rc, sa, vk, tx, tv, k3x, k3v);
+        for (int q = 0; q < 3 * N; ++q) { tx[q] = x[q] + h * k3x[q]; tv[q] = v[q] + h * k3v[q]; }
+        rhs_A(N, m, p, rc, sa, vk, tx, tv, k4x, k4v);
+        for (int q = 0; q < 3 * N; ++q) {
+            x[q] += h / 6.0 * (k1x[q] + 2.0 * k2x[q] + 2.0 * k3x[q] + k4x[q]);
+            v[q] += h / 6.0 * (k1v[q] + 2.0 * k2v[q] + 2.0 * k3v[q] + k4v[q]);
+        }
+    }
+    free(buf);
+}
+
+/* One hybrid step B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2); p->weight_mode must be 1.  Returns -1 otherwise. */
+int oracle_step_hybrid(int N, const double* m, double* x, double* v, const oracle_params* p, double dt, int nsub)
+{
+    if (p->weight_mode != 1 || nsub < 1) return -1;
+    double* rc = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* sa = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* vk = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    oracle_rcrit(N, m, x, v, p, rc, sa, vk);              /* the radii of the opening force evaluation */
+    oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
+    oracle_sunkick(N, m, x, v, p, 0.5 * dt);
+    oracle_encounter_drift(N, m, x, v, p, rc, sa, vk, dt, nsub);
+    oracle_sunkick(N, m, x, v, p, 0.5 * dt);
+    oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
+    free(rc); free(sa); free(vk);
+    return 0;
+}
+
 /* ---- O11: diagnostics, PAPER.md:111 (Delta E/E = E(t)/E(0) - 1, likewise L), reading G5 ---- */
 void oracle_energy_angmom(int N, const double* m, const double* x, const double* v,
                           const oracle_params* p, double* E, double L[3])

@@ -28,6 +28,8 @@
  *   oracle_energy_angmom   pinned: two-body closed form, inertial-frame formula
  *   oracle_weight mode 1   pinned: hand value at y = 1/2, limits, -r^2 d/dr[K/r] by central
  *                          differences of the pinned K, two-body force = -grad of the potential
+ *   oracle_step_hybrid     pinned: reduces to oracle_step without encounters, energy through a close
+ *                          encounter (full E) vs the level-0-only step, dt^2 convergence to DOP853
  *   TP2 mode (n_big >= 0)  pinned: hand 3-body values, full-minus-subset identity against the
  *                          pinned all-pairs path, sum m a = 0, bounded dt^2 energy error
  */
@@ -113,6 +115,13 @@ int oracle_step(int N, const double* m, double* x, double* v,
  * force evaluation from the velocities of that moment (reading R7). */
 int oracle_run(int N, const double* m, double* x, double* v,
                const oracle_params* p, double dt, int nsteps);
+
+/* NEXT-1 (not built on the GPU yet; reading R11): the hybrid step with the encounter complement,
+ * B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2), A = flow of Kepler + sum (1-K)-weighted pair terms integrated with
+ * nsub RK4 substeps for all bodies (r_crit,ij held at the opening evaluation's values).  weight_mode must be 1. */
+void oracle_encounter_drift(int N, const double* m, double* x, double* v, const oracle_params* p,
+                            const double* rc, const double* sa, const double* vk, double dt, int nsub);
+int oracle_step_hybrid(int N, const double* m, double* x, double* v, const oracle_params* p, double dt, int nsub);
 
 /* O11.  E = sum m v^2/2 + |sum m v|^2/(2 M_star) - sum G M_star m/r
  *                         - sum_{i<j} G m_i m_j / r_ij ;  L = sum m x cross v. */
