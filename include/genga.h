@@ -104,6 +104,19 @@ typedef struct {
     int    no_fused_step;     /* 1: genga_kick/step/run/leapfrog use the separate per-body kernels instead of the
                                  one cooperative kernel per step (debugging; also taken if the device lacks
                                  cooperative launch)                                                   */
+    int    encounter_mode;    /* NEXT-1 (reading R11), opt-in.  0 (default): every body
+                                 moves on its Kepler orbit during the drift (the level-0 step of north_star).
+                                 1: the hybrid symplectic step: the bodies of an
+                                 encounter GROUP (connected component of the encounter-pair list of the step's
+                                 opening force evaluation) are advanced over dt under their Kepler terms plus the
+                                 complement pair forces G m_j (1 - (K - r dK/dr)) / r^2, in FP64, by enc_nsub
+                                 classical RK4 substeps, r_crit,ij held at the opening evaluation's values.
+                                 Requires weight_mode = 1, n_big < 0 and the cooperative per-body kernel.    */
+    int    enc_nsub;          /* RK4 substeps per step for the bodies of a group; <= 0: default (256)        */
+    double enc_list_scale;    /* encounter mode: pairs with r_ij < enc_list_scale * r_crit,ij are listed (and
+                                 grouped), so that a pair that enters its zone DURING the step is already in a
+                                 group.  1 <= enc_list_scale <= lambda_near; <= 0: default (1.5).  Changes the
+                                 list genga_encounter_pairs returns, not the forces.                      */
 } genga_params;
 
 /* Fill *p with the defaults: G = k^2 (k = 0.01720209895), M_star = 1, n1 = 3, n2 = 0,
@@ -171,6 +184,12 @@ int genga_get_rcrit(genga_handle h, double* rcrit);      /* DEVICE [N]: r_crit,i
 /* Diagnostics of the last force evaluation: number of (body, j-chunk) near-field candidates and
  * whether the candidate list overflowed (exact slow path taken).  HOST outputs.  Synchronises.  */
 int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed);
+
+/* Encounter mode: the groups the last drift integrated (their number, the bodies in them, the largest) and
+ * a status mask, cleared by this call: bit 0 the pair list overflowed when the groups were formed (raise
+ * pair_capacity), bit 1 a group had more than 8 bodies (its bodies drifted on their Kepler orbits instead).
+ * HOST outputs, NULL = skip.  Synchronises.  GENGA_EINVAL unless params.encounter_mode = 1.          */
+int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest, int* status);
 
 /* Per-kernel device timing.  enable is a bit mask: bit k brackets every launch of kernel class k with
  * CUDA events on params.stream; classes: 0 all-pairs kick kernel, 1 near-field kernel, 2 prep kernel,

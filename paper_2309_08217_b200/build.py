@@ -20,7 +20,7 @@ _OBJ_DIR = os.path.join(_HERE, "build")
 
 SOURCES = ["api.cu", "prep.cu", "fused_step.cu", "mega_step.cu", "kick_fp32.cu", "kick_fp64.cu", "nearfield.cu", "drift.cu", "reduce.cu", "probe.cu"]
 HEADERS = ["genga_internal.cuh", "tile_pipeline.cuh", "momentum.cuh", "kepler.cuh", "prep_tile.cuh",
-           "kick32_body.cuh", "kick64_body.cuh", "nearfield_body.cuh", "onbody_body.cuh"]
+           "kick32_body.cuh", "kick64_body.cuh", "nearfield_body.cuh", "onbody_body.cuh", "encounter.cuh"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=true"]

@@ -47,6 +47,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_mom = take((8 + 4 * (NP / 128 + 1) + 8 * (size_t)MOM_MAX_BLOCKS) * 8);
     const size_t o_bs = take(NP * 4);
     const size_t o_bk = take(NP * 8), o_sb = take((size_t)sort_buffer_words() * 4);
+    const size_t o_gl = take(NP * 8);          // labels [NP], member counts [NP]
     if (w && base) {
         char* b = static_cast<char*>(base);
         w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
@@ -59,6 +60,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
         w->mom = (double*)(b + o_mom);
         w->bigslot = (int*)(b + o_bs);
         w->bkeys = (unsigned long long*)(b + o_bk); w->sortbuf = (unsigned int*)(b + o_sb);
+        w->glabel = (int*)(b + o_gl);
     }
     return off;
 }
@@ -171,8 +173,17 @@ static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_d
     a.prep = make_prep_args(h, precision, 0.0);
     a.do_vel = do_vel; a.do_drift = do_drift; a.do_prep = do_prep;
     a.tau_v = tau_v; a.dt = dt; a.mu = h->p.G * h->p.M_star;
+    const bool enc = h->p.encounter_mode == 1 && do_drift;
+    a.enc.on = enc ? 1 : 0; a.enc.nsub = h->p.enc_nsub; a.enc.pair_rule = h->p.pair_rule;
+    a.enc.pair_cap = (unsigned int)h->pair_cap;
+    a.enc.G = h->p.G; a.enc.M_star = h->p.M_star; a.enc.n1 = h->p.n1; a.enc.n2dt = h->p.n2 * h->p.dt_rcrit;
     cudaError_t e;
-    { ProfScope ps(h, do_drift ? 3 : 2); e = launch_onbody(h, a, h->fused_blocks); }
+    if (enc) {                                         // groups of the pair list the last force evaluation left
+        e = launch_groups(h);
+        ++h->launches;
+        if (e != cudaSuccess) return cuda_fail(e, "group_kernel");
+    }
+    { ProfScope ps(h, do_drift ? 3 : 2); e = launch_onbody(h, a, (enc && h->enc_blocks < h->fused_blocks) ? h->enc_blocks : h->fused_blocks); }
     ++h->launches;
     if (e != cudaSuccess) return cuda_fail(e, "onbody_kernel (cooperative launch)");
     h->mom_a_valid = !do_drift;          // slot A holds sum m v of the stored velocities unless the drift changed them
@@ -222,6 +233,7 @@ static bool mega_ready(Handle* h, int precision)
 {
     if (h->fused_blocks <= 0 || h->prof != 0 || h->N > h->mega_nmax) return false;
     if (h->p.n_big >= 0 && h->p.n_big < h->N) return false;          // TP2 mode has its own pair kernel
+    if (h->p.encounter_mode == 1) return false;                      // the groups are formed between two launches
     const int pi = precision == GENGA_FP32 ? 1 : 0;
     if (h->mega_blocks[pi] < 0) h->mega_blocks[pi] = mega_max_blocks(h, precision);
     return h->mega_blocks[pi] > 0;
@@ -233,6 +245,7 @@ static int step_mega(Handle* h, int precision, bool do_vel, double tau_v, bool d
     const int rc = maybe_resort(h);
     if (rc != GENGA_OK) return rc;
     OnBodyArgs a;
+    std::memset(&a.enc, 0, sizeof(a.enc));
     a.prep = make_prep_args(h, precision, 0.0);
     a.prep.scaled = 0;                                               // the fused all-pairs phase reads plain j-records
     a.do_vel = do_vel; a.do_drift = do_drift; a.do_prep = 1;
@@ -315,6 +328,7 @@ void genga_default_params(genga_params* p)
     p->chunk = 0;
     p->mega_nmax = 0;
     p->weight_mode = 0;
+    p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0;
 }
 
 size_t genga_workspace_bytes(int N, const genga_params* p)
@@ -331,6 +345,8 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     if (!(p->M_star > 0.0) || !(p->G > 0.0)) return GENGA_EINVAL;
     if (p->pair_rule != GENGA_PAIR_MAX && p->pair_rule != GENGA_PAIR_MUTUAL_HILL) return GENGA_EINVAL;
     if (p->weight_mode != 0 && p->weight_mode != 1) return GENGA_EINVAL;
+    if (p->encounter_mode != 0 && p->encounter_mode != 1) return GENGA_EINVAL;
+    if (p->encounter_mode == 1 && (p->weight_mode != 1 || (p->n_big >= 0 && p->n_big < N) || p->no_fused_step)) return GENGA_EINVAL;
     *out = nullptr;
     int pc, cc;
     resolve_caps(N, p, &pc, &cc);
@@ -364,7 +380,14 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     {
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-        h->fused_blocks = (coop && !p->no_fused_step) ? onbody_max_blocks(h) : 0;
+        h->fused_blocks = (coop && !p->no_fused_step) ? onbody_max_blocks(h, false) : 0;
+        if (p->encounter_mode == 1) {
+            if (!coop) { delete h; return GENGA_EINVAL; }
+            h->enc_blocks = onbody_max_blocks(h, true);
+            h->p.enc_nsub = p->enc_nsub > 0 ? p->enc_nsub : 256;
+            h->p.enc_list_scale = p->enc_list_scale > 0.0 ? p->enc_list_scale : 1.5;
+            if (h->p.enc_list_scale < 1.0 || h->p.enc_list_scale > h->lambda_near) { delete h; return GENGA_EINVAL; }
+        }
         h->mega_blocks[0] = h->mega_blocks[1] = -1;
         h->mega_nmax = p->mega_nmax > 0 ? p->mega_nmax : (p->mega_nmax < 0 ? 0 : 3000);
     }
@@ -571,6 +594,23 @@ int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed
         CU(cudaMemsetAsync(&h->w.ctr->noconv, 0, sizeof(unsigned int), h->stream));
         return GENGA_ENOCONV;
     }
+    return GENGA_OK;
+}
+
+int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest, int* status)
+{
+    if (!h || h->p.encounter_mode != 1) return GENGA_EINVAL;
+    Counters c;
+    std::memset(&c, 0, sizeof(c));
+    if (h->N) {
+        CU(cudaMemcpyAsync(&c, h->w.ctr, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        if (c.enc_status) CU(cudaMemsetAsync(&h->w.ctr->enc_status, 0, sizeof(unsigned int), h->stream));
+    }
+    if (groups) *groups = (int)c.enc_groups;
+    if (bodies) *bodies = (int)c.enc_bodies;
+    if (largest) *largest = (int)c.enc_maxsize;
+    if (status) *status = (int)c.enc_status;
     return GENGA_OK;
 }
 

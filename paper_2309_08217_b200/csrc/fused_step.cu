@@ -8,22 +8,69 @@ namespace {
 
 using namespace ob;
 
-template <int CHUNK>
+template <int CHUNK, bool ENC>
 __global__ void __launch_bounds__(FUSED_NT)
 onbody_kernel(OnBodyArgs A, Workspace w)
 {
     cg::grid_group grid = cg::this_grid();
-    onbody_body<CHUNK>(A, w, grid);
+    onbody_body<CHUNK, ENC>(A, w, grid);
+}
+
+// Encounter groups (NEXT-1): connected components of the encounter-pair graph by label propagation over the
+// pair list; glabel[b] = smallest body index of b's component, -1 for bodies in no pair (preset by the
+// launcher), -2 for the bodies of a component with more than enc::GMAX members (status bit 2; they drift on
+// their Kepler orbits).  One block.
+__global__ void __launch_bounds__(1024)
+group_kernel(int N, int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr, unsigned int pair_cap,
+             int* __restrict__ glabel)
+{
+    __shared__ int changed;
+    int* gcount = glabel + NP;
+    const unsigned int total = ctr->pair_count;
+    const unsigned int n = total < pair_cap ? total : pair_cap;
+    if (threadIdx.x == 0) {
+        if (total > pair_cap) atomicOr(&ctr->enc_status, 1u);               // list overflowed: groups incomplete
+        ctr->enc_groups = 0u; ctr->enc_bodies = 0u; ctr->enc_maxsize = 0u;
+    }
+    if (n == 0) return;
+    for (unsigned int p = threadIdx.x; p < n; p += blockDim.x) {
+        const int2 ij = pairs[p];
+        glabel[ij.x] = ij.x; glabel[ij.y] = ij.y; gcount[ij.x] = 0; gcount[ij.y] = 0;
+    }
+    __syncthreads();
+    for (int iter = 0; iter < (1 << 20); ++iter) {
+        if (threadIdx.x == 0) changed = 0;
+        __syncthreads();
+        for (unsigned int p = threadIdx.x; p < n; p += blockDim.x) {
+            const int2 ij = pairs[p];
+            const int a = ((volatile int*)glabel)[ij.x], b = ((volatile int*)glabel)[ij.y], m = min(a, b);
+            if (a != m) { atomicMin(&glabel[ij.x], m); changed = 1; }
+            if (b != m) { atomicMin(&glabel[ij.y], m); changed = 1; }
+        }
+        __syncthreads();
+        const int again = changed;
+        __syncthreads();
+        if (!again) break;
+    }
+    // member counts; components too large for the leader's arrays are dissolved (and reported)
+    for (int b = threadIdx.x; b < N; b += blockDim.x) if (glabel[b] >= 0) atomicAdd(&gcount[glabel[b]], 1);
+    __syncthreads();
+    for (int b = threadIdx.x; b < N; b += blockDim.x) {
+        const int l = glabel[b];
+        if (l >= 0 && l != b && gcount[l] > enc::GMAX) { glabel[b] = -2; atomicOr(&ctr->enc_status, 2u); }
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < N; b += blockDim.x) if (glabel[b] == b && gcount[b] > enc::GMAX) glabel[b] = -2;
 }
 
 }  // namespace
 
-int onbody_max_blocks(const Handle* h)
+int onbody_max_blocks(const Handle* h, bool enc)
 {
     int occ = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, onbody_kernel<CHUNK_MAX>, FUSED_NT, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, enc ? onbody_kernel<CHUNK_MAX, true> : onbody_kernel<CHUNK_MAX, false>, FUSED_NT, 0);
     int occ2 = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, onbody_kernel<CHUNK_MIN>, FUSED_NT, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, enc ? onbody_kernel<CHUNK_MIN, true> : onbody_kernel<CHUNK_MIN, false>, FUSED_NT, 0);
     if (occ2 < occ) occ = occ2;
     if (occ < 1) occ = 1;
     long long b = (long long)occ * h->num_sms;
@@ -40,8 +87,22 @@ cudaError_t launch_onbody(const Handle* h, const OnBodyArgs& a, int max_blocks)
     OnBodyArgs args = a;
     Workspace ws = h->w;
     void* params[] = {&args, &ws};
-    const void* fn = (h->chunk == CHUNK_MIN) ? (const void*)onbody_kernel<CHUNK_MIN> : (const void*)onbody_kernel<CHUNK_MAX>;
+    const void* fn;
+    if (a.enc.on && a.do_drift)
+        fn = (h->chunk == CHUNK_MIN) ? (const void*)onbody_kernel<CHUNK_MIN, true> : (const void*)onbody_kernel<CHUNK_MAX, true>;
+    else
+        fn = (h->chunk == CHUNK_MIN) ? (const void*)onbody_kernel<CHUNK_MIN, false> : (const void*)onbody_kernel<CHUNK_MAX, false>;
     return cudaLaunchCooperativeKernel(fn, dim3(blocks), dim3(FUSED_NT), params, 0, h->stream);
+}
+
+// Encounter groups of the pair list the last force evaluation left (encounter mode, before the drift).
+cudaError_t launch_groups(const Handle* h)
+{
+    if (h->N == 0) return cudaSuccess;
+    cudaError_t e = cudaMemsetAsync(h->w.glabel, 0xff, (size_t)h->NP * sizeof(int), h->stream);
+    if (e != cudaSuccess) return e;
+    group_kernel<<<1, 1024, 0, h->stream>>>(h->N, h->NP, h->w.pairs, h->w.ctr, (unsigned int)h->pair_cap, h->w.glabel);
+    return cudaGetLastError();
 }
 
 }  // namespace genga

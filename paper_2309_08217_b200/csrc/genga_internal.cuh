@@ -42,6 +42,11 @@ struct Counters {
     unsigned int overflow;       // 1 if the last near-field pass took the exact slow path
     unsigned int ticket;         // block-completion ticket of the momentum reduction (0 between launches)
     unsigned int extent_bits;    // float bits of max(|x|, |y|) over the bodies (Hilbert sort extent)
+    // encounter mode (encounter.cuh; NEXT-1)
+    unsigned int enc_status;     // sticky until read: 1 pair list overflowed, 2 a group had more than enc::GMAX bodies
+    unsigned int enc_groups;     // encounter groups integrated by the last drift
+    unsigned int enc_bodies;     // bodies in those groups
+    unsigned int enc_maxsize;    // largest group of the last drift
 };
 
 struct Workspace {
@@ -61,6 +66,8 @@ struct Workspace {
     unsigned long long* bkeys;  // [NP] the keys grouped by bucket
     int* bigslot;               // [NP] TP2 mode: slot of big body b (b < n_big)
     unsigned int* sortbuf;      // bucket histogram, starts and cursors of the sort
+    int* glabel;                // [2 NP] encounter mode: smallest body index of the body's encounter group (-1: none,
+                                //        -2: group too large, Kepler drift), then the member count per label
     double4* pk64;    // [NP]   (x, y, z, G m)
     float4*  pk32;    // [NP]   pair-interleaved, see above
     double4* aux;     // [NP]   (m, r_crit, a, v_K): what the exact pair rule O3 needs
@@ -91,6 +98,7 @@ struct Handle {
     // internal order (a performance hint only: results never depend on it)
     int mega_blocks[2];          // co-resident blocks of the one-kernel step per precision; 0 = not used, -1 = not queried yet
     int mega_nmax;               // largest N that takes the one-kernel step
+    int enc_blocks;              // co-resident grid of the per-body kernel built with the encounter integrator
     int fused_blocks;            // co-resident blocks of the fused per-body kernel; 0 = cooperative launch unavailable
     bool pend_vel;               // a closing velocity update v += pend_tau a is still owed (api.cu: sequence)
     double pend_tau;
@@ -123,14 +131,23 @@ struct PrepArgs {
     int scaled;                  // FP32 j-records in the mass-scaled form (kick_fp32.cu, SC variants)
     double preshift;             // pending Sun-kick: x += preshift * mom[SLOT_B] / M_star before anything else
 };
+struct EncArgs {                  // encounter mode (encounter.cuh; NEXT-1, reading R11)
+    int on;                        // 0: every body drifts on its Kepler orbit
+    int nsub;                      // RK4 substeps per step for the bodies of an encounter group
+    int pair_rule;
+    unsigned int pair_cap;
+    double G, M_star, n1, n2dt;
+};
 struct OnBodyArgs {               // the fused per-body kernel of the step (fused_step.cu)
     PrepArgs prep;
+    EncArgs enc;
     int do_vel, do_drift, do_prep;
     double tau_v;                  // v += tau_v a          (do_vel)
     double dt, mu;                 // S(dt/2) D(dt) S(dt/2)  (do_drift; the closing S is applied by phase 3)
 };
 constexpr int MOM_MAX_BLOCKS = 2048;   // most blocks whose momentum partials fit the workspace
-int  onbody_max_blocks(const Handle* h);
+int  onbody_max_blocks(const Handle* h, bool enc);
+cudaError_t launch_groups(const Handle* h);                      // encounter groups from the pair list (encounter.cuh)
 cudaError_t launch_onbody(const Handle* h, const OnBodyArgs& a, int max_blocks);
 int  mega_max_blocks(const Handle* h, int precision);            // the one-kernel step of small systems (mega_step.cu)
 cudaError_t launch_step_mega(const Handle* h, const OnBodyArgs& a, int precision, int max_blocks);

@@ -21,6 +21,7 @@ struct NfParams {
     double M_star, n1, n2dt;
     int pair_rule;
     int weight_mode;                               // 0: W = K, 1: W = K - r dK/dr (reading R10)
+    double list_scale;                             // pairs with r < list_scale r_crit,ij are listed (1 unless encounter mode)
     unsigned int cand_cap, pair_cap;
 };
 
@@ -30,6 +31,7 @@ inline NfParams make_nf_params(const Handle* h)
     P.N = h->N; P.nchunk = h->nchunk;
     P.M_star = h->p.M_star; P.n1 = h->p.n1; P.n2dt = h->p.n2 * h->p.dt_rcrit;
     P.pair_rule = h->p.pair_rule; P.weight_mode = h->p.weight_mode;
+    P.list_scale = (h->p.encounter_mode != 0) ? h->p.enc_list_scale : 1.0;
     P.cand_cap = (unsigned int)h->cand_cap; P.pair_cap = (unsigned int)h->pair_cap;
     return P;
 }
@@ -150,7 +152,7 @@ __device__ __forceinline__ void chunk_on_body(const NfParams& P, Workspace& w, c
             const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
             const double r  = sqrt(r2);
             const double rc = pair_rcrit(P, I.m, A.x, I.rc, A.y, I.a, A.z, I.vk, A.w);
-            if ((I.slot < sj) && (r < rc)) encj = w.order[sj];       // coincident bodies (r = 0) are an encounter
+            if ((I.slot < sj) && (r < P.list_scale * rc)) encj = w.order[sj];       // coincident bodies (r = 0) are an encounter
             if (r > 0.0) {
                 const double W = changeover(r, rc, P.weight_mode);
                 if (W != 0.0) {

@@ -13,6 +13,7 @@
 #include <cooperative_groups.h>
 
 #include "genga_internal.cuh"
+#include "encounter.cuh"
 #include "kepler.cuh"
 #include "momentum.cuh"
 #include "prep_tile.cuh"
@@ -60,8 +61,40 @@ __device__ __forceinline__ void block_partial(double p0, double p1, double p2, d
     __syncthreads();
 }
 
+// Encounter mode (NEXT-1, encounter.cuh): the leader of an encounter group advances all its members through
+// S(dt/2) (the shift s) and the flow of H_A,group over dt, writes them back and returns sum m v' of the group.
+static __device__ __noinline__ void drift_group(const EncArgs& E, Workspace& w, int leader, double dt, double s0, double s1, double s2,
+                                         double& p0, double& p1, double& p2, double& mt)
+{
+    enc::GroupState g;
+    const unsigned int total = w.ctr->pair_count;
+    const unsigned int npairs = total < E.pair_cap ? total : E.pair_cap;
+    enc::group_collect(leader, w.pairs, npairs, w.glabel, g, &w.ctr->enc_status);
+    for (int k = 0; k < g.n; ++k) {
+        const int b = g.body[k];
+        g.m[k] = w.m[b];
+        g.x[k][0] = w.x[3 * b] + s0; g.x[k][1] = w.x[3 * b + 1] + s1; g.x[k][2] = w.x[3 * b + 2] + s2;
+        g.v[k][0] = w.v[3 * b];      g.v[k][1] = w.v[3 * b + 1];      g.v[k][2] = w.v[3 * b + 2];
+    }
+    for (int k = 0; k < g.n; ++k)
+        for (int l = 0; l < g.n; ++l) {
+            const int a = g.body[k], b = g.body[l];
+            g.rc[k][l] = (k == l) ? 0.0
+                       : enc::pair_rcrit(E, g.m[k], g.m[l], w.rcrit[a], w.rcrit[b], w.semi[a], w.semi[b], w.vkep[a], w.vkep[b]);
+        }
+    if (dt != 0.0) enc::group_integrate(E, g, dt);
+    for (int k = 0; k < g.n; ++k) {
+        const int b = g.body[k];
+        w.x[3 * b] = g.x[k][0]; w.x[3 * b + 1] = g.x[k][1]; w.x[3 * b + 2] = g.x[k][2];
+        w.v[3 * b] = g.v[k][0]; w.v[3 * b + 1] = g.v[k][1]; w.v[3 * b + 2] = g.v[k][2];
+        p0 = fma(g.m[k], g.v[k][0], p0); p1 = fma(g.m[k], g.v[k][1], p1); p2 = fma(g.m[k], g.v[k][2], p2); mt += g.m[k];
+    }
+    atomicAdd(&w.ctr->enc_groups, 1u); atomicAdd(&w.ctr->enc_bodies, (unsigned int)g.n);
+    atomicMax(&w.ctr->enc_maxsize, (unsigned int)g.n);
+}
+
 // The kernel as a device function (a cooperative 1-D grid of FUSED_NT-thread blocks).
-template <int CHUNK>
+template <int CHUNK, bool ENC = false>
 __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, cg::grid_group& grid)
 {
     __shared__ double sP[4];
@@ -97,6 +130,13 @@ __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, c
         __syncthreads();                                   // sP is rewritten below
         double p0 = 0, p1 = 0, p2 = 0, mt = 0;
         for (int i = gtid; i < N; i += gsz) {
+            if (ENC) {                                     // bodies of an encounter group: their leader moves them
+                const int lab = w.glabel[i];
+                if (lab >= 0) {
+                    if (lab == i) drift_group(A.enc, w, i, A.dt, s0, s1, s2, p0, p1, p2, mt);
+                    continue;
+                }
+            }
             double x0 = w.x[3 * i] + s0, y0 = w.x[3 * i + 1] + s1, z0 = w.x[3 * i + 2] + s2;
             double vx = w.v[3 * i], vy = w.v[3 * i + 1], vz = w.v[3 * i + 2];
             if (A.dt != 0.0) {

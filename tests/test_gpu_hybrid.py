@@ -1,0 +1,161 @@
+"""GPU parity of the opt-in encounter mode (NEXT-1 of SURVEY.md 8(f); reading R11) against the
+oracle's hybrid step: the oracle integrates the flow of H_A for ALL bodies with no lists and no groups, the
+library moves only the bodies of an encounter group that way and every other body on its Kepler orbit."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2309_08217_b200 import binding as B
+from paper_2309_08217_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+G = W.G_DEFAULT
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_cuda():
+    import torch
+    assert torch.cuda.is_available(), "the gpu-marked tests need a CUDA device"
+    B.load()
+
+
+def workload(name, m, x, v_helio, dt, n2, pair_rule):
+    return W.Workload(name, 0, np.ascontiguousarray(m), np.ascontiguousarray(x), np.ascontiguousarray(v_helio), dt, 1,
+                      n2=n2, pair_rule=pair_rule)
+
+
+def oparams(w):
+    return oracle.Params(G=w.G, M_star=w.M_star, n1=w.n1, n2=w.n2, dt_rcrit=w.dt, pair_rule=w.pair_rule, weight_mode=1)
+
+
+def encounter_system():
+    """Two planets of 3e-5 Msun on nearly equal orbits that pass each other deep inside r_crit within a few
+    steps, and two distant spectators (the system of tests/test_oracle_hybrid.py, heliocentric velocities)."""
+    m = np.array([3e-5, 3e-5, 1e-6, 1e-6])
+    a = np.array([1.0, 1.012, 1.7, 2.6])
+    lam = np.array([0.0, -0.035, 2.0, 4.0])
+    x = np.stack([a * np.cos(lam), a * np.sin(lam), 0.002 * np.array([1, -1, 2, -2.0])], axis=1)
+    vk = np.sqrt(G * (1 + m) / a)
+    v = np.stack([-vk * np.sin(lam), vk * np.cos(lam), np.zeros(4)], axis=1)
+    return workload("enc4", m, x, v, 2.0, 0.4, B.PAIR_MAX)
+
+
+def disc_with_planted_groups(n, seed):
+    """A disc of n small bodies in which a handful of pairs and one triple sit inside their changeover zones."""
+    u = W.uniforms(seed, 6 * n).reshape(n, 6)
+    m = 1e-7 * (0.5 + u[:, 0])
+    a = 0.6 + 2.4 * (np.arange(n) + u[:, 1]) / n
+    x, v = W.elements_to_cartesian(G * (1 + m), a, 0.01 * u[:, 2], 0.005 * u[:, 3], 6.28 * u[:, 4], 6.28 * u[:, 5],
+                                   6.28 * ((np.arange(n) * 0.381966) % 1.0))
+    # plant: body k+1 (and k+2 for the triple) next to body k, a fraction of body k's r_crit away
+    for k, members in ((10, 1), (200, 1), (333, 2), (600, 1), (n - 40, 1)):
+        r = np.linalg.norm(x[k])
+        rc = 3.0 * np.cbrt(2 * m[k] / 3.0) * r
+        for q in range(1, members + 1):
+            x[k + q] = x[k] + rc * np.array([0.35 * q, 0.3 * (-1) ** q, 0.05])
+            v[k + q] = v[k] * (1.0 + 2e-4 * q)
+    return workload("disc+groups", m, x, v, 6.0, 0.0, B.PAIR_MUTUAL_HILL)
+
+
+def hybrid(w, **kw):
+    args = dict(weight_mode=1, encounter_mode=1, mega_nmax=-1)
+    args.update(kw)
+    return B.from_workload(w, **args)
+
+
+def state_err(x, v, xo, vo):
+    ex = np.linalg.norm(x - xo, axis=1) / np.linalg.norm(xo, axis=1)
+    ev = np.linalg.norm(v - vo, axis=1) / np.linalg.norm(vo, axis=1)
+    return max(ex.max(), ev.max())
+
+
+def test_hybrid_steps_through_a_close_encounter_match_the_oracle():
+    w = encounter_system()
+    p = oparams(w)
+    nsub = 512
+    xo, vo = w.x.copy(), oracle.to_democratic(w.m, w.v, w.M_star)
+    E0 = oracle.energy_angmom(w.m, xo, vo, oracle.Params(n1=0.0))[0]
+    g = hybrid(w, enc_nsub=nsub, enc_list_scale=1.5)
+    grouped_steps, worst = 0, 0.0
+    for _ in range(30):
+        xo, vo = oracle.step_hybrid(w.m, xo, vo, p, w.dt, nsub=nsub)
+        g.step(w.dt, B.FP64)
+        x, v = (t.cpu().numpy() for t in g.get_state())
+        groups, bodies, largest, status = g.encounter_stats()
+        assert status == 0
+        grouped_steps += groups
+        worst = max(worst, state_err(x, v, xo, vo))
+    E, _ = g.energy_angmom()
+    g.close()
+    assert grouped_steps >= 5                                   # the pair was integrated as a group for several steps
+    assert worst <= 1e-10, worst
+    assert abs(E / E0 - 1) < 1e-6                                # level 0 alone loses 3.5e-4 here (test_oracle_hybrid.py)
+
+
+def test_hybrid_step_fp32_forces():
+    # the kick in FP32 (policy P32), the encounter integration always in FP64
+    w = encounter_system()
+    p = oparams(w)
+    xo, vo = oracle.step_hybrid(w.m, w.x, oracle.to_democratic(w.m, w.v, w.M_star), p, w.dt, nsub=256)
+    g = hybrid(w, enc_nsub=256)
+    g.step(w.dt, B.FP32)
+    x, v = (t.cpu().numpy() for t in g.get_state())
+    groups, bodies, largest, status = g.encounter_stats()
+    g.close()
+    assert (groups, bodies, largest, status) == (1, 2, 2, 0)
+    assert state_err(x, v, xo, vo) <= 1e-7
+
+
+def test_disc_with_pairs_and_a_triple_one_step():
+    n = 1000
+    w = disc_with_planted_groups(n, 4)
+    p = oparams(w)
+    vd = oracle.to_democratic(w.m, w.v, w.M_star)
+    po = oracle.encounter_pairs(w.m, w.x, vd, p)
+    assert len(po) >= 6
+    xo, vo = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=128)
+    xl, vl = oracle.step(w.m, w.x, vd, p, w.dt)
+    assert state_err(xl, vl, xo, vo) > 1e-6                     # the complement matters for the planted bodies
+    for prec, tol in ((B.FP64, 1e-10), (B.FP32, 1e-7)):
+        g = hybrid(w, enc_nsub=128, enc_list_scale=2.0)
+        g.step(w.dt, prec)
+        x, v = (t.cpu().numpy() for t in g.get_state())
+        groups, bodies, largest, status = g.encounter_stats()
+        g.close()
+        assert status == 0 and 3 <= largest <= 8 and groups >= 5 and bodies >= 11, (groups, bodies, largest, status)
+        assert state_err(x, v, xo, vo) <= tol, (prec, state_err(x, v, xo, vo))
+
+
+def test_without_encounters_the_hybrid_step_is_the_level0_step():
+    w = W.config(0)
+    vd = oracle.to_democratic(w.m, w.v, w.M_star)
+    w.n1 = 0.3                                                   # small zones: no pair within 1.5 r_crit in 5 steps
+    assert len(oracle.encounter_pairs(w.m, w.x, vd, oracle.Params(G=w.G, n1=0.6, pair_rule=w.pair_rule))) == 0
+    out = []
+    for mode in (0, 1):
+        g = B.from_workload(w, weight_mode=1, encounter_mode=mode, mega_nmax=-1)
+        g.run(w.dt, 5, B.FP64)
+        out.append([t.cpu().numpy() for t in g.get_state()])
+        if mode:
+            assert g.encounter_stats() == (0, 0, 0, 0)
+        g.close()
+    # same arithmetic in two separately compiled kernels (and grids): equal up to the rounding of the momentum sums
+    assert state_err(out[1][0], out[1][1], out[0][0], out[0][1]) <= 4e-15
+
+
+def test_oversized_groups_are_reported_and_parameters_checked():
+    u = W.uniforms(13, 6 * 800).reshape(800, 6)
+    m = 3e-6 * (0.5 + u[:, 0])
+    x, v = W.elements_to_cartesian(G * (1 + m), 1.0 + 0.02 * u[:, 1], 0.01 * u[:, 2], 0.005 * u[:, 3],
+                                   0.3 * u[:, 4], 0.3 * u[:, 5], 0.2 * u[:, 0])
+    w = workload("ring", m, x, v, 6.0, 0.0, B.PAIR_MUTUAL_HILL)      # a narrow ring: one percolating group
+    g = hybrid(w, pair_capacity=200000)
+    g.step(w.dt, B.FP64)
+    groups, bodies, largest, status = g.encounter_stats()
+    x, v = (t.cpu().numpy() for t in g.get_state())
+    g.close()
+    assert status & 2 and largest <= 8 and np.isfinite(x).all() and np.isfinite(v).all()
+    for bad in (dict(weight_mode=0), dict(n_big=3), dict(enc_list_scale=0.5), dict(enc_list_scale=3.0), dict(no_fused_step=True)):
+        with pytest.raises(Exception):
+            hybrid(w, **bad).close()
