@@ -392,7 +392,7 @@ def cpu_oracle_kick(w, **kw):
     oracle timed beside the GPU per config / per sweep N.  Returns (seconds, pairs/s, threads)."""
     import oracle
     pk = dict(G=w.G, M_star=w.M_star, n1=w.n1, n2=w.n2, dt_rcrit=w.dt, pair_rule=w.pair_rule)
-    pk.update({k: v for k, v in kw.items() if k in ("n1", "n2", "pair_rule", "n_big")})
+    pk.update({k: v for k, v in kw.items() if k in ("n1", "n2", "pair_rule", "n_big", "weight_mode")})
     p = oracle.Params(**pk)
     vd = oracle.to_democratic(w.m, w.v, w.M_star)
     t0 = time.perf_counter()
@@ -445,6 +445,10 @@ def run_report(args):
     w4.nsteps = 50
     cases.append(("4-eq1", w4, {"n1": 3.0, "n2": 0.4, "pair_rule": B.PAIR_MAX,
                                 "pair_capacity": 40 * w4.N, "cand_capacity": 64 * w4.N}))
+    # NEXT-1: the hybrid step (encounter mode, reading R11) on the performance shape, 200 steps
+    w5 = W.config(4)
+    w5.nsteps = 200
+    cases.append(("4-hybrid", w5, {"weight_mode": 1, "encounter_mode": 1, "enc_nsub": 256, "enc_list_scale": 1.5}))
     for cfg, w, kw in cases:
         nb = kw.get("n_big", -1)
         if not args.no_cpu_baseline:                               # the oracle beside it: one kick per config
@@ -470,6 +474,7 @@ def run_report(args):
             E1, L1 = g.energy_angmom()
             enc_last = int(len(g.encounter_pairs(cap=max(8 * w.N + 4096, kw.get("pair_capacity", 0)))))
             st = g.nearfield_stats()
+            enc_stats = g.encounter_stats() if kw.get("encounter_mode") else None
             g.close()
             evals = w.nsteps + 1
             line = {"report": "config", "config": cfg, "workload": w.name, "N": w.N, "dt_days": w.dt, "steps": w.nsteps,
@@ -482,6 +487,10 @@ def run_report(args):
                     "dE_over_E": E1 / E0 - 1.0,
                     "dL_over_L": float(np.linalg.norm(L1) / np.linalg.norm(L0) - 1.0),
                     "encounter_pairs_last_eval": enc_last, "nearfield_candidates_last_eval": st.candidates}
+            if enc_stats is not None:
+                line["encounter_groups_last_drift"] = {"groups": enc_stats[0], "bodies": enc_stats[1], "largest": enc_stats[2],
+                                                       "status": enc_stats[3], "rk4_substeps": kw.get("enc_nsub"),
+                                                       "list_scale": kw.get("enc_list_scale")}
             if cfg == 1:                                           # encounter-pair counts per step (untimed second run)
                 g = B.from_workload(w, **kw)
                 g.set_tuning(0 if prec == B.FP32 else 1, variant)

@@ -115,7 +115,7 @@ typedef struct {
     int    enc_nsub;          /* RK4 substeps per step for the bodies of a group; <= 0: default (256)        */
     double enc_list_scale;    /* encounter mode: pairs with r_ij < enc_list_scale * r_crit,ij are listed (and
                                  grouped), so that a pair that enters its zone DURING the step is already in a
-                                 group.  1 <= enc_list_scale <= lambda_near; <= 0: default (1.5).  Changes the
+                                 group.  1 <= enc_list_scale <= 4; <= 0: default (1.5).  Changes the
                                  list genga_encounter_pairs returns, not the forces.                      */
 } genga_params;
 

@@ -4,6 +4,7 @@
 #include "genga_internal.cuh"
 
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
 #include <new>
 
@@ -48,6 +49,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_bs = take(NP * 4);
     const size_t o_bk = take(NP * 8), o_sb = take((size_t)sort_buffer_words() * 4);
     const size_t o_gl = take(NP * 8);          // labels [NP], member counts [NP]
+    const size_t o_gi = take(std::min((size_t)pair_cap, NP / 2) * 9 * 4);      // encounter groups: count + 8 members each
     if (w && base) {
         char* b = static_cast<char*>(base);
         w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
@@ -60,7 +62,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
         w->mom = (double*)(b + o_mom);
         w->bigslot = (int*)(b + o_bs);
         w->bkeys = (unsigned long long*)(b + o_bk); w->sortbuf = (unsigned int*)(b + o_sb);
-        w->glabel = (int*)(b + o_gl);
+        w->glabel = (int*)(b + o_gl); w->ginfo = (int*)(b + o_gi);
     }
     return off;
 }
@@ -132,6 +134,8 @@ static PrepArgs make_prep_args(const Handle* h, int precision, double preshift)
         a.floor_rel = (float)(h->near_floor > 3.814697265625e-06 ? h->near_floor : 3.814697265625e-06);
     }
     else                         { a.lambda = 1.0f;                  a.floor_rel = 0.0f; }
+    // encounter mode lists (and must therefore look at) every pair within enc_list_scale r_crit
+    if (h->p.encounter_mode == 1 && a.lambda < (float)h->p.enc_list_scale) a.lambda = (float)h->p.enc_list_scale;
     return a;
 }
 
@@ -386,7 +390,7 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
             h->enc_blocks = onbody_max_blocks(h, true);
             h->p.enc_nsub = p->enc_nsub > 0 ? p->enc_nsub : 256;
             h->p.enc_list_scale = p->enc_list_scale > 0.0 ? p->enc_list_scale : 1.5;
-            if (h->p.enc_list_scale < 1.0 || h->p.enc_list_scale > h->lambda_near) { delete h; return GENGA_EINVAL; }
+            if (h->p.enc_list_scale < 1.0 || h->p.enc_list_scale > 4.0) { delete h; return GENGA_EINVAL; }
         }
         h->mega_blocks[0] = h->mega_blocks[1] = -1;
         h->mega_nmax = p->mega_nmax > 0 ? p->mega_nmax : (p->mega_nmax < 0 ? 0 : 3000);

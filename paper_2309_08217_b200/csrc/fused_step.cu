@@ -19,10 +19,11 @@ onbody_kernel(OnBodyArgs A, Workspace w)
 // Encounter groups (NEXT-1): connected components of the encounter-pair graph by label propagation over the
 // pair list; glabel[b] = smallest body index of b's component, -1 for bodies in no pair (preset by the
 // launcher), -2 for the bodies of a component with more than enc::GMAX members (status bit 2; they drift on
-// their Kepler orbits).  One block.
+// their Kepler orbits).  Then every component gets a group index g and registers its members in
+// ginfo[g * GINFO ..] (count, members; in no particular order: the integrating warp sorts them).  One block.
 __global__ void __launch_bounds__(1024)
 group_kernel(int N, int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr, unsigned int pair_cap,
-             int* __restrict__ glabel)
+             int* __restrict__ glabel, int* __restrict__ ginfo)
 {
     __shared__ int changed;
     int* gcount = glabel + NP;
@@ -61,6 +62,24 @@ group_kernel(int N, int NP, const int2* __restrict__ pairs, Counters* __restrict
     }
     __syncthreads();
     for (int b = threadIdx.x; b < N; b += blockDim.x) if (glabel[b] == b && gcount[b] > enc::GMAX) glabel[b] = -2;
+    __syncthreads();
+    for (int b = threadIdx.x; b < N; b += blockDim.x)
+        if (glabel[b] == b) {                                               // leader of a valid group
+            const unsigned int g = atomicAdd(&ctr->enc_groups, 1u);
+            const int cnt = gcount[b];
+            atomicAdd(&ctr->enc_bodies, (unsigned int)cnt); atomicMax(&ctr->enc_maxsize, (unsigned int)cnt);
+            ginfo[g * enc::GINFO] = 0;
+            gcount[b] = (int)g;
+        }
+    __syncthreads();
+    for (int b = threadIdx.x; b < N; b += blockDim.x) {
+        const int l = glabel[b];
+        if (l >= 0) {
+            int* info = ginfo + (size_t)gcount[l] * enc::GINFO;
+            const int k = atomicAdd(info, 1);
+            if (k < enc::GMAX) info[1 + k] = b;
+        }
+    }
 }
 
 }  // namespace
@@ -101,7 +120,7 @@ cudaError_t launch_groups(const Handle* h)
     if (h->N == 0) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(h->w.glabel, 0xff, (size_t)h->NP * sizeof(int), h->stream);
     if (e != cudaSuccess) return e;
-    group_kernel<<<1, 1024, 0, h->stream>>>(h->N, h->NP, h->w.pairs, h->w.ctr, (unsigned int)h->pair_cap, h->w.glabel);
+    group_kernel<<<1, 1024, 0, h->stream>>>(h->N, h->NP, h->w.pairs, h->w.ctr, (unsigned int)h->pair_cap, h->w.glabel, h->w.ginfo);
     return cudaGetLastError();
 }
 

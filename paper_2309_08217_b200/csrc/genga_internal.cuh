@@ -67,7 +67,8 @@ struct Workspace {
     int* bigslot;               // [NP] TP2 mode: slot of big body b (b < n_big)
     unsigned int* sortbuf;      // bucket histogram, starts and cursors of the sort
     int* glabel;                // [2 NP] encounter mode: smallest body index of the body's encounter group (-1: none,
-                                //        -2: group too large, Kepler drift), then the member count per label
+                                //        -2: group too large, Kepler drift), then [NP] member count / group index per label
+    int* ginfo;                 // [enc::GINFO x max groups] per group: member count, members
     double4* pk64;    // [NP]   (x, y, z, G m)
     float4*  pk32;    // [NP]   pair-interleaved, see above
     double4* aux;     // [NP]   (m, r_crit, a, v_K): what the exact pair rule O3 needs

@@ -2,6 +2,7 @@
 //   phase 1  v_i += tau_v a_i (row a6, closing the previous kick)      and  P  = sum m v   (grid-wide)
 //   phase 2  x_i += (dt/2) P / M_star (row a7, Sun-kick, reading G3), Kepler drift D(dt) (row a8,
 //            always FP64)                                  and  P' = sum m v'  (grid-wide)
+//            [ENC: the bodies of an encounter group are advanced by one warp per group instead, encounter.cuh]
 //   phase 3  x_i += (dt/2) P' / M_star, then r_crit (Eq. 1), packing and bounds (rows a1, a2) for the
 //            next force evaluation.
 // Each phase is optional.  The two grid-wide sums are block partials combined by EVERY block in the
@@ -61,38 +62,6 @@ __device__ __forceinline__ void block_partial(double p0, double p1, double p2, d
     __syncthreads();
 }
 
-// Encounter mode (NEXT-1, encounter.cuh): the leader of an encounter group advances all its members through
-// S(dt/2) (the shift s) and the flow of H_A,group over dt, writes them back and returns sum m v' of the group.
-static __device__ __noinline__ void drift_group(const EncArgs& E, Workspace& w, int leader, double dt, double s0, double s1, double s2,
-                                         double& p0, double& p1, double& p2, double& mt)
-{
-    enc::GroupState g;
-    const unsigned int total = w.ctr->pair_count;
-    const unsigned int npairs = total < E.pair_cap ? total : E.pair_cap;
-    enc::group_collect(leader, w.pairs, npairs, w.glabel, g, &w.ctr->enc_status);
-    for (int k = 0; k < g.n; ++k) {
-        const int b = g.body[k];
-        g.m[k] = w.m[b];
-        g.x[k][0] = w.x[3 * b] + s0; g.x[k][1] = w.x[3 * b + 1] + s1; g.x[k][2] = w.x[3 * b + 2] + s2;
-        g.v[k][0] = w.v[3 * b];      g.v[k][1] = w.v[3 * b + 1];      g.v[k][2] = w.v[3 * b + 2];
-    }
-    for (int k = 0; k < g.n; ++k)
-        for (int l = 0; l < g.n; ++l) {
-            const int a = g.body[k], b = g.body[l];
-            g.rc[k][l] = (k == l) ? 0.0
-                       : enc::pair_rcrit(E, g.m[k], g.m[l], w.rcrit[a], w.rcrit[b], w.semi[a], w.semi[b], w.vkep[a], w.vkep[b]);
-        }
-    if (dt != 0.0) enc::group_integrate(E, g, dt);
-    for (int k = 0; k < g.n; ++k) {
-        const int b = g.body[k];
-        w.x[3 * b] = g.x[k][0]; w.x[3 * b + 1] = g.x[k][1]; w.x[3 * b + 2] = g.x[k][2];
-        w.v[3 * b] = g.v[k][0]; w.v[3 * b + 1] = g.v[k][1]; w.v[3 * b + 2] = g.v[k][2];
-        p0 = fma(g.m[k], g.v[k][0], p0); p1 = fma(g.m[k], g.v[k][1], p1); p2 = fma(g.m[k], g.v[k][2], p2); mt += g.m[k];
-    }
-    atomicAdd(&w.ctr->enc_groups, 1u); atomicAdd(&w.ctr->enc_bodies, (unsigned int)g.n);
-    atomicMax(&w.ctr->enc_maxsize, (unsigned int)g.n);
-}
-
 // The kernel as a device function (a cooperative 1-D grid of FUSED_NT-thread blocks).
 template <int CHUNK, bool ENC = false>
 __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, cg::grid_group& grid)
@@ -130,13 +99,7 @@ __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, c
         __syncthreads();                                   // sP is rewritten below
         double p0 = 0, p1 = 0, p2 = 0, mt = 0;
         for (int i = gtid; i < N; i += gsz) {
-            if (ENC) {                                     // bodies of an encounter group: their leader moves them
-                const int lab = w.glabel[i];
-                if (lab >= 0) {
-                    if (lab == i) drift_group(A.enc, w, i, A.dt, s0, s1, s2, p0, p1, p2, mt);
-                    continue;
-                }
-            }
+            if (ENC) { if (w.glabel[i] >= 0) continue; }   // bodies of an encounter group: moved by their group's warp
             double x0 = w.x[3 * i] + s0, y0 = w.x[3 * i + 1] + s1, z0 = w.x[3 * i + 2] + s2;
             double vx = w.v[3 * i], vy = w.v[3 * i + 1], vz = w.v[3 * i + 2];
             if (A.dt != 0.0) {
@@ -146,6 +109,20 @@ __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, c
             w.x[3 * i] = x0; w.x[3 * i + 1] = y0; w.x[3 * i + 2] = z0;
             const double mi = w.m[i];
             p0 = fma(mi, vx, p0); p1 = fma(mi, vy, p1); p2 = fma(mi, vz, p2); mt += mi;
+        }
+        if (ENC) {
+            // encounter mode (NEXT-1, encounter.cuh): one warp per encounter group advances its members through the
+            // same S(dt/2) and the flow of H_A,group over dt; then their m v' joins the sum, each body's in the
+            // thread that owns the body (so the sum does not depend on which warp moved which group)
+            const int ngroups = (int)__ldcg(&w.ctr->enc_groups);
+            for (int g = gtid >> 5; g < ngroups; g += gsz >> 5) enc::warp_group(A.enc, w, g, A.dt, s0, s1, s2);
+            grid.sync();
+            for (int i = gtid; i < N; i += gsz)
+                if (w.glabel[i] >= 0) {
+                    const double mi = w.m[i];
+                    p0 = fma(mi, __ldcg(&w.v[3 * i]), p0); p1 = fma(mi, __ldcg(&w.v[3 * i + 1]), p1);
+                    p2 = fma(mi, __ldcg(&w.v[3 * i + 2]), p2); mt += mi;
+                }
         }
         block_partial(p0, p1, p2, mt, part2);
         grid.sync();

@@ -156,6 +156,6 @@ def test_oversized_groups_are_reported_and_parameters_checked():
     x, v = (t.cpu().numpy() for t in g.get_state())
     g.close()
     assert status & 2 and largest <= 8 and np.isfinite(x).all() and np.isfinite(v).all()
-    for bad in (dict(weight_mode=0), dict(n_big=3), dict(enc_list_scale=0.5), dict(enc_list_scale=3.0), dict(no_fused_step=True)):
+    for bad in (dict(weight_mode=0), dict(n_big=3), dict(enc_list_scale=0.5), dict(enc_list_scale=5.0), dict(no_fused_step=True)):
         with pytest.raises(Exception):
             hybrid(w, **bad).close()
