@@ -448,7 +448,8 @@ def run_report(args):
     # NEXT-1: the hybrid step (encounter mode, reading R11) on the performance shape, 200 steps
     w5 = W.config(4)
     w5.nsteps = 200
-    cases.append(("4-hybrid", w5, {"weight_mode": 1, "encounter_mode": 1, "enc_nsub": 256, "enc_list_scale": 1.5}))
+    cases.append(("4-hybrid", w5, {"weight_mode": 1, "encounter_mode": 1, "enc_nsub": 256, "enc_list_scale": 8.0,
+                                     "enc_list_vfactor": 1.25, "cand_capacity": 64 * w5.N}))
     for cfg, w, kw in cases:
         nb = kw.get("n_big", -1)
         if not args.no_cpu_baseline:                               # the oracle beside it: one kick per config
@@ -489,8 +490,8 @@ def run_report(args):
                     "encounter_pairs_last_eval": enc_last, "nearfield_candidates_last_eval": st.candidates}
             if enc_stats is not None:
                 line["encounter_groups_last_drift"] = {"groups": enc_stats[0], "bodies": enc_stats[1], "largest": enc_stats[2],
-                                                       "status": enc_stats[3], "rk4_substeps": kw.get("enc_nsub"),
-                                                       "list_scale": kw.get("enc_list_scale")}
+                                                       "missed_pairs_whole_run": enc_stats[3], "status": enc_stats[4], "rk4_substeps": kw.get("enc_nsub"),
+                                                       "list_scale": kw.get("enc_list_scale"), "list_vfactor": kw.get("enc_list_vfactor")}
             if cfg == 1:                                           # encounter-pair counts per step (untimed second run)
                 g = B.from_workload(w, **kw)
                 g.set_tuning(0 if prec == B.FP32 else 1, variant)

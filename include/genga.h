@@ -113,10 +113,15 @@ typedef struct {
                                  classical RK4 substeps, r_crit,ij held at the opening evaluation's values.
                                  Requires weight_mode = 1, n_big < 0 and the cooperative per-body kernel.    */
     int    enc_nsub;          /* RK4 substeps per step for the bodies of a group; <= 0: default (256)        */
-    double enc_list_scale;    /* encounter mode: pairs with r_ij < enc_list_scale * r_crit,ij are listed (and
-                                 grouped), so that a pair that enters its zone DURING the step is already in a
-                                 group.  1 <= enc_list_scale <= 4; <= 0: default (1.5).  Changes the
-                                 list genga_encounter_pairs returns, not the forces.                      */
+    double enc_list_scale;    /* encounter mode: which pairs OUTSIDE their zone are listed (and grouped) as well, so that
+                                 a pair that enters its zone DURING the step is already in a group: those with
+                                 r_ij < enc_list_scale * r_crit,ij  and  r_ij - r_crit,ij < enc_list_vfactor * dt * |v_i - v_j|
+                                 (dt: the step of the running genga_step/run/leapfrog call; params.dt_rcrit before the
+                                 first).  1 <= enc_list_scale <= 8, <= 0: default (8).  Changes the list
+                                 genga_encounter_pairs returns, not the forces.  Pairs that got into their zone
+                                 un-grouped all the same are counted (genga_encounter_stats).                       */
+    double enc_list_vfactor;  /* see enc_list_scale.  0: default (1.25); < 0: no velocity test, every pair inside
+                                 enc_list_scale * r_crit,ij is listed.                                               */
 } genga_params;
 
 /* Fill *p with the defaults: G = k^2 (k = 0.01720209895), M_star = 1, n1 = 3, n2 = 0,
@@ -185,11 +190,14 @@ int genga_get_rcrit(genga_handle h, double* rcrit);      /* DEVICE [N]: r_crit,i
  * whether the candidate list overflowed (exact slow path taken).  HOST outputs.  Synchronises.  */
 int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed);
 
-/* Encounter mode: the groups the last drift integrated (their number, the bodies in them, the largest) and
- * a status mask, cleared by this call: bit 0 the pair list overflowed when the groups were formed (raise
- * pair_capacity), bit 1 a group had more than 8 bodies (its bodies drifted on their Kepler orbits instead).
- * HOST outputs, NULL = skip.  Synchronises.  GENGA_EINVAL unless params.encounter_mode = 1.          */
-int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest, int* status);
+/* Encounter mode: the groups the last drift integrated (their number, the bodies in them, the largest), the
+ * number of pairs that a force evaluation found INSIDE their zone (r_ij < r_crit,ij) although the drift that led
+ * there had not moved them as one group (they entered un-grouped: raise enc_list_scale or shorten dt), and a
+ * status mask; count and mask are cleared by this call.  Mask: 1 the pair list overflowed when the groups were
+ * formed (raise pair_capacity), 2 a group had more than 8 bodies (its bodies drifted on their Kepler orbits
+ * instead), 4 missed_pairs > 0.  HOST outputs, NULL = skip.  Synchronises.  GENGA_EINVAL unless
+ * params.encounter_mode = 1.                                                                          */
+int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest, int* missed_pairs, int* status);
 
 /* Per-kernel device timing.  enable is a bit mask: bit k brackets every launch of kernel class k with
  * CUDA events on params.stream; classes: 0 all-pairs kick kernel, 1 near-field kernel, 2 prep kernel,

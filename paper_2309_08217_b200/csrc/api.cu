@@ -3,6 +3,7 @@
 // here; every step of the path runs in the CUDA kernels of this directory.
 #include "genga_internal.cuh"
 
+#include <cmath>
 #include <cstdio>
 #include <algorithm>
 #include <cstring>
@@ -186,6 +187,7 @@ static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_d
         e = launch_groups(h);
         ++h->launches;
         if (e != cudaSuccess) return cuda_fail(e, "group_kernel");
+        h->enc_labels_valid = true;
     }
     { ProfScope ps(h, do_drift ? 3 : 2); e = launch_onbody(h, a, (enc && h->enc_blocks < h->fused_blocks) ? h->enc_blocks : h->fused_blocks); }
     ++h->launches;
@@ -283,6 +285,7 @@ static int sequence(genga_handle h, int precision, bool lead_kick, double tau_fi
     bool pending = h->pend_vel;
     double tau_prev = h->pend_tau;
     h->pend_vel = false;
+    if (n_sds > 0) h->enc_dt = std::fabs(dt);                        // encounter mode: the listings of this sequence look dt ahead
     const bool mega = mega_ready(h, precision);                      // small system: one launch per force evaluation
     if (lead_kick) {
         if (mega) { if ((rc = step_mega(h, precision, pending, tau_prev, false, 0.0)) != GENGA_OK) return rc; }
@@ -332,7 +335,7 @@ void genga_default_params(genga_params* p)
     p->chunk = 0;
     p->mega_nmax = 0;
     p->weight_mode = 0;
-    p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0;
+    p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0; p->enc_list_vfactor = 0.0;
 }
 
 size_t genga_workspace_bytes(int N, const genga_params* p)
@@ -389,8 +392,10 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
             if (!coop) { delete h; return GENGA_EINVAL; }
             h->enc_blocks = onbody_max_blocks(h, true);
             h->p.enc_nsub = p->enc_nsub > 0 ? p->enc_nsub : 256;
-            h->p.enc_list_scale = p->enc_list_scale > 0.0 ? p->enc_list_scale : 1.5;
-            if (h->p.enc_list_scale < 1.0 || h->p.enc_list_scale > 4.0) { delete h; return GENGA_EINVAL; }
+            h->p.enc_list_scale = p->enc_list_scale > 0.0 ? p->enc_list_scale : 8.0;
+            h->p.enc_list_vfactor = p->enc_list_vfactor == 0.0 ? 1.25 : p->enc_list_vfactor;
+            h->enc_dt = std::fabs(p->dt_rcrit);
+            if (h->p.enc_list_scale < 1.0 || h->p.enc_list_scale > 8.0) { delete h; return GENGA_EINVAL; }
         }
         h->mega_blocks[0] = h->mega_blocks[1] = -1;
         h->mega_nmax = p->mega_nmax > 0 ? p->mega_nmax : (p->mega_nmax < 0 ? 0 : 3000);
@@ -426,7 +431,7 @@ static int set_state_impl(genga_handle h, const double* m, const double* x, cons
     const size_t n = (size_t)h->N;
     if (n == 0) return GENGA_OK;
     if (m) CU(cudaMemcpyAsync(h->w.m, m, n * 8, kind, h->stream));
-    if (x) CU(cudaMemcpyAsync(h->w.x, x, n * 24, kind, h->stream));
+    if (x) { CU(cudaMemcpyAsync(h->w.x, x, n * 24, kind, h->stream)); h->enc_labels_valid = false; }
     if (v) { CU(cudaMemcpyAsync(h->w.v, v, n * 24, kind, h->stream)); h->mom_a_valid = false; }
     if (m) h->mom_a_valid = false;
     if (m) { launch_hcbrt(h); LAUNCHED(h, "hcbrt_kernel"); }
@@ -471,6 +476,7 @@ int genga_drift(genga_handle h, double dt)
     { ProfScope ps(h, 3); launch_drift(h, dt); }
     LAUNCHED(h, "drift_kernel");
     h->mom_a_valid = false;
+    h->enc_labels_valid = false;                     // a plain Kepler drift: no groups led to these positions
     return GENGA_OK;
 }
 
@@ -601,7 +607,7 @@ int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed
     return GENGA_OK;
 }
 
-int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest, int* status)
+int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest, int* missed_pairs, int* status)
 {
     if (!h || h->p.encounter_mode != 1) return GENGA_EINVAL;
     Counters c;
@@ -609,11 +615,14 @@ int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest
     if (h->N) {
         CU(cudaMemcpyAsync(&c, h->w.ctr, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
         CU(cudaStreamSynchronize(h->stream));
+        if (c.enc_missed) c.enc_status |= 4u;
         if (c.enc_status) CU(cudaMemsetAsync(&h->w.ctr->enc_status, 0, sizeof(unsigned int), h->stream));
+        if (c.enc_missed) CU(cudaMemsetAsync(&h->w.ctr->enc_missed, 0, sizeof(unsigned int), h->stream));
     }
     if (groups) *groups = (int)c.enc_groups;
     if (bodies) *bodies = (int)c.enc_bodies;
     if (largest) *largest = (int)c.enc_maxsize;
+    if (missed_pairs) *missed_pairs = (int)c.enc_missed;
     if (status) *status = (int)c.enc_status;
     return GENGA_OK;
 }

@@ -47,6 +47,7 @@ struct Counters {
     unsigned int enc_groups;     // encounter groups integrated by the last drift
     unsigned int enc_bodies;     // bodies in those groups
     unsigned int enc_maxsize;    // largest group of the last drift
+    unsigned int enc_missed;     // sticky until read: pairs found inside their zone after a drift that had not grouped them
 };
 
 struct Workspace {
@@ -100,6 +101,8 @@ struct Handle {
     int mega_blocks[2];          // co-resident blocks of the one-kernel step per precision; 0 = not used, -1 = not queried yet
     int mega_nmax;               // largest N that takes the one-kernel step
     int enc_blocks;              // co-resident grid of the per-body kernel built with the encounter integrator
+    bool enc_labels_valid;       // glabel holds the groups of the drift that led to the current positions
+    double enc_dt;               // |dt| of the drift the next listing is for (the last sequence's; params.dt_rcrit before any)
     int fused_blocks;            // co-resident blocks of the fused per-body kernel; 0 = cooperative launch unavailable
     bool pend_vel;               // a closing velocity update v += pend_tau a is still owed (api.cu: sequence)
     double pend_tau;

@@ -22,6 +22,8 @@ struct NfParams {
     int pair_rule;
     int weight_mode;                               // 0: W = K, 1: W = K - r dK/dr (reading R10)
     double list_scale;                             // pairs with r < list_scale r_crit,ij are listed (1 unless encounter mode)
+    double list_vdt;                               // ... and, if >= 0, only those with r - r_crit,ij < list_vdt |v_i - v_j|
+    int check_missed;                              // encounter mode: count pairs inside their zone that the last drift had not grouped
     unsigned int cand_cap, pair_cap;
 };
 
@@ -32,6 +34,8 @@ inline NfParams make_nf_params(const Handle* h)
     P.M_star = h->p.M_star; P.n1 = h->p.n1; P.n2dt = h->p.n2 * h->p.dt_rcrit;
     P.pair_rule = h->p.pair_rule; P.weight_mode = h->p.weight_mode;
     P.list_scale = (h->p.encounter_mode != 0) ? h->p.enc_list_scale : 1.0;
+    P.list_vdt = (h->p.encounter_mode != 0 && h->p.enc_list_vfactor >= 0.0) ? h->p.enc_list_vfactor * h->enc_dt : -1.0;
+    P.check_missed = (h->p.encounter_mode != 0 && h->enc_labels_valid) ? 1 : 0;
     P.cand_cap = (unsigned int)h->cand_cap; P.pair_cap = (unsigned int)h->pair_cap;
     return P;
 }
@@ -152,7 +156,20 @@ __device__ __forceinline__ void chunk_on_body(const NfParams& P, Workspace& w, c
             const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
             const double r  = sqrt(r2);
             const double rc = pair_rcrit(P, I.m, A.x, I.rc, A.y, I.a, A.z, I.vk, A.w);
-            if ((I.slot < sj) && (r < P.list_scale * rc)) encj = w.order[sj];       // coincident bodies (r = 0) are an encounter
+            if ((I.slot < sj) && (r < P.list_scale * rc)) {                           // coincident bodies (r = 0) are an encounter
+                const int bj = w.order[sj];
+                bool listed = true;
+                if (!(r < rc) && P.list_vdt >= 0.0) {      // encounter mode: outside the zone, listed if it can get there in a step
+                    const double u0 = w.v[3 * bj] - w.v[3 * I.body], u1 = w.v[3 * bj + 1] - w.v[3 * I.body + 1],
+                                 u2 = w.v[3 * bj + 2] - w.v[3 * I.body + 2];
+                    listed = (r - rc) < P.list_vdt * sqrt(fma(u2, u2, fma(u1, u1, u0 * u0)));
+                }
+                if (listed) encj = bj;
+                if (P.check_missed && (r < rc)) {          // in its zone now: was it moved as a group?
+                    const int la = w.glabel[I.body], lb = w.glabel[bj];
+                    if (la != -2 && lb != -2 && (la < 0 || la != lb)) atomicAdd(&w.ctr->enc_missed, 1u);
+                }
+            }
             if (r > 0.0) {
                 const double W = changeover(r, rc, P.weight_mode);
                 if (W != 0.0) {

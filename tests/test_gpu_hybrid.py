@@ -29,16 +29,16 @@ def oparams(w):
     return oracle.Params(G=w.G, M_star=w.M_star, n1=w.n1, n2=w.n2, dt_rcrit=w.dt, pair_rule=w.pair_rule, weight_mode=1)
 
 
-def encounter_system():
+def encounter_system(lam1=-0.035, dt=2.0):
     """Two planets of 3e-5 Msun on nearly equal orbits that pass each other deep inside r_crit within a few
     steps, and two distant spectators (the system of tests/test_oracle_hybrid.py, heliocentric velocities)."""
     m = np.array([3e-5, 3e-5, 1e-6, 1e-6])
     a = np.array([1.0, 1.012, 1.7, 2.6])
-    lam = np.array([0.0, -0.035, 2.0, 4.0])
+    lam = np.array([0.0, lam1, 2.0, 4.0])
     x = np.stack([a * np.cos(lam), a * np.sin(lam), 0.002 * np.array([1, -1, 2, -2.0])], axis=1)
     vk = np.sqrt(G * (1 + m) / a)
     v = np.stack([-vk * np.sin(lam), vk * np.cos(lam), np.zeros(4)], axis=1)
-    return workload("enc4", m, x, v, 2.0, 0.4, B.PAIR_MAX)
+    return workload("enc4", m, x, v, dt, 0.4, B.PAIR_MAX)
 
 
 def disc_with_planted_groups(n, seed):
@@ -76,14 +76,14 @@ def test_hybrid_steps_through_a_close_encounter_match_the_oracle():
     nsub = 512
     xo, vo = w.x.copy(), oracle.to_democratic(w.m, w.v, w.M_star)
     E0 = oracle.energy_angmom(w.m, xo, vo, oracle.Params(n1=0.0))[0]
-    g = hybrid(w, enc_nsub=nsub, enc_list_scale=1.5)
+    g = hybrid(w, enc_nsub=nsub)                                 # default listing: 8 r_crit, velocity test 1.25
     grouped_steps, worst = 0, 0.0
     for _ in range(30):
         xo, vo = oracle.step_hybrid(w.m, xo, vo, p, w.dt, nsub=nsub)
         g.step(w.dt, B.FP64)
         x, v = (t.cpu().numpy() for t in g.get_state())
-        groups, bodies, largest, status = g.encounter_stats()
-        assert status == 0
+        groups, bodies, largest, missed, status = g.encounter_stats()
+        assert status == 0 and missed == 0
         grouped_steps += groups
         worst = max(worst, state_err(x, v, xo, vo))
     E, _ = g.energy_angmom()
@@ -91,6 +91,22 @@ def test_hybrid_steps_through_a_close_encounter_match_the_oracle():
     assert grouped_steps >= 5                                   # the pair was integrated as a group for several steps
     assert worst <= 1e-10, worst
     assert abs(E / E0 - 1) < 1e-6                                # level 0 alone loses 3.5e-4 here (test_oracle_hybrid.py)
+
+
+def test_a_pair_that_enters_its_zone_ungrouped_is_reported():
+    # listing only r < r_crit (enc_list_scale = 1): the step in which the two planets cross into their zone moves
+    # them on Kepler orbits, and the next force evaluation says so
+    w = encounter_system(lam1=0.09, dt=6.0)                      # starts at 1.4 r_crit, closing by 0.03 r_crit per step
+    g = hybrid(w, enc_nsub=64, enc_list_scale=1.0)
+    seen, flagged = 0, 0
+    for _ in range(40):
+        g.step(w.dt, B.FP64)
+        groups, bodies, largest, missed, status = g.encounter_stats()
+        seen += missed
+        flagged += bool(status & 4)
+        assert (missed > 0) == bool(status & 4)
+    g.close()
+    assert seen >= 1 and flagged >= 1
 
 
 def test_hybrid_step_fp32_forces():
@@ -101,9 +117,9 @@ def test_hybrid_step_fp32_forces():
     g = hybrid(w, enc_nsub=256)
     g.step(w.dt, B.FP32)
     x, v = (t.cpu().numpy() for t in g.get_state())
-    groups, bodies, largest, status = g.encounter_stats()
+    groups, bodies, largest, missed, status = g.encounter_stats()
     g.close()
-    assert (groups, bodies, largest, status) == (1, 2, 2, 0)
+    assert (groups, bodies, largest, missed, status) == (1, 2, 2, 0, 0)
     assert state_err(x, v, xo, vo) <= 1e-7
 
 
@@ -118,13 +134,38 @@ def test_disc_with_pairs_and_a_triple_one_step():
     xl, vl = oracle.step(w.m, w.x, vd, p, w.dt)
     assert state_err(xl, vl, xo, vo) > 1e-6                     # the complement matters for the planted bodies
     for prec, tol in ((B.FP64, 1e-10), (B.FP32, 1e-7)):
-        g = hybrid(w, enc_nsub=128, enc_list_scale=2.0)
+        g = hybrid(w, enc_nsub=128)
         g.step(w.dt, prec)
         x, v = (t.cpu().numpy() for t in g.get_state())
-        groups, bodies, largest, status = g.encounter_stats()
+        groups, bodies, largest, missed, status = g.encounter_stats()
         g.close()
+        assert missed == 0
         assert status == 0 and 3 <= largest <= 8 and groups >= 5 and bodies >= 11, (groups, bodies, largest, status)
         assert state_err(x, v, xo, vo) <= tol, (prec, state_err(x, v, xo, vo))
+
+
+def test_hot_disc_pairs_entering_their_zones_are_grouped_in_time():
+    # the performance shape at N = 4000: bodies cross a good part of a zone per step (velocity dispersion x dt is
+    # 0.2 r_crit and more), so pairs ENTER their zones during a step.  The oracle has no lists; agreement over
+    # consecutive steps says the velocity-aware listing grouped them before they got there.
+    w = W.config(4, 4000)
+    p = oparams(w)
+    xo, vo = w.x.copy(), oracle.to_democratic(w.m, w.v, w.M_star)
+    g = hybrid(w, enc_nsub=64)
+    g1 = hybrid(w, enc_nsub=64, enc_list_scale=1.0)              # lists r < r_crit only: entering pairs are missed
+    worst, missed, missed1, grouped = 0.0, 0, 0, 0
+    for _ in range(6):
+        xo, vo = oracle.step_hybrid(w.m, xo, vo, p, w.dt, nsub=64)
+        g.step(w.dt, B.FP64)
+        g1.step(w.dt, B.FP64)
+        x, v = (t.cpu().numpy() for t in g.get_state())
+        st = g.encounter_stats()
+        assert st[4] == 0
+        grouped += st[0]; missed += st[3]; missed1 += g1.encounter_stats()[3]
+        worst = max(worst, state_err(x, v, xo, vo))
+    g.close(); g1.close()
+    assert grouped >= 3 and missed == 0 and worst <= 1e-10, (grouped, missed, worst)
+    assert missed1 >= 1, missed1                                 # the check itself sees what the plain listing misses
 
 
 def test_without_encounters_the_hybrid_step_is_the_level0_step():
@@ -138,7 +179,7 @@ def test_without_encounters_the_hybrid_step_is_the_level0_step():
         g.run(w.dt, 5, B.FP64)
         out.append([t.cpu().numpy() for t in g.get_state()])
         if mode:
-            assert g.encounter_stats() == (0, 0, 0, 0)
+            assert g.encounter_stats() == (0, 0, 0, 0, 0)
         g.close()
     # same arithmetic in two separately compiled kernels (and grids): equal up to the rounding of the momentum sums
     assert state_err(out[1][0], out[1][1], out[0][0], out[0][1]) <= 4e-15
@@ -152,10 +193,10 @@ def test_oversized_groups_are_reported_and_parameters_checked():
     w = workload("ring", m, x, v, 6.0, 0.0, B.PAIR_MUTUAL_HILL)      # a narrow ring: one percolating group
     g = hybrid(w, pair_capacity=200000)
     g.step(w.dt, B.FP64)
-    groups, bodies, largest, status = g.encounter_stats()
+    groups, bodies, largest, missed, status = g.encounter_stats()
     x, v = (t.cpu().numpy() for t in g.get_state())
     g.close()
     assert status & 2 and largest <= 8 and np.isfinite(x).all() and np.isfinite(v).all()
-    for bad in (dict(weight_mode=0), dict(n_big=3), dict(enc_list_scale=0.5), dict(enc_list_scale=5.0), dict(no_fused_step=True)):
+    for bad in (dict(weight_mode=0), dict(n_big=3), dict(enc_list_scale=0.5), dict(enc_list_scale=9.0), dict(no_fused_step=True)):
         with pytest.raises(Exception):
             hybrid(w, **bad).close()
