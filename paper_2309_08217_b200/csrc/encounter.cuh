@@ -144,6 +144,7 @@ __device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, int
     if (dt != 0.0) {
         if (n == 2)      integrate<2>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2);
         else if (n == 3) integrate<3>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2);
+        else if (n == 4) integrate<4>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2);
         else             integrate<0>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2);
     }
     if (active) {

@@ -22,8 +22,8 @@ onbody_kernel(OnBodyArgs A, Workspace w)
 // their Kepler orbits).  Then every component gets a group index g and registers its members in
 // ginfo[g * GINFO ..] (count, members; in no particular order: the integrating warp sorts them).  One block.
 __global__ void __launch_bounds__(1024)
-group_kernel(int N, int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr, unsigned int pair_cap,
-             int* __restrict__ glabel, int* __restrict__ ginfo)
+group_kernel(int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr, unsigned int pair_cap,
+             int* __restrict__ glabel, int* __restrict__ ginfo, int* __restrict__ ulist)
 {
     __shared__ int changed;
     int* gcount = glabel + NP;
@@ -34,11 +34,18 @@ group_kernel(int N, int NP, const int2* __restrict__ pairs, Counters* __restrict
         ctr->enc_groups = 0u; ctr->enc_bodies = 0u; ctr->enc_maxsize = 0u;
     }
     if (n == 0) return;
-    for (unsigned int p = threadIdx.x; p < n; p += blockDim.x) {
-        const int2 ij = pairs[p];
-        glabel[ij.x] = ij.x; glabel[ij.y] = ij.y; gcount[ij.x] = 0; gcount[ij.y] = 0;
+    // the bodies that occur in a pair, each once (gcount is preset to -1 like the labels): every later pass
+    // walks this short list instead of all N bodies
+    __shared__ int nuniq;
+    if (threadIdx.x == 0) nuniq = 0;
+    __syncthreads();
+    for (unsigned int p = threadIdx.x; p < 2u * n; p += blockDim.x) {
+        const int2 ij = pairs[p >> 1];
+        const int b = (p & 1u) ? ij.y : ij.x;
+        if (atomicCAS(&gcount[b], -1, 0) == -1) { glabel[b] = b; ulist[atomicAdd(&nuniq, 1)] = b; }
     }
     __syncthreads();
+    const int nu = nuniq;
     for (int iter = 0; iter < (1 << 20); ++iter) {
         if (threadIdx.x == 0) changed = 0;
         __syncthreads();
@@ -54,16 +61,17 @@ group_kernel(int N, int NP, const int2* __restrict__ pairs, Counters* __restrict
         if (!again) break;
     }
     // member counts; components too large for the leader's arrays are dissolved (and reported)
-    for (int b = threadIdx.x; b < N; b += blockDim.x) if (glabel[b] >= 0) atomicAdd(&gcount[glabel[b]], 1);
+    for (int q = threadIdx.x; q < nu; q += blockDim.x) atomicAdd(&gcount[glabel[ulist[q]]], 1);
     __syncthreads();
-    for (int b = threadIdx.x; b < N; b += blockDim.x) {
-        const int l = glabel[b];
-        if (l >= 0 && l != b && gcount[l] > enc::GMAX) { glabel[b] = -2; atomicOr(&ctr->enc_status, 2u); }
+    for (int q = threadIdx.x; q < nu; q += blockDim.x) {
+        const int b = ulist[q], l = glabel[b];
+        if (l != b && gcount[l] > enc::GMAX) { glabel[b] = -2; atomicOr(&ctr->enc_status, 2u); }
     }
     __syncthreads();
-    for (int b = threadIdx.x; b < N; b += blockDim.x) if (glabel[b] == b && gcount[b] > enc::GMAX) glabel[b] = -2;
+    for (int q = threadIdx.x; q < nu; q += blockDim.x) { const int b = ulist[q]; if (glabel[b] == b && gcount[b] > enc::GMAX) glabel[b] = -2; }
     __syncthreads();
-    for (int b = threadIdx.x; b < N; b += blockDim.x)
+    for (int q = threadIdx.x; q < nu; q += blockDim.x) {
+        const int b = ulist[q];
         if (glabel[b] == b) {                                               // leader of a valid group
             const unsigned int g = atomicAdd(&ctr->enc_groups, 1u);
             const int cnt = gcount[b];
@@ -71,9 +79,10 @@ group_kernel(int N, int NP, const int2* __restrict__ pairs, Counters* __restrict
             ginfo[g * enc::GINFO] = 0;
             gcount[b] = (int)g;
         }
+    }
     __syncthreads();
-    for (int b = threadIdx.x; b < N; b += blockDim.x) {
-        const int l = glabel[b];
+    for (int q = threadIdx.x; q < nu; q += blockDim.x) {
+        const int b = ulist[q], l = glabel[b];
         if (l >= 0) {
             int* info = ginfo + (size_t)gcount[l] * enc::GINFO;
             const int k = atomicAdd(info, 1);
@@ -118,9 +127,9 @@ cudaError_t launch_onbody(const Handle* h, const OnBodyArgs& a, int max_blocks)
 cudaError_t launch_groups(const Handle* h)
 {
     if (h->N == 0) return cudaSuccess;
-    cudaError_t e = cudaMemsetAsync(h->w.glabel, 0xff, (size_t)h->NP * sizeof(int), h->stream);
+    cudaError_t e = cudaMemsetAsync(h->w.glabel, 0xff, 2 * (size_t)h->NP * sizeof(int), h->stream);   // labels and counts: -1
     if (e != cudaSuccess) return e;
-    group_kernel<<<1, 1024, 0, h->stream>>>(h->N, h->NP, h->w.pairs, h->w.ctr, (unsigned int)h->pair_cap, h->w.glabel, h->w.ginfo);
+    group_kernel<<<1, 1024, 0, h->stream>>>(h->NP, h->w.pairs, h->w.ctr, (unsigned int)h->pair_cap, h->w.glabel, h->w.ginfo, h->w.gulist);
     return cudaGetLastError();
 }
 

@@ -70,6 +70,7 @@ struct Workspace {
     int* glabel;                // [2 NP] encounter mode: smallest body index of the body's encounter group (-1: none,
                                 //        -2: group too large, Kepler drift), then [NP] member count / group index per label
     int* ginfo;                 // [enc::GINFO x max groups] per group: member count, members
+    int* gulist;                // [min(2 pair_cap, NP)] the bodies that occur in the pair list, each once
     double4* pk64;    // [NP]   (x, y, z, G m)
     float4*  pk32;    // [NP]   pair-interleaved, see above
     double4* aux;     // [NP]   (m, r_crit, a, v_K): what the exact pair rule O3 needs
