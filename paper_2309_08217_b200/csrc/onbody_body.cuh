@@ -115,7 +115,9 @@ __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, c
             // same S(dt/2) and the flow of H_A,group over dt; then their m v' joins the sum, each body's in the
             // thread that owns the body (so the sum does not depend on which warp moved which group)
             const int ngroups = (int)__ldcg(&w.ctr->enc_groups);
-            for (int g = gtid >> 5; g < ngroups; g += gsz >> 5) enc::warp_group(A.enc, w, g, A.dt, s0, s1, s2);
+            // group g -> block g % gridDim.x, warp (g / gridDim.x) % 8: a few hundred groups spread over all SMs
+            for (int g = blockIdx.x + gridDim.x * (threadIdx.x >> 5); g < ngroups; g += gridDim.x * (FUSED_NT / 32))
+                enc::warp_group(A.enc, w, g, A.dt, s0, s1, s2);
             grid.sync();
             for (int i = gtid; i < N; i += gsz)
                 if (w.glabel[i] >= 0) {
