@@ -683,7 +683,12 @@ const char* genga_version(void) { return "genga_b200 0.1 (sm_100a)"; }
 
 int genga_set_tuning(genga_handle h, int key, int value)
 {
-    if (!h || key < 0 || key > 1) return GENGA_EINVAL;
+    if (!h || key < 0 || key > 3) return GENGA_EINVAL;
+    if (key >= 2) {                                    // grid of the all-pairs kernels in units of half a wave
+        if (value < 0 || value > 64) return GENGA_EINVAL;
+        h->tune[key] = value;
+        return GENGA_OK;
+    }
     const int n = key == 0 ? kick32_num_variants() : kick64_num_variants();
     if (value < 0 || value >= n) return GENGA_EINVAL;
     h->tune[key] = value;

@@ -1,5 +1,6 @@
 // kick_fp64.cu -- kernel wrappers, variants and launcher of the FP64 all-pairs kick (the kernel body
 // and its description are in kick64_body.cuh).
+#include <algorithm>
 #include "kick64_body.cuh"
 
 namespace genga {
@@ -66,8 +67,14 @@ void launch_kick64(const Handle* h)
     const Variant64& V = variant64(h->tune[1]);
     const int nib = (h->N + V.bi - 1) / V.bi;          // i-blocks that hold a live body
     const long long U = (long long)nib * h->nchunk;
-    long long G = kick64_grid(h);
+    // Grid: up to four waves of CTAs (the hardware hands out the later ones as SMs free up, which evens out the
+    // CTAs' unequal near-field load and keeps two CTAs resident per SM to the end), but at least 16 chunks per
+    // CTA; genga_set_tuning key 3 overrides it (grid in half waves).
+    const long long wave = kick64_grid(h);
+    long long G = std::min(4 * wave, std::max(wave, U / 16));
+    if (h->tune[3] > 0) G = wave * h->tune[3] / 2;
     if (G > U) G = U;
+    if (G < 1) G = 1;
     const int ci = (h->chunk == CHUNK_MIN) ? 0 : 1;
     V.fn[ci]<<<(int)G, V.nt, V.smem[ci], h->stream>>>(h->N, h->nchunk, nib, h->w, (unsigned int)h->cand_cap);
 }
