@@ -365,7 +365,7 @@ def run_cuda(args):
         "precisions": {"fp32": p32, "fp64": p64},
         "roofline": {"bound": "alu", "kernel": "kick32_kernel", "achieved": p32["kick_kernel_tflops"],
                      "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s", "frac": p32["kick_kernel_frac_of_peak"],
-                     "traffic": 3.742e6,      # dram bytes read + written per kick32 launch (profiles/r1e, ncu --set full)
+                     "traffic": 3.742e6,      # dram bytes read + written per kick32 launch (profiles/r1g, ncu --set full)
                      "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md section 6); "
                                     "MEASURED_PEAKS.json has no FP32/FP64 ALU figure",
                      "flop_per_pair": FLOP_FP32,
