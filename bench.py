@@ -453,8 +453,11 @@ def run_report(args):
     # NEXT-1: the hybrid step (encounter mode, reading R11) on the performance shape, 200 steps
     w5 = W.config(4)
     w5.nsteps = 200
-    cases.append(("4-hybrid", w5, {"weight_mode": 1, "encounter_mode": 1, "enc_nsub": 256, "enc_list_scale": 8.0,
-                                     "enc_list_vfactor": 1.25, "cand_capacity": 64 * w5.N}))
+    hyb = {"weight_mode": 1, "encounter_mode": 1, "enc_nsub": 256, "enc_list_scale": 8.0, "enc_list_vfactor": 1.25}
+    cases.append(("4-hybrid", w5, dict(hyb, cand_capacity=64 * w5.N)))
+    for c in (1, 2, 3):                                            # ... and on the paper-shaped configs, full length
+        wc = W.config(c)
+        cases.append((f"{c}-hybrid", wc, dict(hyb, cand_capacity=64 * wc.N, pair_capacity=40 * wc.N)))
     for cfg, w, kw in cases:
         nb = kw.get("n_big", -1)
         if not args.no_cpu_baseline:                               # the oracle beside it: one kick per config
@@ -480,7 +483,7 @@ def run_report(args):
             E1, L1 = g.energy_angmom()
             enc_last = int(len(g.encounter_pairs(cap=max(8 * w.N + 4096, kw.get("pair_capacity", 0)))))
             st = g.nearfield_stats()
-            enc_stats = g.encounter_stats() if kw.get("encounter_mode") else None
+            enc_stats = g.encounter_stats() if kw.get("encounter_mode") else None    # missed / status: since the warm-up
             g.close()
             evals = w.nsteps + 1
             line = {"report": "config", "config": cfg, "workload": w.name, "N": w.N, "dt_days": w.dt, "steps": w.nsteps,
