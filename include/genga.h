@@ -112,7 +112,7 @@ typedef struct {
                                  complement pair forces G m_j (1 - (K - r dK/dr)) / r^2, in FP64, by enc_nsub
                                  classical RK4 substeps, r_crit,ij held at the opening evaluation's values.
                                  Requires weight_mode = 1, n_big < 0 and the cooperative per-body kernel.    */
-    int    enc_nsub;          /* RK4 substeps per step for the bodies of a group; <= 0: default (256)        */
+    int    enc_nsub;          /* RK4 substeps per step for the bodies of a group (at least; see enc_eta); <= 0: default (256) */
     double enc_list_scale;    /* encounter mode: which pairs OUTSIDE their zone are listed (and grouped) as well, so that
                                  a pair that enters its zone DURING the step is already in a group: those with
                                  r_ij < enc_list_scale * r_crit,ij  and  r_ij - r_crit,ij < enc_list_vfactor * dt * |v_i - v_j|
@@ -122,6 +122,11 @@ typedef struct {
                                  un-grouped all the same are counted (genga_encounter_stats).                       */
     double enc_list_vfactor;  /* see enc_list_scale.  0: default (1.25); < 0: no velocity test, every pair inside
                                  enc_list_scale * r_crit,ij is listed.                                               */
+    double enc_eta;           /* encounter mode: <= 0 (default): fixed substeps dt / enc_nsub, the oracle's scheme.  > 0:
+                                 adaptive substeps min(dt / enc_nsub, enc_eta * tau), tau = the shortest
+                                 r_ij / (|v_i - v_j| + sqrt(2 G (m_i + m_j) / r_ij)) over the group's pairs that are inside
+                                 their zone, never below dt / (256 enc_nsub) (status bit 8 of genga_encounter_stats if
+                                 that floor was hit).  Costs about 15 % of the group integration; 0.02 is a sensible value. */
 } genga_params;
 
 /* Fill *p with the defaults: G = k^2 (k = 0.01720209895), M_star = 1, n1 = 3, n2 = 0,
@@ -195,7 +200,8 @@ int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed
  * there had not moved them as one group (they entered un-grouped: raise enc_list_scale or shorten dt), and a
  * status mask; count and mask are cleared by this call.  Mask: 1 the pair list overflowed when the groups were
  * formed (raise pair_capacity), 2 a group had more than 8 bodies (its bodies drifted on their Kepler orbits
- * instead), 4 missed_pairs > 0.  HOST outputs, NULL = skip.  Synchronises.  GENGA_EINVAL unless
+ * instead), 4 missed_pairs > 0, 8 the adaptive substep hit its floor (an approach too deep to resolve: raise enc_nsub).
+ * HOST outputs, NULL = skip.  Synchronises.  GENGA_EINVAL unless
  * params.encounter_mode = 1.                                                                          */
 int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest, int* missed_pairs, int* status);
 

@@ -44,11 +44,15 @@ __device__ __forceinline__ double rcp_seed(double a) { double r; asm("rcp.approx
 // c01[l] = 0.1 r_crit,kl and i09[l] = 1 / (0.9 r_crit,kl) (0: no zone, the lane itself, an idle lane) for the
 // members l.  NN > 0: the group size at compile time (straight-line code: the pair terms and the Kepler term
 // overlap in the pipeline); NN = 0: n at run time.  Branch-free: a term that does not apply gets weight 0.
-template <int NN>
+// CRIT: also return in tau the shortest time scale q / (|v_rel| + v_escape(q)) over the pairs of this member
+// that are inside their zone (1e300 if none), from which the adaptive substep is taken (vx, vy, vz: own velocity).
+template <int NN, bool CRIT = false>
 __device__ __forceinline__ void member_accel(const EncParams& P, int n, double gm_self,
                                              const double (&c01)[GMAX], const double (&i09)[GMAX],
-                                             double px, double py, double pz, double& a0, double& a1, double& a2)
+                                             double px, double py, double pz, double& a0, double& a1, double& a2,
+                                             double vx = 0.0, double vy = 0.0, double vz = 0.0, double* tau = nullptr)
 {
+    double tmin = 1.0e300;
     {
         const double mu = P.G * P.M_star;
         const double r2 = fma(pz, pz, fma(py, py, px * px));
@@ -76,20 +80,49 @@ __device__ __forceinline__ void member_accel(const EncParams& P, int n, double g
         const double Wc = on ? 1.0 - (K - q * Kp) : 0.0;
         const double s  = ogm * Wc * fma(g * e, fma(1.875, e, 1.5), g);      // G m_l Wc / |d|^3
         a0 = fma(s, d0, a0); a1 = fma(s, d1, a1); a2 = fma(s, d2, a2);
+        if (CRIT) {
+            const double u0 = shfl_d(vx, l) - vx, u1 = shfl_d(vy, l) - vy, u2 = shfl_d(vz, l) - vz;
+            const double vrel = sqrt(fma(u2, u2, fma(u1, u1, u0 * u0)));
+            const double vesc = sqrt(2.0 * (gm_self + ogm) * y0);           // y0 ~ 1/|d| (seed accuracy is plenty here)
+            if (on && y < 1.0) tmin = fmin(tmin, q / (vrel + vesc));
+        }
     }
+    if (CRIT) *tau = tmin;
 }
 
-// nsub RK4 substeps of the flow of H_A,group for this lane's member (state in registers).
-template <int NN>
+// The flow of H_A,group over dt for this lane's member (state in registers): classical RK4 substeps of dt / nsub, or
+// shorter where a pair is deep inside its zone (P.eta > 0: h = min(dt / nsub, eta * tau), tau the shortest
+// q / (|v_rel| + v_escape) over the in-zone pairs of the whole group, never below dt / (256 nsub): status bit 8).
+template <int NN, bool ADAPT>
 __device__ __forceinline__ void integrate(const EncParams& P, int n, double gm, const double (&c01)[GMAX], const double (&i09)[GMAX],
-                                          double dt, double& x0, double& x1, double& x2, double& v0, double& v1, double& v2)
+                                          double dt, double& x0, double& x1, double& x2, double& v0, double& v1, double& v2,
+                                          unsigned int* status)
 {
-    const double h = dt / P.nsub, hh = 0.5 * h, h6 = h / 6.0;
-    for (int s = 0; s < P.nsub; ++s) {
+    const double T = fabs(dt), sgn = (dt < 0.0) ? -1.0 : 1.0;
+    const double hmax = T / P.nsub, hmin = hmax * (1.0 / 256.0);
+    constexpr bool adaptive = ADAPT;
+    double tnow = 0.0;
+    bool floored = false;
+    for (int s = 0; ; ++s) {
+        if (adaptive ? !(T - tnow > 1.0e-9 * hmax) : (s == P.nsub)) break;
         double k0, k1, k2;                                 // stage acceleration
         double sx0, sx1, sx2, sv0, sv1, sv2;               // running sums k1 + 2 k2 + 2 k3 (+ k4)
         double t0, t1, t2, u0, u1, u2;                     // stage position, stage velocity
-        member_accel<NN>(P, n, gm, c01, i09, x0, x1, x2, k0, k1, k2);
+        double habs = hmax;
+        if (adaptive) {
+            double tau;
+            member_accel<NN, true>(P, n, gm, c01, i09, x0, x1, x2, k0, k1, k2, v0, v1, v2, &tau);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) tau = fmin(tau, __shfl_xor_sync(FULL, tau, o));
+            const double want = P.eta * tau;
+            if (want < hmin) floored = true;
+            habs = fmin(hmax, fmax(want, hmin));
+            habs = fmin(habs, T - tnow);
+            tnow += habs;
+        } else {
+            member_accel<NN>(P, n, gm, c01, i09, x0, x1, x2, k0, k1, k2);
+        }
+        const double h = sgn * habs, hh = 0.5 * h, h6 = h / 6.0;
         sx0 = v0; sx1 = v1; sx2 = v2; sv0 = k0; sv1 = k1; sv2 = k2;
         t0 = fma(hh, v0, x0); t1 = fma(hh, v1, x1); t2 = fma(hh, v2, x2);
         u0 = fma(hh, k0, v0); u1 = fma(hh, k1, v1); u2 = fma(hh, k2, v2);
@@ -105,6 +138,7 @@ __device__ __forceinline__ void integrate(const EncParams& P, int n, double gm, 
         x0 = fma(h6, sx0 + u0, x0); x1 = fma(h6, sx1 + u1, x1); x2 = fma(h6, sx2 + u2, x2);
         v0 = fma(h6, sv0 + k0, v0); v1 = fma(h6, sv1 + k1, v1); v2 = fma(h6, sv2 + k2, v2);
     }
+    if (floored && (threadIdx.x & 31) == 0) atomicOr(status, 8u);
 }
 
 // One warp advances group g through S(dt/2) (the shift s, already scaled) and the flow of H_A,group over dt
@@ -142,10 +176,15 @@ __device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, int
     }
     const double gm = P.G * m;
     if (dt != 0.0) {
-        if (n == 2)      integrate<2>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2);
-        else if (n == 3) integrate<3>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2);
-        else if (n == 4) integrate<4>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2);
-        else             integrate<0>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2);
+        unsigned int* st = &w.ctr->enc_status;
+        if (P.eta > 0.0) {                                  // adaptive substeps (opt-in): one generic instance
+            integrate<0, true>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
+        } else {
+            if (n == 2)      integrate<2, false>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
+            else if (n == 3) integrate<3, false>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
+            else if (n == 4) integrate<4, false>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
+            else             integrate<0, false>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
+        }
     }
     if (active) {
         w.x[3 * b] = x0; w.x[3 * b + 1] = x1; w.x[3 * b + 2] = x2;

@@ -43,7 +43,7 @@ struct Counters {
     unsigned int ticket;         // block-completion ticket of the momentum reduction (0 between launches)
     unsigned int extent_bits;    // float bits of max(|x|, |y|) over the bodies (Hilbert sort extent)
     // encounter mode (encounter.cuh; NEXT-1)
-    unsigned int enc_status;     // sticky until read: 1 pair list overflowed, 2 a group had more than enc::GMAX bodies
+    unsigned int enc_status;     // sticky until read: 1 pair list overflowed, 2 a group had more than enc::GMAX bodies, 8 substep floor hit
     unsigned int enc_groups;     // encounter groups integrated by the last drift
     unsigned int enc_bodies;     // bodies in those groups
     unsigned int enc_maxsize;    // largest group of the last drift
@@ -142,6 +142,7 @@ struct EncArgs {                  // encounter mode (encounter.cuh; NEXT-1, read
     int pair_rule;
     unsigned int pair_cap;
     double G, M_star, n1, n2dt;
+    double eta;                    // > 0: adaptive substeps (encounter.cuh: integrate)
 };
 struct OnBodyArgs {               // the fused per-body kernel of the step (fused_step.cu)
     PrepArgs prep;

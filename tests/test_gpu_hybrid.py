@@ -200,3 +200,43 @@ def test_oversized_groups_are_reported_and_parameters_checked():
     for bad in (dict(weight_mode=0), dict(n_big=3), dict(enc_list_scale=0.5), dict(enc_list_scale=9.0), dict(no_fused_step=True)):
         with pytest.raises(Exception):
             hybrid(w, **bad).close()
+
+
+def deep_flyby_system():
+    """Two 10 M_earth planets that pass each other within 1e-4 AU (1e-3 r_crit) in the middle of a 2-day step: the
+    approach lasts a few thousandths of a day, below dt / 256."""
+    m = np.array([3e-5, 3e-5, 1e-6])
+    xa = np.array([1.0, 0.0, 0.0])
+    va = np.array([0.0, np.sqrt(G * (1 + m[0])), 0.0])
+    x = np.stack([xa, xa + np.array([0.004, 3.0e-4, 0.0]), [0.0, 1.9, 0.0]])
+    v = np.stack([va, va + np.array([-0.004, 0.0, 0.0]), [-np.sqrt(G / 1.9), 0.0, 0.0]])
+    return workload("flyby", m, x, v, 2.0, 0.0, B.PAIR_MUTUAL_HILL)
+
+
+def test_adaptive_substeps_resolve_a_deep_flyby():
+    # params.enc_eta > 0 (opt-in): the substep follows r / (v_rel + v_escape) of the in-zone pairs.  Reference:
+    # the oracle's fixed-step scheme converged (100 000 substeps, checked against 50 000).
+    w = deep_flyby_system()
+    p = oparams(w)
+    vd = oracle.to_democratic(w.m, w.v, w.M_star)
+    xo, vo = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=100000)
+    xh, vh = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=50000)
+    assert state_err(xh, vh, xo, vo) <= 1e-8
+    x256, v256 = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=256)
+    err = {}
+    for eta in (-1.0, 0.05):
+        g = hybrid(w, enc_nsub=256, enc_eta=eta)
+        g.step(w.dt, B.FP64)
+        x, v = (t.cpu().numpy() for t in g.get_state())
+        st = g.encounter_stats()
+        g.close()
+        assert st == (1, 2, 2, 0, 0)
+        err[eta] = state_err(x, v, xo, vo)
+        if eta < 0:                                            # the fixed scheme is the oracle's, resolved or not
+            assert state_err(x, v, x256, v256) <= 1e-8
+    assert err[-1.0] > 1e-3, err                                # 256 fixed substeps step over the approach
+    assert err[0.05] <= 1e-7, err                               # 5e-9 measured
+    g = hybrid(w, enc_nsub=64, enc_eta=0.01)                    # the floor dt / (256 enc_nsub) is reported when hit
+    g.step(w.dt, B.FP64)
+    assert g.encounter_stats()[4] == 8
+    g.close()
