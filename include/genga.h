@@ -214,7 +214,9 @@ int genga_kernel_time(genga_handle h, int which, double* ms_total, long long* la
 
 /* Kernel configuration ("tuning", cf. GENGA's self-tuning): key 0 selects the
  * launch/tiling variant of the FP32 all-pairs kernel, key 1 of the FP64 one; value in
- * [0, genga_num_variants(key)); 0 is the default.  Results are identical up to summation order. */
+ * [0, genga_num_variants(key)); 0 is the default.  Keys 2 (FP32) and 3 (FP64) set the grid of that kernel in
+ * half waves of co-resident CTAs, 1..64; 0 (default): up to four waves with at least 16 j-chunks per CTA.
+ * Results are identical up to summation order.  GENGA_EINVAL for any other key or value.           */
 int genga_set_tuning(genga_handle h, int key, int value);
 /* Time every variant of the given precision's all-pairs kernel on the current state (force evaluation
  * = prep + all-pairs + near field, 1 warm-up + 3 timed runs each) and keep the fastest.  HOST

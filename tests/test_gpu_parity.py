@@ -318,6 +318,27 @@ def test_every_kernel_variant_matches_the_oracle():
         assert pair_set(pairs) == pair_set(po), (key, v, chunk)
 
 
+def test_any_grid_of_the_all_pairs_kernels_gives_the_same_forces():
+    # genga_set_tuning keys 2 / 3: the grid of kick32 / kick64 in half waves (default: up to four waves).  The
+    # (i-block, chunk) units are split evenly over whatever grid is launched, so the gates hold for every value.
+    w = W.config(4, 9000)
+    ao, po, _ = oracle_accel(w)
+    for prec, key, tol in ((B.FP32, 2, 1e-4), (B.FP64, 3, 1e-12)):
+        for half_waves in (0, 1, 3, 7, 64):
+            g = B.from_workload(w)
+            g.set_tuning(key, half_waves)
+            g.accel(prec)
+            a = g.get_accel().cpu().numpy()
+            pairs = g.encounter_pairs()
+            g.close()
+            assert rel_err(a, ao).max() <= tol, (prec, half_waves, rel_err(a, ao).max())
+            assert pair_set(pairs) == pair_set(po), (prec, half_waves)
+    g = B.from_workload(w)
+    with pytest.raises(Exception):
+        g.set_tuning(2, 65)
+    g.close()
+
+
 def test_autotune_picks_a_variant_and_keeps_the_state():
     w = W.config(0, 3000)
     g = B.from_workload(w)
