@@ -3,6 +3,7 @@ symbol include/genga.h declares; host-side argument checking; no compute call is
 import ctypes
 import os
 import re
+import subprocess
 
 import pytest
 
@@ -87,3 +88,20 @@ def test_product_path_does_not_import_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", src, flags=re.M), f
                 assert "genga_oracle" not in src, f
+
+
+def test_params_struct_layout_matches_the_c_compiler(tmp_path):
+    # sizeof and every offsetof of genga_params as gcc lays the header out == the ctypes mirror (types and padding,
+    # not just names); the header must also compile as plain C
+    fields = [f[0] for f in binding.GengaParams._fields_]
+    src = tmp_path / "layout.c"
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "genga.h"\nint main(void) {\n'
+                   '  printf("%zu\\n", sizeof(genga_params));\n'
+                   + "".join(f'  printf("%zu\\n", offsetof(genga_params, {f}));\n' for f in fields)
+                   + "  return 0;\n}\n")
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)],
+                   check=True)
+    out = [int(v) for v in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
+    assert out[0] == ctypes.sizeof(binding.GengaParams)
+    assert out[1:] == [getattr(binding.GengaParams, f).offset for f in fields]
