@@ -93,6 +93,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_run.restype = ctypes.c_int
         L.oracle_run.argtypes = [ctypes.c_int, _dp, _dp, _dp, _pp, ctypes.c_double, ctypes.c_int]
         L.oracle_energy_angmom.argtypes = [ctypes.c_int, _dp, _dp, _dp, _pp, _dp, _dp]
+        L.oracle_merge.restype = ctypes.c_int
+        L.oracle_merge.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _ip]
         L.oracle_num_threads.restype = ctypes.c_int
         _lib = L
     return _lib
@@ -276,3 +278,12 @@ def energy_angmom(m, x, v, p: Params):
     L = np.zeros(3)
     lib().oracle_energy_angmom(len(m), _p(m), _p(x), _p(v), ctypes.byref(c), ctypes.byref(E), _p(L))
     return float(E.value), L
+
+
+def merge(m, x, v, R):
+    """NEXT-4, reading R13: step-end perfect mergers.  Returns (m', x', v', R', newidx):
+    the closed-up arrays and, per old body, the new index of the body it is now part of."""
+    m = _a(m).copy(); x = _a(x).copy(); v = _a(v).copy(); R = _a(R).copy()
+    newidx = np.zeros(len(m), dtype=np.int32)
+    n = lib().oracle_merge(len(m), _p(m), _p(x), _p(v), _p(R), newidx.ctypes.data_as(_ip))
+    return m[:n].copy(), x[:n].copy(), v[:n].copy(), R[:n].copy(), newidx

@@ -576,3 +576,63 @@ void oracle_energy_angmom(int N, const double* m, const double* x, const double*
     *E = nsum_value(&e);
     for (int k = 0; k < 3; ++k) L[k] = nsum_value(&Ls[k]);
 }
+
+/* ---- NEXT-4: perfect mergers at a step end (reading R13) ------------------------
+ * Plain definition: brute force over all pairs for the collision graph, components by repeated
+ * relabelling to the smallest index until nothing changes, member sums in ascending index.        */
+int oracle_merge(int N, double* m, double* x, double* v, double* R, int* newidx)
+{
+    if (N <= 0) return 0;
+    int* lab = (int*)malloc(sizeof(int) * (size_t)N);
+    for (int i = 0; i < N; ++i) lab[i] = i;
+    int changed = 1;
+    while (changed) {
+        changed = 0;
+        for (int i = 0; i < N; ++i)
+            for (int j = i + 1; j < N; ++j) {
+                if (lab[i] == lab[j]) continue;
+                double dx = x[3 * j + 0] - x[3 * i + 0];
+                double dy = x[3 * j + 1] - x[3 * i + 1];
+                double dz = x[3 * j + 2] - x[3 * i + 2];
+                double r  = sqrt(dx * dx + dy * dy + dz * dz);
+                if (r < R[i] + R[j]) {
+                    int lo = lab[i] < lab[j] ? lab[i] : lab[j];
+                    lab[i] = lo; lab[j] = lo;
+                    changed = 1;
+                }
+            }
+    }
+    /* merge every component into its smallest index (lab[k] == k there) */
+    for (int r = 0; r < N; ++r) {
+        if (lab[r] != r) continue;
+        int members = 0;
+        nsum M = {0, 0}, V3 = {0, 0}, X[3] = {{0, 0}, {0, 0}, {0, 0}}, P[3] = {{0, 0}, {0, 0}, {0, 0}};
+        for (int k = r; k < N; ++k) {
+            if (lab[k] != r) continue;
+            ++members;
+            nsum_add(&M, m[k]);
+            nsum_add(&V3, R[k] * R[k] * R[k]);
+            for (int d = 0; d < 3; ++d) { nsum_add(&X[d], m[k] * x[3 * k + d]); nsum_add(&P[d], m[k] * v[3 * k + d]); }
+        }
+        if (members < 2) continue;
+        double mt = nsum_value(&M);
+        if (mt > 0.0)
+            for (int d = 0; d < 3; ++d) { x[3 * r + d] = nsum_value(&X[d]) / mt; v[3 * r + d] = nsum_value(&P[d]) / mt; }
+        m[r] = mt;
+        R[r] = cbrt(nsum_value(&V3));
+    }
+    /* close up the arrays in order */
+    int n = 0;
+    int* where = (int*)malloc(sizeof(int) * (size_t)N);
+    for (int i = 0; i < N; ++i) {
+        if (lab[i] != i) continue;
+        where[i] = n;
+        m[n] = m[i]; R[n] = R[i];
+        for (int d = 0; d < 3; ++d) { x[3 * n + d] = x[3 * i + d]; v[3 * n + d] = v[3 * i + d]; }
+        ++n;
+    }
+    if (newidx) for (int i = 0; i < N; ++i) newidx[i] = where[lab[i]];
+    free(where);
+    free(lab);
+    return n;
+}

@@ -128,6 +128,15 @@ int oracle_step_hybrid(int N, const double* m, double* x, double* v, const oracl
 void oracle_energy_angmom(int N, const double* m, const double* x, const double* v,
                           const oracle_params* p, double* E, double L[3]);
 
+/* NEXT-4 ("collisions ... perfect mergers"; reading R13): step-end collision pass.
+ * Collision graph: i ~ j iff r_ij < R_i + R_j (strict; R = physical radii) at the given positions.  Every
+ * connected component of more than one body becomes ONE body at the component's smallest index:
+ * m = sum m_k, x = sum m_k x_k / m, v = sum m_k v_k / m (v: the stored democratic velocities, so
+ * sum m v and sum m x are unchanged), R = cbrt(sum R_k^3); a component of total mass 0 keeps the x, v of
+ * its smallest index.  The other members are removed and the arrays closed up in order.  Sums run
+ * over the members in ascending index.  newidx[N] (may be NULL): the new index of each old body
+ * (of its survivor, for a removed body).  Returns the new body count.                                */
+int oracle_merge(int N, double* m, double* x, double* v, double* R, int* newidx);
 int oracle_num_threads(void);
 
 #ifdef __cplusplus
