@@ -191,6 +191,28 @@ int genga_get_state_host(genga_handle h, double* x, double* v, int heliocentric_
 int genga_get_accel(genga_handle h, double* a);          /* DEVICE [N][3]: a_i of the last force evaluation */
 int genga_get_rcrit(genga_handle h, double* rcrit);      /* DEVICE [N]: r_crit,i of the last force evaluation */
 
+/* ---- perfect mergers at a step end (NEXT-4; "collisions ... perfect mergers"; R13) ----
+ * genga_set_radii: physical radii R_i, DEVICE double[N] borrowed for the call (NULL: all 0 = no body ever
+ * collides, the state after genga_create).  genga_get_radii: DEVICE double[N] output.  Asynchronous.
+ *
+ * genga_merge: bodies i, j collide iff r_ij < R_i + R_j (strict, FP64) at the current positions.  Every
+ * connected component of the collision graph becomes ONE body at the component's smallest index:
+ * m = sum m_k, x = sum m_k x_k / m, v = sum m_k v_k / m (stored velocities: total momentum and the centre of
+ * mass are kept), R = cbrt(sum R_k^3); a component of total mass 0 keeps its first member's x, v.  The other
+ * members are removed and m, x, v, R closed up IN ORDER: afterwards the handle holds N' = N - *n_merged
+ * bodies (genga_num_bodies) and every accessor uses N'.  The workspace is not re-carved.
+ *   Candidates are the pairs of the encounter list of the last force evaluation, so R_i + R_j <= r_crit,ij is
+ * required (status bit 2 is raised if some 2 R_i > r_crit,i); if the positions have changed since that
+ * evaluation (genga_drift, genga_sunkick, genga_set_state) one is run first, in `precision`; when bodies were
+ * merged, one is run afterwards, so that the pair list, a_i and r_crit,i describe the new body set.
+ *   newidx: DEVICE int[N] (N before the call) or NULL: new index of each old body (of the body that absorbed
+ * it).  n_merged, status: HOST outputs (NULL = skip); status bit 1: the pair list had overflowed (pairs may
+ * have been missed).  Synchronises the stream.  GENGA_EINVAL in TP2 mode (small-small pairs are not listed). */
+int genga_set_radii(genga_handle h, const double* R);
+int genga_get_radii(genga_handle h, double* R);
+int genga_merge(genga_handle h, int precision, int* newidx, int* n_merged, int* status);
+int genga_num_bodies(genga_handle h);                    /* current N (shrinks with mergers); < 0 on a NULL handle */
+
 /* Diagnostics of the last force evaluation: number of (body, j-chunk) near-field candidates and
  * whether the candidate list overflowed (exact slow path taken).  HOST outputs.  Synchronises.  */
 int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed);

@@ -26,6 +26,7 @@ SYMBOLS = [
     "genga_set_state", "genga_set_state_host", "genga_resort", "genga_kick", "genga_accel", "genga_drift",
     "genga_sunkick", "genga_step", "genga_run", "genga_leapfrog", "genga_encounter_pairs", "genga_energy_angmom",
     "genga_get_state", "genga_get_state_host", "genga_get_accel", "genga_get_rcrit",
+    "genga_set_radii", "genga_get_radii", "genga_merge", "genga_num_bodies",
     "genga_nearfield_stats", "genga_encounter_stats", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
     "genga_synchronize", "genga_strerror", "genga_last_cuda_error", "genga_version",
     "genga_peak_probe", "genga_set_tuning", "genga_autotune", "genga_num_variants", "genga_variant_name",
@@ -86,6 +87,10 @@ def load() -> ctypes.CDLL:
     L.genga_get_state_host.argtypes = [vp, vp, vp, ctypes.c_int]
     L.genga_get_accel.argtypes = [vp, vp]
     L.genga_get_rcrit.argtypes = [vp, vp]
+    L.genga_set_radii.argtypes = [vp, vp]
+    L.genga_get_radii.argtypes = [vp, vp]
+    L.genga_merge.argtypes = [vp, ctypes.c_int, vp, ip, ip]
+    L.genga_num_bodies.argtypes = [vp]
     L.genga_nearfield_stats.argtypes = [vp, llp, ip]
     L.genga_encounter_stats.argtypes = [vp, ip, ip, ip, ip, ip]
     L.genga_set_profiling.argtypes = [vp, ctypes.c_int]
@@ -244,6 +249,26 @@ class Genga:
         r = torch.empty((self.N,), dtype=torch.float64, device=self.device)
         _check(self._L.genga_get_rcrit(self._h, _dptr(r)), "genga_get_rcrit")
         return r
+
+    def set_radii(self, R=None):
+        """Physical radii (device float64 [N]); None: all 0, no body ever collides."""
+        _check(self._L.genga_set_radii(self._h, _dptr(R)), "genga_set_radii")
+
+    def get_radii(self):
+        torch = self._torch
+        R = torch.empty((self.N,), dtype=torch.float64, device=self.device)
+        _check(self._L.genga_get_radii(self._h, _dptr(R)), "genga_get_radii")
+        return R
+
+    def merge(self, precision=FP64):
+        """Step-end perfect mergers (genga_merge, reading R13).  Returns (n_merged, status, newidx): newidx is a
+        device int32 tensor over the bodies BEFORE the call.  self.N follows the handle."""
+        torch = self._torch
+        newidx = torch.empty((self.N,), dtype=torch.int32, device=self.device)
+        n, s = ctypes.c_int(0), ctypes.c_int(0)
+        _check(self._L.genga_merge(self._h, int(precision), _dptr(newidx), ctypes.byref(n), ctypes.byref(s)), "genga_merge")
+        self.N = int(self._L.genga_num_bodies(self._h))
+        return int(n.value), int(s.value), newidx
 
     # ---- the path ------------------------------------------------------------------------------
     def resort(self):

@@ -52,6 +52,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_gl = take(NP * 8);          // labels [NP], member counts [NP]
     const size_t o_gi = take(std::min((size_t)pair_cap, NP / 2) * 9 * 4);      // encounter groups: count + 8 members each
     const size_t o_gu = take(std::min(2 * (size_t)pair_cap, NP) * 4);
+    const size_t o_rad = take(NP * 8);
     if (w && base) {
         char* b = static_cast<char*>(base);
         w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
@@ -65,6 +66,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
         w->bigslot = (int*)(b + o_bs);
         w->bkeys = (unsigned long long*)(b + o_bk); w->sortbuf = (unsigned int*)(b + o_sb);
         w->glabel = (int*)(b + o_gl); w->ginfo = (int*)(b + o_gi); w->gulist = (int*)(b + o_gu);
+        w->radius = (double*)(b + o_rad);
     }
     return off;
 }
@@ -152,6 +154,7 @@ static int launch_pairs(Handle* h, int precision)
     LAUNCHED(h, "kick_kernel");
     { ProfScope ps(h, 1); launch_nearfield(h); }
     LAUNCHED(h, "nearfield_kernel");
+    h->pairs_current = true;
     return GENGA_OK;
 }
 
@@ -261,6 +264,7 @@ static int step_mega(Handle* h, int precision, bool do_vel, double tau_v, bool d
     const cudaError_t e = launch_step_mega(h, a, precision, h->mega_blocks[precision == GENGA_FP32 ? 1 : 0]);
     ++h->launches;
     if (e != cudaSuccess) return cuda_fail(e, "step_kernel (cooperative launch)");
+    h->pairs_current = true;
     h->mom_a_valid = !do_drift;
     return GENGA_OK;
 }
@@ -434,7 +438,7 @@ static int set_state_impl(genga_handle h, const double* m, const double* x, cons
     const size_t n = (size_t)h->N;
     if (n == 0) return GENGA_OK;
     if (m) CU(cudaMemcpyAsync(h->w.m, m, n * 8, kind, h->stream));
-    if (x) { CU(cudaMemcpyAsync(h->w.x, x, n * 24, kind, h->stream)); h->enc_labels_valid = false; }
+    if (x) { CU(cudaMemcpyAsync(h->w.x, x, n * 24, kind, h->stream)); h->enc_labels_valid = false; h->pairs_current = false; }
     if (v) { CU(cudaMemcpyAsync(h->w.v, v, n * 24, kind, h->stream)); h->mom_a_valid = false; }
     if (m) h->mom_a_valid = false;
     if (m) { launch_hcbrt(h); LAUNCHED(h, "hcbrt_kernel"); }
@@ -450,6 +454,59 @@ int genga_set_state(genga_handle h, const double* m, const double* x, const doub
 int genga_set_state_host(genga_handle h, const double* m, const double* x, const double* v)
 {
     return set_state_impl(h, m, x, v, cudaMemcpyHostToDevice);
+}
+
+int genga_set_radii(genga_handle h, const double* R)
+{
+    if (!h) return GENGA_EINVAL;
+    if (h->N == 0) return GENGA_OK;
+    if (R) CU(cudaMemcpyAsync(h->w.radius, R, (size_t)h->N * 8, cudaMemcpyDeviceToDevice, h->stream));
+    else   CU(cudaMemsetAsync(h->w.radius, 0, (size_t)h->N * 8, h->stream));
+    return GENGA_OK;
+}
+
+int genga_get_radii(genga_handle h, double* R)
+{
+    if (!h || !R) return GENGA_EINVAL;
+    if (h->N) CU(cudaMemcpyAsync(R, h->w.radius, (size_t)h->N * 8, cudaMemcpyDeviceToDevice, h->stream));
+    return GENGA_OK;
+}
+
+int genga_num_bodies(genga_handle h)
+{
+    return h ? h->N : GENGA_EINVAL;
+}
+
+int genga_merge(genga_handle h, int precision, int* newidx, int* n_merged, int* status)
+{
+    if (!h || (precision != GENGA_FP64 && precision != GENGA_FP32)) return GENGA_EINVAL;
+    if (h->p.n_big >= 0 && h->p.n_big < h->N) return GENGA_EINVAL;      // TP2 mode lists no small-small pairs
+    if (n_merged) *n_merged = 0;
+    if (status) *status = 0;
+    if (h->N == 0) return GENGA_OK;
+    int rc = flush_pending(h);
+    if (rc != GENGA_OK) return rc;
+    if (!h->pairs_current && (rc = force_eval(h, precision)) != GENGA_OK) return rc;
+    launch_merge(h, newidx); h->launches += 2;
+    { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_, "merge kernels"); }
+    h->enc_labels_valid = false;                                      // the label arrays served as scratch
+    unsigned int out[2];
+    CU(cudaMemcpyAsync(out, &h->w.ctr->merge_n, sizeof(out), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    if (status) *status = (int)out[1];
+    const int n_new = (int)out[0];
+    if (n_new < 0 || n_new > h->N) return GENGA_ECUDA;
+    if (n_merged) *n_merged = h->N - n_new;
+    if (n_new == h->N) return GENGA_OK;
+    // fewer bodies: the arrays keep their places in the workspace, everything derived from N is redone
+    h->N = n_new; h->NP = padded(n_new);
+    h->nchunk = (n_new + h->chunk - 1) / h->chunk;
+    h->grid_cache[0][0] = h->grid_cache[1][0] = 0;
+    h->evals_since_sort = -1;
+    h->mom_a_valid = false;
+    launch_pad(h); LAUNCHED(h, "pad_kernel");
+    launch_hcbrt(h); LAUNCHED(h, "hcbrt_kernel");
+    return force_eval(h, precision);                                  // pair list, a, r_crit of the new body set
 }
 
 int genga_resort(genga_handle h)
@@ -478,6 +535,7 @@ int genga_drift(genga_handle h, double dt)
     { const int rcf = flush_pending(h); if (rcf != GENGA_OK) return rcf; }
     { ProfScope ps(h, 3); launch_drift(h, dt); }
     LAUNCHED(h, "drift_kernel");
+    h->pairs_current = false;
     h->mom_a_valid = false;
     h->enc_labels_valid = false;                     // a plain Kepler drift: no groups led to these positions
     return GENGA_OK;
@@ -490,6 +548,7 @@ int genga_sunkick(genga_handle h, double tau)
     if (h->N == 0) return GENGA_OK;
     launch_momentum(h); LAUNCHED(h, "momentum_kernel");
     launch_sunkick(h, tau); LAUNCHED(h, "sunkick_kernel");
+    h->pairs_current = false;
     return GENGA_OK;
 }
 

@@ -48,6 +48,9 @@ struct Counters {
     unsigned int enc_bodies;     // bodies in those groups
     unsigned int enc_maxsize;    // largest group of the last drift
     unsigned int enc_missed;     // sticky until read: pairs found inside their zone after a drift that had not grouped them
+    // mergers (merge.cu; NEXT-4): written by the last genga_merge
+    unsigned int merge_n;        // body count after the pass
+    unsigned int merge_status;   // 1 pair list had overflowed, 2 a radius exceeds half its critical radius
 };
 
 struct Workspace {
@@ -83,6 +86,7 @@ struct Workspace {
     double*  red;     // [RED_DOUBLES] reduction scratch / results
     double*  vtmp;    // [NP][3] staging for heliocentric-velocity output
     double*  mom;     // momentum slots and per-block partials of the fused step (momentum.cuh)
+    double*  radius;  // [NP] physical radii R_i (genga_set_radii; 0 = the body never collides)
     Counters* ctr;
 };
 
@@ -108,6 +112,7 @@ struct Handle {
     bool pend_vel;               // a closing velocity update v += pend_tau a is still owed (api.cu: sequence)
     double pend_tau;
     bool mom_a_valid;            // mom[SLOT_A] holds sum m v of the stored velocities
+    bool pairs_current;          // the encounter list was made from the current positions (genga_merge relies on it)
     int grid_cache[2][2];        // per kernel (FP32, FP64): variant + 1 it was computed for, grid size
     int tune[4];                 // genga_set_tuning: [0] kick32 variant, [1] kick64 variant
     int resort_every;            // force evaluations between two sorts
@@ -173,6 +178,7 @@ void launch_shift_drift_mom(const Handle* h, double tau_pre, double dt);   // S(
 void launch_shift_v(const Handle* h, double scale);          // v_i += scale * red[0..2]   (O1)
 void launch_sunkick(const Handle* h, double tau);            // x_i += tau * red[0..2] / M_star
 void launch_drift(const Handle* h, double dt);
+void launch_merge(const Handle* h, int* newidx_dev);            // step-end perfect mergers (merge.cu, reading R13)
 void launch_energy(const Handle* h);                         // red[0] = E, red[1..3] = L
 void launch_copy_v_helio(const Handle* h, const double* mom, double* out);   // out = v + mom[0..2]/M_star
 int  run_peak_probe(int which, int iters, cudaStream_t s, double* ops_per_s, double* ms);
