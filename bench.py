@@ -55,6 +55,9 @@ def parse_args():
                          "JSON line per (config, precision): rates, fractions of peak, dE/E, dL/L, encounter counts")
     ap.add_argument("--variant32", type=int, default=None, help="with --no-autotune: FP32 kernel variant (genga_set_tuning key 0)")
     ap.add_argument("--variant64", type=int, default=None, help="with --no-autotune: FP64 kernel variant (genga_set_tuning key 1)")
+    ap.add_argument("--mergers", action="store_true",
+                    help="NEXT-4: the performance shape with inflated radii and a merger pass (genga_merge) after every step; "
+                         "one JSON line: ms per step with and without the pass, bodies merged, what is conserved")
     ap.add_argument("--hybrid", action="store_true",
                     help="time the hybrid step instead (NEXT-1: weight_mode = 1, encounter_mode = 1, default listing and substeps)")
     ap.add_argument("--no-autotune", action="store_true", help="keep the default kernel variants (no start-up self-tuning)")
@@ -529,10 +532,62 @@ def run_report(args):
             print(json.dumps(line), flush=True)
 
 
+def run_mergers(args):
+    """NEXT-4 (R13): config 4 with radii inflated (bulk density 2 g/cm^3, factor 30, so that the
+    200 steps do see collisions), genga_merge after every step.  Timed with CUDA events around the whole run; the pass
+    synchronises (it returns N'), so its cost includes that round trip."""
+    import numpy as np
+    import torch
+    from paper_2309_08217_b200 import binding as B
+    from paper_2309_08217_b200 import workloads as W
+    B.load()
+    w = W.config(4)
+    steps = args.steps if args.steps else 200
+    AU_M, MSUN_KG, RHO, INFL = 1.495978707e11, 1.98892e30, 2000.0, 30.0
+    R = INFL * (3.0 * w.m * MSUN_KG / (4.0 * np.pi * RHO)) ** (1.0 / 3.0) / AU_M
+    for prec, name in ((B.FP32, "fp32"), (B.FP64, "fp64")):
+        res = {}
+        for mode in ("plain", "merging"):
+            g = B.from_workload(w)
+            g.autotune(prec)
+            if mode == "merging":
+                g.set_radii(torch.from_numpy(R).to(g.device))
+            E0, L0 = g.energy_angmom()
+            g.run(w.dt, 3, prec)                                     # warm-up; a first pass outside the timed region
+            if mode == "merging":
+                g.merge(prec)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            merged_timed = 0
+            for _ in range(steps):
+                g.run(w.dt, 1, prec)
+                if mode == "merging":
+                    n, status, newidx = g.merge(prec)
+                    merged_timed += n
+                    assert status == 0, status
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            E1, L1 = g.energy_angmom()
+            res[mode] = {"ms_per_step": ms / steps, "N_end": g.N, "merged_in_timed_steps": merged_timed,
+                         "dE_over_E": E1 / E0 - 1.0, "dL_over_L": float(np.linalg.norm(L1) / np.linalg.norm(L0) - 1.0)}
+            g.close()
+        print(json.dumps({"report": "mergers", "workload": w.name, "N": w.N, "steps": steps, "precision": name,
+                          "radius_inflation": INFL, "bulk_density_kg_m3": RHO, "R_au": float(R[0]),
+                          "plain": res["plain"], "merging": res["merging"],
+                          "pass_ms": res["merging"]["ms_per_step"] - res["plain"]["ms_per_step"],
+                          "note": "plain: genga_run one step at a time (K(dt/2) ... K(dt/2): two force evaluations per "
+                                  "call); merging: the same plus genga_merge after every step"}), flush=True)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.mergers:
+        run_mergers(args)
         return
     if args.report:
         run_report(args)

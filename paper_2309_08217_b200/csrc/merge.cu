@@ -15,18 +15,21 @@
 #include "genga_internal.cuh"
 
 namespace genga {
+namespace {
 
 constexpr int MERGE_THREADS = 1024;
 
 // label[i] = i, flag[i] = 0; status bit 2 if a body's radius exceeds half its critical radius (then the encounter
 // list need not contain every colliding pair).
 __global__ void merge_init_kernel(int N, const double* __restrict__ R, const double* __restrict__ rcrit,
-                                  int* __restrict__ label, int* __restrict__ flag, unsigned int* __restrict__ status)
+                                  int* __restrict__ label, int* __restrict__ flag, int* __restrict__ newidx,
+                                  unsigned int* __restrict__ status)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     label[i] = i;
     flag[i] = 0;
+    if (newidx) newidx[i] = i;                 // what it stays when nothing collides (the usual step)
     if (R[i] > 0.0 && !(2.0 * R[i] <= rcrit[i])) atomicOr(status, 2u);
 }
 
@@ -53,11 +56,21 @@ merge_kernel(int N, unsigned int pair_cap, const int2* __restrict__ pairs, Count
              int* label, int* flag, double4* acc1, double4* acc2,
              double* stage, int* newidx, unsigned int* out /* [0] N', [1] status */)
 {
-    __shared__ int s_changed;
+    __shared__ int s_changed, s_any;
     __shared__ int s_scan[MERGE_THREADS];
     const int t = threadIdx.x;
     unsigned int np = ctr->pair_count;
     if (np > pair_cap) { np = pair_cap; if (t == 0) atomicOr(&out[1], 1u); }      // list overflowed: pairs may be missing
+
+    // 0 ---- the usual step: no listed pair overlaps, nothing to do (newidx is the identity already)
+    if (t == 0) s_any = 0;
+    __syncthreads();
+    for (unsigned int p = t; p < np; p += MERGE_THREADS) {
+        const int2 ij = pairs[p];
+        if (collide(x, R, ij.x, ij.y)) s_any = 1;
+    }
+    __syncthreads();
+    if (!s_any) { if (t == 0) out[0] = (unsigned int)N; return; }
 
     // 1 ---- components of the collision graph
     for (;;) {
@@ -150,6 +163,8 @@ merge_kernel(int N, unsigned int pair_cap, const int2* __restrict__ pairs, Count
     if (t == 0) out[0] = (unsigned int)n_new;
 }
 
+}  // namespace
+
 void launch_merge(const Handle* h, int* newidx_dev)
 {
     if (h->N == 0) return;
@@ -157,7 +172,7 @@ void launch_merge(const Handle* h, int* newidx_dev)
     int* flag = h->w.glabel + h->NP;
     unsigned int* out = &h->w.ctr->merge_n;
     cudaMemsetAsync(out, 0, 2 * sizeof(unsigned int), h->stream);
-    merge_init_kernel<<<(h->N + 255) / 256, 256, 0, h->stream>>>(h->N, h->w.radius, h->w.rcrit, label, flag, out + 1);
+    merge_init_kernel<<<(h->N + 255) / 256, 256, 0, h->stream>>>(h->N, h->w.radius, h->w.rcrit, label, flag, newidx_dev, out + 1);
     merge_kernel<<<1, MERGE_THREADS, 0, h->stream>>>(h->N, (unsigned int)h->pair_cap, h->w.pairs, h->w.ctr,
                                                      h->w.m, h->w.x, h->w.v, h->w.radius, label, flag,
                                                      h->w.pk64, h->w.aux, h->w.vtmp, newidx_dev, out);
