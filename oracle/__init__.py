@@ -95,6 +95,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_energy_angmom.argtypes = [ctypes.c_int, _dp, _dp, _dp, _pp, _dp, _dp]
         L.oracle_merge.restype = ctypes.c_int
         L.oracle_merge.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _ip]
+        L.oracle_merge_tp2.restype = ctypes.c_int
+        L.oracle_merge_tp2.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _ip, ctypes.c_int, _ip]
         L.oracle_num_threads.restype = ctypes.c_int
         _lib = L
     return _lib
@@ -287,3 +289,13 @@ def merge(m, x, v, R):
     newidx = np.zeros(len(m), dtype=np.int32)
     n = lib().oracle_merge(len(m), _p(m), _p(x), _p(v), _p(R), newidx.ctypes.data_as(_ip))
     return m[:n].copy(), x[:n].copy(), v[:n].copy(), R[:n].copy(), newidx
+
+
+def merge_tp2(m, x, v, R, n_big: int):
+    """oracle.merge under TP2 mode's pair rule (readings R9, R13): only pairs that involve one of the first n_big bodies
+    can collide.  Returns (m', x', v', R', newidx, n_big')."""
+    m = _a(m).copy(); x = _a(x).copy(); v = _a(v).copy(); R = _a(R).copy()
+    newidx = np.zeros(len(m), dtype=np.int32)
+    nb = ctypes.c_int(0)
+    n = lib().oracle_merge_tp2(len(m), _p(m), _p(x), _p(v), _p(R), newidx.ctypes.data_as(_ip), int(n_big), ctypes.byref(nb))
+    return m[:n].copy(), x[:n].copy(), v[:n].copy(), R[:n].copy(), newidx, int(nb.value)

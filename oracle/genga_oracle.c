@@ -582,6 +582,15 @@ void oracle_energy_angmom(int N, const double* m, const double* x, const double*
  * relabelling to the smallest index until nothing changes, member sums in ascending index.        */
 int oracle_merge(int N, double* m, double* x, double* v, double* R, int* newidx)
 {
+    return oracle_merge_tp2(N, m, x, v, R, newidx, -1, (int*)0);
+}
+
+/* The same with TP2 mode's rule for which pairs exist (readings R9, R13): only pairs with i < n_big or
+ * j < n_big can collide (small bodies do not see each other); n_big < 0: every pair.  *n_big_new (may be NULL): the big
+ * bodies left, i.e. the survivors among the first n_big (two big bodies that merge leave one).                        */
+int oracle_merge_tp2(int N, double* m, double* x, double* v, double* R, int* newidx, int n_big, int* n_big_new)
+{
+    if (n_big_new) *n_big_new = n_big;
     if (N <= 0) return 0;
     int* lab = (int*)malloc(sizeof(int) * (size_t)N);
     for (int i = 0; i < N; ++i) lab[i] = i;
@@ -591,6 +600,7 @@ int oracle_merge(int N, double* m, double* x, double* v, double* R, int* newidx)
         for (int i = 0; i < N; ++i)
             for (int j = i + 1; j < N; ++j) {
                 if (lab[i] == lab[j]) continue;
+                if (n_big >= 0 && i >= n_big && j >= n_big) continue;
                 double dx = x[3 * j + 0] - x[3 * i + 0];
                 double dy = x[3 * j + 1] - x[3 * i + 1];
                 double dz = x[3 * j + 2] - x[3 * i + 2];
@@ -632,6 +642,11 @@ int oracle_merge(int N, double* m, double* x, double* v, double* R, int* newidx)
         ++n;
     }
     if (newidx) for (int i = 0; i < N; ++i) newidx[i] = where[lab[i]];
+    if (n_big_new && n_big >= 0) {
+        int nb = 0;
+        for (int i = 0; i < N && i < n_big; ++i) nb += (lab[i] == i);
+        *n_big_new = nb;
+    }
     free(where);
     free(lab);
     return n;

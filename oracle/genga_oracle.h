@@ -137,6 +137,8 @@ void oracle_energy_angmom(int N, const double* m, const double* x, const double*
  * over the members in ascending index.  newidx[N] (may be NULL): the new index of each old body
  * (of its survivor, for a removed body).  Returns the new body count.                                */
 int oracle_merge(int N, double* m, double* x, double* v, double* R, int* newidx);
+/* TP2 mode (reading R9): only pairs with i < n_big or j < n_big exist; *n_big_new = big bodies left.             */
+int oracle_merge_tp2(int N, double* m, double* x, double* v, double* R, int* newidx, int n_big, int* n_big_new);
 int oracle_num_threads(void);
 
 #ifdef __cplusplus

@@ -117,3 +117,38 @@ def test_empty_and_single():
     assert len(oracle.merge(np.zeros(0), z, z, np.zeros(0))[0]) == 0
     m2, x2, _, _, idx = oracle.merge(np.ones(1), np.ones((1, 3)), np.ones((1, 3)), np.ones(1))
     assert len(m2) == 1 and idx.tolist() == [0]
+
+
+def test_tp2_rule_small_bodies_do_not_collide_with_each_other():
+    """Reading R9 + R13: hand case on a line.  Bodies 0, 1 are big.  2 overlaps 0; 3 overlaps 2 only (a small-small
+    contact: no edge, 3 stays); 4 and 5 overlap each other only (stay); 1 overlaps 0 (two bigs merge: one big left)."""
+    x = np.zeros((6, 3)); x[:, 0] = [0.0, 1.5, -1.5, -3.0, 50.0, 51.0]
+    m = np.array([10.0, 6.0, 1.0, 1.0, 1.0, 1.0]); v = np.zeros((6, 3)); v[:, 1] = [0.0, 1.0, 2.0, 3.0, 4.0, 5.0]
+    R = np.ones(6)
+    m2, x2, v2, R2, idx, nb = oracle.merge_tp2(m, x, v, R, 2)
+    assert idx.tolist() == [0, 0, 0, 1, 2, 3] and nb == 1
+    assert m2.tolist() == [17.0, 1.0, 1.0, 1.0]
+    assert x2[:, 0].tolist() == [(6 * 1.5 - 1.5) / 17.0, -3.0, 50.0, 51.0]
+    assert v2[:, 1].tolist() == [(6.0 + 2.0) / 17.0, 3.0, 4.0, 5.0]
+    # the same bodies with every pair allowed: 0-1-2-3 is one chain, 4-5 a pair
+    m3, _, _, _, idx3 = oracle.merge(m, x, v, R)
+    assert idx3.tolist() == [0, 0, 0, 0, 1, 1] and m3.tolist() == [18.0, 2.0]
+    # n_big = N is the all-pairs rule; n_big = 0 lets nothing collide
+    assert oracle.merge_tp2(m, x, v, R, 6)[4].tolist() == idx3.tolist()
+    assert len(oracle.merge_tp2(m, x, v, R, 0)[0]) == 6
+
+
+def test_tp2_rule_equals_the_library_components_of_the_restricted_graph():
+    rng = np.random.default_rng(3)
+    n, nb = 300, 12
+    x = rng.uniform(-1, 1, (n, 3)); R = rng.uniform(0.01, 0.05, n); R[:nb] = 0.25
+    m = rng.uniform(0.5, 2, n); v = rng.normal(size=(n, 3))
+    d = np.linalg.norm(x[:, None, :] - x[None, :, :], axis=2)
+    big = np.arange(n) < nb
+    adj = (d < R[:, None] + R[None, :]) & ~np.eye(n, dtype=bool) & (big[:, None] | big[None, :])
+    ncomp, lab = connected_components(coo_matrix(adj), directed=False)
+    m2, x2, v2, R2, idx, nb2 = oracle.merge_tp2(m, x, v, R, nb)
+    assert len(m2) == ncomp < n - 10
+    assert ((idx[:, None] == idx[None, :]) == (lab[:, None] == lab[None, :])).all()
+    assert nb2 == len(set(idx[:nb].tolist()))
+    np.testing.assert_allclose(m2, np.bincount(idx, weights=m), rtol=1e-14)
