@@ -207,11 +207,14 @@ int genga_get_rcrit(genga_handle h, double* rcrit);      /* DEVICE [N]: r_crit,i
  * merged, one is run afterwards, so that the pair list, a_i and r_crit,i describe the new body set.
  *   newidx: DEVICE int[N] (N before the call) or NULL: new index of each old body (of the body that absorbed
  * it).  n_merged, status: HOST outputs (NULL = skip); status bit 1: the pair list had overflowed (pairs may
- * have been missed).  Synchronises the stream.  GENGA_EINVAL in TP2 mode (small-small pairs are not listed). */
+ * have been missed).  Synchronises the stream.
+ *   TP2 mode (params.n_big): only pairs with a big body exist, so small bodies never merge with each other; the
+ * handle's n_big becomes the number of survivors among the big bodies (genga_num_big_bodies).                  */
 int genga_set_radii(genga_handle h, const double* R);
 int genga_get_radii(genga_handle h, double* R);
 int genga_merge(genga_handle h, int precision, int* newidx, int* n_merged, int* status);
 int genga_num_bodies(genga_handle h);                    /* current N (shrinks with mergers); < 0 on a NULL handle */
+int genga_num_big_bodies(genga_handle h);                /* current params.n_big (-1: every pair interacts, or NULL) */
 
 /* Diagnostics of the last force evaluation: number of (body, j-chunk) near-field candidates and
  * whether the candidate list overflowed (exact slow path taken).  HOST outputs.  Synchronises.  */

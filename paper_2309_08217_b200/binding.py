@@ -26,7 +26,7 @@ SYMBOLS = [
     "genga_set_state", "genga_set_state_host", "genga_resort", "genga_kick", "genga_accel", "genga_drift",
     "genga_sunkick", "genga_step", "genga_run", "genga_leapfrog", "genga_encounter_pairs", "genga_energy_angmom",
     "genga_get_state", "genga_get_state_host", "genga_get_accel", "genga_get_rcrit",
-    "genga_set_radii", "genga_get_radii", "genga_merge", "genga_num_bodies",
+    "genga_set_radii", "genga_get_radii", "genga_merge", "genga_num_bodies", "genga_num_big_bodies",
     "genga_nearfield_stats", "genga_encounter_stats", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
     "genga_synchronize", "genga_strerror", "genga_last_cuda_error", "genga_version",
     "genga_peak_probe", "genga_set_tuning", "genga_autotune", "genga_num_variants", "genga_variant_name",
@@ -91,6 +91,7 @@ def load() -> ctypes.CDLL:
     L.genga_get_radii.argtypes = [vp, vp]
     L.genga_merge.argtypes = [vp, ctypes.c_int, vp, ip, ip]
     L.genga_num_bodies.argtypes = [vp]
+    L.genga_num_big_bodies.argtypes = [vp]
     L.genga_nearfield_stats.argtypes = [vp, llp, ip]
     L.genga_encounter_stats.argtypes = [vp, ip, ip, ip, ip, ip]
     L.genga_set_profiling.argtypes = [vp, ctypes.c_int]
@@ -268,6 +269,7 @@ class Genga:
         n, s = ctypes.c_int(0), ctypes.c_int(0)
         _check(self._L.genga_merge(self._h, int(precision), _dptr(newidx), ctypes.byref(n), ctypes.byref(s)), "genga_merge")
         self.N = int(self._L.genga_num_bodies(self._h))
+        self.n_big = int(self._L.genga_num_big_bodies(self._h))
         return int(n.value), int(s.value), newidx
 
     # ---- the path ------------------------------------------------------------------------------

@@ -148,6 +148,7 @@ static int launch_pairs(Handle* h, int precision)
 {
     if (h->p.n_big >= 0 && h->p.n_big < h->N) {          // TP2 mode: O(n_big N) pairs, FP64 (reading R9)
         if (h->p.n_big > 0) { ProfScope ps(h, 0); launch_tp2(h); LAUNCHED(h, "tp2_kernel"); }
+        h->pairs_current = true;
         return GENGA_OK;
     }
     { ProfScope ps(h, 0); if (precision == GENGA_FP32) launch_kick32(h); else launch_kick64(h); }
@@ -477,10 +478,14 @@ int genga_num_bodies(genga_handle h)
     return h ? h->N : GENGA_EINVAL;
 }
 
+int genga_num_big_bodies(genga_handle h)
+{
+    return h ? h->p.n_big : GENGA_EINVAL;
+}
+
 int genga_merge(genga_handle h, int precision, int* newidx, int* n_merged, int* status)
 {
     if (!h || (precision != GENGA_FP64 && precision != GENGA_FP32)) return GENGA_EINVAL;
-    if (h->p.n_big >= 0 && h->p.n_big < h->N) return GENGA_EINVAL;      // TP2 mode lists no small-small pairs
     if (n_merged) *n_merged = 0;
     if (status) *status = 0;
     if (h->N == 0) return GENGA_OK;
@@ -490,7 +495,8 @@ int genga_merge(genga_handle h, int precision, int* newidx, int* n_merged, int* 
     launch_merge(h, newidx); h->launches += 2;
     { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_, "merge kernels"); }
     h->enc_labels_valid = false;                                      // the label arrays served as scratch
-    unsigned int out[2];
+    const bool tp2 = h->p.n_big >= 0 && h->p.n_big < h->N;
+    unsigned int out[3];
     CU(cudaMemcpyAsync(out, &h->w.ctr->merge_n, sizeof(out), cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
     if (status) *status = (int)out[1];
@@ -500,6 +506,7 @@ int genga_merge(genga_handle h, int precision, int* newidx, int* n_merged, int* 
     if (n_new == h->N) return GENGA_OK;
     // fewer bodies: the arrays keep their places in the workspace, everything derived from N is redone
     h->N = n_new; h->NP = padded(n_new);
+    if (tp2) h->p.n_big = (int)out[2];                                 // merged big bodies leave one big body
     h->nchunk = (n_new + h->chunk - 1) / h->chunk;
     h->grid_cache[0][0] = h->grid_cache[1][0] = 0;
     h->evals_since_sort = -1;

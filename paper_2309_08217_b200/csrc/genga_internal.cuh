@@ -51,6 +51,7 @@ struct Counters {
     // mergers (merge.cu; NEXT-4): written by the last genga_merge
     unsigned int merge_n;        // body count after the pass
     unsigned int merge_status;   // 1 pair list had overflowed, 2 a radius exceeds half its critical radius
+    unsigned int merge_nbig;     // TP2 mode: big bodies after the pass
 };
 
 struct Workspace {

@@ -3,7 +3,9 @@
 // Bodies i, j collide iff r_ij < R_i + R_j (strict, FP64) at the positions of the last force evaluation.  The
 // candidates are the pairs of the encounter list that evaluation left (r_ij < r_crit,ij; the physical radii lie
 // far inside the critical radius, which merge_init_kernel checks per body).  Every connected component of the
-// collision graph becomes one body at its smallest index; the arrays are closed up in order.
+// collision graph becomes one body at its smallest index; the arrays are closed up in order.  In TP2 mode the list
+// holds only pairs with a big body (small bodies do not see each other, readings R9 + R13) and n_big follows the
+// survivors among the big bodies.
 //
 // A rare, tiny operation (a few pairs per step): one block does it, in phases separated by __syncthreads():
 //   1 labels: label[k] = smallest index reachable from k, by relabelling over the colliding pairs until stable;
@@ -54,9 +56,9 @@ __global__ void __launch_bounds__(MERGE_THREADS)
 merge_kernel(int N, unsigned int pair_cap, const int2* __restrict__ pairs, Counters* ctr,
              double* m, double* x, double* v, double* R,
              int* label, int* flag, double4* acc1, double4* acc2,
-             double* stage, int* newidx, unsigned int* out /* [0] N', [1] status */)
+             double* stage, int* newidx, int n_big, unsigned int* out /* [0] N', [1] status, [2] n_big' */)
 {
-    __shared__ int s_changed, s_any;
+    __shared__ int s_changed, s_any, s_nbig;
     __shared__ int s_scan[MERGE_THREADS];
     const int t = threadIdx.x;
     unsigned int np = ctr->pair_count;
@@ -70,7 +72,7 @@ merge_kernel(int N, unsigned int pair_cap, const int2* __restrict__ pairs, Count
         if (collide(x, R, ij.x, ij.y)) s_any = 1;
     }
     __syncthreads();
-    if (!s_any) { if (t == 0) out[0] = (unsigned int)N; return; }
+    if (!s_any) { if (t == 0) { out[0] = (unsigned int)N; out[2] = (unsigned int)(n_big > 0 ? n_big : 0); } return; }
 
     // 1 ---- components of the collision graph
     for (;;) {
@@ -139,8 +141,11 @@ merge_kernel(int N, unsigned int pair_cap, const int2* __restrict__ pairs, Count
     // 4 ---- close up the arrays in order: where[i] = number of survivors before i (kept in flag[])
     const int seg = (N + MERGE_THREADS - 1) / MERGE_THREADS;
     const int lo = min(t * seg, N), hi = min(lo + seg, N);
-    int cnt = 0;
-    for (int i = lo; i < hi; ++i) cnt += (label[i] == i);
+    int cnt = 0, cnt_big = 0;                        // TP2 mode: the survivors among the first n_big stay the big bodies
+    if (t == 0) s_nbig = 0;
+    __syncthreads();
+    for (int i = lo; i < hi; ++i) { const int keep = (label[i] == i); cnt += keep; cnt_big += keep && i < n_big; }
+    if (cnt_big) atomicAdd(&s_nbig, cnt_big);
     s_scan[t] = cnt;
     __syncthreads();
     for (int off = 1; off < MERGE_THREADS; off <<= 1) {
@@ -160,7 +165,7 @@ merge_kernel(int N, unsigned int pair_cap, const int2* __restrict__ pairs, Count
         compact(N, 1, label, flag, m, stage, n_new);
         compact(N, 1, label, flag, R, stage, n_new);
     }
-    if (t == 0) out[0] = (unsigned int)n_new;
+    if (t == 0) { out[0] = (unsigned int)n_new; out[2] = (unsigned int)s_nbig; }
 }
 
 }  // namespace
@@ -171,11 +176,12 @@ void launch_merge(const Handle* h, int* newidx_dev)
     int* label = h->w.glabel;
     int* flag = h->w.glabel + h->NP;
     unsigned int* out = &h->w.ctr->merge_n;
-    cudaMemsetAsync(out, 0, 2 * sizeof(unsigned int), h->stream);
+    cudaMemsetAsync(out, 0, 3 * sizeof(unsigned int), h->stream);
     merge_init_kernel<<<(h->N + 255) / 256, 256, 0, h->stream>>>(h->N, h->w.radius, h->w.rcrit, label, flag, newidx_dev, out + 1);
     merge_kernel<<<1, MERGE_THREADS, 0, h->stream>>>(h->N, (unsigned int)h->pair_cap, h->w.pairs, h->w.ctr,
                                                      h->w.m, h->w.x, h->w.v, h->w.radius, label, flag,
-                                                     h->w.pk64, h->w.aux, h->w.vtmp, newidx_dev, out);
+                                                     h->w.pk64, h->w.aux, h->w.vtmp, newidx_dev,
+                                                     (h->p.n_big >= 0 && h->p.n_big < h->N) ? h->p.n_big : -1, out);
 }
 
 }  // namespace genga

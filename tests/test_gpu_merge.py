@@ -179,7 +179,7 @@ def test_merge_after_a_drift_refreshes_the_pair_list_first():
     g.close()
 
 
-def test_oversized_radius_is_reported_and_tp2_is_refused():
+def test_oversized_radius_is_reported():
     import torch
     w, R = planted(0, 1000, 9, 2, 0, 0)
     g = B.from_workload(w)
@@ -189,11 +189,52 @@ def test_oversized_radius_is_reported_and_tp2_is_refused():
     _, status, _ = g.merge()
     assert status & 2
     g.close()
-    g = B.from_workload(w, n_big=10)
-    g.set_radii(torch.from_numpy(R).to(g.device))
-    with pytest.raises(Exception):
-        g.merge()
-    g.close()
+
+
+def test_tp2_mode_giants_accrete_planetesimals_which_do_not_collide_with_each_other():
+    """Config 3 in TP2 mode (the paper's planetesimal-driven migration runs): planetesimals moved
+    into giants are accreted; overlapping planetesimals are left alone (readings R9 + R13); two giants moved onto
+    each other leave one big body, and the handle's n_big follows."""
+    import torch
+    w = W.config(3, 3000)
+    n = w.N
+    rng = np.random.default_rng(12)
+    x = w.x.copy(); v = w.v.copy()
+    R = np.full(n, 2.0e-5); R[:4] = [4.7e-4, 3.9e-4, 1.7e-4, 1.6e-4]          # roughly the giants' radii in AU
+    ids = 4 + rng.permutation(n - 4)[:16]
+    for k, i in enumerate(ids[:9]):                                     # three planetesimals into each of giants 0, 1, 2
+        gidx = k % 3
+        x[i] = x[gidx] + 0.5 * R[gidx] * rng.normal(size=3) / np.sqrt(3); v[i] = v[gidx] * (1 + 1e-3 * rng.normal())
+    for i, j in zip(ids[9:15:2], ids[10:16:2]):                          # three overlapping small-small pairs
+        x[j] = x[i] + [1.0e-5, 0.0, 0.0]
+    for case_big_merge in (False, True):
+        xx = x.copy()
+        if case_big_merge:
+            xx[3] = xx[2] + [2.0e-4, 0.0, 0.0]                          # giant 3 into giant 2
+        ww = dataclasses.replace(w, x=xx, v=v)
+        g = B.from_workload(ww, n_big=4)
+        g.set_radii(torch.from_numpy(R).to(g.device))
+        g.accel(B.FP64)
+        x0, v0 = (t.cpu().numpy() for t in g.get_state())
+        n_merged, status, newidx = g.merge()
+        mo, xo, vo, Ro, idxo, nbo = oracle.merge_tp2(ww.m, x0, v0, R, 4)
+        assert status == 0 and n_merged == 9 + case_big_merge and g.N == len(mo)
+        assert nbo == 4 - case_big_merge and g.n_big == nbo
+        assert (newidx.cpu().numpy() == idxo).all()
+        x1, v1 = (t.cpu().numpy() for t in g.get_state())
+        assert (np.abs(x1 - xo) / np.linalg.norm(xo, axis=1, keepdims=True)).max() <= 1e-14
+        assert (np.abs(v1 - vo) / np.linalg.norm(vo, axis=1, keepdims=True)).max() <= 1e-14
+        # the shrunk TP2 system against the oracle: forces, pairs, two steps
+        p = oparams(ww, n_big=nbo)
+        ao = oracle.accel(mo, xo, vo, p)
+        a = g.get_accel().cpu().numpy()
+        assert (np.linalg.norm(a - ao, axis=1) / np.linalg.norm(ao, axis=1)).max() <= 1e-12
+        assert set(map(tuple, g.encounter_pairs().tolist())) == set(map(tuple, oracle.encounter_pairs(mo, xo, vo, p).tolist()))
+        g.run(ww.dt, 2, B.FP64)
+        xr, vr = oracle.run(mo, xo, vo, p, ww.dt, 2)
+        x2, _ = (t.cpu().numpy() for t in g.get_state())
+        assert (np.linalg.norm(x2 - xr, axis=1) / np.linalg.norm(xr, axis=1)).max() <= 1e-10
+        g.close()
 
 
 def test_merge_inside_the_hybrid_step():
