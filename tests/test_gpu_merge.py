@@ -258,3 +258,41 @@ def test_merge_inside_the_hybrid_step():
     groups, bodies, largest, missed, st = g.encounter_stats()
     assert missed == 0 and st == 0
     g.close()
+
+
+def test_degenerate_sizes_and_everything_merging_into_one_body():
+    import torch
+    dev = "cuda:0"
+    for n in (0, 1):                                                   # empty and single-body handles
+        m = torch.full((n,), 1e-7, dtype=torch.float64, device=dev)
+        x = torch.ones((n, 3), dtype=torch.float64, device=dev); v = torch.zeros((n, 3), dtype=torch.float64, device=dev)
+        g = B.Genga(m, x, v, device=dev)
+        g.set_radii(torch.ones((n,), dtype=torch.float64, device=dev))
+        n_merged, status, newidx = g.merge()
+        assert n_merged == 0 and g.N == n and newidx.cpu().tolist() == list(range(n))
+        g.close()
+    # 700 bodies (two 512-blocks, ragged) inside one radius: a single component whatever the order of the relabelling
+    w = W.config(0, 700)
+    rng = np.random.default_rng(2)
+    x = w.x[0] + 1.0e-5 * rng.normal(size=(700, 3)); v = w.v[0] * (1 + 1e-4 * rng.normal(size=(700, 1)))
+    ww = dataclasses.replace(w, x=x, v=v)
+    R = np.full(700, 2.0e-4)
+    g, res, pre, orc = merged_pair(ww, R, B.FP64, n1=300.0, pair_capacity=300000)   # r_crit wide enough to list all pairs
+    assert res[0] == 699 and g.N == 1 and len(orc[0]) == 1
+    check_merge(g, res, pre, orc, ww, R)
+    g.step(w.dt, B.FP64)                                                # a one-body system still steps (pure Kepler)
+    xr, vr = oracle.step(orc[0], orc[1], orc[2], oparams(ww, n1=300.0), w.dt)
+    x1, _ = (t.cpu().numpy() for t in g.get_state())
+    assert np.abs(x1 - xr).max() <= 1e-12 * np.linalg.norm(xr)
+    g.close()
+
+
+def test_an_overflowed_pair_list_is_reported():
+    w, R = planted(0, 1000, 13, 12, 0, 0)
+    import torch
+    g = B.from_workload(w, pair_capacity=4)
+    g.set_radii(torch.from_numpy(R).to(g.device))
+    g.accel(B.FP64)
+    _, status, _ = g.merge()
+    assert status & 1                                                  # pairs may have been missed, and the call says so
+    g.close()
