@@ -212,6 +212,7 @@ int genga_get_rcrit(genga_handle h, double* rcrit);      /* DEVICE [N]: r_crit,i
  * handle's n_big becomes the number of survivors among the big bodies (genga_num_big_bodies).                  */
 int genga_set_radii(genga_handle h, const double* R);
 int genga_get_radii(genga_handle h, double* R);
+int genga_get_mass(genga_handle h, double* m);           /* DEVICE double[N]: the masses (they change with mergers) */
 int genga_merge(genga_handle h, int precision, int* newidx, int* n_merged, int* status);
 int genga_num_bodies(genga_handle h);                    /* current N (shrinks with mergers); < 0 on a NULL handle */
 int genga_num_big_bodies(genga_handle h);                /* current params.n_big (-1: every pair interacts, or NULL) */

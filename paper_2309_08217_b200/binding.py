@@ -26,7 +26,7 @@ SYMBOLS = [
     "genga_set_state", "genga_set_state_host", "genga_resort", "genga_kick", "genga_accel", "genga_drift",
     "genga_sunkick", "genga_step", "genga_run", "genga_leapfrog", "genga_encounter_pairs", "genga_energy_angmom",
     "genga_get_state", "genga_get_state_host", "genga_get_accel", "genga_get_rcrit",
-    "genga_set_radii", "genga_get_radii", "genga_merge", "genga_num_bodies", "genga_num_big_bodies",
+    "genga_set_radii", "genga_get_radii", "genga_merge", "genga_get_mass", "genga_num_bodies", "genga_num_big_bodies",
     "genga_nearfield_stats", "genga_encounter_stats", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
     "genga_synchronize", "genga_strerror", "genga_last_cuda_error", "genga_version",
     "genga_peak_probe", "genga_set_tuning", "genga_autotune", "genga_num_variants", "genga_variant_name",
@@ -90,6 +90,7 @@ def load() -> ctypes.CDLL:
     L.genga_set_radii.argtypes = [vp, vp]
     L.genga_get_radii.argtypes = [vp, vp]
     L.genga_merge.argtypes = [vp, ctypes.c_int, vp, ip, ip]
+    L.genga_get_mass.argtypes = [vp, vp]
     L.genga_num_bodies.argtypes = [vp]
     L.genga_num_big_bodies.argtypes = [vp]
     L.genga_nearfield_stats.argtypes = [vp, llp, ip]
@@ -260,6 +261,12 @@ class Genga:
         R = torch.empty((self.N,), dtype=torch.float64, device=self.device)
         _check(self._L.genga_get_radii(self._h, _dptr(R)), "genga_get_radii")
         return R
+
+    def get_mass(self):
+        torch = self._torch
+        m = torch.empty((self.N,), dtype=torch.float64, device=self.device)
+        _check(self._L.genga_get_mass(self._h, _dptr(m)), "genga_get_mass")
+        return m
 
     def merge(self, precision=FP64):
         """Step-end perfect mergers (genga_merge, reading R13).  Returns (n_merged, status, newidx): newidx is a

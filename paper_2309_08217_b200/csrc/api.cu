@@ -473,6 +473,13 @@ int genga_get_radii(genga_handle h, double* R)
     return GENGA_OK;
 }
 
+int genga_get_mass(genga_handle h, double* m)
+{
+    if (!h || !m) return GENGA_EINVAL;
+    if (h->N) CU(cudaMemcpyAsync(m, h->w.m, (size_t)h->N * 8, cudaMemcpyDeviceToDevice, h->stream));
+    return GENGA_OK;
+}
+
 int genga_num_bodies(genga_handle h)
 {
     return h ? h->N : GENGA_EINVAL;

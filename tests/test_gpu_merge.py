@@ -79,13 +79,15 @@ def check_merge(g, res, pre, orc, w, R):
     assert (newidx == idxo).all()                                    # the partition and the order: exact
     x, v = (t.cpu().numpy() for t in g.get_state())
     Rg = g.get_radii().cpu().numpy()
+    mg = g.get_mass().cpu().numpy()
     assert x.shape == xo.shape
+    assert np.abs(mg / np.where(mo > 0, mo, 1.0) - (mo > 0)).max() <= 1e-13      # atomic sums of up to 700 members
     scale_x = np.linalg.norm(xo, axis=1, keepdims=True); scale_v = np.linalg.norm(vo, axis=1, keepdims=True)
     assert (np.abs(x - xo) / scale_x).max() <= 1e-14
     assert (np.abs(v - vo) / scale_v).max() <= 1e-14
     assert np.abs(Rg / Ro - 1).max() <= 1e-14
     alone = np.flatnonzero(np.bincount(idxo)[idxo] == 1)             # bodies nothing happened to: bit-exact
-    assert (x[idxo[alone]] == x0[alone]).all() and (v[idxo[alone]] == v0[alone]).all() and (Rg[idxo[alone]] == R[alone]).all()
+    assert (x[idxo[alone]] == x0[alone]).all() and (v[idxo[alone]] == v0[alone]).all() and (Rg[idxo[alone]] == R[alone]).all() and (mg[idxo[alone]] == w.m[alone]).all()
 
 
 @pytest.mark.parametrize("cfg,n,seed,plant", [
