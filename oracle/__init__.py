@@ -95,6 +95,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_energy_angmom.argtypes = [ctypes.c_int, _dp, _dp, _dp, _pp, _dp, _dp]
         L.oracle_merge.restype = ctypes.c_int
         L.oracle_merge.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _ip]
+        L.oracle_step_hybrid_collide.restype = ctypes.c_int
+        L.oracle_step_hybrid_collide.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _pp, ctypes.c_double, ctypes.c_int, _ip]
         L.oracle_merge_tp2.restype = ctypes.c_int
         L.oracle_merge_tp2.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _ip, ctypes.c_int, _ip]
         L.oracle_num_threads.restype = ctypes.c_int
@@ -299,3 +301,16 @@ def merge_tp2(m, x, v, R, n_big: int):
     nb = ctypes.c_int(0)
     n = lib().oracle_merge_tp2(len(m), _p(m), _p(x), _p(v), _p(R), newidx.ctypes.data_as(_ip), int(n_big), ctypes.byref(nb))
     return m[:n].copy(), x[:n].copy(), v[:n].copy(), R[:n].copy(), newidx, int(nb.value)
+
+
+def step_hybrid_collide(m, x, v, R, p: Params, dt: float, nsub: int):
+    """Reading R14 (oracle only so far): hybrid step with the collision pass after every substep of the A-flow.
+    Returns (m', x', v', R', newidx)."""
+    m = _a(m).copy(); x = _a(x).copy(); v = _a(v).copy(); R = _a(R).copy()
+    newidx = np.zeros(len(m), dtype=np.int32)
+    c = p.c()
+    n = lib().oracle_step_hybrid_collide(len(m), _p(m), _p(x), _p(v), _p(R), ctypes.byref(c), float(dt), int(nsub),
+                                         newidx.ctypes.data_as(_ip))
+    if n < 0:
+        raise ValueError("step_hybrid_collide needs weight_mode = 1 and nsub >= 1")
+    return m[:n].copy(), x[:n].copy(), v[:n].copy(), R[:n].copy(), newidx

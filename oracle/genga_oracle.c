@@ -651,3 +651,42 @@ int oracle_merge_tp2(int N, double* m, double* x, double* v, double* R, int* new
     free(lab);
     return n;
 }
+
+/* ---- NEXT-4, refinement: collisions INSIDE the encounter integration (reading R14; oracle only so far) ----
+ * The hybrid step of reading R11 with the collision pass of reading R13 applied after EVERY RK4 substep of the
+ * A-flow instead of once per step: an overlap is acted on at the first substep end that shows it.  The merged body
+ * inherits the frozen per-body quantities of the opening evaluation (r_crit,i, a_i, v_K,i) from the component's
+ * smallest index; masses are the merged ones.  newidx (may be NULL) maps the bodies before the step to the bodies
+ * after it.  R = 0 for every body reproduces oracle_step_hybrid bit for bit.  Returns N', or -1 on bad params.   */
+int oracle_step_hybrid_collide(int N, double* m, double* x, double* v, double* R, const oracle_params* p,
+                               double dt, int nsub, int* newidx)
+{
+    if (p->weight_mode != 1 || nsub < 1) return -1;
+    size_t n1 = (size_t)(N > 0 ? N : 1);
+    double* rc = (double*)malloc(sizeof(double) * n1);
+    double* sa = (double*)malloc(sizeof(double) * n1);
+    double* vk = (double*)malloc(sizeof(double) * n1);
+    int* step_idx = (int*)malloc(sizeof(int) * n1);
+    int* total = (int*)malloc(sizeof(int) * n1);
+    for (int i = 0; i < N; ++i) total[i] = i;
+    int n = N;
+    oracle_rcrit(n, m, x, v, p, rc, sa, vk);
+    oracle_kick(n, m, x, v, p, 0.5 * dt, NULL);
+    oracle_sunkick(n, m, x, v, p, 0.5 * dt);
+    for (int s = 0; s < nsub; ++s) {
+        oracle_encounter_drift(n, m, x, v, p, rc, sa, vk, dt / nsub, 1);      /* one RK4 substep of the A-flow */
+        int n_new = oracle_merge(n, m, x, v, R, step_idx);
+        if (n_new < n) {
+            int k = 0;                                   /* survivors appear in order of their smallest member */
+            for (int i = 0; i < n; ++i)
+                if (step_idx[i] == k) { rc[k] = rc[i]; sa[k] = sa[i]; vk[k] = vk[i]; ++k; }
+            for (int i = 0; i < N; ++i) total[i] = step_idx[total[i]];
+            n = n_new;
+        }
+    }
+    oracle_sunkick(n, m, x, v, p, 0.5 * dt);
+    oracle_kick(n, m, x, v, p, 0.5 * dt, NULL);
+    if (newidx) for (int i = 0; i < N; ++i) newidx[i] = total[i];
+    free(rc); free(sa); free(vk); free(step_idx); free(total);
+    return n;
+}

@@ -139,6 +139,10 @@ void oracle_energy_angmom(int N, const double* m, const double* x, const double*
 int oracle_merge(int N, double* m, double* x, double* v, double* R, int* newidx);
 /* TP2 mode (reading R9): only pairs with i < n_big or j < n_big exist; *n_big_new = big bodies left.             */
 int oracle_merge_tp2(int N, double* m, double* x, double* v, double* R, int* newidx, int n_big, int* n_big_new);
+/* Reading R14 (NOT built on the GPU yet): the hybrid step with the collision pass after every RK4 substep of the
+ * A-flow; the merged body inherits the frozen r_crit,i, a_i, v_K,i of the component's smallest index.  Returns N'. */
+int oracle_step_hybrid_collide(int N, double* m, double* x, double* v, double* R, const oracle_params* p,
+                               double dt, int nsub, int* newidx);
 int oracle_num_threads(void);
 
 #ifdef __cplusplus
