@@ -32,6 +32,12 @@
  *                          encounter (full E) vs the level-0-only step, dt^2 convergence to DOP853
  *   TP2 mode (n_big >= 0)  pinned: hand 3-body values, full-minus-subset identity against the
  *                          pinned all-pairs path, sum m a = 0, bounded dt^2 energy error
+ *   oracle_merge(_tp2)     pinned: inelastic-collision identities (dT = mu u^2/2, dL = mu x_rel x v_rel),
+ *                          hand values (pair, chain, strictness, massless), scipy connected components,
+ *                          conserved extensive sums (reading R13: WHEN collisions are looked for is a
+ *                          reading -- the paper does not say; "parity unpinned by PAPER.md" for that choice)
+ *   oracle_step_hybrid_collide  pinned: R = 0 is oracle_step_hybrid bit for bit, free-body closed forms,
+ *                          impact parameter, pass-through vs step-end pass (reading R14; no GPU counterpart yet)
  */
 #ifndef GENGA_ORACLE_H
 #define GENGA_ORACLE_H
@@ -116,7 +122,7 @@ int oracle_step(int N, const double* m, double* x, double* v,
 int oracle_run(int N, const double* m, double* x, double* v,
                const oracle_params* p, double dt, int nsteps);
 
-/* NEXT-1 (not built on the GPU yet; reading R11): the hybrid step with the encounter complement,
+/* NEXT-1 (reading R11; GPU: params.encounter_mode = 1): the hybrid step with the encounter complement,
  * B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2), A = flow of Kepler + sum (1-K)-weighted pair terms integrated with
  * nsub RK4 substeps for all bodies (r_crit,ij held at the opening evaluation's values).  weight_mode must be 1. */
 void oracle_encounter_drift(int N, const double* m, double* x, double* v, const oracle_params* p,
