@@ -193,12 +193,13 @@ def test_oversized_radius_is_reported():
     g.close()
 
 
-def test_tp2_mode_giants_accrete_planetesimals_which_do_not_collide_with_each_other():
+@pytest.mark.parametrize("n_pl", [3000, 30000])                          # 30 000: the size of the paper's runs
+def test_tp2_mode_giants_accrete_planetesimals_which_do_not_collide_with_each_other(n_pl):
     """Config 3 in TP2 mode (the paper's planetesimal-driven migration runs): planetesimals moved
     into giants are accreted; overlapping planetesimals are left alone (readings R9 + R13); two giants moved onto
     each other leave one big body, and the handle's n_big follows."""
     import torch
-    w = W.config(3, 3000)
+    w = W.config(3, n_pl)
     n = w.N
     rng = np.random.default_rng(12)
     x = w.x.copy(); v = w.v.copy()
