@@ -15,9 +15,11 @@
  *   step  (reading G3): K(dt/2) S(dt/2) D(dt) S(dt/2) K(dt/2) in democratic
  *        heliocentric variables (heliocentric x, barycentric v).
  *   energy_angmom: total energy E and angular momentum L of the stored state.
+ *   merge ("perfect mergers"; reading R13, optional): overlapping bodies (r_ij < R_i + R_j) become one
+ *        at a step end; N shrinks.  genga_set_radii / genga_merge / genga_num_bodies / genga_get_mass below.
  *
  * Conventions
- *   N        number of bodies, the star excluded.  N = 0 and N = 1 are valid.
+ *   N        number of bodies, the star excluded.  N = 0 and N = 1 are valid.  N only changes in genga_merge.
  *   m        [N]      FP64 masses.  m = 0 (test particle) is valid.
  *   x, v, a  [N][3]   FP64, row-major (a contiguous (N,3) float64 tensor).  x is heliocentric.
  *            The STORED velocity is barycentric ("democratic").  If params.v_is_heliocentric,
