@@ -148,7 +148,7 @@ static int launch_pairs(Handle* h, int precision)
 {
     if (h->p.n_big >= 0 && h->p.n_big < h->N) {          // TP2 mode: O(n_big N) pairs, FP64 (reading R9)
         if (h->p.n_big > 0) { ProfScope ps(h, 0); launch_tp2(h); LAUNCHED(h, "tp2_kernel"); }
-        h->pairs_current = true;
+        h->pairs_current = h->p.n_big > 0;              // only a kernel that rebuilt the list makes it current
         return GENGA_OK;
     }
     { ProfScope ps(h, 0); if (precision == GENGA_FP32) launch_kick32(h); else launch_kick64(h); }
@@ -190,6 +190,11 @@ static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_d
     a.enc.eta = h->p.enc_eta;
     cudaError_t e;
     if (enc) {                                         // groups of the pair list the last force evaluation left
+        if (!h->pairs_current) {                       // no list of the current positions (first call after create /
+            const int rc = force_eval(h, precision);   // set_state / genga_drift / genga_sunkick): make one, or the
+            if (rc != GENGA_OK) return rc;             // complement forces of the pairs inside their zones are lost
+            a.prep = make_prep_args(h, precision, 0.0);
+        }
         e = launch_groups(h);
         ++h->launches;
         if (e != cudaSuccess) return cuda_fail(e, "group_kernel");
@@ -441,7 +446,7 @@ static int set_state_impl(genga_handle h, const double* m, const double* x, cons
     if (m) CU(cudaMemcpyAsync(h->w.m, m, n * 8, kind, h->stream));
     if (x) { CU(cudaMemcpyAsync(h->w.x, x, n * 24, kind, h->stream)); h->enc_labels_valid = false; h->pairs_current = false; }
     if (v) { CU(cudaMemcpyAsync(h->w.v, v, n * 24, kind, h->stream)); h->mom_a_valid = false; }
-    if (m) h->mom_a_valid = false;
+    if (m) { h->mom_a_valid = false; h->pairs_current = false; h->enc_labels_valid = false; }   // r_crit follows m
     if (m) { launch_hcbrt(h); LAUNCHED(h, "hcbrt_kernel"); }
     if (v && h->p.v_is_heliocentric) return to_democratic(h);
     return GENGA_OK;

@@ -55,8 +55,6 @@ __device__ __forceinline__ float min3(float a, float b, float c)
     float r; asm("min.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c)); return r;
 }
 
-constexpr float EPS2 = 1.0e-30f;   // added to r^2 so that the self pair (d = 0 exactly) contributes 0, not NaN;
-                                   // 1e-15 au: nothing for any pair the FP32 path keeps (r > lambda r_crit)
 
 // One j-chunk against the I i-bodies of this thread.  SELF: the chunk holds this warp's own
 // slots; the self pair is then left out of the smallest-r^2 tracking (slot index compare), so a
@@ -66,7 +64,6 @@ __device__ __forceinline__ void pair_loop(const float4* __restrict__ jp, const f
                                           const float (&nz)[I], f2 (&ax)[I], f2 (&ay)[I], f2 (&az)[I],
                                           float (&mn)[I], const int (&self_off)[I])
 {
-    const f2 eps = pk(EPS2, EPS2);
 #pragma unroll UNR
     for (int jj = 0; jj < CHUNK / 2; ++jj) {
         const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
@@ -77,7 +74,7 @@ __device__ __forceinline__ void pair_loop(const float4* __restrict__ jp, const f
             const f2 dx = SC ? fma2(gj, pk(nx[k], nx[k]), xj) : add2(xj, pk(nx[k], nx[k]));
             const f2 dy = SC ? fma2(gj, pk(ny[k], ny[k]), yj) : add2(yj, pk(ny[k], ny[k]));
             const f2 dz = SC ? fma2(gj, pk(nz[k], nz[k]), zj) : add2(zj, pk(nz[k], nz[k]));
-            f2 r2 = (SELF && !SC) ? fma2(dx, dx, eps) : mul2(dx, dx);
+            f2 r2 = mul2(dx, dx);
             r2 = fma2(dy, dy, r2);
             r2 = fma2(dz, dz, r2);
             float r2a, r2b; upk(r2, r2a, r2b);
@@ -86,7 +83,9 @@ __device__ __forceinline__ void pair_loop(const float4* __restrict__ jp, const f
                 const bool sa = (2 * jj == self_off[k]), sb = (2 * jj + 1 == self_off[k]);
                 mn[k] = min3(mn[k], sa ? 3.0e38f : r2a, sb ? 3.0e38f : r2b);
                 ya = rsq(r2a); yb = rsq(r2b);
-                if (SC) { ya = sa ? 0.f : ya; yb = sb ? 0.f : yb; }   // D_self is rounding residue, not 0
+                // the self term is 0 by selection, for any mass: d_self = 0 gives y = inf (plain records), and
+                // D_self is rounding residue (mass-scaled records); a product with y would be NaN or garbage
+                ya = sa ? 0.f : ya; yb = sb ? 0.f : yb;
             } else {
                 if (!FAR) mn[k] = min3(mn[k], r2a, r2b);      // FAR: the chunk's bounding sphere is out of reach
                 ya = rsq(r2a); yb = rsq(r2b);

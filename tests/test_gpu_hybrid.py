@@ -240,3 +240,34 @@ def test_adaptive_substeps_resolve_a_deep_flyby():
     g.step(w.dt, B.FP64)
     assert g.encounter_stats()[4] == 8
     g.close()
+
+
+def test_leapfrog_as_the_first_call_builds_its_own_pair_list():
+    # genga_leapfrog has no leading kick: called right after genga_create (or after set_state(x), genga_drift,
+    # genga_sunkick) there is no pair list of the current positions.  The library must make one before it forms the
+    # groups; otherwise the planted pairs and the triple drift on Kepler orbits and their complement forces are lost.
+    w = disc_with_planted_groups(1000, 4)
+    res = []
+    for prime in (False, True):
+        g = hybrid(w, enc_nsub=128)
+        if prime:
+            g.accel(B.FP64)                                      # list and r_crit of the initial state, explicitly
+        g.leapfrog(w.dt, 1, B.FP64)
+        x, v = (t.cpu().numpy() for t in g.get_state())
+        st = g.encounter_stats()
+        g.close()
+        assert st[3] == 0 and st[4] == 0 and st[0] >= 5 and st[1] >= 11, (prime, st)
+        res.append((x, v))
+    assert state_err(res[0][0], res[0][1], res[1][0], res[1][1]) <= 1e-13
+    g = B.from_workload(w, weight_mode=1, mega_nmax=-1)          # level 0 only: the planted bodies end elsewhere
+    g.leapfrog(w.dt, 1, B.FP64)
+    x0, v0 = (t.cpu().numpy() for t in g.get_state())
+    g.close()
+    assert state_err(res[0][0], res[0][1], x0, v0) > 1e-6
+    # and after a plain drift (which invalidates the list) the same holds
+    g = hybrid(w, enc_nsub=128)
+    g.accel(B.FP64); g.drift(0.0); g.leapfrog(w.dt, 1, B.FP64)
+    x, v = (t.cpu().numpy() for t in g.get_state())
+    st = g.encounter_stats()
+    g.close()
+    assert st[0] >= 5 and state_err(x, v, res[1][0], res[1][1]) <= 1e-13
