@@ -20,7 +20,7 @@ _OBJ_DIR = os.path.join(_HERE, "build")
 
 SOURCES = ["api.cu", "prep.cu", "fused_step.cu", "mega_step.cu", "kick_fp32.cu", "kick_fp64.cu", "nearfield.cu", "drift.cu", "reduce.cu", "merge.cu", "probe.cu"]
 HEADERS = ["genga_internal.cuh", "tile_pipeline.cuh", "momentum.cuh", "kepler.cuh", "prep_tile.cuh",
-           "kick32_body.cuh", "kick64_body.cuh", "nearfield_body.cuh", "onbody_body.cuh", "encounter.cuh"]
+           "kick32_body.cuh", "kick64_body.cuh", "kick_sym_body.cuh", "nearfield_body.cuh", "onbody_body.cuh", "encounter.cuh"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=true"]
@@ -39,8 +39,11 @@ def _newest_header() -> float:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile every .cu to an object (only the stale ones) and link the shared library."""
+    """Compile every .cu to an object (only the stale ones) and link the shared library.
+    ``GENGA_NVCC_EXTRA`` (environment, space separated) appends flags, e.g. ``-DGENGA_SYM_STATS`` for the
+    cycle counters of the symmetric kernels (a debugging build; pass --force with it)."""
     nvcc = _nvcc()
+    extra = os.environ.get("GENGA_NVCC_EXTRA", "").split()
     os.makedirs(_OBJ_DIR, exist_ok=True)
     hdr_t = _newest_header()
     objs, procs = [], []
@@ -49,7 +52,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         o = os.path.join(_OBJ_DIR, src.replace(".cu", ".o"))
         objs.append(o)
         if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr_t):
-            cmd = [nvcc, *NVCC_FLAGS, "-I", _INC, "-c", s, "-o", o]
+            cmd = [nvcc, *NVCC_FLAGS, *extra, "-I", _INC, "-c", s, "-o", o]
             if verbose:
                 cmd.insert(1, "-Xptxas")
                 cmd.insert(2, "-v")

@@ -53,6 +53,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_gi = take(std::min((size_t)pair_cap, NP / 2) * 9 * 4);      // encounter groups: count + 8 members each
     const size_t o_gu = take(std::min(2 * (size_t)pair_cap, NP) * 4);
     const size_t o_rad = take(NP * 8);
+    const size_t o_as = take(NP * 24);
     if (w && base) {
         char* b = static_cast<char*>(base);
         w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
@@ -67,6 +68,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
         w->bkeys = (unsigned long long*)(b + o_bk); w->sortbuf = (unsigned int*)(b + o_sb);
         w->glabel = (int*)(b + o_gl); w->ginfo = (int*)(b + o_gi); w->gulist = (int*)(b + o_gu);
         w->radius = (double*)(b + o_rad);
+        w->aslot = (double*)(b + o_as);
     }
     return off;
 }

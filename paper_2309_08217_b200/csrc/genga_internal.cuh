@@ -31,8 +31,9 @@ struct __align__(16) BoundP { float hq, aq, rf, pad; };
 struct __align__(16) ChunkP { double ox, oy, oz; float hq, aq, rf, rad; float q2max, pad_; };
 static_assert(sizeof(ChunkP) == 48, "ChunkP is staged with 16-byte bulk copies");
 
-// j-side layouts.  FP32: two bodies per 32 bytes (packed for FFMA2 along j):
-//   float4 A = (x0, x1, y0, y1), float4 B = (z0, z1, gm0, gm1).
+// j-side layouts.  FP32: two bodies per pair of float4 (packed for FFMA2 along j), in two planes per chunk:
+//   [CHUNK/2] float4 A = (x0, x1, y0, y1), then [CHUNK/2] float4 B = (z0, z1, gm0, gm1)
+//   (lanes that read consecutive pairs hit consecutive 16-byte words: conflict-free LDS.128).
 // FP64: double4 (x, y, z, gm) per body.
 // FP32 positions are relative to the origin of the body's own chunk (ChunkP).
 struct Counters {
@@ -76,7 +77,7 @@ struct Workspace {
     int* ginfo;                 // [enc::GINFO x max groups] per group: member count, members
     int* gulist;                // [min(2 pair_cap, NP)] the bodies that occur in the pair list, each once
     double4* pk64;    // [NP]   (x, y, z, G m)
-    float4*  pk32;    // [NP]   pair-interleaved, see above
+    float4*  pk32;    // [NP]   two planes per chunk, see above
     double4* aux;     // [NP]   (m, r_crit, a, v_K): what the exact pair rule O3 needs
     BoundP*  bi;      // [NP]   per-body bound parameters
     ChunkP*  bc;      // [NP/chunk] per-chunk maxima and frame origin
@@ -88,6 +89,8 @@ struct Workspace {
     double*  vtmp;    // [NP][3] staging for heliocentric-velocity output
     double*  mom;     // momentum slots and per-block partials of the fused step (momentum.cuh)
     double*  radius;  // [NP] physical radii R_i (genga_set_radii; 0 = the body never collides)
+    double*  aslot;   // [3][NP] sums of the symmetric all-pairs kernels in the internal order (kick_sym_body.cuh: aslot_index),
+                      //         zeroed by the prep step, folded into a[] by the near-field kernel
     Counters* ctr;
 };
 

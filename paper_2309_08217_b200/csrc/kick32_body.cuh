@@ -66,7 +66,7 @@ __device__ __forceinline__ void pair_loop(const float4* __restrict__ jp, const f
 {
 #pragma unroll UNR
     for (int jj = 0; jj < CHUNK / 2; ++jj) {
-        const float4 A = jp[2 * jj], B = jp[2 * jj + 1];
+        const float4 A = jp[jj], B = jp[CHUNK / 2 + jj];     // planes (x0,x1,y0,y1) | (z0,z1,g0,g1)
         const f2 xj = pk(A.x, A.y), yj = pk(A.z, A.w), zj = pk(B.x, B.y), gj = pk(B.z, B.w);
 #pragma unroll
         for (int k = 0; k < I; ++k) {

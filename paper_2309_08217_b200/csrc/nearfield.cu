@@ -84,7 +84,8 @@ tp2_kernel(NfParams P, int n_big, Workspace w)
 void launch_nearfield(const Handle* h)
 {
     if (h->N == 0) return;
-    const NfParams P = make_nf_params(h);
+    NfParams P = make_nf_params(h);
+    P.gather = 1;
     int blocks = h->num_sms * 16;
     const long long need = ((long long)h->N + 15) / 16;          // a warp per four bodies is plenty (candidates << N)
     if (blocks > need && need > 0) blocks = (int)((need < h->num_sms) ? h->num_sms : need);

@@ -25,6 +25,7 @@ struct NfParams {
     double list_vdt;                               // ... and, if >= 0, only those with r - r_crit,ij < list_vdt |v_i - v_j|
     int check_missed;                              // encounter mode: count pairs inside their zone that the last drift had not grouped
     unsigned int cand_cap, pair_cap;
+    int gather, NP;                                // fold aslot[] (sums of the symmetric all-pairs kernels) into a[] first
 };
 
 inline NfParams make_nf_params(const Handle* h)
@@ -37,6 +38,7 @@ inline NfParams make_nf_params(const Handle* h)
     P.list_vdt = (h->p.encounter_mode != 0 && h->p.enc_list_vfactor >= 0.0) ? h->p.enc_list_vfactor * h->enc_dt : -1.0;
     P.check_missed = (h->p.encounter_mode != 0 && h->enc_labels_valid) ? 1 : 0;
     P.cand_cap = (unsigned int)h->cand_cap; P.pair_cap = (unsigned int)h->pair_cap;
+    P.gather = 0; P.NP = h->NP;
     return P;
 }
 
@@ -211,6 +213,19 @@ __device__ __forceinline__ void nearfield_body(const NfParams& P, Workspace& w)
     int* near_list = s_near[threadIdx.x >> 5];
 
     if (count <= P.cand_cap) {
+        if (P.gather) {
+            // the symmetric all-pairs kernels leave their sums in aslot[] (internal order, pairs split for coalescing):
+            // a[order[s]] += aslot[s'].  Atomic, because other warps add near-field terms to the same a[] meanwhile.
+            for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < P.N; s += gridDim.x * blockDim.x) {
+                const int b = s & (CHUNK - 1);
+                const int k = (s - b) + (b & 1) * (CHUNK / 2) + (b >> 1);
+                const double vx = w.aslot[k], vy = w.aslot[P.NP + k], vz = w.aslot[2 * P.NP + k];
+                if (vx != 0.0 || vy != 0.0 || vz != 0.0) {
+                    const int i = w.order[s];
+                    atomicAdd(&w.a[3 * i + 0], vx); atomicAdd(&w.a[3 * i + 1], vy); atomicAdd(&w.a[3 * i + 2], vz);
+                }
+            }
+        }
         for (unsigned int q = warp; q < count; q += nwarp) {
             const int2 cd = w.cand[q];
             const IBody I = load_ibody(w, cd.x);

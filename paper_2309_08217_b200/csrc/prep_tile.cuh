@@ -25,7 +25,7 @@ __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int t
                                           double shx, double shy, double shz)
 {
     __shared__ unsigned int smax[PREP_NT / 32][5];
-    __shared__ double sorg[PREP_NT / CHUNK][3];
+    __shared__ float sbox[PREP_NT / 32][6];                // per warp: min and max of the live positions
     const int s = tile * PREP_NT + threadIdx.x;            // slot; tiles cover NP exactly (NP % 512 == 0)
     const bool live = s < A.N;
     const int i = w.order[s];                              // body held by this slot (= s for padding)
@@ -71,16 +71,41 @@ __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int t
         if (!(rf >= 0.f)) rf = 3.0e38f;
     }
     w.a[3 * i + 0] = 0.0; w.a[3 * i + 1] = 0.0; w.a[3 * i + 2] = 0.0;
+    w.aslot[s] = 0.0; w.aslot[A.NP + s] = 0.0; w.aslot[2 * A.NP + s] = 0.0;   // any one-to-one slot mapping zeroes it all
     w.pk64[s] = make_double4(px, py, pz, gm);
     w.aux[s]  = ax4;
-    // local frame of this slot's chunk: origin = position of the chunk's first slot (FP32 policy P32),
-    // handed over through shared memory (the chunk's 64 slots are two warps of this block)
-    if ((s & (CHUNK - 1)) == 0) {
-        const int c = threadIdx.x / CHUNK;
-        sorg[c][0] = px; sorg[c][1] = py; sorg[c][2] = pz;
+    // local frame of this slot's chunk (FP32 policy P32): origin = centre of the bounding box of the chunk's live
+    // bodies (any FP64 point would do; the centre halves the chunk radius against a corner), found by warp
+    // reductions handed over through shared memory (a chunk is CHUNK / 32 warps of this block)
+    {
+        float lo0 = live ? (float)px : 3.0e38f, lo1 = live ? (float)py : 3.0e38f, lo2 = live ? (float)pz : 3.0e38f;
+        float hi0 = live ? (float)px : -3.0e38f, hi1 = live ? (float)py : -3.0e38f, hi2 = live ? (float)pz : -3.0e38f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo0 = fminf(lo0, __shfl_xor_sync(0xffffffffu, lo0, o)); hi0 = fmaxf(hi0, __shfl_xor_sync(0xffffffffu, hi0, o));
+            lo1 = fminf(lo1, __shfl_xor_sync(0xffffffffu, lo1, o)); hi1 = fmaxf(hi1, __shfl_xor_sync(0xffffffffu, hi1, o));
+            lo2 = fminf(lo2, __shfl_xor_sync(0xffffffffu, lo2, o)); hi2 = fmaxf(hi2, __shfl_xor_sync(0xffffffffu, hi2, o));
+        }
+        if ((threadIdx.x & 31) == 0) {
+            float* b = sbox[threadIdx.x >> 5];
+            b[0] = lo0; b[1] = lo1; b[2] = lo2; b[3] = hi0; b[4] = hi1; b[5] = hi2;
+        }
     }
     __syncthreads();
-    const double ox = sorg[threadIdx.x / CHUNK][0], oy = sorg[threadIdx.x / CHUNK][1], oz = sorg[threadIdx.x / CHUNK][2];
+    auto chunk_origin = [&](int c, double& ox_, double& oy_, double& oz_) {
+        float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+        for (int ww = 0; ww < CHUNK / 32; ++ww)
+            for (int t = 0; t < 3; ++t) {
+                lo[t] = fminf(lo[t], sbox[c * (CHUNK / 32) + ww][t]);
+                hi[t] = fmaxf(hi[t], sbox[c * (CHUNK / 32) + ww][3 + t]);
+            }
+        const bool any = lo[0] <= hi[0] && lo[1] <= hi[1] && lo[2] <= hi[2];      // false: no live body (or NaN state)
+        ox_ = any ? (double)(0.5f * lo[0] + 0.5f * hi[0]) : 0.0;
+        oy_ = any ? (double)(0.5f * lo[1] + 0.5f * hi[1]) : 0.0;
+        oz_ = any ? (double)(0.5f * lo[2] + 0.5f * hi[2]) : 0.0;
+    };
+    double ox, oy, oz;
+    chunk_origin(threadIdx.x / CHUNK, ox, oy, oz);
     const double qx = px - ox, qy = py - oy, qz = pz - oz;
     float rad = 0.f;                                        // |x - o|, rounded up; padding does not count
     if (live) {
@@ -94,15 +119,18 @@ __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int t
     const bool massive = live && (gm >= 1.0e-30) && (gm <= 1.0e30);
     float q2 = 0.f;
     {
-        float* f = reinterpret_cast<float*>(w.pk32) + 8 * (s >> 1) + (s & 1);
+        // two planes per chunk, two bodies per float4: [CHUNK/2] (x0, x1, y0, y1), then [CHUNK/2] (z0, z1, g0, g1)
+        const int cb = s & ~(CHUNK - 1), u = (s & (CHUNK - 1)) >> 1;
+        float* fa = reinterpret_cast<float*>(w.pk32 + cb + u) + (s & 1);
+        float* fb = reinterpret_cast<float*>(w.pk32 + cb + CHUNK / 2 + u) + (s & 1);
         if (!A.scaled) {
-            f[0] = (float)qx; f[2] = (float)qy; f[4] = (float)qz; f[6] = (float)gm;
+            fa[0] = (float)qx; fa[2] = (float)qy; fb[0] = (float)qz; fb[2] = (float)gm;
         } else if (massive) {
             const double q = rsqrt(gm);
-            f[0] = (float)(q * qx); f[2] = (float)(q * qy); f[4] = (float)(q * qz); f[6] = (float)q;
+            fa[0] = (float)(q * qx); fa[2] = (float)(q * qy); fb[0] = (float)(q * qz); fb[2] = (float)q;
             q2 = __double2float_ru(q * q * (1.0 + 1.0e-6));
         } else {
-            f[0] = 1.0e18f; f[2] = 0.f; f[4] = 0.f; f[6] = 0.f;
+            fa[0] = 1.0e18f; fa[2] = 0.f; fb[0] = 0.f; fb[2] = 0.f;
         }
     }
     const float rfc = (A.scaled && live && !massive) ? 3.0e38f : rf;   // massless j: (i, this chunk) always FP64
@@ -132,11 +160,11 @@ __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int t
         q.rf  = fmaxf(__uint_as_float(mx[2]), __fmul_ru(__fmul_ru(2.0f * A.floor_rel, q.rad), 1.000001f));
         q.q2max = A.scaled ? __uint_as_float(mx[4]) : 1.0f;   // scales the bound to the kernel's r'^2 = q^2 r^2
         q.pad_ = 0.f;
-        q.ox = sorg[c][0]; q.oy = sorg[c][1]; q.oz = sorg[c][2];
+        chunk_origin(c, q.ox, q.oy, q.oz);
         w.bc[tile * (PREP_NT / CHUNK) + c] = q;
     }
     if (s == 0) { w.ctr->cand_count = 0u; w.ctr->pair_count = 0u; w.ctr->overflow = 0u; }
-    __syncthreads();                                       // smax / sorg may be reused by the next tile
+    __syncthreads();                                       // smax / sbox may be reused by the next tile
 }
 
 }  // namespace genga

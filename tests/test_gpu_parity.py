@@ -279,11 +279,18 @@ def test_step_fp32_conserves_like_paper_says():
 
 
 def _fp32_variants_to_gate():
-    """Every FP32 all-pairs variant whose arithmetic differs from the default's (the mass-scaled records) plus
-    variant 0; the autotuned choice is run on top of these (it is one of them, whichever the box prefers)."""
+    """Every FP32 all-pairs variant whose arithmetic differs from the default's (the mass-scaled records, the
+    symmetric kernels that evaluate every unordered pair once) plus variant 0; the autotuned choice is run on top
+    of these (it is one of them, whichever the box prefers)."""
     B.load()
     n = B.num_variants(0)
-    return [0] + [v for v in range(1, n) if "scaledtrue" in B.variant_name(0, v)]
+    return [0] + [v for v in range(1, n) if "scaledtrue" in B.variant_name(0, v) or "sym" in B.variant_name(0, v)]
+
+
+def _fp64_variants_to_gate():
+    """Variant 0 and the symmetric FP64 kernels (different summation structure: Newton's third law, register ring)."""
+    B.load()
+    return [0] + [v for v in range(1, B.num_variants(1)) if "sym" in B.variant_name(1, v)]
 
 
 def _gate32(tag, a, pairs, ao, po):
@@ -302,6 +309,10 @@ def test_full_size_c4_kick_both_precisions():
     assert rel_err(a64, ao).max() <= 1e-12
     a64t, p64t, _, _ = gpu_accel(w, B.FP64, autotune=True)
     assert rel_err(a64t, ao).max() <= 1e-12 and pair_set(p64t) == pair_set(po)
+    for v in _fp64_variants_to_gate()[1:]:
+        a, p, _, st = gpu_accel(w, B.FP64, variant=v)
+        assert rel_err(a, ao).max() <= 1e-12, (B.variant_name(1, v), rel_err(a, ao).max())
+        assert pair_set(p) == pair_set(po) and not st.overflowed, B.variant_name(1, v)
     a32, p32, _, st32 = gpu_accel(w, B.FP32, autotune=True)
     _gate32("autotuned", a32, p32, ao, po)
     for v in _fp32_variants_to_gate():
@@ -393,6 +404,10 @@ def test_full_size_configs_1_to_3_kick_both_precisions(cfg):
     assert np.max(np.abs(rc / rco - 1)) <= 1e-14
     assert rel_err(a64, ao).max() <= 1e-12
     assert pair_set(p64) == pair_set(po)
+    for v in _fp64_variants_to_gate()[1:]:
+        a, p, _, st = gpu_accel(w, B.FP64, variant=v)
+        assert rel_err(a, ao).max() <= 1e-12, (cfg, B.variant_name(1, v), rel_err(a, ao).max())
+        assert pair_set(p) == pair_set(po) and not st.overflowed, (cfg, B.variant_name(1, v))
     a32, p32, _, st32 = gpu_accel(w, B.FP32, autotune=True)
     _gate32(("autotuned", cfg), a32, p32, ao, po)
     for v in _fp32_variants_to_gate():
@@ -445,6 +460,7 @@ def test_sweep_maximum_size_131072_both_precisions():
     # default variants, the autotuned ones (what bench.py --sweep times) and every mass-scaled FP32 variant
     runs = [(B.FP64, dict()), (B.FP64, dict(autotune=True)), (B.FP32, dict()), (B.FP32, dict(autotune=True))]
     runs += [(B.FP32, dict(variant=v)) for v in _fp32_variants_to_gate()[1:]]
+    runs += [(B.FP64, dict(variant=v)) for v in _fp64_variants_to_gate()[1:]]
     for prec, how in runs:
         a, pairs, _, st = gpu_accel(w, prec, pair_capacity=1 << 20, **how)
         err = rel_err(a[sel], ao)
@@ -622,3 +638,44 @@ def test_fp32_self_term_with_heavy_bodies():
                 e = rel_err(a, ao)
                 assert np.median(e) <= 1e-5 and e.max() <= 1e-4, (w.name, v_, nmax, np.median(e), e.max())
                 assert pair_set(pairs) == pair_set(po), (w.name, v_, nmax)
+
+
+def test_symmetric_kernels_on_the_special_cases():
+    # the kernels that evaluate every unordered pair once (kick_sym_body.cuh), through the cases the row kernels are
+    # tested on: dense changeover zones, Eq. 1 as printed, candidate-list overflow, tiny systems, test particles and
+    # coincident bodies, heavy bodies, weight mode 1, any grid
+    sym32 = [v for v in range(B.num_variants(0)) if "sym" in B.variant_name(0, v)]
+    sym64 = [v for v in range(B.num_variants(1)) if "sym" in B.variant_name(1, v)]
+    assert sym32 and sym64
+    ring = clustered(7, 900)
+    eq1 = W.config(0, 1024)
+    tiny = W.config(0, 6); tiny.m[1] = 0.0; tiny.x[3] = tiny.x[2]
+    heavy = W.config(3, 1200); heavy.m[0] = 5 * 9.5e-4
+    cases = [(ring, dict(), dict()), (eq1, dict(n1=3.0, n2=0.4, pair_rule=B.PAIR_MAX), dict()),
+             (W.config(0, 1200), dict(), dict(cand_capacity=16)), (tiny, dict(), dict()), (W.config(0, 2), dict(), dict()),
+             (W.config(0, 65), dict(), dict()), (heavy, dict(), dict()), (ring, dict(weight_mode=1), dict()),
+             (W.config(4, 9000), dict(), dict())]
+    for w, okw, gkw in cases:
+        p = oparams(w, **okw)
+        vd = oracle.to_democratic(w.m, w.v, w.M_star)
+        ao = oracle.accel(w.m, w.x, vd, p)
+        po = oracle.encounter_pairs(w.m, w.x, vd, p)
+        scale = np.linalg.norm(ao, axis=1); scale[scale == 0] = 1.0
+        for key, prec, vs in ((0, B.FP32, sym32), (1, B.FP64, sym64)):
+            for v in vs:
+                for half_waves in (0, 1, 5):
+                    kw = dict(okw); kw.update(gkw); kw["pair_capacity"] = 2 * len(po) + 1024
+                    g = B.from_workload(w, **kw)
+                    g.set_tuning(key, v); g.set_tuning(2 + key, half_waves)
+                    g.accel(prec)
+                    a = g.get_accel().cpu().numpy()
+                    pairs = g.encounter_pairs()
+                    st = g.nearfield_stats()
+                    g.close()
+                    tag = (w.name, w.N, okw, gkw, B.variant_name(key, v), half_waves)
+                    assert np.all(np.isfinite(a)), tag
+                    err = np.linalg.norm(a - ao, axis=1) / scale
+                    exact = prec == B.FP64 or st.overflowed          # the overflow path is all-FP64
+                    assert err.max() <= (1e-12 if exact else 1e-4), (tag, err.max())
+                    assert pair_set(pairs) == pair_set(po), tag
+                    assert st.overflowed == ("cand_capacity" in gkw), tag
