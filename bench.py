@@ -39,6 +39,21 @@ PEAK_FP32_TFLOPS = SMS * 128 * 2 * SM_MAX_HZ / 1e12      # 74.45: 128 FP32 lanes
 PEAK_FP64_TFLOPS = SMS * 64 * 2 * SM_MAX_HZ / 1e12       # 37.22: 64 FP64 lanes/SM (DFMA probe confirms)
 
 
+def capture_traffic(variant_name, precision):
+    """DRAM bytes per launch of the all-pairs kernel from the committed ncu capture (profiles/kick_traffic.json, written
+    from `ncu --set full`: dram__bytes_read.sum + dram__bytes_write.sum).  None unless the capture is of the very
+    variant this run times."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "kick_traffic.json")) as f:
+            rec = json.load(f)
+        for e in rec["captures"]:
+            if e["precision"] == precision and e["variant"] == variant_name:
+                return e["dram_bytes_per_launch"], f"{e['capture']} (git {e['git']}, N = {e['N']})"
+    except Exception:
+        pass
+    return None, "no ncu capture of this kernel variant is committed (profiles/kick_traffic.json)"
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -61,6 +76,9 @@ def parse_args():
     ap.add_argument("--hybrid", action="store_true",
                     help="time the hybrid step instead (NEXT-1: weight_mode = 1, encounter_mode = 1, default listing and substeps)")
     ap.add_argument("--no-autotune", action="store_true", help="keep the default kernel variants (no start-up self-tuning)")
+    ap.add_argument("--no-tables", action="store_true",
+                    help="skip the per-config table (configs 0-3, full step counts) and the N sweep that a default run adds "
+                         "to its JSON line under 'configs' and 'sweep' (each row with its own clock record)")
     return ap.parse_args()
 
 
@@ -119,9 +137,14 @@ class ClockSampler:
             self._thr.join()
 
     def summary(self):
-        return {"sm_mhz": statistics.median(self.sm) if self.sm else None,
-                "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons),
-                "power_w_max": max(self.power) if self.power else None, "samples": len(self.sm)}
+        out = {"sm_mhz": statistics.median(self.sm) if self.sm else None,
+               "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons),
+               "power_w_max": max(self.power) if self.power else None, "samples": len(self.sm)}
+        # a row measured under a slowdown, or with the SM clock stuck well below max for no stated reason, does not count
+        bad = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"} & self.reasons
+        stuck = bool(self.sm) and self.sm_max and not self.reasons and out["sm_mhz"] < 0.85 * self.sm_max
+        out["rejected"] = bool(bad or stuck)
+        return out
 
 
 def make_workload(args, rank):
@@ -354,6 +377,10 @@ def run_cuda(args):
     p32 = per_prec("fp32", t32, FLOP_FP32, PEAK_FP32_TFLOPS)
     p64 = per_prec("fp64", t64, FLOP_FP64, PEAK_FP64_TFLOPS)
 
+    kname32 = "kick32_sym_kernel" if "sym" in p32["kernel_variant"] else "kick32_kernel"
+    kname64 = "kick64_sym_kernel" if "sym" in p64["kernel_variant"] else "kick64_kernel"
+    tr32 = capture_traffic(p32["kernel_variant"], "fp32")
+    tr64 = capture_traffic(p64["kernel_variant"], "fp64")
     line = {
         "metric": METRIC, "value": p32["pair_interactions_per_s"], "unit": UNIT, "n_gpus": world,
         "steps": K, "warmup": args.warmup, "ms_per_step": t32 / K, "higher_is_better": True,
@@ -366,18 +393,27 @@ def run_cuda(args):
                    **({"encounter_mode": 1, "note": "--hybrid: the opt-in hybrid step (NEXT-1), not the headline configuration"}
                       if args.hybrid else {})},
         "precisions": {"fp32": p32, "fp64": p64},
-        "roofline": {"bound": "alu", "kernel": "kick32_kernel", "achieved": p32["kick_kernel_tflops"],
+        "roofline": {"bound": "alu", "kernel": kname32, "achieved": p32["kick_kernel_tflops"],
                      "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s", "frac": p32["kick_kernel_frac_of_peak"],
-                     "traffic": 3.742e6,      # dram bytes read + written per kick32 launch (profiles/r1g, ncu --set full)
-                     "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md section 6); "
-                                    "MEASURED_PEAKS.json has no FP32/FP64 ALU figure",
+                     "traffic": tr32[0], "traffic_source": tr32[1],
+                     "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md section 7); "
+                                    "MEASURED_PEAKS.json has no FP32/FP64 ALU figure.  'frac' (the headline) divides by this "
+                                    "derived peak; 'frac_of_measured' by the FFMA2 / DFMA rate the in-library probe reached "
+                                    "in this very run ('peak_measured')",
                      "flop_per_pair": FLOP_FP32,
-                     "fp64": {"kernel": "kick64_kernel", "traffic": 3.111e6, "achieved": p64["kick_kernel_tflops"],
+                     "convention": "achieved = 18 (25) flop x N (N - 1) ordered pairs / kernel time: the flops of the plain "
+                                   "per-ordered-pair sequence (SURVEY.md 8(d)).  The symmetric kernels evaluate each unordered "
+                                   "pair once (16 FP32 / 20 FP64 operations for both directions), so they execute fewer "
+                                   "flops than this convention counts; the time is what is measured",
+                     "fp64": {"kernel": kname64, "traffic": tr64[0], "traffic_source": tr64[1],
+                              "achieved": p64["kick_kernel_tflops"],
                               "peak": PEAK_FP64_TFLOPS, "frac": p64["kick_kernel_frac_of_peak"],
                               "flop_per_pair": FLOP_FP64}},
         "e2e": {"value": whole_job_rate(world, pairs, e2e_steps, te32), "unit": UNIT,
                 "h2d_bytes_per_step": e2e["fp32"][1], "d2h_bytes_per_step": e2e["fp32"][2], "steps": e2e_steps,
-                "fp64_value": whole_job_rate(world, pairs, e2e_steps, te64)},
+                "fp64_value": whole_job_rate(world, pairs, e2e_steps, te64),
+                "ms_per_step": te32 / e2e_steps, "device_ms_per_step": t32 / K,
+                "e2e_over_device": (te32 / e2e_steps) / (t32 / K)},
         "gpu_launches": res["fp32"]["launches"],
         "clocks": sampler.summary(),
     }
@@ -411,8 +447,9 @@ def cpu_oracle_kick(w, **kw):
     return dt, pairs / dt, oracle.num_threads()
 
 
-def run_sweep(args):
-    """N = 2^10 .. 2^17 (BASELINE.json configs[4]): N x steps/s per precision, device-timed."""
+def run_sweep(args, cpu=True):
+    """N = 2^10 .. 2^17 (BASELINE.json configs[4]): N x steps/s per precision, device-timed; every row carries the
+    clock record sampled while it ran (a row with 'rejected' does not count)."""
     import torch
     from paper_2309_08217_b200 import binding as B
     from paper_2309_08217_b200 import workloads as W
@@ -421,20 +458,72 @@ def run_sweep(args):
         w = W.config(4, n)
         row = {"N": n}
         steps = 200 if n <= 32768 else 20
-        for prec, name in ((B.FP32, "fp32"), (B.FP64, "fp64")):
-            g = B.from_workload(w)
-            if not args.no_autotune:
-                g.autotune(prec)
-            r = time_steps(torch, g, w, prec, steps, 3, None, None, profile_timed=False)
-            row[name] = {"ms_per_step": r["total_ms"] / steps, "body_steps_per_s": n * steps / (r["total_ms"] * 1e-3),
-                         "pair_interactions_per_s": n * (n - 1.0) * steps / (r["total_ms"] * 1e-3),
-                         "kick_kernel_ms": r["kernel_ms"][0], "nearfield_ms": r["kernel_ms"][1]}
-            g.close()
-        if not args.no_cpu_baseline:
+        pairs = n * (n - 1.0)
+        sampler = ClockSampler(torch.cuda.current_device())
+        with sampler:
+            for prec, name, flop, peak in ((B.FP32, "fp32", FLOP_FP32, PEAK_FP32_TFLOPS), (B.FP64, "fp64", FLOP_FP64, PEAK_FP64_TFLOPS)):
+                g = B.from_workload(w)
+                variant = 0 if args.no_autotune else g.autotune(prec)[0]
+                r = time_steps(torch, g, w, prec, steps, 3, None, None, profile_timed=False)
+                row[name] = {"ms_per_step": r["total_ms"] / steps, "body_steps_per_s": n * steps / (r["total_ms"] * 1e-3),
+                             "pair_interactions_per_s": pairs * steps / (r["total_ms"] * 1e-3),
+                             "step_frac_of_peak": flop * pairs * steps / (r["total_ms"] * 1e-3) / 1e12 / peak,
+                             "kick_kernel_ms": r["kernel_ms"][0], "nearfield_ms": r["kernel_ms"][1],
+                             "kick_kernel_frac_of_peak": flop * pairs / (r["kernel_ms"][0] * 1e-3) / 1e12 / peak,
+                             "launches_per_step": r["launches"] / steps,
+                             "kernel_variant": B.variant_name(0 if prec == B.FP32 else 1, variant)}
+                g.close()
+        row["clocks"] = sampler.summary()
+        if cpu and not args.no_cpu_baseline:
             sec, pps, thr = cpu_oracle_kick(w)
             row["cpu_oracle_kick"] = {"seconds": sec, "pair_interactions_per_s": pps, "cores": thr}
         out.append(row)
     return out
+
+
+def run_configs_table(args):
+    """north_star: 'report ... at each config'.  BASELINE.json configs 0-3 at their full sizes and step counts (config 4 is
+    the headline measurement itself), both precisions, each row with its own clock record: ms per step, rates, fraction
+    of peak of the whole step, dE/E and dL/L over the run, encounter pairs of the last evaluation."""
+    import numpy as np
+    import torch
+    from paper_2309_08217_b200 import binding as B
+    from paper_2309_08217_b200 import workloads as W
+    rows = []
+    for cfg in (0, 1, 2, 3):
+        w = W.config(cfg)
+        pairs = w.N * (w.N - 1.0)
+        sampler = ClockSampler(torch.cuda.current_device())
+        row = {"config": cfg, "workload": w.name, "N": w.N, "dt_days": w.dt, "steps": w.nsteps}
+        with sampler:
+            for prec, name, flop, peak in ((B.FP32, "fp32", FLOP_FP32, PEAK_FP32_TFLOPS), (B.FP64, "fp64", FLOP_FP64, PEAK_FP64_TFLOPS)):
+                g = B.from_workload(w)
+                variant = 0 if args.no_autotune else g.autotune(prec)[0]
+                g.run(w.dt, 3, prec)                               # warm-up
+                g.close()
+                g = B.from_workload(w)
+                g.set_tuning(0 if prec == B.FP32 else 1, variant)
+                E0, L0 = g.energy_angmom()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record()
+                g.run(w.dt, w.nsteps, prec)                        # K(dt/2) [S D S K(dt)]^(n-1) S D S K(dt/2)
+                e1.record()
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1)
+                E1, L1 = g.energy_angmom()
+                enc = int(len(g.encounter_pairs(cap=8 * w.N + 4096)))
+                g.close()
+                evals = w.nsteps + 1
+                row[name] = {"ms_per_step": ms / w.nsteps, "body_steps_per_s": w.N * w.nsteps / (ms * 1e-3),
+                             "pair_interactions_per_s": pairs * evals / (ms * 1e-3),
+                             "step_frac_of_peak": flop * pairs * evals / (ms * 1e-3) / 1e12 / peak,
+                             "dE_over_E": E1 / E0 - 1.0, "dL_over_L": float(np.linalg.norm(L1) / np.linalg.norm(L0) - 1.0),
+                             "encounter_pairs_last_eval": enc,
+                             "kernel_variant": B.variant_name(0 if prec == B.FP32 else 1, variant)}
+        row["clocks"] = sampler.summary()
+        rows.append(row)
+    return rows
 
 
 def run_report(args):
@@ -478,10 +567,12 @@ def run_report(args):
             g.set_tuning(0 if prec == B.FP32 else 1, variant)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize()
-            e0.record()
-            g.run(w.dt, w.nsteps, prec)                            # K(dt/2) [S D S K(dt)]^(n-1) S D S K(dt/2)
-            e1.record()
-            torch.cuda.synchronize()
+            sampler = ClockSampler(torch.cuda.current_device())
+            with sampler:                                          # every row carries its own clock record
+                e0.record()
+                g.run(w.dt, w.nsteps, prec)                        # K(dt/2) [S D S K(dt)]^(n-1) S D S K(dt/2)
+                e1.record()
+                torch.cuda.synchronize()
             ms = e0.elapsed_time(e1)
             E1, L1 = g.energy_angmom()
             enc_last = int(len(g.encounter_pairs(cap=max(8 * w.N + 4096, kw.get("pair_capacity", 0)))))
@@ -498,7 +589,8 @@ def run_report(args):
                     "step_frac_of_peak": flop * pairs * evals / (ms * 1e-3) / 1e12 / peak,
                     "dE_over_E": E1 / E0 - 1.0,
                     "dL_over_L": float(np.linalg.norm(L1) / np.linalg.norm(L0) - 1.0),
-                    "encounter_pairs_last_eval": enc_last, "nearfield_candidates_last_eval": st.candidates}
+                    "encounter_pairs_last_eval": enc_last, "nearfield_candidates_last_eval": st.candidates,
+                    "clocks": sampler.summary()}
             if enc_stats is not None:
                 line["encounter_groups_last_drift"] = {"groups": enc_stats[0], "bodies": enc_stats[1], "largest": enc_stats[2],
                                                        "missed_pairs_whole_run": enc_stats[3], "status": enc_stats[4], "rk4_substeps": kw.get("enc_nsub"),
@@ -597,14 +689,21 @@ def main():
         return
     line, w = got
     line["alu_probe"] = alu_probes()
+    rf = line["roofline"]
+    rf["peak_measured"] = line["alu_probe"]["ffma2_tflops"]
+    rf["frac_of_measured"] = rf["achieved"] / rf["peak_measured"]
+    rf["fp64"]["peak_measured"] = line["alu_probe"]["dfma_tflops"]
+    rf["fp64"]["frac_of_measured"] = rf["fp64"]["achieved"] / rf["fp64"]["peak_measured"]
     if line["n_gpus"] == 1 and not args.no_cpu_baseline:
         times, threads = cpu_oracle_steps(w, 4)          # ~10-20 s of host time at N = 40 000
         pairs = w.N * (w.N - 1.0)
         line["cpu_baseline"] = {"value": pairs * len(times) / sum(times), "unit": UNIT, "cores": threads,
                                 "kind": "oracle", "sample": f"{len(times)} full merged-leapfrog steps of the "
                                 f"N={w.N} workload ({sum(times):.1f} s of host time)"}
-    if args.sweep and line["n_gpus"] == 1:
-        line["sweep"] = run_sweep(args)
+    if line["n_gpus"] == 1 and (args.sweep or not args.no_tables):
+        line["sweep"] = run_sweep(args, cpu=args.sweep)           # --sweep: with the oracle's kick timed beside each N
+    if line["n_gpus"] == 1 and not args.no_tables:
+        line["configs"] = run_configs_table(args)
     print(json.dumps(line), flush=True)
     import torch.distributed as dist
     if dist.is_available() and dist.is_initialized():

@@ -264,9 +264,9 @@ const char* genga_version(void);
 
 /* ALU peak probes: run a register-only dependent-chain kernel on every SM
  * for iters iterations and return achieved instr throughput.  which: 0 FFMA, 1 FFMA2 (packed),
- * 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H, 5 the FP32 pair loop of the kick on its own (6: without MUFU,
- * 7: without the min; these three report PAIRS per second).  *ops_per_s (HOST) = lane-operations
- * per second (an FFMA2 counts 2).  stream as in params.  Synchronises.                                     */
+ * 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H (anything else: GENGA_EINVAL).  *ops_per_s (HOST) = lane-operations
+ * per second (an FFMA2 counts 2).  stream as in params.  Synchronises.  bench.py prints these beside the
+ * derived peaks its roofline fractions are quoted against.                                              */
 int genga_peak_probe(int which, int iters, void* stream, double* ops_per_s, double* ms);
 
 #ifdef __cplusplus
