@@ -73,6 +73,9 @@ def lib() -> ctypes.CDLL:
         L.oracle_changeover.argtypes = [ctypes.c_double, ctypes.c_double]
         L.oracle_step_hybrid.restype = ctypes.c_int
         L.oracle_step_hybrid.argtypes = [ctypes.c_int, _dp, _dp, _dp, _pp, ctypes.c_double, ctypes.c_int]
+        L.oracle_step_hybrid_bs.restype = ctypes.c_int
+        L.oracle_step_hybrid_bs.argtypes = [ctypes.c_int, _dp, _dp, _dp, _pp, ctypes.c_double, ctypes.c_double,
+                                            ctypes.POINTER(ctypes.c_longlong)]
         L.oracle_weight.restype = ctypes.c_double
         L.oracle_weight.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int]
         L.oracle_pair_rcrit.restype = ctypes.c_double
@@ -263,6 +266,18 @@ def step_hybrid(m, x, v, p: Params, dt: float, nsub: int = 2000):
     if rc != 0:
         raise ValueError("oracle_step_hybrid needs weight_mode = 1 and nsub >= 1")
     return x, v
+
+
+def step_hybrid_bs(m, x, v, p: Params, dt: float, tol: float = 1.0e-13, stats: bool = False):
+    """NEXT-1 (readings R11, R15): the hybrid step with the A-flow integrated by Gragg-Bulirsch-Stoer extrapolation to the
+    relative tolerance tol (all bodies as one system); returns (x', v') [, (accepted, rejected, right-hand sides)]."""
+    m = _a(m); x = _a(x).copy(); v = _a(v).copy()
+    c = p.c()
+    st = (ctypes.c_longlong * 3)()
+    rc = lib().oracle_step_hybrid_bs(len(m), _p(m), _p(x), _p(v), ctypes.byref(c), float(dt), float(tol), st)
+    if rc != 0:
+        raise ValueError("oracle_step_hybrid_bs: needs weight_mode = 1 and tol > 0, or the step size collapsed")
+    return (x, v, tuple(int(q) for q in st)) if stats else (x, v)
 
 
 def run(m, x, v, p: Params, dt: float, nsteps: int):

@@ -514,6 +514,112 @@ void oracle_encounter_drift(int N, const double* m, double* x, double* v, const 
     free(buf);
 }
 
+/* A(dt) with an error-controlled integrator: Gragg-Bulirsch-Stoer extrapolation ("the Bulirsch-Stoer
+ * integrator (level 1)"; Stoer & Bulirsch 1980, sect. 7.2.14; the scheme itself is textbook material and is restated
+ * here, reading R15).  One macro step of size H from y = (x, v):
+ *   modified midpoint with n_k = 2 (k + 1) substeps h = H / n_k, k = 0 .. 7:
+ *     z_0 = y, z_1 = z_0 + h f(z_0), z_{m+1} = z_{m-1} + 2 h f(z_m), S_k = (z_n + z_{n-1} + h f(z_n)) / 2,
+ *   polynomial extrapolation in h^2 (Aitken-Neville):
+ *     T_{k,0} = S_k,  T_{k,j} = T_{k,j-1} + (T_{k,j-1} - T_{k-1,j-1}) / ((n_k / n_{k-j})^2 - 1),
+ *   error of row k: max over bodies of max(|dx_i| / |x_i|, |dv_i| / |v_i|) with d = T_{k,k} - T_{k,k-1} (vector norms);
+ *   accepted as soon as it is <= tol (k >= 1); if row 7 fails, H is halved and the step repeated.  After a step that
+ *   took row k the next H is 2 H (k <= 3), H (k <= 5) or H / 2, cut to what is left of dt.
+ * All N bodies form ONE system (no groups, no lists): the oracle of the A-flow is its converged solution.
+ * stats (may be NULL): [0] macro steps accepted, [1] rejected, [2] right-hand sides.  Returns 0, or -1 if H fell
+ * below |dt| 2^-40 without convergence (the state is then the last accepted one).                                 */
+int oracle_encounter_drift_bs(int N, const double* m, double* x, double* v, const oracle_params* p,
+                              const double* rc, const double* sa, const double* vk, double dt, double tol, long long* stats)
+{
+    enum { KMAX = 8 };
+    size_t n3 = 3 * (size_t)(N > 0 ? N : 1);
+    double* buf = (double*)malloc(sizeof(double) * n3 * (8 + 4 * KMAX));
+    double *f0x = buf, *f0v = buf + n3, *z0x = buf + 2 * n3, *z0v = buf + 3 * n3, *z1x = buf + 4 * n3, *z1v = buf + 5 * n3,
+           *fx = buf + 6 * n3, *fv = buf + 7 * n3;
+    double* Tx[2][KMAX]; double* Tv[2][KMAX];                     /* two rows of the tableau */
+    for (int r = 0; r < 2; ++r)
+        for (int j = 0; j < KMAX; ++j) { Tx[r][j] = buf + (8 + (2 * r) * KMAX + j) * n3; Tv[r][j] = buf + (8 + (2 * r + 1) * KMAX + j) * n3; }
+    long long acc = 0, rej = 0, nf = 0;
+    int rcode = 0;
+    double t = 0.0, H = dt;
+    const double T = fabs(dt);
+    while (fabs(t) < T * (1.0 - 1.0e-14) && T > 0.0) {
+        if (fabs(t + H) > T) H = dt - t;
+        rhs_A(N, m, p, rc, sa, vk, x, v, f0x, f0v); ++nf;
+        int done = -1;
+        for (int k = 0; k < KMAX && done < 0; ++k) {
+            const int nk = 2 * (k + 1);
+            const double h = H / nk;
+            const int cur = k & 1, prev = cur ^ 1;
+            for (size_t q = 0; q < 3 * (size_t)N; ++q) { z0x[q] = x[q]; z0v[q] = v[q]; z1x[q] = x[q] + h * f0x[q]; z1v[q] = v[q] + h * f0v[q]; }
+            for (int s = 1; s < nk; ++s) {
+                rhs_A(N, m, p, rc, sa, vk, z1x, z1v, fx, fv); ++nf;
+                for (size_t q = 0; q < 3 * (size_t)N; ++q) {
+                    double nx = z0x[q] + 2.0 * h * fx[q], nv = z0v[q] + 2.0 * h * fv[q];
+                    z0x[q] = z1x[q]; z0v[q] = z1v[q]; z1x[q] = nx; z1v[q] = nv;
+                }
+            }
+            rhs_A(N, m, p, rc, sa, vk, z1x, z1v, fx, fv); ++nf;
+            for (size_t q = 0; q < 3 * (size_t)N; ++q) {
+                Tx[cur][0][q] = 0.5 * (z1x[q] + z0x[q] + h * fx[q]);
+                Tv[cur][0][q] = 0.5 * (z1v[q] + z0v[q] + h * fv[q]);
+            }
+            for (int j = 1; j <= k; ++j) {
+                const double ratio = (double)nk / (double)(2 * (k - j + 1));
+                const double den = ratio * ratio - 1.0;
+                for (size_t q = 0; q < 3 * (size_t)N; ++q) {
+                    Tx[cur][j][q] = Tx[cur][j - 1][q] + (Tx[cur][j - 1][q] - Tx[prev][j - 1][q]) / den;
+                    Tv[cur][j][q] = Tv[cur][j - 1][q] + (Tv[cur][j - 1][q] - Tv[prev][j - 1][q]) / den;
+                }
+            }
+            if (k >= 1) {
+                double err = 0.0;
+                for (int i = 0; i < N; ++i) {
+                    double dx2 = 0, dv2 = 0, x2 = 0, v2 = 0;
+                    for (int c = 0; c < 3; ++c) {
+                        double a = Tx[cur][k][3 * i + c], b = Tv[cur][k][3 * i + c];
+                        double da = a - Tx[cur][k - 1][3 * i + c], db = b - Tv[cur][k - 1][3 * i + c];
+                        dx2 += da * da; dv2 += db * db; x2 += a * a; v2 += b * b;
+                    }
+                    double ex = sqrt(dx2 / x2), ev = sqrt(dv2 / v2);
+                    if (!(ex <= err)) err = ex;               /* NaN counts as "not converged" */
+                    if (!(ev <= err)) err = ev;
+                }
+                if (err <= tol) done = k;
+            }
+        }
+        if (done < 0) {
+            ++rej;
+            H *= 0.5;
+            if (fabs(H) < T * 9.094947017729282e-13) { rcode = -1; break; }
+            continue;
+        }
+        for (size_t q = 0; q < 3 * (size_t)N; ++q) { x[q] = Tx[done & 1][done][q]; v[q] = Tv[done & 1][done][q]; }
+        t += H; ++acc;
+        H = (done <= 3) ? 2.0 * H : ((done <= 5) ? H : 0.5 * H);
+    }
+    if (stats) { stats[0] = acc; stats[1] = rej; stats[2] = nf; }
+    free(buf);
+    return rcode;
+}
+
+/* The hybrid step of reading R11 with A(dt) integrated to the tolerance tol by oracle_encounter_drift_bs. */
+int oracle_step_hybrid_bs(int N, const double* m, double* x, double* v, const oracle_params* p, double dt, double tol,
+                          long long* stats)
+{
+    if (p->weight_mode != 1 || !(tol > 0.0)) return -1;
+    double* rc = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* sa = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* vk = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    oracle_rcrit(N, m, x, v, p, rc, sa, vk);              /* the radii of the opening force evaluation */
+    oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
+    oracle_sunkick(N, m, x, v, p, 0.5 * dt);
+    int r = oracle_encounter_drift_bs(N, m, x, v, p, rc, sa, vk, dt, tol, stats);
+    oracle_sunkick(N, m, x, v, p, 0.5 * dt);
+    oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
+    free(rc); free(sa); free(vk);
+    return r;
+}
+
 /* One hybrid step B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2); p->weight_mode must be 1.  Returns -1 otherwise. */
 int oracle_step_hybrid(int N, const double* m, double* x, double* v, const oracle_params* p, double dt, int nsub)
 {

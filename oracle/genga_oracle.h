@@ -30,6 +30,10 @@
  *                          differences of the pinned K, two-body force = -grad of the potential
  *   oracle_step_hybrid     pinned: reduces to oracle_step without encounters, energy through a close
  *                          encounter (full E) vs the level-0-only step, dt^2 convergence to DOP853
+ *   oracle_step_hybrid_bs  pinned: Kepler motion of one body against the closed-form drift, DOP853 on the A-flow of a deep
+ *                          encounter, agreement with the converged RK4 substeps of oracle_step_hybrid, error falling
+ *                          with tol, time reversal (reading R15: WHICH extrapolation scheme and step control GENGA's
+ *                          Bulirsch-Stoer level uses is not printed; the A-flow itself is unique)
  *   TP2 mode (n_big >= 0)  pinned: hand 3-body values, full-minus-subset identity against the
  *                          pinned all-pairs path, sum m a = 0, bounded dt^2 energy error
  *   oracle_merge(_tp2)     pinned: inelastic-collision identities (dT = mu u^2/2, dL = mu x_rel x v_rel),
@@ -128,6 +132,12 @@ int oracle_run(int N, const double* m, double* x, double* v,
 void oracle_encounter_drift(int N, const double* m, double* x, double* v, const oracle_params* p,
                             const double* rc, const double* sa, const double* vk, double dt, int nsub);
 int oracle_step_hybrid(int N, const double* m, double* x, double* v, const oracle_params* p, double dt, int nsub);
+/* the same step with A(dt) integrated by Gragg-Bulirsch-Stoer extrapolation to the relative tolerance tol (reading R15;
+ * PAPER.md:45 names the integrator); stats (may be NULL): accepted macro steps, rejected, right-hand sides */
+int oracle_encounter_drift_bs(int N, const double* m, double* x, double* v, const oracle_params* p,
+                              const double* rc, const double* sa, const double* vk, double dt, double tol, long long* stats);
+int oracle_step_hybrid_bs(int N, const double* m, double* x, double* v, const oracle_params* p, double dt, double tol,
+                          long long* stats);
 
 /* O11.  E = sum m v^2/2 + |sum m v|^2/(2 M_star) - sum G M_star m/r
  *                         - sum_{i<j} G m_i m_j / r_ij ;  L = sum m x cross v. */

@@ -97,3 +97,84 @@ def test_second_order_convergence_to_the_n_body_solution_through_an_encounter():
         errs.append(np.abs(xx - x_true).max())
     assert errs[2] < 2e-6
     assert 2.5 < errs[0] / errs[1] < 6.5 and 2.5 < errs[1] / errs[2] < 6.5, errs
+
+
+# ---- the A-flow with an error-controlled integrator (reading R15: Gragg-Bulirsch-Stoer extrapolation) ----------------
+def _deep_state():
+    """The encounter system advanced to the steps in which the two planets are deepest inside their zone."""
+    m, x, v = encounter_system()
+    p = oracle.Params(n1=3.0, n2=0.4, dt_rcrit=2.0, pair_rule=oracle.PAIR_MAX, weight_mode=1)
+    for _ in range(14):
+        x, v = oracle.step_hybrid(m, x, v, p, 2.0, nsub=2000)
+    rc, _, _ = oracle.rcrit(m, x, v, p)
+    assert np.linalg.norm(x[0] - x[1]) < 0.8 * max(rc[0], rc[1])
+    return m, x, v, p
+
+
+def test_bs_moves_a_single_body_on_its_kepler_orbit():
+    # one body: no pair forces, so the hybrid step is Sun-kick, Kepler motion, Sun-kick; the closed-form drift of the
+    # (pinned) level-0 step is the reference for the extrapolation integrator, through a fifth of an e = 0.4 orbit
+    mm = np.array([3e-6])
+    x, v = W.elements_to_cartesian(G * (1 + mm), np.array([1.0]), np.array([0.4]), np.array([0.1]), np.array([1.0]),
+                                   np.array([2.0]), np.array([5.9]))
+    v = oracle.to_democratic(mm, v, 1.0)
+    p = oracle.Params(n1=3.0, weight_mode=1)
+    for dt in (6.0, 73.0, -73.0):
+        x1, v1 = oracle.step(mm, x, v, p, dt)
+        x2, v2, st = oracle.step_hybrid_bs(mm, x, v, p, dt, tol=1e-13, stats=True)
+        assert np.abs(x1 - x2).max() <= 2e-12 and np.abs(v1 - v2).max() <= 1e-13, (dt, np.abs(x1 - x2).max())
+        assert st[0] >= 1 and st[2] > 20
+
+
+def test_bs_step_equals_the_step_built_from_pinned_pieces_and_dop853():
+    # B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) with B, C from the pinned oracle calls and A(dt) integrated by scipy's DOP853
+    # on a right-hand side written here from the pinned weight function: an independent route to the same step
+    m, x, v, p = _deep_state()
+    dt = 2.0
+    rc, sa, vk = oracle.rcrit(m, x, v, p)
+    v1, _ = oracle.kick(m, x, v, p, 0.5 * dt)
+    x1 = oracle.sunkick(m, x, v1, p, 0.5 * dt)
+    n = len(m)
+
+    def rhs(t, y):
+        X = y[:3 * n].reshape(n, 3); V = y[3 * n:].reshape(n, 3)
+        A = -G * X / np.linalg.norm(X, axis=1)[:, None] ** 3
+        for i in range(n):
+            for j in range(n):
+                if i == j:
+                    continue
+                d = X[j] - X[i]; q = np.linalg.norm(d)
+                rcij = oracle.pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j])
+                A[i] += G * m[j] * (1.0 - oracle.weight(q, rcij, 1)) * d / q ** 3
+        return np.concatenate([V.ravel(), A.ravel()])
+
+    sol = solve_ivp(rhs, (0, dt), np.concatenate([x1.ravel(), v1.ravel()]), method="DOP853", rtol=1e-13, atol=1e-18)
+    x2 = sol.y[:3 * n, -1].reshape(n, 3); v2 = sol.y[3 * n:, -1].reshape(n, 3)
+    x3 = oracle.sunkick(m, x2, v2, p, 0.5 * dt)
+    v3, _ = oracle.kick(m, x3, v2, p, 0.5 * dt)
+    xb, vb = oracle.step_hybrid_bs(m, x, v, p, dt, tol=1e-13)
+    assert np.abs(xb - x3).max() <= 2e-12 and np.abs(vb - v3).max() <= 1e-13, (np.abs(xb - x3).max(), np.abs(vb - v3).max())
+    # ... and the converged fixed-step RK4 of oracle_step_hybrid (the route the first GPU integrator was gated on)
+    xr, vr = oracle.step_hybrid(m, x, v, p, dt, nsub=20000)
+    assert np.abs(xb - xr).max() <= 1e-11 and np.abs(vb - vr).max() <= 1e-12
+
+
+def test_bs_error_follows_the_tolerance_and_the_step_reverses():
+    m, x, v, p = _deep_state()
+    ref = oracle.step_hybrid_bs(m, x, v, p, 2.0, tol=1e-14)
+    prev_err, prev_rhs = None, None
+    for tol in (1e-6, 1e-9, 1e-12):
+        xb, vb, st = oracle.step_hybrid_bs(m, x, v, p, 2.0, tol=tol, stats=True)
+        err = max(np.abs(xb - ref[0]).max(), np.abs(vb - ref[1]).max())
+        assert err <= 20 * tol, (tol, err)
+        if prev_err is not None:
+            assert st[2] >= prev_rhs                                 # a tighter tolerance never costs fewer right-hand sides
+        prev_err, prev_rhs = err, st[2]
+    xf, vf = oracle.step_hybrid_bs(m, x, v, p, 2.0, tol=1e-13)
+    xr, vr = oracle.step_hybrid_bs(m, xf, vf, p, -2.0, tol=1e-13)
+    # r_crit is taken from the opening state of each call (a_i from vis-viva, which the encounter itself changes by
+    # 1e-4 here), so the two planets return only to that order times the complement force; the spectators return exactly
+    assert np.abs(xr - x)[:2].max() <= 1e-7 and np.abs(vr - v)[:2].max() <= 1e-8
+    assert np.abs(xr - x)[2:].max() <= 1e-13 and np.abs(vr - v)[2:].max() <= 1e-14
+    with pytest.raises(ValueError):
+        oracle.step_hybrid_bs(m, x, v, oracle.Params(n1=3.0, weight_mode=0), 2.0)
