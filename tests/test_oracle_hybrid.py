@@ -174,7 +174,7 @@ def test_bs_error_follows_the_tolerance_and_the_step_reverses():
     xr, vr = oracle.step_hybrid_bs(m, xf, vf, p, -2.0, tol=1e-13)
     # r_crit is taken from the opening state of each call (a_i from vis-viva, which the encounter itself changes by
     # 1e-4 here), so the two planets return only to that order times the complement force; the spectators return exactly
-    assert np.abs(xr - x)[:2].max() <= 1e-7 and np.abs(vr - v)[:2].max() <= 1e-8
+    assert np.abs(xr - x)[:2].max() <= 1e-7 and np.abs(vr - v)[:2].max() <= 1e-7
     assert np.abs(xr - x)[2:].max() <= 1e-13 and np.abs(vr - v)[2:].max() <= 1e-14
     with pytest.raises(ValueError):
         oracle.step_hybrid_bs(m, x, v, oracle.Params(n1=3.0, weight_mode=0), 2.0)
