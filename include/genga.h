@@ -111,10 +111,13 @@ typedef struct {
                                  1: the hybrid symplectic step: the bodies of an
                                  encounter GROUP (connected component of the encounter-pair list of the step's
                                  opening force evaluation) are advanced over dt under their Kepler terms plus the
-                                 complement pair forces G m_j (1 - (K - r dK/dr)) / r^2, in FP64, by enc_nsub
-                                 classical RK4 substeps, r_crit,ij held at the opening evaluation's values.
+                                 complement pair forces G m_j (1 - (K - r dK/dr)) / r^2, in FP64, by Bulirsch-Stoer
+                                 extrapolation to enc_tol (or enc_nsub RK4 substeps), r_crit,ij held at the opening
+                                 evaluation's values.  Groups of up to 16 bodies take a warp, up to 256 a CTA; larger
+                                 ones are dissolved (their bodies drift on Kepler orbits) and reported (status bit 2).
                                  Requires weight_mode = 1, n_big < 0 and the cooperative per-body kernel.    */
-    int    enc_nsub;          /* RK4 substeps per step for the bodies of a group (at least; see enc_eta); <= 0: default (256) */
+    int    enc_nsub;          /* > 0: the groups are integrated with classical RK4, enc_nsub equal substeps per step (the scheme of
+                                 oracle_step_hybrid); <= 0 (default): Gragg-Bulirsch-Stoer extrapolation to enc_tol            */
     double enc_list_scale;    /* encounter mode: which pairs OUTSIDE their zone are listed (and grouped) as well, so that
                                  a pair that enters its zone DURING the step is already in a group: those with
                                  r_ij < enc_list_scale * r_crit,ij  and  r_ij - r_crit,ij < enc_list_vfactor * dt * |v_i - v_j|
@@ -124,11 +127,10 @@ typedef struct {
                                  un-grouped all the same are counted (genga_encounter_stats).                       */
     double enc_list_vfactor;  /* see enc_list_scale.  0: default (1.25); < 0: no velocity test, every pair inside
                                  enc_list_scale * r_crit,ij is listed.                                               */
-    double enc_eta;           /* encounter mode: <= 0 (default): fixed substeps dt / enc_nsub, the oracle's scheme.  > 0:
-                                 adaptive substeps min(dt / enc_nsub, enc_eta * tau), tau = the shortest
-                                 r_ij / (|v_i - v_j| + sqrt(2 G (m_i + m_j) / r_ij)) over the group's pairs that are inside
-                                 their zone, never below dt / (256 enc_nsub) (status bit 8 of genga_encounter_stats if
-                                 that floor was hit).  Costs about 15 % of the group integration; 0.02 is a sensible value. */
+    double enc_tol;           /* encounter mode, enc_nsub <= 0: relative tolerance of the Bulirsch-Stoer integration of the groups
+                                 (reading R15): a macro step is accepted when the last extrapolation
+                                 correction of every member is below enc_tol in |dx|/|x| and |dv|/|v|; <= 0: default 1e-12.
+                                 genga_encounter_stats status bit 8: the step size collapsed (dt 2^-30) without convergence  */
 } genga_params;
 
 /* Fill *p with the defaults: G = k^2 (k = 0.01720209895), M_star = 1, n1 = 3, n2 = 0,

@@ -189,7 +189,8 @@ static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_d
     a.enc.on = enc ? 1 : 0; a.enc.nsub = h->p.enc_nsub; a.enc.pair_rule = h->p.pair_rule;
     a.enc.pair_cap = (unsigned int)h->pair_cap;
     a.enc.G = h->p.G; a.enc.M_star = h->p.M_star; a.enc.n1 = h->p.n1; a.enc.n2dt = h->p.n2 * h->p.dt_rcrit;
-    a.enc.eta = h->p.enc_eta;
+    a.enc.tol = h->p.enc_tol;
+    a.enc.maxgroups = (int)std::min((size_t)h->pair_cap, (size_t)h->NP / 2);
     cudaError_t e;
     if (enc) {                                         // groups of the pair list the last force evaluation left
         if (!h->pairs_current) {                       // no list of the current positions (first call after create /
@@ -349,7 +350,7 @@ void genga_default_params(genga_params* p)
     p->chunk = 0;
     p->mega_nmax = 0;
     p->weight_mode = 0;
-    p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0; p->enc_list_vfactor = 0.0; p->enc_eta = 0.0;
+    p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0; p->enc_list_vfactor = 0.0; p->enc_tol = 0.0;
 }
 
 size_t genga_workspace_bytes(int N, const genga_params* p)
@@ -405,11 +406,11 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
         if (p->encounter_mode == 1) {
             if (!coop) { delete h; return GENGA_EINVAL; }
             h->enc_blocks = onbody_max_blocks(h, true);
-            h->p.enc_nsub = p->enc_nsub > 0 ? p->enc_nsub : 256;
+            h->p.enc_nsub = p->enc_nsub > 0 ? p->enc_nsub : 0;                 // 0: Bulirsch-Stoer to enc_tol
             h->p.enc_list_scale = p->enc_list_scale > 0.0 ? p->enc_list_scale : 8.0;
             h->p.enc_list_vfactor = p->enc_list_vfactor == 0.0 ? 1.25 : p->enc_list_vfactor;
             h->enc_dt = std::fabs(p->dt_rcrit);
-            h->p.enc_eta = p->enc_eta;
+            h->p.enc_tol = p->enc_tol > 0.0 ? p->enc_tol : 1.0e-12;
             if (h->p.enc_list_scale < 1.0 || h->p.enc_list_scale > 8.0) { delete h; return GENGA_EINVAL; }
         }
         h->mega_blocks[0] = h->mega_blocks[1] = -1;

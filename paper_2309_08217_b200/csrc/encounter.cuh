@@ -1,14 +1,24 @@
-// encounter.cuh -- NEXT-1 (reading R11), opt-in (params.encounter_mode = 1): the
+// encounter.cuh -- NEXT-1 (readings R11, R15), opt-in (params.encounter_mode = 1): the
 // encounter complement of the hybrid symplectic step.  PAPER.md:45: "a changeover function smoothly switches"
-// a pair between the fixed-step level-0 integrator and the close-encounter integrator; PAPER.md:55, 159:
-// close-encounter pairs and groups; encounter forces always in double precision.
+// a pair between the fixed-step level-0 integrator and "the Bulirsch-Stoer integrator (level 1)"; PAPER.md:55,
+// 159: close-encounter pairs and groups ("one big encounter group"); encounter forces always in
+// double precision.
 //
 // During A(dt) a body that belongs to no encounter pair moves on its Kepler orbit (kepler.cuh).  The bodies of
 // an encounter GROUP (a connected component of the pair list of the opening force evaluation) move under
 //     H_A,group = sum_k (|p_k|^2 / 2 m_k - G M m_k / r_k) - sum_{k<l in group} G m_k m_l (1 - K(r_kl)) / r_kl,
-// integrated in FP64 with classical RK4 substeps by ONE WARP per group, lane k holding member k's state in
-// registers and reading the other members' stage positions by warp shuffles.  Pair weight (1 - K) + r K' (the complement of the kick's K - r K'); r_crit,kl held at the values
-// of the opening force evaluation (w.rcrit / w.semi / w.vkep / w.m, API order).
+// pair weight (1 - K) + r K' (the complement of the kick's K - r K'), r_crit,kl held at the values of the opening
+// force evaluation (w.rcrit / w.semi / w.vkep / w.m, API order), all in FP64.
+//
+// A group is integrated by a TEAM with one thread per member: a warp for groups of up to WMAX = 16 bodies (the pair
+// constants 1 / (0.9 r_crit,kl) in a table in shared memory), the whole CTA for groups of up to GBIG = 256 bodies
+// (pair constants recomputed per pair: such groups are rare).  Members sit in ascending body index; a force
+// evaluation writes the member's stage position to a double-buffered slab in shared memory, synchronises the team
+// once and sums over the other members.  Integrators (the choice is params.enc_nsub):
+//   * Gragg-Bulirsch-Stoer extrapolation to the relative tolerance params.enc_tol (default, reading R15): modified
+//     midpoint with 2, 4, .. 16 substeps, polynomial extrapolation in h^2, error = largest |dx|/|x|, |dv|/|v| over
+//     the members; a step that does not converge in 8 rows is halved.  Status bit 8: the step size collapsed.
+//   * classical RK4 with enc_nsub equal substeps (the scheme of the first oracle, oracle_step_hybrid).
 #pragma once
 
 #include "genga_internal.cuh"
@@ -16,8 +26,10 @@
 namespace genga {
 namespace enc {
 
-constexpr int GMAX = 8;            // largest encounter group (members sit in lanes 0 .. n-1 of the group's warp)
-constexpr int GINFO = GMAX + 1;    // ints per group in Workspace::ginfo: member count, members
+constexpr int WMAX = 16;           // largest group a warp integrates
+constexpr int GBIG = 256;          // largest group at all: one CTA of the per-body kernel, one thread per member
+constexpr int KMAX = 8;            // rows of the extrapolation tableau (substep counts 2, 4, .. 16)
+constexpr unsigned int FULL = 0xffffffffu;
 
 using EncParams = EncArgs;
 
@@ -31,165 +43,309 @@ __device__ __forceinline__ double pair_rcrit(const EncParams& P, double mi, doub
     return fmax(rci, rcj);
 }
 
-constexpr unsigned int FULL = 0xffffffffu;
-
-__device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(FULL, v, src); }
-
 // 1/sqrt and 1/x from the MUFU seeds (rsqrt/rcp.approx.f64: about 2^-20 relative) with a cubic correction:
 // relative error O(e^3) ~ 1e-18, i.e. a few ulp, at a fraction of the dependent latency of sqrt and divide.
 __device__ __forceinline__ double rsq_seed(double a) { double r; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r; }
 __device__ __forceinline__ double rcp_seed(double a) { double r; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r; }
 
-// dv/dt of this lane's member at the stage positions (px, py, pz); every lane of the warp must call it.
-// c01[l] = 0.1 r_crit,kl and i09[l] = 1 / (0.9 r_crit,kl) (0: no zone, the lane itself, an idle lane) for the
-// members l.  NN > 0: the group size at compile time (straight-line code: the pair terms and the Kepler term
-// overlap in the pipeline); NN = 0: n at run time.  Branch-free: a term that does not apply gets weight 0.
-// CRIT: also return in tau the shortest time scale q / (|v_rel| + v_escape(q)) over the pairs of this member
-// that are inside their zone (1e300 if none), from which the adaptive substep is taken (vx, vy, vz: own velocity).
-template <int NN, bool CRIT = false>
-__device__ __forceinline__ void member_accel(const EncParams& P, int n, double gm_self,
-                                             const double (&c01)[GMAX], const double (&i09)[GMAX],
-                                             double px, double py, double pz, double& a0, double& a1, double& a2,
-                                             double vx = 0.0, double vy = 0.0, double vz = 0.0, double* tau = nullptr)
+// ---- shared memory of the teams ----------------------------------------------------------------------------------
+struct WarpSlab {
+    double pos[2][3][WMAX];        // stage positions of the members, double buffered
+    double gm[WMAX];
+    double i09[WMAX][WMAX];        // [l][k] = 1 / (0.9 r_crit,kl), 0: no zone (k == l, idle slots)
+};
+struct BlockSlab {
+    double pos[2][3][GBIG];
+    double gm[GBIG], m[GBIG], rc[GBIG], sa[GBIG], vk[GBIG];
+    double red[8];
+    int    body[GBIG];
+};
+union EncSmem { WarpSlab w[8]; BlockSlab b; };     // warp teams and the CTA team never run at the same time
+
+struct WarpTeam {
+    WarpSlab& s; int n, k;                              // k: member index of this lane, -1 for an idle lane
+    __device__ __forceinline__ void sync() const { __syncwarp(); }
+    __device__ __forceinline__ double maxall(double v) const
+    {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(FULL, v, o));
+        return v;
+    }
+    __device__ __forceinline__ double* px(int b) const { return s.pos[b][0]; }
+    __device__ __forceinline__ double* py(int b) const { return s.pos[b][1]; }
+    __device__ __forceinline__ double* pz(int b) const { return s.pos[b][2]; }
+    __device__ __forceinline__ double gm(int l) const { return s.gm[l]; }
+    __device__ __forceinline__ double inv09(const EncParams&, int l) const { return s.i09[l][k]; }
+};
+struct BlockTeam {
+    BlockSlab& s; int n, k;
+    __device__ __forceinline__ void sync() const { __syncthreads(); }
+    __device__ __forceinline__ double maxall(double v) const
+    {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(FULL, v, o));
+        __syncthreads();                                   // red[] may still be read from the previous call
+        if ((threadIdx.x & 31) == 0) s.red[threadIdx.x >> 5] = v;
+        __syncthreads();
+        double r = s.red[0];
+#pragma unroll
+        for (int q = 1; q < 8; ++q) r = fmax(r, s.red[q]);
+        return r;
+    }
+    __device__ __forceinline__ double* px(int b) const { return s.pos[b][0]; }
+    __device__ __forceinline__ double* py(int b) const { return s.pos[b][1]; }
+    __device__ __forceinline__ double* pz(int b) const { return s.pos[b][2]; }
+    __device__ __forceinline__ double gm(int l) const { return s.gm[l]; }
+    __device__ __forceinline__ double inv09(const EncParams& P, int l) const
+    {
+        const double rc = pair_rcrit(P, s.m[k], s.m[l], s.rc[k], s.rc[l], s.sa[k], s.sa[l], s.vk[k], s.vk[l]);
+        return (rc > 0.0) ? 1.0 / (0.9 * rc) : 0.0;
+    }
+};
+
+// dv/dt of this thread's member at the stage position (x, y, z): the member publishes its position in buffer buf,
+// the team synchronises once, every member sums the Kepler term and the complement terms of the other members.
+// Branch-free per pair: a term that does not apply gets weight 0.  Every thread of the team must call it.
+template <class Team>
+__device__ __forceinline__ void accel(const Team& T, const EncParams& P, int& buf, double x, double y, double z,
+                                      double& a0, double& a1, double& a2)
 {
-    double tmin = 1.0e300;
+    double* X = T.px(buf); double* Y = T.py(buf); double* Z = T.pz(buf);
+    if (T.k >= 0) { X[T.k] = x; Y[T.k] = y; Z[T.k] = z; }
+    T.sync();
+    buf ^= 1;                                              // the next evaluation writes the other buffer
+    a0 = 0.0; a1 = 0.0; a2 = 0.0;
+    if (T.k < 0) return;
     {
         const double mu = P.G * P.M_star;
-        const double r2 = fma(pz, pz, fma(py, py, px * px));
+        const double r2 = fma(z, z, fma(y, y, x * x));
         const double y0 = rsq_seed(r2), t = y0 * y0, e = fma(-r2, t, 1.0), g = y0 * t;
         const double ir3 = -mu * fma(g * e, fma(1.875, e, 1.5), g);         // -mu / r^3
-        a0 = px * ir3; a1 = py * ir3; a2 = pz * ir3;
+        a0 = x * ir3; a1 = y * ir3; a2 = z * ir3;
     }
-#pragma unroll
-    for (int l = 0; l < (NN > 0 ? NN : GMAX); ++l) {
-        if (NN == 0 && l >= n) break;                       // n is uniform over the warp
-        const double ox = shfl_d(px, l), oy = shfl_d(py, l), oz = shfl_d(pz, l), ogm = shfl_d(gm_self, l);
-        const double d0 = ox - px, d1 = oy - py, d2 = oz - pz;
+    for (int l = 0; l < T.n; ++l) {
+        const double i09 = (l == T.k) ? 0.0 : T.inv09(P, l);
+        const double d0 = X[l] - x, d1 = Y[l] - y, d2 = Z[l] - z;
         const double q2 = fma(d2, d2, fma(d1, d1, d0 * d0));
-        const bool   on = (i09[l] > 0.0) && (q2 > 0.0);
+        const bool   on = (i09 > 0.0) && (q2 > 0.0);
         const double qs = on ? q2 : 1.0;
         const double y0 = rsq_seed(qs), t = y0 * y0, e = fma(-qs, t, 1.0), g = y0 * t;
         const double q0 = qs * y0;
         const double q  = fma(q0 * e, fma(0.375, e, 0.5), q0);              // |d|
-        const double y  = fmin(fmax((q - c01[l]) * i09[l], 0.0), 1.0);       // y <= 0: Wc = 1, y >= 1: Wc = 0
-        const double D  = fma(2.0 * y, y - 1.0, 1.0);                        // 2y^2 - 2y + 1, in [1/2, 1]
+        const double yy = fmin(fmax(fma(q, i09, -1.0 / 9.0), 0.0), 1.0);     // (q - 0.1 rc) / (0.9 rc); <= 0: Wc = 1, >= 1: Wc = 0
+        const double D  = fma(2.0 * yy, yy - 1.0, 1.0);                      // 2y^2 - 2y + 1, in [1/2, 1]
         const double r0 = rcp_seed(D), f = fma(-D, r0, 1.0);
         const double iD = fma(r0 * f, 1.0 + f, r0);
-        const double K  = y * y * iD;
-        const double Kp = 2.0 * y * (1.0 - y) * iD * iD * i09[l];            // dK/dr (0 at both ends)
+        const double K  = yy * yy * iD;
+        const double Kp = 2.0 * yy * (1.0 - yy) * iD * iD * i09;             // dK/dr (0 at both ends)
         const double Wc = on ? 1.0 - (K - q * Kp) : 0.0;
-        const double s  = ogm * Wc * fma(g * e, fma(1.875, e, 1.5), g);      // G m_l Wc / |d|^3
+        const double s  = T.gm(l) * Wc * fma(g * e, fma(1.875, e, 1.5), g);  // G m_l Wc / |d|^3
         a0 = fma(s, d0, a0); a1 = fma(s, d1, a1); a2 = fma(s, d2, a2);
-        if (CRIT) {
-            const double u0 = shfl_d(vx, l) - vx, u1 = shfl_d(vy, l) - vy, u2 = shfl_d(vz, l) - vz;
-            const double vrel = sqrt(fma(u2, u2, fma(u1, u1, u0 * u0)));
-            const double vesc = sqrt(2.0 * (gm_self + ogm) * y0);           // y0 ~ 1/|d| (seed accuracy is plenty here)
-            if (on && y < 1.0) tmin = fmin(tmin, q / (vrel + vesc));
-        }
     }
-    if (CRIT) *tau = tmin;
 }
 
-// The flow of H_A,group over dt for this lane's member (state in registers): classical RK4 substeps of dt / nsub, or
-// shorter where a pair is deep inside its zone (P.eta > 0: h = min(dt / nsub, eta * tau), tau the shortest
-// q / (|v_rel| + v_escape) over the in-zone pairs of the whole group, never below dt / (256 nsub): status bit 8).
-template <int NN, bool ADAPT>
-__device__ __forceinline__ void integrate(const EncParams& P, int n, double gm, const double (&c01)[GMAX], const double (&i09)[GMAX],
-                                          double dt, double& x0, double& x1, double& x2, double& v0, double& v1, double& v2,
-                                          unsigned int* status)
+// A(dt) by classical RK4 with nsub equal substeps (oracle_step_hybrid's scheme, restricted to the group).
+template <class Team>
+__device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P, double dt, double (&y)[6])
 {
-    const double T = fabs(dt), sgn = (dt < 0.0) ? -1.0 : 1.0;
-    const double hmax = T / P.nsub, hmin = hmax * (1.0 / 256.0);
-    constexpr bool adaptive = ADAPT;
-    double tnow = 0.0;
-    bool floored = false;
-    for (int s = 0; ; ++s) {
-        if (adaptive ? !(T - tnow > 1.0e-9 * hmax) : (s == P.nsub)) break;
-        double k0, k1, k2;                                 // stage acceleration
-        double sx0, sx1, sx2, sv0, sv1, sv2;               // running sums k1 + 2 k2 + 2 k3 (+ k4)
-        double t0, t1, t2, u0, u1, u2;                     // stage position, stage velocity
-        double habs = hmax;
-        if (adaptive) {
-            double tau;
-            member_accel<NN, true>(P, n, gm, c01, i09, x0, x1, x2, k0, k1, k2, v0, v1, v2, &tau);
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) tau = fmin(tau, __shfl_xor_sync(FULL, tau, o));
-            const double want = P.eta * tau;
-            if (want < hmin) floored = true;
-            habs = fmin(hmax, fmax(want, hmin));
-            habs = fmin(habs, T - tnow);
-            tnow += habs;
-        } else {
-            member_accel<NN>(P, n, gm, c01, i09, x0, x1, x2, k0, k1, k2);
-        }
-        const double h = sgn * habs, hh = 0.5 * h, h6 = h / 6.0;
-        sx0 = v0; sx1 = v1; sx2 = v2; sv0 = k0; sv1 = k1; sv2 = k2;
-        t0 = fma(hh, v0, x0); t1 = fma(hh, v1, x1); t2 = fma(hh, v2, x2);
-        u0 = fma(hh, k0, v0); u1 = fma(hh, k1, v1); u2 = fma(hh, k2, v2);
-        member_accel<NN>(P, n, gm, c01, i09, t0, t1, t2, k0, k1, k2);
-        sx0 += 2.0 * u0; sx1 += 2.0 * u1; sx2 += 2.0 * u2; sv0 += 2.0 * k0; sv1 += 2.0 * k1; sv2 += 2.0 * k2;
-        t0 = fma(hh, u0, x0); t1 = fma(hh, u1, x1); t2 = fma(hh, u2, x2);
-        u0 = fma(hh, k0, v0); u1 = fma(hh, k1, v1); u2 = fma(hh, k2, v2);
-        member_accel<NN>(P, n, gm, c01, i09, t0, t1, t2, k0, k1, k2);
-        sx0 += 2.0 * u0; sx1 += 2.0 * u1; sx2 += 2.0 * u2; sv0 += 2.0 * k0; sv1 += 2.0 * k1; sv2 += 2.0 * k2;
-        t0 = fma(h, u0, x0); t1 = fma(h, u1, x1); t2 = fma(h, u2, x2);
-        u0 = fma(h, k0, v0); u1 = fma(h, k1, v1); u2 = fma(h, k2, v2);
-        member_accel<NN>(P, n, gm, c01, i09, t0, t1, t2, k0, k1, k2);
-        x0 = fma(h6, sx0 + u0, x0); x1 = fma(h6, sx1 + u1, x1); x2 = fma(h6, sx2 + u2, x2);
-        v0 = fma(h6, sv0 + k0, v0); v1 = fma(h6, sv1 + k1, v1); v2 = fma(h6, sv2 + k2, v2);
+    const double h = dt / P.nsub, hh = 0.5 * h, h6 = h / 6.0;
+    int buf = 0;
+    for (int s = 0; s < P.nsub; ++s) {
+        double k0, k1, k2, sx[3], sv[3], t[3], u[3];
+        accel(T, P, buf, y[0], y[1], y[2], k0, k1, k2);
+        sx[0] = y[3]; sx[1] = y[4]; sx[2] = y[5]; sv[0] = k0; sv[1] = k1; sv[2] = k2;
+        t[0] = fma(hh, y[3], y[0]); t[1] = fma(hh, y[4], y[1]); t[2] = fma(hh, y[5], y[2]);
+        u[0] = fma(hh, k0, y[3]); u[1] = fma(hh, k1, y[4]); u[2] = fma(hh, k2, y[5]);
+        accel(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
+        sx[0] += 2.0 * u[0]; sx[1] += 2.0 * u[1]; sx[2] += 2.0 * u[2]; sv[0] += 2.0 * k0; sv[1] += 2.0 * k1; sv[2] += 2.0 * k2;
+        t[0] = fma(hh, u[0], y[0]); t[1] = fma(hh, u[1], y[1]); t[2] = fma(hh, u[2], y[2]);
+        u[0] = fma(hh, k0, y[3]); u[1] = fma(hh, k1, y[4]); u[2] = fma(hh, k2, y[5]);
+        accel(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
+        sx[0] += 2.0 * u[0]; sx[1] += 2.0 * u[1]; sx[2] += 2.0 * u[2]; sv[0] += 2.0 * k0; sv[1] += 2.0 * k1; sv[2] += 2.0 * k2;
+        t[0] = fma(h, u[0], y[0]); t[1] = fma(h, u[1], y[1]); t[2] = fma(h, u[2], y[2]);
+        u[0] = fma(h, k0, y[3]); u[1] = fma(h, k1, y[4]); u[2] = fma(h, k2, y[5]);
+        accel(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
+        y[0] = fma(h6, sx[0] + u[0], y[0]); y[1] = fma(h6, sx[1] + u[1], y[1]); y[2] = fma(h6, sx[2] + u[2], y[2]);
+        y[3] = fma(h6, sv[0] + k0, y[3]); y[4] = fma(h6, sv[1] + k1, y[4]); y[5] = fma(h6, sv[2] + k2, y[5]);
     }
-    if (floored && (threadIdx.x & 31) == 0) atomicOr(status, 8u);
 }
 
-// One warp advances group g through S(dt/2) (the shift s, already scaled) and the flow of H_A,group over dt
-// (nsub RK4 substeps) and writes its members back.  Members are taken in ascending body index, so the result
-// does not depend on the order in which group_kernel registered them.
-__device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, int g, double dt, double s0, double s1, double s2)
+// A(dt) by Gragg-Bulirsch-Stoer extrapolation to the relative tolerance P.tol (reading R15).  The tableau is kept in
+// the difference form of polynomial extrapolation (one column of differences per row), which yields the extrapolated
+// value and the last correction, i.e. the error estimate T_kk - T_k,k-1, without storing two rows.
+template <class Team>
+__device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, double dt, double (&y)[6], unsigned int* status)
+{
+    const double Tabs = fabs(dt);
+    double t = 0.0, H = dt;
+    int buf = 0;
+    bool collapsed = false;
+    while (fabs(t) < Tabs * (1.0 - 1.0e-14)) {
+        if (fabs(t + H) > Tabs) H = dt - t;
+        double f0[3];
+        accel(T, P, buf, y[0], y[1], y[2], f0[0], f0[1], f0[2]);
+        double d[KMAX][6], hsq[KMAX], yz[6], dy[6];
+        int done = -1;
+        for (int k = 0; k < KMAX && done < 0; ++k) {
+            const int nk = 2 * (k + 1);
+            const double h = H / nk, h2 = 2.0 * h;
+            double z0[6], z1[6], f[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { z0[c] = y[c]; z0[3 + c] = y[3 + c]; z1[c] = fma(h, y[3 + c], y[c]); z1[3 + c] = fma(h, f0[c], y[3 + c]); }
+            for (int s = 1; s < nk; ++s) {
+                accel(T, P, buf, z1[0], z1[1], z1[2], f[0], f[1], f[2]);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const double nx = fma(h2, z1[3 + c], z0[c]), nv = fma(h2, f[c], z0[3 + c]);
+                    z0[c] = z1[c]; z0[3 + c] = z1[3 + c]; z1[c] = nx; z1[3 + c] = nv;
+                }
+            }
+            accel(T, P, buf, z1[0], z1[1], z1[2], f[0], f[1], f[2]);
+            double est[6];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                est[c] = 0.5 * (z1[c] + z0[c] + h * z1[3 + c]);
+                est[3 + c] = 0.5 * (z1[3 + c] + z0[3 + c] + h * f[c]);
+            }
+            // polynomial extrapolation to h^2 = 0 through the rows 0 .. k
+            hsq[k] = h * h;
+#pragma unroll
+            for (int c = 0; c < 6; ++c) { yz[c] = est[c]; dy[c] = est[c]; }
+            if (k == 0) {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) d[0][c] = est[c];
+            } else {
+                double cc[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) cc[c] = est[c];
+                for (int j = 0; j < k; ++j) {
+                    const double delta = 1.0 / (hsq[k - j - 1] - hsq[k]);
+                    const double f1 = hsq[k] * delta, f2 = hsq[k - j - 1] * delta;
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) {
+                        const double q = d[j][c];
+                        d[j][c] = dy[c];
+                        const double dl = cc[c] - q;
+                        dy[c] = f1 * dl; cc[c] = f2 * dl;
+                        yz[c] += dy[c];
+                    }
+                }
+#pragma unroll
+                for (int c = 0; c < 6; ++c) d[k][c] = dy[c];
+                double e = 0.0;
+                if (T.k >= 0) {
+                    const double ex = (dy[0] * dy[0] + dy[1] * dy[1] + dy[2] * dy[2]) / (yz[0] * yz[0] + yz[1] * yz[1] + yz[2] * yz[2]);
+                    const double ev = (dy[3] * dy[3] + dy[4] * dy[4] + dy[5] * dy[5]) / (yz[3] * yz[3] + yz[4] * yz[4] + yz[5] * yz[5]);
+                    e = fmax(ex, ev);
+                    if (!(e == e)) e = 1.0e300;           // NaN: not converged
+                }
+                e = T.maxall(e);
+                if (e <= P.tol * P.tol) done = k;         // squared norms against the squared tolerance
+            }
+        }
+        if (done < 0) {
+            H *= 0.5;
+            if (fabs(H) < Tabs * 9.3e-10) { collapsed = true; break; }      // dt 2^-30: give up, keep the last accepted state
+            continue;
+        }
+#pragma unroll
+        for (int c = 0; c < 6; ++c) y[c] = yz[c];
+        t += H;
+        H = (done <= 3) ? 2.0 * H : ((done <= 5) ? H : 0.5 * H);
+    }
+    if (collapsed && T.k == 0) atomicOr(status, 8u);
+}
+
+template <class Team>
+__device__ __forceinline__ void integrate(const Team& T, const EncParams& P, double dt, double (&y)[6], unsigned int* status)
+{
+    if (dt == 0.0) return;
+    if (P.nsub > 0) integrate_rk4(T, P, dt, y);
+    else            integrate_bs(T, P, dt, y, status);
+}
+
+// Groups in Workspace::ginfo (written by group_kernel): ginfo[2 g] = offset of the member list, ginfo[2 g + 1] = member
+// count; the member lists (body indices, in no particular order) follow from ginfo[2 maxgroups] on.
+__device__ __forceinline__ const int* group_members(const Workspace& w, int maxgroups, int g, int& n)
+{
+    n = w.ginfo[2 * g + 1];
+    return w.ginfo + 2 * (size_t)maxgroups + w.ginfo[2 * g];
+}
+
+// One warp advances a group of n <= WMAX bodies through S(dt/2) (the shift s, already scaled) and the flow of
+// H_A,group over dt, and writes its members back.  Members are taken in ascending body index, so the result does
+// not depend on the order in which group_kernel registered them.
+__device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, WarpSlab& slab, const int* mem, int n,
+                                           double dt, double s0, double s1, double s2)
 {
     const int lane = threadIdx.x & 31;
-    const int* info = w.ginfo + (size_t)g * GINFO;
-    const int n = min(info[0], GMAX);
-    const int b_in = (lane < n) ? info[1 + lane] : 0x7fffffff;
+    const int b_in = (lane < n) ? mem[lane] : 0x7fffffff;
     int rank = 0;
-#pragma unroll
-    for (int l = 0; l < GMAX; ++l) { const int o = __shfl_sync(FULL, b_in, l); if (l < n && o < b_in) ++rank; }
+    for (int l = 0; l < n; ++l) { const int o = __shfl_sync(FULL, b_in, l); if (o < b_in) ++rank; }
     int b = -1;
-#pragma unroll
-    for (int l = 0; l < GMAX; ++l) {
+    for (int l = 0; l < n; ++l) {
         const int o = __shfl_sync(FULL, b_in, l), r = __shfl_sync(FULL, rank, l);
-        if (l < n && r == lane) b = o;
+        if (r == lane) b = o;
     }
     const bool active = lane < n;
     double m = 0.0, rci = 0.0, sa = 0.0, vk = 0.0;
-    double x0 = 1.0, x1 = 0.0, x2 = 0.0, v0 = 0.0, v1 = 0.0, v2 = 0.0;      // idle lanes: a harmless unit orbit
+    double y[6] = {1.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     if (active) {
         m = w.m[b]; rci = w.rcrit[b]; sa = w.semi[b]; vk = w.vkep[b];
-        x0 = w.x[3 * b] + s0; x1 = w.x[3 * b + 1] + s1; x2 = w.x[3 * b + 2] + s2;
-        v0 = w.v[3 * b]; v1 = w.v[3 * b + 1]; v2 = w.v[3 * b + 2];
+        y[0] = w.x[3 * b] + s0; y[1] = w.x[3 * b + 1] + s1; y[2] = w.x[3 * b + 2] + s2;
+        y[3] = w.v[3 * b]; y[4] = w.v[3 * b + 1]; y[5] = w.v[3 * b + 2];
     }
-    double c01[GMAX], i09[GMAX];
-#pragma unroll
-    for (int l = 0; l < GMAX; ++l) {
-        const double ml = shfl_d(m, l), rcl = shfl_d(rci, l), sal = shfl_d(sa, l), vkl = shfl_d(vk, l);
-        const double rc = (active && l < n && l != lane) ? pair_rcrit(P, m, ml, rci, rcl, sa, sal, vk, vkl) : 0.0;
-        c01[l] = 0.1 * rc; i09[l] = (rc > 0.0) ? 1.0 / (0.9 * rc) : 0.0;
-    }
-    const double gm = P.G * m;
-    if (dt != 0.0) {
-        unsigned int* st = &w.ctr->enc_status;
-        if (P.eta > 0.0) {                                  // adaptive substeps (opt-in): one generic instance
-            integrate<0, true>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
-        } else {
-            if (n == 2)      integrate<2, false>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
-            else if (n == 3) integrate<3, false>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
-            else if (n == 4) integrate<4, false>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
-            else             integrate<0, false>(P, n, gm, c01, i09, dt, x0, x1, x2, v0, v1, v2, st);
+    __syncwarp();                                           // the slab may still be read by the previous group's last sum
+    for (int l = 0; l < n; ++l) {
+        const double ml = __shfl_sync(FULL, m, l), rcl = __shfl_sync(FULL, rci, l), sal = __shfl_sync(FULL, sa, l),
+                     vkl = __shfl_sync(FULL, vk, l);
+        if (active) {
+            const double rc = (l != lane) ? pair_rcrit(P, m, ml, rci, rcl, sa, sal, vk, vkl) : 0.0;
+            slab.i09[l][lane] = (rc > 0.0) ? 1.0 / (0.9 * rc) : 0.0;
         }
     }
+    if (active) slab.gm[lane] = P.G * m;
+    __syncwarp();
+    const WarpTeam T{slab, n, active ? lane : -1};
+    integrate(T, P, dt, y, &w.ctr->enc_status);
     if (active) {
-        w.x[3 * b] = x0; w.x[3 * b + 1] = x1; w.x[3 * b + 2] = x2;
-        w.v[3 * b] = v0; w.v[3 * b + 1] = v1; w.v[3 * b + 2] = v2;
+        w.x[3 * b] = y[0]; w.x[3 * b + 1] = y[1]; w.x[3 * b + 2] = y[2];
+        w.v[3 * b] = y[3]; w.v[3 * b + 1] = y[4]; w.v[3 * b + 2] = y[5];
     }
+}
+
+// The whole CTA (GBIG threads) advances a group of WMAX < n <= GBIG bodies.  Must be called by all threads.
+__device__ __forceinline__ void block_group(const EncParams& P, Workspace& w, BlockSlab& slab, const int* mem, int n,
+                                            double dt, double s0, double s1, double s2)
+{
+    const int tid = threadIdx.x;
+    __syncthreads();                                        // the slab (a union with the warp slabs) is free
+    const int b_in = (tid < n) ? mem[tid] : 0x7fffffff;
+    if (tid < n) slab.body[tid] = b_in;
+    __syncthreads();
+    int rank = 0;
+    if (tid < n) for (int l = 0; l < n; ++l) if (slab.body[l] < b_in) ++rank;
+    __syncthreads();
+    if (tid < n) slab.body[rank] = b_in;                    // ascending body index (indices are distinct)
+    __syncthreads();
+    const bool active = tid < n;
+    double y[6] = {1.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    int b = -1;
+    if (active) {
+        b = slab.body[tid];
+        const double m = w.m[b];
+        slab.m[tid] = m; slab.gm[tid] = P.G * m; slab.rc[tid] = w.rcrit[b]; slab.sa[tid] = w.semi[b]; slab.vk[tid] = w.vkep[b];
+        y[0] = w.x[3 * b] + s0; y[1] = w.x[3 * b + 1] + s1; y[2] = w.x[3 * b + 2] + s2;
+        y[3] = w.v[3 * b]; y[4] = w.v[3 * b + 1]; y[5] = w.v[3 * b + 2];
+    }
+    __syncthreads();
+    const BlockTeam T{slab, n, active ? tid : -1};
+    integrate(T, P, dt, y, &w.ctr->enc_status);
+    if (active) {
+        w.x[3 * b] = y[0]; w.x[3 * b + 1] = y[1]; w.x[3 * b + 2] = y[2];
+        w.v[3 * b] = y[3]; w.v[3 * b + 1] = y[4]; w.v[3 * b + 2] = y[5];
+    }
+    __syncthreads();
 }
 
 }  // namespace enc

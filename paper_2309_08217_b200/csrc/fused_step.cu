@@ -1,5 +1,6 @@
 // fused_step.cu -- kernel wrapper and launcher of the cooperative per-body kernel of the step (body and
 // description in onbody_body.cuh).
+#include <algorithm>
 #include "onbody_body.cuh"
 
 namespace genga {
@@ -18,14 +19,17 @@ onbody_kernel(OnBodyArgs A, Workspace w)
 
 // Encounter groups (NEXT-1): connected components of the encounter-pair graph by label propagation over the
 // pair list; glabel[b] = smallest body index of b's component, -1 for bodies in no pair (preset by the
-// launcher), -2 for the bodies of a component with more than enc::GMAX members (status bit 2; they drift on
-// their Kepler orbits).  Then every component gets a group index g and registers its members in
-// ginfo[g * GINFO ..] (count, members; in no particular order: the integrating warp sorts them).  One block.
+// launcher), -2 for the bodies of a component with more than enc::GBIG members (status bit 2; they drift on
+// their Kepler orbits).  Then every component gets a group index g, a slice of the member array
+// (ginfo[2 g] = offset, ginfo[2 g + 1] = count) and registers its members there (in no particular order: the
+// integrating team sorts them).  One block.
 __global__ void __launch_bounds__(1024)
 group_kernel(int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr, unsigned int pair_cap,
-             int* __restrict__ glabel, int* __restrict__ ginfo, int* __restrict__ ulist)
+             int* __restrict__ glabel, int* __restrict__ ginfo, int* __restrict__ ulist, int maxgroups)
 {
     __shared__ int changed;
+    __shared__ int cursor;
+    int* members = ginfo + 2 * (size_t)maxgroups;
     int* gcount = glabel + NP;
     const unsigned int total = ctr->pair_count;
     const unsigned int n = total < pair_cap ? total : pair_cap;
@@ -37,7 +41,7 @@ group_kernel(int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr,
     // the bodies that occur in a pair, each once (gcount is preset to -1 like the labels): every later pass
     // walks this short list instead of all N bodies
     __shared__ int nuniq;
-    if (threadIdx.x == 0) nuniq = 0;
+    if (threadIdx.x == 0) { nuniq = 0; cursor = 0; }
     __syncthreads();
     for (unsigned int p = threadIdx.x; p < 2u * n; p += blockDim.x) {
         const int2 ij = pairs[p >> 1];
@@ -65,10 +69,10 @@ group_kernel(int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr,
     __syncthreads();
     for (int q = threadIdx.x; q < nu; q += blockDim.x) {
         const int b = ulist[q], l = glabel[b];
-        if (l != b && gcount[l] > enc::GMAX) { glabel[b] = -2; atomicOr(&ctr->enc_status, 2u); }
+        if (l != b && gcount[l] > enc::GBIG) { glabel[b] = -2; atomicOr(&ctr->enc_status, 2u); }
     }
     __syncthreads();
-    for (int q = threadIdx.x; q < nu; q += blockDim.x) { const int b = ulist[q]; if (glabel[b] == b && gcount[b] > enc::GMAX) glabel[b] = -2; }
+    for (int q = threadIdx.x; q < nu; q += blockDim.x) { const int b = ulist[q]; if (glabel[b] == b && gcount[b] > enc::GBIG) glabel[b] = -2; }
     __syncthreads();
     for (int q = threadIdx.x; q < nu; q += blockDim.x) {
         const int b = ulist[q];
@@ -76,7 +80,8 @@ group_kernel(int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr,
             const unsigned int g = atomicAdd(&ctr->enc_groups, 1u);
             const int cnt = gcount[b];
             atomicAdd(&ctr->enc_bodies, (unsigned int)cnt); atomicMax(&ctr->enc_maxsize, (unsigned int)cnt);
-            ginfo[g * enc::GINFO] = 0;
+            ginfo[2 * g] = atomicAdd(&cursor, cnt);
+            ginfo[2 * g + 1] = 0;
             gcount[b] = (int)g;
         }
     }
@@ -84,9 +89,9 @@ group_kernel(int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr,
     for (int q = threadIdx.x; q < nu; q += blockDim.x) {
         const int b = ulist[q], l = glabel[b];
         if (l >= 0) {
-            int* info = ginfo + (size_t)gcount[l] * enc::GINFO;
-            const int k = atomicAdd(info, 1);
-            if (k < enc::GMAX) info[1 + k] = b;
+            const int g = gcount[l];
+            const int k = atomicAdd(&ginfo[2 * g + 1], 1);
+            members[ginfo[2 * g] + k] = b;
         }
     }
 }
@@ -129,7 +134,8 @@ cudaError_t launch_groups(const Handle* h)
     if (h->N == 0) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(h->w.glabel, 0xff, 2 * (size_t)h->NP * sizeof(int), h->stream);   // labels and counts: -1
     if (e != cudaSuccess) return e;
-    group_kernel<<<1, 1024, 0, h->stream>>>(h->NP, h->w.pairs, h->w.ctr, (unsigned int)h->pair_cap, h->w.glabel, h->w.ginfo, h->w.gulist);
+    group_kernel<<<1, 1024, 0, h->stream>>>(h->NP, h->w.pairs, h->w.ctr, (unsigned int)h->pair_cap, h->w.glabel, h->w.ginfo, h->w.gulist,
+                                        (int)std::min((size_t)h->pair_cap, (size_t)h->NP / 2));
     return cudaGetLastError();
 }
 

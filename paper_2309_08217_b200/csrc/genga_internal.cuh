@@ -44,7 +44,7 @@ struct Counters {
     unsigned int ticket;         // block-completion ticket of the momentum reduction (0 between launches)
     unsigned int extent_bits;    // float bits of max(|x|, |y|) over the bodies (Hilbert sort extent)
     // encounter mode (encounter.cuh; NEXT-1)
-    unsigned int enc_status;     // sticky until read: 1 pair list overflowed, 2 a group had more than enc::GMAX bodies, 8 substep floor hit
+    unsigned int enc_status;     // sticky until read: 1 pair list overflowed, 2 a group had more than enc::GBIG bodies, 8 the Bulirsch-Stoer step size collapsed
     unsigned int enc_groups;     // encounter groups integrated by the last drift
     unsigned int enc_bodies;     // bodies in those groups
     unsigned int enc_maxsize;    // largest group of the last drift
@@ -74,7 +74,7 @@ struct Workspace {
     unsigned int* sortbuf;      // bucket histogram, starts and cursors of the sort
     int* glabel;                // [2 NP] encounter mode: smallest body index of the body's encounter group (-1: none,
                                 //        -2: group too large, Kepler drift), then [NP] member count / group index per label
-    int* ginfo;                 // [enc::GINFO x max groups] per group: member count, members
+    int* ginfo;                 // [2 x max groups] (offset, member count) per group, then the member lists (body indices)
     int* gulist;                // [min(2 pair_cap, NP)] the bodies that occur in the pair list, each once
     double4* pk64;    // [NP]   (x, y, z, G m)
     float4*  pk32;    // [NP]   two planes per chunk, see above
@@ -147,11 +147,12 @@ struct PrepArgs {
 };
 struct EncArgs {                  // encounter mode (encounter.cuh; NEXT-1, reading R11)
     int on;                        // 0: every body drifts on its Kepler orbit
-    int nsub;                      // RK4 substeps per step for the bodies of an encounter group
+    int nsub;                      // > 0: RK4 with nsub substeps per step for the bodies of an encounter group; 0: Bulirsch-Stoer
     int pair_rule;
     unsigned int pair_cap;
     double G, M_star, n1, n2dt;
-    double eta;                    // > 0: adaptive substeps (encounter.cuh: integrate)
+    double tol;                    // nsub <= 0: relative tolerance of the Bulirsch-Stoer integration (encounter.cuh)
+    int maxgroups;                 // layout of Workspace::ginfo: [2 maxgroups] (offset, count) per group, then the member lists
 };
 struct OnBodyArgs {               // the fused per-body kernel of the step (fused_step.cu)
     PrepArgs prep;

@@ -111,13 +111,28 @@ __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, c
             p0 = fma(mi, vx, p0); p1 = fma(mi, vy, p1); p2 = fma(mi, vz, p2); mt += mi;
         }
         if (ENC) {
-            // encounter mode (NEXT-1, encounter.cuh): one warp per encounter group advances its members through the
-            // same S(dt/2) and the flow of H_A,group over dt; then their m v' joins the sum, each body's in the
+            // encounter mode (NEXT-1, encounter.cuh): one team (a warp, or the CTA for a large group) per encounter group
+            // advances its members through the same S(dt/2) and the flow of H_A,group over dt; then their m v' joins the sum, each body's in the
             // thread that owns the body (so the sum does not depend on which warp moved which group)
+            __shared__ enc::EncSmem esm;
             const int ngroups = (int)__ldcg(&w.ctr->enc_groups);
-            // group g -> block g % gridDim.x, warp (g / gridDim.x) % 8: a few hundred groups spread over all SMs
-            for (int g = blockIdx.x + gridDim.x * (threadIdx.x >> 5); g < ngroups; g += gridDim.x * (FUSED_NT / 32))
-                enc::warp_group(A.enc, w, g, A.dt, s0, s1, s2);
+            // groups of more than enc::WMAX bodies first, each by a whole CTA (the j-th such group by CTA j mod grid)
+            int nbig = 0;
+            for (int g = 0; g < ngroups; ++g) {
+                int n;
+                const int* mem = enc::group_members(w, A.enc.maxgroups, g, n);
+                if (n > enc::WMAX) {
+                    if (nbig % (int)gridDim.x == (int)blockIdx.x) enc::block_group(A.enc, w, esm.b, mem, n, A.dt, s0, s1, s2);
+                    ++nbig;
+                }
+            }
+            __syncthreads();
+            // the others by one warp each: group g -> block g % gridDim.x, warp (g / gridDim.x) % 8
+            for (int g = blockIdx.x + gridDim.x * (threadIdx.x >> 5); g < ngroups; g += gridDim.x * (FUSED_NT / 32)) {
+                int n;
+                const int* mem = enc::group_members(w, A.enc.maxgroups, g, n);
+                if (n <= enc::WMAX) enc::warp_group(A.enc, w, esm.w[threadIdx.x >> 5], mem, n, A.dt, s0, s1, s2);
+            }
             grid.sync();
             for (int i = gtid; i < N; i += gsz)
                 if (w.glabel[i] >= 0) {

@@ -196,7 +196,7 @@ def test_oversized_groups_are_reported_and_parameters_checked():
     groups, bodies, largest, missed, status = g.encounter_stats()
     x, v = (t.cpu().numpy() for t in g.get_state())
     g.close()
-    assert status & 2 and largest <= 8 and np.isfinite(x).all() and np.isfinite(v).all()
+    assert status & 2 and largest <= 256 and np.isfinite(x).all() and np.isfinite(v).all()
     for bad in (dict(weight_mode=0), dict(n_big=3), dict(enc_list_scale=0.5), dict(enc_list_scale=9.0), dict(no_fused_step=True)):
         with pytest.raises(Exception):
             hybrid(w, **bad).close()
@@ -213,33 +213,106 @@ def deep_flyby_system():
     return workload("flyby", m, x, v, 2.0, 0.0, B.PAIR_MUTUAL_HILL)
 
 
-def test_adaptive_substeps_resolve_a_deep_flyby():
-    # params.enc_eta > 0 (opt-in): the substep follows r / (v_rel + v_escape) of the in-zone pairs.  Reference:
-    # the oracle's fixed-step scheme converged (100 000 substeps, checked against 50 000).
+def test_bulirsch_stoer_resolves_a_deep_flyby():
+    # default integrator of the groups (enc_nsub = 0): Bulirsch-Stoer extrapolation to enc_tol (reading R15).  Reference:
+    # the oracle's extrapolation integrator over ALL bodies (no groups), itself pinned against DOP853 and the converged RK4.
     w = deep_flyby_system()
     p = oparams(w)
     vd = oracle.to_democratic(w.m, w.v, w.M_star)
-    xo, vo = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=100000)
-    xh, vh = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=50000)
-    assert state_err(xh, vh, xo, vo) <= 1e-8
+    xo, vo = oracle.step_hybrid_bs(w.m, w.x, vd, p, w.dt, tol=1e-13)
+    xh, vh = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=100000)
+    assert state_err(xh, vh, xo, vo) <= 1e-8                     # the two oracles agree where RK4 has converged that far
     x256, v256 = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=256)
     err = {}
-    for eta in (-1.0, 0.05):
-        g = hybrid(w, enc_nsub=256, enc_eta=eta)
+    for kw in (dict(enc_nsub=256), dict(), dict(enc_tol=1e-9)):
+        g = hybrid(w, **kw)
         g.step(w.dt, B.FP64)
         x, v = (t.cpu().numpy() for t in g.get_state())
         st = g.encounter_stats()
         g.close()
-        assert st == (1, 2, 2, 0, 0)
-        err[eta] = state_err(x, v, xo, vo)
-        if eta < 0:                                            # the fixed scheme is the oracle's, resolved or not
+        assert st == (1, 2, 2, 0, 0), st
+        err[tuple(kw.items())] = state_err(x, v, xo, vo)
+        if "enc_nsub" in kw:                                   # the fixed scheme is the first oracle's, resolved or not
             assert state_err(x, v, x256, v256) <= 1e-8
-    assert err[-1.0] > 1e-3, err                                # 256 fixed substeps step over the approach
-    assert err[0.05] <= 1e-7, err                               # 5e-9 measured
-    g = hybrid(w, enc_nsub=64, enc_eta=0.01)                    # the floor dt / (256 enc_nsub) is reported when hit
+    assert err[(("enc_nsub", 256),)] > 1e-3, err                # 256 fixed substeps step over the approach
+    # the flyby amplifies an error made before the closest approach about a thousandfold (the outgoing direction
+    # depends on the impact parameter of 1e-4 AU), so the state error is ~1e3 x the tolerance of the integration
+    assert err[()] <= 5e-9, err                                 # tolerance 1e-12 (default): 9e-10 measured
+    assert err[(("enc_tol", 1e-9),)] <= 1e-6, err
+
+
+def chain_cluster_disc(n, seed, sizes):
+    """A disc of n small bodies with planted chains: `sizes[j]` bodies in a row, each 0.35 r_crit from the next, so
+    that every chain is ONE encounter group of that size."""
+    u = W.uniforms(seed, 6 * n).reshape(n, 6)
+    m = 1e-7 * (0.5 + u[:, 0])
+    a = 0.6 + 2.4 * (np.arange(n) + u[:, 1]) / n
+    x, v = W.elements_to_cartesian(G * (1 + m), a, 0.01 * u[:, 2], 0.005 * u[:, 3], 6.28 * u[:, 4], 6.28 * u[:, 5],
+                                   6.28 * ((np.arange(n) * 0.381966) % 1.0))
+    k = 20
+    for size in sizes:
+        r = np.linalg.norm(x[k])
+        rc = 3.0 * np.cbrt(2 * m[k] / 3.0) * r
+        t = np.cross([0.0, 0.0, 1.0], x[k] / r)                    # along the orbit
+        for q in range(1, size):
+            x[k + q] = x[k] + rc * (0.35 * q * t + 0.05 * (-1) ** q * x[k] / r + [0.0, 0.0, 0.02 * (q % 3)])
+            v[k + q] = v[k] * (1.0 + 1e-4 * (q % 5))
+        k += size + 37
+    return workload("disc+chains", m, x, v, 6.0, 0.0, B.PAIR_MUTUAL_HILL)
+
+
+def test_large_groups_are_integrated_by_a_warp_or_a_cta():
+    # groups of 14 (one warp, pair table in shared memory) and of 23 and 60 bodies (the whole CTA): one hybrid step
+    # against the oracle, which knows nothing about groups
+    w = chain_cluster_disc(900, 9, (14, 23, 60, 3))
+    p = oparams(w)
+    vd = oracle.to_democratic(w.m, w.v, w.M_star)
+    po = oracle.encounter_pairs(w.m, w.x, vd, p)
+    import scipy.sparse as sp
+    from scipy.sparse.csgraph import connected_components
+    adj = sp.coo_matrix((np.ones(len(po)), (po[:, 0], po[:, 1])), shape=(w.N, w.N))
+    _, lab = connected_components(adj, directed=False)
+    sizes = np.bincount(lab)
+    assert sorted(sizes[sizes > 2].tolist())[-3:] == [14, 23, 60] or max(sizes) >= 60, sorted(sizes[sizes > 1].tolist())
+    xo, vo = oracle.step_hybrid_bs(w.m, w.x, vd, p, w.dt, tol=1e-13)
+    xl, vl = oracle.step(w.m, w.x, vd, p, w.dt)
+    assert state_err(xl, vl, xo, vo) > 1e-6                     # the complement matters for the chains
+    for prec, kw, tol in ((B.FP64, dict(), 1e-10), (B.FP32, dict(), 1e-7), (B.FP64, dict(enc_tol=1e-13), 1e-10)):
+        g = hybrid(w, **kw)
+        g.step(w.dt, prec)
+        x, v = (t.cpu().numpy() for t in g.get_state())
+        groups, bodies, largest, missed, status = g.encounter_stats()
+        g.close()
+        assert status == 0 and missed == 0 and largest >= 60 and bodies >= 100, (groups, bodies, largest, missed, status)
+        assert state_err(x, v, xo, vo) <= tol, (prec, kw, state_err(x, v, xo, vo))
+    # the RK4 scheme through the same teams: the first oracle with the same substeps
+    xr, vr = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=64)
+    g = hybrid(w, enc_nsub=64)
     g.step(w.dt, B.FP64)
-    assert g.encounter_stats()[4] == 8
+    x, v = (t.cpu().numpy() for t in g.get_state())
     g.close()
+    assert state_err(x, v, xr, vr) <= 1e-10
+
+
+def test_bs_steps_through_a_close_encounter_match_the_oracle():
+    w = encounter_system()
+    p = oparams(w)
+    xo, vo = w.x.copy(), oracle.to_democratic(w.m, w.v, w.M_star)
+    E0 = oracle.energy_angmom(w.m, xo, vo, oracle.Params(n1=0.0))[0]
+    g = hybrid(w)                                                # Bulirsch-Stoer, tolerance 1e-12
+    worst, grouped = 0.0, 0
+    for _ in range(30):
+        xo, vo = oracle.step_hybrid_bs(w.m, xo, vo, p, w.dt, tol=1e-13)
+        g.step(w.dt, B.FP64)
+        x, v = (t.cpu().numpy() for t in g.get_state())
+        st = g.encounter_stats()
+        assert st[3] == 0 and st[4] == 0
+        grouped += st[0]
+        worst = max(worst, state_err(x, v, xo, vo))
+    E, _ = g.energy_angmom()
+    g.close()
+    assert grouped >= 5 and worst <= 1e-10, (grouped, worst)
+    assert abs(E / E0 - 1) < 1e-6
 
 
 def test_leapfrog_as_the_first_call_builds_its_own_pair_list():
