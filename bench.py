@@ -545,7 +545,7 @@ def run_report(args):
     # NEXT-1: the hybrid step (encounter mode, reading R11) on the performance shape, 200 steps
     w5 = W.config(4)
     w5.nsteps = 200
-    hyb = {"weight_mode": 1, "encounter_mode": 1, "enc_nsub": 256, "enc_list_scale": 8.0, "enc_list_vfactor": 1.25}
+    hyb = {"weight_mode": 1, "encounter_mode": 1, "enc_list_scale": 8.0, "enc_list_vfactor": 1.25}   # groups: Bulirsch-Stoer, tol 1e-12
     cases.append(("4-hybrid", w5, dict(hyb, cand_capacity=64 * w5.N)))
     for c in (1, 2, 3):                                            # ... and on the paper-shaped configs, full length
         wc = W.config(c)
@@ -578,6 +578,7 @@ def run_report(args):
             enc_last = int(len(g.encounter_pairs(cap=max(8 * w.N + 4096, kw.get("pair_capacity", 0)))))
             st = g.nearfield_stats()
             enc_stats = g.encounter_stats() if kw.get("encounter_mode") else None    # missed / status: since the warm-up
+            enc_work = g.encounter_work() if kw.get("encounter_mode") else None
             g.close()
             evals = w.nsteps + 1
             line = {"report": "config", "config": cfg, "workload": w.name, "N": w.N, "dt_days": w.dt, "steps": w.nsteps,
@@ -593,7 +594,9 @@ def run_report(args):
                     "clocks": sampler.summary()}
             if enc_stats is not None:
                 line["encounter_groups_last_drift"] = {"groups": enc_stats[0], "bodies": enc_stats[1], "largest": enc_stats[2],
-                                                       "missed_pairs_whole_run": enc_stats[3], "status": enc_stats[4], "rk4_substeps": kw.get("enc_nsub"),
+                                                       "missed_pairs_whole_run": enc_stats[3], "status": enc_stats[4],
+                                                       "integrator": (f"RK4 x {kw['enc_nsub']}" if kw.get("enc_nsub") else f"Bulirsch-Stoer tol {kw.get('enc_tol', 1e-12):g}"),
+                                                       "rhs_total_max_rejected_last_drift": enc_work,
                                                        "list_scale": kw.get("enc_list_scale"), "list_vfactor": kw.get("enc_list_vfactor")}
             if cfg == 1:                                           # encounter-pair counts per step (untimed second run)
                 g = B.from_workload(w, **kw)

@@ -235,6 +235,11 @@ int genga_nearfield_stats(genga_handle h, long long* candidates, int* overflowed
  * params.encounter_mode = 1.                                                                          */
 int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest, int* missed_pairs, int* status);
 
+/* Encounter mode: the work of the group integrations of the LAST drift: force evaluations
+ * summed over all groups, the most any one group needed (the drift waits for that group) and the Bulirsch-Stoer
+ * macro steps that were rejected.  HOST pointers (any may be NULL); synchronises.  GENGA_EINVAL outside encounter mode. */
+int genga_encounter_work(genga_handle h, long long* rhs_total, int* rhs_max, int* rejected);
+
 /* Per-kernel device timing.  enable is a bit mask: bit k brackets every launch of kernel class k with
  * CUDA events on params.stream; classes: 0 all-pairs kick kernel, 1 near-field kernel, 2 prep kernel,
  * 3 drift kernel (15 = all, 0 = off).  genga_kernel_time returns, for class which, the summed

@@ -27,7 +27,7 @@ SYMBOLS = [
     "genga_sunkick", "genga_step", "genga_run", "genga_leapfrog", "genga_encounter_pairs", "genga_energy_angmom",
     "genga_get_state", "genga_get_state_host", "genga_get_accel", "genga_get_rcrit",
     "genga_set_radii", "genga_get_radii", "genga_merge", "genga_get_mass", "genga_num_bodies", "genga_num_big_bodies",
-    "genga_nearfield_stats", "genga_encounter_stats", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
+    "genga_nearfield_stats", "genga_encounter_stats", "genga_encounter_work", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
     "genga_synchronize", "genga_strerror", "genga_last_cuda_error", "genga_version",
     "genga_peak_probe", "genga_set_tuning", "genga_autotune", "genga_num_variants", "genga_variant_name",
 ]
@@ -95,6 +95,7 @@ def load() -> ctypes.CDLL:
     L.genga_num_big_bodies.argtypes = [vp]
     L.genga_nearfield_stats.argtypes = [vp, llp, ip]
     L.genga_encounter_stats.argtypes = [vp, ip, ip, ip, ip, ip]
+    L.genga_encounter_work.argtypes = [vp, llp, ip, ip]
     L.genga_set_profiling.argtypes = [vp, ctypes.c_int]
     L.genga_kernel_time.argtypes = [vp, ctypes.c_int, dp, llp, ctypes.c_int]
     L.genga_launch_count.argtypes = [vp]; L.genga_launch_count.restype = ctypes.c_longlong
@@ -335,6 +336,13 @@ class Genga:
         _check(self._L.genga_encounter_stats(self._h, ctypes.byref(g), ctypes.byref(b), ctypes.byref(l), ctypes.byref(m),
                                              ctypes.byref(s)), "genga_encounter_stats")
         return int(g.value), int(b.value), int(l.value), int(m.value), int(s.value)
+
+    def encounter_work(self):
+        """Encounter mode: (force evaluations of all group integrations of the last drift, the most any group needed,
+        rejected Bulirsch-Stoer macro steps)."""
+        t, mx, rj = ctypes.c_longlong(0), ctypes.c_int(0), ctypes.c_int(0)
+        _check(self._L.genga_encounter_work(self._h, ctypes.byref(t), ctypes.byref(mx), ctypes.byref(rj)), "genga_encounter_work")
+        return int(t.value), int(mx.value), int(rj.value)
 
     def set_profiling(self, enable=True):
         """enable: True (all kernel classes), False, or a bit mask (1 kick, 2 near field, 4 prep, 8 drift)."""

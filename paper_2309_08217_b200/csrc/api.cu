@@ -711,6 +711,21 @@ int genga_encounter_stats(genga_handle h, int* groups, int* bodies, int* largest
     return GENGA_OK;
 }
 
+int genga_encounter_work(genga_handle h, long long* rhs_total, int* rhs_max, int* rejected)
+{
+    if (!h || h->p.encounter_mode != 1) return GENGA_EINVAL;
+    Counters c;
+    std::memset(&c, 0, sizeof(c));
+    if (h->N) {
+        CU(cudaMemcpyAsync(&c, h->w.ctr, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    if (rhs_total) *rhs_total = (long long)c.enc_rhs_sum;
+    if (rhs_max) *rhs_max = (int)c.enc_rhs_max;
+    if (rejected) *rejected = (int)c.enc_rejected;
+    return GENGA_OK;
+}
+
 int genga_set_profiling(genga_handle h, int enable)
 {
     if (!h) return GENGA_EINVAL;

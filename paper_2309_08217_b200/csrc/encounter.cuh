@@ -17,7 +17,9 @@
 // once and sums over the other members.  Integrators (the choice is params.enc_nsub):
 //   * Gragg-Bulirsch-Stoer extrapolation to the relative tolerance params.enc_tol (default, reading R15): modified
 //     midpoint with 2, 4, .. 16 substeps, polynomial extrapolation in h^2, error = largest |dx|/|x|, |dv|/|v| over
-//     the members; a step that does not converge in 8 rows is halved.  Status bit 8: the step size collapsed.
+//     the members; a step that does not converge in 8 rows, or whose corrections stop falling (a pair crossing the
+//     edge of its zone, where K is only C^1), is cut to a quarter; a step that converged in few rows is followed by
+//     a longer one.  Status bit 8: the step size collapsed.
 //   * classical RK4 with enc_nsub equal substeps (the scheme of the first oracle, oracle_step_hybrid).
 #pragma once
 
@@ -123,8 +125,12 @@ __device__ __forceinline__ void accel(const Team& T, const EncParams& P, int& bu
         const double ir3 = -mu * fma(g * e, fma(1.875, e, 1.5), g);         // -mu / r^3
         a0 = x * ir3; a1 = y * ir3; a2 = z * ir3;
     }
-    for (int l = 0; l < T.n; ++l) {
-        const double i09 = (l == T.k) ? 0.0 : T.inv09(P, l);
+    // the other members, starting with the next one (member k takes l = k + 1, k + 2, .. cyclically): a pair costs
+    // one pass of this dependent chain, which is what the drift's duration is made of
+#pragma unroll 2
+    for (int j = 1; j < T.n; ++j) {
+        const int l = (T.k + j < T.n) ? T.k + j : T.k + j - T.n;
+        const double i09 = T.inv09(P, l);
         const double d0 = X[l] - x, d1 = Y[l] - y, d2 = Z[l] - z;
         const double q2 = fma(d2, d2, fma(d1, d1, d0 * d0));
         const bool   on = (i09 > 0.0) && (q2 > 0.0);
@@ -146,7 +152,7 @@ __device__ __forceinline__ void accel(const Team& T, const EncParams& P, int& bu
 
 // A(dt) by classical RK4 with nsub equal substeps (oracle_step_hybrid's scheme, restricted to the group).
 template <class Team>
-__device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P, double dt, double (&y)[6])
+__device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr)
 {
     const double h = dt / P.nsub, hh = 0.5 * h, h6 = h / 6.0;
     int buf = 0;
@@ -168,23 +174,27 @@ __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P,
         y[0] = fma(h6, sx[0] + u[0], y[0]); y[1] = fma(h6, sx[1] + u[1], y[1]); y[2] = fma(h6, sx[2] + u[2], y[2]);
         y[3] = fma(h6, sv[0] + k0, y[3]); y[4] = fma(h6, sv[1] + k1, y[4]); y[5] = fma(h6, sv[2] + k2, y[5]);
     }
+    if (T.k == 0) { atomicAdd(&ctr->enc_rhs_sum, 4u * (unsigned int)P.nsub); atomicMax(&ctr->enc_rhs_max, 4u * (unsigned int)P.nsub); }
 }
 
 // A(dt) by Gragg-Bulirsch-Stoer extrapolation to the relative tolerance P.tol (reading R15).  The tableau is kept in
 // the difference form of polynomial extrapolation (one column of differences per row), which yields the extrapolated
 // value and the last correction, i.e. the error estimate T_kk - T_k,k-1, without storing two rows.
 template <class Team>
-__device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, double dt, double (&y)[6], unsigned int* status)
+__device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr)
 {
     const double Tabs = fabs(dt);
     double t = 0.0, H = dt;
     int buf = 0;
     bool collapsed = false;
+    unsigned int nrhs = 0u, nrej = 0u;
     while (fabs(t) < Tabs * (1.0 - 1.0e-14)) {
         if (fabs(t + H) > Tabs) H = dt - t;
         double f0[3];
         accel(T, P, buf, y[0], y[1], y[2], f0[0], f0[1], f0[2]);
+        ++nrhs;
         double d[KMAX][6], hsq[KMAX], yz[6], dy[6];
+        double eprev = 1.0e300;
         int done = -1;
         for (int k = 0; k < KMAX && done < 0; ++k) {
             const int nk = 2 * (k + 1);
@@ -201,6 +211,7 @@ __device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, 
                 }
             }
             accel(T, P, buf, z1[0], z1[1], z1[2], f[0], f[1], f[2]);
+            nrhs += (unsigned int)nk;
             double est[6];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
@@ -241,27 +252,35 @@ __device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, 
                 }
                 e = T.maxall(e);
                 if (e <= P.tol * P.tol) done = k;         // squared norms against the squared tolerance
+                // A pair that crosses the edge of its zone inside the step (K is C^1 there) makes the corrections
+                // stagnate instead of falling row by row: give the step up early rather than after all 8 rows.
+                else if (k >= 3 && e > 0.04 * eprev) k = KMAX;
+                eprev = e;
             }
         }
         if (done < 0) {
-            H *= 0.5;
+            ++nrej;
+            H *= 0.25;
             if (fabs(H) < Tabs * 9.3e-10) { collapsed = true; break; }      // dt 2^-30: give up, keep the last accepted state
             continue;
         }
 #pragma unroll
         for (int c = 0; c < 6; ++c) y[c] = yz[c];
         t += H;
-        H = (done <= 3) ? 2.0 * H : ((done <= 5) ? H : 0.5 * H);
+        H = (done <= 2) ? 4.0 * H : ((done <= 4) ? 2.0 * H : ((done <= 5) ? H : 0.5 * H));
     }
-    if (collapsed && T.k == 0) atomicOr(status, 8u);
+    if (T.k == 0) {
+        if (collapsed) atomicOr(&ctr->enc_status, 8u);
+        atomicAdd(&ctr->enc_rhs_sum, nrhs); atomicMax(&ctr->enc_rhs_max, nrhs); atomicAdd(&ctr->enc_rejected, nrej);
+    }
 }
 
 template <class Team>
-__device__ __forceinline__ void integrate(const Team& T, const EncParams& P, double dt, double (&y)[6], unsigned int* status)
+__device__ __forceinline__ void integrate(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr)
 {
     if (dt == 0.0) return;
-    if (P.nsub > 0) integrate_rk4(T, P, dt, y);
-    else            integrate_bs(T, P, dt, y, status);
+    if (P.nsub > 0) integrate_rk4(T, P, dt, y, ctr);
+    else            integrate_bs(T, P, dt, y, ctr);
 }
 
 // Groups in Workspace::ginfo (written by group_kernel): ginfo[2 g] = offset of the member list, ginfo[2 g + 1] = member
@@ -307,7 +326,7 @@ __device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, War
     if (active) slab.gm[lane] = P.G * m;
     __syncwarp();
     const WarpTeam T{slab, n, active ? lane : -1};
-    integrate(T, P, dt, y, &w.ctr->enc_status);
+    integrate(T, P, dt, y, w.ctr);
     if (active) {
         w.x[3 * b] = y[0]; w.x[3 * b + 1] = y[1]; w.x[3 * b + 2] = y[2];
         w.v[3 * b] = y[3]; w.v[3 * b + 1] = y[4]; w.v[3 * b + 2] = y[5];
@@ -340,7 +359,7 @@ __device__ __forceinline__ void block_group(const EncParams& P, Workspace& w, Bl
     }
     __syncthreads();
     const BlockTeam T{slab, n, active ? tid : -1};
-    integrate(T, P, dt, y, &w.ctr->enc_status);
+    integrate(T, P, dt, y, w.ctr);
     if (active) {
         w.x[3 * b] = y[0]; w.x[3 * b + 1] = y[1]; w.x[3 * b + 2] = y[2];
         w.v[3 * b] = y[3]; w.v[3 * b + 1] = y[4]; w.v[3 * b + 2] = y[5];

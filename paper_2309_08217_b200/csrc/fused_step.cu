@@ -36,6 +36,7 @@ group_kernel(int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr,
     if (threadIdx.x == 0) {
         if (total > pair_cap) atomicOr(&ctr->enc_status, 1u);               // list overflowed: groups incomplete
         ctr->enc_groups = 0u; ctr->enc_bodies = 0u; ctr->enc_maxsize = 0u;
+        ctr->enc_rhs_sum = 0u; ctr->enc_rhs_max = 0u; ctr->enc_rejected = 0u;
     }
     if (n == 0) return;
     // the bodies that occur in a pair, each once (gcount is preset to -1 like the labels): every later pass

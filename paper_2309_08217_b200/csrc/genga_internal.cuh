@@ -49,6 +49,9 @@ struct Counters {
     unsigned int enc_bodies;     // bodies in those groups
     unsigned int enc_maxsize;    // largest group of the last drift
     unsigned int enc_missed;     // sticky until read: pairs found inside their zone after a drift that had not grouped them
+    unsigned int enc_rhs_sum;    // force evaluations of the group integrations of the last drift: all groups, ...
+    unsigned int enc_rhs_max;    // ... the most any group needed (the drift waits for that group), ...
+    unsigned int enc_rejected;   // ... and Bulirsch-Stoer macro steps that were rejected
     // mergers (merge.cu; NEXT-4): written by the last genga_merge
     unsigned int merge_n;        // body count after the pass
     unsigned int merge_status;   // 1 pair list had overflowed, 2 a radius exceeds half its critical radius
