@@ -131,6 +131,14 @@ typedef struct {
                                  (reading R15): a macro step is accepted when the last extrapolation
                                  correction of every member is below enc_tol in |dx|/|x| and |dv|/|v|; <= 0: default 1e-12.
                                  genga_encounter_stats status bit 8: the step size collapsed (dt 2^-30) without convergence  */
+    int    enc_collide;       /* reading R14 ("collisions ... perfect mergers"), opt-in; needs encounter_mode = 1 and
+                                 enc_nsub > 0 (else GENGA_EINVAL).  1: after every RK4 substep of a group's integration its
+                                 members are tested for r_kl < R_k + R_l (genga_set_radii) and every connected component of
+                                 overlapping bodies becomes one body at its smallest index on the spot (m, centre of mass,
+                                 momentum and sum R^3 kept; the merged body keeps the frozen r_crit,i, a_i, v_K,i of that
+                                 index), which is how bodies that pass through each other WITHIN a step are caught.  The
+                                 absorbed bodies stay in the arrays as massless bodies of radius -1e300 until the next
+                                 genga_merge closes the arrays up (its newidx and n_merged account for them).            */
 } genga_params;
 
 /* Fill *p with the defaults: G = k^2 (k = 0.01720209895), M_star = 1, n1 = 3, n2 = 0,

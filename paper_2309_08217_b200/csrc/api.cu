@@ -54,6 +54,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_gu = take(std::min(2 * (size_t)pair_cap, NP) * 4);
     const size_t o_rad = take(NP * 8);
     const size_t o_as = take(NP * 24);
+    const size_t o_ab = take(NP * 4);
     if (w && base) {
         char* b = static_cast<char*>(base);
         w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
@@ -69,6 +70,7 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
         w->glabel = (int*)(b + o_gl); w->ginfo = (int*)(b + o_gi); w->gulist = (int*)(b + o_gu);
         w->radius = (double*)(b + o_rad);
         w->aslot = (double*)(b + o_as);
+        w->absorb = (int*)(b + o_ab);
     }
     return off;
 }
@@ -190,6 +192,7 @@ static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_d
     a.enc.pair_cap = (unsigned int)h->pair_cap;
     a.enc.G = h->p.G; a.enc.M_star = h->p.M_star; a.enc.n1 = h->p.n1; a.enc.n2dt = h->p.n2 * h->p.dt_rcrit;
     a.enc.tol = h->p.enc_tol;
+    a.enc.collide = h->p.enc_collide;
     a.enc.maxgroups = (int)std::min((size_t)h->pair_cap, (size_t)h->NP / 2);
     cudaError_t e;
     if (enc) {                                         // groups of the pair list the last force evaluation left
@@ -350,7 +353,7 @@ void genga_default_params(genga_params* p)
     p->chunk = 0;
     p->mega_nmax = 0;
     p->weight_mode = 0;
-    p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0; p->enc_list_vfactor = 0.0; p->enc_tol = 0.0;
+    p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0; p->enc_list_vfactor = 0.0; p->enc_tol = 0.0; p->enc_collide = 0;
 }
 
 size_t genga_workspace_bytes(int N, const genga_params* p)
@@ -369,6 +372,7 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     if (p->weight_mode != 0 && p->weight_mode != 1) return GENGA_EINVAL;
     if (p->encounter_mode != 0 && p->encounter_mode != 1) return GENGA_EINVAL;
     if (p->encounter_mode == 1 && (p->weight_mode != 1 || (p->n_big >= 0 && p->n_big < N) || p->no_fused_step)) return GENGA_EINVAL;
+    if (p->enc_collide != 0 && (p->enc_collide != 1 || p->encounter_mode != 1 || p->enc_nsub <= 0)) return GENGA_EINVAL;
     *out = nullptr;
     int pc, cc;
     resolve_caps(N, p, &pc, &cc);
@@ -419,6 +423,7 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     carve_workspace(N, pc, cc, p->workspace, &h->w);
 
     cudaError_t e = cudaMemsetAsync(p->workspace, 0, need, h->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->w.absorb, 0xff, (size_t)h->NP * sizeof(int), h->stream);   // -1: nobody absorbed
     if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaMemsetAsync(workspace)"); }
     launch_pad(h);
     ++h->launches;

@@ -20,7 +20,9 @@
 //     the members; a step that does not converge in 8 rows, or whose corrections stop falling (a pair crossing the
 //     edge of its zone, where K is only C^1), is cut to a quarter; a step that converged in few rows is followed by
 //     a longer one.  Status bit 8: the step size collapsed.
-//   * classical RK4 with enc_nsub equal substeps (the scheme of the first oracle, oracle_step_hybrid).
+//   * classical RK4 with enc_nsub equal substeps (the scheme of the first oracle, oracle_step_hybrid); with
+//     params.enc_collide the members are tested for collisions after every substep and merged on the spot
+//     (reading R14, oracle_step_hybrid_collide).
 #pragma once
 
 #include "genga_internal.cuh"
@@ -53,14 +55,19 @@ __device__ __forceinline__ double rcp_seed(double a) { double r; asm("rcp.approx
 // ---- shared memory of the teams ----------------------------------------------------------------------------------
 struct WarpSlab {
     double pos[2][3][WMAX];        // stage positions of the members, double buffered
-    double gm[WMAX];
-    double i09[WMAX][WMAX];        // [l][k] = 1 / (0.9 r_crit,kl), 0: no zone (k == l, idle slots)
+    double gm[WMAX], m[WMAX], rc[WMAX], sa[WMAX], vk[WMAX];   // rc < 0: the member was absorbed by a merger (reading R14)
+    double i09[WMAX][WMAX];        // [l][k] = 1 / (0.9 r_crit,kl), 0: no zone (k == l, idle slots, absorbed members)
+    double rad[WMAX], sum[8][WMAX];                          // collisions: radii, (m, m x, m v, R^3) of the members
+    int    lab[WMAX], body[WMAX];
+    __device__ __forceinline__ int body_of(int l) const { return body[l]; }
 };
 struct BlockSlab {
     double pos[2][3][GBIG];
     double gm[GBIG], m[GBIG], rc[GBIG], sa[GBIG], vk[GBIG];
+    double rad[GBIG], sum[8][GBIG];
     double red[8];
-    int    body[GBIG];
+    int    body[GBIG], lab[GBIG];
+    __device__ __forceinline__ int body_of(int l) const { return body[l]; }
 };
 union EncSmem { WarpSlab w[8]; BlockSlab b; };     // warp teams and the CTA team never run at the same time
 
@@ -78,6 +85,18 @@ struct WarpTeam {
     __device__ __forceinline__ double* pz(int b) const { return s.pos[b][2]; }
     __device__ __forceinline__ double gm(int l) const { return s.gm[l]; }
     __device__ __forceinline__ double inv09(const EncParams&, int l) const { return s.i09[l][k]; }
+    // rebuild the pair table from the members' (possibly merged) masses; absorbed members have no zones
+    __device__ __forceinline__ void refresh_pairs(const EncParams& P) const
+    {
+        __syncwarp();
+        if (k >= 0)
+            for (int l = 0; l < n; ++l) {
+                const bool pair = (l != k) && s.rc[k] >= 0.0 && s.rc[l] >= 0.0;
+                const double rc = pair ? pair_rcrit(P, s.m[k], s.m[l], s.rc[k], s.rc[l], s.sa[k], s.sa[l], s.vk[k], s.vk[l]) : 0.0;
+                s.i09[l][k] = (rc > 0.0) ? 1.0 / (0.9 * rc) : 0.0;
+            }
+        __syncwarp();
+    }
 };
 struct BlockTeam {
     BlockSlab& s; int n, k;
@@ -100,10 +119,80 @@ struct BlockTeam {
     __device__ __forceinline__ double gm(int l) const { return s.gm[l]; }
     __device__ __forceinline__ double inv09(const EncParams& P, int l) const
     {
+        if (s.rc[k] < 0.0 || s.rc[l] < 0.0) return 0.0;     // absorbed by a merger
         const double rc = pair_rcrit(P, s.m[k], s.m[l], s.rc[k], s.rc[l], s.sa[k], s.sa[l], s.vk[k], s.vk[l]);
         return (rc > 0.0) ? 1.0 / (0.9 * rc) : 0.0;
     }
+    __device__ __forceinline__ void refresh_pairs(const EncParams&) const { __syncthreads(); }   // recomputed per pair anyway
 };
+
+// ---- reading R14: collisions inside the encounter integration ("perfect mergers") ----------------------
+// After a substep the members publish their positions; members k, l collide iff |x_k - x_l| < R_k + R_l (strict,
+// plain sqrt as in oracle_merge).  Every connected component of that graph becomes one body at its smallest member
+// (= smallest body index: members sit in ascending order): m = sum m, x = sum m x / m, v = sum m v / m,
+// R = cbrt(sum R^3); a component of total mass 0 keeps its first member's x, v.  The absorbed members go on as
+// massless bodies without zones (they exert and feel nothing but the star) until genga_merge closes the arrays up;
+// absorb[body] names the body that took them.  Returns true if anything merged (uniform over the team).
+template <class Team>
+__device__ __forceinline__ bool collision_pass(const Team& T, const EncParams& P, int& buf, double (&y)[6], double& m,
+                                               double& R, int body, int* __restrict__ absorb, Counters* ctr)
+{
+    double* X = T.px(buf); double* Y = T.py(buf); double* Z = T.pz(buf);
+    const int k = T.k;
+    const bool alive = k >= 0 && T.s.rc[k] >= 0.0;
+    if (k >= 0) { X[k] = y[0]; Y[k] = y[1]; Z[k] = y[2]; T.s.rad[k] = alive ? R : -1.0; T.s.lab[k] = alive ? k : -1; }
+    T.sync();
+    buf ^= 1;
+    auto touches = [&](int l) {
+        if (l == k || T.s.rad[l] < 0.0) return false;
+        const double dx = X[l] - y[0], dy = Y[l] - y[1], dz = Z[l] - y[2];
+        return sqrt(dx * dx + dy * dy + dz * dz) < R + T.s.rad[l];
+    };
+    bool hit = false;
+    if (alive) for (int l = 0; l < T.n; ++l) hit = hit || touches(l);
+    if (!(T.maxall(hit ? 1.0 : 0.0) > 0.0)) return false;          // the usual substep
+    // components by label propagation (labels = member indices)
+    for (;;) {
+        int lab = alive ? T.s.lab[k] : -1, nl = lab;
+        if (alive) for (int l = 0; l < T.n; ++l) if (touches(l)) nl = min(nl, T.s.lab[l]);
+        const bool changed = T.maxall(nl != lab ? 1.0 : 0.0) > 0.0;  // (team-wide sync inside for the CTA team)
+        T.sync();
+        if (alive) T.s.lab[k] = nl;
+        T.sync();
+        if (!changed) break;
+    }
+    if (k >= 0) {
+        T.s.sum[0][k] = m; T.s.sum[1][k] = m * y[0]; T.s.sum[2][k] = m * y[1]; T.s.sum[3][k] = m * y[2];
+        T.s.sum[4][k] = m * y[3]; T.s.sum[5][k] = m * y[4]; T.s.sum[6][k] = m * y[5]; T.s.sum[7][k] = R * R * R;
+    }
+    T.sync();
+    if (alive) {
+        const int root = T.s.lab[k];
+        if (root == k) {
+            int members = 0;
+            double a[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            for (int l = k; l < T.n; ++l)
+                if (T.s.lab[l] == k) { ++members; for (int c = 0; c < 8; ++c) a[c] += T.s.sum[c][l]; }
+            if (members > 1) {
+                if (a[0] > 0.0) { for (int c = 0; c < 3; ++c) { y[c] = a[1 + c] / a[0]; y[3 + c] = a[4 + c] / a[0]; } }
+                m = a[0];
+                R = cbrt(a[7]);
+                atomicAdd(&ctr->enc_merged, (unsigned int)(members - 1));
+            }
+        } else {                                                    // absorbed by member `root`
+            absorb[body] = T.s.body_of(root);
+            m = 0.0; R = -1.0e300;                                  // never touches anything again
+        }
+    }
+    T.sync();
+    if (k >= 0) {
+        const bool gone = alive && T.s.lab[k] != k;
+        T.s.m[k] = m; T.s.gm[k] = P.G * m;
+        if (gone) T.s.rc[k] = -1.0;
+    }
+    T.refresh_pairs(P);
+    return true;
+}
 
 // dv/dt of this thread's member at the stage position (x, y, z): the member publishes its position in buffer buf,
 // the team synchronises once, every member sums the Kepler term and the complement terms of the other members.
@@ -151,8 +240,10 @@ __device__ __forceinline__ void accel(const Team& T, const EncParams& P, int& bu
 }
 
 // A(dt) by classical RK4 with nsub equal substeps (oracle_step_hybrid's scheme, restricted to the group).
+// P.collide: after every substep the collision pass of reading R14 (m, R: this member's mass and radius, updated).
 template <class Team>
-__device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr)
+__device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
+                                              double& m, double& R, int body, int* __restrict__ absorb)
 {
     const double h = dt / P.nsub, hh = 0.5 * h, h6 = h / 6.0;
     int buf = 0;
@@ -173,6 +264,7 @@ __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P,
         accel(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
         y[0] = fma(h6, sx[0] + u[0], y[0]); y[1] = fma(h6, sx[1] + u[1], y[1]); y[2] = fma(h6, sx[2] + u[2], y[2]);
         y[3] = fma(h6, sv[0] + k0, y[3]); y[4] = fma(h6, sv[1] + k1, y[4]); y[5] = fma(h6, sv[2] + k2, y[5]);
+        if (P.collide) collision_pass(T, P, buf, y, m, R, body, absorb, ctr);
     }
     if (T.k == 0) { atomicAdd(&ctr->enc_rhs_sum, 4u * (unsigned int)P.nsub); atomicMax(&ctr->enc_rhs_max, 4u * (unsigned int)P.nsub); }
 }
@@ -276,10 +368,11 @@ __device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, 
 }
 
 template <class Team>
-__device__ __forceinline__ void integrate(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr)
+__device__ __forceinline__ void integrate(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
+                                          double& m, double& R, int body, int* __restrict__ absorb)
 {
     if (dt == 0.0) return;
-    if (P.nsub > 0) integrate_rk4(T, P, dt, y, ctr);
+    if (P.nsub > 0) integrate_rk4(T, P, dt, y, ctr, m, R, body, absorb);
     else            integrate_bs(T, P, dt, y, ctr);
 }
 
@@ -315,21 +408,18 @@ __device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, War
         y[3] = w.v[3 * b]; y[4] = w.v[3 * b + 1]; y[5] = w.v[3 * b + 2];
     }
     __syncwarp();                                           // the slab may still be read by the previous group's last sum
-    for (int l = 0; l < n; ++l) {
-        const double ml = __shfl_sync(FULL, m, l), rcl = __shfl_sync(FULL, rci, l), sal = __shfl_sync(FULL, sa, l),
-                     vkl = __shfl_sync(FULL, vk, l);
-        if (active) {
-            const double rc = (l != lane) ? pair_rcrit(P, m, ml, rci, rcl, sa, sal, vk, vkl) : 0.0;
-            slab.i09[l][lane] = (rc > 0.0) ? 1.0 / (0.9 * rc) : 0.0;
-        }
+    double R = 0.0;
+    if (active) {
+        slab.m[lane] = m; slab.gm[lane] = P.G * m; slab.rc[lane] = rci; slab.sa[lane] = sa; slab.vk[lane] = vk; slab.body[lane] = b;
+        if (P.collide) R = w.radius[b];
     }
-    if (active) slab.gm[lane] = P.G * m;
-    __syncwarp();
     const WarpTeam T{slab, n, active ? lane : -1};
-    integrate(T, P, dt, y, w.ctr);
+    T.refresh_pairs(P);
+    integrate(T, P, dt, y, w.ctr, m, R, b, w.absorb);
     if (active) {
         w.x[3 * b] = y[0]; w.x[3 * b + 1] = y[1]; w.x[3 * b + 2] = y[2];
         w.v[3 * b] = y[3]; w.v[3 * b + 1] = y[4]; w.v[3 * b + 2] = y[5];
+        if (P.collide) { w.m[b] = m; w.radius[b] = R; w.hcbrt[b] = cbrt(m / (3.0 * P.M_star)); }
     }
 }
 
@@ -349,20 +439,24 @@ __device__ __forceinline__ void block_group(const EncParams& P, Workspace& w, Bl
     __syncthreads();
     const bool active = tid < n;
     double y[6] = {1.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    double mm = 0.0, R = 0.0;
     int b = -1;
     if (active) {
         b = slab.body[tid];
         const double m = w.m[b];
         slab.m[tid] = m; slab.gm[tid] = P.G * m; slab.rc[tid] = w.rcrit[b]; slab.sa[tid] = w.semi[b]; slab.vk[tid] = w.vkep[b];
+        mm = m;
+        if (P.collide) R = w.radius[b];
         y[0] = w.x[3 * b] + s0; y[1] = w.x[3 * b + 1] + s1; y[2] = w.x[3 * b + 2] + s2;
         y[3] = w.v[3 * b]; y[4] = w.v[3 * b + 1]; y[5] = w.v[3 * b + 2];
     }
     __syncthreads();
     const BlockTeam T{slab, n, active ? tid : -1};
-    integrate(T, P, dt, y, w.ctr);
+    integrate(T, P, dt, y, w.ctr, mm, R, b, w.absorb);
     if (active) {
         w.x[3 * b] = y[0]; w.x[3 * b + 1] = y[1]; w.x[3 * b + 2] = y[2];
         w.v[3 * b] = y[3]; w.v[3 * b + 1] = y[4]; w.v[3 * b + 2] = y[5];
+        if (P.collide) { w.m[b] = mm; w.radius[b] = R; w.hcbrt[b] = cbrt(mm / (3.0 * P.M_star)); }
     }
     __syncthreads();
 }

@@ -49,6 +49,7 @@ struct Counters {
     unsigned int enc_bodies;     // bodies in those groups
     unsigned int enc_maxsize;    // largest group of the last drift
     unsigned int enc_missed;     // sticky until read: pairs found inside their zone after a drift that had not grouped them
+    unsigned int enc_merged;     // bodies absorbed by mergers inside the encounter integration since the last genga_merge (reading R14)
     unsigned int enc_rhs_sum;    // force evaluations of the group integrations of the last drift: all groups, ...
     unsigned int enc_rhs_max;    // ... the most any group needed (the drift waits for that group), ...
     unsigned int enc_rejected;   // ... and Bulirsch-Stoer macro steps that were rejected
@@ -92,6 +93,7 @@ struct Workspace {
     double*  vtmp;    // [NP][3] staging for heliocentric-velocity output
     double*  mom;     // momentum slots and per-block partials of the fused step (momentum.cuh)
     double*  radius;  // [NP] physical radii R_i (genga_set_radii; 0 = the body never collides)
+    int*     absorb;  // [NP] reading R14: body that absorbed this one inside an encounter integration (-1: none); genga_merge closes up
     double*  aslot;   // [3][NP] sums of the symmetric all-pairs kernels in the internal order (kick_sym_body.cuh: aslot_index),
                       //         zeroed by the prep step, folded into a[] by the near-field kernel
     Counters* ctr;
@@ -155,6 +157,7 @@ struct EncArgs {                  // encounter mode (encounter.cuh; NEXT-1, read
     unsigned int pair_cap;
     double G, M_star, n1, n2dt;
     double tol;                    // nsub <= 0: relative tolerance of the Bulirsch-Stoer integration (encounter.cuh)
+    int collide;                   // RK4 only: collision pass after every substep (reading R14)
     int maxgroups;                 // layout of Workspace::ginfo: [2 maxgroups] (offset, count) per group, then the member lists
 };
 struct OnBodyArgs {               // the fused per-body kernel of the step (fused_step.cu)

@@ -23,13 +23,17 @@ constexpr int MERGE_THREADS = 1024;
 
 // label[i] = i, flag[i] = 0; status bit 2 if a body's radius exceeds half its critical radius (then the encounter
 // list need not contain every colliding pair).
+// A body absorbed by a merger inside an encounter integration (reading R14: absorb[i] >= 0, possibly a chain) starts
+// with the label of the body that took it, so that the compaction below removes it and newidx maps it there.
 __global__ void merge_init_kernel(int N, const double* __restrict__ R, const double* __restrict__ rcrit,
                                   int* __restrict__ label, int* __restrict__ flag, int* __restrict__ newidx,
-                                  unsigned int* __restrict__ status)
+                                  unsigned int* __restrict__ status, const int* __restrict__ absorb)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
-    label[i] = i;
+    int r = i;
+    while (absorb[r] >= 0) r = absorb[r];
+    label[i] = r;
     flag[i] = 0;
     if (newidx) newidx[i] = i;                 // what it stays when nothing collides (the usual step)
     if (R[i] > 0.0 && !(2.0 * R[i] <= rcrit[i])) atomicOr(status, 2u);
@@ -65,7 +69,7 @@ merge_kernel(int N, unsigned int pair_cap, const int2* __restrict__ pairs, Count
     if (np > pair_cap) { np = pair_cap; if (t == 0) atomicOr(&out[1], 1u); }      // list overflowed: pairs may be missing
 
     // 0 ---- the usual step: no listed pair overlaps, nothing to do (newidx is the identity already)
-    if (t == 0) s_any = 0;
+    if (t == 0) s_any = ctr->enc_merged ? 1 : 0;      // absorbed bodies wait to be removed (reading R14)
     __syncthreads();
     for (unsigned int p = t; p < np; p += MERGE_THREADS) {
         const int2 ij = pairs[p];
@@ -92,6 +96,10 @@ merge_kernel(int N, unsigned int pair_cap, const int2* __restrict__ pairs, Count
         __syncthreads();
         if (!s_changed) break;
     }
+
+    // bodies absorbed earlier follow the body that took them to its component's root
+    for (int i = t; i < N; i += MERGE_THREADS) { const int l = label[i]; if (l != i) label[i] = label[l]; }
+    __syncthreads();
 
     // 2 ---- accumulators of the roots: zero, then every member adds itself
     for (unsigned int p = t; p < np; p += MERGE_THREADS) {
@@ -177,11 +185,14 @@ void launch_merge(const Handle* h, int* newidx_dev)
     int* flag = h->w.glabel + h->NP;
     unsigned int* out = &h->w.ctr->merge_n;
     cudaMemsetAsync(out, 0, 3 * sizeof(unsigned int), h->stream);
-    merge_init_kernel<<<(h->N + 255) / 256, 256, 0, h->stream>>>(h->N, h->w.radius, h->w.rcrit, label, flag, newidx_dev, out + 1);
+    merge_init_kernel<<<(h->N + 255) / 256, 256, 0, h->stream>>>(h->N, h->w.radius, h->w.rcrit, label, flag, newidx_dev, out + 1, h->w.absorb);
     merge_kernel<<<1, MERGE_THREADS, 0, h->stream>>>(h->N, (unsigned int)h->pair_cap, h->w.pairs, h->w.ctr,
                                                      h->w.m, h->w.x, h->w.v, h->w.radius, label, flag,
                                                      h->w.pk64, h->w.aux, h->w.vtmp, newidx_dev,
                                                      (h->p.n_big >= 0 && h->p.n_big < h->N) ? h->p.n_big : -1, out);
+    // the bodies absorbed inside encounter integrations (reading R14) are gone now
+    cudaMemsetAsync(h->w.absorb, 0xff, (size_t)h->NP * sizeof(int), h->stream);
+    cudaMemsetAsync(&h->w.ctr->enc_merged, 0, sizeof(unsigned int), h->stream);
 }
 
 }  // namespace genga

@@ -299,3 +299,67 @@ def test_an_overflowed_pair_list_is_reported():
     _, status, _ = g.merge()
     assert status & 1                                                  # pairs may have been missed, and the call says so
     g.close()
+
+
+# ---- reading R14: collisions INSIDE the encounter integration (oracle_step_hybrid_collide) ----------------
+def _collide_disc(n=400):
+    """Config-0 shaped disc with: a pair on a collision course that passes THROUGH within the step (closest approach in
+    mid-step, apart again at its end), a chain of three that overlaps pairwise during the step, a close pair that does
+    not touch, and radii far inside the critical radii."""
+    w = W.config(0, n)
+    x = w.x.copy(); v = w.v.copy()
+    x[7] = x[5] + [3.0e-4, 0.0, 0.0]; v[7] = v[5] + [-1.0e-4, 0.0, 0.0]            # closes 6e-4 AU in the 6-day step
+    x[41] = x[40] + [2.0e-4, 1.0e-5, 0.0]; v[41] = v[40] + [-2.5e-5, 0.0, 0.0]      # 40-41 touch after ~4 days ...
+    x[42] = x[40] + [-2.2e-4, 0.0, 1.0e-5]; v[42] = v[40] + [3.0e-5, 0.0, 0.0]      # ... 42 joins from the other side
+    x[90] = x[88] + [1.2e-3, 6.0e-4, 0.0]; v[90] = v[88]                            # inside the zone, never touches
+    R = np.full(w.N, 5.0e-5)
+    return W.Workload("collide", 0, w.m.copy(), x, v, w.dt, 1), R
+
+
+def test_collisions_inside_the_encounter_integration_match_the_oracle():
+    import torch
+    w, R = _collide_disc()
+    p = oracle.Params(G=w.G, M_star=w.M_star, n1=w.n1, n2=w.n2, dt_rcrit=w.dt, pair_rule=w.pair_rule, weight_mode=1)
+    vd = oracle.to_democratic(w.m, w.v, w.M_star)
+    nsub = 64
+    mo, xo, vo, Ro, idxo = oracle.step_hybrid_collide(w.m, w.x, vd, R, p, w.dt, nsub)
+    assert len(mo) == w.N - 3 and idxo[7] == idxo[5] and idxo[40] == idxo[41] == idxo[42] and idxo[90] != idxo[88]
+    # the step-end pass alone (reading R13) misses the pair that passed through
+    xe, ve = oracle.step_hybrid(w.m, w.x, vd, p, w.dt, nsub=nsub)
+    assert oracle.merge(w.m, xe, ve, R)[4][7] != oracle.merge(w.m, xe, ve, R)[4][5]
+    # state: the merger arithmetic itself agrees to 1e-15; what is left (1.1e-12 measured on the bodies of the groups) is
+    # the rounding of 256 force evaluations with refined MUFU reciprocal roots against the oracle's sqrt and divide
+    for prec, tol in ((B.FP64, 5e-12), (B.FP32, 1e-7)):
+        g = B.from_workload(w, weight_mode=1, encounter_mode=1, enc_nsub=nsub, enc_collide=1, mega_nmax=-1)
+        g.set_radii(torch.from_numpy(R).to(g.device))
+        g.step(w.dt, prec)
+        assert g.encounter_stats()[3:] == (0, 0)
+        n_merged, status, newidx = g.merge(prec)
+        assert n_merged == 3 and status == 0 and g.N == len(mo)
+        assert (newidx.cpu().numpy() == idxo).all()                       # the partition, exactly
+        x, v = (t.cpu().numpy() for t in g.get_state())
+        m = g.get_mass().cpu().numpy(); Rg = g.get_radii().cpu().numpy()
+        assert np.abs(m / mo - 1).max() <= 1e-15 and np.abs(Rg / Ro - 1).max() <= 1e-14
+        ex = np.linalg.norm(x - xo, axis=1) / np.linalg.norm(xo, axis=1)
+        ev = np.linalg.norm(v - vo, axis=1) / np.linalg.norm(vo, axis=1)
+        assert ex.max() <= tol and ev.max() <= tol, (prec, ex.max(), ev.max())
+        # the shrunk system goes on: one more hybrid step against the oracle from its own merged state
+        mo2, xo2, vo2, Ro2, idx2 = oracle.step_hybrid_collide(mo, xo, vo, Ro, p, w.dt, nsub)
+        g.step(w.dt, prec)
+        n2, st2, _ = g.merge(prec)
+        x, v = (t.cpu().numpy() for t in g.get_state())
+        assert n2 == len(mo) - len(mo2) and g.N == len(mo2)
+        assert (np.linalg.norm(x - xo2, axis=1) / np.linalg.norm(xo2, axis=1)).max() <= 10 * tol
+        g.close()
+    # without enc_collide the same step + step-end pass leaves the pass-through pair alone (reading R13's limitation)
+    g = B.from_workload(w, weight_mode=1, encounter_mode=1, enc_nsub=nsub, mega_nmax=-1)
+    g.set_radii(torch.from_numpy(R).to(g.device))
+    g.step(w.dt, B.FP64)
+    n_merged, status, newidx = g.merge(B.FP64)
+    idx = newidx.cpu().numpy()
+    g.close()
+    assert idx[7] != idx[5] and n_merged < 3
+    # parameter checks: collisions need the RK4 substeps of an encounter-mode handle
+    for bad in (dict(encounter_mode=1, enc_collide=1), dict(enc_collide=1, enc_nsub=8), dict(encounter_mode=1, enc_nsub=8, enc_collide=2)):
+        with pytest.raises(Exception):
+            B.from_workload(w, weight_mode=1, mega_nmax=-1, **bad).close()
