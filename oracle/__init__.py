@@ -76,6 +76,11 @@ def lib() -> ctypes.CDLL:
         L.oracle_step_hybrid_bs.restype = ctypes.c_int
         L.oracle_step_hybrid_bs.argtypes = [ctypes.c_int, _dp, _dp, _dp, _pp, ctypes.c_double, ctypes.c_double,
                                             ctypes.POINTER(ctypes.c_longlong)]
+        L.oracle_level_weight.restype = ctypes.c_double
+        L.oracle_level_weight.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_double]
+        L.oracle_step_multilevel.restype = ctypes.c_int
+        L.oracle_step_multilevel.argtypes = [ctypes.c_int, _dp, _dp, _dp, _pp, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+                                             ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_longlong)]
         L.oracle_weight.restype = ctypes.c_double
         L.oracle_weight.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int]
         L.oracle_pair_rcrit.restype = ctypes.c_double
@@ -277,6 +282,22 @@ def step_hybrid_bs(m, x, v, p: Params, dt: float, tol: float = 1.0e-13, stats: b
     rc = lib().oracle_step_hybrid_bs(len(m), _p(m), _p(x), _p(v), ctypes.byref(c), float(dt), float(tol), st)
     if rc != 0:
         raise ValueError("oracle_step_hybrid_bs: needs weight_mode = 1 and tol > 0, or the step size collapsed")
+    return (x, v, tuple(int(q) for q in st)) if stats else (x, v)
+
+
+def level_weight(r: float, rcrit: float, l: int, L: int, F: float) -> float:
+    """Reading R16: shell weight of level l (l < L: W_l - W_{l-1}; l == L: the Bulirsch-Stoer remainder 1 - W_{L-1})."""
+    return float(lib().oracle_level_weight(float(r), float(rcrit), int(l), int(L), float(F)))
+
+
+def step_multilevel(m, x, v, p: Params, dt: float, L: int, S: int, F: float, tol: float = 1.0e-13, stats: bool = False):
+    """NEXT-3 (reading R16): the hybrid step with L changeover levels, S sub-steps per level and radius ratio F."""
+    m = _a(m); x = _a(x).copy(); v = _a(v).copy()
+    c = p.c()
+    st = (ctypes.c_longlong * 3)()
+    rc = lib().oracle_step_multilevel(len(m), _p(m), _p(x), _p(v), ctypes.byref(c), float(dt), int(L), int(S), float(F), float(tol), st)
+    if rc != 0:
+        raise ValueError("oracle_step_multilevel: needs weight_mode = 1, tol > 0, L >= 1, S >= 1, F > 1 (or the step size collapsed)")
     return (x, v, tuple(int(q) for q in st)) if stats else (x, v)
 
 

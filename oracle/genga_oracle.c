@@ -463,8 +463,17 @@ int oracle_run(int N, const double* m, double* x, double* v,
  * equal substeps: plain and slow, no encounter groups, no pair lists), with the pair weight
  * Wc = 1 - W = (1 - K) + r K' and r_crit,ij held at the values of the opening force evaluation.  With no pair
  * inside a zone Wc = 0 everywhere and A is the Kepler drift, so the step reduces to oracle_step.           */
+static void rhs_A_s(int N, const double* m, const oracle_params* p, const double* rc, const double* sa,
+                    const double* vk, const double* x, const double* v, double* dx, double* dv, double rscale);
 static void rhs_A(int N, const double* m, const oracle_params* p, const double* rc, const double* sa,
                   const double* vk, const double* x, const double* v, double* dx, double* dv)
+{
+    rhs_A_s(N, m, p, rc, sa, vk, x, v, dx, dv, 1.0);
+}
+/* rscale: the critical radii are multiplied by it (1 for the two-level step; 1 / F^(L-1) for the innermost level of the
+ * multi-level step, reading R16) */
+static void rhs_A_s(int N, const double* m, const oracle_params* p, const double* rc, const double* sa,
+                    const double* vk, const double* x, const double* v, double* dx, double* dv, double rscale)
 {
     const double mu = p->G * p->M_star;
 #pragma omp parallel for schedule(static)
@@ -479,7 +488,7 @@ static void rhs_A(int N, const double* m, const oracle_params* p, const double* 
             double q2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
             double q  = sqrt(q2);
             if (!(q > 0.0)) continue;
-            double rcij = oracle_pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j]);
+            double rcij = rscale * oracle_pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j]);
             double Wc = 1.0 - oracle_weight(q, rcij, 1);
             if (Wc == 0.0) continue;
             double s = p->G * m[j] * Wc / (q2 * q);
@@ -527,8 +536,15 @@ void oracle_encounter_drift(int N, const double* m, double* x, double* v, const 
  * All N bodies form ONE system (no groups, no lists): the oracle of the A-flow is its converged solution.
  * stats (may be NULL): [0] macro steps accepted, [1] rejected, [2] right-hand sides.  Returns 0, or -1 if H fell
  * below |dt| 2^-40 without convergence (the state is then the last accepted one).                                 */
+static int drift_bs(int N, const double* m, double* x, double* v, const oracle_params* p, const double* rc,
+                    const double* sa, const double* vk, double dt, double tol, long long* stats, double rscale);
 int oracle_encounter_drift_bs(int N, const double* m, double* x, double* v, const oracle_params* p,
                               const double* rc, const double* sa, const double* vk, double dt, double tol, long long* stats)
+{
+    return drift_bs(N, m, x, v, p, rc, sa, vk, dt, tol, stats, 1.0);
+}
+static int drift_bs(int N, const double* m, double* x, double* v, const oracle_params* p, const double* rc,
+                    const double* sa, const double* vk, double dt, double tol, long long* stats, double rscale)
 {
     enum { KMAX = 8 };
     size_t n3 = 3 * (size_t)(N > 0 ? N : 1);
@@ -544,7 +560,7 @@ int oracle_encounter_drift_bs(int N, const double* m, double* x, double* v, cons
     const double T = fabs(dt);
     while (fabs(t) < T * (1.0 - 1.0e-14) && T > 0.0) {
         if (fabs(t + H) > T) H = dt - t;
-        rhs_A(N, m, p, rc, sa, vk, x, v, f0x, f0v); ++nf;
+        rhs_A_s(N, m, p, rc, sa, vk, x, v, f0x, f0v, rscale); ++nf;
         int done = -1;
         for (int k = 0; k < KMAX && done < 0; ++k) {
             const int nk = 2 * (k + 1);
@@ -552,13 +568,13 @@ int oracle_encounter_drift_bs(int N, const double* m, double* x, double* v, cons
             const int cur = k & 1, prev = cur ^ 1;
             for (size_t q = 0; q < 3 * (size_t)N; ++q) { z0x[q] = x[q]; z0v[q] = v[q]; z1x[q] = x[q] + h * f0x[q]; z1v[q] = v[q] + h * f0v[q]; }
             for (int s = 1; s < nk; ++s) {
-                rhs_A(N, m, p, rc, sa, vk, z1x, z1v, fx, fv); ++nf;
+                rhs_A_s(N, m, p, rc, sa, vk, z1x, z1v, fx, fv, rscale); ++nf;
                 for (size_t q = 0; q < 3 * (size_t)N; ++q) {
                     double nx = z0x[q] + 2.0 * h * fx[q], nv = z0v[q] + 2.0 * h * fv[q];
                     z0x[q] = z1x[q]; z0v[q] = z1v[q]; z1x[q] = nx; z1v[q] = nv;
                 }
             }
-            rhs_A(N, m, p, rc, sa, vk, z1x, z1v, fx, fv); ++nf;
+            rhs_A_s(N, m, p, rc, sa, vk, z1x, z1v, fx, fv, rscale); ++nf;
             for (size_t q = 0; q < 3 * (size_t)N; ++q) {
                 Tx[cur][0][q] = 0.5 * (z1x[q] + z0x[q] + h * fx[q]);
                 Tv[cur][0][q] = 0.5 * (z1v[q] + z0v[q] + h * fv[q]);
@@ -597,7 +613,7 @@ int oracle_encounter_drift_bs(int N, const double* m, double* x, double* v, cons
         t += H; ++acc;
         H = (done <= 3) ? 2.0 * H : ((done <= 5) ? H : 0.5 * H);
     }
-    if (stats) { stats[0] = acc; stats[1] = rej; stats[2] = nf; }
+    if (stats) { stats[0] += acc; stats[1] += rej; stats[2] += nf; }
     free(buf);
     return rcode;
 }
@@ -613,7 +629,92 @@ int oracle_step_hybrid_bs(int N, const double* m, double* x, double* v, const or
     oracle_rcrit(N, m, x, v, p, rc, sa, vk);              /* the radii of the opening force evaluation */
     oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
     oracle_sunkick(N, m, x, v, p, 0.5 * dt);
+    if (stats) { stats[0] = 0; stats[1] = 0; stats[2] = 0; }
     int r = oracle_encounter_drift_bs(N, m, x, v, p, rc, sa, vk, dt, tol, stats);
+    oracle_sunkick(N, m, x, v, p, 0.5 * dt);
+    oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
+    free(rc); free(sa); free(vk);
+    return r;
+}
+
+/* ---- NEXT-3, second half: multi-level changeover, reading R16 ---------------------------
+ * "a hierarchical method that uses multiple changeover functions ... instead of switching directly to
+ * the Bulirsch-Stoer method, another symplectic integration step with a reduced time step can be applied in between";
+ * "the number of levels and the number of sub-steps".  Grimm et al. 2022 is not in the container; the
+ * reading (recursive shells as in Duncan et al. 1998, whom the paper cites, with Chambers' K on every level):
+ *   L levels of changeover, S sub-steps per level, radius ratio F:  level l uses r_crit,ij / F^l and the step dt / S^l.
+ *   W_l(r) = weight(r, r_crit,ij / F^l) (K - r K', reading R10), W_{-1} = 0.  The pair potential V = -G m_i m_j / r is
+ *   cut into shells  V = W_0 V + sum_{l=1}^{L-1} (W_l - W_{l-1}) V + (1 - W_{L-1}) V  (as forces; the weights add to 1):
+ *   shell 0 is the level-0 kick (step dt), shell l a kick with the step dt / S^l, the remainder stays with the Kepler
+ *   terms in the Bulirsch-Stoer integration (level L) over dt / S^(L-1).  Recursively, flow_l(tau) of
+ *   H_Kep + (1 - W_{l-1}) V:   flow_L(tau) = Bulirsch-Stoer;   flow_l(tau) = [ kick_l(h/2) flow_{l+1}(h) kick_l(h/2) ]^S,
+ *   h = tau / S;   step = B(dt/2) C(dt/2) flow_1(dt) C(dt/2) B(dt/2).
+ * L = 1 is the two-level hybrid step of R11 / R15.  Critical radii: those of the opening force evaluation.         */
+double oracle_level_weight(double r, double rcrit, int l, int L, double F)
+{
+    double lo = 0.0, hi = 1.0, sc = 1.0;
+    for (int k = 0; k < l - 1; ++k) sc /= F;
+    if (l >= 1) lo = oracle_weight(r, rcrit * sc, 1);            /* W_{l-1} */
+    if (l < L)  hi = oracle_weight(r, rcrit * (l >= 1 ? sc / F : 1.0), 1);   /* W_l; l == L: the remainder 1 - W_{L-1} */
+    return hi - lo;
+}
+
+/* v_i += tau * sum_j G m_j w_l(r_ij) (x_j - x_i) / r_ij^3 with the shell weight of level l (1 <= l < L) */
+static void shell_kick(int N, const double* m, const double* x, double* v, const oracle_params* p, const double* rc,
+                       const double* sa, const double* vk, int l, int L, double F, double tau)
+{
+    double* a = (double*)calloc(3 * (size_t)(N > 0 ? N : 1), sizeof(double));
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        nsum s3[3] = {{0, 0}, {0, 0}, {0, 0}};
+        for (int j = 0; j < N; ++j) {
+            if (j == i || !interacts(p, i, j)) continue;
+            double d[3] = {x[3 * j] - x[3 * i], x[3 * j + 1] - x[3 * i + 1], x[3 * j + 2] - x[3 * i + 2]};
+            double q2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            double q  = sqrt(q2);
+            if (!(q > 0.0)) continue;
+            double rcij = oracle_pair_rcrit(p, m[i], m[j], rc[i], rc[j], sa[i], sa[j], vk[i], vk[j]);
+            double wl = oracle_level_weight(q, rcij, l, L, F);
+            if (wl == 0.0) continue;
+            double s = p->G * m[j] * wl / (q2 * q);
+            for (int k = 0; k < 3; ++k) nsum_add(&s3[k], s * d[k]);
+        }
+        for (int k = 0; k < 3; ++k) a[3 * i + k] = nsum_value(&s3[k]);
+    }
+    for (size_t q = 0; q < 3 * (size_t)N; ++q) v[q] += tau * a[q];
+    free(a);
+}
+
+static int level_flow(int N, const double* m, double* x, double* v, const oracle_params* p, const double* rc,
+                      const double* sa, const double* vk, int l, int L, int S, double F, double tau, double tol, long long* stats)
+{
+    if (l >= L) {
+        double sc = 1.0;
+        for (int k = 0; k < L - 1; ++k) sc /= F;
+        return drift_bs(N, m, x, v, p, rc, sa, vk, tau, tol, stats, sc);
+    }
+    int rcode = 0;
+    const double h = tau / S;
+    for (int s = 0; s < S; ++s) {
+        shell_kick(N, m, x, v, p, rc, sa, vk, l, L, F, 0.5 * h);
+        if (level_flow(N, m, x, v, p, rc, sa, vk, l + 1, L, S, F, h, tol, stats) != 0) rcode = -1;
+        shell_kick(N, m, x, v, p, rc, sa, vk, l, L, F, 0.5 * h);
+    }
+    return rcode;
+}
+
+int oracle_step_multilevel(int N, const double* m, double* x, double* v, const oracle_params* p, double dt,
+                           int L, int S, double F, double tol, long long* stats)
+{
+    if (p->weight_mode != 1 || !(tol > 0.0) || L < 1 || S < 1 || !(F > 1.0)) return -1;
+    double* rc = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* sa = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    double* vk = (double*)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+    oracle_rcrit(N, m, x, v, p, rc, sa, vk);              /* the radii of the opening force evaluation */
+    oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
+    oracle_sunkick(N, m, x, v, p, 0.5 * dt);
+    if (stats) { stats[0] = 0; stats[1] = 0; stats[2] = 0; }
+    int r = level_flow(N, m, x, v, p, rc, sa, vk, 1, L, S, F, dt, tol, stats);
     oracle_sunkick(N, m, x, v, p, 0.5 * dt);
     oracle_kick(N, m, x, v, p, 0.5 * dt, NULL);
     free(rc); free(sa); free(vk);

@@ -34,6 +34,12 @@
  *                          encounter, agreement with the converged RK4 substeps of oracle_step_hybrid, error falling
  *                          with tol, time reversal (reading R15: WHICH extrapolation scheme and step control GENGA's
  *                          Bulirsch-Stoer level uses is not printed; the A-flow itself is unique)
+ *   oracle_step_multilevel pinned: the shell weights add to 1 and are each >= 0, hand value of a shell; L = 1 is
+ *                          oracle_step_hybrid_bs bit for bit; without encounters it is oracle_step; S = 1 with any L is
+ *                          the two-level step to the integration tolerance; second-order convergence to the DOP853
+ *                          N-body solution through an encounter; energy through the encounter against the level count
+ *                          (reading R16: the level structure of Grimm et al. 2022 is NOT in PAPER.md -- parity unpinned
+ *                          by the paper for that choice)
  *   TP2 mode (n_big >= 0)  pinned: hand 3-body values, full-minus-subset identity against the
  *                          pinned all-pairs path, sum m a = 0, bounded dt^2 energy error
  *   oracle_merge(_tp2)     pinned: inelastic-collision identities (dT = mu u^2/2, dL = mu x_rel x v_rel),
@@ -138,6 +144,11 @@ int oracle_encounter_drift_bs(int N, const double* m, double* x, double* v, cons
                               const double* rc, const double* sa, const double* vk, double dt, double tol, long long* stats);
 int oracle_step_hybrid_bs(int N, const double* m, double* x, double* v, const oracle_params* p, double dt, double tol,
                           long long* stats);
+/* NEXT-3, reading R16: L levels of changeover with radius ratio F and S sub-steps per level; shell
+ * weight of level l (0 <= l < L: W_l - W_{l-1}; l == L: the remainder 1 - W_{L-1} that Bulirsch-Stoer integrates) */
+double oracle_level_weight(double r, double rcrit, int l, int L, double F);
+int oracle_step_multilevel(int N, const double* m, double* x, double* v, const oracle_params* p, double dt,
+                           int L, int S, double F, double tol, long long* stats);
 
 /* O11.  E = sum m v^2/2 + |sum m v|^2/(2 M_star) - sum G M_star m/r
  *                         - sum_{i<j} G m_i m_j / r_ij ;  L = sum m x cross v. */
