@@ -139,6 +139,15 @@ typedef struct {
                                  index), which is how bodies that pass through each other WITHIN a step are caught.  The
                                  absorbed bodies stay in the arrays as massless bodies of radius -1e300 until the next
                                  genga_merge closes the arrays up (its newidx and n_merged account for them).            */
+    int    enc_levels;        /* NEXT-3, reading R16 ("levels" and "sub-steps"): number of changeover levels of
+                                 the encounter integration; <= 1 (default): the two-level step (level 0 + Bulirsch-Stoer).
+                                 L > 1 (<= 4; needs encounter_mode = 1 and enc_nsub <= 0): level l = 1 .. L - 1 is a symplectic
+                                 kick-flow-kick with the step dt / enc_substeps^l on the shell
+                                 (W(r; r_crit / F^l) - W(r; r_crit / F^(l-1))) of the pair potential, F = enc_level_ratio,
+                                 and Bulirsch-Stoer integrates the Kepler terms plus the innermost remainder
+                                 1 - W(r; r_crit / F^(L-1)) over dt / enc_substeps^(L-1).                                 */
+    int    enc_substeps;      /* sub-steps per level; <= 0: default 3                                                     */
+    double enc_level_ratio;   /* radius ratio F > 1 between consecutive levels; 0: default enc_substeps^(2/3) (Kepler scaling) */
 } genga_params;
 
 /* Fill *p with the defaults: G = k^2 (k = 0.01720209895), M_star = 1, n1 = 3, n2 = 0,

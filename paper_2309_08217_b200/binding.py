@@ -42,7 +42,7 @@ class GengaParams(ctypes.Structure):
         ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
         ("pair_capacity", ctypes.c_int), ("cand_capacity", ctypes.c_int), ("resort_every", ctypes.c_int),
         ("chunk", ctypes.c_int), ("mega_nmax", ctypes.c_int), ("n_big", ctypes.c_int), ("weight_mode", ctypes.c_int), ("no_fused_step", ctypes.c_int),
-        ("encounter_mode", ctypes.c_int), ("enc_nsub", ctypes.c_int), ("enc_list_scale", ctypes.c_double), ("enc_list_vfactor", ctypes.c_double), ("enc_tol", ctypes.c_double), ("enc_collide", ctypes.c_int),
+        ("encounter_mode", ctypes.c_int), ("enc_nsub", ctypes.c_int), ("enc_list_scale", ctypes.c_double), ("enc_list_vfactor", ctypes.c_double), ("enc_tol", ctypes.c_double), ("enc_collide", ctypes.c_int), ("enc_levels", ctypes.c_int), ("enc_substeps", ctypes.c_int), ("enc_level_ratio", ctypes.c_double),
     ]
 
 
@@ -164,7 +164,7 @@ class Genga:
     def __init__(self, m, x, v, *, G=None, M_star=1.0, n1=3.0, n2=0.0, dt_rcrit=0.0,
                  pair_rule=PAIR_MUTUAL_HILL, v_is_heliocentric=True, lambda_near=0.0, near_floor=-1.0,
                  pair_capacity=0, cand_capacity=0, resort_every=0, chunk=0, mega_nmax=0, n_big=-1, weight_mode=0, no_fused_step=False,
-                 encounter_mode=0, enc_nsub=0, enc_list_scale=0.0, enc_list_vfactor=0.0, enc_tol=0.0, enc_collide=0, stream=None, device=None):
+                 encounter_mode=0, enc_nsub=0, enc_list_scale=0.0, enc_list_vfactor=0.0, enc_tol=0.0, enc_collide=0, enc_levels=0, enc_substeps=0, enc_level_ratio=0.0, stream=None, device=None):
         import torch
         self._torch = torch
         self._L = load()
@@ -181,7 +181,7 @@ class Genga:
         p.pair_capacity, p.cand_capacity = int(pair_capacity), int(cand_capacity)
         p.resort_every = int(resort_every)
         p.no_fused_step = int(bool(no_fused_step))
-        p.encounter_mode = int(encounter_mode); p.enc_nsub = int(enc_nsub); p.enc_list_scale = float(enc_list_scale); p.enc_list_vfactor = float(enc_list_vfactor); p.enc_tol = float(enc_tol); p.enc_collide = int(enc_collide)
+        p.encounter_mode = int(encounter_mode); p.enc_nsub = int(enc_nsub); p.enc_list_scale = float(enc_list_scale); p.enc_list_vfactor = float(enc_list_vfactor); p.enc_tol = float(enc_tol); p.enc_collide = int(enc_collide); p.enc_levels = int(enc_levels); p.enc_substeps = int(enc_substeps); p.enc_level_ratio = float(enc_level_ratio)
         p.n_big = int(n_big)
         p.chunk = int(chunk)
         p.mega_nmax = int(mega_nmax)

@@ -193,6 +193,7 @@ static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_d
     a.enc.G = h->p.G; a.enc.M_star = h->p.M_star; a.enc.n1 = h->p.n1; a.enc.n2dt = h->p.n2 * h->p.dt_rcrit;
     a.enc.tol = h->p.enc_tol;
     a.enc.collide = h->p.enc_collide;
+    a.enc.levels = h->p.enc_levels; a.enc.levels_sub = h->p.enc_substeps; a.enc.level_ratio = h->p.enc_level_ratio;
     a.enc.maxgroups = (int)std::min((size_t)h->pair_cap, (size_t)h->NP / 2);
     cudaError_t e;
     if (enc) {                                         // groups of the pair list the last force evaluation left
@@ -353,7 +354,7 @@ void genga_default_params(genga_params* p)
     p->chunk = 0;
     p->mega_nmax = 0;
     p->weight_mode = 0;
-    p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0; p->enc_list_vfactor = 0.0; p->enc_tol = 0.0; p->enc_collide = 0;
+    p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0; p->enc_list_vfactor = 0.0; p->enc_tol = 0.0; p->enc_collide = 0; p->enc_levels = 0; p->enc_substeps = 0; p->enc_level_ratio = 0.0;
 }
 
 size_t genga_workspace_bytes(int N, const genga_params* p)
@@ -373,6 +374,8 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     if (p->encounter_mode != 0 && p->encounter_mode != 1) return GENGA_EINVAL;
     if (p->encounter_mode == 1 && (p->weight_mode != 1 || (p->n_big >= 0 && p->n_big < N) || p->no_fused_step)) return GENGA_EINVAL;
     if (p->enc_collide != 0 && (p->enc_collide != 1 || p->encounter_mode != 1 || p->enc_nsub <= 0)) return GENGA_EINVAL;
+    if (p->enc_levels > 1 && (p->encounter_mode != 1 || p->enc_nsub > 0 || p->enc_levels > 4 || p->enc_substeps < 0 ||
+                              (p->enc_level_ratio != 0.0 && !(p->enc_level_ratio > 1.0)))) return GENGA_EINVAL;
     *out = nullptr;
     int pc, cc;
     resolve_caps(N, p, &pc, &cc);
@@ -415,6 +418,9 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
             h->p.enc_list_vfactor = p->enc_list_vfactor == 0.0 ? 1.25 : p->enc_list_vfactor;
             h->enc_dt = std::fabs(p->dt_rcrit);
             h->p.enc_tol = p->enc_tol > 0.0 ? p->enc_tol : 1.0e-12;
+            h->p.enc_levels = p->enc_levels > 1 ? p->enc_levels : 1;
+            h->p.enc_substeps = p->enc_substeps > 0 ? p->enc_substeps : 3;
+            h->p.enc_level_ratio = p->enc_level_ratio > 1.0 ? p->enc_level_ratio : std::cbrt((double)h->p.enc_substeps * h->p.enc_substeps);
             if (h->p.enc_list_scale < 1.0 || h->p.enc_list_scale > 8.0) { delete h; return GENGA_EINVAL; }
         }
         h->mega_blocks[0] = h->mega_blocks[1] = -1;

@@ -20,6 +20,8 @@
 //     the members; a step that does not converge in 8 rows, or whose corrections stop falling (a pair crossing the
 //     edge of its zone, where K is only C^1), is cut to a quarter; a step that converged in few rows is followed by
 //     a longer one.  Status bit 8: the step size collapsed.
+//   * with params.enc_levels > 1 (reading R16): symplectic sub-levels with reduced steps between level 0 and the
+//     Bulirsch-Stoer integration, which then only sees the innermost remainder of the pair potential.
 //   * classical RK4 with enc_nsub equal substeps (the scheme of the first oracle, oracle_step_hybrid); with
 //     params.enc_collide the members are tested for collisions after every substep and merged on the spot
 //     (reading R14, oracle_step_hybrid_collide).
@@ -194,12 +196,27 @@ __device__ __forceinline__ bool collision_pass(const Team& T, const EncParams& P
     return true;
 }
 
+// W(q) = K - q K' for the zone of inverse width i09 = 1 / (0.9 r_crit) (readings G1, R10), branch-free: 0 below
+// 0.1 r_crit, 1 from r_crit on.
+__device__ __forceinline__ double zone_weight(double q, double i09)
+{
+    const double yy = fmin(fmax(fma(q, i09, -1.0 / 9.0), 0.0), 1.0);     // (q - 0.1 rc) / (0.9 rc)
+    const double D  = fma(2.0 * yy, yy - 1.0, 1.0);                      // 2y^2 - 2y + 1, in [1/2, 1]
+    const double r0 = rcp_seed(D), f = fma(-D, r0, 1.0);
+    const double iD = fma(r0 * f, 1.0 + f, r0);
+    const double K  = yy * yy * iD;
+    const double Kp = 2.0 * yy * (1.0 - yy) * iD * iD * i09;             // dK/dr (0 at both ends)
+    return K - q * Kp;
+}
+
 // dv/dt of this thread's member at the stage position (x, y, z): the member publishes its position in buffer buf,
-// the team synchronises once, every member sums the Kepler term and the complement terms of the other members.
-// Branch-free per pair: a term that does not apply gets weight 0.  Every thread of the team must call it.
-template <class Team>
+// the team synchronises once, every member sums over the other members.  KEPLER: with the star's term -mu x / r^3.
+// Pair weight: W(q; r_crit / fhi) - W(q; r_crit / flo), where fhi <= 0 stands for the constant 1: the complement of
+// the two-level step is (flo, fhi) = (1, 0); shell l of the multi-level step (reading R16) is (F^(l-1), F^l), its
+// innermost remainder (F^(L-1), 0).  Branch-free per pair.  Every thread of the team must call it.
+template <bool KEPLER, class Team>
 __device__ __forceinline__ void accel(const Team& T, const EncParams& P, int& buf, double x, double y, double z,
-                                      double& a0, double& a1, double& a2)
+                                      double& a0, double& a1, double& a2, double flo = 1.0, double fhi = 0.0)
 {
     double* X = T.px(buf); double* Y = T.py(buf); double* Z = T.pz(buf);
     if (T.k >= 0) { X[T.k] = x; Y[T.k] = y; Z[T.k] = z; }
@@ -207,7 +224,7 @@ __device__ __forceinline__ void accel(const Team& T, const EncParams& P, int& bu
     buf ^= 1;                                              // the next evaluation writes the other buffer
     a0 = 0.0; a1 = 0.0; a2 = 0.0;
     if (T.k < 0) return;
-    {
+    if (KEPLER) {
         const double mu = P.G * P.M_star;
         const double r2 = fma(z, z, fma(y, y, x * x));
         const double y0 = rsq_seed(r2), t = y0 * y0, e = fma(-r2, t, 1.0), g = y0 * t;
@@ -227,19 +244,13 @@ __device__ __forceinline__ void accel(const Team& T, const EncParams& P, int& bu
         const double y0 = rsq_seed(qs), t = y0 * y0, e = fma(-qs, t, 1.0), g = y0 * t;
         const double q0 = qs * y0;
         const double q  = fma(q0 * e, fma(0.375, e, 0.5), q0);              // |d|
-        const double yy = fmin(fmax(fma(q, i09, -1.0 / 9.0), 0.0), 1.0);     // (q - 0.1 rc) / (0.9 rc); <= 0: Wc = 1, >= 1: Wc = 0
-        const double D  = fma(2.0 * yy, yy - 1.0, 1.0);                      // 2y^2 - 2y + 1, in [1/2, 1]
-        const double r0 = rcp_seed(D), f = fma(-D, r0, 1.0);
-        const double iD = fma(r0 * f, 1.0 + f, r0);
-        const double K  = yy * yy * iD;
-        const double Kp = 2.0 * yy * (1.0 - yy) * iD * iD * i09;             // dK/dr (0 at both ends)
-        const double Wc = on ? 1.0 - (K - q * Kp) : 0.0;
+        const double whi = (fhi > 0.0) ? zone_weight(q, i09 * fhi) : 1.0;
+        const double Wc = on ? whi - zone_weight(q, i09 * flo) : 0.0;
         const double s  = T.gm(l) * Wc * fma(g * e, fma(1.875, e, 1.5), g);  // G m_l Wc / |d|^3
         a0 = fma(s, d0, a0); a1 = fma(s, d1, a1); a2 = fma(s, d2, a2);
     }
 }
 
-// A(dt) by classical RK4 with nsub equal substeps (oracle_step_hybrid's scheme, restricted to the group).
 // P.collide: after every substep the collision pass of reading R14 (m, R: this member's mass and radius, updated).
 template <class Team>
 __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
@@ -249,19 +260,19 @@ __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P,
     int buf = 0;
     for (int s = 0; s < P.nsub; ++s) {
         double k0, k1, k2, sx[3], sv[3], t[3], u[3];
-        accel(T, P, buf, y[0], y[1], y[2], k0, k1, k2);
+        accel<true>(T, P, buf, y[0], y[1], y[2], k0, k1, k2);
         sx[0] = y[3]; sx[1] = y[4]; sx[2] = y[5]; sv[0] = k0; sv[1] = k1; sv[2] = k2;
         t[0] = fma(hh, y[3], y[0]); t[1] = fma(hh, y[4], y[1]); t[2] = fma(hh, y[5], y[2]);
         u[0] = fma(hh, k0, y[3]); u[1] = fma(hh, k1, y[4]); u[2] = fma(hh, k2, y[5]);
-        accel(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
+        accel<true>(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
         sx[0] += 2.0 * u[0]; sx[1] += 2.0 * u[1]; sx[2] += 2.0 * u[2]; sv[0] += 2.0 * k0; sv[1] += 2.0 * k1; sv[2] += 2.0 * k2;
         t[0] = fma(hh, u[0], y[0]); t[1] = fma(hh, u[1], y[1]); t[2] = fma(hh, u[2], y[2]);
         u[0] = fma(hh, k0, y[3]); u[1] = fma(hh, k1, y[4]); u[2] = fma(hh, k2, y[5]);
-        accel(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
+        accel<true>(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
         sx[0] += 2.0 * u[0]; sx[1] += 2.0 * u[1]; sx[2] += 2.0 * u[2]; sv[0] += 2.0 * k0; sv[1] += 2.0 * k1; sv[2] += 2.0 * k2;
         t[0] = fma(h, u[0], y[0]); t[1] = fma(h, u[1], y[1]); t[2] = fma(h, u[2], y[2]);
         u[0] = fma(h, k0, y[3]); u[1] = fma(h, k1, y[4]); u[2] = fma(h, k2, y[5]);
-        accel(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
+        accel<true>(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
         y[0] = fma(h6, sx[0] + u[0], y[0]); y[1] = fma(h6, sx[1] + u[1], y[1]); y[2] = fma(h6, sx[2] + u[2], y[2]);
         y[3] = fma(h6, sv[0] + k0, y[3]); y[4] = fma(h6, sv[1] + k1, y[4]); y[5] = fma(h6, sv[2] + k2, y[5]);
         if (P.collide) collision_pass(T, P, buf, y, m, R, body, absorb, ctr);
@@ -273,7 +284,8 @@ __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P,
 // the difference form of polynomial extrapolation (one column of differences per row), which yields the extrapolated
 // value and the last correction, i.e. the error estimate T_kk - T_k,k-1, without storing two rows.
 template <class Team>
-__device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr)
+__device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
+                                             double flo = 1.0)
 {
     const double Tabs = fabs(dt);
     double t = 0.0, H = dt;
@@ -283,7 +295,7 @@ __device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, 
     while (fabs(t) < Tabs * (1.0 - 1.0e-14)) {
         if (fabs(t + H) > Tabs) H = dt - t;
         double f0[3];
-        accel(T, P, buf, y[0], y[1], y[2], f0[0], f0[1], f0[2]);
+        accel<true>(T, P, buf, y[0], y[1], y[2], f0[0], f0[1], f0[2], flo);
         ++nrhs;
         double d[KMAX][6], hsq[KMAX], yz[6], dy[6];
         double eprev = 1.0e300;
@@ -295,14 +307,14 @@ __device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, 
 #pragma unroll
             for (int c = 0; c < 3; ++c) { z0[c] = y[c]; z0[3 + c] = y[3 + c]; z1[c] = fma(h, y[3 + c], y[c]); z1[3 + c] = fma(h, f0[c], y[3 + c]); }
             for (int s = 1; s < nk; ++s) {
-                accel(T, P, buf, z1[0], z1[1], z1[2], f[0], f[1], f[2]);
+                accel<true>(T, P, buf, z1[0], z1[1], z1[2], f[0], f[1], f[2], flo);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     const double nx = fma(h2, z1[3 + c], z0[c]), nv = fma(h2, f[c], z0[3 + c]);
                     z0[c] = z1[c]; z0[3 + c] = z1[3 + c]; z1[c] = nx; z1[3 + c] = nv;
                 }
             }
-            accel(T, P, buf, z1[0], z1[1], z1[2], f[0], f[1], f[2]);
+            accel<true>(T, P, buf, z1[0], z1[1], z1[2], f[0], f[1], f[2], flo);
             nrhs += (unsigned int)nk;
             double est[6];
 #pragma unroll
@@ -367,13 +379,47 @@ __device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, 
     }
 }
 
+// Reading R16: flow_l(tau) of H_Kep + (1 - W_{l-1}) V for the group.  l == levels: Bulirsch-Stoer
+// with the innermost remainder; otherwise levels_sub times [ kick_l(h/2) flow_{l+1}(h) kick_l(h/2) ], h = tau / sub,
+// kick_l: v += (h/2) a with the shell weight W_l - W_{l-1} (radius ratio F per level).  fl = F^(l-1).
+constexpr int LMAX = 4;            // most changeover levels (no recursion on the device: the levels are unrolled)
+
+template <class Team>
+__device__ __noinline__ void bs_call(const Team& T, const EncParams& P, double tau, double (&y)[6], Counters* ctr, double fl)
+{
+    integrate_bs(T, P, tau, y, ctr, fl);
+}
+
+template <int LVL, class Team>
+__device__ __forceinline__ void level_flow(const Team& T, const EncParams& P, double fl, double tau, double (&y)[6], Counters* ctr)
+{
+    if constexpr (LVL >= LMAX) {
+        bs_call(T, P, tau, y, ctr, fl);
+    } else {
+        if (LVL >= P.levels) { bs_call(T, P, tau, y, ctr, fl); return; }
+        const double h = tau / P.levels_sub, hh = 0.5 * h, fh = fl * P.level_ratio;
+        int buf = 0;
+        for (int s = 0; s < P.levels_sub; ++s) {
+            double a0, a1, a2;
+            accel<false>(T, P, buf, y[0], y[1], y[2], a0, a1, a2, fl, fh);
+            y[3] = fma(hh, a0, y[3]); y[4] = fma(hh, a1, y[4]); y[5] = fma(hh, a2, y[5]);
+            T.sync();                                       // the slab buffers are reused by the inner level
+            level_flow<LVL + 1>(T, P, fh, h, y, ctr);
+            T.sync();
+            accel<false>(T, P, buf, y[0], y[1], y[2], a0, a1, a2, fl, fh);
+            y[3] = fma(hh, a0, y[3]); y[4] = fma(hh, a1, y[4]); y[5] = fma(hh, a2, y[5]);
+        }
+    }
+}
+
 template <class Team>
 __device__ __forceinline__ void integrate(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
                                           double& m, double& R, int body, int* __restrict__ absorb)
 {
     if (dt == 0.0) return;
-    if (P.nsub > 0) integrate_rk4(T, P, dt, y, ctr, m, R, body, absorb);
-    else            integrate_bs(T, P, dt, y, ctr);
+    if (P.nsub > 0)        integrate_rk4(T, P, dt, y, ctr, m, R, body, absorb);
+    else if (P.levels > 1) level_flow<1>(T, P, 1.0, dt, y, ctr);
+    else                   integrate_bs(T, P, dt, y, ctr);
 }
 
 // Groups in Workspace::ginfo (written by group_kernel): ginfo[2 g] = offset of the member list, ginfo[2 g + 1] = member

@@ -157,6 +157,8 @@ struct EncArgs {                  // encounter mode (encounter.cuh; NEXT-1, read
     unsigned int pair_cap;
     double G, M_star, n1, n2dt;
     double tol;                    // nsub <= 0: relative tolerance of the Bulirsch-Stoer integration (encounter.cuh)
+    int levels, levels_sub;        // reading R16: changeover levels (1: the two-level step) and sub-steps per level
+    double level_ratio;            // radius ratio between consecutive levels
     int collide;                   // RK4 only: collision pass after every substep (reading R14)
     int maxgroups;                 // layout of Workspace::ginfo: [2 maxgroups] (offset, count) per group, then the member lists
 };

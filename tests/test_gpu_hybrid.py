@@ -344,3 +344,45 @@ def test_leapfrog_as_the_first_call_builds_its_own_pair_list():
     st = g.encounter_stats()
     g.close()
     assert st[0] >= 5 and state_err(x, v, res[1][0], res[1][1]) <= 1e-13
+
+
+def test_multilevel_changeover_matches_the_oracle():
+    # NEXT-3, reading R16: L changeover levels with S sub-steps each and radius ratio F between
+    # level 0 and the Bulirsch-Stoer integration.  The oracle recurses over ALL bodies; the library over each group.
+    w = encounter_system()
+    p = oparams(w)
+    for L, S, F in ((2, 3, 2.08), (3, 2, 1.7), (2, 4, 0.0)):
+        Fo = F if F > 0 else float(np.cbrt(S * S))                # the default ratio: S^(2/3)
+        xo, vo = w.x.copy(), oracle.to_democratic(w.m, w.v, w.M_star)
+        E0 = oracle.energy_angmom(w.m, xo, vo, oracle.Params(n1=0.0))[0]
+        g = hybrid(w, enc_levels=L, enc_substeps=S, enc_level_ratio=F)
+        worst, grouped = 0.0, 0
+        for _ in range(30):
+            xo, vo = oracle.step_multilevel(w.m, xo, vo, p, w.dt, L, S, Fo, tol=1e-13)
+            g.step(w.dt, B.FP64)
+            x, v = (t.cpu().numpy() for t in g.get_state())
+            st = g.encounter_stats()
+            assert st[3] == 0 and st[4] == 0
+            grouped += st[0]
+            worst = max(worst, state_err(x, v, xo, vo))
+        E, _ = g.energy_angmom()
+        g.close()
+        assert grouped >= 5 and worst <= 1e-10, (L, S, F, grouped, worst)
+        assert abs(E / E0 - 1) < 1e-6
+    # a disc with planted pairs, a triple and chains of 14 and 23 bodies (warp and CTA teams), three levels
+    w = chain_cluster_disc(700, 5, (14, 23, 3, 2))
+    p = oparams(w)
+    vd = oracle.to_democratic(w.m, w.v, w.M_star)
+    xo, vo = oracle.step_multilevel(w.m, w.x, vd, p, w.dt, 3, 3, 2.08, tol=1e-13)
+    x2, v2 = oracle.step_hybrid_bs(w.m, w.x, vd, p, w.dt, tol=1e-13)
+    assert state_err(x2, v2, xo, vo) > 1e-9                      # the levels are a different splitting, not a relabelling
+    g = hybrid(w, enc_levels=3, enc_substeps=3, enc_level_ratio=2.08)
+    g.step(w.dt, B.FP64)
+    x, v = (t.cpu().numpy() for t in g.get_state())
+    st = g.encounter_stats()
+    g.close()
+    assert st[3] == 0 and st[4] == 0 and st[2] >= 23
+    assert state_err(x, v, xo, vo) <= 1e-10, state_err(x, v, xo, vo)
+    for bad in (dict(enc_levels=2, enc_nsub=16), dict(enc_levels=5), dict(enc_levels=2, enc_level_ratio=0.9)):
+        with pytest.raises(Exception):
+            hybrid(w, **bad).close()
