@@ -209,7 +209,12 @@ int genga_energy_angmom(genga_handle h, double* E, double L[3]);
  * x heliocentric; v as stored (barycentric) unless heliocentric_v != 0 (O1 inverse).            */
 int genga_get_state(genga_handle h, double* x, double* v, int heliocentric_v);
 int genga_get_state_host(genga_handle h, double* x, double* v, int heliocentric_v);
-int genga_get_accel(genga_handle h, double* a);          /* DEVICE [N][3]: a_i of the last force evaluation */
+int genga_get_accel(genga_handle h, double* a);          /* DEVICE [N][3]: a_i of the last force evaluation.  The a_i are
+                                                             sums of per-(body, chunk) partials added with FP64 atomics
+                                                             in no fixed order (all-pairs kernels, near field, merged
+                                                             states in genga_merge): equal from run to run to rounding
+                                                             (1e-16 relative), not bit for bit.  The momentum sums of
+                                                             the step are combined in a fixed order.                   */
 int genga_get_rcrit(genga_handle h, double* rcrit);      /* DEVICE [N]: r_crit,i of the last force evaluation */
 
 /* ---- perfect mergers at a step end (NEXT-4; "collisions ... perfect mergers"; R13) ----
