@@ -252,7 +252,7 @@ __device__ __forceinline__ void accel(const Team& T, const EncParams& P, int& bu
 }
 
 // P.collide: after every substep the collision pass of reading R14 (m, R: this member's mass and radius, updated).
-template <class Team>
+template <bool COLL, class Team>
 __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
                                               double& m, double& R, int body, int* __restrict__ absorb)
 {
@@ -275,7 +275,7 @@ __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P,
         accel<true>(T, P, buf, t[0], t[1], t[2], k0, k1, k2);
         y[0] = fma(h6, sx[0] + u[0], y[0]); y[1] = fma(h6, sx[1] + u[1], y[1]); y[2] = fma(h6, sx[2] + u[2], y[2]);
         y[3] = fma(h6, sv[0] + k0, y[3]); y[4] = fma(h6, sv[1] + k1, y[4]); y[5] = fma(h6, sv[2] + k2, y[5]);
-        if (P.collide) collision_pass(T, P, buf, y, m, R, body, absorb, ctr);
+        if (COLL && P.collide) collision_pass(T, P, buf, y, m, R, body, absorb, ctr);
     }
     if (T.k == 0) { atomicAdd(&ctr->enc_rhs_sum, 4u * (unsigned int)P.nsub); atomicMax(&ctr->enc_rhs_max, 4u * (unsigned int)P.nsub); }
 }
@@ -412,14 +412,16 @@ __device__ __forceinline__ void level_flow(const Team& T, const EncParams& P, do
     }
 }
 
-template <class Team>
+// FULL: with the in-drift collisions (reading R14) and the sub-levels (reading R16).  The per-body kernel is compiled
+// twice: the plain instance (Bulirsch-Stoer or RK4 of the two-level step) keeps its registers; the full one spills.
+template <bool FULL_FEATURES, class Team>
 __device__ __forceinline__ void integrate(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
                                           double& m, double& R, int body, int* __restrict__ absorb)
 {
     if (dt == 0.0) return;
-    if (P.nsub > 0)        integrate_rk4(T, P, dt, y, ctr, m, R, body, absorb);
-    else if (P.levels > 1) level_flow<1>(T, P, 1.0, dt, y, ctr);
-    else                   integrate_bs(T, P, dt, y, ctr);
+    if (P.nsub > 0)                         integrate_rk4<FULL_FEATURES>(T, P, dt, y, ctr, m, R, body, absorb);
+    else if (FULL_FEATURES && P.levels > 1) level_flow<1>(T, P, 1.0, dt, y, ctr);
+    else                                    integrate_bs(T, P, dt, y, ctr);
 }
 
 // Groups in Workspace::ginfo (written by group_kernel): ginfo[2 g] = offset of the member list, ginfo[2 g + 1] = member
@@ -433,6 +435,7 @@ __device__ __forceinline__ const int* group_members(const Workspace& w, int maxg
 // One warp advances a group of n <= WMAX bodies through S(dt/2) (the shift s, already scaled) and the flow of
 // H_A,group over dt, and writes its members back.  Members are taken in ascending body index, so the result does
 // not depend on the order in which group_kernel registered them.
+template <bool FULL_FEATURES>
 __device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, WarpSlab& slab, const int* mem, int n,
                                            double dt, double s0, double s1, double s2)
 {
@@ -461,7 +464,7 @@ __device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, War
     }
     const WarpTeam T{slab, n, active ? lane : -1};
     T.refresh_pairs(P);
-    integrate(T, P, dt, y, w.ctr, m, R, b, w.absorb);
+    integrate<FULL_FEATURES>(T, P, dt, y, w.ctr, m, R, b, w.absorb);
     if (active) {
         w.x[3 * b] = y[0]; w.x[3 * b + 1] = y[1]; w.x[3 * b + 2] = y[2];
         w.v[3 * b] = y[3]; w.v[3 * b + 1] = y[4]; w.v[3 * b + 2] = y[5];
@@ -470,6 +473,7 @@ __device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, War
 }
 
 // The whole CTA (GBIG threads) advances a group of WMAX < n <= GBIG bodies.  Must be called by all threads.
+template <bool FULL_FEATURES>
 __device__ __forceinline__ void block_group(const EncParams& P, Workspace& w, BlockSlab& slab, const int* mem, int n,
                                             double dt, double s0, double s1, double s2)
 {
@@ -498,7 +502,7 @@ __device__ __forceinline__ void block_group(const EncParams& P, Workspace& w, Bl
     }
     __syncthreads();
     const BlockTeam T{slab, n, active ? tid : -1};
-    integrate(T, P, dt, y, w.ctr, mm, R, b, w.absorb);
+    integrate<FULL_FEATURES>(T, P, dt, y, w.ctr, mm, R, b, w.absorb);
     if (active) {
         w.x[3 * b] = y[0]; w.x[3 * b + 1] = y[1]; w.x[3 * b + 2] = y[2];
         w.v[3 * b] = y[3]; w.v[3 * b + 1] = y[4]; w.v[3 * b + 2] = y[5];

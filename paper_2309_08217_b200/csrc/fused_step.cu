@@ -9,8 +9,8 @@ namespace {
 
 using namespace ob;
 
-template <int CHUNK, bool ENC>
-__global__ void __launch_bounds__(FUSED_NT)
+template <int CHUNK, int ENC>
+__global__ void __launch_bounds__(FUSED_NT, ENC ? 1 : 2)
 onbody_kernel(OnBodyArgs A, Workspace w)
 {
     cg::grid_group grid = cg::this_grid();
@@ -102,9 +102,12 @@ group_kernel(int NP, const int2* __restrict__ pairs, Counters* __restrict__ ctr,
 int onbody_max_blocks(const Handle* h, bool enc)
 {
     int occ = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, enc ? onbody_kernel<CHUNK_MAX, true> : onbody_kernel<CHUNK_MAX, false>, FUSED_NT, 0);
+    const bool full = h->p.enc_collide != 0 || h->p.enc_levels > 1;
+    const void* f1 = !enc ? (const void*)onbody_kernel<CHUNK_MAX, 0> : (full ? (const void*)onbody_kernel<CHUNK_MAX, 2> : (const void*)onbody_kernel<CHUNK_MAX, 1>);
+    const void* f2 = !enc ? (const void*)onbody_kernel<CHUNK_MIN, 0> : (full ? (const void*)onbody_kernel<CHUNK_MIN, 2> : (const void*)onbody_kernel<CHUNK_MIN, 1>);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f1, FUSED_NT, 0);
     int occ2 = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, enc ? onbody_kernel<CHUNK_MIN, true> : onbody_kernel<CHUNK_MIN, false>, FUSED_NT, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, f2, FUSED_NT, 0);
     if (occ2 < occ) occ = occ2;
     if (occ < 1) occ = 1;
     long long b = (long long)occ * h->num_sms;
@@ -122,10 +125,13 @@ cudaError_t launch_onbody(const Handle* h, const OnBodyArgs& a, int max_blocks)
     Workspace ws = h->w;
     void* params[] = {&args, &ws};
     const void* fn;
-    if (a.enc.on && a.do_drift)
-        fn = (h->chunk == CHUNK_MIN) ? (const void*)onbody_kernel<CHUNK_MIN, true> : (const void*)onbody_kernel<CHUNK_MAX, true>;
-    else
-        fn = (h->chunk == CHUNK_MIN) ? (const void*)onbody_kernel<CHUNK_MIN, false> : (const void*)onbody_kernel<CHUNK_MAX, false>;
+    if (a.enc.on && a.do_drift) {
+        if (a.enc.collide || a.enc.levels > 1)
+            fn = (h->chunk == CHUNK_MIN) ? (const void*)onbody_kernel<CHUNK_MIN, 2> : (const void*)onbody_kernel<CHUNK_MAX, 2>;
+        else
+            fn = (h->chunk == CHUNK_MIN) ? (const void*)onbody_kernel<CHUNK_MIN, 1> : (const void*)onbody_kernel<CHUNK_MAX, 1>;
+    } else
+        fn = (h->chunk == CHUNK_MIN) ? (const void*)onbody_kernel<CHUNK_MIN, 0> : (const void*)onbody_kernel<CHUNK_MAX, 0>;
     return cudaLaunchCooperativeKernel(fn, dim3(blocks), dim3(FUSED_NT), params, 0, h->stream);
 }
 

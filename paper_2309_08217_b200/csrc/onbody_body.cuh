@@ -63,7 +63,8 @@ __device__ __forceinline__ void block_partial(double p0, double p1, double p2, d
 }
 
 // The kernel as a device function (a cooperative 1-D grid of FUSED_NT-thread blocks).
-template <int CHUNK, bool ENC = false>
+// ENC: 0 no encounter groups, 1 groups by Bulirsch-Stoer / RK4 (two-level step), 2 also in-drift collisions and sub-levels
+template <int CHUNK, int ENC = 0>
 __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, cg::grid_group& grid)
 {
     __shared__ double sP[4];
@@ -122,7 +123,7 @@ __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, c
                 int n;
                 const int* mem = enc::group_members(w, A.enc.maxgroups, g, n);
                 if (n > enc::WMAX) {
-                    if (nbig % (int)gridDim.x == (int)blockIdx.x) enc::block_group(A.enc, w, esm.b, mem, n, A.dt, s0, s1, s2);
+                    if (nbig % (int)gridDim.x == (int)blockIdx.x) enc::block_group<(ENC > 1)>(A.enc, w, esm.b, mem, n, A.dt, s0, s1, s2);
                     ++nbig;
                 }
             }
@@ -131,7 +132,7 @@ __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, c
             for (int g = blockIdx.x + gridDim.x * (threadIdx.x >> 5); g < ngroups; g += gridDim.x * (FUSED_NT / 32)) {
                 int n;
                 const int* mem = enc::group_members(w, A.enc.maxgroups, g, n);
-                if (n <= enc::WMAX) enc::warp_group(A.enc, w, esm.w[threadIdx.x >> 5], mem, n, A.dt, s0, s1, s2);
+                if (n <= enc::WMAX) enc::warp_group<(ENC > 1)>(A.enc, w, esm.w[threadIdx.x >> 5], mem, n, A.dt, s0, s1, s2);
             }
             grid.sync();
             for (int i = gtid; i < N; i += gsz)
