@@ -72,7 +72,7 @@ __device__ __forceinline__ f2 shf2(f2 v, int src) { return __shfl_sync(0xfffffff
 __device__ __forceinline__ double shd(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
 // Shared memory of one warp.  Travelling positions: FP32 16 B per body in two planes per chunk
-// ([CHUNK/2] (x0,x1,y0,y1) then [CHUNK/2] (z0,z1,Gm0,Gm1), chunk-relative), FP64 double4 per body.
+// ([CHUNK/2] (x0,x1,y0,y1) then [CHUNK/2] (z0,z1,Gm0,Gm1), chunk-relative), FP64 32 B per body in four planes (tile64).
 template <bool F32, int CHUNK>
 struct __align__(16) WarpSm {
     static constexpr int POS_BYTES = F32 ? 16 : 32;
@@ -151,7 +151,7 @@ __device__ __forceinline__ void tile32(int lane, const float4* __restrict__ pB, 
     for (int q = 0; q < KP; ++q) { bx[q] = 0ull; by[q] = 0ull; bz[q] = 0ull; mja[q] = 3.0e38f; mjb[q] = 3.0e38f; }
     const int src = (lane + 1) & 31;
 
-#pragma unroll 2      // two steps per iteration: no register renaming moves at the loop end
+#pragma unroll 4      // several steps per iteration: fewer register renaming moves at the loop end
     for (int st = 0; st < 32; ++st) {
         const int owner = (lane + st) & 31;
 #pragma unroll
@@ -265,9 +265,10 @@ __device__ __forceinline__ void tile32(int lane, const float4* __restrict__ pB, 
 // correction: t = y0^2, e = 1 - r^2 t, 1/r^3 = y0^3 (1 + 3/2 e + 15/8 e^2) + O(e^3) (truncation < 1e-17).
 // 20 FP64 operations per unordered pair.  The travelling set is taken two bodies per lane at a time (CHUNK/64
 // rings of 32 steps), which keeps the tile in 128 registers.  Tracking compares the high words of r^2.
-//   pB   set B in shared memory, double4 (x, y, z, G m) per body (absolute positions)
+//   pB   set B in shared memory (absolute positions): four planes of CHUNK/2 double2, plane 2h + 0 = (x, y) and
+//        plane 2h + 1 = (z, G m) of the bodies 2u + h
 template <int CHUNK, int MODE>
-__device__ __forceinline__ void tile64(int lane, const double4* __restrict__ pB, const ChunkP& Ac, const ChunkP& Bc,
+__device__ __forceinline__ void tile64(int lane, const double2* __restrict__ pB, const ChunkP& Ac, const ChunkP& Bc,
                                        const double (&xi)[CHUNK / 32], const double (&yi)[CHUNK / 32],
                                        const double (&zi)[CHUNK / 32], const double (&gi)[CHUNK / 32],
                                        double* __restrict__ aS, double* __restrict__ gT, int NP, int cA, int cB, int N,
@@ -290,7 +291,8 @@ __device__ __forceinline__ void tile64(int lane, const double4* __restrict__ pB,
             const int u = ((lane + st) & 31) + 32 * k;
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                const double4 J = pB[2 * u + h];
+                const double2 Jxy = pB[(2 * h) * (CHUNK / 2) + u], Jzg = pB[(2 * h + 1) * (CHUNK / 2) + u];
+                const double4 J = make_double4(Jxy.x, Jxy.y, Jzg.x, Jzg.y);
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
                     const double dx = J.x - xi[p], dy = J.y - yi[p], dz = J.z - zi[p];
@@ -416,8 +418,13 @@ __device__ __forceinline__ void kick_sym_body(int N, int NP, int nchunk, Workspa
         const char* src = F32 ? reinterpret_cast<const char*>(w.pk32 + (size_t)cB * CHUNK)
                               : reinterpret_cast<const char*>(w.pk64 + (size_t)cB * CHUNK);
 #pragma unroll
-        for (int k = 0; k < CHUNK * Sm::POS_BYTES / 512; ++k)
-            cp_async16(&sm.pos[buf][(k * 32 + lane) * 16], src + (size_t)(k * 32 + lane) * 16);
+        for (int k = 0; k < CHUNK * Sm::POS_BYTES / 512; ++k) {
+            const int piece = k * 32 + lane;                          // 16-byte pieces of the chunk, in memory order
+            // FP64: body b = 2u + h is the pieces 2b (x, y) and 2b + 1 (z, G m); they go to plane 2h + (0 | 1), entry u,
+            // so that lanes reading consecutive pairs u hit consecutive 16-byte words (no bank conflicts in the ring)
+            const int dst = F32 ? piece : (piece & 3) * (CHUNK / 2) + (piece >> 2);
+            cp_async16(&sm.pos[buf][dst * 16], src + (size_t)piece * 16);
+        }
         if (lane < 3) cp_async16(reinterpret_cast<char*>(&sm.bcB[buf]) + 16 * lane, reinterpret_cast<const char*>(w.bc + cB) + 16 * lane);
         cp_async_commit();
     };
@@ -480,7 +487,7 @@ __device__ __forceinline__ void kick_sym_body(int N, int NP, int nchunk, Workspa
             else if (mode == 1) tile32<CHUNK, 1>(lane, pB, Ac, Bc, xS, gi32, aS, gT, NP, A, B, N, w, cand_cap);
             else                tile32<CHUNK, 2>(lane, pB, Ac, Bc, xS, gi32, aS, gT, NP, A, B, N, w, cand_cap);
         } else {
-            const double4* pB = reinterpret_cast<const double4*>(&sm.pos[buf][0]);
+            const double2* pB = reinterpret_cast<const double2*>(&sm.pos[buf][0]);
             if (mode == 0)      tile64<CHUNK, 0>(lane, pB, Ac, Bc, xi, yi, zi, gi64, aS, gT, NP, A, B, N, w, cand_cap);
             else if (mode == 1) tile64<CHUNK, 1>(lane, pB, Ac, Bc, xi, yi, zi, gi64, aS, gT, NP, A, B, N, w, cand_cap);
             else                tile64<CHUNK, 2>(lane, pB, Ac, Bc, xi, yi, zi, gi64, aS, gT, NP, A, B, N, w, cand_cap);
