@@ -96,6 +96,12 @@ typedef struct {
     int    mega_nmax;         /* systems of up to this many bodies run a whole force evaluation (per-body
                                  kernel, all-pairs kick, near field) as ONE cooperative kernel (7 % faster at
                                  N <= 2048, slower from N = 4096 on); 0: default (3000), < 0: never                                                              */
+    int    lean_nmax;         /* systems of up to this many bodies run whole SEQUENCES of force evaluations and steps
+                                 (genga_kick/step/run/leapfrog) in one kernel in which every CTA holds the whole
+                                 system in shared memory and only the pair sums are shared out: one grid-wide
+                                 barrier per step instead of three launches (csrc/lean_step.cu; not in TP2 or
+                                 encounter mode, not while profiling).  0: default (4096, the most an SM's
+                                 shared memory holds), < 0: never                                          */
     int    n_big;             /* TP2 mode ("the giant planets feel the forces of the planetesimals,
                                  but the planetesimals do not feel each other"; reading R9): a pair
                                  (i, j) interacts iff i < n_big or j < n_big.  < 0 (default): every pair.

@@ -55,6 +55,8 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
     const size_t o_rad = take(NP * 8);
     const size_t o_as = take(NP * 24);
     const size_t o_ab = take(NP * 4);
+    const size_t o_a2 = take(NP * 24);
+    const size_t o_lx = take((size_t)LEANX_WORDS * 8);
     if (w && base) {
         char* b = static_cast<char*>(base);
         w->m = (double*)(b + o_m); w->x = (double*)(b + o_x); w->v = (double*)(b + o_v); w->a = (double*)(b + o_a);
@@ -71,6 +73,8 @@ size_t carve_workspace(int N, int pair_cap, int cand_cap, void* base, Workspace*
         w->radius = (double*)(b + o_rad);
         w->aslot = (double*)(b + o_as);
         w->absorb = (int*)(b + o_ab);
+        w->a2 = (double*)(b + o_a2);
+        w->leanx = (unsigned long long*)(b + o_lx);
     }
     return off;
 }
@@ -282,6 +286,49 @@ static int step_mega(Handle* h, int precision, bool do_vel, double tau_v, bool d
     return GENGA_OK;
 }
 
+// The small-system kernel (lean_step.cu): usable for this call?
+static bool lean_ready(Handle* h, int precision)
+{
+    if (h->fused_blocks <= 0 || h->prof != 0 || h->N > h->lean_nmax) return false;
+    if (h->p.n_big >= 0 && h->p.n_big < h->N) return false;          // TP2 mode has its own pair kernel
+    if (h->p.encounter_mode == 1) return false;                      // the groups are formed between two launches
+    const int pi = precision == GENGA_FP32 ? 1 : 0;
+    if (h->lean_blocks[pi] < 0) h->lean_blocks[pi] = lean_max_blocks(h, precision);
+    return h->lean_blocks[pi] > 0;
+}
+
+// The sequence of sequence() below in as few launches of the small-system kernel as the re-sorts allow: the
+// order may only change between two launches.  pending / tau_prev: the velocity update still owed on entry.
+static int sequence_lean(Handle* h, int precision, bool lead_kick, double tau_first, int n_sds, double dt,
+                         double tau_mid, bool pending, double tau_prev)
+{
+    const int E = (lead_kick ? 1 : 0) + n_sds;
+    int e0 = 0;
+    while (e0 < E) {
+        if (h->evals_since_sort < 0 || h->evals_since_sort >= h->resort_every) {
+            const int rc = resort(h);
+            if (rc != GENGA_OK) return rc;
+        }
+        int c = h->resort_every - h->evals_since_sort;
+        if (c > E - e0) c = E - e0;
+        if (c > 4096) c = 4096;                                      // one launch should not hold the device for much longer than a second
+        const int lead = (lead_kick && e0 == 0) ? 1 : 0;
+        const bool pend = e0 == 0 ? pending : true;
+        const double tp = e0 == 0 ? tau_prev : ((lead_kick && e0 == 1) ? tau_first : tau_mid);
+        const PrepArgs a = make_prep_args(h, precision, 0.0);
+        const cudaError_t e = launch_lean(h, a, precision, lead, c - lead, pend ? 1 : 0, tp, tau_first, tau_mid, dt,
+                                          h->lean_blocks[precision == GENGA_FP32 ? 1 : 0], h->lean_seq);
+        h->lean_seq += 2ull * (unsigned long long)(c - lead) + 1ull;  // two exchanges per step (+ one a lone kick may do)
+        ++h->launches;
+        if (e != cudaSuccess) return cuda_fail(e, "lean_kernel (cooperative launch)");
+        std::swap(h->w.a, h->w.a2);                                   // the kernel leaves the new accelerations in the other buffer
+        h->evals_since_sort += c;
+        e0 += c;
+    }
+    h->pairs_current = true;
+    return GENGA_OK;
+}
+
 // K(tau_first)? then n_sds times [S(dt/2) D(dt) S(dt/2) K(tau)], tau = tau_mid except tau_last for the last
 // one.  Fused path: one per-body kernel between two force evaluations (3 launches per step).
 static int sequence(genga_handle h, int precision, bool lead_kick, double tau_first, int n_sds, double dt,
@@ -305,6 +352,11 @@ static int sequence(genga_handle h, int precision, bool lead_kick, double tau_fi
     double tau_prev = h->pend_tau;
     h->pend_vel = false;
     if (n_sds > 0) h->enc_dt = std::fabs(dt);                        // encounter mode: the listings of this sequence look dt ahead
+    if ((lead_kick || n_sds > 0) && lean_ready(h, precision)) {      // small system: the whole sequence in one kernel
+        if ((rc = sequence_lean(h, precision, lead_kick, tau_first, n_sds, dt, tau_mid, pending, tau_prev)) != GENGA_OK) return rc;
+        h->pend_vel = true; h->pend_tau = n_sds > 0 ? tau_last : tau_first; h->mom_a_valid = false;
+        return GENGA_OK;
+    }
     const bool mega = mega_ready(h, precision);                      // small system: one launch per force evaluation
     if (lead_kick) {
         if (mega) { if ((rc = step_mega(h, precision, pending, tau_prev, false, 0.0)) != GENGA_OK) return rc; }
@@ -353,6 +405,7 @@ void genga_default_params(genga_params* p)
     p->n_big = -1;
     p->chunk = 0;
     p->mega_nmax = 0;
+    p->lean_nmax = 0;
     p->weight_mode = 0;
     p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0; p->enc_list_vfactor = 0.0; p->enc_tol = 0.0; p->enc_collide = 0; p->enc_levels = 0; p->enc_substeps = 0; p->enc_level_ratio = 0.0;
 }
@@ -402,7 +455,7 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     // default: every 8 force evaluations where the all-pairs kernel dominates, every 32 for small systems
     // (the refresh is five tiny kernels, ~25 us, which a 40 us step should not pay too often)
     const bool tp2 = p->n_big >= 0 && p->n_big < N;             // O(n_big N) pairs: the order hardly matters
-    h->resort_every = p->resort_every > 0 ? p->resort_every : (tp2 ? 64 : (N >= 16384 ? 8 : 32));
+    h->resort_every = p->resort_every > 0 ? p->resort_every : (tp2 ? 64 : (N >= 16384 ? 8 : (N <= 4096 ? 128 : 32)));
     h->evals_since_sort = -1;
     h->stream = static_cast<cudaStream_t>(p->stream);
     h->num_sms = sms;
@@ -424,6 +477,9 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
             if (h->p.enc_list_scale < 1.0 || h->p.enc_list_scale > 8.0) { delete h; return GENGA_EINVAL; }
         }
         h->mega_blocks[0] = h->mega_blocks[1] = -1;
+        h->lean_blocks[0] = h->lean_blocks[1] = -1;
+        h->lean_seq = 0;
+        h->lean_nmax = p->lean_nmax > 0 ? std::min(p->lean_nmax, lean_nmax_limit()) : (p->lean_nmax < 0 ? 0 : lean_nmax_limit());
         h->mega_nmax = p->mega_nmax > 0 ? p->mega_nmax : (p->mega_nmax < 0 ? 0 : 3000);
     }
     carve_workspace(N, pc, cc, p->workspace, &h->w);

@@ -65,6 +65,7 @@ struct Workspace {
     double* x;        // [NP][3]
     double* v;        // [NP][3]
     double* a;        // [NP][3]  acceleration of the last force evaluation
+    double* a2;       // [NP][3]  the other acceleration buffer of the small-system kernel (lean_step.cu); a and a2 change places
     // per-body derived
     double* hcbrt;    // [NP] cbrt(m / 3 M_star), cached when masses change
     double* rcrit;    // [NP]
@@ -96,8 +97,11 @@ struct Workspace {
     int*     absorb;  // [NP] reading R14: body that absorbed this one inside an encounter integration (-1: none); genga_merge closes up
     double*  aslot;   // [3][NP] sums of the symmetric all-pairs kernels in the internal order (kick_sym_body.cuh: aslot_index),
                       //         zeroed by the prep step, folded into a[] by the near-field kernel
+    unsigned long long* leanx;   // [LEANX_WORDS] exchange slots of the small-system kernel (lean_step.cu: exchange_sums); written by
+                      //         nothing else, and only ever with growing sequence numbers (zero at genga_create)
     Counters* ctr;
 };
+constexpr int LEANX_WORDS = 8192;
 
 constexpr int RED_DOUBLES = 8 + 8 * 1024;   // [0..7] results, [8..8+4096) pair-potential partials, then momentum partials
 
@@ -114,6 +118,9 @@ struct Handle {
     // internal order (a performance hint only: results never depend on it)
     int mega_blocks[2];          // co-resident blocks of the one-kernel step per precision; 0 = not used, -1 = not queried yet
     int mega_nmax;               // largest N that takes the one-kernel step
+    int lean_blocks[2];          // CTAs of the small-system kernel (lean_step.cu) per precision; 0 = not used, -1 = not queried yet
+    int lean_nmax;               // largest N that takes it
+    unsigned long long lean_seq; // grid-wide exchanges its launches have done (the slots in w.mom carry the number, never cleared)
     int enc_blocks;              // co-resident grid of the per-body kernel built with the encounter integrator
     bool enc_labels_valid;       // glabel holds the groups of the drift that led to the current positions
     double enc_dt;               // |dt| of the drift the next listing is for (the last sequence's; params.dt_rcrit before any)
@@ -175,6 +182,11 @@ cudaError_t launch_groups(const Handle* h);                      // encounter gr
 cudaError_t launch_onbody(const Handle* h, const OnBodyArgs& a, int max_blocks);
 int  mega_max_blocks(const Handle* h, int precision);            // the one-kernel step of small systems (mega_step.cu)
 cudaError_t launch_step_mega(const Handle* h, const OnBodyArgs& a, int precision, int max_blocks);
+int  lean_max_blocks(const Handle* h, int precision);            // sequences of steps of a small system in one kernel (lean_step.cu)
+int  lean_nmax_limit();
+cudaError_t launch_lean(const Handle* h, const PrepArgs& prep, int precision, int lead, int n_sds, int pend,
+                        double tau_prev, double tau_first, double tau_mid, double dt, int max_blocks,
+                        unsigned long long seq0);                 // leaves a in w.a2; seq0: grid-wide exchanges done so far
 void launch_hcbrt(const Handle* h);
 void launch_pad(const Handle* h);                            // padding bodies: x = (PAD_POS,0,0), v = 0, m = 0
 int  sort_buffer_words();

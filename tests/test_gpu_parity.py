@@ -583,6 +583,7 @@ def test_one_kernel_step_of_small_systems():
         for prec, tol in ((B.FP64, 1e-12), (B.FP32, 1e-4)):
             res = {}
             for nmax in (1 << 20, -1):                         # one-kernel step / separate kernels
+                kw = dict(kw, lean_nmax=-1)                    # (not the small-system kernel: it has its own test below)
                 g = B.from_workload(w, mega_nmax=nmax, pair_capacity=4 * len(po) + 64, **kw)
                 l0 = g.launch_count()
                 g.kick(w.dt, prec)
@@ -607,6 +608,62 @@ def test_one_kernel_step_of_small_systems():
                     assert (np.linalg.norm(u - v_, axis=1) / np.linalg.norm(v_, axis=1)).max() <= 1e-13
 
 
+def test_small_system_kernel_runs_whole_sequences():
+    # N <= params.lean_nmax (csrc/lean_step.cu): whole sequences of kicks and steps in ONE launch, the CTAs own their
+    # bodies, one grid-wide exchange per step, near pairs in FP64 from shared memory.  Against the oracle: accelerations
+    # and the encounter list of a kick, the state after runs of several steps in one call (genga_run, genga_leapfrog,
+    # genga_step), with a re-sort in the middle of a sequence, for tiny and ragged N, a mass spectrum with test particles
+    # and a coincident pair, Eq. 1 as printed with the max rule, weight mode 1, a dense ring, and N at the kernel's limit.
+    spec = W.config(2, 1700); spec.m[5] = 0.0; spec.m[1203] = 0.0; spec.x[900] = spec.x[899]
+    tiny = W.config(0, 6); tiny.m[1] = 0.0; tiny.x[3] = tiny.x[2]
+    cases = [(W.config(0), {}, {}), (clustered(3, 700), {}, {}), (W.config(2, 900), dict(n1=3.0, n2=0.4, pair_rule=B.PAIR_MAX), {}),
+             (spec, {}, {}), (tiny, {}, {}), (W.config(0, 1), {}, {}), (W.config(0, 2), {}, {}), (W.config(0, 33), {}, {}),
+             (clustered(7, 900), dict(weight_mode=1), {}), (W.config(4, 2560), {}, {}), (W.config(0, 1025), {}, dict(resort_every=3))]
+    for w, okw, gkw in cases:
+        p = oparams(w, **okw)
+        vd = oracle.to_democratic(w.m, w.v, w.M_star)
+        vo, ao = oracle.kick(w.m, w.x, vd, p, w.dt)
+        po = oracle.encounter_pairs(w.m, w.x, vd, p)
+        xr, vr = oracle.run(w.m, w.x, vd, p, w.dt, 5)
+        for prec, tol in ((B.FP64, 1e-12), (B.FP32, 1e-4)):
+            g = B.from_workload(w, pair_capacity=4 * len(po) + 64, **okw, **gkw)
+            l0 = g.launch_count()
+            g.kick(w.dt, prec)
+            assert g.launch_count() - l0 <= 7                  # the sort (momentum + five kernels) and ONE launch
+            a = g.get_accel().cpu().numpy()
+            ok = np.linalg.norm(ao, axis=1) > 0
+            assert rel_err(a[ok], ao[ok]).max() <= tol if ok.any() else True, (w.name, w.m.size, prec, rel_err(a[ok], ao[ok]).max())
+            assert np.all(a[~ok] == 0.0)
+            assert pair_set(g.encounter_pairs()) == pair_set(po), (w.name, w.m.size, prec)
+            _, v = g.get_state()
+            assert (np.linalg.norm(v.cpu().numpy() - vo, axis=1) / np.linalg.norm(vo, axis=1)).max() <= (1e-13 if prec == B.FP64 else 1e-9)
+            g.close()
+            res = {}
+            for how in ("run", "steps"):
+                for lean in (0, -1):                           # the small-system kernel / the separate kernels
+                    g = B.from_workload(w, lean_nmax=lean, mega_nmax=-1, **okw, **gkw)
+                    l0 = g.launch_count()
+                    if how == "steps":                         # kicks that follow kicks, single steps, a negative closing kick
+                        g.step(w.dt, prec); g.step(w.dt, prec)
+                        g.kick(0.5 * w.dt, prec); g.leapfrog(w.dt, 3, prec); g.kick(-0.5 * w.dt, prec)
+                    else:
+                        g.run(w.dt, 5, prec)
+                    res[how, lean] = tuple(t.cpu().numpy() for t in g.get_state()) + (g.launch_count() - l0,)
+                    st = g.nearfield_stats()
+                    assert lean == -1 or (st.candidates == 0 and not st.overflowed)   # this kernel keeps no candidate list
+                    g.close()
+            if "resort_every" not in gkw:
+                assert res["run", 0][2] <= 8 < res["run", -1][2]   # the sort, one launch, the flush of the deferred velocity update
+            gate = 1e-11 if prec == B.FP64 else 2e-7
+            for got, ref in zip(res["run", 0][:2], (xr, vr)):
+                e = np.linalg.norm(got - ref, axis=1) / np.linalg.norm(ref, axis=1)
+                assert e.max() <= gate, (w.name, w.m.size, prec, e.max())
+            if prec == B.FP64:                                 # (two FP32 paths differ by their FP32 rounding)
+                for how in ("run", "steps"):
+                    for u, v_ in zip(res[how, 0][:2], res[how, -1][:2]):
+                        assert (np.linalg.norm(u - v_, axis=1) / np.linalg.norm(v_, axis=1)).max() <= 1e-13, (w.name, how)
+
+
 def test_fp32_self_term_with_heavy_bodies():
     # a body's own FP32 term must be exactly 0 for any mass: with the self pair at r = 0 the plain-record loop forms
     # y = inf (G m y^3 overflowed to inf * 0 = NaN for G m > 3.4e-7 when the term was left to an epsilon in r^2).
@@ -627,8 +684,8 @@ def test_fp32_self_term_with_heavy_bodies():
     for w, kw in cases:
         ao, po, _ = oracle_accel(w)
         for v_ in range(B.num_variants(0)):
-            for nmax in (1 << 20, -1):                              # one-kernel step (plain records) / separate kernels
-                g = B.from_workload(w, mega_nmax=nmax, **kw)
+            for nmax in (1 << 20, -1, 0):                           # one-kernel step (plain records) / separate kernels / small-system kernel
+                g = B.from_workload(w, mega_nmax=nmax, lean_nmax=(0 if nmax == 0 else -1), **kw)
                 g.set_tuning(0, v_)
                 g.kick(0.0, B.FP32)                                 # the path genga_step takes (mega kernel when N <= mega_nmax)
                 a = g.get_accel().cpu().numpy()
