@@ -472,6 +472,18 @@ def run_sweep(args, cpu=True):
                              "kick_kernel_frac_of_peak": flop * pairs / (r["kernel_ms"][0] * 1e-3) / 1e12 / peak,
                              "launches_per_step": r["launches"] / steps,
                              "kernel_variant": B.variant_name(0 if prec == B.FP32 else 1, variant)}
+                # the same steps as ONE genga_leapfrog(steps) call, as a run issues them (small systems then take whole
+                # sequences of steps in one launch: csrc/lean_step.cu)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                l0 = g.launch_count()
+                torch.cuda.synchronize()
+                e0.record()
+                g.leapfrog(w.dt, steps, prec)
+                e1.record()
+                torch.cuda.synchronize()
+                ms1 = e0.elapsed_time(e1)
+                row[name].update({"one_call_ms_per_step": ms1 / steps, "one_call_body_steps_per_s": n * steps / (ms1 * 1e-3),
+                                  "one_call_launches_per_step": (g.launch_count() - l0) / steps})
                 g.close()
         row["clocks"] = sampler.summary()
         if cpu and not args.no_cpu_baseline:

@@ -100,8 +100,11 @@ typedef struct {
                                  (genga_kick/step/run/leapfrog) in one kernel in which every CTA holds the whole
                                  system in shared memory and only the pair sums are shared out: one grid-wide
                                  barrier per step instead of three launches (csrc/lean_step.cu; not in TP2 or
-                                 encounter mode, not while profiling).  0: default (4096, the most an SM's
-                                 shared memory holds), < 0: never                                          */
+                                 encounter mode, not while profiling).  0: default (2560, the most an SM's
+                                 shared memory holds at 80 bytes per body), < 0: never                     */
+    int    lean_min_evals;    /* ... and only for sequences of at least this many force evaluations: a launch
+                                 of that kernel first loads the whole system into every CTA (~11 us at
+                                 N = 1024), which a single genga_step does not win back.  0: default (4)  */
     int    n_big;             /* TP2 mode ("the giant planets feel the forces of the planetesimals,
                                  but the planetesimals do not feel each other"; reading R9): a pair
                                  (i, j) interacts iff i < n_big or j < n_big.  < 0 (default): every pair.

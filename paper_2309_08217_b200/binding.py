@@ -41,7 +41,7 @@ class GengaParams(ctypes.Structure):
         ("lambda_near", ctypes.c_double), ("near_floor", ctypes.c_double),
         ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
         ("pair_capacity", ctypes.c_int), ("cand_capacity", ctypes.c_int), ("resort_every", ctypes.c_int),
-        ("chunk", ctypes.c_int), ("mega_nmax", ctypes.c_int), ("lean_nmax", ctypes.c_int), ("n_big", ctypes.c_int), ("weight_mode", ctypes.c_int), ("no_fused_step", ctypes.c_int),
+        ("chunk", ctypes.c_int), ("mega_nmax", ctypes.c_int), ("lean_nmax", ctypes.c_int), ("lean_min_evals", ctypes.c_int), ("n_big", ctypes.c_int), ("weight_mode", ctypes.c_int), ("no_fused_step", ctypes.c_int),
         ("encounter_mode", ctypes.c_int), ("enc_nsub", ctypes.c_int), ("enc_list_scale", ctypes.c_double), ("enc_list_vfactor", ctypes.c_double), ("enc_tol", ctypes.c_double), ("enc_collide", ctypes.c_int), ("enc_levels", ctypes.c_int), ("enc_substeps", ctypes.c_int), ("enc_level_ratio", ctypes.c_double),
     ]
 
@@ -163,7 +163,7 @@ class Genga:
 
     def __init__(self, m, x, v, *, G=None, M_star=1.0, n1=3.0, n2=0.0, dt_rcrit=0.0,
                  pair_rule=PAIR_MUTUAL_HILL, v_is_heliocentric=True, lambda_near=0.0, near_floor=-1.0,
-                 pair_capacity=0, cand_capacity=0, resort_every=0, chunk=0, mega_nmax=0, lean_nmax=0, n_big=-1, weight_mode=0, no_fused_step=False,
+                 pair_capacity=0, cand_capacity=0, resort_every=0, chunk=0, mega_nmax=0, lean_nmax=0, lean_min_evals=0, n_big=-1, weight_mode=0, no_fused_step=False,
                  encounter_mode=0, enc_nsub=0, enc_list_scale=0.0, enc_list_vfactor=0.0, enc_tol=0.0, enc_collide=0, enc_levels=0, enc_substeps=0, enc_level_ratio=0.0, stream=None, device=None):
         import torch
         self._torch = torch
@@ -186,6 +186,7 @@ class Genga:
         p.chunk = int(chunk)
         p.mega_nmax = int(mega_nmax)
         p.lean_nmax = int(lean_nmax)
+        p.lean_min_evals = int(lean_min_evals)
         p.weight_mode = int(weight_mode)
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         p.stream = ctypes.c_void_p(self._stream.cuda_stream)

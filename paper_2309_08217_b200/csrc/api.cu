@@ -352,7 +352,7 @@ static int sequence(genga_handle h, int precision, bool lead_kick, double tau_fi
     double tau_prev = h->pend_tau;
     h->pend_vel = false;
     if (n_sds > 0) h->enc_dt = std::fabs(dt);                        // encounter mode: the listings of this sequence look dt ahead
-    if ((lead_kick || n_sds > 0) && lean_ready(h, precision)) {      // small system: the whole sequence in one kernel
+    if ((lead_kick ? 1 : 0) + n_sds >= h->lean_min_evals && lean_ready(h, precision)) {   // small system: the whole sequence in one kernel
         if ((rc = sequence_lean(h, precision, lead_kick, tau_first, n_sds, dt, tau_mid, pending, tau_prev)) != GENGA_OK) return rc;
         h->pend_vel = true; h->pend_tau = n_sds > 0 ? tau_last : tau_first; h->mom_a_valid = false;
         return GENGA_OK;
@@ -406,6 +406,7 @@ void genga_default_params(genga_params* p)
     p->chunk = 0;
     p->mega_nmax = 0;
     p->lean_nmax = 0;
+    p->lean_min_evals = 0;
     p->weight_mode = 0;
     p->encounter_mode = 0; p->enc_nsub = 0; p->enc_list_scale = 0.0; p->enc_list_vfactor = 0.0; p->enc_tol = 0.0; p->enc_collide = 0; p->enc_levels = 0; p->enc_substeps = 0; p->enc_level_ratio = 0.0;
 }
@@ -479,6 +480,7 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
         h->mega_blocks[0] = h->mega_blocks[1] = -1;
         h->lean_blocks[0] = h->lean_blocks[1] = -1;
         h->lean_seq = 0;
+        h->lean_min_evals = p->lean_min_evals > 0 ? p->lean_min_evals : 4;
         h->lean_nmax = p->lean_nmax > 0 ? std::min(p->lean_nmax, lean_nmax_limit()) : (p->lean_nmax < 0 ? 0 : lean_nmax_limit());
         h->mega_nmax = p->mega_nmax > 0 ? p->mega_nmax : (p->mega_nmax < 0 ? 0 : 3000);
     }

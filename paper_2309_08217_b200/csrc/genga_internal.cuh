@@ -120,6 +120,7 @@ struct Handle {
     int mega_nmax;               // largest N that takes the one-kernel step
     int lean_blocks[2];          // CTAs of the small-system kernel (lean_step.cu) per precision; 0 = not used, -1 = not queried yet
     int lean_nmax;               // largest N that takes it
+    int lean_min_evals;          // ... and the shortest sequence of force evaluations that does
     unsigned long long lean_seq; // grid-wide exchanges its launches have done (the slots in w.mom carry the number, never cleared)
     int enc_blocks;              // co-resident grid of the per-body kernel built with the encounter integrator
     bool enc_labels_valid;       // glabel holds the groups of the drift that led to the current positions

@@ -626,7 +626,7 @@ def test_small_system_kernel_runs_whole_sequences():
         po = oracle.encounter_pairs(w.m, w.x, vd, p)
         xr, vr = oracle.run(w.m, w.x, vd, p, w.dt, 5)
         for prec, tol in ((B.FP64, 1e-12), (B.FP32, 1e-4)):
-            g = B.from_workload(w, pair_capacity=4 * len(po) + 64, **okw, **gkw)
+            g = B.from_workload(w, pair_capacity=4 * len(po) + 64, lean_min_evals=1, **okw, **gkw)
             l0 = g.launch_count()
             g.kick(w.dt, prec)
             assert g.launch_count() - l0 <= 7                  # the sort (momentum + five kernels) and ONE launch
@@ -641,7 +641,7 @@ def test_small_system_kernel_runs_whole_sequences():
             res = {}
             for how in ("run", "steps"):
                 for lean in (0, -1):                           # the small-system kernel / the separate kernels
-                    g = B.from_workload(w, lean_nmax=lean, mega_nmax=-1, **okw, **gkw)
+                    g = B.from_workload(w, lean_nmax=lean, lean_min_evals=1, mega_nmax=-1, **okw, **gkw)
                     l0 = g.launch_count()
                     if how == "steps":                         # kicks that follow kicks, single steps, a negative closing kick
                         g.step(w.dt, prec); g.step(w.dt, prec)
@@ -685,7 +685,7 @@ def test_fp32_self_term_with_heavy_bodies():
         ao, po, _ = oracle_accel(w)
         for v_ in range(B.num_variants(0)):
             for nmax in (1 << 20, -1, 0):                           # one-kernel step (plain records) / separate kernels / small-system kernel
-                g = B.from_workload(w, mega_nmax=nmax, lean_nmax=(0 if nmax == 0 else -1), **kw)
+                g = B.from_workload(w, mega_nmax=nmax, lean_nmax=(0 if nmax == 0 else -1), lean_min_evals=1, **kw)
                 g.set_tuning(0, v_)
                 g.kick(0.0, B.FP32)                                 # the path genga_step takes (mega kernel when N <= mega_nmax)
                 a = g.get_accel().cpu().numpy()
