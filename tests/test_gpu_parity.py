@@ -613,10 +613,13 @@ def test_small_system_kernel_runs_whole_sequences():
     # bodies, one grid-wide exchange per step, near pairs in FP64 from shared memory.  Against the oracle: accelerations
     # and the encounter list of a kick, the state after runs of several steps in one call (genga_run, genga_leapfrog,
     # genga_step), with a re-sort in the middle of a sequence, for tiny and ragged N, a mass spectrum with test particles
-    # and a coincident pair, Eq. 1 as printed with the max rule, weight mode 1, a dense ring, and N at the kernel's limit.
+    # and a coincident pair, Eq. 1 as printed with the max rule and with the mutual-Hill rule, unbound and nearly parabolic
+    # bodies (the bound of their pairs is infinite), weight mode 1, a dense ring, and N at the kernel's limit.
     spec = W.config(2, 1700); spec.m[5] = 0.0; spec.m[1203] = 0.0; spec.x[900] = spec.x[899]
     tiny = W.config(0, 6); tiny.m[1] = 0.0; tiny.x[3] = tiny.x[2]
+    fly = W.config(0, 400); fly.v[7] *= 1.6; fly.v[9] *= np.sqrt(2.0) * (1.0 + 1e-9); fly.v[11] *= np.sqrt(2.0) * (1.0 - 1e-9)   # unbound and (nearly) parabolic bodies
     cases = [(W.config(0), {}, {}), (clustered(3, 700), {}, {}), (W.config(2, 900), dict(n1=3.0, n2=0.4, pair_rule=B.PAIR_MAX), {}),
+             (W.config(0, 600), dict(n1=3.0, n2=0.4), {}), (fly, {}, {}),
              (spec, {}, {}), (tiny, {}, {}), (W.config(0, 1), {}, {}), (W.config(0, 2), {}, {}), (W.config(0, 33), {}, {}),
              (clustered(7, 900), dict(weight_mode=1), {}), (W.config(4, 2560), {}, {}), (W.config(0, 1025), {}, dict(resort_every=3))]
     for w, okw, gkw in cases:
