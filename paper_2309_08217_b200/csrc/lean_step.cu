@@ -180,10 +180,11 @@ __host__ __device__ constexpr int lean_ib(bool f32) { return f32 ? 4 : 2; }     
 // the ranges' partials are added in a fixed order -> aloc[3 (s - s_lo) + c].  A pass of a warp is free of calls and
 // branches: IB bodies against 32 j-bodies; FP32 kernel: FP32 terms summed in FP32 per lane (at most N / 32 terms),
 // lanes and ranges combined in FP64; FP64 kernel: the refined-rsqrt term of nearfield_body.cuh.  A pair inside its near
-// bound contributes nothing there: bit `it` of a lane's mask records it, and after a block of 32 passes the flagged
-// pairs are queued (si, sj, zone bound) for the whole CTA, which evaluates them in FP64 (near_pair), one thread per
-// pair, and adds the terms to aloc (atomically: the order of these few additions is not fixed).  A pair that finds the
-// queue full is evaluated on the spot.  rfg2: Rf^2 of this CTA (see the head of the file); rfo2: without the frame
+// bound contributes nothing there: bit `it` of a lane's mask records it, and after a block of 32 passes the lane looks at
+// its flagged pairs in FP64: outside lambda^-1 of its bound a pair is certainly outside its changeover zone and gets
+// the plain FP64 term at once; the others are queued (si, sj, zone bound) for the whole CTA, which evaluates them
+// (near_pair -> exact_pair), one thread per pair, and adds the terms to aloc (atomically: the order of these few
+// additions is not fixed).  A pair that finds the queue full is evaluated on the spot.  rfg2: Rf^2 of this CTA (see the head of the file); rfo2: without the frame
 // guard; ilam2: lambda^-2 rounded up; list: append the encounter pairs to the list (the last evaluation of the call).
 template <bool F32>
 __device__ __forceinline__ void lean_kick(const LeanSm<F32>& S, const LeanArgs& L, const Workspace& w, int N, int g0, int g1,
@@ -276,6 +277,13 @@ __device__ __forceinline__ void lean_kick(const LeanSm<F32>& S, const LeanArgs& 
                     m &= m - 1u;
                     if (j == sib[b]) continue;
                     const float zc = fmaxf(fmaxf(cn[b], S.C[j]), rfo2) * ilam2;
+                    const double dx = S.X[j] - S.X[sib[b]], dy = S.Y[j] - S.Y[sib[b]], dz = S.Z[j] - S.Z[sib[b]];
+                    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                    if (r2 > (double)zc) {                                   // certainly outside its zone: the plain FP64 term, here and now
+                        const double s = S.GM[j] / (r2 * sqrt(r2));
+                        ex[b] = fma(s, dx, ex[b]); ey[b] = fma(s, dy, ey[b]); ez[b] = fma(s, dz, ez[b]);
+                        continue;
+                    }
                     const int k = atomicAdd(qn, 1);
                     if (k < LEAN_QCAP) S.queue[k] = make_int4(sib[b], j, __float_as_int(zc), 0);
                     else near_pair<F32>(S, L, w, sib[b], j, zc, list, ex[b], ey[b], ez[b]);
