@@ -457,7 +457,10 @@ lean_kernel(const __grid_constant__ LeanArgs L, const __grid_constant__ Workspac
     unsigned long long* pg1 = w.leanx;
     unsigned long long* pg2 = pg1 + 2 * LEAN_SLOTW;
     unsigned long long seq = L.seq0;
-    double4* xg = w.pk64;                                         // the drifted (x, |v|^2) of every slot
+    // the drifted (x, |v|^2) of every slot, in two buffers that alternate from step to step: with one exchange per step a fast
+    // CTA may publish step e + 1 while a slow one is still loading step e; it cannot get to step e + 2 before that one has
+    // published step e + 1, i.e. is done loading
+    double4* const xgb[2] = {w.pk64, w.aux};
 
     // per-thread part of the near bounds of an evaluation (see below): bound_orbit of every slot this thread loads
     const float n2dtf = __double2float_ru(lam * A.n2 * A.dt_rcrit);
@@ -534,7 +537,7 @@ lean_kernel(const __grid_constant__ LeanArgs L, const __grid_constant__ Workspac
             if (own) {
                 double x0 = S.X[so] + sc * sP[0], y0 = S.Y[so] + sc * sP[1], z0 = S.Z[so] + sc * sP[2];
                 if (L.dt != 0.0) { if (!kepler_drift(L.mu, L.dt, x0, y0, z0, vx, vy, vz)) atomicAdd(&w.ctr->noconv, 1u); }
-                double2* g2 = reinterpret_cast<double2*>(&xg[so]);
+                double2* g2 = reinterpret_cast<double2*>(&xgb[e & 1][so]);
                 __stcg(g2, make_double2(x0, y0)); __stcg(g2 + 1, make_double2(z0, vx * vx + vy * vy + vz * vz));
                 p0 = mo * vx; p1 = mo * vy; p2 = mo * vz; mt = mo;
             }
@@ -546,7 +549,7 @@ lean_kernel(const __grid_constant__ LeanArgs L, const __grid_constant__ Workspac
             const double s0 = sc * sP[0], s1 = sc * sP[1], s2 = sc * sP[2];
             asum = acnt = vkmax = 0.f;
             for (int s = t; s < N; s += LEAN_NT) {
-                const double2* g2 = reinterpret_cast<const double2*>(&xg[s]);
+                const double2* g2 = reinterpret_cast<const double2*>(&xgb[e & 1][s]);
                 const double2 qa = __ldcg(g2), qb = __ldcg(g2 + 1);
                 const double px = qa.x + s0, py = qa.y + s1, pz = qb.x + s2;
                 S.X[s] = px; S.Y[s] = py; S.Z[s] = pz; S.V2[s] = qb.y;
