@@ -383,7 +383,12 @@ static int flush_pending(genga_handle h)
 {
     if (!h->pend_vel) return GENGA_OK;
     h->pend_vel = false;
-    return onbody(h, GENGA_FP64, true, h->pend_tau, false, 0.0, false);
+    if (h->N == 0) return GENGA_OK;
+    // one plain kernel: v += tau a and, in its epilogue, sum m v of the new velocities (slot A), which a read of the
+    // heliocentric velocities needs next; the cooperative per-body kernel would cost three times as much here
+    launch_velupdate_mom(h, h->pend_tau); LAUNCHED(h, "velupdate_mom_kernel");
+    h->mom_a_valid = true;
+    return GENGA_OK;
 }
 
 extern "C" {
