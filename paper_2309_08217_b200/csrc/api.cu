@@ -192,6 +192,8 @@ static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_d
     a.do_vel = do_vel; a.do_drift = do_drift; a.do_prep = do_prep;
     a.tau_v = tau_v; a.dt = dt; a.mu = h->p.G * h->p.M_star;
     const bool enc = h->p.encounter_mode == 1 && do_drift;
+    // (not with encounter groups: their warps read velocities that other blocks have just updated, which the barrier of the sum orders)
+    a.reuse_P = (do_drift && h->mom_b_valid && !enc) ? 1 : 0;
     a.enc.on = enc ? 1 : 0; a.enc.nsub = h->p.enc_nsub; a.enc.pair_rule = h->p.pair_rule;
     a.enc.pair_cap = (unsigned int)h->pair_cap;
     a.enc.G = h->p.G; a.enc.M_star = h->p.M_star; a.enc.n1 = h->p.n1; a.enc.n2dt = h->p.n2 * h->p.dt_rcrit;
@@ -215,6 +217,7 @@ static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_d
     ++h->launches;
     if (e != cudaSuccess) return cuda_fail(e, "onbody_kernel (cooperative launch)");
     h->mom_a_valid = !do_drift;          // slot A holds sum m v of the stored velocities unless the drift changed them
+    if (do_drift) h->mom_b_valid = !(h->p.n_big >= 0 && h->p.n_big < h->N);   // slot B: sum m v' (reading R17; not in TP2 mode)
     return GENGA_OK;
 }
 
@@ -278,11 +281,13 @@ static int step_mega(Handle* h, int precision, bool do_vel, double tau_v, bool d
     a.prep.scaled = 0;                                               // the fused all-pairs phase reads plain j-records
     a.do_vel = do_vel; a.do_drift = do_drift; a.do_prep = 1;
     a.tau_v = tau_v; a.dt = dt; a.mu = h->p.G * h->p.M_star;
+    a.reuse_P = (do_drift && h->mom_b_valid) ? 1 : 0;
     const cudaError_t e = launch_step_mega(h, a, precision, h->mega_blocks[precision == GENGA_FP32 ? 1 : 0]);
     ++h->launches;
     if (e != cudaSuccess) return cuda_fail(e, "step_kernel (cooperative launch)");
     h->pairs_current = true;
     h->mom_a_valid = !do_drift;
+    if (do_drift) h->mom_b_valid = true;                             // (mega_ready excludes TP2 mode)
     return GENGA_OK;
 }
 
@@ -355,6 +360,7 @@ static int sequence(genga_handle h, int precision, bool lead_kick, double tau_fi
     if ((lead_kick ? 1 : 0) + n_sds >= h->lean_min_evals && lean_ready(h, precision)) {   // small system: the whole sequence in one kernel
         if ((rc = sequence_lean(h, precision, lead_kick, tau_first, n_sds, dt, tau_mid, pending, tau_prev)) != GENGA_OK) return rc;
         h->pend_vel = true; h->pend_tau = n_sds > 0 ? tau_last : tau_first; h->mom_a_valid = false;
+        if (n_sds > 0) h->mom_b_valid = true;                        // the kernel's last drift left sum m v' in slot B
         return GENGA_OK;
     }
     const bool mega = mega_ready(h, precision);                      // small system: one launch per force evaluation
@@ -522,8 +528,8 @@ static int set_state_impl(genga_handle h, const double* m, const double* x, cons
     if (n == 0) return GENGA_OK;
     if (m) CU(cudaMemcpyAsync(h->w.m, m, n * 8, kind, h->stream));
     if (x) { CU(cudaMemcpyAsync(h->w.x, x, n * 24, kind, h->stream)); h->enc_labels_valid = false; h->pairs_current = false; }
-    if (v) { CU(cudaMemcpyAsync(h->w.v, v, n * 24, kind, h->stream)); h->mom_a_valid = false; }
-    if (m) { h->mom_a_valid = false; h->pairs_current = false; h->enc_labels_valid = false; }   // r_crit follows m
+    if (v) { CU(cudaMemcpyAsync(h->w.v, v, n * 24, kind, h->stream)); h->mom_a_valid = false; h->mom_b_valid = false; }
+    if (m) { h->mom_a_valid = false; h->mom_b_valid = false; h->pairs_current = false; h->enc_labels_valid = false; }   // r_crit follows m
     if (m) { launch_hcbrt(h); LAUNCHED(h, "hcbrt_kernel"); }
     if (v && h->p.v_is_heliocentric) return to_democratic(h);
     return GENGA_OK;
@@ -600,6 +606,7 @@ int genga_merge(genga_handle h, int precision, int* newidx, int* n_merged, int* 
     h->grid_cache[0][0] = h->grid_cache[1][0] = 0;
     h->evals_since_sort = -1;
     h->mom_a_valid = false;
+    h->mom_b_valid = false;
     launch_pad(h); LAUNCHED(h, "pad_kernel");
     launch_hcbrt(h); LAUNCHED(h, "hcbrt_kernel");
     return force_eval(h, precision);                                  // pair list, a, r_crit of the new body set
@@ -633,6 +640,7 @@ int genga_drift(genga_handle h, double dt)
     LAUNCHED(h, "drift_kernel");
     h->pairs_current = false;
     h->mom_a_valid = false;
+    h->mom_b_valid = false;
     h->enc_labels_valid = false;                     // a plain Kepler drift: no groups led to these positions
     return GENGA_OK;
 }

@@ -129,6 +129,8 @@ struct Handle {
     bool pend_vel;               // a closing velocity update v += pend_tau a is still owed (api.cu: sequence)
     double pend_tau;
     bool mom_a_valid;            // mom[SLOT_A] holds sum m v of the stored velocities
+    bool mom_b_valid;            // mom[SLOT_B] holds sum m v' of the last drift and only kicks have touched v since: by reading R17
+                                 // it is the momentum the next Sun-kick needs (never set in TP2 mode: forces are not reciprocal there)
     bool pairs_current;          // the encounter list was made from the current positions (genga_merge relies on it)
     int grid_cache[2][2];        // per kernel (FP32, FP64): variant + 1 it was computed for, grid size
     int tune[4];                 // genga_set_tuning: [0] kick32 variant, [1] kick64 variant
@@ -174,6 +176,7 @@ struct OnBodyArgs {               // the fused per-body kernel of the step (fuse
     PrepArgs prep;
     EncArgs enc;
     int do_vel, do_drift, do_prep;
+    int reuse_P;                   // do_drift: take sum m v from mom[SLOT_B] instead of summing it (reading R17)
     double tau_v;                  // v += tau_v a          (do_vel)
     double dt, mu;                 // S(dt/2) D(dt) S(dt/2)  (do_drift; the closing S is applied by phase 3)
 };

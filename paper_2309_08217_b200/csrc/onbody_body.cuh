@@ -74,7 +74,18 @@ __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, c
     double* part2 = part1 + 4 * MOM_MAX_BLOCKS;
 
     // ---- phase 1: close the previous kick, total momentum of the stored velocities ----------------
-    {
+    if (A.do_drift && A.reuse_P) {
+        // reading R17: a kick does not change the total momentum (reciprocal pair forces), so sum m v of the velocities this
+        // phase produces is the sum m v' the previous drift left in slot B: no sum, no grid-wide barrier.  (Each thread
+        // updates and later drifts the same bodies i = gtid + k gsz: no other ordering is needed.)
+        if (A.do_vel)
+            for (int i = gtid; i < N; i += gsz) {
+                w.v[3 * i + 0] = fma(A.tau_v, w.a[3 * i + 0], w.v[3 * i + 0]); w.v[3 * i + 1] = fma(A.tau_v, w.a[3 * i + 1], w.v[3 * i + 1]);
+                w.v[3 * i + 2] = fma(A.tau_v, w.a[3 * i + 2], w.v[3 * i + 2]);
+            }
+        if (threadIdx.x < 4) sP[threadIdx.x] = w.mom[MOM_SLOT_B + threadIdx.x];
+        __syncthreads();
+    } else {
         double p0 = 0, p1 = 0, p2 = 0, mt = 0;
         for (int i = gtid; i < N; i += gsz) {
             double v0 = w.v[3 * i + 0], v1 = w.v[3 * i + 1], v2 = w.v[3 * i + 2];
