@@ -200,6 +200,11 @@ int genga_step(genga_handle h, double dt, int precision);
 /* nsteps steps with adjacent half-kicks merged: K(dt/2) [S D S K(dt)]^(nsteps-1) S D S K(dt/2),
  * nsteps + 1 force evaluations (reading R7).                                          */
 int genga_run(genga_handle h, double dt, int nsteps, int precision);
+/* (genga_run and genga_leapfrog hand systems of up to params.lean_nmax bodies to one kernel for the whole
+ * sequence: issue the steps of a run in one call rather than one by one.  Inside such a call the momentum of
+ * the Sun-kick before a drift is the one summed after the previous drift, reading R17, and the
+ * sums of the few pairs inside their near bound are added in no fixed order: the accelerations of bodies
+ * with two or more such pairs are reproducible to rounding, not bit for bit.)                            */
 
 /* The body of that loop on its own: [S(dt/2) D(dt) S(dt/2) K(dt)]^nsteps, one force evaluation
  * per step.  genga_kick(dt/2), genga_leapfrog(n), genga_kick(-dt/2) equals genga_run(n) up to
