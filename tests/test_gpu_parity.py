@@ -614,7 +614,8 @@ def test_small_system_kernel_runs_whole_sequences():
     # and the encounter list of a kick, the state after runs of several steps in one call (genga_run, genga_leapfrog,
     # genga_step), with a re-sort in the middle of a sequence, for tiny and ragged N, a mass spectrum with test particles
     # and a coincident pair, Eq. 1 as printed with the max rule and with the mutual-Hill rule, unbound and nearly parabolic
-    # bodies (the bound of their pairs is infinite), weight mode 1, a dense ring, and N at the kernel's limit.
+    # bodies (the bound of their pairs is infinite), weight mode 1, a dense ring (35 683 encounter pairs among 700 bodies:
+    # ~800 zone pairs per CTA and evaluation, three times what a CTA queues), and N at the kernel's limit.
     spec = W.config(2, 1700); spec.m[5] = 0.0; spec.m[1203] = 0.0; spec.x[900] = spec.x[899]
     tiny = W.config(0, 6); tiny.m[1] = 0.0; tiny.x[3] = tiny.x[2]
     fly = W.config(0, 400); fly.v[7] *= 1.6; fly.v[9] *= np.sqrt(2.0) * (1.0 + 1e-9); fly.v[11] *= np.sqrt(2.0) * (1.0 - 1e-9)   # unbound and (nearly) parabolic bodies
