@@ -56,7 +56,8 @@ typedef enum {
     GENGA_ENOMEM    = -2,   /* params.workspace_bytes < genga_workspace_bytes(N, params)            */
     GENGA_ECAPACITY = -3,   /* encounter-pair list overflow: first cap pairs written, *count = total */
     GENGA_ECUDA     = -4,   /* a CUDA runtime call failed; genga_last_cuda_error() has the text      */
-    GENGA_ENOCONV   = -5    /* Kepler solver failed to converge for >= 1 body (state still written)  */
+    GENGA_ENOCONV   = -5,   /* Kepler solver failed to converge for >= 1 body (state still written)  */
+    GENGA_ELIMIT    = -6    /* size beyond the fixed maximum of a no-allocation entry point          */
 } genga_status;
 
 /* PAPER.md:223 "Do Kick in single precision = 0 / 1". */
@@ -311,6 +312,30 @@ const char* genga_version(void);
  * per second (an FFMA2 counts 2).  stream as in params.  Synchronises.  bench.py prints these beside the
  * derived peaks its roofline fractions are quoted against.                                              */
 int genga_peak_probe(int which, int iters, void* stream, double* ops_per_s, double* ms);
+
+/* ---- an entry point that allocates nothing ---------------------------------------------------------------
+ * E and L (O11) of a state given as plain DEVICE arrays, for callers that cannot allocate (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): no handle, no workspace.
+ * Its scratch (the bodies packed into padded tiles, the per-block partials of the pair potential) is a
+ * file-scope __device__ array of the library (csrc/noalloc.cu), 4.2 MB that every GPU holds from the moment
+ * it loads the library until the process exits.  The call makes no cudaMalloc / cudaFree and calls no
+ * allocating library routine; the first call on a device asks the runtime for the array's device address.
+ *   N      bodies, 0 <= N <= GENGA_STATIC_NMAX; more: GENGA_ELIMIT (text: genga_static_last_error())
+ *   m      DEVICE double[N]; x, v: DEVICE double[N][3], x heliocentric, v barycentric (democratic variables:
+ *          what genga_get_state returns with heliocentric_v = 0)
+ *   G, M_star   as in genga_params (M_star > 0)
+ *   stream cudaStream_t (NULL: the default stream) of the CURRENT device; the arrays must live there
+ *   out4   DEVICE double[4], receives (E, Lx, Ly, Lz); written asynchronously on `stream`
+ * Same arithmetic as genga_energy_angmom (every pair interacts: no TP2 case); the results agree to rounding
+ * (the summation order of the pair potential follows the padding: 128 here, 512 there).
+ * ALL calls share the one array, which keeps the last call's contents (nothing in it needs clearing: a call
+ * rewrites all it reads): calls on one stream are ordered and safe, calls that OVERLAP on the GPU (different
+ * streams or unordered host threads) race on it and return garbage.  Asynchronous; nothing is synchronised. */
+#define GENGA_STATIC_NMAX 131072
+int genga_energy_angmom_static(int N, const double* m, const double* x, const double* v, double G, double M_star,
+                               void* stream, double* out4);
+/* Text of the last error of genga_energy_angmom_static in this host thread ("" if none).                    */
+const char* genga_static_last_error(void);
 
 #ifdef __cplusplus
 }

@@ -18,7 +18,8 @@ FP32 = 1
 PAIR_MAX = 0
 PAIR_MUTUAL_HILL = 1
 
-OK, EINVAL, ENOMEM, ECAPACITY, ECUDA, ENOCONV = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOMEM, ECAPACITY, ECUDA, ENOCONV, ELIMIT = 0, -1, -2, -3, -4, -5, -6
+STATIC_NMAX = 131072          # GENGA_STATIC_NMAX of include/genga.h
 
 # every symbol include/genga.h declares (tests check the library exports all of them)
 SYMBOLS = [
@@ -30,6 +31,7 @@ SYMBOLS = [
     "genga_nearfield_stats", "genga_encounter_stats", "genga_encounter_work", "genga_set_profiling", "genga_kernel_time", "genga_launch_count",
     "genga_synchronize", "genga_strerror", "genga_last_cuda_error", "genga_version",
     "genga_peak_probe", "genga_set_tuning", "genga_autotune", "genga_num_variants", "genga_variant_name",
+    "genga_energy_angmom_static", "genga_static_last_error",
 ]
 
 
@@ -108,6 +110,8 @@ def load() -> ctypes.CDLL:
     L.genga_autotune.argtypes = [vp, ctypes.c_int, ip, dp]
     L.genga_num_variants.argtypes = [ctypes.c_int]
     L.genga_variant_name.argtypes = [ctypes.c_int, ctypes.c_int]; L.genga_variant_name.restype = ctypes.c_char_p
+    L.genga_energy_angmom_static.argtypes = [ctypes.c_int, vp, vp, vp, ctypes.c_double, ctypes.c_double, vp, vp]
+    L.genga_static_last_error.argtypes = []; L.genga_static_last_error.restype = ctypes.c_char_p
     for name in SYMBOLS:
         fn = getattr(L, name)
         if fn.restype is ctypes.c_int and name not in ("genga_launch_count",):
@@ -138,6 +142,17 @@ def peak_probe(which: int, iters: int = 4096, stream: int = 0):
     _check(load().genga_peak_probe(which, iters, ctypes.c_void_p(stream), ctypes.byref(ops), ctypes.byref(ms)),
            "genga_peak_probe")
     return ops.value, ms.value
+
+
+def energy_angmom_static(N: int, m_ptr: int, x_ptr: int, v_ptr: int, G: float, M_star: float, stream: int, out4_ptr: int) -> None:
+    """genga_energy_angmom_static (the entry point that allocates nothing): raw DEVICE addresses in, (E, Lx, Ly, Lz)
+    written to the DEVICE address out4_ptr, asynchronously on `stream`.  Marshalling only: this wrapper allocates nothing
+    either.  Raises GengaError (code ELIMIT for N > STATIC_NMAX) with the library's own text."""
+    L = load()
+    code = L.genga_energy_angmom_static(int(N), ctypes.c_void_p(m_ptr), ctypes.c_void_p(x_ptr), ctypes.c_void_p(v_ptr),
+                                        float(G), float(M_star), ctypes.c_void_p(stream), ctypes.c_void_p(out4_ptr))
+    if code != OK:
+        raise GengaError(code, f"genga_energy_angmom_static: {L.genga_strerror(code).decode()}: {L.genga_static_last_error().decode()}")
 
 
 def num_variants(key: int) -> int:

@@ -18,7 +18,7 @@ _INC = os.path.join(os.path.dirname(_HERE), "include")
 LIB_PATH = os.path.join(_HERE, "libgenga_b200.so")
 _OBJ_DIR = os.path.join(_HERE, "build")
 
-SOURCES = ["api.cu", "prep.cu", "fused_step.cu", "mega_step.cu", "lean_step.cu", "kick_fp32.cu", "kick_fp64.cu", "nearfield.cu", "drift.cu", "reduce.cu", "merge.cu", "probe.cu"]
+SOURCES = ["api.cu", "prep.cu", "fused_step.cu", "mega_step.cu", "lean_step.cu", "kick_fp32.cu", "kick_fp64.cu", "nearfield.cu", "drift.cu", "reduce.cu", "merge.cu", "probe.cu", "noalloc.cu"]
 HEADERS = ["genga_internal.cuh", "tile_pipeline.cuh", "momentum.cuh", "kepler.cuh", "prep_tile.cuh",
            "kick32_body.cuh", "kick64_body.cuh", "kick_sym_body.cuh", "nearfield_body.cuh", "onbody_body.cuh", "encounter.cuh"]
 

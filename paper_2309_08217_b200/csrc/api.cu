@@ -853,6 +853,7 @@ const char* genga_strerror(int code)
         case GENGA_ECAPACITY: return "encounter-pair list capacity exceeded";
         case GENGA_ECUDA:     return "CUDA error";
         case GENGA_ENOCONV:   return "Kepler solver did not converge";
+        case GENGA_ELIMIT:    return "size beyond the fixed maximum of a no-allocation entry point (genga_static_last_error)";
         default:              return "unknown error";
     }
 }
