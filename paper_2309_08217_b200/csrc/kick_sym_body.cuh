@@ -402,7 +402,11 @@ __device__ __forceinline__ void kick_sym_body(int N, int NP, int nchunk, Workspa
     // tiles (A, B >= A), row by row: row A starts at tile A n - A (A - 1) / 2 and has n - A tiles
     const long long n = nchunk;
     const long long NTILE = n * (n + 1) / 2;
-    const long long nwarp = (long long)gridDim.x * (blockDim.x >> 5), gw = (long long)blockIdx.x * (blockDim.x >> 5) + wid;
+    // Range gw of the tiles goes to warp (gw / gridDim.x) of CTA (gw % gridDim.x): neighbouring ranges sit on different
+    // SMs.  The ranges are not equally dear -- the last ones are the short rows at the corner of the triangle, all
+    // diagonal and near tiles and a row change every few tiles -- and with CTA b holding the ranges 12 b .. 12 b + 11
+    // the last dozen SMs finished 20 % after the others (N = 16 384: 110 against 92 us; now 100).
+    const long long nwarp = (long long)gridDim.x * (blockDim.x >> 5), gw = (long long)wid * gridDim.x + blockIdx.x;
     long long t = (NTILE * gw) / nwarp;
     const long long t1 = (NTILE * (gw + 1)) / nwarp;
     if (t >= t1) return;
