@@ -28,7 +28,7 @@ struct __align__(16) BoundP { float hq, aq, rf, pad; };
 // per-chunk record staged next to the j-tile: the maxima of the bound parameters over the chunk
 // and the origin of the chunk's local frame (FP32 policy P32: the FP32 kernel sees positions
 // relative to o; Rf already contains the frame guard floor * 2 * max_j |x_j - o|).
-struct __align__(16) ChunkP { double ox, oy, oz; float hq, aq, rf, rad; float q2max, pad_; };
+struct __align__(16) ChunkP { double ox, oy, oz; float hq, aq, rf, rad; float q2max, uni; };   // uni = 1: every slot of the chunk is live and all carry bitwise the same G m (else 0)
 static_assert(sizeof(ChunkP) == 48, "ChunkP is staged with 16-byte bulk copies");
 
 // j-side layouts.  FP32: two bodies per pair of float4 (packed for FFMA2 along j), in two planes per chunk:

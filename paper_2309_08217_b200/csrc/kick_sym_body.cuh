@@ -123,7 +123,9 @@ __device__ __forceinline__ bool tile_is_far(const ChunkP& A, const ChunkP& B)
 //   pB   set B in shared memory: planes [CHUNK/2] (x0,x1,y0,y1), [CHUNK/2] (z0,z1,Gm0,Gm1), relative to Bc's origin
 //   xS   this warp's stationary FP64 positions [3][CHUNK];  gi: G m of the lane's stationary bodies
 //   aS   this warp's stationary FP64 sums [3][CHUNK];  gT: aslot[] at chunk B (component stride NP)
-template <int CHUNK, int MODE>
+//   UNI  (far tiles only) both chunks are uniform in mass (ChunkP::uni): G m_B and -G m_A are factored out of the pair loop
+//        (14 instead of 16 packed operations per two unordered pairs) and multiplied in, in FP64, when the sums leave the tile
+template <int CHUNK, int MODE, bool UNI = false>
 __device__ __forceinline__ void tile32(int lane, const float4* __restrict__ pB, const ChunkP& Ac, const ChunkP& Bc,
                                        const double* __restrict__ xS, const float (&gi)[CHUNK / 32],
                                        double* __restrict__ aS, double* __restrict__ gT, int NP, int cA, int cB, int N,
@@ -131,6 +133,7 @@ __device__ __forceinline__ void tile32(int lane, const float4* __restrict__ pB, 
 {
     constexpr int P = CHUNK / 32, KP = CHUNK / 64;
     constexpr bool NEAR = MODE != 0, SELF = MODE == 2;
+    static_assert(!UNI || MODE == 0, "mass factored out for far tiles only");
     f2 nx[P], ny[P], nz[P], ng[P], ax[P], ay[P], az[P];
     float mn[P];
     {
@@ -180,12 +183,12 @@ __device__ __forceinline__ void tile32(int lane, const float4* __restrict__ pB, 
                 const f2 y = pk(ya, yb);
                 const f2 t = mul2(y, y);
                 const f2 y3 = mul2(t, y);
-                const f2 si = mul2(gj, y3);                    // G m_j / r^3: force on the stationary body
+                const f2 si = UNI ? y3 : mul2(gj, y3);         // G m_j / r^3: force on the stationary body (UNI: 1 / r^3)
                 ax[p] = fma2(si, dx, ax[p]);
                 ay[p] = fma2(si, dy, ay[p]);
                 az[p] = fma2(si, dz, az[p]);
                 if (!SELF) {
-                    const f2 sj = mul2(ng[p], y3);             // -G m_i / r^3: reaction on the travelling bodies
+                    const f2 sj = UNI ? y3 : mul2(ng[p], y3);  // -G m_i / r^3: reaction on the travelling bodies (UNI: 1 / r^3)
                     bx[q] = fma2(sj, dx, bx[q]);
                     by[q] = fma2(sj, dy, by[q]);
                     bz[q] = fma2(sj, dz, bz[q]);
@@ -224,6 +227,16 @@ __device__ __forceinline__ void tile32(int lane, const float4* __restrict__ pB, 
         }
         double2* d;
         double2 v;
+        if (UNI) {                                       // the common G m of chunk B (as the kernel sees it: the FP32 record's)
+            const double gB = (double)pB[CHUNK / 2].z;
+            d = reinterpret_cast<double2*>(aS + 0 * CHUNK + 2 * u); v = *d;
+            v.x = fma(gB, (double)px[0], v.x); v.y = fma(gB, (double)px[1], v.y); *d = v;
+            d = reinterpret_cast<double2*>(aS + 1 * CHUNK + 2 * u); v = *d;
+            v.x = fma(gB, (double)py[0], v.x); v.y = fma(gB, (double)py[1], v.y); *d = v;
+            d = reinterpret_cast<double2*>(aS + 2 * CHUNK + 2 * u); v = *d;
+            v.x = fma(gB, (double)pz[0], v.x); v.y = fma(gB, (double)pz[1], v.y); *d = v;
+            continue;
+        }
         d = reinterpret_cast<double2*>(aS + 0 * CHUNK + 2 * u); v = *d;
         v.x += keep[0] ? (double)px[0] : 0.0; v.y += keep[1] ? (double)px[1] : 0.0; *d = v;
         d = reinterpret_cast<double2*>(aS + 1 * CHUNK + 2 * u); v = *d;
@@ -249,12 +262,13 @@ __device__ __forceinline__ void tile32(int lane, const float4* __restrict__ pB, 
             float x0, x1, y0, y1, z0, z1;
             upk(bx[q], x0, x1); upk(by[q], y0, y1); upk(bz[q], z0, z1);
             const int slot0 = cB * CHUNK + 2 * u;
+            const double sc = UNI ? -(double)gi[0] : 1.0;      // UNI: the common -G m of chunk A, still to be multiplied in
             if (keep[0] && slot0 < N) {
-                atomicAdd(gT + u, (double)x0); atomicAdd(gT + NP + u, (double)y0); atomicAdd(gT + 2 * NP + u, (double)z0);
+                atomicAdd(gT + u, sc * (double)x0); atomicAdd(gT + NP + u, sc * (double)y0); atomicAdd(gT + 2 * NP + u, sc * (double)z0);
             }
             if (keep[1] && slot0 + 1 < N) {
-                atomicAdd(gT + CHUNK / 2 + u, (double)x1); atomicAdd(gT + NP + CHUNK / 2 + u, (double)y1);
-                atomicAdd(gT + 2 * NP + CHUNK / 2 + u, (double)z1);
+                atomicAdd(gT + CHUNK / 2 + u, sc * (double)x1); atomicAdd(gT + NP + CHUNK / 2 + u, sc * (double)y1);
+                atomicAdd(gT + 2 * NP + CHUNK / 2 + u, sc * (double)z1);
             }
         }
     }
@@ -267,7 +281,7 @@ __device__ __forceinline__ void tile32(int lane, const float4* __restrict__ pB, 
 // rings of 32 steps), which keeps the tile in 128 registers.  Tracking compares the high words of r^2.
 //   pB   set B in shared memory (absolute positions): four planes of CHUNK/2 double2, plane 2h + 0 = (x, y) and
 //        plane 2h + 1 = (z, G m) of the bodies 2u + h
-template <int CHUNK, int MODE>
+template <int CHUNK, int MODE, bool UNI = false>
 __device__ __forceinline__ void tile64(int lane, const double2* __restrict__ pB, const ChunkP& Ac, const ChunkP& Bc,
                                        const double (&xi)[CHUNK / 32], const double (&yi)[CHUNK / 32],
                                        const double (&zi)[CHUNK / 32], const double (&gi)[CHUNK / 32],
@@ -276,6 +290,9 @@ __device__ __forceinline__ void tile64(int lane, const double2* __restrict__ pB,
 {
     constexpr int P = CHUNK / 32, KP = CHUNK / 64;
     constexpr bool NEAR = MODE != 0, SELF = MODE == 2;
+    static_assert(!UNI || MODE == 0, "mass factored out for far tiles only");
+    const double gB = UNI ? pB[CHUNK / 2].y : 1.0;     // UNI: the common G m of chunk B (plane 1, entry 0: body 0's (z, G m)) ...
+    const double gA = UNI ? gi[0] : 1.0;               // ... and of chunk A: 18 instead of 20 FP64 operations per unordered pair
     double ax[P], ay[P], az[P];
     int mn[P];
 #pragma unroll
@@ -317,12 +334,12 @@ __device__ __forceinline__ void tile64(int lane, const double2* __restrict__ pB,
                     const double y3 = y0 * t;
                     const double ye = y3 * e;
                     const double s0 = fma(ye, c, y3);
-                    const double si = J.w * s0;
+                    const double si = UNI ? s0 : J.w * s0;
                     ax[p] = fma(si, dx, ax[p]);
                     ay[p] = fma(si, dy, ay[p]);
                     az[p] = fma(si, dz, az[p]);
                     if (!SELF) {
-                        const double sj = gi[p] * s0;
+                        const double sj = UNI ? s0 : gi[p] * s0;
                         bx[h] = fma(-sj, dx, bx[h]);
                         by[h] = fma(-sj, dy, by[h]);
                         bz[h] = fma(-sj, dz, bz[h]);
@@ -353,11 +370,11 @@ __device__ __forceinline__ void tile64(int lane, const double2* __restrict__ pB,
             }
             const int slot0 = cB * CHUNK + 2 * u;
             if (keep[0] && slot0 < N) {
-                atomicAdd(gT + u, bx[0]); atomicAdd(gT + NP + u, by[0]); atomicAdd(gT + 2 * NP + u, bz[0]);
+                atomicAdd(gT + u, gA * bx[0]); atomicAdd(gT + NP + u, gA * by[0]); atomicAdd(gT + 2 * NP + u, gA * bz[0]);
             }
             if (keep[1] && slot0 + 1 < N) {
-                atomicAdd(gT + CHUNK / 2 + u, bx[1]); atomicAdd(gT + NP + CHUNK / 2 + u, by[1]);
-                atomicAdd(gT + 2 * NP + CHUNK / 2 + u, bz[1]);
+                atomicAdd(gT + CHUNK / 2 + u, gA * bx[1]); atomicAdd(gT + NP + CHUNK / 2 + u, gA * by[1]);
+                atomicAdd(gT + 2 * NP + CHUNK / 2 + u, gA * bz[1]);
             }
         }
     }
@@ -380,11 +397,11 @@ __device__ __forceinline__ void tile64(int lane, const double2* __restrict__ pB,
         double2* d;
         double2 v;
         d = reinterpret_cast<double2*>(aS + 0 * CHUNK + 2 * u); v = *d;
-        v.x += keep[0] ? ax[2 * k] : 0.0; v.y += keep[1] ? ax[2 * k + 1] : 0.0; *d = v;
+        v.x += keep[0] ? gB * ax[2 * k] : 0.0; v.y += keep[1] ? gB * ax[2 * k + 1] : 0.0; *d = v;
         d = reinterpret_cast<double2*>(aS + 1 * CHUNK + 2 * u); v = *d;
-        v.x += keep[0] ? ay[2 * k] : 0.0; v.y += keep[1] ? ay[2 * k + 1] : 0.0; *d = v;
+        v.x += keep[0] ? gB * ay[2 * k] : 0.0; v.y += keep[1] ? gB * ay[2 * k + 1] : 0.0; *d = v;
         d = reinterpret_cast<double2*>(aS + 2 * CHUNK + 2 * u); v = *d;
-        v.x += keep[0] ? az[2 * k] : 0.0; v.y += keep[1] ? az[2 * k + 1] : 0.0; *d = v;
+        v.x += keep[0] ? gB * az[2 * k] : 0.0; v.y += keep[1] ? gB * az[2 * k + 1] : 0.0; *d = v;
     }
 }
 
@@ -482,17 +499,20 @@ __device__ __forceinline__ void kick_sym_body(int N, int NP, int nchunk, Workspa
         const ChunkP& Ac = sm.bcA;
         const ChunkP& Bc = sm.bcB[buf];
         const int mode = (A == B) ? 2 : (tile_is_far(Ac, Bc) ? 0 : 1);
+        const bool uni = Ac.uni != 0.f && Bc.uni != 0.f;              // both chunks uniform in mass: G m factored out of the pair loop
         double* aS = &sm.accS[0][0];
         double* gT = w.aslot + (size_t)B * CHUNK;
         if constexpr (F32) {
             const float4* pB = reinterpret_cast<const float4*>(&sm.pos[buf][0]);
             const double* xS = &sm.xiS[0][0];
-            if (mode == 0)      tile32<CHUNK, 0>(lane, pB, Ac, Bc, xS, gi32, aS, gT, NP, A, B, N, w, cand_cap);
+            if (mode == 0 && uni) tile32<CHUNK, 0, true>(lane, pB, Ac, Bc, xS, gi32, aS, gT, NP, A, B, N, w, cand_cap);
+            else if (mode == 0) tile32<CHUNK, 0>(lane, pB, Ac, Bc, xS, gi32, aS, gT, NP, A, B, N, w, cand_cap);
             else if (mode == 1) tile32<CHUNK, 1>(lane, pB, Ac, Bc, xS, gi32, aS, gT, NP, A, B, N, w, cand_cap);
             else                tile32<CHUNK, 2>(lane, pB, Ac, Bc, xS, gi32, aS, gT, NP, A, B, N, w, cand_cap);
         } else {
             const double2* pB = reinterpret_cast<const double2*>(&sm.pos[buf][0]);
-            if (mode == 0)      tile64<CHUNK, 0>(lane, pB, Ac, Bc, xi, yi, zi, gi64, aS, gT, NP, A, B, N, w, cand_cap);
+            if (mode == 0 && uni) tile64<CHUNK, 0, true>(lane, pB, Ac, Bc, xi, yi, zi, gi64, aS, gT, NP, A, B, N, w, cand_cap);
+            else if (mode == 0) tile64<CHUNK, 0>(lane, pB, Ac, Bc, xi, yi, zi, gi64, aS, gT, NP, A, B, N, w, cand_cap);
             else if (mode == 1) tile64<CHUNK, 1>(lane, pB, Ac, Bc, xi, yi, zi, gi64, aS, gT, NP, A, B, N, w, cand_cap);
             else                tile64<CHUNK, 2>(lane, pB, Ac, Bc, xi, yi, zi, gi64, aS, gT, NP, A, B, N, w, cand_cap);
         }

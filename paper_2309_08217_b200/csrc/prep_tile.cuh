@@ -26,6 +26,8 @@ __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int t
 {
     __shared__ unsigned int smax[PREP_NT / 32][5];
     __shared__ float sbox[PREP_NT / 32][6];                // per warp: min and max of the live positions
+    __shared__ double sgm[PREP_NT / 32];                   // per warp: G m of its first slot, and whether all 32 slots are
+    __shared__ int suni[PREP_NT / 32];                     //           live with bitwise that same G m
     const int s = tile * PREP_NT + threadIdx.x;            // slot; tiles cover NP exactly (NP % 512 == 0)
     const bool live = s < A.N;
     const int i = w.order[s];                              // body held by this slot (= s for padding)
@@ -144,7 +146,9 @@ __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int t
     unsigned int m2 = warp_max_u32(__float_as_uint(rfc));
     unsigned int m3 = warp_max_u32(__float_as_uint(rad));
     unsigned int m4 = warp_max_u32(__float_as_uint(q2));
-    if (lane == 0) { smax[wid][0] = m0; smax[wid][1] = m1; smax[wid][2] = m2; smax[wid][3] = m3; smax[wid][4] = m4; }
+    const double gm0 = __shfl_sync(0xffffffffu, gm, 0);
+    const int uniw = __all_sync(0xffffffffu, live && gm == gm0);
+    if (lane == 0) { smax[wid][0] = m0; smax[wid][1] = m1; smax[wid][2] = m2; smax[wid][3] = m3; smax[wid][4] = m4; sgm[wid] = gm0; suni[wid] = uniw; }
     __syncthreads();
     if (threadIdx.x < PREP_NT / CHUNK) {
         const int c = threadIdx.x;
@@ -159,7 +163,10 @@ __device__ __forceinline__ void prep_tile(const PrepArgs& A, Workspace& w, int t
         // the FP32 separation <= 2^-24 (1 + 2 R_chunk / r))
         q.rf  = fmaxf(__uint_as_float(mx[2]), __fmul_ru(__fmul_ru(2.0f * A.floor_rel, q.rad), 1.000001f));
         q.q2max = A.scaled ? __uint_as_float(mx[4]) : 1.0f;   // scales the bound to the kernel's r'^2 = q^2 r^2
-        q.pad_ = 0.f;
+        bool uni = true;                                    // uniform-mass chunk: the symmetric kernels then factor G m out of the pair loop
+        for (int ww = 0; ww < CHUNK / 32; ++ww)
+            uni = uni && suni[c * (CHUNK / 32) + ww] && sgm[c * (CHUNK / 32) + ww] == sgm[c * (CHUNK / 32)];
+        q.uni = uni ? 1.f : 0.f;
         chunk_origin(c, q.ox, q.oy, q.oz);
         w.bc[tile * (PREP_NT / CHUNK) + c] = q;
     }

@@ -716,6 +716,14 @@ def test_symmetric_kernels_on_the_special_cases():
              (W.config(0, 1200), dict(), dict(cand_capacity=16)), (tiny, dict(), dict()), (W.config(0, 2), dict(), dict()),
              (W.config(0, 65), dict(), dict()), (heavy, dict(), dict()), (ring, dict(weight_mode=1), dict()),
              (W.config(4, 9000), dict(), dict())]
+    # uniform-mass chunks (the far tiles between two of them factor G m out of the pair loop): an equal-mass disc whose inner
+    # half is three times as heavy -- chunks are compact patches, so most are uniform, with one or the other mass, and those
+    # across the boundary are mixed; and the same with every 500th body massless (a test particle breaks its chunk's uniformity)
+    two = W.config(4, 6000)
+    rr = np.linalg.norm(two.x, axis=1)
+    two.m[rr < np.median(rr)] *= 3.0
+    two_tp = W.config(4, 6000); two_tp.m[:] = two.m; two_tp.m[::500] = 0.0
+    cases += [(two, dict(), dict()), (two_tp, dict(), dict()), (two, dict(), dict(chunk=128))]
     for w, okw, gkw in cases:
         p = oparams(w, **okw)
         vd = oracle.to_democratic(w.m, w.v, w.M_star)
