@@ -403,8 +403,10 @@ def run_cuda(args):
                      "flop_per_pair": FLOP_FP32,
                      "convention": "achieved = 18 (25) flop x N (N - 1) ordered pairs / kernel time: the flops of the plain "
                                    "per-ordered-pair sequence (SURVEY.md 8(d)).  The symmetric kernels evaluate each unordered "
-                                   "pair once (16 FP32 / 20 FP64 operations for both directions), so they execute fewer "
-                                   "flops than this convention counts; the time is what is measured",
+                                   "pair once (16 FP32 / 20 FP64 operations for both directions; 14 / 18 in far tiles between "
+                                   "uniform-mass chunks, where G m is factored out of the loop: every far tile of this equal-mass "
+                                   "workload), so they execute fewer flops than this convention counts and 'frac' can exceed 1; "
+                                   "the time is what is measured",
                      "fp64": {"kernel": kname64, "traffic": tr64[0], "traffic_source": tr64[1],
                               "achieved": p64["kick_kernel_tflops"],
                               "peak": PEAK_FP64_TFLOPS, "frac": p64["kick_kernel_frac_of_peak"],
