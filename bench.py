@@ -48,10 +48,10 @@ def capture_traffic(variant_name, precision):
             rec = json.load(f)
         for e in rec["captures"]:
             if e["precision"] == precision and e["variant"] == variant_name:
-                return e["dram_bytes_per_launch"], f"{e['capture']} (git {e['git']}, N = {e['N']})"
+                return e["dram_bytes_per_launch"], f"{e['capture']} (git {e['git']}, N = {e['N']})", e.get("pipe_busy_pct")
     except Exception:
         pass
-    return None, "no ncu capture of this kernel variant is committed (profiles/kick_traffic.json)"
+    return None, "no ncu capture of this kernel variant is committed (profiles/kick_traffic.json)", None
 
 
 def parse_args():
@@ -396,6 +396,7 @@ def run_cuda(args):
         "roofline": {"bound": "alu", "kernel": kname32, "achieved": p32["kick_kernel_tflops"],
                      "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s", "frac": p32["kick_kernel_frac_of_peak"],
                      "traffic": tr32[0], "traffic_source": tr32[1],
+                     "pipe_busy_pct_capture": tr32[2],       # the FMA pipe's busy cycles in that capture (what 'frac' is NOT: see convention)
                      "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md section 7); "
                                     "MEASURED_PEAKS.json has no FP32/FP64 ALU figure.  'frac' (the headline) divides by this "
                                     "derived peak; 'frac_of_measured' by the FFMA2 / DFMA rate the in-library probe reached "
@@ -407,7 +408,7 @@ def run_cuda(args):
                                    "uniform-mass chunks, where G m is factored out of the loop: every far tile of this equal-mass "
                                    "workload), so they execute fewer flops than this convention counts and 'frac' can exceed 1; "
                                    "the time is what is measured",
-                     "fp64": {"kernel": kname64, "traffic": tr64[0], "traffic_source": tr64[1],
+                     "fp64": {"kernel": kname64, "traffic": tr64[0], "traffic_source": tr64[1], "pipe_busy_pct_capture": tr64[2],
                               "achieved": p64["kick_kernel_tflops"],
                               "peak": PEAK_FP64_TFLOPS, "frac": p64["kick_kernel_frac_of_peak"],
                               "flop_per_pair": FLOP_FP64}},
