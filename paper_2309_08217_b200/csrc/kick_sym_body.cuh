@@ -419,11 +419,18 @@ __device__ __forceinline__ void kick_sym_body(int N, int NP, int nchunk, Workspa
     // tiles (A, B >= A), row by row: row A starts at tile A n - A (A - 1) / 2 and has n - A tiles
     const long long n = nchunk;
     const long long NTILE = n * (n + 1) / 2;
-    // Range gw of the tiles goes to warp (gw / gridDim.x) of CTA (gw % gridDim.x): neighbouring ranges sit on different
-    // SMs.  The ranges are not equally dear -- the last ones are the short rows at the corner of the triangle, all
-    // diagonal and near tiles and a row change every few tiles -- and with CTA b holding the ranges 12 b .. 12 b + 11
-    // the last dozen SMs finished 20 % after the others (N = 16 384: 110 against 92 us; now 100).
-    const long long nwarp = (long long)gridDim.x * (blockDim.x >> 5), gw = (long long)wid * gridDim.x + blockIdx.x;
+    // Which range gw of the tiles a warp takes.  (1) Neighbouring ranges go to different SMs: the ranges are not equally
+    // dear -- the last ones are the short rows at the corner of the triangle, all diagonal and near tiles and a row change
+    // every few tiles -- and with CTA b holding the ranges 12 b .. 12 b + 11 the last dozen SMs finished 20 % after the
+    // others (N = 16 384).  (2) The warps that share a sub-partition (wid, wid + 4, ...) take ADJACENT ranges: the issue
+    // slots of a sub-partition are what the ring loops compete for, and adjacent ranges differ by at most one tile in
+    // all (N = 16 384: 13 or 14 tiles per sub-partition; ranges a multiple of 37 apart all had 4, or all 5: 12 or 15).
+    // (2) puts three dear ranges into one sub-partition, though, where (1) alone has one dear warp among the twelve of an
+    // SM: with many tiles per warp, where the counts hardly matter, (1) alone is better (N = 40 000: 0.441 against 0.458 ms).
+    const int nwq = (int)(blockDim.x >> 7);                          // warps per sub-partition
+    const long long nwarp = (long long)gridDim.x * (blockDim.x >> 5);
+    const long long gw = (NTILE < 12 * nwarp) ? ((long long)blockIdx.x + (long long)gridDim.x * (wid & 3)) * nwq + (wid >> 2)
+                                              : (long long)wid * gridDim.x + blockIdx.x;
     long long t = (NTILE * gw) / nwarp;
     const long long t1 = (NTILE * (gw + 1)) / nwarp;
     if (t >= t1) return;
