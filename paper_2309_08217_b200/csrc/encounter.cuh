@@ -19,7 +19,9 @@
 //     midpoint with 2, 4, .. 16 substeps, polynomial extrapolation in h^2, error = largest |dx|/|x|, |dv|/|v| over
 //     the members; a step that does not converge in 8 rows, or whose corrections stop falling (a pair crossing the
 //     edge of its zone, where K is only C^1), is cut to a quarter; a step that converged in few rows is followed by
-//     a longer one.  Status bit 8: the step size collapsed.
+//     a longer one.  Status bit 8: the step size collapsed.  A warp team of up to 4 members runs the rows of the tableau
+//     in parallel (integrate_bs_rows: lane = row x member, 2 r + 1 rounds of force evaluations for r rows instead of their
+//     sum); teams of 3 to 6 members evaluate the ordered pairs of a force evaluation one per lane (accel).
 //   * with params.enc_levels > 1 (reading R16): symplectic sub-levels with reduced steps between level 0 and the
 //     Bulirsch-Stoer integration, which then only sees the innermost remainder of the pair potential.
 //   * classical RK4 with enc_nsub equal substeps (the scheme of the first oracle, oracle_step_hybrid); with
@@ -73,8 +75,12 @@ struct BlockSlab {
 };
 union EncSmem { WarpSlab w[8]; BlockSlab b; };     // warp teams and the CTA team never run at the same time
 
+constexpr int PAIR_NMAX = 6;        // warp teams of up to this many members evaluate their pair terms one per lane (accel)
+
 struct WarpTeam {
+    static constexpr bool PAIR_LANES = true;            // the 32 lanes of the warp all call accel: idle ones can take pairs
     WarpSlab& s; int n, k;                              // k: member index of this lane, -1 for an idle lane
+    int pi, pl;                                         // the ordered pair this lane evaluates in accel (member pl on member pi), -1: none
     __device__ __forceinline__ void sync() const { __syncwarp(); }
     __device__ __forceinline__ double maxall(double v) const
     {
@@ -101,6 +107,7 @@ struct WarpTeam {
     }
 };
 struct BlockTeam {
+    static constexpr bool PAIR_LANES = false;
     BlockSlab& s; int n, k;
     __device__ __forceinline__ void sync() const { __syncthreads(); }
     __device__ __forceinline__ double maxall(double v) const
@@ -223,6 +230,41 @@ __device__ __forceinline__ void accel(const Team& T, const EncParams& P, int& bu
     T.sync();
     buf ^= 1;                                              // the next evaluation writes the other buffer
     a0 = 0.0; a1 = 0.0; a2 = 0.0;
+    if constexpr (Team::PAIR_LANES) {
+        // A warp team of up to PAIR_NMAX members has a lane for every ORDERED pair (n (n - 1) <= 30): lane p takes the term of
+        // member l on member i, i = p / (n - 1), and the member lanes collect theirs by shuffles.  The dependent chain of an
+        // evaluation is then one pair (plus n - 1 shuffles) instead of n - 1 pairs: the drift waits for the slowest group.
+        if (T.n >= 3 && T.n <= PAIR_NMAX) {                 // (a pair of bodies has nothing to gain)
+            const int n1 = T.n - 1;
+            const bool valid = T.pi >= 0;
+            const int i = valid ? T.pi : 0, l = valid ? T.pl : 0;
+            const double i09 = valid ? T.s.i09[l][i] : 0.0;
+            const double d0 = X[l] - X[i], d1 = Y[l] - Y[i], d2 = Z[l] - Z[i];
+            const double q2 = fma(d2, d2, fma(d1, d1, d0 * d0));
+            const bool   on = (i09 > 0.0) && (q2 > 0.0);
+            const double qs = on ? q2 : 1.0;
+            const double y0 = rsq_seed(qs), t = y0 * y0, e = fma(-qs, t, 1.0), g = y0 * t;
+            const double q0 = qs * y0;
+            const double q  = fma(q0 * e, fma(0.375, e, 0.5), q0);              // |d|
+            const double whi = (fhi > 0.0) ? zone_weight(q, i09 * fhi) : 1.0;
+            const double Wc = on ? whi - zone_weight(q, i09 * flo) : 0.0;
+            const double sc = T.gm(l) * Wc * fma(g * e, fma(1.875, e, 1.5), g);  // G m_l Wc / |d|^3
+            const double c0 = sc * d0, c1 = sc * d1, c2 = sc * d2;
+            if (KEPLER && T.k >= 0) {
+                const double mu = P.G * P.M_star;
+                const double r2 = fma(z, z, fma(y, y, x * x));
+                const double u0 = rsq_seed(r2), tt = u0 * u0, ee = fma(-r2, tt, 1.0), gg = u0 * tt;
+                const double ir3 = -mu * fma(gg * ee, fma(1.875, ee, 1.5), gg);  // -mu / r^3
+                a0 = x * ir3; a1 = y * ir3; a2 = z * ir3;
+            }
+            const int base = (T.k >= 0) ? T.k * n1 : 0;
+            for (int j = 0; j < n1; ++j) {
+                const double v0 = __shfl_sync(FULL, c0, base + j), v1 = __shfl_sync(FULL, c1, base + j), v2 = __shfl_sync(FULL, c2, base + j);
+                if (T.k >= 0) { a0 += v0; a1 += v1; a2 += v2; }
+            }
+            return;
+        }
+    }
     if (T.k < 0) return;
     if (KEPLER) {
         const double mu = P.G * P.M_star;
@@ -280,6 +322,159 @@ __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P,
     if (T.k == 0) { atomicAdd(&ctr->enc_rhs_sum, 4u * (unsigned int)P.nsub); atomicMax(&ctr->enc_rhs_max, 4u * (unsigned int)P.nsub); }
 }
 
+// Gragg-Bulirsch-Stoer for a warp team of up to ROWS_NMAX members with the rows of the extrapolation tableau IN PARALLEL:
+// the rows (2, 4, .. 16 modified-midpoint substeps over the same macro step H) do not depend on one another, and a warp that
+// integrates a pair of bodies has 30 idle lanes.  Lane r n + k carries member k through row r (n_r = 2 (r + 1) substeps);
+// the members of a row see each other's stage positions by shuffles (no shared-memory slab, no barrier).  A macro step
+// costs 17 rounds of force evaluations whatever row converges, against 3 + 5 + .. (2 k + 3) = 24, 35, 48 rounds when the
+// rows run one after the other and row k = 3, 4, 5 converges, and 80 for a rejected step.  Same arithmetic per row, same
+// tableau, same acceptance and step-size rules as integrate_bs: the results are bitwise those of the sequential form.
+// Every lane keeps the state of ITS member (y, replicated over the rows).  Must be called by the whole warp, converged.
+constexpr int ROWS_NMAX = 32 / KMAX;
+
+__device__ __forceinline__ void rows_accel(const WarpTeam& T, const EncParams& P, int rbase, int mem, double x, double y, double z,
+                                           double& a0, double& a1, double& a2, double flo)
+{
+    const double mu = P.G * P.M_star;
+    const double r2 = fma(z, z, fma(y, y, x * x));
+    const double u0 = rsq_seed(r2), tt = u0 * u0, ee = fma(-r2, tt, 1.0), gg = u0 * tt;
+    const double ir3 = -mu * fma(gg * ee, fma(1.875, ee, 1.5), gg);             // -mu / r^3
+    a0 = x * ir3; a1 = y * ir3; a2 = z * ir3;
+    for (int j = 1; j < T.n; ++j) {                                             // the other members, in the order of accel()
+        const int l = (mem + j < T.n) ? mem + j : mem + j - T.n;
+        const double xl = __shfl_sync(FULL, x, rbase + l), yl = __shfl_sync(FULL, y, rbase + l), zl = __shfl_sync(FULL, z, rbase + l);
+        const double i09 = T.s.i09[l][mem];
+        const double d0 = xl - x, d1 = yl - y, d2 = zl - z;
+        const double q2 = fma(d2, d2, fma(d1, d1, d0 * d0));
+        const bool   on = (i09 > 0.0) && (q2 > 0.0);
+        const double qs = on ? q2 : 1.0;
+        const double y0 = rsq_seed(qs), t = y0 * y0, e = fma(-qs, t, 1.0), g = y0 * t;
+        const double q0 = qs * y0;
+        const double q  = fma(q0 * e, fma(0.375, e, 0.5), q0);                  // |d|
+        const double Wc = on ? 1.0 - zone_weight(q, i09 * flo) : 0.0;
+        const double sc = T.gm(l) * Wc * fma(g * e, fma(1.875, e, 1.5), g);      // G m_l Wc / |d|^3
+        a0 = fma(sc, d0, a0); a1 = fma(sc, d1, a1); a2 = fma(sc, d2, a2);
+    }
+}
+
+__device__ __forceinline__ void integrate_bs_rows(const WarpTeam& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
+                                                  double flo)
+{
+    const int lane = threadIdx.x & 31, n = T.n;
+    const bool act = lane < KMAX * n;
+    const int row = act ? lane / n : 0, mem = act ? lane - row * n : 0, rbase = row * n;
+    const int nk = 2 * (row + 1);
+    // every lane takes over the state of its member
+#pragma unroll
+    for (int c = 0; c < 6; ++c) y[c] = __shfl_sync(FULL, y[c], mem);
+    const double Tabs = fabs(dt);
+    double t = 0.0, H = dt;
+    bool collapsed = false;
+    unsigned int nrhs = 0u, nrej = 0u;
+    // Rows actually run: two beyond the row that converged last time (17 rounds for all eight would be more than the
+    // sequential form needs when row 2 or 3 converges); if they do not settle the step, it is redone with all eight.  The
+    // decisions are taken row by row in the same order either way, so the result does not depend on this guess.
+    int rows_use = KMAX;
+    while (fabs(t) < Tabs * (1.0 - 1.0e-14)) {
+        if (fabs(t + H) > Tabs) H = dt - t;
+        double f0[3];
+        rows_accel(T, P, rbase, mem, y[0], y[1], y[2], f0[0], f0[1], f0[2], flo);
+        ++nrhs;
+        const double h = H / nk, h2 = 2.0 * h;
+        double z0[6], z1[6], f[3], est[6];
+        double d[KMAX][6], hsq[KMAX], yz[6], dy[6];
+        int done = -1;
+        for (int ru = rows_use;;) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { z0[c] = y[c]; z0[3 + c] = y[3 + c]; z1[c] = fma(h, y[3 + c], y[c]); z1[3 + c] = fma(h, f0[c], y[3 + c]); }
+#pragma unroll
+        for (int c = 0; c < 6; ++c) est[c] = 0.0;
+        for (int s = 1; s <= 2 * ru; ++s) {                                      // round s: the rows with n_r >= s are still under way
+            rows_accel(T, P, rbase, mem, z1[0], z1[1], z1[2], f[0], f[1], f[2], flo);
+            if (s < nk) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const double nx = fma(h2, z1[3 + c], z0[c]), nv = fma(h2, f[c], z0[3 + c]);
+                    z0[c] = z1[c]; z0[3 + c] = z1[3 + c]; z1[c] = nx; z1[3 + c] = nv;
+                }
+            } else if (s == nk) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    est[c] = 0.5 * (z1[c] + z0[c] + h * z1[3 + c]);
+                    est[3 + c] = 0.5 * (z1[3 + c] + z0[3 + c] + h * f[c]);
+                }
+            }
+        }
+        nrhs += 2u * (unsigned int)ru;
+        // the tableau, row by row as in integrate_bs, every lane for its own member: row k's estimate comes from lane k n + mem
+        double eprev = 1.0e300;
+        bool stalled = false;
+        done = -1;
+        for (int k = 0; k < ru && done < 0 && !stalled; ++k) {
+            double ek[6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) ek[c] = __shfl_sync(FULL, est[c], k * n + mem);
+            const double hk = H / (2 * (k + 1));
+            hsq[k] = hk * hk;
+#pragma unroll
+            for (int c = 0; c < 6; ++c) { yz[c] = ek[c]; dy[c] = ek[c]; }
+            if (k == 0) {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) d[0][c] = ek[c];
+            } else {
+                double cc[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) cc[c] = ek[c];
+                for (int j = 0; j < k; ++j) {
+                    const double delta = 1.0 / (hsq[k - j - 1] - hsq[k]);
+                    const double f1 = hsq[k] * delta, f2 = hsq[k - j - 1] * delta;
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) {
+                        const double q = d[j][c];
+                        d[j][c] = dy[c];
+                        const double dl = cc[c] - q;
+                        dy[c] = f1 * dl; cc[c] = f2 * dl;
+                        yz[c] += dy[c];
+                    }
+                }
+#pragma unroll
+                for (int c = 0; c < 6; ++c) d[k][c] = dy[c];
+                double e = 0.0;
+                if (act) {
+                    const double ex = (dy[0] * dy[0] + dy[1] * dy[1] + dy[2] * dy[2]) / (yz[0] * yz[0] + yz[1] * yz[1] + yz[2] * yz[2]);
+                    const double ev = (dy[3] * dy[3] + dy[4] * dy[4] + dy[5] * dy[5]) / (yz[3] * yz[3] + yz[4] * yz[4] + yz[5] * yz[5]);
+                    e = fmax(ex, ev);
+                    if (!(e == e)) e = 1.0e300;           // NaN: not converged
+                }
+                e = T.maxall(e);
+                if (e <= P.tol * P.tol) done = k;
+                else if (k >= 3 && e > 0.04 * eprev) stalled = true;
+                eprev = e;
+            }
+        }
+        if (done >= 0 || stalled || ru == KMAX) break;
+        ru = KMAX;                                                               // not settled by the rows run: all eight
+        }
+        if (done < 0) {
+            ++nrej;
+            H *= 0.25;
+            rows_use = 6;
+            if (fabs(H) < Tabs * 9.3e-10) { collapsed = true; break; }
+            continue;
+        }
+        rows_use = min(KMAX, max(3, done + 2));
+#pragma unroll
+        for (int c = 0; c < 6; ++c) y[c] = yz[c];
+        t += H;
+        H = (done <= 2) ? 4.0 * H : ((done <= 4) ? 2.0 * H : ((done <= 5) ? H : 0.5 * H));
+    }
+    if (lane == 0) {
+        if (collapsed) atomicOr(&ctr->enc_status, 8u);
+        atomicAdd(&ctr->enc_rhs_sum, nrhs); atomicMax(&ctr->enc_rhs_max, nrhs); atomicAdd(&ctr->enc_rejected, nrej);
+    }
+}
+
+
 // A(dt) by Gragg-Bulirsch-Stoer extrapolation to the relative tolerance P.tol (reading R15).  The tableau is kept in
 // the difference form of polynomial extrapolation (one column of differences per row), which yields the extrapolated
 // value and the last correction, i.e. the error estimate T_kk - T_k,k-1, without storing two rows.
@@ -287,6 +482,9 @@ template <class Team>
 __device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
                                              double flo = 1.0)
 {
+    if constexpr (Team::PAIR_LANES) {
+        if (T.n <= ROWS_NMAX) { integrate_bs_rows(T, P, dt, y, ctr, flo); return; }   // the rows of the tableau in parallel
+    }
     const double Tabs = fabs(dt);
     double t = 0.0, H = dt;
     int buf = 0;
@@ -462,7 +660,9 @@ __device__ __forceinline__ void warp_group(const EncParams& P, Workspace& w, War
         slab.m[lane] = m; slab.gm[lane] = P.G * m; slab.rc[lane] = rci; slab.sa[lane] = sa; slab.vk[lane] = vk; slab.body[lane] = b;
         if (P.collide) R = w.radius[b];
     }
-    const WarpTeam T{slab, n, active ? lane : -1};
+    int pi = -1, pl = -1;
+    if (n >= 3 && n <= PAIR_NMAX && lane < n * (n - 1)) { pi = lane / (n - 1); const int jj = lane - pi * (n - 1); pl = jj + (jj >= pi ? 1 : 0); }
+    const WarpTeam T{slab, n, active ? lane : -1, pi, pl};
     T.refresh_pairs(P);
     integrate<FULL_FEATURES>(T, P, dt, y, w.ctr, m, R, b, w.absorb);
     if (active) {
