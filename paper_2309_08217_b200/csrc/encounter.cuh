@@ -328,7 +328,8 @@ __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P,
 // the members of a row see each other's stage positions by shuffles (no shared-memory slab, no barrier).  A macro step
 // costs 17 rounds of force evaluations whatever row converges, against 3 + 5 + .. (2 k + 3) = 24, 35, 48 rounds when the
 // rows run one after the other and row k = 3, 4, 5 converges, and 80 for a rejected step.  Same arithmetic per row, same
-// tableau, same acceptance and step-size rules as integrate_bs: the results are bitwise those of the sequential form.
+// acceptance and step-size rules as integrate_bs; the tableau is spread over the lanes as well (no arrays in local memory, no
+// divisions per macro step), which changes its rounding, not its values.
 // Every lane keeps the state of ITS member (y, replicated over the rows).  Must be called by the whole warp, converged.
 constexpr int ROWS_NMAX = 32 / KMAX;
 
@@ -367,6 +368,15 @@ __device__ __forceinline__ void integrate_bs_rows(const WarpTeam& T, const EncPa
     // every lane takes over the state of its member
 #pragma unroll
     for (int c = 0; c < 6; ++c) y[c] = __shfl_sync(FULL, y[c], mem);
+    // Aitken-Neville in h^2 with the tableau spread over the lanes: lane (r, k) holds T[r][j] of its member, column after
+    // column, and takes T[r-1][j-1] from the lane n below: T[r][j] = T[r][j-1] + (T[r][j-1] - T[r-1][j-1]) / ((n_r / n_(r-j))^2 - 1).
+    // (The sequential form keeps the same tableau as differences in an array; the two agree to rounding.)
+    double cj[KMAX];
+#pragma unroll
+    for (int j = 1; j < KMAX; ++j) {
+        const double q = (j <= row) ? (double)(row + 1) / (double)(row + 1 - j) : 2.0;
+        cj[j] = 1.0 / (q * q - 1.0);
+    }
     const double Tabs = fabs(dt);
     double t = 0.0, H = dt;
     bool collapsed = false;
@@ -382,7 +392,6 @@ __device__ __forceinline__ void integrate_bs_rows(const WarpTeam& T, const EncPa
         ++nrhs;
         const double h = H / nk, h2 = 2.0 * h;
         double z0[6], z1[6], f[3], est[6];
-        double d[KMAX][6], hsq[KMAX], yz[6], dy[6];
         int done = -1;
         for (int ru = rows_use;;) {
 #pragma unroll
@@ -406,51 +415,46 @@ __device__ __forceinline__ void integrate_bs_rows(const WarpTeam& T, const EncPa
             }
         }
         nrhs += 2u * (unsigned int)ru;
-        // the tableau, row by row as in integrate_bs, every lane for its own member: row k's estimate comes from lane k n + mem
+        // the tableau (see above): after column j the lanes of row r >= j hold T[r][j]; last = T[r][r] - T[r][r-1]
+        double last[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+        for (int j = 1; j < KMAX; ++j) {
+            if (j < ru) {
+                double prev[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) prev[c] = __shfl_sync(FULL, est[c], (lane >= n) ? lane - n : lane);
+                if (act && row >= j && row < ru) {
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) {
+                        const double corr = (est[c] - prev[c]) * cj[j];
+                        est[c] += corr;
+                        if (j == row) last[c] = corr;
+                    }
+                }
+            }
+        }
+        // error of row r: its last correction against its value, the largest over the members of the row
+        double e = 0.0;
+        if (act && row >= 1 && row < ru) {
+            const double ex = (last[0] * last[0] + last[1] * last[1] + last[2] * last[2]) / (est[0] * est[0] + est[1] * est[1] + est[2] * est[2]);
+            const double ev = (last[3] * last[3] + last[4] * last[4] + last[5] * last[5]) / (est[3] * est[3] + est[4] * est[4] + est[5] * est[5]);
+            e = fmax(ex, ev);
+            if (!(e == e)) e = 1.0e300;                   // NaN: not converged
+        }
+        {
+            double em = e;
+            for (int l = 0; l < n; ++l) em = fmax(em, __shfl_sync(FULL, e, rbase + l));
+            e = em;
+        }
+        // the decisions, row by row in the order of the sequential form
         double eprev = 1.0e300;
         bool stalled = false;
         done = -1;
-        for (int k = 0; k < ru && done < 0 && !stalled; ++k) {
-            double ek[6];
-#pragma unroll
-            for (int c = 0; c < 6; ++c) ek[c] = __shfl_sync(FULL, est[c], k * n + mem);
-            const double hk = H / (2 * (k + 1));
-            hsq[k] = hk * hk;
-#pragma unroll
-            for (int c = 0; c < 6; ++c) { yz[c] = ek[c]; dy[c] = ek[c]; }
-            if (k == 0) {
-#pragma unroll
-                for (int c = 0; c < 6; ++c) d[0][c] = ek[c];
-            } else {
-                double cc[6];
-#pragma unroll
-                for (int c = 0; c < 6; ++c) cc[c] = ek[c];
-                for (int j = 0; j < k; ++j) {
-                    const double delta = 1.0 / (hsq[k - j - 1] - hsq[k]);
-                    const double f1 = hsq[k] * delta, f2 = hsq[k - j - 1] * delta;
-#pragma unroll
-                    for (int c = 0; c < 6; ++c) {
-                        const double q = d[j][c];
-                        d[j][c] = dy[c];
-                        const double dl = cc[c] - q;
-                        dy[c] = f1 * dl; cc[c] = f2 * dl;
-                        yz[c] += dy[c];
-                    }
-                }
-#pragma unroll
-                for (int c = 0; c < 6; ++c) d[k][c] = dy[c];
-                double e = 0.0;
-                if (act) {
-                    const double ex = (dy[0] * dy[0] + dy[1] * dy[1] + dy[2] * dy[2]) / (yz[0] * yz[0] + yz[1] * yz[1] + yz[2] * yz[2]);
-                    const double ev = (dy[3] * dy[3] + dy[4] * dy[4] + dy[5] * dy[5]) / (yz[3] * yz[3] + yz[4] * yz[4] + yz[5] * yz[5]);
-                    e = fmax(ex, ev);
-                    if (!(e == e)) e = 1.0e300;           // NaN: not converged
-                }
-                e = T.maxall(e);
-                if (e <= P.tol * P.tol) done = k;
-                else if (k >= 3 && e > 0.04 * eprev) stalled = true;
-                eprev = e;
-            }
+        for (int k = 1; k < ru; ++k) {
+            const double ek = __shfl_sync(FULL, e, k * n);
+            if (ek <= P.tol * P.tol) { done = k; break; }
+            if (k >= 3 && ek > 0.04 * eprev) { stalled = true; break; }   // the corrections stopped falling: a zone edge inside the step
+            eprev = ek;
         }
         if (done >= 0 || stalled || ru == KMAX) break;
         ru = KMAX;                                                               // not settled by the rows run: all eight
@@ -464,7 +468,7 @@ __device__ __forceinline__ void integrate_bs_rows(const WarpTeam& T, const EncPa
         }
         rows_use = min(KMAX, max(3, done + 2));
 #pragma unroll
-        for (int c = 0; c < 6; ++c) y[c] = yz[c];
+        for (int c = 0; c < 6; ++c) y[c] = __shfl_sync(FULL, est[c], done * n + mem);
         t += H;
         H = (done <= 2) ? 4.0 * H : ((done <= 4) ? 2.0 * H : ((done <= 5) ? H : 0.5 * H));
     }

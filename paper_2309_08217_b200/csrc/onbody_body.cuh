@@ -127,15 +127,28 @@ __device__ __forceinline__ void onbody_body(const OnBodyArgs& A, Workspace& w, c
             // advances its members through the same S(dt/2) and the flow of H_A,group over dt; then their m v' joins the sum, each body's in the
             // thread that owns the body (so the sum does not depend on which warp moved which group)
             __shared__ enc::EncSmem esm;
+            __shared__ int s_big[64], s_nbig;
             const int ngroups = (int)__ldcg(&w.ctr->enc_groups);
-            // groups of more than enc::WMAX bodies first, each by a whole CTA (the j-th such group by CTA j mod grid)
-            int nbig = 0;
-            for (int g = 0; g < ngroups; ++g) {
-                int n;
-                const int* mem = enc::group_members(w, A.enc.maxgroups, g, n);
-                if (n > enc::WMAX) {
-                    if (nbig % (int)gridDim.x == (int)blockIdx.x) enc::block_group<(ENC > 1)>(A.enc, w, esm.b, mem, n, A.dt, s0, s1, s2);
-                    ++nbig;
+            // groups of more than enc::WMAX bodies first, each by a whole CTA (group g by CTA g mod grid).  Only if there is
+            // one (group_kernel leaves the largest size): walking the group table costs a dependent global load per group
+            // and CTA (430 groups: 0.25 ms, which used to be most of the hybrid step's drift).  The CTA's threads look at
+            // its groups together and queue the large ones (in runs of 64).
+            if ((int)__ldcg(&w.ctr->enc_maxsize) > enc::WMAX) {
+                for (int g0 = (int)blockIdx.x; g0 < ngroups; g0 += 64 * (int)gridDim.x) {
+                    if (threadIdx.x == 0) s_nbig = 0;
+                    __syncthreads();
+                    if (threadIdx.x < 64) {
+                        const int g = g0 + (int)threadIdx.x * (int)gridDim.x;
+                        if (g < ngroups && __ldcg(&w.ginfo[2 * g + 1]) > enc::WMAX) s_big[atomicAdd(&s_nbig, 1)] = g;
+                    }
+                    __syncthreads();
+                    const int nb = s_nbig;
+                    for (int q = 0; q < nb; ++q) {
+                        int n;
+                        const int* mem = enc::group_members(w, A.enc.maxgroups, s_big[q], n);
+                        enc::block_group<(ENC > 1)>(A.enc, w, esm.b, mem, n, A.dt, s0, s1, s2);
+                        __syncthreads();
+                    }
                 }
             }
             __syncthreads();
