@@ -326,8 +326,9 @@ __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P,
 // the rows (2, 4, .. 16 modified-midpoint substeps over the same macro step H) do not depend on one another, and a warp that
 // integrates a pair of bodies has 30 idle lanes.  Lane r n + k carries member k through row r (n_r = 2 (r + 1) substeps);
 // the members of a row see each other's stage positions by shuffles (no shared-memory slab, no barrier).  A macro step
-// costs 17 rounds of force evaluations whatever row converges, against 3 + 5 + .. (2 k + 3) = 24, 35, 48 rounds when the
-// rows run one after the other and row k = 3, 4, 5 converges, and 80 for a rejected step.  Same arithmetic per row, same
+// with r rows costs 2 r + 1 rounds of force evaluations (17 for all eight), against 3 + 5 + .. (2 k + 3) = 24, 35, 48 rounds
+// when the rows run one after the other and row k = 3, 4, 5 converges, and 80 for a rejected step.  Measured: ~1100 cycles per
+// round for a team of three, of which ~300 are the macro step's own (first evaluation, tableau, decisions).  Same arithmetic per row, same
 // acceptance and step-size rules as integrate_bs; the tableau is spread over the lanes as well (no arrays in local memory, no
 // divisions per macro step), which changes its rounding, not its values.
 // Every lane keeps the state of ITS member (y, replicated over the rows).  Must be called by the whole warp, converged.
