@@ -334,18 +334,36 @@ __device__ __forceinline__ void integrate_rk4(const Team& T, const EncParams& P,
 // Every lane keeps the state of ITS member (y, replicated over the rows).  Must be called by the whole warp, converged.
 constexpr int ROWS_NMAX = 32 / KMAX;
 
-__device__ __forceinline__ void rows_accel(const WarpTeam& T, const EncParams& P, int rbase, int mem, double x, double y, double z,
-                                           double& a0, double& a1, double& a2, double flo)
+// Complement weight 1 - W(q; zone of inverse width i09) = 1 - K + q K' with one reciprocal: K = u^2 / D, K' = 2 u (1 - u) i09 / D^2,
+// u = clamp((q - 0.1 rc) / (0.9 rc)), D = 2 u^2 - 2 u + 1  =>  1 - W = (D^2 - u^2 D + 2 q i09 u (1 - u)) / D^2.  (zone_weight() forms
+// K and K' one after the other; the two agree to rounding.  Shorter dependent chain: this is what a round waits for.)
+__device__ __forceinline__ double zone_complement(double q, double i09)
 {
-    const double mu = P.G * P.M_star;
+    const double u  = fmin(fmax(fma(q, i09, -1.0 / 9.0), 0.0), 1.0);
+    const double D  = fma(2.0 * u, u - 1.0, 1.0), D2 = D * D;
+    const double r0 = rcp_seed(D2), f = fma(-D2, r0, 1.0);
+    const double iD2 = fma(r0 * f, 1.0 + f, r0);
+    const double num = fma(2.0 * q * i09, u * (1.0 - u), fma(-u * u, D, D2));
+    return num * iD2;
+}
+
+// Force evaluation of the row-parallel integrator for a team of N members, fully unrolled: the N - 1 pair terms of a
+// lane are independent chains that overlap.  gmo / i09o: G m and 1 / (0.9 r_crit / flo) of the other members, in the
+// order l = mem + 1, mem + 2, .. (cyclic), held in registers for the whole integration.
+template <int N>
+__device__ __forceinline__ void rows_accel(double mu, int rbase, int mem, const double (&gmo)[N > 1 ? N - 1 : 1],
+                                           const double (&i09o)[N > 1 ? N - 1 : 1], double x, double y, double z,
+                                           double& a0, double& a1, double& a2)
+{
     const double r2 = fma(z, z, fma(y, y, x * x));
     const double u0 = rsq_seed(r2), tt = u0 * u0, ee = fma(-r2, tt, 1.0), gg = u0 * tt;
     const double ir3 = -mu * fma(gg * ee, fma(1.875, ee, 1.5), gg);             // -mu / r^3
     a0 = x * ir3; a1 = y * ir3; a2 = z * ir3;
-    for (int j = 1; j < T.n; ++j) {                                             // the other members, in the order of accel()
-        const int l = (mem + j < T.n) ? mem + j : mem + j - T.n;
+#pragma unroll
+    for (int j = 1; j < N; ++j) {                                               // the other members, in the order of accel()
+        const int l = (mem + j < N) ? mem + j : mem + j - N;
         const double xl = __shfl_sync(FULL, x, rbase + l), yl = __shfl_sync(FULL, y, rbase + l), zl = __shfl_sync(FULL, z, rbase + l);
-        const double i09 = T.s.i09[l][mem];
+        const double i09 = i09o[j - 1];
         const double d0 = xl - x, d1 = yl - y, d2 = zl - z;
         const double q2 = fma(d2, d2, fma(d1, d1, d0 * d0));
         const bool   on = (i09 > 0.0) && (q2 > 0.0);
@@ -353,22 +371,31 @@ __device__ __forceinline__ void rows_accel(const WarpTeam& T, const EncParams& P
         const double y0 = rsq_seed(qs), t = y0 * y0, e = fma(-qs, t, 1.0), g = y0 * t;
         const double q0 = qs * y0;
         const double q  = fma(q0 * e, fma(0.375, e, 0.5), q0);                  // |d|
-        const double Wc = on ? 1.0 - zone_weight(q, i09 * flo) : 0.0;
-        const double sc = T.gm(l) * Wc * fma(g * e, fma(1.875, e, 1.5), g);      // G m_l Wc / |d|^3
+        const double Wc = on ? zone_complement(q, i09) : 0.0;
+        const double sc = gmo[j - 1] * Wc * fma(g * e, fma(1.875, e, 1.5), g);   // G m_l Wc / |d|^3
         a0 = fma(sc, d0, a0); a1 = fma(sc, d1, a1); a2 = fma(sc, d2, a2);
     }
 }
 
+template <int N>
 __device__ __forceinline__ void integrate_bs_rows(const WarpTeam& T, const EncParams& P, double dt, double (&y)[6], Counters* ctr,
                                                   double flo)
 {
-    const int lane = threadIdx.x & 31, n = T.n;
+    constexpr int n = N;
+    const int lane = threadIdx.x & 31;
     const bool act = lane < KMAX * n;
     const int row = act ? lane / n : 0, mem = act ? lane - row * n : 0, rbase = row * n;
     const int nk = 2 * (row + 1);
     // every lane takes over the state of its member
 #pragma unroll
     for (int c = 0; c < 6; ++c) y[c] = __shfl_sync(FULL, y[c], mem);
+    const double mu = P.G * P.M_star;
+    double gmo[N - 1], i09o[N - 1];
+#pragma unroll
+    for (int j = 1; j < N; ++j) {
+        const int l = (mem + j < N) ? mem + j : mem + j - N;
+        gmo[j - 1] = T.gm(l); i09o[j - 1] = T.s.i09[l][mem] * flo;
+    }
     // Aitken-Neville in h^2 with the tableau spread over the lanes: lane (r, k) holds T[r][j] of its member, column after
     // column, and takes T[r-1][j-1] from the lane n below: T[r][j] = T[r][j-1] + (T[r][j-1] - T[r-1][j-1]) / ((n_r / n_(r-j))^2 - 1).
     // (The sequential form keeps the same tableau as differences in an array; the two agree to rounding.)
@@ -389,7 +416,7 @@ __device__ __forceinline__ void integrate_bs_rows(const WarpTeam& T, const EncPa
     while (fabs(t) < Tabs * (1.0 - 1.0e-14)) {
         if (fabs(t + H) > Tabs) H = dt - t;
         double f0[3];
-        rows_accel(T, P, rbase, mem, y[0], y[1], y[2], f0[0], f0[1], f0[2], flo);
+        rows_accel<N>(mu, rbase, mem, gmo, i09o, y[0], y[1], y[2], f0[0], f0[1], f0[2]);
         ++nrhs;
         const double h = H / nk, h2 = 2.0 * h;
         double z0[6], z1[6], f[3], est[6];
@@ -400,7 +427,7 @@ __device__ __forceinline__ void integrate_bs_rows(const WarpTeam& T, const EncPa
 #pragma unroll
         for (int c = 0; c < 6; ++c) est[c] = 0.0;
         for (int s = 1; s <= 2 * ru; ++s) {                                      // round s: the rows with n_r >= s are still under way
-            rows_accel(T, P, rbase, mem, z1[0], z1[1], z1[2], f[0], f[1], f[2], flo);
+            rows_accel<N>(mu, rbase, mem, gmo, i09o, z1[0], z1[1], z1[2], f[0], f[1], f[2]);
             if (s < nk) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -488,7 +515,11 @@ __device__ __forceinline__ void integrate_bs(const Team& T, const EncParams& P, 
                                              double flo = 1.0)
 {
     if constexpr (Team::PAIR_LANES) {
-        if (T.n <= ROWS_NMAX) { integrate_bs_rows(T, P, dt, y, ctr, flo); return; }   // the rows of the tableau in parallel
+        // the rows of the tableau in parallel
+        if (T.n == 2) { integrate_bs_rows<2>(T, P, dt, y, ctr, flo); return; }
+        if (T.n == 3) { integrate_bs_rows<3>(T, P, dt, y, ctr, flo); return; }
+        if (T.n == 4) { integrate_bs_rows<4>(T, P, dt, y, ctr, flo); return; }
+        static_assert(ROWS_NMAX == 4, "one instance per team size");
     }
     const double Tabs = fabs(dt);
     double t = 0.0, H = dt;
