@@ -120,6 +120,9 @@ cudaError_t launch_onbody(const Handle* h, const OnBodyArgs& a, int max_blocks)
 {
     if (h->N == 0) return cudaSuccess;
     int blocks = h->NP / PREP_NT;
+    // with encounter groups: every co-resident CTA, whatever N -- a group takes a warp for as long as its integration lasts,
+    // and a grid sized for the per-body phases (N = 10 000: 40 CTAs) made 1 100 groups queue three and four deep per warp
+    if (a.enc.on && a.do_drift) blocks = max_blocks;
     if (blocks > max_blocks) blocks = max_blocks;
     OnBodyArgs args = a;
     Workspace ws = h->w;
