@@ -465,13 +465,15 @@ lean_kernel(const __grid_constant__ LeanArgs L, const __grid_constant__ Workspac
     // per-thread part of the near bounds of an evaluation (see below): bound_orbit of every slot this thread loads
     const float n2dtf = __double2float_ru(lam * A.n2 * A.dt_rcrit);
     const float ln1f = __double2float_ru(lam * A.n1);
-    float asum = 0.f, acnt = 0.f, vkmax = 0.f;
+    float asum = 0.f, acnt = 0.f, vkmax = 0.f, amax_t = 0.f;
+    float cap = -1.f;                                         // mutual-Hill rule: 4 x the mean semi-major axis, fixed at the first evaluation of the call
     auto note_orbit = [&](int s, double px, double py, double pz, double v2) {
         float aq, vk2;
         bound_orbit((float)px, (float)py, (float)pz, __double2float_ru(v2), muf, imuf, aq, vk2);
         if (hill) {
             S.C[s] = aq;                                          // turned into c_s once Amax is known
-            if (aq < 1.0e30f) { asum += aq; acnt += 1.f; }
+            if (cap < 0.f) { if (aq < 1.0e30f) { asum += aq; acnt += 1.f; } }
+            else if (aq <= cap) amax_t = fmaxf(amax_t, aq);
             vkmax = fmaxf(vkmax, vk2);
         } else {
             // max rule: c = (lambda r_crit)^2 from the upper bounds (HQ: cbrt(m / 3 M) rounded up)
@@ -547,7 +549,7 @@ lean_kernel(const __grid_constant__ LeanArgs L, const __grid_constant__ Workspac
             if (last && cta == 0 && t < 4) w.mom[MOM_SLOT_B + t] = sP[t];
             // closing S(dt/2): everybody's position, shifted as its owner shifts it
             const double s0 = sc * sP[0], s1 = sc * sP[1], s2 = sc * sP[2];
-            asum = acnt = vkmax = 0.f;
+            asum = acnt = vkmax = amax_t = 0.f;
             for (int s = t; s < N; s += LEAN_NT) {
                 const double2* g2 = reinterpret_cast<const double2*>(&xgb[e & 1][s]);
                 const double2 qa = __ldcg(g2), qb = __ldcg(g2 + 1);
@@ -568,22 +570,28 @@ lean_kernel(const __grid_constant__ LeanArgs L, const __grid_constant__ Workspac
             w.rcrit[bo] = fmax(A.n1 * (sa * w.hcbrt[bo]), A.n2 * A.dt_rcrit * vk); w.semi[bo] = sa; w.vkep[bo] = vk;
         }
         // near bounds of everybody (bound_orbit was taken when the positions were loaded): Amax, then c_s
-        float rfo = 0.f;
+        // (Any cap gives a valid bound: a body beyond it gets c = inf, i.e. all its pairs in FP64.  So the cap of the call's
+        // first evaluation serves the later ones, whose loading loop then collects Amax on the way: one reduction per step.)
+        float rfo = 0.f, amax = 0.f;
         if (hill) {
-            asum = block_reduce_f<false>(asum, sR1);
-            acnt = block_reduce_f<false>(acnt, sR2);
-            const float cap = 4.0f * asum / fmaxf(acnt, 1.f);
-            float amax = 0.f;
-            for (int s = t; s < N; s += LEAN_NT) { const float aq = S.C[s]; if (aq <= cap) amax = fmaxf(amax, aq); }
-            amax = block_reduce_f<true>(amax, sR3);
-            if (A.n2 * A.dt_rcrit != 0.0) rfo = n2dtf * (sqrtf(block_reduce_f<true>(vkmax, sR4)) * 1.000001f) * 1.000002f;
-            for (int s = t; s < N; s += LEAN_NT) {
-                const float tq = S.HQ[s] * amax;
-                float c = (S.C[s] <= cap) ? tq * tq * 1.000001f : 3.0e38f;
-                if (!(c >= 0.f)) c = 3.0e38f;
-                S.C[s] = c;
+            if (cap < 0.f) {
+                asum = block_reduce_f<false>(asum, sR1);
+                acnt = block_reduce_f<false>(acnt, sR2);
+                cap = 4.0f * asum / fmaxf(acnt, 1.f);
+                if (!(cap >= 0.f)) cap = 0.f;                 // (NaN state: everything in FP64)
+                for (int s = t; s < N; s += LEAN_NT) { const float aq = S.C[s]; if (aq <= cap) amax_t = fmaxf(amax_t, aq); }
             }
+            amax = block_reduce_f<true>(amax_t, sR3);
+            if (A.n2 * A.dt_rcrit != 0.0) rfo = n2dtf * (sqrtf(block_reduce_f<true>(vkmax, sR4)) * 1.000001f) * 1.000002f;
         }
+        auto hill_c = [&](int s) {                            // c_s from a_s (left in C by the loading loop) and Amax
+            const float tq = S.HQ[s] * amax;
+            float c = (S.C[s] <= cap) ? tq * tq * 1.000001f : 3.0e38f;
+            if (!(c >= 0.f)) c = 3.0e38f;
+            return c;
+        };
+        if (hill && !F32)
+            for (int s = t; s < N; s += LEAN_NT) S.C[s] = hill_c(s);
         // warp 0: origin of the CTA's frame (centre of the bounding box of its bodies) and their radius about it
         if (wid == 0) {
             float lo0 = 3.0e38f, lo1 = 3.0e38f, lo2 = 3.0e38f, hi0 = -3.0e38f, hi1 = -3.0e38f, hi2 = -3.0e38f;
@@ -626,8 +634,10 @@ lean_kernel(const __grid_constant__ LeanArgs L, const __grid_constant__ Workspac
         __syncthreads();
         if (F32) {
             const double ox = sO[0], oy = sO[1], oz = sO[2];
-            for (int s = t; s < N; s += LEAN_NT)
+            for (int s = t; s < N; s += LEAN_NT) {
+                if (hill) S.C[s] = hill_c(s);
                 S.R[s] = make_float4((float)(S.X[s] - ox), (float)(S.Y[s] - oy), (float)(S.Z[s] - oz), S.R[s].w);
+            }
             __syncthreads();
         }
         LEAN_STAMP(3);
