@@ -676,6 +676,7 @@ LeanPlan lean_plan(int N, int precision, int blocks)
     if (p.G > p.NI) p.G = p.NI;
     if (p.G < 1) p.G = 1;
     const int ngmax = (p.NI + p.G - 1) / p.G;
+    p.G = (p.NI + ngmax - 1) / ngmax;                 // no more CTAs than that many groups each need (N = 2048, FP32: 128 x 4, not 68 x 3 + 80 x 4)
     p.nbmax = ngmax * IB;
     p.JS = 1;
     while (ngmax * p.JS * 2 <= LEAN_NW && N / (p.JS * 2) >= 64) p.JS *= 2;
