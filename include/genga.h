@@ -93,7 +93,8 @@ typedef struct {
                                  (heavy bodies first, then along a Hilbert curve in the x-y plane; a
                                  performance hint only).  <= 0: default (8; 32 if N < 16384).              */
     int    chunk;             /* j-bodies per chunk (granularity of the near flag and of the FP32 frames): 64 or
-                                 128; anything else selects the default (128, or 64 for N < 14 000)       */
+                                 128; anything else selects the default per force evaluation (64 below N = 14 000
+                                 with FP32 forces and below N = 20 000 with FP64 forces, else 128)            */
     int    mega_nmax;         /* systems of up to this many bodies run a whole force evaluation (per-body
                                  kernel, all-pairs kick, near field) as ONE cooperative kernel (7 % faster at
                                  N <= 2048, slower from N = 4096 on); 0: default (3000), < 0: never                                                              */

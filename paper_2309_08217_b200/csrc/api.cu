@@ -121,6 +121,18 @@ static int resort(Handle* h)
 }
 
 // ---- force evaluation -------------------------------------------------------------------------
+// Chunk size of the next force evaluation: 128, or 64 for smaller systems (more tiles to spread over the warps).  The
+// symmetric FP64 kernel keeps gaining from 64-body chunks up to N ~ 20 000 (N = 16 384: 223 against 240 us), the FP32 one
+// up to ~14 000 (N = 16 384: 123 against 116 us).  params.chunk overrides.  Everything that depends on the chunk size
+// (packing, frames, bounds, candidate list) is rebuilt by every evaluation, so it may change from one to the next.
+static void set_chunk(Handle* h, int precision)
+{
+    int c = h->p.chunk;
+    if (c != CHUNK_MIN && c != CHUNK_MAX) c = (h->N < (precision == GENGA_FP64 ? 20000 : 14000)) ? CHUNK_MIN : CHUNK_MAX;
+    if (c != h->chunk) { h->chunk = c; h->grid_cache[0][0] = h->grid_cache[1][0] = 0; }
+    h->nchunk = (h->N + h->chunk - 1) / h->chunk;      // j-chunks that hold a live body (pure padding is skipped)
+}
+
 static int maybe_resort(Handle* h)
 {
     if (h->evals_since_sort < 0 || h->evals_since_sort >= h->resort_every) {
@@ -171,6 +183,7 @@ static int force_eval(Handle* h, int precision, double preshift = 0.0)
 {
     if (precision != GENGA_FP64 && precision != GENGA_FP32) return GENGA_EINVAL;
     if (h->N == 0) return GENGA_OK;
+    set_chunk(h, precision);
     const int rc = maybe_resort(h);
     if (rc != GENGA_OK) return rc;
     const PrepArgs a = make_prep_args(h, precision, preshift);
@@ -185,6 +198,7 @@ static int onbody(Handle* h, int precision, bool do_vel, double tau_v, bool do_d
     if (h->N == 0) return GENGA_OK;
     OnBodyArgs a;
     if (do_prep) {
+        set_chunk(h, precision);
         const int rc = maybe_resort(h);
         if (rc != GENGA_OK) return rc;
     }
@@ -273,6 +287,7 @@ static bool mega_ready(Handle* h, int precision)
 // [v += tau_v a] [S(dt/2) D(dt)] S(dt/2), r_crit, pack, all-pairs kick, near field: one cooperative launch.
 static int step_mega(Handle* h, int precision, bool do_vel, double tau_v, bool do_drift, double dt)
 {
+    set_chunk(h, precision);
     const int rc = maybe_resort(h);
     if (rc != GENGA_OK) return rc;
     OnBodyArgs a;
@@ -456,7 +471,7 @@ int genga_create(genga_handle* out, int N, const double* m, const double* x, con
     if (!h) return GENGA_ENOMEM;
     std::memset(static_cast<Handle*>(h), 0, sizeof(Handle));
     h->N = N; h->NP = padded(N);
-    // chunk size: 128, or 64 for small systems (twice the units to spread over the CTAs); params.chunk overrides
+    // chunk size until the first force evaluation chooses its own (set_chunk)
     h->chunk = (p->chunk == CHUNK_MIN || p->chunk == CHUNK_MAX) ? p->chunk : (N < 14000 ? CHUNK_MIN : CHUNK_MAX);
     h->nchunk = (N + h->chunk - 1) / h->chunk;      // j-chunks that hold a live body (pure padding is skipped)
     h->p = *p;

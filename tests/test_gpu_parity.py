@@ -668,6 +668,33 @@ def test_small_system_kernel_runs_whole_sequences():
                         assert (np.linalg.norm(u - v_, axis=1) / np.linalg.norm(v_, axis=1)).max() <= 1e-13, (w.name, how)
 
 
+def test_default_chunk_follows_the_precision():
+    # without params.chunk a force evaluation picks its chunk size itself: 64 below N = 14 000 (FP32) / 20 000 (FP64), else
+    # 128.  Between the two thresholds alternating precisions re-pack with alternating chunk sizes on one handle.
+    w = W.config(4, 15000)
+    ao, po, _ = oracle_accel(w)
+    g = B.from_workload(w)
+    for prec in (B.FP64, B.FP32, B.FP64, B.FP32):
+        g.accel(prec)
+        a = g.get_accel().cpu().numpy()
+        if prec == B.FP64:
+            assert rel_err(a, ao).max() <= 1e-12
+            assert pair_set(g.encounter_pairs()) == pair_set(po)
+        else:
+            _gate32("default chunk", a, g.encounter_pairs(), ao, po)
+    xs = {}
+    for order in ((B.FP64,), (B.FP32, B.FP64)):                 # an FP32 evaluation in between leaves nothing behind
+        h = B.from_workload(w)
+        for prec in order:
+            h.accel(prec)
+        h.run(w.dt, 2, B.FP64)
+        xs[order] = h.get_state()[0].cpu().numpy()
+        h.close()
+    d = np.linalg.norm(xs[(B.FP64,)] - xs[(B.FP32, B.FP64)], axis=1) / np.linalg.norm(xs[(B.FP64,)], axis=1)
+    assert d.max() <= 1e-13                                      # (the symmetric kernels' sums are reproducible to rounding only)
+    g.close()
+
+
 def test_fp32_self_term_with_heavy_bodies():
     # a body's own FP32 term must be exactly 0 for any mass: with the self pair at r = 0 the plain-record loop forms
     # y = inf (G m y^3 overflowed to inf * 0 = NaN for G m > 3.4e-7 when the term was left to an epsilon in r^2).
